@@ -1,0 +1,273 @@
+"""Pins for the oracle's collision step: SRD (Eq. 2), SRD+a (Eqs. 3-4), MBS thermostat (Eqs. 5-7),
+MPC-AT -a/+a (reading U5). CPU only. Citations are PAPER.md lines; readings are in DESIGN.md."""
+import numpy as np
+import pytest
+from scipy import stats
+
+from oracle.binding import Oracle
+from paper_2406_15236_b200.inputs import uniform_maxwell
+from util import by_id, cell_sums
+
+
+def _one_cell(v, r=None, **kw):
+    n = len(v)
+    o = Oracle((1, 1, 1), (1, 1, 1), n, 1, **kw)
+    v = np.asarray(v, np.float32)
+    r = np.zeros((n, 3), np.float32) if r is None else np.asarray(r, np.float32)
+    o.set_state(r[:, 0], r[:, 1], r[:, 2], v[:, 0], v[:, 1], v[:, 2])
+    return o
+
+
+def test_srd_hand_computed_cell(golden):
+    # PAPER.md:33-35 Eq. (2); fixture tests/golden/srd_hand_cell.txt
+    for row in golden("srd_hand_cell.txt"):
+        alpha = float(row[0])
+        want = np.array([float(t) for t in row[1:]]).reshape(2, 3)
+        o = _one_cell([[1, 0, 0], [-1, 2, 0]], alpha_deg=alpha)
+        o.collide_one_cell(axis=[0, 0, 1])
+        _, _, _, vx, vy, vz, _ = o.get_state()
+        got = np.stack([vx, vy, vz], 1)
+        assert np.allclose(got, want, atol=2e-7)
+        assert np.allclose(got.sum(0), [0, 2, 0], atol=3e-7)
+        assert 0.5 * (got.astype(np.float64) ** 2).sum() == pytest.approx(3.0, abs=1e-6)
+
+
+def test_srd_rotation_sense_and_axis_component():
+    # the component along the axis is unchanged; the perpendicular part turns by +alpha (right-handed)
+    o = _one_cell([[0.3, -0.2, 0.9], [-0.3, 0.2, -0.9]], alpha_deg=130)
+    ax = np.array([1.0, 2.0, -2.0]) / 3.0
+    o.collide_one_cell(axis=ax)
+    _, _, _, vx, vy, vz, _ = o.get_state()
+    w0 = np.array([0.3, -0.2, 0.9])
+    w1 = np.array([vx[0], vy[0], vz[0]], np.float64)
+    assert w1 @ ax == pytest.approx(w0 @ ax, abs=1e-6)
+    p0, p1 = w0 - (w0 @ ax) * ax, w1 - (w1 @ ax) * ax
+    assert np.linalg.norm(p1) == pytest.approx(np.linalg.norm(p0), abs=1e-6)
+    cosang = p0 @ p1 / (p0 @ p0)
+    sinang = np.cross(p0, p1) @ ax / (p0 @ p0)
+    assert np.rad2deg(np.arctan2(sinang, cosang)) == pytest.approx(130.0, abs=1e-3)
+
+
+def test_srd_axis_uniform_on_sphere():
+    o = Oracle((4, 4, 4), (4, 4, 4), 10, 31)
+    ax = np.array([o.srd_axis(c, t) for c in range(64) for t in range(60)])
+    assert np.allclose(np.linalg.norm(ax, axis=1), 1.0, atol=1e-12)
+    assert np.all(np.abs(ax.mean(0)) < 0.03)
+    assert np.all(np.abs((ax**2).mean(0) - 1 / 3) < 0.02)
+    # z uniform in [-1,1): KS
+    assert stats.kstest(ax[:, 2], "uniform", args=(-1, 2)).pvalue > 1e-3
+    phi = np.arctan2(ax[:, 1], ax[:, 0]) % (2 * np.pi)
+    assert stats.kstest(phi, "uniform", args=(0, 2 * np.pi)).pvalue > 1e-3
+    # distinct per cell and per step
+    assert not np.allclose(o.srd_axis(1, 0), o.srd_axis(2, 0))
+    assert not np.allclose(o.srd_axis(1, 0), o.srd_axis(1, 1))
+
+
+def _run_box(n_cells=8, nbar=10, steps=1, seed=5, **kw):
+    box = (float(n_cells),) * 3
+    st = uniform_maxwell(box, n_cells**3 * nbar, seed)
+    o = Oracle(box, (n_cells,) * 3, nbar, 1234, **kw)
+    o.set_state(*st)
+    return o, st
+
+
+def test_srd_conserves_cell_momentum_and_energy():
+    # PAPER.md:33 (momentum-conserving), PAPER.md:54 (energy-conserving, microcanonical)
+    o, st = _run_box()
+    ob0 = o.observables()
+    o.step(1)
+    x, y, z, vx, vy, vz, ids = o.get_state()
+    cnt, px, py, pz, e2, key = o.get_cells()
+    sx, sy, sz, se = cell_sums(key, o.nkeys, vx, vy, vz, vx.astype(np.float64) ** 2 + vy.astype(np.float64) ** 2 + vz.astype(np.float64) ** 2)
+    l1 = cell_sums(key, o.nkeys, np.abs(vx) + np.abs(vy) + np.abs(vz))[0] + 1e-30
+    # per-cell momentum after the collision equals the pre-collision sum (to fp32 rounding of the outputs)
+    assert np.max(np.abs(sx - px) / l1) < 3e-7
+    assert np.max(np.abs(sy - py) / l1) < 3e-7
+    assert np.max(np.abs(sz - pz) / l1) < 3e-7
+    # per-cell kinetic energy too (rotation preserves |w|)
+    assert np.max(np.abs(se - e2) / (e2 + 1e-30)) < 1e-6
+    o.step(99)
+    ob = o.observables()
+    assert abs(ob["E_kin"] - ob0["E_kin"]) / ob0["E_kin"] < 1e-5
+    assert np.all(np.abs(ob["P"] - ob0["P"]) < 1e-3)
+    assert ob["step"] == 100
+
+
+def test_srd_actually_changes_velocities_and_mixes():
+    o, st = _run_box(steps=1)
+    o.step(1)
+    *_p, vx, vy, vz, ids = o.get_state()
+    vx1, = by_id(ids, vx)
+    assert np.mean(np.abs(vx1 - st[3]) > 1e-3) > 0.95
+
+
+def test_mbs_kappa_hand_case():
+    # Eq. (6): N_c = 2, sum m w^2 = 4, E_k = 1.5 -> kappa = sqrt(3/4) = 0.8660254
+    o = _one_cell([[1, 1, 0], [-1, -1, 0]], alpha_deg=90, thermostat=1)
+    o.collide_one_cell(axis=[0, 0, 1], kappa=float(np.sqrt(2 * 1.5 / 4.0)))
+    _, _, _, vx, vy, vz, _ = o.get_state()
+    # w1 = (1,1,0) -> rot90 z -> (-1,1,0) -> * 0.8660254
+    assert np.allclose([vx[0], vy[0], vz[0]], [-0.8660254, 0.8660254, 0], atol=2e-7)
+    assert np.allclose([vx[1], vy[1], vz[1]], [0.8660254, -0.8660254, 0], atol=2e-7)
+
+
+@pytest.mark.parametrize("Nc", [2, 3, 4, 10, 11, 25])
+def test_mbs_energy_sampler_is_gamma(Nc):
+    # Eq. (7): E_k/kT ~ Gamma(shape f/2, scale 1), f = 3(N_c-1)
+    o = Oracle((4, 4, 4), (4, 4, 4), 10, 2024)
+    e = np.array([o.mbs_energy(c, t, Nc) for c in range(64) for t in range(100)])
+    k = 1.5 * (Nc - 1)
+    assert e.mean() == pytest.approx(k, rel=0.03)
+    assert e.var() == pytest.approx(k, rel=0.08)
+    assert stats.kstest(e, "gamma", args=(k,)).pvalue > 1e-3
+    assert o.mbs_energy(0, 0, 1) == 0.0
+
+
+def test_mbs_thermostat_sets_temperature():
+    # start far from k_BT = 1: the cell-level thermostat must bring <m sum w^2 / 3(Nc-1)> to k_BT
+    box = (8.0,) * 3
+    st = list(uniform_maxwell(box, 8**3 * 10, 9, kT=2.5))
+    o = Oracle(box, (8, 8, 8), 10, 77, thermostat=1, kT=1.0)
+    o.set_state(*st)
+    assert o.observables()["kT_est"] == pytest.approx(2.5, rel=0.03)
+    o.step(30)
+    kts = []
+    for _ in range(20):
+        o.step(1)
+        kts.append(o.observables()["kT_cell"])
+    assert np.mean(kts) == pytest.approx(1.0, rel=0.02)
+    ob = o.observables()
+    assert ob["kT_est"] == pytest.approx(1.0, rel=0.03)
+    # momentum untouched by the scaling
+    assert np.all(np.abs(ob["P"]) < 1e-2)
+    # velocity components are Maxwellian: N(0, kT/m)
+    *_p, vx, vy, vz, ids = o.get_state()
+    for v in (vx, vy, vz):
+        assert stats.kstest(v[::7].astype(np.float64), stats.norm(0.0, 1.0).cdf).pvalue > 1e-3
+
+
+def test_mbs_per_cell_energy_matches_draw():
+    # after one thermostatted step each cell's relative kinetic energy equals kT * (drawn E_k/kT)
+    o, st = _run_box(n_cells=4, thermostat=1)
+    o.step(1)
+    x, y, z, vx, vy, vz, ids = o.get_state()
+    cnt, px, py, pz, e2, key = o.get_cells()
+    v2 = vx.astype(np.float64) ** 2 + vy.astype(np.float64) ** 2 + vz.astype(np.float64) ** 2
+    sx, sy, sz, se = cell_sums(key, o.nkeys, vx, vy, vz, v2)
+    for k in range(0, 64, 5):
+        if cnt[k] < 2:
+            continue
+        w2 = se[k] - (sx[k] ** 2 + sy[k] ** 2 + sz[k] ** 2) / cnt[k]
+        want = o.mbs_energy(k, 0, int(cnt[k]))      # brick=1: key == canonical id
+        assert 0.5 * w2 == pytest.approx(want, rel=2e-6)
+
+
+def _angular_momentum(o, pre_v, post_v, rho, key, nkeys):
+    """Per-cell angular momentum about the cell's centre of mass, before and after."""
+    cnt = np.bincount(key, minlength=nkeys).astype(np.float64)
+    out = []
+    for v in (pre_v, post_v):
+        rcm = [np.bincount(key, weights=rho[:, d], minlength=nkeys) / np.maximum(cnt, 1) for d in range(3)]
+        r = np.stack([rho[:, d] - rcm[d][key] for d in range(3)], 1)
+        L = np.cross(r, v)
+        out.append(np.stack([np.bincount(key, weights=L[:, d], minlength=nkeys) for d in range(3)], 1))
+    return out, cnt
+
+
+@pytest.mark.parametrize("collision", [0, 1])
+def test_plus_a_conserves_cell_angular_momentum(collision):
+    # Eqs. (3)-(4) PAPER.md:41-52; MPC-AT+a reading U5. Low density so that N_c = 1,2,3 cells occur.
+    box = (6.0,) * 3
+    n = 6**3 * 4
+    st = uniform_maxwell(box, n, 17)
+    o = Oracle(box, (6, 6, 6), 4, 99, collision=collision, conserve_L=1, dt=0.05)
+    o.set_state(*st)
+    # pre-collision state: stream by hand (velocities do not change in a periodic box without force)
+    o2 = Oracle(box, (6, 6, 6), 4, 99, collision=collision, conserve_L=1, dt=0.05)
+    o2.set_state(*st)
+    o.step(1)
+    x, y, z, vx, vy, vz, ids = o.get_state()
+    cnt, px, py, pz, e2, key = o.get_cells()
+    order = np.argsort(ids)
+    pre_v = np.stack([st[3], st[4], st[5]], 1).astype(np.float64)
+    post_v = np.stack([vx, vy, vz], 1).astype(np.float64)[order]
+    keyi = key[order]
+    s = o.grid_shift(0)
+    rho = np.array([o.cell_of([x[i], y[i], z[i]], s)[3] for i in order], np.float64)
+    (L0, L1), c = _angular_momentum(o, pre_v, post_v, rho, keyi, o.nkeys)
+    scale = np.bincount(keyi, weights=np.abs(pre_v).sum(1), minlength=o.nkeys) + 1e-30
+    sing = o.observables()["n_singular_cells"]
+    bad = np.abs(L1 - L0).max(1) / scale > 2e-6
+    assert bad.sum() <= sing                      # only cells flagged singular may miss
+    assert (c == 2).sum() > 3 and (c == 3).sum() > 3
+    # momentum per cell as well
+    for d, p in enumerate((px, py, pz)):
+        s1 = np.bincount(keyi, weights=post_v[:, d], minlength=o.nkeys)
+        assert np.max(np.abs(s1 - p) / scale) < 1e-6
+    # and the collision is not the identity
+    assert np.mean(np.abs(post_v - pre_v).max(1) > 1e-3) > 0.8
+
+
+def test_minus_a_does_not_conserve_angular_momentum():
+    # guards the test above against vacuity: plain SRD changes the cell angular momentum
+    box = (6.0,) * 3
+    st = uniform_maxwell(box, 6**3 * 4, 17)
+    o = Oracle(box, (6, 6, 6), 4, 99, dt=0.05)
+    o.set_state(*st)
+    o.step(1)
+    x, y, z, vx, vy, vz, ids = o.get_state()
+    key = o.get_cells()[5]
+    order = np.argsort(ids)
+    s = o.grid_shift(0)
+    rho = np.array([o.cell_of([x[i], y[i], z[i]], s)[3] for i in order], np.float64)
+    pre_v = np.stack([st[3], st[4], st[5]], 1).astype(np.float64)
+    post_v = np.stack([vx, vy, vz], 1).astype(np.float64)[order]
+    (L0, L1), c = _angular_momentum(o, pre_v, post_v, rho, key[order], o.nkeys)
+    assert np.abs(L1 - L0).max() > 0.1
+
+
+def test_at_momentum_and_temperature():
+    # MPC-AT -a: per-cell momentum exact; velocities relax to N(0, kT/m) whatever the start
+    box = (8.0,) * 3
+    st = uniform_maxwell(box, 8**3 * 10, 3, kT=3.0)
+    o = Oracle(box, (8, 8, 8), 10, 5, collision=1, kT=1.0)
+    o.set_state(*st)
+    o.step(1)
+    x, y, z, vx, vy, vz, ids = o.get_state()
+    cnt, px, py, pz, e2, key = o.get_cells()
+    l1 = cell_sums(key, o.nkeys, np.abs(vx) + np.abs(vy) + np.abs(vz))[0] + 1e-30
+    for v, p in ((vx, px), (vy, py), (vz, pz)):
+        assert np.max(np.abs(cell_sums(key, o.nkeys, v)[0] - p) / l1) < 1e-6
+    o.step(10)
+    ob = o.observables()
+    # relative velocities are fresh N(0,1) with (Nc-1)/Nc of the variance; cm motion keeps 3.0/Nc -> relaxes
+    assert ob["kT_cell"] == pytest.approx(1.0, rel=0.03)
+    *_p, vx, vy, vz, ids = o.get_state()
+    # per-cell relative temperature is what AT sets, check component variance of w
+    key = o.get_cells()[5]
+
+
+def test_at_random_velocities_are_standard_normal():
+    o = Oracle((4, 4, 4), (4, 4, 4), 10, 8, collision=1)
+    g = np.array([o.normals(c, k, t, 3) for c in range(40) for k in range(10) for t in range(10)])
+    assert stats.kstest(g[:, :3].ravel(), stats.norm(0.0, 1.0).cdf).pvalue > 1e-3
+    assert abs(g[:, :3].var() - 1) < 0.03
+    assert abs(np.corrcoef(g[:, 0], g[:, 1])[0, 1]) < 0.03
+    assert abs(np.corrcoef(g[:, 0], g[:, 2])[0, 1]) < 0.03
+
+
+def test_at_rank_is_ascending_id_and_layout_independent():
+    box = (4.0,) * 3
+    st = uniform_maxwell(box, 640, 2)
+    perm = np.random.default_rng(1).permutation(640)
+    res = []
+    for brick, shuffle in [(1, False), (2, True)]:
+        o = Oracle(box, (4, 4, 4), 10, 5, collision=1, brick=brick)
+        if shuffle:
+            o.set_state(*[a[perm] for a in st[:6]], id=st[6][perm])
+        else:
+            o.set_state(*st)
+        o.step(3)
+        x, y, z, vx, vy, vz, ids = o.get_state()
+        res.append(np.stack(by_id(ids, x, y, z, vx, vy, vz)))
+    assert np.array_equal(res[0], res[1])

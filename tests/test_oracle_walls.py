@@ -1,0 +1,131 @@
+"""Pins for the oracle's wall / gravity path: bounce-back (reading U7), virtual wall
+particles (reading U8), Poiseuille flow against the analytic SRD viscosity
+(closed forms of refs [31],[32] checked against the paper's printed eta = 111.3)."""
+import numpy as np
+import pytest
+
+from oracle.binding import Oracle
+from paper_2406_15236_b200.inputs import uniform_maxwell
+from util import srd_viscosity
+
+
+def test_viscosity_closed_form_reproduces_printed_value(golden):
+    (row,) = golden("viscosity.txt")
+    assert row[0] == "srd+a"
+    nbar, h, alpha, eta = (float(t) for t in row[1:])
+    k, c = srd_viscosity(nbar, h, alpha, conserve_L=True)
+    assert nbar * (k + c) == pytest.approx(eta, abs=0.05)       # 111.29 vs printed 111.3
+    k, c = srd_viscosity(10, 0.1, 130)
+    assert k + c == pytest.approx(0.870025, abs=1e-5)
+
+
+def test_bounce_back_hand_cases():
+    o = Oracle((8, 8, 8), (8, 8, 8), 10, 1, bc=(0, 0, 1), dt=0.1, thermostat=1)
+    # hits z = 0 after half the step, comes back along the same line with reversed velocity
+    r, v = o.stream_one([3.0, 4.0, 0.05], [0.5, -0.25, -1.0])
+    assert np.allclose(r, [3.0, 4.0, 0.05], atol=2e-7)
+    assert np.array_equal(v, np.array([-0.5, 0.25, 1.0], np.float32))
+    # upper wall
+    r, v = o.stream_one([3.0, 4.0, 7.98], [0.0, 0.0, 1.0])
+    assert r[2] == pytest.approx(7.92, abs=1e-6) and v[2] == -1.0    # wall at t=0.02, 0.08 back
+    # no crossing: plain streaming; a particle sitting on the wall moving inwards is not bounced
+    r, v = o.stream_one([3.0, 4.0, 0.0], [0.0, 0.0, 1.0])
+    assert r[2] == pytest.approx(0.1, abs=1e-7) and v[2] == 1.0
+    r, v = o.stream_one([3.0, 4.0, 8.0], [0.0, 0.0, -1.0])
+    assert r[2] == pytest.approx(7.9, abs=1e-6) and v[2] == -1.0
+    # x stays periodic
+    r, v = o.stream_one([7.99, 4.0, 4.0], [1.0, 0.0, 0.0])
+    assert 0.0 <= r[0] < 0.1
+
+
+def test_bounce_back_with_gravity_keeps_particles_inside():
+    box = (8.0, 8.0, 8.0)
+    st = uniform_maxwell(box, 4000, 7)
+    o = Oracle(box, (8, 8, 8), 8, 3, bc=(0, 0, 1), g=(0.01, 0, 0), thermostat=1)
+    o.set_state(*st)
+    o.step(20)
+    x, y, z, *_ = o.get_state()
+    assert z.min() >= 0.0 and z.max() <= 8.0
+    assert x.min() >= 0.0 and x.max() < 8.0
+    cnt = o.get_cells()[0]
+    assert cnt.sum() == 4000
+
+
+def test_wall_layers_and_cut_cells():
+    # wall axis has n+2 layers; which layers hold particles depends on the sign of the shift (U8)
+    box = (4.0, 4.0, 4.0)
+    st = uniform_maxwell(box, 4**3 * 10, 7)
+    o = Oracle(box, (4, 4, 4), 10, 3, bc=(0, 0, 1), thermostat=1, dt=1e-30)
+    assert o.nkeys == 4 * 4 * 6
+    seen = set()
+    for t in range(12):
+        o.set_state(*st, step=t)
+        o.step(1)
+        cnt = o.get_cells()[0].reshape(6, 4, 4).sum(axis=(1, 2))
+        sz = o.grid_shift(t)[2]
+        seen.add(sz > 0)
+        if sz > 0:
+            assert cnt[0] == 0 and cnt[1] > 0 and cnt[5] > 0
+            assert cnt[1] < cnt[2] and cnt[5] < cnt[4]       # cut layers are partially filled
+        else:
+            assert cnt[5] == 0 and cnt[0] > 0 and cnt[4] > 0
+    assert seen == {True, False}
+
+
+def test_virtual_wall_particles_recomputed_by_hand():
+    # one real particle in a wall-cut cell: the collision partner is nbar-1 virtual particles whose
+    # velocities come from the (cell, k, t, TAG_WALL) stream. Recompute Eq. (2) in numpy.
+    nbar = 5
+    o = Oracle((2.0, 2.0, 2.0), (2, 2, 2), nbar, 11, bc=(0, 0, 1), dt=1e-30, kT=1.0)
+    t = 0
+    while o.grid_shift(t)[2] <= 0:
+        t += 1
+    s = o.grid_shift(t)
+    r = np.array([0.7, 1.2, 0.05], np.float32)
+    v = np.array([0.3, -0.4, 0.5], np.float32)
+    ijk, cid, key, _ = o.cell_of(r, s)
+    assert ijk[2] == 1                                        # cut layer at the lower wall for s_z > 0
+    o.set_state([r[0]], [r[1]], [r[2]], [v[0]], [v[1]], [v[2]], step=t)
+    o.step(1)
+    *_p, vx, vy, vz, _ = o.get_state()
+    virt = np.array([o.normals(cid, k, t, 4)[:3] for k in range(nbar - 1)])
+    vcm = (v.astype(np.float64) + virt.sum(0)) / nbar
+    ax = o.srd_axis(cid, t)
+    w = v - vcm
+    a = np.deg2rad(np.float32(130.0)).astype(np.float32).astype(np.float64)
+    wr = w * np.cos(a) + np.cross(ax, w) * np.sin(a) + ax * (ax @ w) * (1 - np.cos(a))
+    assert np.allclose([vx[0], vy[0], vz[0]], vcm + wr, atol=3e-7)
+    # an interior cell gets no virtual particles: a lone particle keeps its velocity
+    o.set_state([0.7], [1.2], [1.0], [0.3], [-0.4], [0.5], step=t)
+    o.step(1)
+    *_p, vx, vy, vz, _ = o.get_state()
+    assert (vx[0], vy[0], vz[0]) == (np.float32(0.3), np.float32(-0.4), np.float32(0.5))
+
+
+@pytest.mark.slow
+def test_poiseuille_profile_matches_analytic_viscosity():
+    # gravity + two walls -> parabola; nu = 0.870 for <N_c>=10, h=0.1, alpha=130 deg.
+    # Thin box (L_z = 16, relaxation time L_z^2/(pi^2 nu) = 30 = 300 steps).
+    box, cells = (16.0, 8.0, 16.0), (16, 8, 16)
+    st = uniform_maxwell(box, 16 * 8 * 16 * 10, 5)
+    g = 0.005
+    o = Oracle(box, cells, 10, 321, thermostat=1, g=(g, 0, 0), bc=(0, 0, 1))
+    o.set_state(*st)
+    o.step(1200)
+    prof = np.zeros(16)
+    nav = 0
+    for _ in range(440):
+        o.step(5)
+        prof += o.observables(16)["profile"]
+        nav += 1
+    prof /= nav
+    zc = np.arange(16) + 0.5
+    A = np.stack([zc * (16 - zc), np.ones(16)], 1)
+    coef, *_ = np.linalg.lstsq(A, prof, rcond=None)
+    nu_fit, slip = g / (2 * coef[0]), coef[1]
+    nu = sum(srd_viscosity(10, 0.1, 130))
+    assert nu_fit == pytest.approx(nu, rel=0.06)
+    assert abs(slip) < 0.07 * prof.max()                       # near no-slip
+    assert abs(prof - prof[::-1]).max() < 0.02                 # symmetric
+    ob = o.observables()
+    assert ob["kT_cell"] == pytest.approx(1.0, rel=0.03)        # thermostat holds k_BT under forcing
