@@ -1,0 +1,140 @@
+/* mpc_b200.h -- C ABI of the B200-native multiparticle collision dynamics (MPC) fluid step.
+ *
+ * What one call of mpc_step(ctx, 1) computes (arXiv 2406.15236 "HTMPC", cited as PAPER.md:<line>):
+ *   MOVE              r_i <- r_i + h v_i                          Eq. (1)
+ *                     (+ constant acceleration; bounce-back at no-slip walls)
+ *   PROCESS           random shift of the collision lattice, cell index of every particle,
+ *                     per-cell sums (count, momentum, energy, ...)
+ *   REORDER           every `rebin_every` steps the particles are re-sorted by (cell key, id)
+ *                     (counting sort: histogram, prefix sum, scatter)
+ *   PROCESS_CELLS     v_cm, rotation axis, thermostat factor kappa   Eqs. (2),(5)-(7)
+ *   ROTATE_VELOCITIES v_i <- v_cm + kappa D(alpha)(v_i - v_cm) [+ omega x r_ic]   Eqs. (2)-(5)
+ *                     or MPC-AT: v_i <- v_cm + v_ran_i - mean(v_ran) [+ omega x r_ic]  (U5)
+ * in the paper's order (Fig. 1c). Random numbers are Philox-4x32-10 blocks with
+ * key = seed and counter = (index, sub, step, tag); the stream layout is fixed in DESIGN.md "RNG".
+ *
+ * Conventions
+ *   - Every function returns an int status: MPC_OK (0) or a negative MPC_E* code. Nothing throws,
+ *     aborts or prints. mpc_last_error() gives a message for the last failure on that context.
+ *   - "device pointer" = CUDA global memory of the current device; "host pointer" = ordinary host
+ *     memory (pinned memory makes the *_host copies asynchronous to the host, nothing else changes).
+ *   - The library never allocates device memory. The caller (e.g. a torch tensor) owns the
+ *     workspace passed to mpc_bind and every buffer passed to set/get calls; the library owns only
+ *     the host-side context, released by mpc_destroy.
+ *   - All work is enqueued on the CUDA stream given to mpc_bind. Calls that return data to the host
+ *     (mpc_observables, mpc_get_state_host) synchronise that stream; the others do not.
+ *   - Particle arrays are fp32 structure-of-arrays x,y,z,vx,vy,vz plus a uint32 id per particle
+ *     (PAPER.md:170). The internal particle order changes at every reorder; get_state returns the
+ *     current internal order together with the ids (the caller un-permutes by id).
+ *   - Not thread-safe per context; different contexts are independent.
+ */
+#ifndef MPC_B200_H
+#define MPC_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MPC_OK      0
+#define MPC_EINVAL -1 /* bad argument or unsupported combination of options            */
+#define MPC_ESTATE -2 /* call order: step before bind/set_state, get_cells before a step */
+#define MPC_ENOMEM -3 /* workspace too small for the requested number of particles      */
+#define MPC_ECUDA  -4 /* a CUDA call failed; sticky until mpc_destroy                   */
+
+typedef struct mpc_ctx mpc_ctx; /* opaque */
+
+typedef struct {
+  int   collision;   /* 0 = SRD rotation (Eq. 2); 1 = MPC-AT (Andersen thermostat, U5)       */
+  int   conserve_L;  /* 0 = -a; 1 = +a, cell-level angular-momentum conservation (Eqs. 3-4)            */
+  int   thermostat;  /* 0 = none; 1 = cell-level Maxwell-Boltzmann scaling (Eqs. 5-7); ignored for AT  */
+  float alpha;       /* SRD rotation angle in radians (cos/sin taken once in double, cast to fp32)     */
+  float dt;          /* MPC time step h                                                                */
+  float kT;          /* k_B T of the thermostat / of virtual wall particles / of MPC-AT                */
+  float mass;        /* particle mass m (all fluid particles are identical)               */
+  float g[3];        /* constant acceleration (force / mass); must be 0 along a wall normal            */
+  int   bc[3];       /* per axis: 0 = periodic; 1 = no-slip walls at 0 and L (at most one wall axis)   */
+  int   grid_shift;  /* 1 = random lattice shift in [-a/2,a/2)^3 every step; 0 = off     */
+  int   rebin_every; /* reorder when step % rebin_every == 0; >= 1; MPC-AT requires 1                  */
+  int   brick;       /* edge B of the brick-major memory key (1 = row-major); memory order only        */
+} mpc_params;
+
+typedef struct {
+  unsigned long long n;                /* number of particles                                          */
+  double P[3];                         /* total momentum m * sum v                                     */
+  double E_kin;                        /* (m/2) sum |v|^2                                              */
+  double kT_est;                       /* m sum |v - <v>|^2 / (3 (N-1))                                */
+  double kT_cell;                      /* sum_c m sum |v - v_cm,c|^2 / sum_c 3 (N_c - 1), cells with
+                                          N_c >= 2, from the last step's pre-collision sums; 0 if none */
+  unsigned max_cell_count;             /* largest N_c of the last step; 0 if no step was taken         */
+  unsigned long long n_singular_cells; /* +a only: cells whose inertia tensor was rejected (U10)       */
+  unsigned long long step;             /* step counter t                                               */
+} mpc_obs;
+
+/* Create a context. box[d] = L_d, cells[d] = number of fluid cells n_d; cells must be cubic
+ * (L_x/n_x == L_y/n_y == L_z/n_z == a). n_per_cell = <N_c>, used for the virtual-wall-particle fill
+ * (round(n_per_cell)) and for sizing. Allocates nothing on the device.
+ * MPC_EINVAL: NULL argument, non-cubic cells, non-positive sizes/dt/kT/mass, rebin_every < 1,
+ * brick < 1, more than one wall axis, force along a wall normal, walls with +a or MPC-AT,
+ * SRD+a with thermostat (U6), MPC-AT with rebin_every != 1, key space >= 2^32. */
+int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_per_cell,
+               const mpc_params* p, unsigned long long seed);
+
+/* Number of keys K of the memory-order cell index (>= number of cells; brick padding and wall
+ * layers included). Per-cell outputs of mpc_get_cells have K entries. */
+int mpc_num_keys(const mpc_ctx*, unsigned long long* nkeys);
+
+/* Bytes of device workspace needed for up to n_max particles. `compact` = 0: reorder through a
+ * second copy of the particle arrays (fastest); 1: reorder property-wise through one 4-byte-per-
+ * particle buffer, for systems where the second copy does not fit. */
+int mpc_workspace_bytes(const mpc_ctx*, unsigned long long n_max, int compact, size_t* bytes);
+
+/* Hand the library its workspace (device pointer, 256-byte aligned, `bytes` long, zeroing not
+ * required) and the CUDA stream (a cudaStream_t cast to void*; NULL = legacy default stream).
+ * The mode (compact or not) is chosen from `bytes`. MPC_ENOMEM if too small for n_max. */
+int mpc_bind(mpc_ctx*, void* workspace, size_t bytes, unsigned long long n_max, void* cuda_stream);
+
+/* Copy a state in. Device pointers (mpc_set_state) or host pointers (mpc_set_state_host), n each.
+ * id == NULL numbers the particles 0..n-1; ids given must be unique. `step` sets the step counter
+ * t (the RNG streams depend on it). Positions must lie in [0, L_d) on periodic axes and in
+ * [0, L_d] on the wall axis. Asynchronous on the bound stream. */
+int mpc_set_state(mpc_ctx*, unsigned long long n, const float* x, const float* y, const float* z,
+                  const float* vx, const float* vy, const float* vz, const unsigned* id, unsigned step);
+int mpc_set_state_host(mpc_ctx*, unsigned long long n, const float* x, const float* y, const float* z,
+                       const float* vx, const float* vy, const float* vz, const unsigned* id, unsigned step);
+
+/* Advance nsteps MPC steps (nsteps >= 0). Asynchronous: only kernel launches and memsets on the
+ * bound stream, no host synchronisation. Requires max |v| h < L/2 (single periodic wrap, U2). */
+int mpc_step(mpc_ctx*, int nsteps);
+
+/* Copy the state out, in the current internal order, with ids. Any pointer may be NULL (skipped).
+ * Device pointers: asynchronous. Host pointers: synchronises the stream before returning. */
+int mpc_get_state(mpc_ctx*, float* x, float* y, float* z, float* vx, float* vy, float* vz, unsigned* id);
+int mpc_get_state_host(mpc_ctx*, float* x, float* y, float* z, float* vx, float* vy, float* vz, unsigned* id);
+
+/* System observables ("Properties<FINALIZE>") into a HOST struct; synchronises.
+ * profile_host: NULL, or n_w host floats receiving the layer-averaged velocity component along the
+ * force axis (first axis with g != 0, else x) as a function of the layer floor(r_w / a) along the
+ * wall axis w (z if there is no wall), the shear-profile binning of PAPER.md:212. */
+int mpc_observables(mpc_ctx*, mpc_obs* host_out, float* profile_host);
+
+/* Test hook: the last step's pre-collision cell sums over real particles. Device pointers, any may
+ * be NULL: count[K], px/py/pz[K] = m * sum v, e2[K] = sum |v|^2, key[n] = memory key of every
+ * particle in the current order. Asynchronous. MPC_ESTATE before the first step. */
+int mpc_get_cells(mpc_ctx*, unsigned* count, float* px, float* py, float* pz, float* e2, unsigned* key);
+
+/* Test hook: one Philox-4x32-10 block computed by the library's generator (host side; the device
+ * code uses the same function). */
+void mpc_philox4x32_10(const unsigned ctr[4], const unsigned key[2], unsigned out[4]);
+
+/* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
+unsigned long long mpc_launch_count(const mpc_ctx*);
+
+const char* mpc_last_error(const mpc_ctx*);
+int mpc_destroy(mpc_ctx*);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MPC_B200_H */

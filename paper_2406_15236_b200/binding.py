@@ -1,0 +1,204 @@
+"""Thin Python binding of the C ABI in include/mpc_b200.h: argument marshalling only.
+
+Every step of the MPC path runs in the CUDA kernels of libmpc_b200.so. PyTorch supplies device
+memory (the workspace and the I/O tensors) and the CUDA stream, nothing else. There is no CPU
+fallback: if the library is missing it must be built (paper_2406_15236_b200.build), and every
+compute call needs a CUDA device."""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libmpc_b200.so")
+
+MPC_OK, MPC_EINVAL, MPC_ESTATE, MPC_ENOMEM, MPC_ECUDA = 0, -1, -2, -3, -4
+
+# every symbol include/mpc_b200.h declares
+SYMBOLS = ["mpc_create", "mpc_num_keys", "mpc_workspace_bytes", "mpc_bind", "mpc_set_state", "mpc_set_state_host",
+           "mpc_step", "mpc_get_state", "mpc_get_state_host", "mpc_observables", "mpc_get_cells",
+           "mpc_philox4x32_10", "mpc_launch_count", "mpc_last_error", "mpc_destroy"]
+
+
+class mpc_params(C.Structure):
+    _fields_ = [("collision", C.c_int), ("conserve_L", C.c_int), ("thermostat", C.c_int),
+                ("alpha", C.c_float), ("dt", C.c_float), ("kT", C.c_float), ("mass", C.c_float),
+                ("g", C.c_float * 3), ("bc", C.c_int * 3), ("grid_shift", C.c_int),
+                ("rebin_every", C.c_int), ("brick", C.c_int)]
+
+
+class mpc_obs(C.Structure):
+    _fields_ = [("n", C.c_ulonglong), ("P", C.c_double * 3), ("E_kin", C.c_double),
+                ("kT_est", C.c_double), ("kT_cell", C.c_double), ("max_cell_count", C.c_uint),
+                ("n_singular_cells", C.c_ulonglong), ("step", C.c_ulonglong)]
+
+
+class MPCError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load():
+    """dlopen libmpc_b200.so and declare the prototypes. Fails loudly if the library is not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise MPCError(f"{LIB_PATH} is missing: run `python -m paper_2406_15236_b200.build` "
+                       "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, ull, fp, up = C.c_void_p, C.c_ulonglong, C.c_void_p, C.c_void_p
+    L.mpc_create.argtypes = [C.POINTER(vp), C.POINTER(C.c_float), C.POINTER(C.c_int), C.c_float,
+                             C.POINTER(mpc_params), ull]
+    L.mpc_num_keys.argtypes = [vp, C.POINTER(ull)]
+    L.mpc_workspace_bytes.argtypes = [vp, ull, C.c_int, C.POINTER(C.c_size_t)]
+    L.mpc_bind.argtypes = [vp, vp, C.c_size_t, ull, vp]
+    L.mpc_set_state.argtypes = [vp, ull, fp, fp, fp, fp, fp, fp, up, C.c_uint]
+    L.mpc_set_state_host.argtypes = L.mpc_set_state.argtypes
+    L.mpc_step.argtypes = [vp, C.c_int]
+    L.mpc_get_state.argtypes = [vp, fp, fp, fp, fp, fp, fp, up]
+    L.mpc_get_state_host.argtypes = L.mpc_get_state.argtypes
+    L.mpc_observables.argtypes = [vp, C.POINTER(mpc_obs), vp]
+    L.mpc_get_cells.argtypes = [vp, up, fp, fp, fp, fp, up]
+    L.mpc_philox4x32_10.argtypes = [C.POINTER(C.c_uint), C.POINTER(C.c_uint), C.POINTER(C.c_uint)]
+    L.mpc_philox4x32_10.restype = None
+    L.mpc_launch_count.argtypes = [vp]
+    L.mpc_launch_count.restype = ull
+    L.mpc_last_error.argtypes = [vp]
+    L.mpc_last_error.restype = C.c_char_p
+    L.mpc_destroy.argtypes = [vp]
+    for s in SYMBOLS:
+        getattr(L, s)
+    _lib = L
+    return L
+
+
+def philox4x32_10(ctr, key):
+    c = (C.c_uint * 4)(*[int(v) for v in ctr])
+    k = (C.c_uint * 2)(*[int(v) for v in key])
+    o = (C.c_uint * 4)()
+    load().mpc_philox4x32_10(c, k, o)
+    return np.array(o[:], np.uint32)
+
+
+def make_params(collision=0, conserve_L=0, thermostat=0, alpha_deg=130.0, dt=0.1, kT=1.0, mass=1.0,
+                g=(0.0, 0.0, 0.0), bc=(0, 0, 0), grid_shift=1, rebin_every=1, brick=1):
+    p = mpc_params()
+    p.collision, p.conserve_L, p.thermostat = collision, conserve_L, thermostat
+    p.alpha = np.float32(np.deg2rad(alpha_deg))
+    p.dt, p.kT, p.mass = dt, kT, mass
+    p.g[:] = g
+    p.bc[:] = bc
+    p.grid_shift, p.rebin_every, p.brick = grid_shift, rebin_every, brick
+    return p
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+class MPC:
+    """One MPC system on one GPU. Tensors passed in/out are torch CUDA tensors (device API) or
+    pinned/pageable host tensors / numpy arrays (the *_host API)."""
+
+    def __init__(self, box, cells, n_per_cell, seed, n_max, device="cuda:0", compact=False, stream=None, **kw):
+        import torch
+
+        self._torch = torch
+        self.lib = load()
+        self.params = make_params(**kw)
+        self._h = C.c_void_p()
+        rc = self.lib.mpc_create(C.byref(self._h), (C.c_float * 3)(*box), (C.c_int * 3)(*cells),
+                                 float(n_per_cell), C.byref(self.params), int(seed))
+        if rc != MPC_OK:
+            self._h = None
+            raise MPCError(f"mpc_create failed: {rc}")
+        nk = C.c_ulonglong()
+        self._check(self.lib.mpc_num_keys(self._h, C.byref(nk)))
+        self.nkeys = nk.value
+        self.box, self.cells, self.n_max, self.n = tuple(box), tuple(cells), int(n_max), 0
+        self.device = torch.device(device)
+        nbytes = C.c_size_t()
+        self._check(self.lib.mpc_workspace_bytes(self._h, self.n_max, 1 if compact else 0, C.byref(nbytes)))
+        self.workspace_bytes = nbytes.value
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes.value, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self._check(self.lib.mpc_bind(self._h, C.c_void_p(self.workspace.data_ptr()), nbytes.value, self.n_max,
+                                      C.c_void_p(self.stream.cuda_stream)))
+
+    def _check(self, rc):
+        if rc != MPC_OK:
+            msg = self.lib.mpc_last_error(self._h).decode() if self._h else ""
+            raise MPCError(f"mpc error {rc}: {msg}")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.mpc_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        self.close()
+
+    # ---- state ----
+    def set_state(self, x, y, z, vx, vy, vz, id=None, step=0):
+        ts = [x, y, z, vx, vy, vz]
+        for t in ts:
+            assert t.is_cuda and t.dtype == self._torch.float32 and t.is_contiguous()
+        self.n = ts[0].numel()
+        self._check(self.lib.mpc_set_state(self._h, self.n, *[_ptr(t) for t in ts], _ptr(id), step))
+
+    def set_state_host(self, x, y, z, vx, vy, vz, id=None, step=0):
+        """Host arrays: numpy arrays or CPU torch tensors (pinned makes the copies asynchronous)."""
+        torch = self._torch
+        ts = [torch.as_tensor(a) for a in (x, y, z, vx, vy, vz)]
+        for t in ts:
+            assert (not t.is_cuda) and t.dtype == torch.float32 and t.is_contiguous()
+        idt = None if id is None else torch.as_tensor(id)
+        self.n = ts[0].numel()
+        self._keep = (ts, idt)
+        self._check(self.lib.mpc_set_state_host(self._h, self.n, *[_ptr(t) for t in ts], _ptr(idt), step))
+
+    def step(self, nsteps=1):
+        self._check(self.lib.mpc_step(self._h, int(nsteps)))
+
+    def get_state(self):
+        torch = self._torch
+        out = [torch.empty(self.n, dtype=torch.float32, device=self.device) for _ in range(6)]
+        ids = torch.empty(self.n, dtype=torch.int32, device=self.device)
+        self._check(self.lib.mpc_get_state(self._h, *[_ptr(t) for t in out], _ptr(ids)))
+        return (*out, ids)
+
+    def get_state_host(self, out=None):
+        """Returns numpy arrays (x,y,z,vx,vy,vz,id); `out` may supply 7 pre-allocated host tensors."""
+        torch = self._torch
+        if out is None:
+            out = [torch.empty(self.n, dtype=torch.float32) for _ in range(6)] + [torch.empty(self.n, dtype=torch.int32)]
+        self._check(self.lib.mpc_get_state_host(self._h, *[_ptr(t) for t in out]))
+        res = [t.numpy() for t in out]
+        res[6] = res[6].view(np.uint32)
+        return tuple(res)
+
+    def get_cells(self):
+        torch = self._torch
+        cnt = torch.empty(self.nkeys, dtype=torch.int32, device=self.device)
+        p = [torch.empty(self.nkeys, dtype=torch.float32, device=self.device) for _ in range(4)]
+        key = torch.empty(self.n, dtype=torch.int32, device=self.device)
+        self._check(self.lib.mpc_get_cells(self._h, _ptr(cnt), *[_ptr(t) for t in p], _ptr(key)))
+        return cnt, p[0], p[1], p[2], p[3], key
+
+    def observables(self, profile_bins=0):
+        o = mpc_obs()
+        prof = np.zeros(max(profile_bins, 1), np.float32)
+        self._check(self.lib.mpc_observables(self._h, C.byref(o), prof.ctypes.data_as(C.c_void_p) if profile_bins else None))
+        d = dict(n=o.n, P=np.array(o.P[:]), E_kin=o.E_kin, kT_est=o.kT_est, kT_cell=o.kT_cell,
+                 max_cell_count=o.max_cell_count, n_singular_cells=o.n_singular_cells, step=o.step)
+        if profile_bins:
+            d["profile"] = prof
+        return d
+
+    @property
+    def launch_count(self):
+        return int(self.lib.mpc_launch_count(self._h))

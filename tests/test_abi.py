@@ -1,0 +1,76 @@
+"""CPU-side checks of the boundary: the C-ABI library loads, exports every symbol include/mpc_b200.h
+declares, validates arguments, and its host-side Philox agrees with the known-answer vectors.
+No compute call is made (no GPU here)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2406_15236_b200 as pkg
+from paper_2406_15236_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.load()
+
+
+def test_header_symbols_are_exported(lib):
+    hdr = open(os.path.join(ROOT, "include", "mpc_b200.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(mpc_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(binding.SYMBOLS)
+    for s in declared:
+        assert hasattr(lib, s)
+
+
+def test_library_philox_known_answers(lib, golden):
+    for r in golden("philox_kat.txt"):
+        v = [int(t, 16) for t in r]
+        assert [int(o) for o in pkg.philox4x32_10(v[0:4], v[4:6])] == v[6:10]
+
+
+def _create(lib, box=(8, 8, 8), cells=(8, 8, 8), npc=10.0, **kw):
+    h = C.c_void_p()
+    p = binding.make_params(**kw)
+    rc = lib.mpc_create(C.byref(h), (C.c_float * 3)(*box), (C.c_int * 3)(*cells), npc, C.byref(p), 1)
+    return rc, h
+
+
+def test_create_validates_arguments(lib):
+    rc, h = _create(lib)
+    assert rc == 0
+    nk = C.c_ulonglong()
+    assert lib.mpc_num_keys(h, C.byref(nk)) == 0 and nk.value == 512
+    assert lib.mpc_step(h, 1) == binding.MPC_ESTATE          # not bound
+    assert b"mpc_bind" in lib.mpc_last_error(h)
+    nb = C.c_size_t()
+    assert lib.mpc_workspace_bytes(h, 5120, 0, C.byref(nb)) == 0
+    nb2 = C.c_size_t()
+    assert lib.mpc_workspace_bytes(h, 5120, 1, C.byref(nb2)) == 0
+    assert 0 < nb2.value < nb.value
+    assert lib.mpc_destroy(h) == 0
+    assert _create(lib, box=(8, 8, 9))[0] == binding.MPC_EINVAL
+    assert _create(lib, cells=(8, 8, 0))[0] == binding.MPC_EINVAL
+    assert _create(lib, rebin_every=0)[0] == binding.MPC_EINVAL
+    assert _create(lib, brick=3)[0] == binding.MPC_EINVAL
+    assert _create(lib, bc=(1, 0, 1))[0] == binding.MPC_EINVAL
+    assert _create(lib, bc=(0, 0, 1), g=(0, 0, 0.1))[0] == binding.MPC_EINVAL
+    assert _create(lib, collision=1, rebin_every=2)[0] == binding.MPC_EINVAL
+    assert _create(lib, conserve_L=1, thermostat=1)[0] == binding.MPC_EINVAL
+    rc, h = _create(lib, cells=(8, 8, 8), bc=(0, 0, 1), thermostat=1, brick=4)
+    assert rc == 0
+    assert lib.mpc_num_keys(h, C.byref(nk)) == 0 and nk.value == 8 * 8 * 12     # 10 layers padded to 3 bricks of 4
+    lib.mpc_destroy(h)
+
+
+def test_no_cpu_fallback_without_library(monkeypatch):
+    monkeypatch.setattr(binding, "_lib", None)
+    monkeypatch.setattr(binding, "LIB_PATH", "/nonexistent/libmpc_b200.so")
+    with pytest.raises(binding.MPCError):
+        binding.load()

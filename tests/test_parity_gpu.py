@@ -1,0 +1,278 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+Tolerances are BASELINE.json north_star's: keys / counts / sort order bit-exact, positions <= 1e-5 a,
+velocities <= 2e-5 sqrt(kT/m) absolute, per-cell momentum sums <= 1e-5 relative (L1 scale, U13)."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle.binding import Oracle  # noqa: E402
+from paper_2406_15236_b200 import MPC  # noqa: E402
+from paper_2406_15236_b200.inputs import uniform_maxwell  # noqa: E402
+
+POS_TOL, VEL_TOL, MOM_TOL = 1e-5, 2e-5, 1e-5
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_set(g, st, step=0):
+    x, y, z, vx, vy, vz, ids = st
+    g.set_state(*[dev(a) for a in (x, y, z, vx, vy, vz)], id=dev(ids.view(np.int32)), step=step)
+
+
+def gpu_get(g):
+    out = g.get_state()
+    torch.cuda.synchronize()
+    arrs = [t.cpu().numpy() for t in out]
+    arrs[6] = arrs[6].view(np.uint32)
+    return arrs
+
+
+def compare_step(o, g, kT=1.0, mass=1.0, a=1.0, check_order=True, vel_tol=VEL_TOL):
+    """Compare the states and the last step's cell data of oracle `o` and GPU system `g`."""
+    so, sg = o.get_state(), gpu_get(g)
+    if check_order:
+        assert np.array_equal(so[6], sg[6]), "particle order (ids) differs"
+        oo = og = slice(None)
+    else:
+        oo, og = np.argsort(so[6]), np.argsort(sg[6])
+        assert np.array_equal(so[6][oo], sg[6][og])
+    for d in range(3):
+        assert np.max(np.abs(so[d][oo].astype(np.float64) - sg[d][og]), initial=0) <= POS_TOL * a
+    sc = np.sqrt(kT / mass)
+    for d in range(3, 6):
+        err = np.max(np.abs(so[d][oo].astype(np.float64) - sg[d][og]), initial=0)
+        assert err <= vel_tol * sc, f"velocity component {d - 3}: {err}"
+    cnt_o, px, py, pz, e2, key_o = o.get_cells()
+    cnt_g, gx, gy, gz, ge, key_g = [t.cpu().numpy() for t in g.get_cells()]
+    assert np.array_equal(key_o[oo], key_g.view(np.uint32)[og]), "cell keys differ"
+    assert np.array_equal(cnt_o, cnt_g.view(np.uint32)), "cell counts differ"
+    # U13: relative to the L1 scale of the summands, m * sum |v_i| ~ count * mean|v|; use e2-based bound
+    l1 = mass * np.sqrt(np.maximum(e2, 1e-30) * np.maximum(cnt_o, 1))     # >= m * sum |v| / sqrt(3) by Cauchy-Schwarz
+    for po, pg in ((px, gx), (py, gy), (pz, gz)):
+        rel = np.abs(po - pg) / np.maximum(l1, 1e-30)
+        assert np.max(rel[cnt_o > 0], initial=0) <= MOM_TOL
+    return so, sg
+
+
+def make_pair(box, cells, nbar, seed, n, **kw):
+    o = Oracle(box, cells, nbar, seed, **kw)
+    g = MPC(box, cells, nbar, seed, n_max=max(n, 1), **kw)
+    return o, g
+
+
+CASES = {
+    # BASELINE.json config 1 shape: 16^3 cells, 10/cell, SRD, no thermostat
+    "cfg1_srd": dict(cells=(16, 16, 16), nbar=10, kw=dict()),
+    "srd_mbs_brick4": dict(cells=(16, 12, 8), nbar=10, kw=dict(thermostat=1, brick=4)),
+    "srd_mbs_low_density": dict(cells=(12, 12, 12), nbar=3, kw=dict(thermostat=1)),
+    "srd_a2": dict(cells=(8, 8, 8), nbar=10, kw=dict(thermostat=1), a=2.0),
+    "at": dict(cells=(12, 12, 12), nbar=10, kw=dict(collision=1, dt=0.02)),
+    "at_brick2": dict(cells=(10, 12, 6), nbar=5, kw=dict(collision=1, dt=0.02, brick=2)),
+    "walls_gravity": dict(cells=(16, 8, 8), nbar=10, kw=dict(thermostat=1, bc=(0, 0, 1), g=(0.001, 0, 0))),
+    "walls_x_brick4": dict(cells=(8, 8, 16), nbar=10, kw=dict(thermostat=1, bc=(1, 0, 0), g=(0, 0.01, 0), brick=4)),
+    "noshift": dict(cells=(8, 8, 8), nbar=10, kw=dict(grid_shift=0)),
+}
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_single_step_parity(name):
+    c = CASES[name]
+    a = c.get("a", 1.0)
+    cells = c["cells"]
+    box = tuple(float(n) * a for n in cells)
+    n = int(np.prod(cells)) * c["nbar"] + 37                   # ragged tail: not a multiple of any block size
+    st = uniform_maxwell(box, n, 100 + len(name))
+    o, g = make_pair(box, cells, c["nbar"], 1234, n, **c["kw"])
+    o.set_state(*st)
+    gpu_set(g, st)
+    o.step(1)
+    g.step(1)
+    compare_step(o, g, a=a)
+
+
+@pytest.mark.parametrize("name", ["cfg1_srd", "srd_mbs_brick4", "at", "walls_gravity"])
+def test_lockstep_parity_many_steps(name):
+    # U15: after every step the oracle state is copied to the GPU, then both advance one step
+    c = CASES[name]
+    cells = c["cells"]
+    box = tuple(float(n) for n in cells)
+    n = int(np.prod(cells)) * c["nbar"]
+    st = uniform_maxwell(box, n, 7)
+    o, g = make_pair(box, cells, c["nbar"], 99, n, **c["kw"])
+    o.set_state(*st)
+    for t in range(12):
+        gpu_set(g, o.get_state(), step=t)
+        o.step(1)
+        g.step(1)
+        compare_step(o, g)
+
+
+@pytest.mark.parametrize("every", [3, 10])
+def test_stale_order_parity(every):
+    # reorder only every `every` steps: between reorders both keep the stale order (U3)
+    cells, nbar = (12, 12, 12), 10
+    box = tuple(float(n) for n in cells)
+    n = int(np.prod(cells)) * nbar
+    st = uniform_maxwell(box, n, 8)
+    kw = dict(thermostat=1, rebin_every=every, brick=4)
+    o, g = make_pair(box, cells, nbar, 5, n, **kw)
+    o.set_state(*st)
+    for t in range(every + 2):
+        gpu_set(g, o.get_state(), step=t)
+        o.step(1)
+        g.step(1)
+        compare_step(o, g)
+
+
+def test_gpu_is_bit_reproducible_and_order_independent():
+    # fixed-point cell sums: the trajectory does not depend on the memory order,
+    # the reorder interval, the key layout, or the run
+    cells, nbar = (16, 16, 16), 10
+    box = (16.0, 16.0, 16.0)
+    n = 16**3 * nbar
+    st = uniform_maxwell(box, n, 3)
+    res = []
+    for kw in (dict(), dict(), dict(rebin_every=7), dict(brick=8), dict(brick=4, rebin_every=1000)):
+        g = MPC(box, cells, nbar, 42, n_max=n, thermostat=1, **kw)
+        gpu_set(g, st)
+        g.step(25)
+        s = gpu_get(g)
+        order = np.argsort(s[6])
+        res.append(np.stack([s[d][order] for d in range(6)]))
+    for r in res[1:]:
+        assert np.array_equal(r, res[0])
+
+
+def test_free_running_conservation_cfg1():
+    # BASELINE.json config 1: 100 steps, no thermostat: momentum and kinetic energy conserved
+    cells, nbar = (16, 16, 16), 10
+    box = (16.0, 16.0, 16.0)
+    n = 16**3 * nbar
+    st = uniform_maxwell(box, n, 1)
+    g = MPC(box, cells, nbar, 1234, n_max=n)
+    gpu_set(g, st)
+    ob0 = g.observables()
+    g.step(100)
+    ob = g.observables()
+    assert ob["step"] == 100 and ob["n"] == n
+    assert abs(ob["E_kin"] - ob0["E_kin"]) / ob0["E_kin"] < 1e-5
+    assert np.all(np.abs(ob["P"] - ob0["P"]) < 0.05)           # sum of 40960 fp32-rounded updates x 100 steps
+    assert ob["kT_est"] == pytest.approx(1.0, rel=0.02)
+    # same run on the oracle agrees statistically (free-running trajectories diverge, U15)
+    o = Oracle(box, cells, nbar, 1234)
+    o.set_state(*st)
+    o.step(100)
+    oo = o.observables()
+    assert ob["E_kin"] == pytest.approx(oo["E_kin"], rel=1e-5)
+    assert abs(ob["max_cell_count"] - oo["max_cell_count"]) <= 6
+
+
+def test_observables_match_oracle():
+    cells, nbar = (12, 8, 10), 10
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    st = uniform_maxwell(box, n, 12)
+    kw = dict(thermostat=1, bc=(0, 0, 1), g=(0.01, 0, 0))
+    o, g = make_pair(box, cells, nbar, 77, n, **kw)
+    o.set_state(*st)
+    gpu_set(g, st)
+    o.step(1)
+    g.step(1)
+    a, b = o.observables(10), g.observables(10)
+    assert a["n"] == b["n"] and a["step"] == b["step"] and a["max_cell_count"] == b["max_cell_count"]
+    assert np.allclose(a["P"], b["P"], atol=2e-2)
+    assert b["E_kin"] == pytest.approx(a["E_kin"], rel=1e-6)
+    assert b["kT_est"] == pytest.approx(a["kT_est"], rel=1e-6)
+    assert b["kT_cell"] == pytest.approx(a["kT_cell"], rel=1e-5)
+    assert np.allclose(a["profile"], b["profile"], atol=1e-5)
+
+
+def test_edge_cases():
+    box, cells = (4.0, 4.0, 4.0), (4, 4, 4)
+    # empty system
+    g = MPC(box, cells, 10, 1, n_max=16)
+    e = torch.empty(0, dtype=torch.float32, device="cuda")
+    g.set_state(e, e, e, e, e, e)
+    g.step(3)
+    ob = g.observables()
+    assert ob["n"] == 0 and ob["step"] == 3
+    # one particle: collision with itself leaves it unchanged; streaming wraps
+    o, g = make_pair(box, cells, 10, 1, 1)
+    st = [np.array([v], np.float32) for v in (3.95, 0.0, 2.0, 1.0, -1.0, 0.5)] + [np.array([0], np.uint32)]
+    o.set_state(*st)
+    gpu_set(g, st)
+    o.step(2)
+    g.step(2)
+    so, sg = compare_step(o, g)
+    assert sg[3][0] == np.float32(1.0) and sg[4][0] == np.float32(-1.0)
+    # particles exactly on cell faces and box faces, zero velocity, no shift: keys are floor(r)
+    o, g = make_pair(box, cells, 10, 1, 64, grid_shift=0)
+    gx, gy, gz = np.meshgrid(np.arange(4.0), np.arange(4.0), np.arange(4.0), indexing="ij")
+    z = np.zeros(64, np.float32)
+    st = [gx.ravel().astype(np.float32), gy.ravel().astype(np.float32), gz.ravel().astype(np.float32), z, z, z,
+          np.arange(64, dtype=np.uint32)]
+    o.set_state(*st)
+    gpu_set(g, st)
+    o.step(1)
+    g.step(1)
+    compare_step(o, g)
+    cnt = g.get_cells()[0].cpu().numpy()
+    assert np.all(cnt == 1)
+    # all particles in one cell (maximum occupancy, heavy atomic contention)
+    n = 3000
+    o, g = make_pair(box, cells, 10, 1, n, thermostat=1)
+    rng = np.random.default_rng(0)
+    st = [np.full(n, 1.5, np.float32) + rng.uniform(-0.2, 0.2, n).astype(np.float32) for _ in range(3)]
+    st += [rng.normal(0, 1, n).astype(np.float32) * 0.01 for _ in range(3)] + [np.arange(n, dtype=np.uint32)]
+    o.set_state(*st)
+    gpu_set(g, st)
+    o.step(1)
+    g.step(1)
+    compare_step(o, g)
+    assert g.observables()["max_cell_count"] >= n // 8
+
+
+def test_host_api_roundtrip_and_errors():
+    box, cells = (8.0, 8.0, 8.0), (8, 8, 8)
+    n = 5120
+    st = uniform_maxwell(box, n, 2)
+    g = MPC(box, cells, 10, 9, n_max=n, thermostat=1)
+    g.set_state_host(*st[:6], id=st[6].view(np.int32), step=5)
+    back = g.get_state_host()
+    for a, b in zip(st, back):
+        assert np.array_equal(a, b)
+    g.step(2)
+    g2 = MPC(box, cells, 10, 9, n_max=n, thermostat=1)
+    gpu_set(g2, st, step=5)
+    g2.step(2)
+    for a, b in zip(g.get_state_host(), gpu_get(g2)):
+        assert np.array_equal(a, b)
+    # errors
+    from paper_2406_15236_b200 import MPCError
+    with pytest.raises(MPCError):
+        big = uniform_maxwell(box, n + 1, 2)
+        g.set_state_host(*big[:6])
+    g3 = MPC(box, cells, 10, 9, n_max=n)
+    with pytest.raises(MPCError):
+        g3.step(1)                     # no state yet
+    with pytest.raises(MPCError):
+        g3.get_cells()
+
+
+def test_compact_workspace_gives_identical_results():
+    cells, nbar = (12, 12, 12), 10
+    box = (12.0, 12.0, 12.0)
+    n = 12**3 * nbar
+    st = uniform_maxwell(box, n, 4)
+    res = []
+    for compact in (False, True):
+        g = MPC(box, cells, nbar, 6, n_max=n, compact=compact, thermostat=1, rebin_every=2, brick=4)
+        gpu_set(g, st)
+        g.step(5)
+        res.append(gpu_get(g))
+    for a, b in zip(*res):
+        assert np.array_equal(a, b)
