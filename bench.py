@@ -1,0 +1,310 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the MPC hot path (BASELINE.json metric: particle-updates/s on one B200
+and achieved HBM GB/s vs the roofline).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5] [--nbar 10] [--impl reference]
+
+A "step" is one full MPC step (stream, shift, key, [reorder], cell sums, cell finalize, collide) over
+all particles of the workload. Default workload = BASELINE.json configs[4] ("cfg5"): SRD, 512^3
+cells, 10 particles/cell (1.342e9 particles, 32 GB of fp32 state), alpha = 130 deg, dt = 0.1,
+k_BT = 1 cell thermostat, reorder every 10 steps. Inputs are seeded synthetic (uniform positions,
+Maxwell velocities; paper_2406_15236_b200/inputs.py) and far larger than L2, so nothing is flushed
+between steps. N > 1 (under torchrun) runs N independent replicas, one per GPU ("replicas only",
+DESIGN.md): no data-path collective, `value` = all ranks' particle-updates / max-over-ranks time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+WORKLOADS = {
+    # name: (cells, nbar, params, default steps, default warmup)
+    "cfg1": dict(cells=(16, 16, 16), nbar=10, kw=dict(), rebin_every=1),
+    "cfg2": dict(cells=(64, 64, 64), nbar=10, kw=dict(thermostat=1), rebin_every=1),
+    "cfg3": dict(cells=(128, 128, 128), nbar=10, kw=dict(collision=1, dt=0.02), rebin_every=1),   # +a: see DESIGN.md
+    "cfg4": dict(cells=(256, 64, 64), nbar=10, kw=dict(thermostat=1, bc=(0, 0, 1), g=(0.001, 0, 0)), rebin_every=1),
+    "cfg5": dict(cells=(512, 512, 512), nbar=10, kw=dict(thermostat=1), rebin_every=10),
+}
+# algorithmic bytes per particle-step (SURVEY.md 8d / DESIGN.md "Roofline"): read r,v 24 B + write r,v 24 B
+# + per-cell record written once and read once (SRD+MBS: 20 B each way) -> 48 + 40/<N_c>
+def algorithmic_bytes_per_update(nbar, collision=0, conserve_L=0):
+    if collision == 1 or conserve_L:
+        return 48.0 + (88.0 + 48.0) / nbar
+    return 48.0 + 40.0 / nbar
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([t.strip() for t in out.split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i].lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(self.rows)}
+
+
+def oracle_rate(wl, nbar, budget_s=12.0):
+    """The CPU oracle, as it stands, on a bounded sample of the workload: same parameters on a 64^3-cell
+    box (or the workload itself if smaller), single thread. Returns (updates/s, description, steps)."""
+    from oracle.binding import Oracle
+    from paper_2406_15236_b200.inputs import uniform_maxwell
+
+    cells = tuple(min(c, 64) for c in wl["cells"])
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    kw = dict(wl["kw"])
+    kw.update(rebin_every=wl["rebin_every"], brick=1)
+    o = Oracle(box, cells, nbar, 1234, **kw)
+    rest = "g" in kw
+    o.set_state(*uniform_maxwell(box, n, 1234, rest=rest))
+    t0 = time.perf_counter()
+    o.step(1)
+    t1 = time.perf_counter() - t0
+    steps = int(max(2, min(200, budget_s / max(t1, 1e-6))))
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    return n * steps / dt, f"{cells[0]}x{cells[1]}x{cells[2]} cells x {nbar}/cell ({n} particles), {steps} steps, same parameters", steps, dt / steps
+
+
+def run_reference(args, wl, rank, world):
+    if rank != 0:
+        return
+    nbar = args.nbar
+    cells = tuple(min(c, 64) for c in wl["cells"])
+    from oracle.binding import Oracle
+    from paper_2406_15236_b200.inputs import uniform_maxwell
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    kw = dict(wl["kw"])
+    kw.update(rebin_every=wl["rebin_every"], brick=1)
+    o = Oracle(box, cells, nbar, 1234, **kw)
+    o.set_state(*uniform_maxwell(box, n, 1234, rest="g" in kw))
+    o.step(args.warmup)
+    t0 = time.perf_counter()
+    o.step(args.steps)
+    dt = time.perf_counter() - t0
+    val = n * args.steps / dt
+    sample = f"{cells[0]}x{cells[1]}x{cells[2]} cells x {nbar}/cell ({n} particles) per step, same parameters as the workload"
+    line = {"impl": "reference", "metric": "MPC particle-updates/sec", "value": val, "unit": "particle-updates/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": args.workload, "cells": list(wl["cells"]), "n_per_cell": nbar,
+                       "note": "CPU oracle (oracle/mpc_oracle.cpp, single thread) timed on a bounded sample of the workload"},
+            "cpu_baseline": {"value": val, "unit": "particle-updates/s", "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "particle-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS))
+    ap.add_argument("--nbar", type=int, default=None, help="particles per cell (cfg5 sweep: 5, 10, 20)")
+    ap.add_argument("--brick", type=int, default=8)
+    ap.add_argument("--rebin-every", type=int, default=None)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--compact", action="store_true", help="property-wise reorder workspace")
+    args = ap.parse_args()
+    wl = dict(WORKLOADS[args.workload])
+    if args.nbar is None:
+        args.nbar = wl["nbar"]
+    if args.rebin_every is not None:
+        wl["rebin_every"] = args.rebin_every
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        run_reference(args, wl, rank, world)
+        return
+
+    import torch
+
+    from paper_2406_15236_b200 import MPC
+    from paper_2406_15236_b200.inputs import uniform_maxwell_cuda
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    device = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(device)
+
+    cells, nbar = wl["cells"], args.nbar
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    kw = dict(wl["kw"])
+    kw.update(rebin_every=wl["rebin_every"], brick=args.brick)
+    compact = args.compact or (n * 72 + int(np.prod(cells)) * 80 > 150e9)
+    sim = MPC(box, cells, nbar, 1234 + rank, n_max=n, device=str(device), compact=compact, **kw)
+    rest = "g" in kw
+    st = list(uniform_maxwell_cuda(box, n, 1234 + rank, device=str(device)))
+    if rest:
+        for v in st[3:]:
+            v.zero_()
+    sim.set_state(*st)
+    torch.cuda.synchronize()
+    del st
+    torch.cuda.empty_cache()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- warm-up (untimed), then EXACTLY K timed steps, CUDA events on the launching stream ----
+    sim.step(args.warmup)
+    barrier()
+    sim.profile_enable(True)
+    sim.profile_read()
+    l0 = sim.launch_count
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        barrier()
+        ev0.record(sim.stream)
+        sim.step(args.steps)
+        ev1.record(sim.stream)
+        barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = sim.launch_count - l0
+    prof = sim.profile_read()
+    sim.profile_enable(False)
+    if dist is not None:
+        t = torch.tensor([ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ob = sim.observables()
+    value = world * n * args.steps / (ms * 1e-3)
+
+    # ---- roofline of the dominant kernel family (live CUDA-event times from the timed region) ----
+    peak, peak_src = measured_peaks()
+    balg = algorithmic_bytes_per_update(nbar, kw.get("collision", 0), kw.get("conserve_L", 0))
+    fam = {k: v for k, v in prof.items() if v[1] > 0}
+    total_fam_ms = sum(v[0] for v in fam.values())
+    dom = max(fam, key=lambda k: fam[k][0]) if fam else None
+    roofline = None
+    if dom:
+        dms, dcnt = fam[dom]
+        # per launch of the dominant kernel: its share of the step's algorithmic bytes
+        fam_bytes = kernel_algorithmic_bytes(dom, n, int(np.prod(cells)), nbar)
+        ach = fam_bytes / (dms / dcnt * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                    "traffic": None, "peak_source": peak_src, "avg_ms": dms / dcnt, "launches_timed": dcnt,
+                    "algorithmic_bytes_per_launch": fam_bytes,
+                    "step_frac_of_roofline": value / world * balg / 1e9 / peak,
+                    "step_frac_of_8000": value / world * balg / 1e9 / 8000.0,
+                    "family_ms_per_step": {k: v[0] / args.steps for k, v in sorted(fam.items(), key=lambda kv: -kv[1][0])},
+                    "family_share": {k: v[0] / total_fam_ms for k, v in fam.items()}}
+
+    line = {"metric": "MPC particle-updates/sec", "value": value, "unit": "particle-updates/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": args.workload, "cells": list(cells), "n_per_cell": nbar, "particles": n,
+                       "collision": "MPC-AT" if kw.get("collision") else "SRD", "thermostat": bool(kw.get("thermostat", 0)),
+                       "rebin_every": wl["rebin_every"], "brick": args.brick, "compact_workspace": bool(compact),
+                       "l2": "inputs larger than L2 (no flush)" if n * 24 > 4 * 126e6 else "state fits in L2; HBM fraction not meaningful",
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "algorithmic_bytes_per_update": balg},
+            "gpu_launches": int(launches), "clocks": clocks.summary(), "roofline": roofline,
+            "check": {"kT_cell": ob["kT_cell"], "kT_est": ob["kT_est"], "max_cell_count": ob["max_cell_count"], "step": ob["step"]}}
+
+    # ---- e2e: the same job through the host-buffer C ABI (pinned host state in, K steps, state out) ----
+    if not args.no_e2e and rank == 0 and world == 1:
+        line["e2e"] = run_e2e(sim, n, args.steps)
+    elif world > 1:
+        line["e2e"] = None
+    # ---- CPU oracle beside it (rank 0, N = 1 only) ----
+    if not args.no_cpu_baseline and rank == 0 and world == 1:
+        v, sample, _, _ = oracle_rate(wl, nbar)
+        line["cpu_baseline"] = {"value": v, "unit": "particle-updates/s", "cores": 1, "kind": "oracle", "sample": sample}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def kernel_algorithmic_bytes(family, n, ncells, nbar):
+    """Algorithmic bytes one launch of a kernel family must move."""
+    per_particle = {"stream_key": 24 + 12 + 4, "accum": 12 + 4, "collide": 12 + 4 + 12, "gather": 4 + 32 + 32,
+                    "scatter_ids": 8 + 4, "rank": 8 + 4, "sweep": 48}.get(family, 0)
+    per_cell = {"accum": 20, "cell": 20 + 32, "collide": 32, "scan": 8, "memset": 32, "sweep": 40}.get(family, 0)
+    return float(per_particle) * n + float(per_cell) * ncells
+
+
+def run_e2e(sim, n, steps):
+    import torch
+
+    host = [torch.empty(n, dtype=torch.float32, pin_memory=True) for _ in range(6)]
+    hid = torch.empty(n, dtype=torch.int32, pin_memory=True)
+    sim.get_state_host(out=host + [hid])                   # current state -> pinned host buffers (untimed)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    sim.set_state_host(*host, id=hid, step=0)              # H2D inside the timed region
+    sim.step(steps)
+    ob = sim.observables()                                 # D2H of the step result (synchronises)
+    sim.get_state_host(out=host + [hid])                   # D2H of the final state
+    dt = time.perf_counter() - t0
+    del ob
+    return {"value": n * steps / dt, "unit": "particle-updates/s", "h2d_bytes_per_step": 28.0 * n / steps,
+            "d2h_bytes_per_step": 28.0 * n / steps, "seconds": dt, "steps": steps,
+            "note": "one job = mpc_set_state_host (pinned) + mpc_step(K) + mpc_observables + mpc_get_state_host"}
+
+
+if __name__ == "__main__":
+    main()

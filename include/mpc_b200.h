@@ -131,6 +131,16 @@ void mpc_philox4x32_10(const unsigned ctr[4], const unsigned key[2], unsigned ou
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 unsigned long long mpc_launch_count(const mpc_ctx*);
 
+/* Optional per-kernel-family timing with CUDA events recorded on the bound stream (bench.py's live
+ * roofline measurement). mpc_profile_enable(ctx, 1) starts recording an event pair around every
+ * kernel family of every following step (at most 16384 pairs between reads; later launches are
+ * counted but not timed); mpc_profile_read synchronises the stream, returns for each of the
+ * *n_families (<= 16) families its name, the summed device time in ms and the number of timed
+ * sections since the last read, and resets the accumulators. Arrays are host pointers with room for
+ * 16 entries; names point to static strings. */
+int mpc_profile_enable(mpc_ctx*, int on);
+int mpc_profile_read(mpc_ctx*, int* n_families, const char** names, double* total_ms, unsigned long long* launches);
+
 const char* mpc_last_error(const mpc_ctx*);
 int mpc_destroy(mpc_ctx*);
 

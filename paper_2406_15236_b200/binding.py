@@ -17,7 +17,8 @@ MPC_OK, MPC_EINVAL, MPC_ESTATE, MPC_ENOMEM, MPC_ECUDA = 0, -1, -2, -3, -4
 # every symbol include/mpc_b200.h declares
 SYMBOLS = ["mpc_create", "mpc_num_keys", "mpc_workspace_bytes", "mpc_bind", "mpc_set_state", "mpc_set_state_host",
            "mpc_step", "mpc_get_state", "mpc_get_state_host", "mpc_observables", "mpc_get_cells",
-           "mpc_philox4x32_10", "mpc_launch_count", "mpc_last_error", "mpc_destroy"]
+           "mpc_philox4x32_10", "mpc_launch_count", "mpc_profile_enable", "mpc_profile_read", "mpc_last_error",
+           "mpc_destroy"]
 
 
 class mpc_params(C.Structure):
@@ -66,6 +67,8 @@ def load():
     L.mpc_philox4x32_10.restype = None
     L.mpc_launch_count.argtypes = [vp]
     L.mpc_launch_count.restype = ull
+    L.mpc_profile_enable.argtypes = [vp, C.c_int]
+    L.mpc_profile_read.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_char_p), C.POINTER(C.c_double), C.POINTER(ull)]
     L.mpc_last_error.argtypes = [vp]
     L.mpc_last_error.restype = C.c_char_p
     L.mpc_destroy.argtypes = [vp]
@@ -198,6 +201,18 @@ class MPC:
         if profile_bins:
             d["profile"] = prof
         return d
+
+    def profile_enable(self, on=True):
+        self._check(self.lib.mpc_profile_enable(self._h, 1 if on else 0))
+
+    def profile_read(self):
+        """{family: (total_ms, timed_sections)} since the last read; synchronises the stream."""
+        n = C.c_int()
+        names = (C.c_char_p * 16)()
+        ms = (C.c_double * 16)()
+        cnt = (C.c_ulonglong * 16)()
+        self._check(self.lib.mpc_profile_read(self._h, C.byref(n), names, ms, cnt))
+        return {names[i].decode(): (ms[i], cnt[i]) for i in range(n.value)}
 
     @property
     def launch_count(self):

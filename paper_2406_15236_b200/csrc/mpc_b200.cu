@@ -25,10 +25,10 @@ namespace mpc {
 // ------------------------------------------------------------------------------------------------
 // fixed-point cell sums (the paper's reproducibility option): integer atomics make
 // the sums independent of the order of arrival, so a run is bit-reproducible.
-constexpr float FX_V = 1048576.0f;          // 2^20 per unit velocity  -> |sum v_d|   < 2048
-constexpr float FX_E = 262144.0f;           // 2^18 per unit velocity^2 -> sum |v|^2  < 16384
-constexpr double FX_V_INV = 1.0 / 1048576.0;
-constexpr double FX_E_INV = 1.0 / 262144.0;
+// Scales are powers of two relative to the thermal velocity u = 2^round(log2 sqrt(kT/m)), so the
+// conversion is exact up to the final rounding and the precision does not depend on the unit system:
+//   velocity sums : 2^20 / u    ->  |sum v_d|  < 2048 u      (resolution 9.5e-7 u)
+//   energy sums   : 2^18 / u^2  ->  sum |v|^2  < 16384 u^2   (resolution 3.8e-6 u^2)
 constexpr int SUMS_W = 8;                   // ints per cell (32 B, one sector)
 constexpr int REC_W = 8;                    // floats per cell record (32 B, one sector)
 constexpr int OBS_BLOCKS = 1184;            // 148 SMs x 8
@@ -50,6 +50,8 @@ struct Geo {
   uint32_t k0, k1, t;
   float cosa, sina;
   float kT, mass, sigma;   // sigma = sqrt(kT/m)
+  float fxv, fxe;          // fixed-point scales (powers of two)
+  double fxv_inv, fxe_inv;
   int nbar;
   int collision, thermostat;
   uint32_t nkeys;
@@ -295,12 +297,12 @@ __global__ void __launch_bounds__(256) k_accum(Geo G, size_t n, const float* __r
   const float a = vx[i], b = vy[i], c = vz[i];
   int* s = sums + (size_t)k * SUMS_W;
   atomicAdd((unsigned*)s, 1u);
-  atomicAdd(s + 1, __float2int_rn(a * FX_V));
-  atomicAdd(s + 2, __float2int_rn(b * FX_V));
-  atomicAdd(s + 3, __float2int_rn(c * FX_V));
+  atomicAdd(s + 1, __float2int_rn(a * G.fxv));
+  atomicAdd(s + 2, __float2int_rn(b * G.fxv));
+  atomicAdd(s + 3, __float2int_rn(c * G.fxv));
   if (!AT) {
     const float e = fmaf(a, a, fmaf(b, b, c * c));
-    atomicAdd((unsigned*)(s + 4), __float2uint_rn(e * FX_E));
+    atomicAdd((unsigned*)(s + 4), __float2uint_rn(e * G.fxe));
   } else {
     int ix, iy, iz;
     key_to_cell(G, k, ix, iy, iz);
@@ -308,9 +310,9 @@ __global__ void __launch_bounds__(256) k_accum(Geo G, size_t n, const float* __r
     const Block4 o = philox(canonical_id(G, ix, iy, iz), rank, G.t, TAG_AT, G.k0, G.k1);
     float g0, g1, g2;
     normals3(o, g0, g1, g2);
-    atomicAdd(s + 5, __float2int_rn(G.sigma * g0 * FX_V));
-    atomicAdd(s + 6, __float2int_rn(G.sigma * g1 * FX_V));
-    atomicAdd(s + 7, __float2int_rn(G.sigma * g2 * FX_V));
+    atomicAdd(s + 5, __float2int_rn(G.sigma * g0 * G.fxv));
+    atomicAdd(s + 6, __float2int_rn(G.sigma * g1 * G.fxv));
+    atomicAdd(s + 7, __float2int_rn(G.sigma * g2 * G.fxv));
   }
 }
 
@@ -347,17 +349,17 @@ __global__ void __launch_bounds__(128) k_cell(Geo G, const int* __restrict__ sum
   int ix, iy, iz;
   key_to_cell(G, k, ix, iy, iz);
   const uint32_t cid = canonical_id(G, ix, iy, iz);
-  double S0 = (double)s0.y * FX_V_INV, S1 = (double)s0.z * FX_V_INV, S2 = (double)s0.w * FX_V_INV;
+  double S0 = (double)s0.y * G.fxv_inv, S1 = (double)s0.z * G.fxv_inv, S2 = (double)s0.w * G.fxv_inv;
   float4 r0, r1;
   if (G.collision == 1) {
     const double inv = 1.0 / (double)nreal;
-    r0.x = (float)((S0 - (double)s1.y * FX_V_INV) * inv);
-    r0.y = (float)((S1 - (double)s1.z * FX_V_INV) * inv);
-    r0.z = (float)((S2 - (double)s1.w * FX_V_INV) * inv);
+    r0.x = (float)((S0 - (double)s1.y * G.fxv_inv) * inv);
+    r0.y = (float)((S1 - (double)s1.z * G.fxv_inv) * inv);
+    r0.z = (float)((S2 - (double)s1.w * G.fxv_inv) * inv);
     r0.w = 1.0f;
     r1 = make_float4(0.f, 0.f, 0.f, 0.f);
   } else {
-    double E = (double)(uint32_t)s1.x * FX_E_INV;
+    double E = (double)(uint32_t)s1.x * G.fxe_inv;
     uint32_t Nc = nreal;
     if (G.wall >= 0) {
       // virtual wall particles fill wall-cut cells up to nbar (U8)
@@ -469,8 +471,8 @@ __global__ void __launch_bounds__(256) k_obs_cells(Geo G, const int* __restrict_
     mx = max(mx, nc);
     if (nc < 2u) continue;
     const unsigned e = (unsigned)sums[k * SUMS_W + 4];
-    const double S0 = s0.y * FX_V_INV, S1 = s0.z * FX_V_INV, S2 = s0.w * FX_V_INV;
-    num += (double)G.mass * ((double)e * FX_E_INV - (S0 * S0 + S1 * S1 + S2 * S2) / nc);
+    const double S0 = s0.y * G.fxv_inv, S1 = s0.z * G.fxv_inv, S2 = s0.w * G.fxv_inv;
+    num += (double)G.mass * ((double)e * G.fxe_inv - (S0 * S0 + S1 * S1 + S2 * S2) / nc);
     den += 3.0 * (nc - 1u);
   }
   atomicMax(&smax, mx);
@@ -499,10 +501,10 @@ __global__ void __launch_bounds__(256) k_export_cells(Geo G, const int* __restri
   if (k >= G.nkeys) return;
   const int* s = sums + k * SUMS_W;
   if (count) count[k] = (unsigned)s[0];
-  if (px) px[k] = (float)((double)G.mass * s[1] * FX_V_INV);
-  if (py) py[k] = (float)((double)G.mass * s[2] * FX_V_INV);
-  if (pz) pz[k] = (float)((double)G.mass * s[3] * FX_V_INV);
-  if (e2) e2[k] = AT ? 0.0f : (float)((double)(unsigned)s[4] * FX_E_INV);
+  if (px) px[k] = (float)((double)G.mass * s[1] * G.fxv_inv);
+  if (py) py[k] = (float)((double)G.mass * s[2] * G.fxv_inv);
+  if (pz) pz[k] = (float)((double)G.mass * s[3] * G.fxv_inv);
+  if (e2) e2[k] = AT ? 0.0f : (float)((double)(unsigned)s[4] * G.fxe_inv);
 }
 
 }  // namespace mpc
@@ -511,6 +513,11 @@ __global__ void __launch_bounds__(256) k_export_cells(Geo G, const int* __restri
 // host side
 // =================================================================================================
 using namespace mpc;
+
+enum Family { F_STREAM = 0, F_SCAN, F_SCATTER, F_RANK, F_GATHER, F_ACCUM, F_CELL, F_COLLIDE, F_MEMSET, F_OBS, F_COUNT };
+static const char* const FAMILY_NAMES[F_COUNT] = {"stream_key", "scan", "scatter_ids", "rank", "gather", "accum", "cell",
+                                                  "collide", "memset", "observables"};
+constexpr int PROF_MAX_PAIRS = 16384;
 
 struct mpc_ctx {
   Geo G;
@@ -532,6 +539,13 @@ struct mpc_ctx {
   float* rec;
   double* obs;      // OBS_BLOCKS*8 doubles + 2*MAX_PROFILE doubles
   double* hbuf;     // host staging for mpc_observables
+  // optional per-family timing with CUDA events on the bound stream (mpc_profile_*)
+  bool prof_on;
+  cudaEvent_t* prof_ev;          // 2 * PROF_MAX_PAIRS events, created on first enable
+  int* prof_fam;                 // family of every recorded pair
+  int prof_pairs;
+  double prof_ms[F_COUNT];
+  unsigned long long prof_launches[F_COUNT];
   unsigned long long launches;
   char err[256];
 };
@@ -571,6 +585,18 @@ int cuda_fail(mpc_ctx* c, cudaError_t e, const char* where) {
   if (c) { snprintf(c->err, sizeof(c->err), "%s: %s", where, cudaGetErrorString(e)); c->sticky = true; }
   return MPC_ECUDA;
 }
+struct FamilyTimer {   // records an event pair around the launches of one kernel family
+  mpc_ctx* c; int slot;
+  FamilyTimer(mpc_ctx* c_, int fam) : c(c_), slot(-1) {
+    if (!c->prof_on) return;
+    c->prof_launches[fam]++;
+    if (c->prof_pairs >= PROF_MAX_PAIRS) return;
+    slot = c->prof_pairs++;
+    c->prof_fam[slot] = fam;
+    cudaEventRecord(c->prof_ev[2 * slot], c->stream);
+  }
+  ~FamilyTimer() { if (slot >= 0) cudaEventRecord(c->prof_ev[2 * slot + 1], c->stream); }
+};
 #define CU(call)                                                 \
   do {                                                           \
     cudaError_t e_ = (call);                                     \
@@ -596,6 +622,7 @@ void host_shift(const mpc_ctx* c, uint32_t t, float s[3]) {
 
 int do_scan(mpc_ctx* c) {
   const size_t nk = c->G.nkeys, nb = (nk + SCAN_TILE - 1) / SCAN_TILE;
+  FamilyTimer ft(c, F_SCAN);
   k_scan_reduce<<<(unsigned)nb, SCAN_T, 0, c->stream>>>(c->hist, nk, c->bsum);
   LAUNCH_CHECK("k_scan_reduce");
   k_scan_top<<<1, 1024, 0, c->stream>>>(c->bsum, nb);
@@ -609,11 +636,18 @@ int do_reorder(mpc_ctx* c) {
   const size_t n = c->n;
   int rc = do_scan(c);
   if (rc) return rc;
-  CU(cudaMemsetAsync(c->hist, 0, (size_t)c->G.nkeys * 4, c->stream));   // reuse as cursor
-  k_scatter_ids<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->A[7], c->A[6], c->offset, c->hist, c->slot_id);
-  LAUNCH_CHECK("k_scatter_ids");
-  k_rank<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->A[7], c->A[6], c->offset, c->slot_id, c->perm);
-  LAUNCH_CHECK("k_rank");
+  { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->hist, 0, (size_t)c->G.nkeys * 4, c->stream)); }   // reuse as cursor
+  {
+    FamilyTimer ft(c, F_SCATTER);
+    k_scatter_ids<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->A[7], c->A[6], c->offset, c->hist, c->slot_id);
+    LAUNCH_CHECK("k_scatter_ids");
+  }
+  {
+    FamilyTimer ft(c, F_RANK);
+    k_rank<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->A[7], c->A[6], c->offset, c->slot_id, c->perm);
+    LAUNCH_CHECK("k_rank");
+  }
+  FamilyTimer ftg(c, F_GATHER);
   if (!c->compact) {
     Arrays8 src, dst;
     for (int a = 0; a < 8; ++a) { src.p[a] = c->A[a]; dst.p[a] = c->Bf[a]; }
@@ -638,30 +672,45 @@ int one_step(mpc_ctx* c) {
   host_shift(c, c->t, G.s);
   const bool rebin = (c->t % (uint32_t)c->p.rebin_every) == 0u;
   float** F = reinterpret_cast<float**>(c->A);
-  CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * SUMS_W * 4, c->stream));
-  if (rebin) CU(cudaMemsetAsync(c->hist, 0, (size_t)G.nkeys * 4, c->stream));
+  {
+    FamilyTimer ft(c, F_MEMSET);
+    CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * SUMS_W * 4, c->stream));
+    if (rebin) CU(cudaMemsetAsync(c->hist, 0, (size_t)G.nkeys * 4, c->stream));
+  }
   if (n == 0) { c->t++; c->have_cells = true; return MPC_OK; }
   uint32_t* hist = rebin ? c->hist : nullptr;
   const bool wall = G.wall >= 0, grav = (G.g[0] != 0.f || G.g[1] != 0.f || G.g[2] != 0.f);
   const unsigned gb = nblk(n, 256);
+  {
+  FamilyTimer ft(c, F_STREAM);
   if (wall && grav) k_stream_key<true, true><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->A[7], hist);
   else if (wall) k_stream_key<true, false><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->A[7], hist);
   else if (grav) k_stream_key<false, true><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->A[7], hist);
   else k_stream_key<false, false><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->A[7], hist);
   LAUNCH_CHECK("k_stream_key");
+  }
   if (rebin) {
     const int rc = do_reorder(c);
     if (rc) return rc;
     F = reinterpret_cast<float**>(c->A);
   }
-  if (G.collision == 1) k_accum<true><<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->A[7], c->offset, c->sums);
-  else k_accum<false><<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->A[7], c->offset, c->sums);
-  LAUNCH_CHECK("k_accum");
-  k_cell<<<nblk(G.nkeys, 128), 128, 0, c->stream>>>(G, c->sums, c->rec);
-  LAUNCH_CHECK("k_cell");
-  if (G.collision == 1) k_collide<true><<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->A[7], c->offset, c->rec);
-  else k_collide<false><<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->A[7], c->offset, c->rec);
-  LAUNCH_CHECK("k_collide");
+  {
+    FamilyTimer ft(c, F_ACCUM);
+    if (G.collision == 1) k_accum<true><<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->A[7], c->offset, c->sums);
+    else k_accum<false><<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->A[7], c->offset, c->sums);
+    LAUNCH_CHECK("k_accum");
+  }
+  {
+    FamilyTimer ft(c, F_CELL);
+    k_cell<<<nblk(G.nkeys, 128), 128, 0, c->stream>>>(G, c->sums, c->rec);
+    LAUNCH_CHECK("k_cell");
+  }
+  {
+    FamilyTimer ft(c, F_COLLIDE);
+    if (G.collision == 1) k_collide<true><<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->A[7], c->offset, c->rec);
+    else k_collide<false><<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->A[7], c->offset, c->rec);
+    LAUNCH_CHECK("k_collide");
+  }
   c->t++;
   c->have_cells = true;
   return MPC_OK;
@@ -719,9 +768,8 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   if (p->collision == 0 && p->conserve_L && p->thermostat) return MPC_EINVAL;
   if (p->collision == 1 && p->rebin_every != 1) return MPC_EINVAL;
   if (p->conserve_L) return MPC_EINVAL;   // +a: not built yet
-  mpc_ctx* c = new (std::nothrow) mpc_ctx();
+  mpc_ctx* c = new (std::nothrow) mpc_ctx();   // value-initialised: all zero
   if (!c) return MPC_ENOMEM;
-  memset(c, 0, sizeof(*c));
   c->p = *p; c->seed = seed;
   c->hbuf = new (std::nothrow) double[OBS_HOST_DOUBLES];
   if (!c->hbuf) { delete c; return MPC_ENOMEM; }
@@ -744,6 +792,9 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   G.cosa = (float)cos((double)p->alpha); G.sina = (float)sin((double)p->alpha);
   G.k0 = (uint32_t)(seed & 0xffffffffull); G.k1 = (uint32_t)(seed >> 32);
   G.nbar = (int)lround((double)n_per_cell);
+  const int ue = (int)lround(log2((double)G.sigma));        // thermal velocity rounded to a power of two
+  G.fxv = (float)ldexp(1.0, 20 - ue); G.fxv_inv = ldexp(1.0, ue - 20);
+  G.fxe = (float)ldexp(1.0, 18 - 2 * ue); G.fxe_inv = ldexp(1.0, 2 * ue - 18);
   G.collision = p->collision; G.thermostat = p->thermostat;
   *out = c;
   return MPC_OK;
@@ -881,10 +932,48 @@ void mpc_philox4x32_10(const unsigned ctr[4], const unsigned key[2], unsigned ou
 
 unsigned long long mpc_launch_count(const mpc_ctx* c) { return c ? c->launches : 0ull; }
 
+int mpc_profile_enable(mpc_ctx* c, int on) {
+  if (!c) return MPC_EINVAL;
+  if (c->sticky) return MPC_ECUDA;
+  if (on && !c->prof_ev) {
+    c->prof_ev = new (std::nothrow) cudaEvent_t[2 * PROF_MAX_PAIRS];
+    c->prof_fam = new (std::nothrow) int[PROF_MAX_PAIRS];
+    if (!c->prof_ev || !c->prof_fam) return fail(c, MPC_ENOMEM, "profile buffers");
+    for (int i = 0; i < 2 * PROF_MAX_PAIRS; ++i) CU(cudaEventCreate(&c->prof_ev[i]));
+  }
+  c->prof_on = on != 0;
+  return MPC_OK;
+}
+
+int mpc_profile_read(mpc_ctx* c, int* n_families, const char** names, double* total_ms, unsigned long long* launches) {
+  if (!c || !n_families) return MPC_EINVAL;
+  if (c->sticky) return MPC_ECUDA;
+  if (c->prof_pairs) CU(cudaStreamSynchronize(c->stream));
+  for (int i = 0; i < c->prof_pairs; ++i) {
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]));
+    c->prof_ms[c->prof_fam[i]] += ms;
+  }
+  c->prof_pairs = 0;
+  *n_families = F_COUNT;
+  for (int f = 0; f < F_COUNT; ++f) {
+    if (names) names[f] = FAMILY_NAMES[f];
+    if (total_ms) total_ms[f] = c->prof_ms[f];
+    if (launches) launches[f] = c->prof_launches[f];
+    c->prof_ms[f] = 0.0; c->prof_launches[f] = 0;
+  }
+  return MPC_OK;
+}
+
 const char* mpc_last_error(const mpc_ctx* c) { return c ? c->err : "null context"; }
 
 int mpc_destroy(mpc_ctx* c) {
-  if (c) delete[] c->hbuf;
+  if (c) {
+    delete[] c->hbuf;
+    if (c->prof_ev) for (int i = 0; i < 2 * PROF_MAX_PAIRS; ++i) cudaEventDestroy(c->prof_ev[i]);
+    delete[] c->prof_ev;
+    delete[] c->prof_fam;
+  }
   delete c;
   return MPC_OK;
 }

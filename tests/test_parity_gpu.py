@@ -223,17 +223,31 @@ def test_edge_cases():
     cnt = g.get_cells()[0].cpu().numpy()
     assert np.all(cnt == 1)
     # all particles in one cell (maximum occupancy, heavy atomic contention)
-    n = 3000
-    o, g = make_pair(box, cells, 10, 1, n, thermostat=1)
+    n = 1500
+    o, g = make_pair(box, cells, 10, 1, n, thermostat=1, dt=0.01)
     rng = np.random.default_rng(0)
     st = [np.full(n, 1.5, np.float32) + rng.uniform(-0.2, 0.2, n).astype(np.float32) for _ in range(3)]
-    st += [rng.normal(0, 1, n).astype(np.float32) * 0.01 for _ in range(3)] + [np.arange(n, dtype=np.uint32)]
+    st += [rng.normal(0, 1, n).astype(np.float32) for _ in range(3)] + [np.arange(n, dtype=np.uint32)]
     o.set_state(*st)
     gpu_set(g, st)
     o.step(1)
     g.step(1)
     compare_step(o, g)
     assert g.observables()["max_cell_count"] >= n // 8
+
+
+def test_precision_is_relative_to_thermal_velocity():
+    # same system in units where kT = 1e-4 (velocities 100x smaller): tolerance scales with sqrt(kT/m)
+    cells, nbar, kT = (10, 10, 10), 10, 1e-4
+    box = (10.0, 10.0, 10.0)
+    n = 10**3 * nbar
+    st = uniform_maxwell(box, n, 5, kT=kT)
+    o, g = make_pair(box, cells, nbar, 3, n, thermostat=1, kT=kT, dt=10.0)
+    o.set_state(*st)
+    gpu_set(g, st)
+    o.step(1)
+    g.step(1)
+    compare_step(o, g, kT=kT)
 
 
 def test_host_api_roundtrip_and_errors():
