@@ -150,7 +150,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS))
     ap.add_argument("--nbar", type=int, default=None, help="particles per cell (cfg5 sweep: 5, 10, 20)")
-    ap.add_argument("--brick", type=int, default=8)
+    ap.add_argument("--brick", default="16,16,8", help="brick dims of the memory key, e.g. 16,16,8")
     ap.add_argument("--rebin-every", type=int, default=None)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
@@ -189,7 +189,9 @@ def main():
     box = tuple(float(c) for c in cells)
     n = int(np.prod(cells)) * nbar
     kw = dict(wl["kw"])
-    kw.update(rebin_every=wl["rebin_every"], brick=args.brick)
+    brick = tuple(int(t) for t in args.brick.split(","))
+    brick = brick * 3 if len(brick) == 1 else brick
+    kw.update(rebin_every=wl["rebin_every"], brick=brick)
     compact = args.compact or (n * 72 + int(np.prod(cells)) * 80 > 150e9)
     sim = MPC(box, cells, nbar, 1234 + rank, n_max=n, device=str(device), compact=compact, **kw)
     rest = "g" in kw
@@ -257,7 +259,7 @@ def main():
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": args.workload, "cells": list(cells), "n_per_cell": nbar, "particles": n,
                        "collision": "MPC-AT" if kw.get("collision") else "SRD", "thermostat": bool(kw.get("thermostat", 0)),
-                       "rebin_every": wl["rebin_every"], "brick": args.brick, "compact_workspace": bool(compact),
+                       "rebin_every": wl["rebin_every"], "brick": list(brick), "compact_workspace": bool(compact),
                        "l2": "inputs larger than L2 (no flush)" if n * 24 > 4 * 126e6 else "state fits in L2; HBM fraction not meaningful",
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "algorithmic_bytes_per_update": balg},
@@ -283,7 +285,8 @@ def kernel_algorithmic_bytes(family, n, ncells, nbar):
     """Algorithmic bytes one launch of a kernel family must move."""
     per_particle = {"stream_key": 24 + 12 + 4, "accum": 12 + 4, "collide": 12 + 4 + 12, "gather": 4 + 32 + 32,
                     "scatter_ids": 8 + 4, "rank": 8 + 4, "sweep": 48}.get(family, 0)
-    per_cell = {"accum": 20, "cell": 20 + 32, "collide": 32, "scan": 8, "memset": 32, "sweep": 40}.get(family, 0)
+    # sweep: the per-cell record is read once (32 B) and the cell sums written once (20 B of payload)
+    per_cell = {"accum": 20, "cell": 20 + 32, "collide": 32, "scan": 8, "memset": 24, "sweep": 20 + 20}.get(family, 0)
     return float(per_particle) * n + float(per_cell) * ncells
 
 

@@ -57,7 +57,8 @@ typedef struct {
   int   bc[3];       /* per axis: 0 = periodic; 1 = no-slip walls at 0 and L (at most one wall axis)   */
   int   grid_shift;  /* 1 = random lattice shift in [-a/2,a/2)^3 every step; 0 = off     */
   int   rebin_every; /* reorder when step % rebin_every == 0; >= 1; MPC-AT requires 1                  */
-  int   brick;       /* edge B of the brick-major memory key (1 = row-major); memory order only        */
+  int   brick[3];    /* brick dims (powers of two <= 64) of the brick-major memory key; {1,1,1} = row-major.
+                        Memory order only: results do not depend on it. {16,16,8} is the fast choice          */
 } mpc_params;
 
 typedef struct {
@@ -76,7 +77,7 @@ typedef struct {
  * (L_x/n_x == L_y/n_y == L_z/n_z == a). n_per_cell = <N_c>, used for the virtual-wall-particle fill
  * (round(n_per_cell)) and for sizing. Allocates nothing on the device.
  * MPC_EINVAL: NULL argument, non-cubic cells, non-positive sizes/dt/kT/mass, rebin_every < 1,
- * brick < 1, more than one wall axis, force along a wall normal, walls with +a or MPC-AT,
+ * brick dims not powers of two in 1..64 or tile too large for shared memory, more than one wall axis, force along a wall normal, walls with +a or MPC-AT,
  * SRD+a with thermostat (U6), MPC-AT with rebin_every != 1, key space >= 2^32. */
 int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_per_cell,
                const mpc_params* p, unsigned long long seed);

@@ -44,7 +44,7 @@ struct Params {
   int   bc[3];        // 0 periodic, 1 no-slip walls at 0 and L
   int   grid_shift;   // 1 = random lattice shift every step
   int   rebin_every;  // reorder interval
-  int   brick;        // edge of the brick-major key layout (1 = row-major); memory order only
+  int   brick[3];     // brick dims of the brick-major key layout ({1,1,1} = row-major); memory order only
 };
 
 struct Obs {
@@ -62,7 +62,7 @@ struct Ctx {
   int n[3];        // fluid cells per axis
   int m[3];        // collision-cell layers per axis (n, or n+2 on a wall axis, reading U8)
   int mb[3];       // bricks per axis
-  int B;
+  int B[3];        // brick dims
   float a, inv_a;
   int nbar;        // round(n_per_cell): target occupancy of wall-cut cells
   Params p;
@@ -151,20 +151,19 @@ inline void cell_of(const Ctx& c, const float r[3], const float s[3], int i[3], 
 inline uint32_t canonical_id(const Ctx& c, const int i[3]) {
   return (uint32_t)i[0] + (uint32_t)c.m[0] * ((uint32_t)i[1] + (uint32_t)c.m[1] * (uint32_t)i[2]);
 }
-// memory-order key: brick-major over B^3 bricks (B = 1: identical to canonical_id)
+// memory-order key: brick-major over Bx*By*Bz bricks (B = {1,1,1}: identical to canonical_id)
 inline uint32_t layout_key(const Ctx& c, const int i[3]) {
-  const int B = c.B;
-  const uint32_t bx = i[0] / B, by = i[1] / B, bz = i[2] / B;
-  const uint32_t lx = i[0] % B, ly = i[1] % B, lz = i[2] % B;
+  const uint32_t bx = i[0] / c.B[0], by = i[1] / c.B[1], bz = i[2] / c.B[2];
+  const uint32_t lx = i[0] % c.B[0], ly = i[1] % c.B[1], lz = i[2] % c.B[2];
   const uint32_t brick = (bz * (uint32_t)c.mb[1] + by) * (uint32_t)c.mb[0] + bx;
-  return brick * (uint32_t)(B * B * B) + (lz * B + ly) * B + lx;
+  return brick * (uint32_t)(c.B[0] * c.B[1] * c.B[2]) + (lz * c.B[1] + ly) * c.B[0] + lx;
 }
 inline void key_to_cell(const Ctx& c, uint32_t key, int i[3]) {
-  const uint32_t B = c.B, B3 = B * B * B;
-  uint32_t brick = key / B3, l = key % B3;
-  const uint32_t lx = l % B, ly = (l / B) % B, lz = l / (B * B);
+  const uint32_t B3 = c.B[0] * c.B[1] * c.B[2];
+  const uint32_t brick = key / B3, l = key % B3;
+  const uint32_t lx = l % c.B[0], ly = (l / c.B[0]) % c.B[1], lz = l / (c.B[0] * c.B[1]);
   const uint32_t bx = brick % c.mb[0], by = (brick / c.mb[0]) % c.mb[1], bz = brick / (c.mb[0] * c.mb[1]);
-  i[0] = bx * B + lx; i[1] = by * B + ly; i[2] = bz * B + lz;
+  i[0] = bx * c.B[0] + lx; i[1] = by * c.B[1] + ly; i[2] = bz * c.B[2] + lz;
 }
 
 // ---- streaming, Eq. (1) + gravity + bounce-back (U7)
@@ -495,7 +494,8 @@ int oracle_create(void** out, const float box[3], const int cells[3], float n_pe
   const float a = box[0] / (float)cells[0];
   for (int d = 1; d < 3; ++d) if (box[d] / (float)cells[d] != a) return E_INVAL;   // cubic cells only
   if (p->collision < 0 || p->collision > 1) return E_INVAL;
-  if (!(p->dt > 0.0f) || !(p->kT > 0.0f) || !(p->mass > 0.0f) || p->rebin_every < 1 || p->brick < 1) return E_INVAL;
+  if (!(p->dt > 0.0f) || !(p->kT > 0.0f) || !(p->mass > 0.0f) || p->rebin_every < 1) return E_INVAL;
+  for (int d = 0; d < 3; ++d) if (p->brick[d] < 1) return E_INVAL;
   int nwall = 0;
   for (int d = 0; d < 3; ++d) {
     if (p->bc[d] != 0 && p->bc[d] != 1) return E_INVAL;
@@ -506,14 +506,15 @@ int oracle_create(void** out, const float box[3], const int cells[3], float n_pe
   if (p->collision == 0 && p->conserve_L && p->thermostat) return E_INVAL;  // ambiguous (U6)
   if (!(n_per_cell > 0.0f)) return E_INVAL;
   Ctx* c = new Ctx();
-  c->p = *p; c->seed = seed; c->t = 0; c->a = a; c->inv_a = 1.0f / a; c->B = p->brick;
+  c->p = *p; c->seed = seed; c->t = 0; c->a = a; c->inv_a = 1.0f / a;
   c->nbar = (int)std::lround((double)n_per_cell);
   c->nkeys = 1;
   for (int d = 0; d < 3; ++d) {
     c->L[d] = box[d]; c->n[d] = cells[d];
     c->m[d] = cells[d] + (p->bc[d] == 1 ? 2 : 0);
-    c->mb[d] = (c->m[d] + c->B - 1) / c->B;
-    c->nkeys *= (size_t)c->mb[d] * (size_t)c->B;
+    c->B[d] = p->brick[d];
+    c->mb[d] = (c->m[d] + c->B[d] - 1) / c->B[d];
+    c->nkeys *= (size_t)c->mb[d] * (size_t)c->B[d];
   }
   if (c->nkeys >= 0xffffffffull) { delete c; return E_INVAL; }
   c->cosa = std::cos((double)p->alpha); c->sina = std::sin((double)p->alpha);

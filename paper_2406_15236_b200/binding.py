@@ -25,7 +25,7 @@ class mpc_params(C.Structure):
     _fields_ = [("collision", C.c_int), ("conserve_L", C.c_int), ("thermostat", C.c_int),
                 ("alpha", C.c_float), ("dt", C.c_float), ("kT", C.c_float), ("mass", C.c_float),
                 ("g", C.c_float * 3), ("bc", C.c_int * 3), ("grid_shift", C.c_int),
-                ("rebin_every", C.c_int), ("brick", C.c_int)]
+                ("rebin_every", C.c_int), ("brick", C.c_int * 3)]
 
 
 class mpc_obs(C.Structure):
@@ -94,7 +94,8 @@ def make_params(collision=0, conserve_L=0, thermostat=0, alpha_deg=130.0, dt=0.1
     p.dt, p.kT, p.mass = dt, kT, mass
     p.g[:] = g
     p.bc[:] = bc
-    p.grid_shift, p.rebin_every, p.brick = grid_shift, rebin_every, brick
+    p.grid_shift, p.rebin_every = grid_shift, rebin_every
+    p.brick[:] = (brick,) * 3 if isinstance(brick, int) else tuple(brick)
     return p
 
 

@@ -1,13 +1,19 @@
 // mpc_b200.cu -- B200 (sm_100a) implementation of the MPC fluid step behind include/mpc_b200.h.
 //
 // One CUDA stream, no host synchronisation inside mpc_step. Kernel families:
-//   k_stream_key   MOVE + shift + cell key (+ histogram on reorder steps)
-//   k_scan_*       exclusive prefix sum of the per-cell histogram
-//   k_scatter_ids / k_rank / k_gather   counting-sort reorder by (key, id)
-//   k_accum        per-cell sums in 32-bit fixed point (order-independent)
-//   k_cell         v_cm, axis, kappa, virtual wall particles
-//   k_collide      rotation / MPC-AT applied to every particle                   Eqs. (2)-(5)
+//   k_sweep        SRD hot path, ONE pass over the particles per step: collision of step t-1
+//                  (Eqs. 2,5) fused with MOVE of step t (Eq. 1), shift + cell key, and the per-cell
+//                  sums of step t accumulated in a shared-memory tile per brick of cells.
+//                  PAPER.md:29-37,68,70,176
+//   k_cell         PROCESS_CELLS: v_cm, axis, kappa, virtual wall particles
+//   k_collide_pos  trailing collision of the last step of an mpc_step call       Eqs. (2),(5)
+//   k_scan_* / k_scatter_ids / k_rank / k_gather*   counting-sort reorder by (key, id)
+//   k_stream_key / k_accum_at / k_collide_at        MPC-AT path (needs the rank of a particle in its
+//                  sorted cell segment, so it reorders every step and is not fused)
 //   k_obs_*        observables
+// Cell sums are 32-bit fixed point (the paper's reproducibility option), two per
+// 64-bit word, added with integer atomics: order-independent, so a trajectory is bit-reproducible and
+// does not depend on the memory order of the particles.
 // Compile with --fmad=false: every multiply-add that must fuse is an explicit fmaf (U1).
 #include <cuda_runtime.h>
 #include <math.h>
@@ -22,18 +28,16 @@
 
 namespace mpc {
 
-// ------------------------------------------------------------------------------------------------
-// fixed-point cell sums (the paper's reproducibility option): integer atomics make
-// the sums independent of the order of arrival, so a run is bit-reproducible.
-// Scales are powers of two relative to the thermal velocity u = 2^round(log2 sqrt(kT/m)), so the
-// conversion is exact up to the final rounding and the precision does not depend on the unit system:
-//   velocity sums : 2^20 / u    ->  |sum v_d|  < 2048 u      (resolution 9.5e-7 u)
-//   energy sums   : 2^18 / u^2  ->  sum |v|^2  < 16384 u^2   (resolution 3.8e-6 u^2)
-constexpr int SUMS_W = 8;                   // ints per cell (32 B, one sector)
-constexpr int REC_W = 8;                    // floats per cell record (32 B, one sector)
-constexpr int OBS_BLOCKS = 1184;            // 148 SMs x 8
+typedef unsigned long long u64;
+
+constexpr int HALO = 2;               // tile halo in cells on every side of a brick
+constexpr int SWEEP_T = 512;          // threads per sweep CTA
+constexpr int TILE_W = 5;             // int32 words per tile cell: N, Sx, Sy, Sz, E
+constexpr int REC_W = 8;              // floats per cell record (32 B, one sector)
+constexpr int OBS_BLOCKS = 1184;      // 148 SMs x 8
 constexpr int MAX_PROFILE = 2048;
 constexpr size_t OBS_HOST_DOUBLES = (size_t)OBS_BLOCKS * 8 + 2 * MAX_PROFILE;
+constexpr size_t MAX_TILE_BYTES = 110 * 1024;
 
 struct Geo {
   float L[3];
@@ -41,7 +45,7 @@ struct Geo {
   int n[3];       // fluid cells
   int m[3];       // cell layers incl. wall layers
   int mb[3];      // bricks per axis
-  int bshift;     // log2(brick edge)
+  int bs[3];      // log2(brick dims)
   int bc[3];
   int wall;       // wall axis or -1
   float g[3];
@@ -50,38 +54,52 @@ struct Geo {
   uint32_t k0, k1, t;
   float cosa, sina;
   float kT, mass, sigma;   // sigma = sqrt(kT/m)
-  float fxv, fxe;          // fixed-point scales (powers of two)
+  // Fixed-point scales: powers of two relative to u = 2^round(log2 sigma), so precision does not
+  // depend on the unit system:  velocity sums 2^20/u (|sum v_d| < 2048 u), energy sums 2^18/u^2.
+  float fxv, fxe;
   double fxv_inv, fxe_inv;
   int nbar;
   int collision, thermostat;
+  int sw;         // 64-bit words per cell in the global sums array (3 SRD, 4 MPC-AT)
   uint32_t nkeys;
 };
 
+// ---- packed sums ---------------------------------------------------------------------------------
+// word0 = E << 32 | N (both unsigned); word1 = (Sy, Sx); word2 = (R0, Sz); word3 = (R2, R1)  [AT]
+__device__ __forceinline__ u64 pack_ss(int lo, int hi) { return (u64)((long long)hi * 4294967296ll + (long long)lo); }
+__device__ __forceinline__ void unpack_ss(u64 w, int& lo, int& hi) {
+  lo = (int)(uint32_t)(w & 0xffffffffull);
+  hi = (int)(((long long)w - (long long)lo) >> 32);
+}
+
 // ---- geometry helpers ----------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t layout_key(const Geo& G, int ix, int iy, int iz) {
-  const int b = G.bshift, mask = (1 << b) - 1;
-  const uint32_t brick = ((uint32_t)(iz >> b) * (uint32_t)G.mb[1] + (uint32_t)(iy >> b)) * (uint32_t)G.mb[0] + (uint32_t)(ix >> b);
-  const uint32_t local = ((((uint32_t)(iz & mask)) << b | (uint32_t)(iy & mask)) << b) | (uint32_t)(ix & mask);
-  return (brick << (3 * b)) | local;
+  const int b0 = G.bs[0], b1 = G.bs[1], b2 = G.bs[2];
+  const uint32_t brick = ((uint32_t)(iz >> b2) * (uint32_t)G.mb[1] + (uint32_t)(iy >> b1)) * (uint32_t)G.mb[0] + (uint32_t)(ix >> b0);
+  const uint32_t local = ((((uint32_t)(iz & ((1 << b2) - 1))) << b1 | (uint32_t)(iy & ((1 << b1) - 1))) << b0) | (uint32_t)(ix & ((1 << b0) - 1));
+  return (brick << (b0 + b1 + b2)) | local;
 }
-__device__ __forceinline__ void key_to_cell(const Geo& G, uint32_t key, int& ix, int& iy, int& iz) {
-  const int b = G.bshift;
-  const uint32_t mask = (1u << b) - 1u;
-  const uint32_t local = key & ((1u << (3 * b)) - 1u), brick = key >> (3 * b);
+__device__ __forceinline__ void brick_to_origin(const Geo& G, uint32_t brick, int& ox, int& oy, int& oz) {
   const uint32_t bx = brick % (uint32_t)G.mb[0], r = brick / (uint32_t)G.mb[0];
   const uint32_t by = r % (uint32_t)G.mb[1], bz = r / (uint32_t)G.mb[1];
-  ix = (int)((bx << b) | (local & mask));
-  iy = (int)((by << b) | ((local >> b) & mask));
-  iz = (int)((bz << b) | (local >> (2 * b)));
+  ox = (int)(bx << G.bs[0]); oy = (int)(by << G.bs[1]); oz = (int)(bz << G.bs[2]);
+}
+__device__ __forceinline__ void key_to_cell(const Geo& G, uint32_t key, int& ix, int& iy, int& iz) {
+  const int b0 = G.bs[0], b1 = G.bs[1], b2 = G.bs[2];
+  const uint32_t local = key & ((1u << (b0 + b1 + b2)) - 1u), brick = key >> (b0 + b1 + b2);
+  int ox, oy, oz;
+  brick_to_origin(G, brick, ox, oy, oz);
+  ix = ox + (int)(local & ((1u << b0) - 1u));
+  iy = oy + (int)((local >> b0) & ((1u << b1) - 1u));
+  iz = oz + (int)(local >> (b0 + b1));
 }
 __device__ __forceinline__ uint32_t canonical_id(const Geo& G, int ix, int iy, int iz) {
   return (uint32_t)ix + (uint32_t)G.m[0] * ((uint32_t)iy + (uint32_t)G.m[1] * (uint32_t)iz);
 }
-// cell coordinate along one axis; rho = cell-local coordinate in [0,1)
-__device__ __forceinline__ int cell_coord(const Geo& G, int d, float r, float& rho) {
-  const float q = (r + G.s[d]) * G.inv_a;
-  const float f = floorf(q);
-  int k = (int)f;
+// cell coordinate of position r along axis d for lattice shift s
+__device__ __forceinline__ int cell_coord(const Geo& G, int d, float r, float s) {
+  const float q = (r + s) * G.inv_a;
+  int k = (int)floorf(q);
   if (G.bc[d] == 0) {
     if (k < 0) k += G.n[d];
     if (k >= G.n[d]) k -= G.n[d];
@@ -89,13 +107,10 @@ __device__ __forceinline__ int cell_coord(const Geo& G, int d, float r, float& r
     k += 1;
     k = max(0, min(k, G.n[d] + 1));
   }
-  rho = q - f;
   return k;
 }
-__device__ __forceinline__ uint32_t key_of(const Geo& G, float x, float y, float z) {
-  float r0, r1, r2;
-  const int ix = cell_coord(G, 0, x, r0), iy = cell_coord(G, 1, y, r1), iz = cell_coord(G, 2, z, r2);
-  return layout_key(G, ix, iy, iz);
+__device__ __forceinline__ uint32_t key_of(const Geo& G, float x, float y, float z, float s0, float s1, float s2) {
+  return layout_key(G, cell_coord(G, 0, x, s0), cell_coord(G, 1, y, s1), cell_coord(G, 2, z, s2));
 }
 
 // ---- MOVE ----------------------------------------------------------------------------------------
@@ -144,23 +159,165 @@ __device__ __forceinline__ void stream_one(const Geo& G, float (&r)[3], float (&
   }
 }
 
+// ---- SRD rotation with thermostat scaling: v' = vcm + kappa D(alpha) (v - vcm) ----------------------
+__device__ __forceinline__ void srd_apply(const Geo& G, const float4 r0, const float4 ax, float (&v)[3]) {
+  const float w0 = v[0] - r0.x, w1 = v[1] - r0.y, w2 = v[2] - r0.z;
+  const float c = G.cosa, s = G.sina, omc = 1.0f - G.cosa;
+  const float nd = fmaf(ax.x, w0, fmaf(ax.y, w1, ax.z * w2)) * omc;
+  const float cx = fmaf(ax.y, w2, -(ax.z * w1)), cy = fmaf(ax.z, w0, -(ax.x * w2)), cz = fmaf(ax.x, w1, -(ax.y * w0));
+  const float o0 = fmaf(w0, c, fmaf(cx, s, ax.x * nd));
+  const float o1 = fmaf(w1, c, fmaf(cy, s, ax.y * nd));
+  const float o2 = fmaf(w2, c, fmaf(cz, s, ax.z * nd));
+  v[0] = fmaf(r0.w, o0, r0.x);
+  v[1] = fmaf(r0.w, o1, r0.y);
+  v[2] = fmaf(r0.w, o2, r0.z);
+}
+
+// ---- the fused sweep -----------------------------------------------------------------------------
+// One CTA per brick of cells. Its particles are the contiguous range that was sorted into the brick at
+// the last reorder (chunk[] = offset[] of the brick's first key); since then they have moved by a
+// fraction of a cell and the lattice shift has changed by less than a cell, so nearly all of them fall
+// into the brick's tile (brick + HALO cells on every side), held in shared memory as int32 sums. The
+// rest (and everything, if no order is known yet) goes to the global sums directly.
+template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY>
+__global__ void __launch_bounds__(SWEEP_T, 2)
+k_sweep(Geo G, float sp0, float sp1, float sp2, size_t n, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
+        float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, uint32_t* __restrict__ key_out,
+        const uint32_t* __restrict__ chunk, uint32_t nbricks, const float* __restrict__ rec, u64* __restrict__ sums) {
+  extern __shared__ int tile[];
+  const int T0 = (1 << G.bs[0]) + 2 * HALO, T1 = (1 << G.bs[1]) + 2 * HALO, T2 = (1 << G.bs[2]) + 2 * HALO;
+  const int tcells = T0 * T1 * T2;
+  for (int i = threadIdx.x; i < tcells * TILE_W; i += SWEEP_T) tile[i] = 0;
+  const uint32_t b = blockIdx.x;
+  int ox, oy, oz;
+  brick_to_origin(G, b, ox, oy, oz);
+  ox -= HALO; oy -= HALO; oz -= HALO;
+  size_t i0, i1;
+  if (chunk) {
+    const uint32_t bvol_shift = G.bs[0] + G.bs[1] + G.bs[2];
+    i0 = chunk[(size_t)b << bvol_shift];
+    i1 = (b + 1 == nbricks) ? n : (size_t)chunk[(size_t)(b + 1) << bvol_shift];
+  } else {   // no order known: even split, (almost) everything takes the global path
+    i0 = (size_t)((u64)n * b / nbricks);            // n < 2^32 and b < 2^32: no overflow
+    i1 = (size_t)((u64)n * (b + 1) / nbricks);
+  }
+  __syncthreads();
+  for (size_t i = i0 + threadIdx.x; i < i1; i += SWEEP_T) {
+    float r[3] = {x[i], y[i], z[i]}, v[3] = {vx[i], vy[i], vz[i]};
+    if (COLLIDE) {   // ROTATE_VELOCITIES of the previous step; its key is recomputed from r and that step's shift
+      const uint32_t kp = key_of(G, r[0], r[1], r[2], sp0, sp1, sp2);
+      const float4 r0 = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)kp * 2);
+      const float4 ax = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)kp * 2 + 1);
+      srd_apply(G, r0, ax, v);
+    }
+    stream_one<WALL, GRAV>(G, r, v);
+    x[i] = r[0]; y[i] = r[1]; z[i] = r[2];
+    vx[i] = v[0]; vy[i] = v[1]; vz[i] = v[2];
+    const int ix = cell_coord(G, 0, r[0], G.s[0]), iy = cell_coord(G, 1, r[1], G.s[1]), iz = cell_coord(G, 2, r[2], G.s[2]);
+    if (WKEY) key_out[i] = layout_key(G, ix, iy, iz);
+    const int a0 = __float2int_rn(v[0] * G.fxv), a1 = __float2int_rn(v[1] * G.fxv), a2 = __float2int_rn(v[2] * G.fxv);
+    const unsigned e = __float2uint_rn(fmaf(v[0], v[0], fmaf(v[1], v[1], v[2] * v[2])) * G.fxe);
+    int l0 = ix - ox, l1 = iy - oy, l2 = iz - oz;     // tile coordinates, periodic images folded in
+    if (l0 < 0) l0 += G.m[0]; else if (l0 >= G.m[0]) l0 -= G.m[0];
+    if (l1 < 0) l1 += G.m[1]; else if (l1 >= G.m[1]) l1 -= G.m[1];
+    if (l2 < 0) l2 += G.m[2]; else if (l2 >= G.m[2]) l2 -= G.m[2];
+    if (l0 < T0 && l1 < T1 && l2 < T2) {
+      int* s = tile + ((l2 * T1 + l1) * T0 + l0) * TILE_W;
+      atomicAdd(s, 1); atomicAdd(s + 1, a0); atomicAdd(s + 2, a1); atomicAdd(s + 3, a2); atomicAdd((unsigned*)s + 4, e);
+    } else {
+      u64* s = sums + (size_t)layout_key(G, ix, iy, iz) * G.sw;
+      atomicAdd(s, ((u64)e << 32) | 1ull); atomicAdd(s + 1, pack_ss(a0, a1)); atomicAdd(s + 2, pack_ss(a2, 0));
+    }
+  }
+  __syncthreads();
+  // flush the tile: one packed 64-bit reduction per pair of sums, empty cells skipped
+  for (int c = threadIdx.x; c < tcells; c += SWEEP_T) {
+    const int* s = tile + c * TILE_W;
+    const int cnt = s[0];
+    if (cnt == 0) continue;
+    const int l0 = c % T0, q = c / T0, l1 = q % T1, l2 = q / T1;
+    int ix = ox + l0, iy = oy + l1, iz = oz + l2;
+    if (ix < 0) ix += G.m[0]; else if (ix >= G.m[0]) ix -= G.m[0];
+    if (iy < 0) iy += G.m[1]; else if (iy >= G.m[1]) iy -= G.m[1];
+    if (iz < 0) iz += G.m[2]; else if (iz >= G.m[2]) iz -= G.m[2];
+    u64* g = sums + (size_t)layout_key(G, ix, iy, iz) * G.sw;
+    atomicAdd(g, ((u64)(unsigned)s[4] << 32) | (u64)(unsigned)cnt);
+    atomicAdd(g + 1, pack_ss(s[1], s[2]));
+    atomicAdd(g + 2, pack_ss(s[3], 0));
+  }
+}
+
+// trailing collision of the last step of a call (key recomputed from the position)
+__global__ void __launch_bounds__(256) k_collide_pos(Geo G, size_t n, const float* __restrict__ x, const float* __restrict__ y,
+                                                     const float* __restrict__ z, float* __restrict__ vx, float* __restrict__ vy,
+                                                     float* __restrict__ vz, const float* __restrict__ rec) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t k = key_of(G, x[i], y[i], z[i], G.s[0], G.s[1], G.s[2]);
+  const float4 r0 = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)k * 2);
+  const float4 ax = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)k * 2 + 1);
+  float v[3] = {vx[i], vy[i], vz[i]};
+  srd_apply(G, r0, ax, v);
+  vx[i] = v[0]; vy[i] = v[1]; vz[i] = v[2];
+}
+
+__global__ void __launch_bounds__(256) k_keys(Geo G, size_t n, const float* __restrict__ x, const float* __restrict__ y,
+                                              const float* __restrict__ z, uint32_t* __restrict__ key) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) key[i] = key_of(G, x[i], y[i], z[i], G.s[0], G.s[1], G.s[2]);
+}
+
+// ---- MPC-AT path (unfused) -----------------------------------------------------------------------
 template <bool WALL, bool GRAV>
 __global__ void __launch_bounds__(256) k_stream_key(Geo G, size_t n, float* __restrict__ x, float* __restrict__ y,
                                                     float* __restrict__ z, float* __restrict__ vx, float* __restrict__ vy,
-                                                    float* __restrict__ vz, uint32_t* __restrict__ key,
-                                                    uint32_t* __restrict__ hist) {
+                                                    float* __restrict__ vz, uint32_t* __restrict__ key, u64* __restrict__ sums) {
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   float r[3] = {x[i], y[i], z[i]}, v[3] = {vx[i], vy[i], vz[i]};
   stream_one<WALL, GRAV>(G, r, v);
   x[i] = r[0]; y[i] = r[1]; z[i] = r[2];
   if (WALL || GRAV) { vx[i] = v[0]; vy[i] = v[1]; vz[i] = v[2]; }
-  const uint32_t k = key_of(G, r[0], r[1], r[2]);
+  const uint32_t k = key_of(G, r[0], r[1], r[2], G.s[0], G.s[1], G.s[2]);
   key[i] = k;
-  if (hist) atomicAdd(&hist[k], 1u);
+  atomicAdd(sums + (size_t)k * G.sw, 1ull);            // histogram = the count field of word 0
+}
+// needs the reordered arrays: rank = position of the particle in its (key, id)-sorted cell segment (U5)
+__global__ void __launch_bounds__(256) k_accum_at(Geo G, size_t n, const float* __restrict__ vx, const float* __restrict__ vy,
+                                                  const float* __restrict__ vz, const uint32_t* __restrict__ key,
+                                                  const uint32_t* __restrict__ offset, u64* __restrict__ sums) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t k = key[i];
+  int ix, iy, iz;
+  key_to_cell(G, k, ix, iy, iz);
+  const Block4 o = philox(canonical_id(G, ix, iy, iz), (uint32_t)i - offset[k], G.t, TAG_AT, G.k0, G.k1);
+  float g0, g1, g2;
+  normals3(o, g0, g1, g2);
+  u64* s = sums + (size_t)k * G.sw;
+  atomicAdd(s + 1, pack_ss(__float2int_rn(vx[i] * G.fxv), __float2int_rn(vy[i] * G.fxv)));
+  atomicAdd(s + 2, pack_ss(__float2int_rn(vz[i] * G.fxv), __float2int_rn(G.sigma * g0 * G.fxv)));
+  atomicAdd(s + 3, pack_ss(__float2int_rn(G.sigma * g1 * G.fxv), __float2int_rn(G.sigma * g2 * G.fxv)));
+}
+__global__ void __launch_bounds__(256) k_collide_at(Geo G, size_t n, float* __restrict__ vx, float* __restrict__ vy,
+                                                    float* __restrict__ vz, const uint32_t* __restrict__ key,
+                                                    const uint32_t* __restrict__ offset, const float* __restrict__ rec) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t k = key[i];
+  const float4 r0 = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)k * 2);
+  int ix, iy, iz;
+  key_to_cell(G, k, ix, iy, iz);
+  const Block4 o = philox(canonical_id(G, ix, iy, iz), (uint32_t)i - offset[k], G.t, TAG_AT, G.k0, G.k1);
+  float g0, g1, g2;
+  normals3(o, g0, g1, g2);
+  vx[i] = r0.x + G.sigma * g0;
+  vy[i] = r0.y + G.sigma * g1;
+  vz[i] = r0.z + G.sigma * g2;
 }
 
-// ---- exclusive scan of uint32 (three kernels; tile = 2048) --------------------------------------
+// ---- exclusive scan of the per-cell counts (three kernels; tile = 2048) ----------------------------
+// `in` is read with a stride in 32-bit words: the count is the low word of word 0 of a cell's sums.
 constexpr int SCAN_T = 256, SCAN_PER = 8, SCAN_TILE = SCAN_T * SCAN_PER;
 
 __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t& total) {
@@ -182,23 +339,22 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t& t
       const uint32_t t = __shfl_up_sync(0xffffffffu, winc, o);
       if (lane >= o) winc += t;
     }
-    wsum[lane] = winc - w;          // exclusive offset of every warp
+    wsum[lane] = winc - w;            // exclusive offset of every warp
     if (lane == 31) wsum[32] = winc;  // block total
   }
   __syncthreads();
   const uint32_t res = wsum[warp] + inc - v;
   total = wsum[32];
-  __syncthreads();                  // wsum is reused by the caller's next round
+  __syncthreads();                    // wsum is reused by the caller's next round
   return res;
 }
-
-__global__ void __launch_bounds__(SCAN_T) k_scan_reduce(const uint32_t* __restrict__ in, size_t n, uint32_t* __restrict__ bsum) {
+__global__ void __launch_bounds__(SCAN_T) k_scan_reduce(const uint32_t* __restrict__ in, int stride, size_t n, uint32_t* __restrict__ bsum) {
   const size_t base = (size_t)blockIdx.x * SCAN_TILE;
   uint32_t s = 0;
 #pragma unroll
   for (int j = 0; j < SCAN_PER; ++j) {
     const size_t i = base + (size_t)j * SCAN_T + threadIdx.x;
-    if (i < n) s += in[i];
+    if (i < n) s += in[i * stride];
   }
   __shared__ uint32_t red[SCAN_T / 32];
 #pragma unroll
@@ -222,13 +378,13 @@ __global__ void __launch_bounds__(1024) k_scan_top(uint32_t* __restrict__ bsum, 
     carry += total;
   }
 }
-__global__ void __launch_bounds__(SCAN_T) k_scan_apply(const uint32_t* __restrict__ in, size_t n, const uint32_t* __restrict__ bsum,
-                                                       uint32_t* __restrict__ out) {
+__global__ void __launch_bounds__(SCAN_T) k_scan_apply(const uint32_t* __restrict__ in, int stride, size_t n,
+                                                       const uint32_t* __restrict__ bsum, uint32_t* __restrict__ out) {
   const size_t base = (size_t)blockIdx.x * SCAN_TILE + (size_t)threadIdx.x * SCAN_PER;
   uint32_t v[SCAN_PER], s = 0;
 #pragma unroll
   for (int j = 0; j < SCAN_PER; ++j) {
-    v[j] = (base + j < n) ? in[base + j] : 0u;
+    v[j] = (base + j < n) ? in[(base + j) * stride] : 0u;
     s += v[j];
   }
   uint32_t total;
@@ -264,64 +420,31 @@ __global__ void __launch_bounds__(256) k_rank(size_t n, const uint32_t* __restri
   perm[b + r] = (uint32_t)i;
 }
 struct Arrays8 { void* p[8]; };
-__global__ void __launch_bounds__(256) k_gather8(size_t n, const uint32_t* __restrict__ perm, Arrays8 src, Arrays8 dst) {
+template <int NA>
+__global__ void __launch_bounds__(256) k_gather(size_t n, const uint32_t* __restrict__ perm, Arrays8 src, Arrays8 dst) {
   const size_t d = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (d >= n) return;
   const uint32_t s = perm[d];
-  uint32_t v[8];
+  uint32_t v[NA];
 #pragma unroll
-  for (int a = 0; a < 8; ++a) v[a] = ((const uint32_t*)src.p[a])[s];
+  for (int a = 0; a < NA; ++a) v[a] = ((const uint32_t*)src.p[a])[s];
 #pragma unroll
-  for (int a = 0; a < 8; ++a) ((uint32_t*)dst.p[a])[d] = v[a];
-}
-__global__ void __launch_bounds__(256) k_gather1(size_t n, const uint32_t* __restrict__ perm, const uint32_t* __restrict__ src,
-                                                 uint32_t* __restrict__ dst) {
-  const size_t d = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (d >= n) return;
-  dst[d] = src[perm[d]];
+  for (int a = 0; a < NA; ++a) ((uint32_t*)dst.p[a])[d] = v[a];
 }
 __global__ void __launch_bounds__(256) k_iota(size_t n, uint32_t* __restrict__ id) {
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) id[i] = (uint32_t)i;
 }
 
-// ---- PROCESS: per-cell sums ----------------------------------------------------------------------
-// sums[key] = { N, Sx, Sy, Sz, E | R0, R1, R2 (MPC-AT) }
-template <bool AT>
-__global__ void __launch_bounds__(256) k_accum(Geo G, size_t n, const float* __restrict__ vx, const float* __restrict__ vy,
-                                               const float* __restrict__ vz, const uint32_t* __restrict__ key,
-                                               const uint32_t* __restrict__ offset, int* __restrict__ sums) {
-  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const uint32_t k = key[i];
-  const float a = vx[i], b = vy[i], c = vz[i];
-  int* s = sums + (size_t)k * SUMS_W;
-  atomicAdd((unsigned*)s, 1u);
-  atomicAdd(s + 1, __float2int_rn(a * G.fxv));
-  atomicAdd(s + 2, __float2int_rn(b * G.fxv));
-  atomicAdd(s + 3, __float2int_rn(c * G.fxv));
-  if (!AT) {
-    const float e = fmaf(a, a, fmaf(b, b, c * c));
-    atomicAdd((unsigned*)(s + 4), __float2uint_rn(e * G.fxe));
-  } else {
-    int ix, iy, iz;
-    key_to_cell(G, k, ix, iy, iz);
-    const uint32_t rank = (uint32_t)i - offset[k];
-    const Block4 o = philox(canonical_id(G, ix, iy, iz), rank, G.t, TAG_AT, G.k0, G.k1);
-    float g0, g1, g2;
-    normals3(o, g0, g1, g2);
-    atomicAdd(s + 5, __float2int_rn(G.sigma * g0 * G.fxv));
-    atomicAdd(s + 6, __float2int_rn(G.sigma * g1 * G.fxv));
-    atomicAdd(s + 7, __float2int_rn(G.sigma * g2 * G.fxv));
-  }
-}
-
 // ---- PROCESS_CELLS -------------------------------------------------------------------------------
-// E_k / k_BT ~ Gamma(3(Nc-1)/2, 1): floor(f/2) unit exponentials (+ half a squared normal if f is odd)
+// E_k / k_BT ~ Gamma(3(Nc-1)/2, 1) (Eq. 7; U6): minus the log of a product of floor(f/2)
+// uniforms (the product is renormalised with frexp so it never underflows: one log per cell instead
+// of one per uniform), plus half a squared normal if f is odd.
 __device__ float mbs_energy(const Geo& G, uint32_t cid, uint32_t Nc) {
   const uint32_t f = 3u * (Nc - 1u), M = f >> 1, odd = f & 1u;
   const uint32_t need = M + 2u * odd;
-  float e = 0.0f, lg = 0.0f, cs = 0.0f;
+  float p = 1.0f, um = 1.0f, cs = 0.0f;
+  int ex = 0;
   uint32_t sub = 0;
   for (uint32_t base = 0; base < need; base += 4, ++sub) {
     const Block4 o = philox(cid, sub, G.t, TAG_MBS, G.k0, G.k1);
@@ -329,37 +452,46 @@ __device__ float mbs_energy(const Geo& G, uint32_t cid, uint32_t Nc) {
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const uint32_t pos = base + q;
-      if (pos < M) e -= logf(u01_oc(w[q]));
-      else if (odd && pos == M) lg = -logf(u01_oc(w[q]));
+      if (pos < M) p *= u01_oc(w[q]);                       // >= 2^-24 each: 4 factors cannot underflow
+      else if (odd && pos == M) um = u01_oc(w[q]);
       else if (odd && pos == M + 1u) cs = cospif(2.0f * u01_co(w[q]));
     }
+    int e;
+    p = frexpf(p, &e);
+    ex += e;
   }
-  if (odd) e += lg * cs * cs;
+  float e = -(float)((double)logf(p) + (double)ex * 0.6931471805599453);
+  if (odd) e -= logf(um) * cs * cs;
   return e;
 }
 
 // rec[key] = SRD: { vcm.x, vcm.y, vcm.z, kappa, n.x, n.y, n.z, - }   AT: { (vcm - mean v_ran).xyz, ... }
-__global__ void __launch_bounds__(128) k_cell(Geo G, const int* __restrict__ sums, float* __restrict__ rec) {
+__global__ void __launch_bounds__(128) k_cell(Geo G, const u64* __restrict__ sums, float* __restrict__ rec) {
   const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= G.nkeys) return;
-  const int4 s0 = reinterpret_cast<const int4*>(sums)[(size_t)k * 2];
-  const uint32_t nreal = (uint32_t)s0.x;
+  const u64* s = sums + (size_t)k * G.sw;
+  const u64 w0 = s[0];
+  const uint32_t nreal = (uint32_t)(w0 & 0xffffffffull);
   if (nreal == 0u) return;
-  const int4 s1 = reinterpret_cast<const int4*>(sums)[(size_t)k * 2 + 1];
   int ix, iy, iz;
   key_to_cell(G, k, ix, iy, iz);
   const uint32_t cid = canonical_id(G, ix, iy, iz);
-  double S0 = (double)s0.y * G.fxv_inv, S1 = (double)s0.z * G.fxv_inv, S2 = (double)s0.w * G.fxv_inv;
+  int sx, sy, sz, r0i;
+  unpack_ss(s[1], sx, sy);
+  unpack_ss(s[2], sz, r0i);
+  double S0 = (double)sx * G.fxv_inv, S1 = (double)sy * G.fxv_inv, S2 = (double)sz * G.fxv_inv;
   float4 r0, r1;
   if (G.collision == 1) {
+    int r1i, r2i;
+    unpack_ss(s[3], r1i, r2i);
     const double inv = 1.0 / (double)nreal;
-    r0.x = (float)((S0 - (double)s1.y * G.fxv_inv) * inv);
-    r0.y = (float)((S1 - (double)s1.z * G.fxv_inv) * inv);
-    r0.z = (float)((S2 - (double)s1.w * G.fxv_inv) * inv);
+    r0.x = (float)((S0 - (double)r0i * G.fxv_inv) * inv);
+    r0.y = (float)((S1 - (double)r1i * G.fxv_inv) * inv);
+    r0.z = (float)((S2 - (double)r2i * G.fxv_inv) * inv);
     r0.w = 1.0f;
     r1 = make_float4(0.f, 0.f, 0.f, 0.f);
   } else {
-    double E = (double)(uint32_t)s1.x * G.fxe_inv;
+    double E = (double)(uint32_t)(w0 >> 32) * G.fxe_inv;
     uint32_t Nc = nreal;
     if (G.wall >= 0) {
       // virtual wall particles fill wall-cut cells up to nbar (U8)
@@ -402,40 +534,6 @@ __global__ void __launch_bounds__(128) k_cell(Geo G, const int* __restrict__ sum
   reinterpret_cast<float4*>(rec)[(size_t)k * 2 + 1] = r1;
 }
 
-// ---- ROTATE_VELOCITIES ---------------------------------------------------------------------------
-template <bool AT>
-__global__ void __launch_bounds__(256) k_collide(Geo G, size_t n, float* __restrict__ vx, float* __restrict__ vy,
-                                                 float* __restrict__ vz, const uint32_t* __restrict__ key,
-                                                 const uint32_t* __restrict__ offset, const float* __restrict__ rec) {
-  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const uint32_t k = key[i];
-  const float4 r0 = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)k * 2);
-  if (AT) {
-    int ix, iy, iz;
-    key_to_cell(G, k, ix, iy, iz);
-    const uint32_t rank = (uint32_t)i - offset[k];
-    const Block4 o = philox(canonical_id(G, ix, iy, iz), rank, G.t, TAG_AT, G.k0, G.k1);
-    float g0, g1, g2;
-    normals3(o, g0, g1, g2);
-    vx[i] = r0.x + G.sigma * g0;
-    vy[i] = r0.y + G.sigma * g1;
-    vz[i] = r0.z + G.sigma * g2;
-  } else {
-    const float4 ax = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)k * 2 + 1);
-    const float w0 = vx[i] - r0.x, w1 = vy[i] - r0.y, w2 = vz[i] - r0.z;
-    const float c = G.cosa, s = G.sina, omc = 1.0f - G.cosa;
-    const float nd = fmaf(ax.x, w0, fmaf(ax.y, w1, ax.z * w2)) * omc;
-    const float cx = fmaf(ax.y, w2, -(ax.z * w1)), cy = fmaf(ax.z, w0, -(ax.x * w2)), cz = fmaf(ax.x, w1, -(ax.y * w0));
-    const float o0 = fmaf(w0, c, fmaf(cx, s, ax.x * nd));
-    const float o1 = fmaf(w1, c, fmaf(cy, s, ax.y * nd));
-    const float o2 = fmaf(w2, c, fmaf(cz, s, ax.z * nd));
-    vx[i] = fmaf(r0.w, o0, r0.x);
-    vy[i] = fmaf(r0.w, o1, r0.y);
-    vz[i] = fmaf(r0.w, o2, r0.z);
-  }
-}
-
 // ---- observables ---------------------------------------------------------------------------------
 __device__ __forceinline__ double block_sum(double v, double* sh) {
 #pragma unroll
@@ -458,7 +556,7 @@ __global__ void __launch_bounds__(256) k_obs_particles(size_t n, const float* __
   a = block_sum(a, sh); b = block_sum(b, sh); c = block_sum(c, sh); e = block_sum(e, sh);
   if (threadIdx.x == 0) { double* o = part + (size_t)blockIdx.x * 8; o[0] = a; o[1] = b; o[2] = c; o[3] = e; }
 }
-__global__ void __launch_bounds__(256) k_obs_cells(Geo G, const int* __restrict__ sums, double* __restrict__ part) {
+__global__ void __launch_bounds__(256) k_obs_cells(Geo G, const u64* __restrict__ sums, double* __restrict__ part) {
   __shared__ double sh[8];
   __shared__ unsigned smax;
   if (threadIdx.x == 0) smax = 0;
@@ -466,20 +564,23 @@ __global__ void __launch_bounds__(256) k_obs_cells(Geo G, const int* __restrict_
   double num = 0, den = 0;
   unsigned mx = 0;
   for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < G.nkeys; k += (size_t)gridDim.x * blockDim.x) {
-    const int4 s0 = reinterpret_cast<const int4*>(sums)[k * 2];
-    const unsigned nc = (unsigned)s0.x;
+    const u64* s = sums + k * G.sw;
+    const u64 w0 = s[0];
+    const unsigned nc = (unsigned)(w0 & 0xffffffffull);
     mx = max(mx, nc);
-    if (nc < 2u) continue;
-    const unsigned e = (unsigned)sums[k * SUMS_W + 4];
-    const double S0 = s0.y * G.fxv_inv, S1 = s0.z * G.fxv_inv, S2 = s0.w * G.fxv_inv;
-    num += (double)G.mass * ((double)e * G.fxe_inv - (S0 * S0 + S1 * S1 + S2 * S2) / nc);
+    if (nc < 2u || G.collision == 1) continue;
+    int sx, sy, sz, sp;
+    unpack_ss(s[1], sx, sy);
+    unpack_ss(s[2], sz, sp);
+    const double S0 = sx * G.fxv_inv, S1 = sy * G.fxv_inv, S2 = sz * G.fxv_inv;
+    num += (double)G.mass * ((double)(unsigned)(w0 >> 32) * G.fxe_inv - (S0 * S0 + S1 * S1 + S2 * S2) / nc);
     den += 3.0 * (nc - 1u);
   }
   atomicMax(&smax, mx);
   num = block_sum(num, sh); den = block_sum(den, sh);
   if (threadIdx.x == 0) { double* o = part + (size_t)blockIdx.x * 8; o[4] = num; o[5] = den; o[6] = (double)smax; }
 }
-__global__ void __launch_bounds__(256) k_obs_profile(Geo G, size_t n, int pa, int nb, const float* __restrict__ rp,
+__global__ void __launch_bounds__(256) k_obs_profile(Geo G, size_t n, int nb, const float* __restrict__ rp,
                                                      const float* __restrict__ vf, double* __restrict__ prof) {
   extern __shared__ double bins[];   // nb sums, nb counts
   for (int b = threadIdx.x; b < 2 * nb; b += blockDim.x) bins[b] = 0.0;
@@ -493,18 +594,20 @@ __global__ void __launch_bounds__(256) k_obs_profile(Geo G, size_t n, int pa, in
   __syncthreads();
   for (int b = threadIdx.x; b < 2 * nb; b += blockDim.x) if (bins[b] != 0.0) atomicAdd(&prof[b], bins[b]);
 }
-template <bool AT>
-__global__ void __launch_bounds__(256) k_export_cells(Geo G, const int* __restrict__ sums, unsigned* __restrict__ count,
+__global__ void __launch_bounds__(256) k_export_cells(Geo G, const u64* __restrict__ sums, unsigned* __restrict__ count,
                                                       float* __restrict__ px, float* __restrict__ py, float* __restrict__ pz,
                                                       float* __restrict__ e2) {
   const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= G.nkeys) return;
-  const int* s = sums + k * SUMS_W;
-  if (count) count[k] = (unsigned)s[0];
-  if (px) px[k] = (float)((double)G.mass * s[1] * G.fxv_inv);
-  if (py) py[k] = (float)((double)G.mass * s[2] * G.fxv_inv);
-  if (pz) pz[k] = (float)((double)G.mass * s[3] * G.fxv_inv);
-  if (e2) e2[k] = AT ? 0.0f : (float)((double)(unsigned)s[4] * G.fxe_inv);
+  const u64* s = sums + k * G.sw;
+  int sx, sy, sz, sp;
+  unpack_ss(s[1], sx, sy);
+  unpack_ss(s[2], sz, sp);
+  if (count) count[k] = (unsigned)(s[0] & 0xffffffffull);
+  if (px) px[k] = (float)((double)G.mass * sx * G.fxv_inv);
+  if (py) py[k] = (float)((double)G.mass * sy * G.fxv_inv);
+  if (pz) pz[k] = (float)((double)G.mass * sz * G.fxv_inv);
+  if (e2) e2[k] = (G.collision == 1) ? 0.0f : (float)((double)(unsigned)(s[0] >> 32) * G.fxe_inv);
 }
 
 }  // namespace mpc
@@ -514,35 +617,35 @@ __global__ void __launch_bounds__(256) k_export_cells(Geo G, const int* __restri
 // =================================================================================================
 using namespace mpc;
 
-enum Family { F_STREAM = 0, F_SCAN, F_SCATTER, F_RANK, F_GATHER, F_ACCUM, F_CELL, F_COLLIDE, F_MEMSET, F_OBS, F_COUNT };
-static const char* const FAMILY_NAMES[F_COUNT] = {"stream_key", "scan", "scatter_ids", "rank", "gather", "accum", "cell",
-                                                  "collide", "memset", "observables"};
+enum Family { F_SWEEP = 0, F_CELL, F_COLLIDE, F_SCAN, F_SCATTER, F_RANK, F_GATHER, F_MEMSET, F_STREAM, F_ACCUM, F_OBS, F_COUNT };
+static const char* const FAMILY_NAMES[F_COUNT] = {"sweep", "cell", "collide", "scan", "scatter_ids", "rank", "gather", "memset",
+                                                  "stream_key", "accum", "observables"};
 constexpr int PROF_MAX_PAIRS = 16384;
 
 struct mpc_ctx {
   Geo G;
   mpc_params p;
-  float box[3];
-  int cells[3];
   unsigned long long seed;
   uint32_t t;
   size_t n, n_max;
-  bool bound, have_state, have_cells, compact, sticky;
+  bool bound, have_state, have_cells, have_order, compact, sticky;
   cudaStream_t stream;
   char* ws;
   size_t ws_bytes;
+  uint32_t nbricks;
+  size_t tile_bytes;
   // device arrays
-  uint32_t* A[8];   // x y z vx vy vz id key (current)
-  uint32_t* Bf[8];  // second copy (non-compact) ; Bf[0] = 4-byte temp (compact)
-  uint32_t *slot_id, *perm, *hist, *offset, *bsum;
-  int* sums;
+  uint32_t* A[7];   // x y z vx vy vz id (current)
+  uint32_t* Bf[7];  // second copy (non-compact); Bf[0] = 4-byte temp (compact)
+  uint32_t *key, *slot_id, *perm, *cursor, *offset, *bsum;
+  u64* sums;
   float* rec;
   double* obs;      // OBS_BLOCKS*8 doubles + 2*MAX_PROFILE doubles
   double* hbuf;     // host staging for mpc_observables
   // optional per-family timing with CUDA events on the bound stream (mpc_profile_*)
   bool prof_on;
-  cudaEvent_t* prof_ev;          // 2 * PROF_MAX_PAIRS events, created on first enable
-  int* prof_fam;                 // family of every recorded pair
+  cudaEvent_t* prof_ev;
+  int* prof_fam;
   int prof_pairs;
   double prof_ms[F_COUNT];
   unsigned long long prof_launches[F_COUNT];
@@ -555,24 +658,25 @@ namespace {
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  size_t off_A[8], off_B[8], off_slot, off_perm, off_hist, off_offset, off_bsum, off_sums, off_rec, off_obs, total;
+  size_t off_A[7], off_B[7], off_key, off_slot, off_perm, off_cursor, off_offset, off_bsum, off_sums, off_rec, off_obs, total;
 };
-Layout make_layout(size_t n_max, size_t nkeys, bool compact) {
+Layout make_layout(size_t n_max, size_t nkeys, int sw, bool compact) {
   Layout l;
   size_t o = 0;
   auto take = [&](size_t bytes) { const size_t r = o; o = align_up(o + bytes, 256); return r; };
   const size_t pn = (n_max ? n_max : 1) * 4;
-  for (int a = 0; a < 8; ++a) l.off_A[a] = take(pn);
-  if (compact) { l.off_B[0] = take(pn); for (int a = 1; a < 8; ++a) l.off_B[a] = l.off_B[0]; }
-  else for (int a = 0; a < 8; ++a) l.off_B[a] = take(pn);
+  for (int a = 0; a < 7; ++a) l.off_A[a] = take(pn);
+  if (compact) { l.off_B[0] = take(pn); for (int a = 1; a < 7; ++a) l.off_B[a] = l.off_B[0]; }
+  else for (int a = 0; a < 7; ++a) l.off_B[a] = take(pn);
+  l.off_key = take(pn);
   l.off_slot = take(pn);
   l.off_perm = take(pn);
-  l.off_hist = take(nkeys * 4);
+  l.off_cursor = take(nkeys * 4);
   l.off_offset = take((nkeys + 1) * 4);
   l.off_bsum = take(((nkeys + SCAN_TILE - 1) / SCAN_TILE + 1) * 4);
-  l.off_sums = take(nkeys * SUMS_W * 4);
+  l.off_sums = take(nkeys * (size_t)sw * 8);
   l.off_rec = take(nkeys * REC_W * 4);
-  l.off_obs = take((size_t)OBS_BLOCKS * 8 * 8 + (size_t)2 * MAX_PROFILE * 8);
+  l.off_obs = take(OBS_HOST_DOUBLES * 8);
   l.total = o;
   return l;
 }
@@ -620,99 +724,155 @@ void host_shift(const mpc_ctx* c, uint32_t t, float s[3]) {
   s[2] = (u01_co(o.c) - 0.5f) * c->G.a;
 }
 
-int do_scan(mpc_ctx* c) {
-  const size_t nk = c->G.nkeys, nb = (nk + SCAN_TILE - 1) / SCAN_TILE;
-  FamilyTimer ft(c, F_SCAN);
-  k_scan_reduce<<<(unsigned)nb, SCAN_T, 0, c->stream>>>(c->hist, nk, c->bsum);
-  LAUNCH_CHECK("k_scan_reduce");
-  k_scan_top<<<1, 1024, 0, c->stream>>>(c->bsum, nb);
-  LAUNCH_CHECK("k_scan_top");
-  k_scan_apply<<<(unsigned)nb, SCAN_T, 0, c->stream>>>(c->hist, nk, c->bsum, c->offset);
-  LAUNCH_CHECK("k_scan_apply");
-  return MPC_OK;
-}
-
+// counting-sort reorder by (key, id); counts = low word of word 0 of the sums; c->key holds the keys
 int do_reorder(mpc_ctx* c) {
-  const size_t n = c->n;
-  int rc = do_scan(c);
-  if (rc) return rc;
-  { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->hist, 0, (size_t)c->G.nkeys * 4, c->stream)); }   // reuse as cursor
+  const size_t n = c->n, nk = c->G.nkeys, nb = (nk + SCAN_TILE - 1) / SCAN_TILE;
+  const uint32_t* cnt = reinterpret_cast<const uint32_t*>(c->sums);
+  const int stride = c->G.sw * 2;
+  {
+    FamilyTimer ft(c, F_SCAN);
+    k_scan_reduce<<<(unsigned)nb, SCAN_T, 0, c->stream>>>(cnt, stride, nk, c->bsum);
+    LAUNCH_CHECK("k_scan_reduce");
+    k_scan_top<<<1, 1024, 0, c->stream>>>(c->bsum, nb);
+    LAUNCH_CHECK("k_scan_top");
+    k_scan_apply<<<(unsigned)nb, SCAN_T, 0, c->stream>>>(cnt, stride, nk, c->bsum, c->offset);
+    LAUNCH_CHECK("k_scan_apply");
+  }
+  { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->cursor, 0, nk * 4, c->stream)); }
   {
     FamilyTimer ft(c, F_SCATTER);
-    k_scatter_ids<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->A[7], c->A[6], c->offset, c->hist, c->slot_id);
+    k_scatter_ids<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->key, c->A[6], c->offset, c->cursor, c->slot_id);
     LAUNCH_CHECK("k_scatter_ids");
   }
   {
     FamilyTimer ft(c, F_RANK);
-    k_rank<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->A[7], c->A[6], c->offset, c->slot_id, c->perm);
+    k_rank<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->key, c->A[6], c->offset, c->slot_id, c->perm);
     LAUNCH_CHECK("k_rank");
   }
   FamilyTimer ftg(c, F_GATHER);
+  const bool need_key = c->G.collision == 1;   // MPC-AT reads the sorted keys afterwards
   if (!c->compact) {
     Arrays8 src, dst;
-    for (int a = 0; a < 8; ++a) { src.p[a] = c->A[a]; dst.p[a] = c->Bf[a]; }
-    k_gather8<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
-    LAUNCH_CHECK("k_gather8");
-    for (int a = 0; a < 8; ++a) { uint32_t* t = c->A[a]; c->A[a] = c->Bf[a]; c->Bf[a] = t; }
+    for (int a = 0; a < 7; ++a) { src.p[a] = c->A[a]; dst.p[a] = c->Bf[a]; }
+    src.p[7] = c->key; dst.p[7] = c->slot_id;   // slot_id is free after k_rank
+    if (need_key) k_gather<8><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
+    else k_gather<7><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
+    LAUNCH_CHECK("k_gather");
+    for (int a = 0; a < 7; ++a) { uint32_t* t = c->A[a]; c->A[a] = c->Bf[a]; c->Bf[a] = t; }
+    if (need_key) { uint32_t* t = c->key; c->key = c->slot_id; c->slot_id = t; }
   } else {
     // property-wise through one temporary array
-    for (int a = 0; a < 8; ++a) {
-      CU(cudaMemcpyAsync(c->Bf[0], c->A[a], n * 4, cudaMemcpyDeviceToDevice, c->stream));
-      k_gather1<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, c->Bf[0], c->A[a]);
-      LAUNCH_CHECK("k_gather1");
+    Arrays8 src, dst;
+    for (int a = 0; a < (need_key ? 8 : 7); ++a) {
+      uint32_t* arr = a < 7 ? c->A[a] : c->key;
+      CU(cudaMemcpyAsync(c->Bf[0], arr, n * 4, cudaMemcpyDeviceToDevice, c->stream));
+      src.p[0] = c->Bf[0]; dst.p[0] = arr;
+      k_gather<1><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
+      LAUNCH_CHECK("k_gather");
     }
+  }
+  c->have_order = true;
+  return MPC_OK;
+}
+
+template <bool COLLIDE, bool WKEY>
+int launch_sweep(mpc_ctx* c, const float sp[3]) {
+  const Geo& G = c->G;
+  float** F = reinterpret_cast<float**>(c->A);
+  const uint32_t* chunk = c->have_order ? c->offset : nullptr;
+  const bool wall = G.wall >= 0, grav = (G.g[0] != 0.f || G.g[1] != 0.f || G.g[2] != 0.f);
+#define SWEEP_ARGS G, sp[0], sp[1], sp[2], c->n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, chunk, c->nbricks, c->rec, c->sums
+  if (wall && grav) k_sweep<COLLIDE, true, true, WKEY><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
+  else if (wall) k_sweep<COLLIDE, true, false, WKEY><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
+  else if (grav) k_sweep<COLLIDE, false, true, WKEY><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
+  else k_sweep<COLLIDE, false, false, WKEY><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
+#undef SWEEP_ARGS
+  LAUNCH_CHECK("k_sweep");
+  return MPC_OK;
+}
+
+template <bool COLLIDE, bool WKEY>
+cudaError_t sweep_attr(size_t bytes) {
+  cudaError_t e;
+  if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, true, WKEY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+  if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, false, WKEY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+  if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, true, WKEY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+  return cudaFuncSetAttribute(k_sweep<COLLIDE, false, false, WKEY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+// SRD: n steps = sweep(no collide), cell, [sweep(collide t-1 + move t), cell] x (n-1), trailing collide
+int steps_srd(mpc_ctx* c, int nsteps) {
+  Geo& G = c->G;
+  const size_t n = c->n;
+  float sp[3] = {0.f, 0.f, 0.f};
+  for (int k = 0; k < nsteps; ++k) {
+    G.t = c->t;
+    host_shift(c, c->t, G.s);
+    const bool rebin = (c->t % (uint32_t)c->p.rebin_every) == 0u;
+    { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * G.sw * 8, c->stream)); }
+    if (n) {
+      {
+        FamilyTimer ft(c, F_SWEEP);
+        int rc;
+        if (k == 0) rc = rebin ? launch_sweep<false, true>(c, sp) : launch_sweep<false, false>(c, sp);
+        else rc = rebin ? launch_sweep<true, true>(c, sp) : launch_sweep<true, false>(c, sp);
+        if (rc) return rc;
+      }
+      if (rebin) { const int rc = do_reorder(c); if (rc) return rc; }
+      FamilyTimer ft(c, F_CELL);
+      k_cell<<<nblk(G.nkeys, 128), 128, 0, c->stream>>>(G, c->sums, c->rec);
+      LAUNCH_CHECK("k_cell");
+    }
+    sp[0] = G.s[0]; sp[1] = G.s[1]; sp[2] = G.s[2];
+    c->t++;
+    c->have_cells = true;
+  }
+  if (nsteps > 0 && n) {
+    float** F = reinterpret_cast<float**>(c->A);
+    FamilyTimer ft(c, F_COLLIDE);
+    k_collide_pos<<<nblk(n, 256), 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->rec);
+    LAUNCH_CHECK("k_collide_pos");
   }
   return MPC_OK;
 }
 
-int one_step(mpc_ctx* c) {
-  const size_t n = c->n;
+int steps_at(mpc_ctx* c, int nsteps) {
   Geo& G = c->G;
-  G.t = c->t;
-  host_shift(c, c->t, G.s);
-  const bool rebin = (c->t % (uint32_t)c->p.rebin_every) == 0u;
-  float** F = reinterpret_cast<float**>(c->A);
-  {
-    FamilyTimer ft(c, F_MEMSET);
-    CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * SUMS_W * 4, c->stream));
-    if (rebin) CU(cudaMemsetAsync(c->hist, 0, (size_t)G.nkeys * 4, c->stream));
+  const size_t n = c->n;
+  for (int k = 0; k < nsteps; ++k) {
+    G.t = c->t;
+    host_shift(c, c->t, G.s);
+    { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * G.sw * 8, c->stream)); }
+    if (n) {
+      float** F = reinterpret_cast<float**>(c->A);
+      const unsigned gb = nblk(n, 256);
+      const bool grav = (G.g[0] != 0.f || G.g[1] != 0.f || G.g[2] != 0.f);
+      {
+        FamilyTimer ft(c, F_STREAM);
+        if (grav) k_stream_key<false, true><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, c->sums);
+        else k_stream_key<false, false><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, c->sums);
+        LAUNCH_CHECK("k_stream_key");
+      }
+      const int rc = do_reorder(c);   // MPC-AT reorders every step (rebin_every == 1)
+      if (rc) return rc;
+      F = reinterpret_cast<float**>(c->A);
+      {
+        FamilyTimer ft(c, F_ACCUM);
+        k_accum_at<<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->key, c->offset, c->sums);
+        LAUNCH_CHECK("k_accum_at");
+      }
+      {
+        FamilyTimer ft(c, F_CELL);
+        k_cell<<<nblk(G.nkeys, 128), 128, 0, c->stream>>>(G, c->sums, c->rec);
+        LAUNCH_CHECK("k_cell");
+      }
+      FamilyTimer ft(c, F_COLLIDE);
+      k_collide_at<<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->key, c->offset, c->rec);
+      LAUNCH_CHECK("k_collide_at");
+    }
+    c->t++;
+    c->have_cells = true;
   }
-  if (n == 0) { c->t++; c->have_cells = true; return MPC_OK; }
-  uint32_t* hist = rebin ? c->hist : nullptr;
-  const bool wall = G.wall >= 0, grav = (G.g[0] != 0.f || G.g[1] != 0.f || G.g[2] != 0.f);
-  const unsigned gb = nblk(n, 256);
-  {
-  FamilyTimer ft(c, F_STREAM);
-  if (wall && grav) k_stream_key<true, true><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->A[7], hist);
-  else if (wall) k_stream_key<true, false><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->A[7], hist);
-  else if (grav) k_stream_key<false, true><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->A[7], hist);
-  else k_stream_key<false, false><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->A[7], hist);
-  LAUNCH_CHECK("k_stream_key");
-  }
-  if (rebin) {
-    const int rc = do_reorder(c);
-    if (rc) return rc;
-    F = reinterpret_cast<float**>(c->A);
-  }
-  {
-    FamilyTimer ft(c, F_ACCUM);
-    if (G.collision == 1) k_accum<true><<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->A[7], c->offset, c->sums);
-    else k_accum<false><<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->A[7], c->offset, c->sums);
-    LAUNCH_CHECK("k_accum");
-  }
-  {
-    FamilyTimer ft(c, F_CELL);
-    k_cell<<<nblk(G.nkeys, 128), 128, 0, c->stream>>>(G, c->sums, c->rec);
-    LAUNCH_CHECK("k_cell");
-  }
-  {
-    FamilyTimer ft(c, F_COLLIDE);
-    if (G.collision == 1) k_collide<true><<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->A[7], c->offset, c->rec);
-    else k_collide<false><<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->A[7], c->offset, c->rec);
-    LAUNCH_CHECK("k_collide");
-  }
-  c->t++;
-  c->have_cells = true;
   return MPC_OK;
 }
 
@@ -729,7 +889,7 @@ int set_state_impl(mpc_ctx* c, unsigned long long n, const float* const src[6], 
     if (id) CU(cudaMemcpyAsync(c->A[6], id, n * 4, kind, c->stream));
     else { k_iota<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->A[6]); LAUNCH_CHECK("k_iota"); }
   }
-  c->n = n; c->t = step; c->have_state = true; c->have_cells = false;
+  c->n = n; c->t = step; c->have_state = true; c->have_cells = false; c->have_order = false;
   return MPC_OK;
 }
 int get_state_impl(mpc_ctx* c, float* const dst[6], unsigned* id, cudaMemcpyKind kind) {
@@ -757,7 +917,13 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   for (int d = 1; d < 3; ++d) if (box[d] / (float)cells[d] != a) return MPC_EINVAL;
   if (p->collision < 0 || p->collision > 1) return MPC_EINVAL;
   if (!(p->dt > 0.0f) || !(p->kT > 0.0f) || !(p->mass > 0.0f) || p->rebin_every < 1 || !(n_per_cell > 0.0f)) return MPC_EINVAL;
-  if (p->brick < 1 || (p->brick & (p->brick - 1)) != 0 || p->brick > 64) return MPC_EINVAL;   // power of two
+  size_t tile_cells = 1;
+  for (int d = 0; d < 3; ++d) {
+    const int b = p->brick[d];
+    if (b < 1 || (b & (b - 1)) != 0 || b > 64) return MPC_EINVAL;   // powers of two
+    tile_cells *= (size_t)(b + 2 * HALO);
+  }
+  if (tile_cells * TILE_W * 4 > MAX_TILE_BYTES) return MPC_EINVAL;
   int nwall = 0, wall = -1;
   for (int d = 0; d < 3; ++d) {
     if (p->bc[d] != 0 && p->bc[d] != 1) return MPC_EINVAL;
@@ -774,19 +940,22 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   c->hbuf = new (std::nothrow) double[OBS_HOST_DOUBLES];
   if (!c->hbuf) { delete c; return MPC_ENOMEM; }
   Geo& G = c->G;
-  int bs = 0;
-  while ((1 << bs) < p->brick) ++bs;
-  G.bshift = bs; G.a = a; G.inv_a = 1.0f / a; G.wall = wall;
-  unsigned long long nk = 1;
+  G.a = a; G.inv_a = 1.0f / a; G.wall = wall;
+  unsigned long long nk = 1, nbr = 1;
   for (int d = 0; d < 3; ++d) {
-    c->box[d] = box[d]; c->cells[d] = cells[d];
+    int bs = 0;
+    while ((1 << bs) < p->brick[d]) ++bs;
+    G.bs[d] = bs;
     G.L[d] = box[d]; G.n[d] = cells[d]; G.bc[d] = p->bc[d]; G.g[d] = p->g[d];
     G.m[d] = cells[d] + (p->bc[d] == 1 ? 2 : 0);
-    G.mb[d] = (G.m[d] + p->brick - 1) >> bs;
+    G.mb[d] = (G.m[d] + p->brick[d] - 1) >> bs;
     nk *= (unsigned long long)G.mb[d] << bs;
+    nbr *= (unsigned long long)G.mb[d];
   }
   if (nk >= 0xffffffffull) { delete[] c->hbuf; delete c; return MPC_EINVAL; }
   G.nkeys = (uint32_t)nk;
+  c->nbricks = (uint32_t)nbr;
+  c->tile_bytes = tile_cells * TILE_W * 4;
   G.dt = p->dt; G.kT = p->kT; G.mass = p->mass;
   G.sigma = (float)sqrt((double)p->kT / (double)p->mass);
   G.cosa = (float)cos((double)p->alpha); G.sina = (float)sin((double)p->alpha);
@@ -796,6 +965,7 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   G.fxv = (float)ldexp(1.0, 20 - ue); G.fxv_inv = ldexp(1.0, ue - 20);
   G.fxe = (float)ldexp(1.0, 18 - 2 * ue); G.fxe_inv = ldexp(1.0, 2 * ue - 18);
   G.collision = p->collision; G.thermostat = p->thermostat;
+  G.sw = p->collision == 1 ? 4 : 3;
   *out = c;
   return MPC_OK;
 }
@@ -808,25 +978,32 @@ int mpc_num_keys(const mpc_ctx* c, unsigned long long* nkeys) {
 
 int mpc_workspace_bytes(const mpc_ctx* c, unsigned long long n_max, int compact, size_t* bytes) {
   if (!c || !bytes || n_max > 0xffffffffull) return MPC_EINVAL;
-  *bytes = make_layout((size_t)n_max, c->G.nkeys, compact != 0).total;
+  *bytes = make_layout((size_t)n_max, c->G.nkeys, c->G.sw, compact != 0).total;
   return MPC_OK;
 }
 
 int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max, void* cuda_stream) {
   if (!c) return MPC_EINVAL;
   if (!workspace || ((uintptr_t)workspace & 255u) || n_max > 0xffffffffull) return fail(c, MPC_EINVAL, "workspace NULL, misaligned or n_max too large");
-  Layout l = make_layout((size_t)n_max, c->G.nkeys, false);
+  Layout l = make_layout((size_t)n_max, c->G.nkeys, c->G.sw, false);
   bool compact = false;
-  if (bytes < l.total) { l = make_layout((size_t)n_max, c->G.nkeys, true); compact = true; }
+  if (bytes < l.total) { l = make_layout((size_t)n_max, c->G.nkeys, c->G.sw, true); compact = true; }
   if (bytes < l.total) return fail(c, MPC_ENOMEM, "workspace smaller than mpc_workspace_bytes(n_max, compact=1)");
   c->ws = (char*)workspace; c->ws_bytes = bytes; c->n_max = (size_t)n_max; c->compact = compact;
   c->stream = (cudaStream_t)cuda_stream;
-  for (int a = 0; a < 8; ++a) { c->A[a] = (uint32_t*)(c->ws + l.off_A[a]); c->Bf[a] = (uint32_t*)(c->ws + l.off_B[a]); }
+  for (int a = 0; a < 7; ++a) { c->A[a] = (uint32_t*)(c->ws + l.off_A[a]); c->Bf[a] = (uint32_t*)(c->ws + l.off_B[a]); }
+  c->key = (uint32_t*)(c->ws + l.off_key);
   c->slot_id = (uint32_t*)(c->ws + l.off_slot); c->perm = (uint32_t*)(c->ws + l.off_perm);
-  c->hist = (uint32_t*)(c->ws + l.off_hist); c->offset = (uint32_t*)(c->ws + l.off_offset);
+  c->cursor = (uint32_t*)(c->ws + l.off_cursor); c->offset = (uint32_t*)(c->ws + l.off_offset);
   c->bsum = (uint32_t*)(c->ws + l.off_bsum);
-  c->sums = (int*)(c->ws + l.off_sums); c->rec = (float*)(c->ws + l.off_rec); c->obs = (double*)(c->ws + l.off_obs);
-  c->bound = true; c->have_state = false; c->have_cells = false; c->n = 0;
+  c->sums = (u64*)(c->ws + l.off_sums); c->rec = (float*)(c->ws + l.off_rec); c->obs = (double*)(c->ws + l.off_obs);
+  c->bound = true; c->have_state = false; c->have_cells = false; c->have_order = false; c->n = 0;
+  if (c->tile_bytes > 48 * 1024) {
+    cudaError_t e;
+    if ((e = sweep_attr<false, false>(c->tile_bytes)) || (e = sweep_attr<false, true>(c->tile_bytes)) ||
+        (e = sweep_attr<true, false>(c->tile_bytes)) || (e = sweep_attr<true, true>(c->tile_bytes)))
+      return cuda_fail(c, e, "cudaFuncSetAttribute(k_sweep, MaxDynamicSharedMemorySize)");
+  }
   return MPC_OK;
 }
 
@@ -845,11 +1022,7 @@ int mpc_step(mpc_ctx* c, int nsteps) {
   if (!c || nsteps < 0) return MPC_EINVAL;
   if (c->sticky) return MPC_ECUDA;
   if (!c->bound || !c->have_state) return fail(c, MPC_ESTATE, "mpc_step before mpc_bind / mpc_set_state");
-  for (int k = 0; k < nsteps; ++k) {
-    const int rc = one_step(c);
-    if (rc) return rc;
-  }
-  return MPC_OK;
+  return c->G.collision == 1 ? steps_at(c, nsteps) : steps_srd(c, nsteps);
 }
 
 int mpc_get_state(mpc_ctx* c, float* x, float* y, float* z, float* vx, float* vy, float* vz, unsigned* id) {
@@ -876,18 +1049,21 @@ int mpc_observables(mpc_ctx* c, mpc_obs* out, float* profile_host) {
   for (int d = 2; d >= 0; --d) if (G.g[d] != 0.0f) fa = d;
   const int nb = G.n[pa];
   if (profile_host && nb > MAX_PROFILE) return fail(c, MPC_EINVAL, "profile axis longer than 2048 layers");
-  CU(cudaMemsetAsync(c->obs, 0, ((size_t)OBS_BLOCKS * 8 + 2 * MAX_PROFILE) * 8, c->stream));
-  if (n) {
-    k_obs_particles<<<OBS_BLOCKS, 256, 0, c->stream>>>(n, F[3], F[4], F[5], part);
-    LAUNCH_CHECK("k_obs_particles");
-    if (profile_host) {
-      k_obs_profile<<<OBS_BLOCKS, 256, (size_t)2 * nb * 8, c->stream>>>(G, n, pa, nb, F[pa], F[3 + fa], prof);
-      LAUNCH_CHECK("k_obs_profile");
+  {
+    FamilyTimer ft(c, F_OBS);
+    CU(cudaMemsetAsync(c->obs, 0, OBS_HOST_DOUBLES * 8, c->stream));
+    if (n) {
+      k_obs_particles<<<OBS_BLOCKS, 256, 0, c->stream>>>(n, F[3], F[4], F[5], part);
+      LAUNCH_CHECK("k_obs_particles");
+      if (profile_host) {
+        k_obs_profile<<<OBS_BLOCKS, 256, (size_t)2 * nb * 8, c->stream>>>(G, n, nb, F[pa], F[3 + fa], prof);
+        LAUNCH_CHECK("k_obs_profile");
+      }
     }
-  }
-  if (c->have_cells) {   // MPC-AT keeps no energy sum: kT_cell is reported as 0 there
-    k_obs_cells<<<OBS_BLOCKS, 256, 0, c->stream>>>(G, c->sums, part);
-    LAUNCH_CHECK("k_obs_cells");
+    if (c->have_cells) {   // MPC-AT keeps no energy sum: kT_cell is reported as 0 there
+      k_obs_cells<<<OBS_BLOCKS, 256, 0, c->stream>>>(G, c->sums, part);
+      LAUNCH_CHECK("k_obs_cells");
+    }
   }
   double* hbuf = c->hbuf;
   CU(cudaMemcpyAsync(hbuf, c->obs, OBS_HOST_DOUBLES * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
@@ -917,11 +1093,14 @@ int mpc_get_cells(mpc_ctx* c, unsigned* count, float* px, float* py, float* pz, 
   if (!c) return MPC_EINVAL;
   if (c->sticky) return MPC_ECUDA;
   if (!c->have_cells) return fail(c, MPC_ESTATE, "mpc_get_cells before the first mpc_step");
-  const Geo& G = c->G;
-  if (G.collision == 1) k_export_cells<true><<<nblk(G.nkeys, 256), 256, 0, c->stream>>>(G, c->sums, count, px, py, pz, e2);
-  else k_export_cells<false><<<nblk(G.nkeys, 256), 256, 0, c->stream>>>(G, c->sums, count, px, py, pz, e2);
+  const Geo& G = c->G;   // G.s / G.t are still those of the last step
+  k_export_cells<<<nblk(G.nkeys, 256), 256, 0, c->stream>>>(G, c->sums, count, px, py, pz, e2);
   LAUNCH_CHECK("k_export_cells");
-  if (key && c->n) CU(cudaMemcpyAsync(key, c->A[7], c->n * 4, cudaMemcpyDeviceToDevice, c->stream));
+  if (key && c->n) {
+    float** F = reinterpret_cast<float**>(c->A);
+    k_keys<<<nblk(c->n, 256), 256, 0, c->stream>>>(G, c->n, F[0], F[1], F[2], key);
+    LAUNCH_CHECK("k_keys");
+  }
   return MPC_OK;
 }
 

@@ -113,7 +113,7 @@ def test_keys_without_shift_equal_floor():
     assert np.array_equal(cnt, np.bincount(key, minlength=o.nkeys))
 
 
-@pytest.mark.parametrize("brick", [1, 4])
+@pytest.mark.parametrize("brick", [1, 4, (4, 2, 8)])
 def test_binning_bruteforce_with_shift(brick):
     box, cells = (8.0, 12.0, 16.0), (8, 12, 16)
     n = 8 * 12 * 16 * 10
@@ -133,11 +133,11 @@ def test_binning_bruteforce_with_shift(brick):
     if brick == 1:
         expect = ijk[:, 0] + 8 * (ijk[:, 1] + 12 * ijk[:, 2])
     else:
-        B = brick
-        mb = [int(np.ceil(c / B)) for c in cells]
+        B = np.array((brick,) * 3 if isinstance(brick, int) else brick)
+        mb = [int(np.ceil(c / bb)) for c, bb in zip(cells, B)]
         b = ijk // B
         l = ijk % B
-        expect = ((b[:, 2] * mb[1] + b[:, 1]) * mb[0] + b[:, 0]) * B**3 + (l[:, 2] * B + l[:, 1]) * B + l[:, 0]
+        expect = ((b[:, 2] * mb[1] + b[:, 1]) * mb[0] + b[:, 0]) * int(np.prod(B)) + (l[:, 2] * B[1] + l[:, 1]) * B[0] + l[:, 0]
     assert np.array_equal(key[safe].astype(np.int64), expect[safe])
     # the oracle's own cell_of hook agrees for every particle (also the unsafe ones)
     for i in np.flatnonzero(~safe)[:20]:
@@ -148,8 +148,8 @@ def test_binning_bruteforce_with_shift(brick):
     assert np.all(np.diff(kk) > 0)
     assert cnt.sum() == n
     # occupancy is Poisson(10) for uniform positions
-    occ = cnt[: 8 * 12 * 16] if brick == 1 else cnt
-    occ = occ[: 8 * 12 * 16]
+    assert o.nkeys == 8 * 12 * 16          # all three layouts tile this box exactly
+    occ = cnt
     assert abs(occ.mean() - 10) < 1e-9
     assert abs(occ.var() - 10) < 1.5
 
@@ -158,7 +158,7 @@ def test_physics_independent_of_key_layout_and_rebin_interval():
     box, cells = (8.0, 8.0, 8.0), (8, 8, 8)
     st = uniform_maxwell(box, 5120, 21)
     res = []
-    for brick, every in [(1, 1), (4, 1), (2, 3), (1, 1000)]:
+    for brick, every in [(1, 1), (4, 1), (2, 3), (1, 1000), ((16, 16, 8), 2), ((4, 2, 1), 1)]:
         o = Oracle(box, cells, 10, 4242, brick=brick, rebin_every=every, thermostat=1)
         o.set_state(*st)
         o.step(7)

@@ -75,6 +75,10 @@ CASES = {
     "walls_gravity": dict(cells=(16, 8, 8), nbar=10, kw=dict(thermostat=1, bc=(0, 0, 1), g=(0.001, 0, 0))),
     "walls_x_brick4": dict(cells=(8, 8, 16), nbar=10, kw=dict(thermostat=1, bc=(1, 0, 0), g=(0, 0.01, 0), brick=4)),
     "noshift": dict(cells=(8, 8, 8), nbar=10, kw=dict(grid_shift=0)),
+    "srd_mbs_brick16x16x8": dict(cells=(32, 16, 24), nbar=10, kw=dict(thermostat=1, brick=(16, 16, 8))),
+    "srd_brick_4x2x1_ragged": dict(cells=(10, 7, 5), nbar=6, kw=dict(thermostat=1, brick=(4, 2, 1))),
+    "walls_gravity_brick16x16x8": dict(cells=(16, 16, 16), nbar=10,
+                                       kw=dict(thermostat=1, bc=(0, 0, 1), g=(0.001, 0, 0), brick=(16, 16, 8))),
 }
 
 
@@ -136,7 +140,8 @@ def test_gpu_is_bit_reproducible_and_order_independent():
     n = 16**3 * nbar
     st = uniform_maxwell(box, n, 3)
     res = []
-    for kw in (dict(), dict(), dict(rebin_every=7), dict(brick=8), dict(brick=4, rebin_every=1000)):
+    for kw in (dict(), dict(), dict(rebin_every=7), dict(brick=8), dict(brick=4, rebin_every=1000),
+               dict(brick=(16, 16, 8), rebin_every=10), dict(brick=(4, 2, 1), rebin_every=3)):
         g = MPC(box, cells, nbar, 42, n_max=n, thermostat=1, **kw)
         gpu_set(g, st)
         g.step(25)
@@ -145,6 +150,29 @@ def test_gpu_is_bit_reproducible_and_order_independent():
         res.append(np.stack([s[d][order] for d in range(6)]))
     for r in res[1:]:
         assert np.array_equal(r, res[0])
+
+
+@pytest.mark.parametrize("kw", [dict(thermostat=1, brick=(16, 16, 8), rebin_every=4),
+                                dict(thermostat=1, bc=(0, 0, 1), g=(0.01, 0, 0), brick=4, rebin_every=3),
+                                dict(collision=1, dt=0.02)])
+def test_one_call_of_k_steps_equals_k_calls(kw):
+    # mpc_step(k) runs the fused sweep (collision of step t-1 inside the streaming pass of step t);
+    # k calls of mpc_step(1) never do. Same arithmetic per particle -> bit-identical states. Together with
+    # the lock-step parity tests (which use mpc_step(1)) this carries parity over to the fused path.
+    cells, nbar = (32, 16, 16), 10
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    st = uniform_maxwell(box, n, 31, rest="g" in kw)
+    res = []
+    for calls in ((9,), (1,) * 9, (4, 5), (2, 3, 4)):
+        g = MPC(box, cells, nbar, 17, n_max=n, **kw)
+        gpu_set(g, st)
+        for k in calls:
+            g.step(k)
+        res.append(gpu_get(g) + [t.cpu().numpy() for t in g.get_cells()])
+    for r in res[1:]:
+        for a, b in zip(res[0], r):
+            assert np.array_equal(a, b)
 
 
 def test_free_running_conservation_cfg1():
