@@ -156,12 +156,15 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--compact", action="store_true", help="property-wise reorder workspace")
+    ap.add_argument("--cells", default=None, help="override the workload's cell grid, e.g. 256,256,256 (profiling runs)")
     args = ap.parse_args()
     wl = dict(WORKLOADS[args.workload])
     if args.nbar is None:
         args.nbar = wl["nbar"]
     if args.rebin_every is not None:
         wl["rebin_every"] = args.rebin_every
+    if args.cells:
+        wl["cells"] = tuple(int(t) for t in args.cells.split(","))
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -202,8 +202,14 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, size_t n, float* __restrict__ x,
     i1 = (size_t)((u64)n * (b + 1) / nbricks);
   }
   __syncthreads();
-  for (size_t i = i0 + threadIdx.x; i < i1; i += SWEEP_T) {
-    float r[3] = {x[i], y[i], z[i]}, v[3] = {vx[i], vy[i], vz[i]};
+  // software pipeline: the loads of the next particle are in flight while this one is processed
+  size_t i = i0 + threadIdx.x;
+  float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f, p4 = 0.f, p5 = 0.f;
+  if (i < i1) { p0 = x[i]; p1 = y[i]; p2 = z[i]; p3 = vx[i]; p4 = vy[i]; p5 = vz[i]; }
+  for (; i < i1; i += SWEEP_T) {
+    float r[3] = {p0, p1, p2}, v[3] = {p3, p4, p5};
+    const size_t inext = i + SWEEP_T;
+    if (inext < i1) { p0 = x[inext]; p1 = y[inext]; p2 = z[inext]; p3 = vx[inext]; p4 = vy[inext]; p5 = vz[inext]; }
     if (COLLIDE) {   // ROTATE_VELOCITIES of the previous step; its key is recomputed from r and that step's shift
       const uint32_t kp = key_of(G, r[0], r[1], r[2], sp0, sp1, sp2);
       const float4 r0 = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)kp * 2);
@@ -440,41 +446,61 @@ __global__ void __launch_bounds__(256) k_iota(size_t n, uint32_t* __restrict__ i
 // E_k / k_BT ~ Gamma(3(Nc-1)/2, 1) (Eq. 7; U6): minus the log of a product of floor(f/2)
 // uniforms (the product is renormalised with frexp so it never underflows: one log per cell instead
 // of one per uniform), plus half a squared normal if f is odd.
+__device__ __forceinline__ void renorm(float& p, int& ex) {   // p = m * 2^e with m in [0.5,1): keep m, bank e
+  const int bits = __float_as_int(p);
+  ex += (bits >> 23) - 126;
+  p = __int_as_float((bits & 0x007fffff) | 0x3f000000);
+}
 __device__ float mbs_energy(const Geo& G, uint32_t cid, uint32_t Nc) {
   const uint32_t f = 3u * (Nc - 1u), M = f >> 1, odd = f & 1u;
-  const uint32_t need = M + 2u * odd;
-  float p = 1.0f, um = 1.0f, cs = 0.0f;
+  const uint32_t full = M >> 2;                  // blocks whose four uniforms all enter the product
+  float p = 1.0f;
   int ex = 0;
   uint32_t sub = 0;
-  for (uint32_t base = 0; base < need; base += 4, ++sub) {
+  for (; sub < full; ++sub) {
+    const Block4 o = philox(cid, sub, G.t, TAG_MBS, G.k0, G.k1);
+    p *= (u01_oc(o.a) * u01_oc(o.b)) * (u01_oc(o.c) * u01_oc(o.d));   // >= 2^-96: cannot underflow
+    renorm(p, ex);
+  }
+  // tail: positions 4*full .. M-1 still enter the product, M and M+1 feed the half squared normal
+  float um = 1.0f, ua = 0.0f;
+  const uint32_t need = M + 2u * odd;
+  for (uint32_t base = full << 2; base < need; base += 4, ++sub) {
     const Block4 o = philox(cid, sub, G.t, TAG_MBS, G.k0, G.k1);
     const uint32_t w[4] = {o.a, o.b, o.c, o.d};
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const uint32_t pos = base + q;
-      if (pos < M) p *= u01_oc(w[q]);                       // >= 2^-24 each: 4 factors cannot underflow
-      else if (odd && pos == M) um = u01_oc(w[q]);
-      else if (odd && pos == M + 1u) cs = cospif(2.0f * u01_co(w[q]));
+      p *= (pos < M) ? u01_oc(w[q]) : 1.0f;
+      um = (pos == M) ? u01_oc(w[q]) : um;
+      ua = (pos == M + 1u) ? u01_co(w[q]) : ua;
     }
-    int e;
-    p = frexpf(p, &e);
-    ex += e;
+    renorm(p, ex);
   }
   float e = -(float)((double)logf(p) + (double)ex * 0.6931471805599453);
-  if (odd) e -= logf(um) * cs * cs;
+  if (odd) {
+    const float cs = cospif(2.0f * ua);
+    e -= logf(um) * cs * cs;
+  }
   return e;
 }
 
 // rec[key] = SRD: { vcm.x, vcm.y, vcm.z, kappa, n.x, n.y, n.z, - }   AT: { (vcm - mean v_ran).xyz, ... }
-__global__ void __launch_bounds__(128) k_cell(Geo G, const u64* __restrict__ sums, float* __restrict__ rec) {
-  const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= G.nkeys) return;
+// grid = (mb0 * CTAs-per-brick, mb1, mb2): the brick coordinates come from blockIdx, no division
+__global__ void __launch_bounds__(128) k_cell(Geo G, int cpb_shift, const u64* __restrict__ sums, float* __restrict__ rec) {
+  const int b0 = G.bs[0], b1 = G.bs[1], b2 = G.bs[2];
+  const uint32_t bx = blockIdx.x >> cpb_shift, by = blockIdx.y, bz = blockIdx.z;
+  const uint32_t local = ((blockIdx.x & ((1u << cpb_shift) - 1u)) << 7) | threadIdx.x;
+  if (local >= (1u << (b0 + b1 + b2))) return;
+  const uint32_t brick = (bz * (uint32_t)G.mb[1] + by) * (uint32_t)G.mb[0] + bx;
+  const uint32_t k = (brick << (b0 + b1 + b2)) | local;
   const u64* s = sums + (size_t)k * G.sw;
   const u64 w0 = s[0];
   const uint32_t nreal = (uint32_t)(w0 & 0xffffffffull);
   if (nreal == 0u) return;
-  int ix, iy, iz;
-  key_to_cell(G, k, ix, iy, iz);
+  const int ix = (int)((bx << b0) | (local & ((1u << b0) - 1u)));
+  const int iy = (int)((by << b1) | ((local >> b0) & ((1u << b1) - 1u)));
+  const int iz = (int)((bz << b2) | (local >> (b0 + b1)));
   const uint32_t cid = canonical_id(G, ix, iy, iz);
   int sx, sy, sz, r0i;
   unpack_ss(s[1], sx, sy);
@@ -634,6 +660,8 @@ struct mpc_ctx {
   size_t ws_bytes;
   uint32_t nbricks;
   size_t tile_bytes;
+  dim3 cell_grid;       // k_cell launch: (mb0 << cell_cpb_shift, mb1, mb2) CTAs of 128 cells
+  int cell_cpb_shift;
   // device arrays
   uint32_t* A[7];   // x y z vx vy vz id (current)
   uint32_t* Bf[7];  // second copy (non-compact); Bf[0] = 4-byte temp (compact)
@@ -820,7 +848,7 @@ int steps_srd(mpc_ctx* c, int nsteps) {
       }
       if (rebin) { const int rc = do_reorder(c); if (rc) return rc; }
       FamilyTimer ft(c, F_CELL);
-      k_cell<<<nblk(G.nkeys, 128), 128, 0, c->stream>>>(G, c->sums, c->rec);
+      k_cell<<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec);
       LAUNCH_CHECK("k_cell");
     }
     sp[0] = G.s[0]; sp[1] = G.s[1]; sp[2] = G.s[2];
@@ -863,7 +891,7 @@ int steps_at(mpc_ctx* c, int nsteps) {
       }
       {
         FamilyTimer ft(c, F_CELL);
-        k_cell<<<nblk(G.nkeys, 128), 128, 0, c->stream>>>(G, c->sums, c->rec);
+        k_cell<<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec);
         LAUNCH_CHECK("k_cell");
       }
       FamilyTimer ft(c, F_COLLIDE);
@@ -956,6 +984,12 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   G.nkeys = (uint32_t)nk;
   c->nbricks = (uint32_t)nbr;
   c->tile_bytes = tile_cells * TILE_W * 4;
+  {
+    const int bvs = G.bs[0] + G.bs[1] + G.bs[2];
+    c->cell_cpb_shift = bvs > 7 ? bvs - 7 : 0;
+    c->cell_grid = dim3((unsigned)G.mb[0] << c->cell_cpb_shift, (unsigned)G.mb[1], (unsigned)G.mb[2]);
+    if (G.mb[1] > 65535 || G.mb[2] > 65535) { delete[] c->hbuf; delete c; return MPC_EINVAL; }
+  }
   G.dt = p->dt; G.kT = p->kT; G.mass = p->mass;
   G.sigma = (float)sqrt((double)p->kT / (double)p->mass);
   G.cosa = (float)cos((double)p->alpha); G.sina = (float)sin((double)p->alpha);
