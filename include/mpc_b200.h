@@ -76,7 +76,7 @@ typedef struct {
 /* Create a context. box[d] = L_d, cells[d] = number of fluid cells n_d; cells must be cubic
  * (L_x/n_x == L_y/n_y == L_z/n_z == a). n_per_cell = <N_c>, used for the virtual-wall-particle fill
  * (round(n_per_cell)) and for sizing. Allocates nothing on the device.
- * MPC_EINVAL: NULL argument, non-cubic cells, non-positive sizes/dt/kT/mass, rebin_every < 1,
+ * MPC_EINVAL: NULL argument, fewer than 3 cells along an axis, non-cubic cells, non-positive sizes/dt/kT/mass, rebin_every < 1,
  * brick dims not powers of two in 1..64 or tile too large for shared memory, more than one wall axis, force along a wall normal, walls with +a or MPC-AT,
  * SRD+a with thermostat (U6), MPC-AT with rebin_every != 1, key space >= 2^32. */
 int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_per_cell,

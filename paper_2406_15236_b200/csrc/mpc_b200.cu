@@ -179,39 +179,72 @@ __device__ __forceinline__ void srd_apply(const Geo& G, const float4 r0, const f
 // fraction of a cell and the lattice shift has changed by less than a cell, so nearly all of them fall
 // into the brick's tile (brick + HALO cells on every side), held in shared memory as int32 sums. The
 // rest (and everything, if no order is known yet) goes to the global sums directly.
-template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY>
+// B0,B1,B2 = log2 of the brick dims at compile time (the {16,16,8} fast path), or -1: read from Geo.
+template <int B0, int B1, int B2>
+struct BrickShape {
+  static constexpr bool fixed = B0 >= 0;
+  __device__ __forceinline__ static int s0(const Geo& G) { return fixed ? B0 : G.bs[0]; }
+  __device__ __forceinline__ static int s1(const Geo& G) { return fixed ? B1 : G.bs[1]; }
+  __device__ __forceinline__ static int s2(const Geo& G) { return fixed ? B2 : G.bs[2]; }
+  __device__ __forceinline__ static uint32_t key(const Geo& G, int ix, int iy, int iz) {
+    const int b0 = s0(G), b1 = s1(G), b2 = s2(G);
+    const uint32_t brick = ((uint32_t)(iz >> b2) * (uint32_t)G.mb[1] + (uint32_t)(iy >> b1)) * (uint32_t)G.mb[0] + (uint32_t)(ix >> b0);
+    const uint32_t local = ((((uint32_t)(iz & ((1 << b2) - 1))) << b1 | (uint32_t)(iy & ((1 << b1) - 1))) << b0) | (uint32_t)(ix & ((1 << b0) - 1));
+    return (brick << (b0 + b1 + b2)) | local;
+  }
+};
+// floor index of a coordinate, not yet folded into [0, m)
+__device__ __forceinline__ int cell_raw(const Geo& G, float r, float s) { return __float2int_rd((r + s) * G.inv_a); }
+// fold an index known to lie in [-m, 2m) into [0, m)
+__device__ __forceinline__ int fold(int k, int m) {
+  k += (k < 0) ? m : 0;
+  k -= (k >= m) ? m : 0;
+  return k;
+}
+
+template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS>
 __global__ void __launch_bounds__(SWEEP_T, 2)
-k_sweep(Geo G, float sp0, float sp1, float sp2, size_t n, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
+k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
         float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, uint32_t* __restrict__ key_out,
         const uint32_t* __restrict__ chunk, uint32_t nbricks, const float* __restrict__ rec, u64* __restrict__ sums) {
   extern __shared__ int tile[];
-  const int T0 = (1 << G.bs[0]) + 2 * HALO, T1 = (1 << G.bs[1]) + 2 * HALO, T2 = (1 << G.bs[2]) + 2 * HALO;
+  const int T0 = (1 << BS::s0(G)) + 2 * HALO, T1 = (1 << BS::s1(G)) + 2 * HALO, T2 = (1 << BS::s2(G)) + 2 * HALO;
   const int tcells = T0 * T1 * T2;
   for (int i = threadIdx.x; i < tcells * TILE_W; i += SWEEP_T) tile[i] = 0;
   const uint32_t b = blockIdx.x;
+  const int m0 = G.m[0], m1 = G.m[1], m2 = G.m[2];
   int ox, oy, oz;
-  brick_to_origin(G, b, ox, oy, oz);
-  ox -= HALO; oy -= HALO; oz -= HALO;
-  size_t i0, i1;
-  if (chunk) {
-    const uint32_t bvol_shift = G.bs[0] + G.bs[1] + G.bs[2];
-    i0 = chunk[(size_t)b << bvol_shift];
-    i1 = (b + 1 == nbricks) ? n : (size_t)chunk[(size_t)(b + 1) << bvol_shift];
-  } else {   // no order known: even split, (almost) everything takes the global path
-    i0 = (size_t)((u64)n * b / nbricks);            // n < 2^32 and b < 2^32: no overflow
-    i1 = (size_t)((u64)n * (b + 1) / nbricks);
+  {
+    const uint32_t bx = b % (uint32_t)G.mb[0], q = b / (uint32_t)G.mb[0];
+    const uint32_t by = q % (uint32_t)G.mb[1], bz = q / (uint32_t)G.mb[1];
+    ox = (int)(bx << BS::s0(G)) - HALO; oy = (int)(by << BS::s1(G)) - HALO; oz = (int)(bz << BS::s2(G)) - HALO;
   }
+  uint32_t i0, i1;
+  if (chunk) {
+    const uint32_t bvol_shift = BS::s0(G) + BS::s1(G) + BS::s2(G);
+    i0 = chunk[(size_t)b << bvol_shift];
+    i1 = (b + 1 == nbricks) ? n : chunk[(size_t)(b + 1) << bvol_shift];
+  } else {   // no order known: even split, (almost) everything takes the global path
+    i0 = (uint32_t)((u64)n * b / nbricks);
+    i1 = (uint32_t)((u64)n * (b + 1) / nbricks);
+  }
+  // index offsets added before the floor index is folded: +1 on a wall axis (layer 0 lies in the wall)
+  const int w0 = (WALL && G.bc[0]) ? 1 : 0, w1 = (WALL && G.bc[1]) ? 1 : 0, w2 = (WALL && G.bc[2]) ? 1 : 0;
   __syncthreads();
   // software pipeline: the loads of the next particle are in flight while this one is processed
-  size_t i = i0 + threadIdx.x;
+  uint32_t i = i0 + threadIdx.x;
   float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f, p4 = 0.f, p5 = 0.f;
   if (i < i1) { p0 = x[i]; p1 = y[i]; p2 = z[i]; p3 = vx[i]; p4 = vy[i]; p5 = vz[i]; }
   for (; i < i1; i += SWEEP_T) {
     float r[3] = {p0, p1, p2}, v[3] = {p3, p4, p5};
-    const size_t inext = i + SWEEP_T;
+    const uint32_t inext = i + SWEEP_T;
     if (inext < i1) { p0 = x[inext]; p1 = y[inext]; p2 = z[inext]; p3 = vx[inext]; p4 = vy[inext]; p5 = vz[inext]; }
     if (COLLIDE) {   // ROTATE_VELOCITIES of the previous step; its key is recomputed from r and that step's shift
-      const uint32_t kp = key_of(G, r[0], r[1], r[2], sp0, sp1, sp2);
+      int kx = cell_raw(G, r[0], sp0) + w0, ky = cell_raw(G, r[1], sp1) + w1, kz = cell_raw(G, r[2], sp2) + w2;
+      if (WALL) { kx = G.bc[0] ? max(0, min(kx, m0 - 1)) : fold(kx, m0); ky = G.bc[1] ? max(0, min(ky, m1 - 1)) : fold(ky, m1);
+                  kz = G.bc[2] ? max(0, min(kz, m2 - 1)) : fold(kz, m2); }
+      else { kx = fold(kx, m0); ky = fold(ky, m1); kz = fold(kz, m2); }
+      const uint32_t kp = BS::key(G, kx, ky, kz);
       const float4 r0 = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)kp * 2);
       const float4 ax = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)kp * 2 + 1);
       srd_apply(G, r0, ax, v);
@@ -219,20 +252,24 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, size_t n, float* __restrict__ x,
     stream_one<WALL, GRAV>(G, r, v);
     x[i] = r[0]; y[i] = r[1]; z[i] = r[2];
     vx[i] = v[0]; vy[i] = v[1]; vz[i] = v[2];
-    const int ix = cell_coord(G, 0, r[0], G.s[0]), iy = cell_coord(G, 1, r[1], G.s[1]), iz = cell_coord(G, 2, r[2], G.s[2]);
-    if (WKEY) key_out[i] = layout_key(G, ix, iy, iz);
+    int cx = cell_raw(G, r[0], G.s[0]) + w0, cy = cell_raw(G, r[1], G.s[1]) + w1, cz = cell_raw(G, r[2], G.s[2]) + w2;
+    if (WALL) { if (G.bc[0]) cx = max(0, min(cx, m0 - 1)); if (G.bc[1]) cy = max(0, min(cy, m1 - 1)); if (G.bc[2]) cz = max(0, min(cz, m2 - 1)); }
     const int a0 = __float2int_rn(v[0] * G.fxv), a1 = __float2int_rn(v[1] * G.fxv), a2 = __float2int_rn(v[2] * G.fxv);
     const unsigned e = __float2uint_rn(fmaf(v[0], v[0], fmaf(v[1], v[1], v[2] * v[2])) * G.fxe);
-    int l0 = ix - ox, l1 = iy - oy, l2 = iz - oz;     // tile coordinates, periodic images folded in
-    if (l0 < 0) l0 += G.m[0]; else if (l0 >= G.m[0]) l0 -= G.m[0];
-    if (l1 < 0) l1 += G.m[1]; else if (l1 >= G.m[1]) l1 -= G.m[1];
-    if (l2 < 0) l2 += G.m[2]; else if (l2 >= G.m[2]) l2 -= G.m[2];
-    if (l0 < T0 && l1 < T1 && l2 < T2) {
+    // tile coordinates: one fold takes care of the periodic image of the cell and of the tile origin
+    const int l0 = fold(cx - ox, m0), l1 = fold(cy - oy, m1), l2 = fold(cz - oz, m2);
+    const bool inside = (l0 < T0) & (l1 < T1) & (l2 < T2);
+    if (inside) {
       int* s = tile + ((l2 * T1 + l1) * T0 + l0) * TILE_W;
       atomicAdd(s, 1); atomicAdd(s + 1, a0); atomicAdd(s + 2, a1); atomicAdd(s + 3, a2); atomicAdd((unsigned*)s + 4, e);
-    } else {
-      u64* s = sums + (size_t)layout_key(G, ix, iy, iz) * G.sw;
-      atomicAdd(s, ((u64)e << 32) | 1ull); atomicAdd(s + 1, pack_ss(a0, a1)); atomicAdd(s + 2, pack_ss(a2, 0));
+    }
+    if (WKEY || !inside) {
+      const uint32_t kc = BS::key(G, fold(cx, m0), fold(cy, m1), fold(cz, m2));
+      if (WKEY) key_out[i] = kc;
+      if (!inside) {
+        u64* s = sums + (size_t)kc * G.sw;
+        atomicAdd(s, ((u64)e << 32) | 1ull); atomicAdd(s + 1, pack_ss(a0, a1)); atomicAdd(s + 2, pack_ss(a2, 0));
+      }
     }
   }
   __syncthreads();
@@ -242,11 +279,7 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, size_t n, float* __restrict__ x,
     const int cnt = s[0];
     if (cnt == 0) continue;
     const int l0 = c % T0, q = c / T0, l1 = q % T1, l2 = q / T1;
-    int ix = ox + l0, iy = oy + l1, iz = oz + l2;
-    if (ix < 0) ix += G.m[0]; else if (ix >= G.m[0]) ix -= G.m[0];
-    if (iy < 0) iy += G.m[1]; else if (iy >= G.m[1]) iy -= G.m[1];
-    if (iz < 0) iz += G.m[2]; else if (iz >= G.m[2]) iz -= G.m[2];
-    u64* g = sums + (size_t)layout_key(G, ix, iy, iz) * G.sw;
+    u64* g = sums + (size_t)BS::key(G, fold(ox + l0, m0), fold(oy + l1, m1), fold(oz + l2, m2)) * G.sw;
     atomicAdd(g, ((u64)(unsigned)s[4] << 32) | (u64)(unsigned)cnt);
     atomicAdd(g + 1, pack_ss(s[1], s[2]));
     atomicAdd(g + 2, pack_ss(s[3], 0));
@@ -654,7 +687,7 @@ struct mpc_ctx {
   unsigned long long seed;
   uint32_t t;
   size_t n, n_max;
-  bool bound, have_state, have_cells, have_order, compact, sticky;
+  bool bound, have_state, have_cells, have_order, compact, sticky, fast_brick;
   cudaStream_t stream;
   char* ws;
   size_t ws_bytes;
@@ -803,29 +836,41 @@ int do_reorder(mpc_ctx* c) {
   return MPC_OK;
 }
 
-template <bool COLLIDE, bool WKEY>
-int launch_sweep(mpc_ctx* c, const float sp[3]) {
+typedef BrickShape<-1, -1, -1> BSgeneric;
+typedef BrickShape<4, 4, 3> BSfast;   // {16,16,8}
+
+template <bool COLLIDE, bool WKEY, class BS>
+int launch_sweep_bs(mpc_ctx* c, const float sp[3]) {
   const Geo& G = c->G;
   float** F = reinterpret_cast<float**>(c->A);
   const uint32_t* chunk = c->have_order ? c->offset : nullptr;
   const bool wall = G.wall >= 0, grav = (G.g[0] != 0.f || G.g[1] != 0.f || G.g[2] != 0.f);
-#define SWEEP_ARGS G, sp[0], sp[1], sp[2], c->n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, chunk, c->nbricks, c->rec, c->sums
-  if (wall && grav) k_sweep<COLLIDE, true, true, WKEY><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
-  else if (wall) k_sweep<COLLIDE, true, false, WKEY><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
-  else if (grav) k_sweep<COLLIDE, false, true, WKEY><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
-  else k_sweep<COLLIDE, false, false, WKEY><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
+#define SWEEP_ARGS G, sp[0], sp[1], sp[2], (uint32_t)c->n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, chunk, c->nbricks, c->rec, c->sums
+  if (wall && grav) k_sweep<COLLIDE, true, true, WKEY, BS><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
+  else if (wall) k_sweep<COLLIDE, true, false, WKEY, BS><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
+  else if (grav) k_sweep<COLLIDE, false, true, WKEY, BS><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
+  else k_sweep<COLLIDE, false, false, WKEY, BS><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
 #undef SWEEP_ARGS
   LAUNCH_CHECK("k_sweep");
   return MPC_OK;
 }
+template <bool COLLIDE, bool WKEY>
+int launch_sweep(mpc_ctx* c, const float sp[3]) {
+  return c->fast_brick ? launch_sweep_bs<COLLIDE, WKEY, BSfast>(c, sp) : launch_sweep_bs<COLLIDE, WKEY, BSgeneric>(c, sp);
+}
 
+template <bool COLLIDE, bool WKEY, class BS>
+cudaError_t sweep_attr_bs(size_t bytes) {
+  cudaError_t e;
+  if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, true, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+  if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, false, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+  if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, true, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+  return cudaFuncSetAttribute(k_sweep<COLLIDE, false, false, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
 template <bool COLLIDE, bool WKEY>
 cudaError_t sweep_attr(size_t bytes) {
-  cudaError_t e;
-  if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, true, WKEY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
-  if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, false, WKEY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
-  if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, true, WKEY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
-  return cudaFuncSetAttribute(k_sweep<COLLIDE, false, false, WKEY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  cudaError_t e = sweep_attr_bs<COLLIDE, WKEY, BSgeneric>(bytes);
+  return e ? e : sweep_attr_bs<COLLIDE, WKEY, BSfast>(bytes);
 }
 
 // SRD: n steps = sweep(no collide), cell, [sweep(collide t-1 + move t), cell] x (n-1), trailing collide
@@ -940,7 +985,8 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   if (!out) return MPC_EINVAL;
   *out = nullptr;
   if (!box || !cells || !p) return MPC_EINVAL;
-  for (int d = 0; d < 3; ++d) if (cells[d] < 1 || !(box[d] > 0.0f)) return MPC_EINVAL;
+  // >= 3 cells per axis: with fewer, a particle shares a collision cell with its own periodic image
+  for (int d = 0; d < 3; ++d) if (cells[d] < 3 || !(box[d] > 0.0f)) return MPC_EINVAL;
   const float a = box[0] / (float)cells[0];
   for (int d = 1; d < 3; ++d) if (box[d] / (float)cells[d] != a) return MPC_EINVAL;
   if (p->collision < 0 || p->collision > 1) return MPC_EINVAL;
@@ -984,6 +1030,7 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   G.nkeys = (uint32_t)nk;
   c->nbricks = (uint32_t)nbr;
   c->tile_bytes = tile_cells * TILE_W * 4;
+  c->fast_brick = (G.bs[0] == 4 && G.bs[1] == 4 && G.bs[2] == 3);
   {
     const int bvs = G.bs[0] + G.bs[1] + G.bs[2];
     c->cell_cpb_shift = bvs > 7 ? bvs - 7 : 0;

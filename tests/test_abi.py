@@ -57,6 +57,7 @@ def test_create_validates_arguments(lib):
     assert lib.mpc_destroy(h) == 0
     assert _create(lib, box=(8, 8, 9))[0] == binding.MPC_EINVAL
     assert _create(lib, cells=(8, 8, 0))[0] == binding.MPC_EINVAL
+    assert _create(lib, box=(8, 8, 2), cells=(8, 8, 2))[0] == binding.MPC_EINVAL
     assert _create(lib, rebin_every=0)[0] == binding.MPC_EINVAL
     assert _create(lib, brick=3)[0] == binding.MPC_EINVAL
     assert _create(lib, bc=(1, 0, 1))[0] == binding.MPC_EINVAL
