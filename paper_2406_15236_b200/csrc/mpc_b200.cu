@@ -159,6 +159,14 @@ __device__ __forceinline__ void stream_one(const Geo& G, float (&r)[3], float (&
   }
 }
 
+// 256-bit read-only load of one 32-byte cell record (sm_100: LDG.E.ENL2.256): one L1 request instead of two
+__device__ __forceinline__ void load_rec(const float* __restrict__ rec, uint32_t key, float4& r0, float4& ax) {
+  const float* p = rec + (size_t)key * REC_W;
+  asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=f"(r0.x), "=f"(r0.y), "=f"(r0.z), "=f"(r0.w), "=f"(ax.x), "=f"(ax.y), "=f"(ax.z), "=f"(ax.w)
+               : "l"(p));
+}
+
 // ---- SRD rotation with thermostat scaling: v' = vcm + kappa D(alpha) (v - vcm) ----------------------
 __device__ __forceinline__ void srd_apply(const Geo& G, const float4 r0, const float4 ax, float (&v)[3]) {
   const float w0 = v[0] - r0.x, w1 = v[1] - r0.y, w2 = v[2] - r0.z;
@@ -245,8 +253,8 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
                   kz = G.bc[2] ? max(0, min(kz, m2 - 1)) : fold(kz, m2); }
       else { kx = fold(kx, m0); ky = fold(ky, m1); kz = fold(kz, m2); }
       const uint32_t kp = BS::key(G, kx, ky, kz);
-      const float4 r0 = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)kp * 2);
-      const float4 ax = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)kp * 2 + 1);
+      float4 r0, ax;
+      load_rec(rec, kp, r0, ax);
       srd_apply(G, r0, ax, v);
     }
     stream_one<WALL, GRAV>(G, r, v);
@@ -293,8 +301,8 @@ __global__ void __launch_bounds__(256) k_collide_pos(Geo G, size_t n, const floa
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const uint32_t k = key_of(G, x[i], y[i], z[i], G.s[0], G.s[1], G.s[2]);
-  const float4 r0 = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)k * 2);
-  const float4 ax = __ldg(reinterpret_cast<const float4*>(rec) + (size_t)k * 2 + 1);
+  float4 r0, ax;
+  load_rec(rec, k, r0, ax);
   float v[3] = {vx[i], vy[i], vz[i]};
   srd_apply(G, r0, ax, v);
   vx[i] = v[0]; vy[i] = v[1]; vz[i] = v[2];
