@@ -59,13 +59,18 @@ struct Geo {
   float fxv, fxe;
   double fxv_inv, fxe_inv;
   int nbar;
-  int collision, thermostat;
-  int sw;         // 64-bit words per cell in the global sums array (3 SRD, 4 MPC-AT)
+  int collision, thermostat, conserve_L;
+  int generic;    // 1 = unfused path (MPC-AT and every +a variant), 0 = fused SRD sweep
+  int sw;         // 64-bit words per cell in the global sums array (3 SRD, 4 MPC-AT, 10 with +a)
+  int rw;         // floats per cell record (8, or 16 with +a)
   uint32_t nkeys;
 };
 
 // ---- packed sums ---------------------------------------------------------------------------------
-// word0 = E << 32 | N (both unsigned); word1 = (Sy, Sx); word2 = (R0, Sz); word3 = (R2, R1)  [AT]
+// word0 = E << 32 | N (both unsigned); word1 = (Sy, Sx); word2 = (R0, Sz); word3 = (R2, R1)  [AT: R = sum v_ran]
+// +a adds, in cell-local coordinates rho in [0,1)^3 (U9), scale 2^20 for rho terms:
+// word4 = (rho_y, rho_x); word5 = (Qxx, rho_z); word6 = (Qzz, Qyy); word7 = (Qxz, Qxy); word8 = (Lx, Qyz);
+// word9 = (Lz, Ly)   with Q = sum rho rho^T, L = sum rho x u, u = v - D v (SRD) or v - v_ran (AT)
 __device__ __forceinline__ u64 pack_ss(int lo, int hi) { return (u64)((long long)hi * 4294967296ll + (long long)lo); }
 __device__ __forceinline__ void unpack_ss(u64 w, int& lo, int& hi) {
   lo = (int)(uint32_t)(w & 0xffffffffull);
@@ -363,6 +368,183 @@ __global__ void __launch_bounds__(256) k_collide_at(Geo G, size_t n, float* __re
   vz[i] = r0.z + G.sigma * g2;
 }
 
+// ---- +a variants (Eqs. 3-4; MPC-AT+a, U5): unfused path --------------------------------
+constexpr float FX_RHO = 4194304.0f;            // 2^22 per unit of cell-local coordinate (products too): N_c < 512
+constexpr double FX_RHO_INV = 1.0 / 4194304.0;
+constexpr float FX_L = 4.0f;                    // angular-momentum terms: 4x the velocity scale (|rho x u| < 512 u)
+
+__device__ __forceinline__ void srd_axis(const Geo& G, uint32_t cid, float& ax, float& ay, float& az) {
+  const Block4 o = philox(cid, 0u, G.t, TAG_AXIS, G.k0, G.k1);
+  az = 2.0f * u01_co(o.a) - 1.0f;
+  const float rr = sqrtf((1.0f - az) * (1.0f + az));
+  float sp, cp;
+  sincospif(2.0f * u01_co(o.b), &sp, &cp);
+  ax = rr * cp; ay = rr * sp;
+}
+// D(alpha) w for unit axis n (Rodrigues, right-handed)
+__device__ __forceinline__ void rotate(const Geo& G, float nx, float ny, float nz, const float (&w)[3], float (&o)[3]) {
+  const float c = G.cosa, s = G.sina;
+  const float nd = fmaf(nx, w[0], fmaf(ny, w[1], nz * w[2])) * (1.0f - c);
+  const float cx = fmaf(ny, w[2], -(nz * w[1])), cy = fmaf(nz, w[0], -(nx * w[2])), cz = fmaf(nx, w[1], -(ny * w[0]));
+  o[0] = fmaf(w[0], c, fmaf(cx, s, nx * nd));
+  o[1] = fmaf(w[1], c, fmaf(cy, s, ny * nd));
+  o[2] = fmaf(w[2], c, fmaf(cz, s, nz * nd));
+}
+__device__ __forceinline__ float cell_frac(const Geo& G, float r, float s) {
+  const float q = (r + s) * G.inv_a;
+  return q - floorf(q);
+}
+
+template <bool AT>
+__global__ void __launch_bounds__(256) k_accum_a(Geo G, size_t n, const float* __restrict__ x, const float* __restrict__ y,
+                                                 const float* __restrict__ z, const float* __restrict__ vx,
+                                                 const float* __restrict__ vy, const float* __restrict__ vz,
+                                                 const uint32_t* __restrict__ key, const uint32_t* __restrict__ offset,
+                                                 u64* __restrict__ sums) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t k = key[i];
+  int ix, iy, iz;
+  key_to_cell(G, k, ix, iy, iz);
+  const uint32_t cid = canonical_id(G, ix, iy, iz);
+  const float v[3] = {vx[i], vy[i], vz[i]};
+  const float r0 = cell_frac(G, x[i], G.s[0]), r1 = cell_frac(G, y[i], G.s[1]), r2 = cell_frac(G, z[i], G.s[2]);
+  float u[3], g[3] = {0.f, 0.f, 0.f};
+  if (AT) {
+    const Block4 o = philox(cid, (uint32_t)i - offset[k], G.t, TAG_AT, G.k0, G.k1);
+    normals3(o, g[0], g[1], g[2]);
+    g[0] *= G.sigma; g[1] *= G.sigma; g[2] *= G.sigma;
+    u[0] = v[0] - g[0]; u[1] = v[1] - g[1]; u[2] = v[2] - g[2];
+  } else {
+    float ax, ay, az, d[3];
+    srd_axis(G, cid, ax, ay, az);
+    rotate(G, ax, ay, az, v, d);
+    u[0] = v[0] - d[0]; u[1] = v[1] - d[1]; u[2] = v[2] - d[2];
+  }
+  const float l0 = fmaf(r1, u[2], -(r2 * u[1])), l1 = fmaf(r2, u[0], -(r0 * u[2])), l2 = fmaf(r0, u[1], -(r1 * u[0]));
+  u64* s = sums + (size_t)k * G.sw;
+  auto fv = [&](float a) { return __float2int_rn(a * G.fxv); };
+  auto fq = [&](float a) { return __float2int_rn(a * FX_RHO); };
+  atomicAdd(s + 1, pack_ss(fv(v[0]), fv(v[1])));
+  atomicAdd(s + 2, pack_ss(fv(v[2]), AT ? fv(g[0]) : 0));
+  if (AT) atomicAdd(s + 3, pack_ss(fv(g[1]), fv(g[2])));
+  atomicAdd(s + 4, pack_ss(fq(r0), fq(r1)));
+  atomicAdd(s + 5, pack_ss(fq(r2), fq(r0 * r0)));
+  atomicAdd(s + 6, pack_ss(fq(r1 * r1), fq(r2 * r2)));
+  atomicAdd(s + 7, pack_ss(fq(r0 * r1), fq(r0 * r2)));
+  atomicAdd(s + 8, pack_ss(fq(r1 * r2), fv(l0 * FX_L)));
+  atomicAdd(s + 9, pack_ss(fv(l1 * FX_L), fv(l2 * FX_L)));
+}
+
+// rec[key] (16 floats) = { base.xyz, 1 | axis.xyz, - | omega.xyz, - | rho_cm.xyz, - }
+//   SRD+a: base = v_cm ; AT+a: base = v_cm - mean(v_ran)
+template <bool AT>
+__global__ void __launch_bounds__(128) k_cell_a(Geo G, int cpb_shift, const u64* __restrict__ sums, float* __restrict__ rec,
+                                                u64* __restrict__ nsing) {
+  const int b0 = G.bs[0], b1 = G.bs[1], b2 = G.bs[2];
+  const uint32_t bx = blockIdx.x >> cpb_shift, by = blockIdx.y, bz = blockIdx.z;
+  const uint32_t local = ((blockIdx.x & ((1u << cpb_shift) - 1u)) << 7) | threadIdx.x;
+  if (local >= (1u << (b0 + b1 + b2))) return;
+  const uint32_t brick = (bz * (uint32_t)G.mb[1] + by) * (uint32_t)G.mb[0] + bx;
+  const uint32_t k = (brick << (b0 + b1 + b2)) | local;
+  const u64* s = sums + (size_t)k * G.sw;
+  const uint32_t N = (uint32_t)(s[0] & 0xffffffffull);
+  if (N == 0u) return;
+  const int ix = (int)((bx << b0) | (local & ((1u << b0) - 1u)));
+  const int iy = (int)((by << b1) | ((local >> b0) & ((1u << b1) - 1u)));
+  const int iz = (int)((bz << b2) | (local >> (b0 + b1)));
+  const uint32_t cid = canonical_id(G, ix, iy, iz);
+  int i0, i1, i2, i3, i4, i5;
+  unpack_ss(s[1], i0, i1); unpack_ss(s[2], i2, i3);
+  const double inv = 1.0 / (double)N;
+  const double S[3] = {i0 * G.fxv_inv, i1 * G.fxv_inv, i2 * G.fxv_inv};
+  double R[3] = {i3 * G.fxv_inv, 0.0, 0.0};
+  if (AT) { unpack_ss(s[3], i4, i5); R[1] = i4 * G.fxv_inv; R[2] = i5 * G.fxv_inv; }
+  float ax = 0.f, ay = 0.f, az = 1.f;
+  double Su[3];
+  if (AT) { Su[0] = S[0] - R[0]; Su[1] = S[1] - R[1]; Su[2] = S[2] - R[2]; }
+  else {
+    srd_axis(G, cid, ax, ay, az);
+    // (1 - D) S in double, with the fp32 axis and the fp32 cos/sin the particles used
+    const double c = G.cosa, sn = G.sina, nx = ax, ny = ay, nz = az;
+    const double nd = (nx * S[0] + ny * S[1] + nz * S[2]) * (1.0 - c);
+    const double cx = ny * S[2] - nz * S[1], cy = nz * S[0] - nx * S[2], cz = nx * S[1] - ny * S[0];
+    Su[0] = S[0] - (S[0] * c + cx * sn + nx * nd);
+    Su[1] = S[1] - (S[1] * c + cy * sn + ny * nd);
+    Su[2] = S[2] - (S[2] * c + cz * sn + nz * nd);
+  }
+  double om[3] = {0.0, 0.0, 0.0}, rcm[3] = {0.0, 0.0, 0.0};
+  if (N >= 2u) {
+    int q0, q1, q2, q3, q4, q5, q6, q7, q8, q9, q10, q11;
+    unpack_ss(s[4], q0, q1); unpack_ss(s[5], q2, q3); unpack_ss(s[6], q4, q5);
+    unpack_ss(s[7], q6, q7); unpack_ss(s[8], q8, q9); unpack_ss(s[9], q10, q11);
+    rcm[0] = q0 * FX_RHO_INV * inv; rcm[1] = q1 * FX_RHO_INV * inv; rcm[2] = q2 * FX_RHO_INV * inv;
+    const double a = G.a, m = G.mass, Nd = (double)N;
+    // second moments about the centre of mass, in units of a^2
+    const double Qxx = q3 * FX_RHO_INV - Nd * rcm[0] * rcm[0], Qyy = q4 * FX_RHO_INV - Nd * rcm[1] * rcm[1];
+    const double Qzz = q5 * FX_RHO_INV - Nd * rcm[2] * rcm[2], Qxy = q6 * FX_RHO_INV - Nd * rcm[0] * rcm[1];
+    const double Qxz = q7 * FX_RHO_INV - Nd * rcm[0] * rcm[2], Qyz = q8 * FX_RHO_INV - Nd * rcm[1] * rcm[2];
+    const double Lr[3] = {q9 * G.fxv_inv * 0.25, q10 * G.fxv_inv * 0.25, q11 * G.fxv_inv * 0.25};
+    const double dL[3] = {m * a * (Lr[0] - (rcm[1] * Su[2] - rcm[2] * Su[1])),
+                          m * a * (Lr[1] - (rcm[2] * Su[0] - rcm[0] * Su[2])),
+                          m * a * (Lr[2] - (rcm[0] * Su[1] - rcm[1] * Su[0]))};
+    const double R2 = a * a * (Qxx + Qyy + Qzz);
+    if (N == 2u) {
+      if (R2 > 0.0) { om[0] = dL[0] / (m * R2); om[1] = dL[1] / (m * R2); om[2] = dL[2] / (m * R2); }
+    } else {
+      const double f = m * a * a;
+      const double xx = f * (Qyy + Qzz), yy = f * (Qxx + Qzz), zz = f * (Qxx + Qyy), xy = -f * Qxy, xz = -f * Qxz, yz = -f * Qyz;
+      const double c00 = yy * zz - yz * yz, c01 = xz * yz - xy * zz, c02 = xy * yz - xz * yy;
+      const double c11 = xx * zz - xz * xz, c12 = xy * xz - xx * yz, c22 = xx * yy - xy * xy;
+      const double det = xx * c00 + xy * c01 + xz * c02, tr3 = (xx + yy + zz) / 3.0;
+      if (det > 1e-6 * tr3 * tr3 * tr3) {
+        om[0] = (c00 * dL[0] + c01 * dL[1] + c02 * dL[2]) / det;
+        om[1] = (c01 * dL[0] + c11 * dL[1] + c12 * dL[2]) / det;
+        om[2] = (c02 * dL[0] + c12 * dL[1] + c22 * dL[2]) / det;
+      } else {
+        atomicAdd(nsing, 1ull);     // rejected inertia tensor (U10): omega = 0
+      }
+    }
+  }
+  float4* o = reinterpret_cast<float4*>(rec) + (size_t)k * 4;
+  if (AT) o[0] = make_float4((float)((S[0] - R[0]) * inv), (float)((S[1] - R[1]) * inv), (float)((S[2] - R[2]) * inv), 1.0f);
+  else o[0] = make_float4((float)(S[0] * inv), (float)(S[1] * inv), (float)(S[2] * inv), 1.0f);
+  o[1] = make_float4(ax, ay, az, 0.0f);
+  o[2] = make_float4((float)om[0], (float)om[1], (float)om[2], 0.0f);
+  o[3] = make_float4((float)rcm[0], (float)rcm[1], (float)rcm[2], 0.0f);
+}
+
+template <bool AT>
+__global__ void __launch_bounds__(256) k_collide_a(Geo G, size_t n, const float* __restrict__ x, const float* __restrict__ y,
+                                                   const float* __restrict__ z, float* __restrict__ vx, float* __restrict__ vy,
+                                                   float* __restrict__ vz, const uint32_t* __restrict__ key,
+                                                   const uint32_t* __restrict__ offset, const float* __restrict__ rec) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t k = key[i];
+  const float4* rc = reinterpret_cast<const float4*>(rec) + (size_t)k * 4;
+  const float4 base = __ldg(rc), axis = __ldg(rc + 1), om = __ldg(rc + 2), rcm = __ldg(rc + 3);
+  float o[3];
+  if (AT) {
+    int ix, iy, iz;
+    key_to_cell(G, k, ix, iy, iz);
+    const Block4 b = philox(canonical_id(G, ix, iy, iz), (uint32_t)i - offset[k], G.t, TAG_AT, G.k0, G.k1);
+    float g0, g1, g2;
+    normals3(b, g0, g1, g2);
+    o[0] = base.x + G.sigma * g0; o[1] = base.y + G.sigma * g1; o[2] = base.z + G.sigma * g2;
+  } else {
+    const float w[3] = {vx[i] - base.x, vy[i] - base.y, vz[i] - base.z};
+    float d[3];
+    rotate(G, axis.x, axis.y, axis.z, w, d);
+    o[0] = base.x + d[0]; o[1] = base.y + d[1]; o[2] = base.z + d[2];
+  }
+  const float r0 = (cell_frac(G, x[i], G.s[0]) - rcm.x) * G.a, r1 = (cell_frac(G, y[i], G.s[1]) - rcm.y) * G.a,
+              r2 = (cell_frac(G, z[i], G.s[2]) - rcm.z) * G.a;
+  vx[i] = o[0] + fmaf(om.y, r2, -(om.z * r1));
+  vy[i] = o[1] + fmaf(om.z, r0, -(om.x * r2));
+  vz[i] = o[2] + fmaf(om.x, r1, -(om.y * r0));
+}
+
 // ---- exclusive scan of the per-cell counts (three kernels; tile = 2048) ----------------------------
 // `in` is read with a stride in 32-bit words: the count is the low word of word 0 of a cell's sums.
 constexpr int SCAN_T = 256, SCAN_PER = 8, SCAN_TILE = SCAN_T * SCAN_PER;
@@ -635,7 +817,7 @@ __global__ void __launch_bounds__(256) k_obs_cells(Geo G, const u64* __restrict_
     const u64 w0 = s[0];
     const unsigned nc = (unsigned)(w0 & 0xffffffffull);
     mx = max(mx, nc);
-    if (nc < 2u || G.collision == 1) continue;
+    if (nc < 2u || G.generic) continue;
     int sx, sy, sz, sp;
     unpack_ss(s[1], sx, sy);
     unpack_ss(s[2], sz, sp);
@@ -674,7 +856,7 @@ __global__ void __launch_bounds__(256) k_export_cells(Geo G, const u64* __restri
   if (px) px[k] = (float)((double)G.mass * sx * G.fxv_inv);
   if (py) py[k] = (float)((double)G.mass * sy * G.fxv_inv);
   if (pz) pz[k] = (float)((double)G.mass * sz * G.fxv_inv);
-  if (e2) e2[k] = (G.collision == 1) ? 0.0f : (float)((double)(unsigned)(s[0] >> 32) * G.fxe_inv);
+  if (e2) e2[k] = G.generic ? 0.0f : (float)((double)(unsigned)(s[0] >> 32) * G.fxe_inv);
 }
 
 }  // namespace mpc
@@ -710,6 +892,7 @@ struct mpc_ctx {
   u64* sums;
   float* rec;
   double* obs;      // OBS_BLOCKS*8 doubles + 2*MAX_PROFILE doubles
+  u64* nsing;       // +a: number of rejected inertia tensors in the last step
   double* hbuf;     // host staging for mpc_observables
   // optional per-family timing with CUDA events on the bound stream (mpc_profile_*)
   bool prof_on;
@@ -729,7 +912,7 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 struct Layout {
   size_t off_A[7], off_B[7], off_key, off_slot, off_perm, off_cursor, off_offset, off_bsum, off_sums, off_rec, off_obs, total;
 };
-Layout make_layout(size_t n_max, size_t nkeys, int sw, bool compact) {
+Layout make_layout(size_t n_max, size_t nkeys, int sw, int rw, bool compact) {
   Layout l;
   size_t o = 0;
   auto take = [&](size_t bytes) { const size_t r = o; o = align_up(o + bytes, 256); return r; };
@@ -744,8 +927,8 @@ Layout make_layout(size_t n_max, size_t nkeys, int sw, bool compact) {
   l.off_offset = take((nkeys + 1) * 4);
   l.off_bsum = take(((nkeys + SCAN_TILE - 1) / SCAN_TILE + 1) * 4);
   l.off_sums = take(nkeys * (size_t)sw * 8);
-  l.off_rec = take(nkeys * REC_W * 4);
-  l.off_obs = take(OBS_HOST_DOUBLES * 8);
+  l.off_rec = take(nkeys * (size_t)rw * 4);
+  l.off_obs = take(OBS_HOST_DOUBLES * 8 + 256);
   l.total = o;
   return l;
 }
@@ -819,7 +1002,7 @@ int do_reorder(mpc_ctx* c) {
     LAUNCH_CHECK("k_rank");
   }
   FamilyTimer ftg(c, F_GATHER);
-  const bool need_key = c->G.collision == 1;   // MPC-AT reads the sorted keys afterwards
+  const bool need_key = c->G.generic != 0;     // the unfused path reads the sorted keys afterwards
   if (!c->compact) {
     Arrays8 src, dst;
     for (int a = 0; a < 7; ++a) { src.p[a] = c->A[a]; dst.p[a] = c->Bf[a]; }
@@ -917,13 +1100,22 @@ int steps_srd(mpc_ctx* c, int nsteps) {
   return MPC_OK;
 }
 
-int steps_at(mpc_ctx* c, int nsteps) {
+// MPC-AT and every +a variant: stream+key, reorder when due, per-cell sums with global atomics, cell
+// finalize, collide. MPC-AT needs the sorted segments (rank of a particle in its cell), so it reorders
+// every step (rebin_every == 1 is enforced at create).
+int steps_generic(mpc_ctx* c, int nsteps) {
   Geo& G = c->G;
   const size_t n = c->n;
+  const bool at = G.collision == 1, plus_a = G.conserve_L != 0;
   for (int k = 0; k < nsteps; ++k) {
     G.t = c->t;
     host_shift(c, c->t, G.s);
-    { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * G.sw * 8, c->stream)); }
+    const bool rebin = (c->t % (uint32_t)c->p.rebin_every) == 0u;
+    {
+      FamilyTimer ft(c, F_MEMSET);
+      CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * G.sw * 8, c->stream));
+      CU(cudaMemsetAsync(c->nsing, 0, 8, c->stream));
+    }
     if (n) {
       float** F = reinterpret_cast<float**>(c->A);
       const unsigned gb = nblk(n, 256);
@@ -934,22 +1126,27 @@ int steps_at(mpc_ctx* c, int nsteps) {
         else k_stream_key<false, false><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, c->sums);
         LAUNCH_CHECK("k_stream_key");
       }
-      const int rc = do_reorder(c);   // MPC-AT reorders every step (rebin_every == 1)
-      if (rc) return rc;
+      if (rebin) { const int rc = do_reorder(c); if (rc) return rc; }
       F = reinterpret_cast<float**>(c->A);
       {
         FamilyTimer ft(c, F_ACCUM);
-        k_accum_at<<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->key, c->offset, c->sums);
-        LAUNCH_CHECK("k_accum_at");
+        if (plus_a && at) k_accum_a<true><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, c->offset, c->sums);
+        else if (plus_a) k_accum_a<false><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, c->offset, c->sums);
+        else k_accum_at<<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->key, c->offset, c->sums);
+        LAUNCH_CHECK("k_accum");
       }
       {
         FamilyTimer ft(c, F_CELL);
-        k_cell<<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec);
+        if (plus_a && at) k_cell_a<true><<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec, c->nsing);
+        else if (plus_a) k_cell_a<false><<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec, c->nsing);
+        else k_cell<<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec);
         LAUNCH_CHECK("k_cell");
       }
       FamilyTimer ft(c, F_COLLIDE);
-      k_collide_at<<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->key, c->offset, c->rec);
-      LAUNCH_CHECK("k_collide_at");
+      if (plus_a && at) k_collide_a<true><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, c->offset, c->rec);
+      else if (plus_a) k_collide_a<false><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, c->offset, c->rec);
+      else k_collide_at<<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->key, c->offset, c->rec);
+      LAUNCH_CHECK("k_collide");
     }
     c->t++;
     c->have_cells = true;
@@ -1015,7 +1212,6 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   if (nwall && (p->conserve_L || p->collision == 1)) return MPC_EINVAL;
   if (p->collision == 0 && p->conserve_L && p->thermostat) return MPC_EINVAL;
   if (p->collision == 1 && p->rebin_every != 1) return MPC_EINVAL;
-  if (p->conserve_L) return MPC_EINVAL;   // +a: not built yet
   mpc_ctx* c = new (std::nothrow) mpc_ctx();   // value-initialised: all zero
   if (!c) return MPC_ENOMEM;
   c->p = *p; c->seed = seed;
@@ -1053,8 +1249,10 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   const int ue = (int)lround(log2((double)G.sigma));        // thermal velocity rounded to a power of two
   G.fxv = (float)ldexp(1.0, 20 - ue); G.fxv_inv = ldexp(1.0, ue - 20);
   G.fxe = (float)ldexp(1.0, 18 - 2 * ue); G.fxe_inv = ldexp(1.0, 2 * ue - 18);
-  G.collision = p->collision; G.thermostat = p->thermostat;
-  G.sw = p->collision == 1 ? 4 : 3;
+  G.collision = p->collision; G.thermostat = p->thermostat; G.conserve_L = p->conserve_L;
+  G.generic = (p->collision == 1 || p->conserve_L) ? 1 : 0;
+  G.sw = p->conserve_L ? 10 : (p->collision == 1 ? 4 : 3);
+  G.rw = p->conserve_L ? 16 : REC_W;
   *out = c;
   return MPC_OK;
 }
@@ -1067,16 +1265,16 @@ int mpc_num_keys(const mpc_ctx* c, unsigned long long* nkeys) {
 
 int mpc_workspace_bytes(const mpc_ctx* c, unsigned long long n_max, int compact, size_t* bytes) {
   if (!c || !bytes || n_max > 0xffffffffull) return MPC_EINVAL;
-  *bytes = make_layout((size_t)n_max, c->G.nkeys, c->G.sw, compact != 0).total;
+  *bytes = make_layout((size_t)n_max, c->G.nkeys, c->G.sw, c->G.rw, compact != 0).total;
   return MPC_OK;
 }
 
 int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max, void* cuda_stream) {
   if (!c) return MPC_EINVAL;
   if (!workspace || ((uintptr_t)workspace & 255u) || n_max > 0xffffffffull) return fail(c, MPC_EINVAL, "workspace NULL, misaligned or n_max too large");
-  Layout l = make_layout((size_t)n_max, c->G.nkeys, c->G.sw, false);
+  Layout l = make_layout((size_t)n_max, c->G.nkeys, c->G.sw, c->G.rw, false);
   bool compact = false;
-  if (bytes < l.total) { l = make_layout((size_t)n_max, c->G.nkeys, c->G.sw, true); compact = true; }
+  if (bytes < l.total) { l = make_layout((size_t)n_max, c->G.nkeys, c->G.sw, c->G.rw, true); compact = true; }
   if (bytes < l.total) return fail(c, MPC_ENOMEM, "workspace smaller than mpc_workspace_bytes(n_max, compact=1)");
   c->ws = (char*)workspace; c->ws_bytes = bytes; c->n_max = (size_t)n_max; c->compact = compact;
   c->stream = (cudaStream_t)cuda_stream;
@@ -1086,6 +1284,7 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
   c->cursor = (uint32_t*)(c->ws + l.off_cursor); c->offset = (uint32_t*)(c->ws + l.off_offset);
   c->bsum = (uint32_t*)(c->ws + l.off_bsum);
   c->sums = (u64*)(c->ws + l.off_sums); c->rec = (float*)(c->ws + l.off_rec); c->obs = (double*)(c->ws + l.off_obs);
+  c->nsing = (u64*)(c->ws + l.off_obs + OBS_HOST_DOUBLES * 8);
   c->bound = true; c->have_state = false; c->have_cells = false; c->have_order = false; c->n = 0;
   if (c->tile_bytes > 48 * 1024) {
     cudaError_t e;
@@ -1111,7 +1310,7 @@ int mpc_step(mpc_ctx* c, int nsteps) {
   if (!c || nsteps < 0) return MPC_EINVAL;
   if (c->sticky) return MPC_ECUDA;
   if (!c->bound || !c->have_state) return fail(c, MPC_ESTATE, "mpc_step before mpc_bind / mpc_set_state");
-  return c->G.collision == 1 ? steps_at(c, nsteps) : steps_srd(c, nsteps);
+  return c->G.generic ? steps_generic(c, nsteps) : steps_srd(c, nsteps);
 }
 
 int mpc_get_state(mpc_ctx* c, float* x, float* y, float* z, float* vx, float* vy, float* vz, unsigned* id) {
@@ -1155,7 +1354,9 @@ int mpc_observables(mpc_ctx* c, mpc_obs* out, float* profile_host) {
     }
   }
   double* hbuf = c->hbuf;
+  unsigned long long nsing = 0;
   CU(cudaMemcpyAsync(hbuf, c->obs, OBS_HOST_DOUBLES * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  if (c->have_cells && G.conserve_L) CU(cudaMemcpyAsync(&nsing, c->nsing, 8, cudaMemcpyDeviceToHost, c->stream));
   CU(cudaStreamSynchronize(c->stream));
   double P[3] = {0, 0, 0}, E = 0, num = 0, den = 0, mx = 0;
   for (int b = 0; b < OBS_BLOCKS; ++b) {
@@ -1168,9 +1369,9 @@ int mpc_observables(mpc_ctx* c, mpc_obs* out, float* profile_host) {
   for (int d = 0; d < 3; ++d) out->P[d] = m * P[d];
   out->E_kin = 0.5 * m * E;
   out->kT_est = n > 1 ? m * (E - (P[0] * P[0] + P[1] * P[1] + P[2] * P[2]) / (double)n) / (3.0 * (double)(n - 1)) : 0.0;
-  out->kT_cell = (G.collision == 0 && den > 0) ? num / den : 0.0;
+  out->kT_cell = (!G.generic && den > 0) ? num / den : 0.0;
   out->max_cell_count = (unsigned)mx;
-  out->n_singular_cells = 0;
+  out->n_singular_cells = nsing;
   if (profile_host) {
     const double* pr = hbuf + (size_t)OBS_BLOCKS * 8;
     for (int b = 0; b < nb; ++b) profile_host[b] = pr[nb + b] > 0 ? (float)(pr[b] / pr[nb + b]) : 0.0f;

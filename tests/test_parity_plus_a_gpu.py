@@ -1,0 +1,127 @@
+"""GPU parity for the angular-momentum-conserving variants SRD+a (Eqs. 3-4) and
+MPC-AT+a (U5). Tolerance per DESIGN.md U10: 2e-5 sqrt(kT/m) where the cell's inertia tensor
+is well conditioned in absolute terms (smallest eigenvalue >= 0.1 m a^2; the typical value at
+<N_c> = 10 is ~1), growing as 1/lambda_min below that (omega = I^-1 dL amplifies the 2^-22 fixed-point
+quantum of the sums), capped at 2e-3."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle.binding import Oracle  # noqa: E402
+from paper_2406_15236_b200 import MPC  # noqa: E402
+from paper_2406_15236_b200.inputs import uniform_maxwell  # noqa: E402
+from test_parity_gpu import gpu_get, gpu_set  # noqa: E402
+
+
+def lambda_min_per_particle(o, so, key, step):
+    """Smallest eigenvalue of every cell's inertia tensor / (m a^2) (N=2: sum |r|^2), per particle."""
+    s = o.grid_shift(step).astype(np.float32)
+    q = np.stack(so[0:3], 1) + s
+    rho = (q - np.floor(q)).astype(np.float64)
+    nk = o.nkeys
+    key = key.astype(np.int64)
+    N = np.bincount(key, minlength=nk).astype(float)
+    rcm = np.stack([np.bincount(key, weights=rho[:, d], minlength=nk) / np.maximum(N, 1) for d in range(3)], 1)
+    r = rho - rcm[key]
+    r2 = (r**2).sum(1)
+    I = np.zeros((nk, 3, 3))
+    for a in range(3):
+        for b in range(3):
+            I[:, a, b] = np.bincount(key, weights=(r2 if a == b else 0) - r[:, a] * r[:, b], minlength=nk)
+    ev = np.linalg.eigvalsh(I)
+    lam = np.where(N == 2, np.bincount(key, weights=r2, minlength=nk), ev[:, 0])
+    det_ratio = np.where(N >= 3, np.prod(ev, axis=1) / np.maximum(ev.mean(axis=1), 1e-300) ** 3, 1.0)
+    return lam[key], N[key], det_ratio[key]
+
+
+@pytest.mark.parametrize("collision,nbar,every,brick", [(0, 10, 1, 4), (0, 10, 3, (16, 16, 8)), (0, 3, 1, 1),
+                                                         (1, 10, 1, 4), (1, 3, 1, (4, 2, 1))])
+def test_plus_a_parity(collision, nbar, every, brick):
+    cells = (16, 16, 8)
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar + 11
+    st = uniform_maxwell(box, n, 5)
+    kw = dict(collision=collision, conserve_L=1, dt=0.05, brick=brick, rebin_every=every)
+    o = Oracle(box, cells, nbar, 77, **kw)
+    g = MPC(box, cells, nbar, 77, n_max=n, **kw)
+    o.set_state(*st)
+    for t in range(every + 1):
+        gpu_set(g, o.get_state(), step=t)
+        o.step(1)
+        g.step(1)
+        so, sg = o.get_state(), gpu_get(g)
+        assert np.array_equal(so[6], sg[6])                                   # sort order
+        for d in range(3):
+            assert np.max(np.abs(so[d] - sg[d])) <= 1e-5
+        cnt_o, px, py, pz, _e, key_o = o.get_cells()
+        cnt_g, gx, gy, gz, _ge, key_g = [a.cpu().numpy() for a in g.get_cells()]
+        assert np.array_equal(key_o, key_g.view(np.uint32))
+        assert np.array_equal(cnt_o, cnt_g.view(np.uint32))
+        lam, N, det_ratio = lambda_min_per_particle(o, so, key_o, t)
+        err = np.max(np.abs(np.stack(so[3:6]).astype(np.float64) - np.stack(sg[3:6])), axis=0)
+        tol = np.clip(2e-5 * 0.1 / np.maximum(lam, 1e-12), 2e-5, 2e-3)
+        # cells whose determinant test (U10) sits within a factor 4 of its threshold may be decided
+        # differently in fp64-from-fp32-sums and in the oracle's direct fp64: compare them loosely
+        borderline = (N >= 3) & (det_ratio < 4e-6 * 27) & (det_ratio > 0.25e-6 * 27)
+        ok = (err <= tol) | borderline
+        assert ok.all(), f"worst err/tol = {np.max(err / tol):.2f} at lambda_min={lam[np.argmax(err / tol)]:.3g}"
+        assert borderline.mean() < 1e-3
+        if nbar == 10:
+            assert np.mean(lam >= 0.1) > 0.97 and np.max(err[lam >= 0.1]) <= 2e-5
+        ns_o, ns_g = o.observables()["n_singular_cells"], g.observables()["n_singular_cells"]
+        assert abs(int(ns_o) - int(ns_g)) <= max(1, int(borderline.sum()))
+
+
+@pytest.mark.parametrize("collision", [0, 1])
+def test_plus_a_conserves_angular_momentum_on_gpu(collision):
+    # the invariant itself, measured on the GPU output (not only agreement with the oracle)
+    cells, nbar = (12, 12, 12), 10
+    box = (12.0, 12.0, 12.0)
+    n = 12**3 * nbar
+    st = uniform_maxwell(box, n, 9)
+    kw = dict(collision=collision, conserve_L=1, dt=0.05, brick=4)
+    g = MPC(box, cells, nbar, 5, n_max=n, **kw)
+    gpu_set(g, st)
+    g.step(1)
+    x, y, z, vx, vy, vz, ids = gpu_get(g)
+    key = g.get_cells()[5].cpu().numpy().view(np.uint32).astype(np.int64)
+    order = np.argsort(ids)
+    o = Oracle(box, cells, nbar, 5, **kw)
+    s = o.grid_shift(0).astype(np.float32)
+    q = np.stack([x, y, z], 1)[order] + s
+    rho = (q - np.floor(q)).astype(np.float64)
+    key = key[order]
+    nk = g.nkeys
+    N = np.bincount(key, minlength=nk).astype(float)
+    rcm = np.stack([np.bincount(key, weights=rho[:, d], minlength=nk) / np.maximum(N, 1) for d in range(3)], 1)
+    r = rho - rcm[key]
+    pre = np.stack(st[3:6], 1).astype(np.float64)
+    post = np.stack([vx, vy, vz], 1).astype(np.float64)[order]
+    L0 = np.stack([np.bincount(key, weights=np.cross(r, pre)[:, d], minlength=nk) for d in range(3)], 1)
+    L1 = np.stack([np.bincount(key, weights=np.cross(r, post)[:, d], minlength=nk) for d in range(3)], 1)
+    scale = np.bincount(key, weights=np.abs(pre).sum(1), minlength=nk) + 1e-30
+    rel = np.abs(L1 - L0).max(1) / scale
+    assert np.quantile(rel, 0.999) < 1e-5
+    P0 = np.stack([np.bincount(key, weights=pre[:, d], minlength=nk) for d in range(3)], 1)
+    P1 = np.stack([np.bincount(key, weights=post[:, d], minlength=nk) for d in range(3)], 1)
+    assert (np.abs(P1 - P0).max(1) / scale).max() < 1e-5
+    assert np.mean(np.abs(post - pre).max(1) > 1e-3) > 0.9
+
+
+def test_at_plus_a_multi_step_call_equals_single_steps():
+    cells, nbar = (16, 16, 8), 10
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    st = uniform_maxwell(box, n, 3)
+    res = []
+    for calls in ((5,), (1,) * 5, (2, 3)):
+        g = MPC(box, cells, nbar, 17, n_max=n, collision=1, conserve_L=1, dt=0.02, brick=(16, 16, 8))
+        gpu_set(g, st)
+        for k in calls:
+            g.step(k)
+        res.append(gpu_get(g))
+    for r in res[1:]:
+        for a, b in zip(res[0], r):
+            assert np.array_equal(a, b)
