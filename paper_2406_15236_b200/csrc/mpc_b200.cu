@@ -55,7 +55,8 @@ struct Geo {
   float cosa, sina;
   float kT, mass, sigma;   // sigma = sqrt(kT/m)
   // Fixed-point scales: powers of two relative to u = 2^round(log2 sigma), so precision does not
-  // depend on the unit system:  velocity sums 2^20/u (|sum v_d| < 2048 u), energy sums 2^18/u^2.
+  // depend on the unit system: velocity sums 2^22/u in int32 (|sum_cell v_d| < 512 u); energy sums
+  // 2^22/u^2, uint32 per tile (< 1024 u^2 per cell and CTA) and 48 bits in the global word.
   float fxv, fxe;
   double fxv_inv, fxe_inv;
   int nbar;
@@ -67,7 +68,7 @@ struct Geo {
 };
 
 // ---- packed sums ---------------------------------------------------------------------------------
-// word0 = E << 32 | N (both unsigned); word1 = (Sy, Sx); word2 = (R0, Sz); word3 = (R2, R1)  [AT: R = sum v_ran]
+// word0 = E << 16 | N (E: 48 bits, N: 16 bits, so at most 65535 particles per cell); word1 = (Sy, Sx); word2 = (R0, Sz); word3 = (R2, R1)  [AT: R = sum v_ran]
 // +a adds, in cell-local coordinates rho in [0,1)^3 (U9), scale 2^20 for rho terms:
 // word4 = (rho_y, rho_x); word5 = (Qxx, rho_z); word6 = (Qzz, Qyy); word7 = (Qxz, Qxy); word8 = (Lx, Qyz);
 // word9 = (Lz, Ly)   with Q = sum rho rho^T, L = sum rho x u, u = v - D v (SRD) or v - v_ran (AT)
@@ -281,7 +282,7 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       if (WKEY) key_out[i] = kc;
       if (!inside) {
         u64* s = sums + (size_t)kc * G.sw;
-        atomicAdd(s, ((u64)e << 32) | 1ull); atomicAdd(s + 1, pack_ss(a0, a1)); atomicAdd(s + 2, pack_ss(a2, 0));
+        atomicAdd(s, ((u64)e << 16) | 1ull); atomicAdd(s + 1, pack_ss(a0, a1)); atomicAdd(s + 2, pack_ss(a2, 0));
       }
     }
   }
@@ -293,7 +294,7 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
     if (cnt == 0) continue;
     const int l0 = c % T0, q = c / T0, l1 = q % T1, l2 = q / T1;
     u64* g = sums + (size_t)BS::key(G, fold(ox + l0, m0), fold(oy + l1, m1), fold(oz + l2, m2)) * G.sw;
-    atomicAdd(g, ((u64)(unsigned)s[4] << 32) | (u64)(unsigned)cnt);
+    atomicAdd(g, ((u64)(unsigned)s[4] << 16) | (u64)(unsigned)cnt);
     atomicAdd(g + 1, pack_ss(s[1], s[2]));
     atomicAdd(g + 2, pack_ss(s[3], 0));
   }
@@ -371,7 +372,6 @@ __global__ void __launch_bounds__(256) k_collide_at(Geo G, size_t n, float* __re
 // ---- +a variants (Eqs. 3-4; MPC-AT+a, U5): unfused path --------------------------------
 constexpr float FX_RHO = 4194304.0f;            // 2^22 per unit of cell-local coordinate (products too): N_c < 512
 constexpr double FX_RHO_INV = 1.0 / 4194304.0;
-constexpr float FX_L = 4.0f;                    // angular-momentum terms: 4x the velocity scale (|rho x u| < 512 u)
 
 __device__ __forceinline__ void srd_axis(const Geo& G, uint32_t cid, float& ax, float& ay, float& az) {
   const Block4 o = philox(cid, 0u, G.t, TAG_AXIS, G.k0, G.k1);
@@ -432,8 +432,8 @@ __global__ void __launch_bounds__(256) k_accum_a(Geo G, size_t n, const float* _
   atomicAdd(s + 5, pack_ss(fq(r2), fq(r0 * r0)));
   atomicAdd(s + 6, pack_ss(fq(r1 * r1), fq(r2 * r2)));
   atomicAdd(s + 7, pack_ss(fq(r0 * r1), fq(r0 * r2)));
-  atomicAdd(s + 8, pack_ss(fq(r1 * r2), fv(l0 * FX_L)));
-  atomicAdd(s + 9, pack_ss(fv(l1 * FX_L), fv(l2 * FX_L)));
+  atomicAdd(s + 8, pack_ss(fq(r1 * r2), fv(l0)));
+  atomicAdd(s + 9, pack_ss(fv(l1), fv(l2)));
 }
 
 // rec[key] (16 floats) = { base.xyz, 1 | axis.xyz, - | omega.xyz, - | rho_cm.xyz, - }
@@ -448,7 +448,7 @@ __global__ void __launch_bounds__(128) k_cell_a(Geo G, int cpb_shift, const u64*
   const uint32_t brick = (bz * (uint32_t)G.mb[1] + by) * (uint32_t)G.mb[0] + bx;
   const uint32_t k = (brick << (b0 + b1 + b2)) | local;
   const u64* s = sums + (size_t)k * G.sw;
-  const uint32_t N = (uint32_t)(s[0] & 0xffffffffull);
+  const uint32_t N = (uint32_t)(s[0] & 0xffffull);
   if (N == 0u) return;
   const int ix = (int)((bx << b0) | (local & ((1u << b0) - 1u)));
   const int iy = (int)((by << b1) | ((local >> b0) & ((1u << b1) - 1u)));
@@ -484,7 +484,7 @@ __global__ void __launch_bounds__(128) k_cell_a(Geo G, int cpb_shift, const u64*
     const double Qxx = q3 * FX_RHO_INV - Nd * rcm[0] * rcm[0], Qyy = q4 * FX_RHO_INV - Nd * rcm[1] * rcm[1];
     const double Qzz = q5 * FX_RHO_INV - Nd * rcm[2] * rcm[2], Qxy = q6 * FX_RHO_INV - Nd * rcm[0] * rcm[1];
     const double Qxz = q7 * FX_RHO_INV - Nd * rcm[0] * rcm[2], Qyz = q8 * FX_RHO_INV - Nd * rcm[1] * rcm[2];
-    const double Lr[3] = {q9 * G.fxv_inv * 0.25, q10 * G.fxv_inv * 0.25, q11 * G.fxv_inv * 0.25};
+    const double Lr[3] = {q9 * G.fxv_inv, q10 * G.fxv_inv, q11 * G.fxv_inv};
     const double dL[3] = {m * a * (Lr[0] - (rcm[1] * Su[2] - rcm[2] * Su[1])),
                           m * a * (Lr[1] - (rcm[2] * Su[0] - rcm[0] * Su[2])),
                           m * a * (Lr[2] - (rcm[0] * Su[1] - rcm[1] * Su[0]))};
@@ -546,7 +546,7 @@ __global__ void __launch_bounds__(256) k_collide_a(Geo G, size_t n, const float*
 }
 
 // ---- exclusive scan of the per-cell counts (three kernels; tile = 2048) ----------------------------
-// `in` is read with a stride in 32-bit words: the count is the low word of word 0 of a cell's sums.
+// `in` is read with a stride in 32-bit words: the count is the low 16 bits of word 0 of a cell's sums.
 constexpr int SCAN_T = 256, SCAN_PER = 8, SCAN_TILE = SCAN_T * SCAN_PER;
 
 __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t& total) {
@@ -583,7 +583,7 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_reduce(const uint32_t* __restri
 #pragma unroll
   for (int j = 0; j < SCAN_PER; ++j) {
     const size_t i = base + (size_t)j * SCAN_T + threadIdx.x;
-    if (i < n) s += in[i * stride];
+    if (i < n) s += in[i * stride] & 0xffffu;
   }
   __shared__ uint32_t red[SCAN_T / 32];
 #pragma unroll
@@ -613,7 +613,7 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const uint32_t* __restric
   uint32_t v[SCAN_PER], s = 0;
 #pragma unroll
   for (int j = 0; j < SCAN_PER; ++j) {
-    v[j] = (base + j < n) ? in[(base + j) * stride] : 0u;
+    v[j] = (base + j < n) ? (in[(base + j) * stride] & 0xffffu) : 0u;
     s += v[j];
   }
   uint32_t total;
@@ -719,7 +719,7 @@ __global__ void __launch_bounds__(128) k_cell(Geo G, int cpb_shift, const u64* _
   const uint32_t k = (brick << (b0 + b1 + b2)) | local;
   const u64* s = sums + (size_t)k * G.sw;
   const u64 w0 = s[0];
-  const uint32_t nreal = (uint32_t)(w0 & 0xffffffffull);
+  const uint32_t nreal = (uint32_t)(w0 & 0xffffull);
   if (nreal == 0u) return;
   const int ix = (int)((bx << b0) | (local & ((1u << b0) - 1u)));
   const int iy = (int)((by << b1) | ((local >> b0) & ((1u << b1) - 1u)));
@@ -740,7 +740,7 @@ __global__ void __launch_bounds__(128) k_cell(Geo G, int cpb_shift, const u64* _
     r0.w = 1.0f;
     r1 = make_float4(0.f, 0.f, 0.f, 0.f);
   } else {
-    double E = (double)(uint32_t)(w0 >> 32) * G.fxe_inv;
+    double E = (double)(w0 >> 16) * G.fxe_inv;
     uint32_t Nc = nreal;
     if (G.wall >= 0) {
       // virtual wall particles fill wall-cut cells up to nbar (U8)
@@ -815,14 +815,14 @@ __global__ void __launch_bounds__(256) k_obs_cells(Geo G, const u64* __restrict_
   for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < G.nkeys; k += (size_t)gridDim.x * blockDim.x) {
     const u64* s = sums + k * G.sw;
     const u64 w0 = s[0];
-    const unsigned nc = (unsigned)(w0 & 0xffffffffull);
+    const unsigned nc = (unsigned)(w0 & 0xffffull);
     mx = max(mx, nc);
     if (nc < 2u || G.generic) continue;
     int sx, sy, sz, sp;
     unpack_ss(s[1], sx, sy);
     unpack_ss(s[2], sz, sp);
     const double S0 = sx * G.fxv_inv, S1 = sy * G.fxv_inv, S2 = sz * G.fxv_inv;
-    num += (double)G.mass * ((double)(unsigned)(w0 >> 32) * G.fxe_inv - (S0 * S0 + S1 * S1 + S2 * S2) / nc);
+    num += (double)G.mass * ((double)(w0 >> 16) * G.fxe_inv - (S0 * S0 + S1 * S1 + S2 * S2) / nc);
     den += 3.0 * (nc - 1u);
   }
   atomicMax(&smax, mx);
@@ -852,11 +852,11 @@ __global__ void __launch_bounds__(256) k_export_cells(Geo G, const u64* __restri
   int sx, sy, sz, sp;
   unpack_ss(s[1], sx, sy);
   unpack_ss(s[2], sz, sp);
-  if (count) count[k] = (unsigned)(s[0] & 0xffffffffull);
+  if (count) count[k] = (unsigned)(s[0] & 0xffffull);
   if (px) px[k] = (float)((double)G.mass * sx * G.fxv_inv);
   if (py) py[k] = (float)((double)G.mass * sy * G.fxv_inv);
   if (pz) pz[k] = (float)((double)G.mass * sz * G.fxv_inv);
-  if (e2) e2[k] = G.generic ? 0.0f : (float)((double)(unsigned)(s[0] >> 32) * G.fxe_inv);
+  if (e2) e2[k] = G.generic ? 0.0f : (float)((double)(s[0] >> 16) * G.fxe_inv);
 }
 
 }  // namespace mpc
@@ -1247,8 +1247,8 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   G.k0 = (uint32_t)(seed & 0xffffffffull); G.k1 = (uint32_t)(seed >> 32);
   G.nbar = (int)lround((double)n_per_cell);
   const int ue = (int)lround(log2((double)G.sigma));        // thermal velocity rounded to a power of two
-  G.fxv = (float)ldexp(1.0, 20 - ue); G.fxv_inv = ldexp(1.0, ue - 20);
-  G.fxe = (float)ldexp(1.0, 18 - 2 * ue); G.fxe_inv = ldexp(1.0, 2 * ue - 18);
+  G.fxv = (float)ldexp(1.0, 22 - ue); G.fxv_inv = ldexp(1.0, ue - 22);
+  G.fxe = (float)ldexp(1.0, 22 - 2 * ue); G.fxe_inv = ldexp(1.0, 2 * ue - 22);
   G.collision = p->collision; G.thermostat = p->thermostat; G.conserve_L = p->conserve_L;
   G.generic = (p->collision == 1 || p->conserve_L) ? 1 : 0;
   G.sw = p->conserve_L ? 10 : (p->collision == 1 ? 4 : 3);
