@@ -32,6 +32,7 @@ typedef unsigned long long u64;
 
 constexpr int HALO = 2;               // tile halo in cells on every side of a brick
 constexpr int SWEEP_T = 512;          // threads per sweep CTA
+constexpr int PF_DIST = 4;           // L2 prefetch distance of the sweep, in iterations of SWEEP_T particles
 constexpr int TILE_W = 5;             // int32 words per tile cell: N, Sx, Sy, Sz, E
 constexpr int REC_W = 8;              // floats per cell record (32 B, one sector)
 constexpr int OBS_BLOCKS = 1184;      // 148 SMs x 8
@@ -253,6 +254,17 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
     float r[3] = {p0, p1, p2}, v[3] = {p3, p4, p5};
     const uint32_t inext = i + SWEEP_T;
     if (inext < i1) { p0 = x[inext]; p1 = y[inext]; p2 = z[inext]; p3 = vx[inext]; p4 = vy[inext]; p5 = vz[inext]; }
+    {   // pull the lines of a later iteration into L2: the register prefetch above then pays L2, not DRAM, latency
+      const uint32_t ifar = i + PF_DIST * SWEEP_T;
+      if (ifar < i1) {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(x + ifar));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(y + ifar));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(z + ifar));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(vx + ifar));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(vy + ifar));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(vz + ifar));
+      }
+    }
     if (COLLIDE) {   // ROTATE_VELOCITIES of the previous step; its key is recomputed from r and that step's shift
       int kx = cell_raw(G, r[0], sp0) + w0, ky = cell_raw(G, r[1], sp1) + w1, kz = cell_raw(G, r[2], sp2) + w2;
       if (WALL) { kx = G.bc[0] ? max(0, min(kx, m0 - 1)) : fold(kx, m0); ky = G.bc[1] ? max(0, min(ky, m1 - 1)) : fold(ky, m1);
