@@ -36,6 +36,9 @@ constexpr int SWEEP_T = 512;          // threads per sweep CTA
 #ifndef SWEEP4_T
 #define SWEEP4_T 512
 #endif
+#ifndef PF4_DIST
+#define PF4_DIST 1
+#endif
 constexpr int PF_DIST = 4;           // L2 prefetch distance of the sweep, in iterations of SWEEP_T particles
 constexpr int TILE_W = 5;             // int32 words per tile cell: N, Sx, Sy, Sz, E
 constexpr int REC_W = 8;              // floats per cell record (32 B, one sector)
@@ -250,7 +253,7 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
   // index offsets added before the floor index is folded: +1 on a wall axis (layer 0 lies in the wall)
   // the CTA takes the 128-byte-aligned groups of 32 particles that START in its range (see k_sweep4)
   i0 = (i0 + 31u) & ~31u;
-  if (b + 1 != nbricks) i1 = (i1 + 31u) & ~31u;
+  if (b + 1 != nbricks) i1 = min((i1 + 31u) & ~31u, n);   // trailing empty bricks: chunk = n, do not round past the end
   const int w0 = (WALL && G.bc[0]) ? 1 : 0, w1 = (WALL && G.bc[1]) ? 1 : 0, w2 = (WALL && G.bc[2]) ? 1 : 0;
   __syncthreads();
   // software pipeline: the loads of the next particle are in flight while this one is processed
@@ -329,9 +332,22 @@ struct SweepCtx {
   int ox, oy, oz, T0, T1, T2, m0, m1, m2, w0, w1, w2;
   float sp0, sp1, sp2;
 };
+// per-thread run of consecutive particles that fall into the same tile cell: their contributions are summed
+// in registers and leave as ONE group of shared atomics (integers: exact, order-independent)
+struct TileAcc {
+  int off;              // word offset of the cell in the tile, -1 = empty
+  int n, a0, a1, a2;
+  unsigned e;
+};
+__device__ __forceinline__ void acc_flush(int* tile, TileAcc& A) {
+  if (A.off >= 0) {
+    int* s = tile + A.off;
+    atomicAdd(s, A.n); atomicAdd(s + 1, A.a0); atomicAdd(s + 2, A.a1); atomicAdd(s + 3, A.a2); atomicAdd((unsigned*)s + 4, A.e);
+  }
+}
 template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS>
 __device__ __forceinline__ uint32_t sweep_particle(const Geo& G, const SweepCtx& C, float (&r)[3], float (&v)[3], bool valid,
-                                                   const float* __restrict__ rec, u64* __restrict__ sums) {
+                                                   const float* __restrict__ rec, u64* __restrict__ sums, TileAcc& A) {
   const int m0 = C.m0, m1 = C.m1, m2 = C.m2;
   if (COLLIDE) {   // ROTATE_VELOCITIES of the previous step; its key is recomputed from r and that step's shift
     int kx = cell_raw(G, r[0], C.sp0) + C.w0, ky = cell_raw(G, r[1], C.sp1) + C.w1, kz = cell_raw(G, r[2], C.sp2) + C.w2;
@@ -351,8 +367,9 @@ __device__ __forceinline__ uint32_t sweep_particle(const Geo& G, const SweepCtx&
   const int l0 = fold(cx - C.ox, m0), l1 = fold(cy - C.oy, m1), l2 = fold(cz - C.oz, m2);
   const bool inside = (l0 < C.T0) & (l1 < C.T1) & (l2 < C.T2);
   if (valid && inside) {
-    int* s = C.tile + ((l2 * C.T1 + l1) * C.T0 + l0) * TILE_W;
-    atomicAdd(s, 1); atomicAdd(s + 1, a0); atomicAdd(s + 2, a1); atomicAdd(s + 3, a2); atomicAdd((unsigned*)s + 4, e);
+    const int off = ((l2 * C.T1 + l1) * C.T0 + l0) * TILE_W;
+    if (off == A.off) { A.n += 1; A.a0 += a0; A.a1 += a1; A.a2 += a2; A.e += e; }
+    else { acc_flush(C.tile, A); A.off = off; A.n = 1; A.a0 = a0; A.a1 = a1; A.a2 = a2; A.e = e; }
   }
   uint32_t kc = 0;
   if (WKEY || !inside) {
@@ -403,14 +420,15 @@ k_sweep4(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__
   // group belongs to exactly one CTA and every 128-bit access of a warp is line-aligned. The few
   // particles this hands to the neighbouring brick's CTA fall into its halo or take the global path.
   const uint32_t g0 = ((i0 + 31u) >> 5) << 3;
-  const uint32_t g1 = (b + 1 == nbricks) ? (uint32_t)(((u64)n + 3ull) >> 2) : (((i1 + 31u) >> 5) << 3);
+  const uint32_t gend = (uint32_t)(((u64)n + 3ull) >> 2);
+  const uint32_t g1 = (b + 1 == nbricks) ? gend : min(((i1 + 31u) >> 5) << 3, gend);
   for (uint32_t g = g0 + threadIdx.x; g < g1; g += SWEEP4_T) {
     const size_t p = (size_t)g << 2;
     float rx[4], ry[4], rz[4], ux[4], uy[4], uz[4];
     unpack4(ldg4(x + p), rx); unpack4(ldg4(y + p), ry); unpack4(ldg4(z + p), rz);
     unpack4(ldg4(vx + p), ux); unpack4(ldg4(vy + p), uy); unpack4(ldg4(vz + p), uz);
     {   // pull the lines of a later iteration into L2
-      const size_t pf = p + (size_t)PF_DIST * SWEEP4_T * 4;
+      const size_t pf = p + (size_t)PF4_DIST * SWEEP4_T * 4;
       if (pf < i1 && (threadIdx.x & 7) == 0) {   // one prefetch per 128-byte line (8 threads x 16 B)
         asm volatile("prefetch.global.L2 [%0];" ::"l"(x + pf));
         asm volatile("prefetch.global.L2 [%0];" ::"l"(y + pf));
@@ -427,12 +445,15 @@ k_sweep4(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__
         if (p + j >= n) { rx[j] = ry[j] = rz[j] = 0.f; ux[j] = uy[j] = uz[j] = 0.f; }
     }
     uint32_t kc[4];
+    TileAcc A;
+    A.off = -1; A.n = 0; A.a0 = A.a1 = A.a2 = 0; A.e = 0u;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
       float r[3] = {rx[j], ry[j], rz[j]}, v[3] = {ux[j], uy[j], uz[j]};
-      kc[j] = sweep_particle<COLLIDE, WALL, GRAV, WKEY, BS>(G, C, r, v, !tail || p + j < n, rec, sums);
+      kc[j] = sweep_particle<COLLIDE, WALL, GRAV, WKEY, BS>(G, C, r, v, !tail || p + j < n, rec, sums, A);
       rx[j] = r[0]; ry[j] = r[1]; rz[j] = r[2]; ux[j] = v[0]; uy[j] = v[1]; uz[j] = v[2];
     }
+    acc_flush(C.tile, A);
     stg4(x + p, rx); stg4(y + p, ry); stg4(z + p, rz); stg4(vx + p, ux); stg4(vy + p, uy); stg4(vz + p, uz);
     if (WKEY) *reinterpret_cast<uint4*>(key_out + p) = make_uint4(kc[0], kc[1], kc[2], kc[3]);
   }
@@ -859,14 +880,15 @@ __device__ float mbs_energy(const Geo& G, uint32_t cid, uint32_t Nc) {
 
 // rec[key] = SRD: { vcm.x, vcm.y, vcm.z, kappa, n.x, n.y, n.z, - }   AT: { (vcm - mean v_ran).xyz, ... }
 // grid = (mb0 * CTAs-per-brick, mb1, mb2): the brick coordinates come from blockIdx, no division
-__global__ void __launch_bounds__(128) k_cell(Geo G, int cpb_shift, const u64* __restrict__ sums, float* __restrict__ rec) {
+// zero != 0: the sums of a cell are cleared once read, which saves the memset before the next step's sweep
+__global__ void __launch_bounds__(128) k_cell(Geo G, int cpb_shift, u64* __restrict__ sums, float* __restrict__ rec, int zero) {
   const int b0 = G.bs[0], b1 = G.bs[1], b2 = G.bs[2];
   const uint32_t bx = blockIdx.x >> cpb_shift, by = blockIdx.y, bz = blockIdx.z;
   const uint32_t local = ((blockIdx.x & ((1u << cpb_shift) - 1u)) << 7) | threadIdx.x;
   if (local >= (1u << (b0 + b1 + b2))) return;
   const uint32_t brick = (bz * (uint32_t)G.mb[1] + by) * (uint32_t)G.mb[0] + bx;
   const uint32_t k = (brick << (b0 + b1 + b2)) | local;
-  const u64* s = sums + (size_t)k * G.sw;
+  u64* s = sums + (size_t)k * G.sw;
   const u64 w0 = s[0];
   const uint32_t nreal = (uint32_t)(w0 & 0xffffull);
   if (nreal == 0u) return;
@@ -877,6 +899,7 @@ __global__ void __launch_bounds__(128) k_cell(Geo G, int cpb_shift, const u64* _
   int sx, sy, sz, r0i;
   unpack_ss(s[1], sx, sy);
   unpack_ss(s[2], sz, r0i);
+  if (zero) { s[0] = 0ull; s[1] = 0ull; s[2] = 0ull; }
   double S0 = (double)sx * G.fxv_inv, S1 = (double)sy * G.fxv_inv, S2 = (double)sz * G.fxv_inv;
   float4 r0, r1;
   if (G.collision == 1) {
@@ -1026,7 +1049,7 @@ struct mpc_ctx {
   unsigned long long seed;
   uint32_t t;
   size_t n, n_max;
-  bool bound, have_state, have_cells, have_order, compact, sticky, fast_brick, vec4;
+  bool bound, have_state, have_cells, have_order, compact, sticky, fast_brick, vec4, sums_clean;
   cudaStream_t stream;
   char* ws;
   size_t ws_bytes;
@@ -1232,7 +1255,8 @@ int steps_srd(mpc_ctx* c, int nsteps) {
     G.t = c->t;
     host_shift(c, c->t, G.s);
     const bool rebin = (c->t % (uint32_t)c->p.rebin_every) == 0u;
-    { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * G.sw * 8, c->stream)); }
+    if (!c->sums_clean) { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * G.sw * 8, c->stream)); }
+    c->sums_clean = false;
     if (n) {
       {
         FamilyTimer ft(c, F_SWEEP);
@@ -1243,8 +1267,12 @@ int steps_srd(mpc_ctx* c, int nsteps) {
       }
       if (rebin) { const int rc = do_reorder(c); if (rc) return rc; }
       FamilyTimer ft(c, F_CELL);
-      k_cell<<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec);
+      // all but the last step of the call: k_cell clears the sums it has read (the last step's stay for
+      // mpc_observables / mpc_get_cells)
+      const int zero = (k + 1 < nsteps) ? 1 : 0;
+      k_cell<<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec, zero);
       LAUNCH_CHECK("k_cell");
+      c->sums_clean = zero != 0;
     }
     sp[0] = G.s[0]; sp[1] = G.s[1]; sp[2] = G.s[2];
     c->t++;
@@ -1298,7 +1326,7 @@ int steps_generic(mpc_ctx* c, int nsteps) {
         FamilyTimer ft(c, F_CELL);
         if (plus_a && at) k_cell_a<true><<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec, c->nsing);
         else if (plus_a) k_cell_a<false><<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec, c->nsing);
-        else k_cell<<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec);
+        else k_cell<<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec, 0);
         LAUNCH_CHECK("k_cell");
       }
       FamilyTimer ft(c, F_COLLIDE);
@@ -1394,7 +1422,7 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   c->nbricks = (uint32_t)nbr;
   c->tile_bytes = tile_cells * TILE_W * 4;
   c->fast_brick = (G.bs[0] == 4 && G.bs[1] == 4 && G.bs[2] == 3);
-  { const char* e = getenv("MPC_SWEEP_VEC"); c->vec4 = !(e && e[0] == '1'); }
+  { const char* e = getenv("MPC_SWEEP_VEC"); c->vec4 = (e && e[0] == '4'); }
   {
     const int bvs = G.bs[0] + G.bs[1] + G.bs[2];
     c->cell_cpb_shift = bvs > 7 ? bvs - 7 : 0;
@@ -1445,7 +1473,7 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
   c->bsum = (uint32_t*)(c->ws + l.off_bsum);
   c->sums = (u64*)(c->ws + l.off_sums); c->rec = (float*)(c->ws + l.off_rec); c->obs = (double*)(c->ws + l.off_obs);
   c->nsing = (u64*)(c->ws + l.off_obs + OBS_HOST_DOUBLES * 8);
-  c->bound = true; c->have_state = false; c->have_cells = false; c->have_order = false; c->n = 0;
+  c->bound = true; c->have_state = false; c->have_cells = false; c->have_order = false; c->sums_clean = false; c->n = 0;
   if (c->tile_bytes > 48 * 1024) {
     cudaError_t e;
     if ((e = sweep_attr<false, false>(c->tile_bytes)) || (e = sweep_attr<false, true>(c->tile_bytes)) ||
