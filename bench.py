@@ -287,9 +287,9 @@ def main():
 def kernel_algorithmic_bytes(family, n, ncells, nbar):
     """Algorithmic bytes one launch of a kernel family must move."""
     per_particle = {"stream_key": 24 + 12 + 4, "accum": 12 + 4, "collide": 12 + 4 + 12, "gather": 4 + 32 + 32,
-                    "scatter_ids": 8 + 4, "rank": 8 + 4, "sweep": 48}.get(family, 0)
+                    "scatter_slots": 8 + 8, "rank": 12 + 4, "sweep": 48, "sweep_gather": 48 + 8 + 4}.get(family, 0)
     # sweep: the per-cell record is read once (32 B) and the cell sums written once (20 B of payload)
-    per_cell = {"accum": 20, "cell": 20 + 32, "collide": 32, "scan": 8, "memset": 24, "sweep": 20 + 20}.get(family, 0)
+    per_cell = {"accum": 20, "cell": 20 + 32, "collide": 32, "scan": 8, "memset": 24, "sweep": 20 + 20, "sweep_gather": 20 + 20}.get(family, 0)
     return float(per_particle) * n + float(per_cell) * ncells
 
 

@@ -7,7 +7,7 @@
 //                  PAPER.md:29-37,68,70,176
 //   k_cell         PROCESS_CELLS: v_cm, axis, kappa, virtual wall particles
 //   k_collide_pos  trailing collision of the last step of an mpc_step call       Eqs. (2),(5)
-//   k_scan_* / k_scatter_ids / k_rank / k_gather*   counting-sort reorder by (key, id)
+//   k_scan_* / k_scatter_slots / k_rank / k_gather*   counting-sort reorder by (key, id)
 //   k_stream_key / k_accum_at / k_collide_at        MPC-AT path (needs the rank of a particle in its
 //                  sorted cell segment, so it reorders every step and is not fused)
 //   k_obs_*        observables
@@ -60,6 +60,7 @@ struct Geo {
   float dt;
   float s[3];     // lattice shift of this step
   uint32_t k0, k1, t;
+  uint32_t rk[20];   // Philox round keys of (k0, k1), see philox_rk
   float cosa, sina;
   float kT, mass, sigma;   // sigma = sqrt(kT/m)
   // Fixed-point scales: powers of two relative to u = 2^round(log2 sigma), so precision does not
@@ -224,11 +225,20 @@ __device__ __forceinline__ int fold(int k, int m) {
   return k;
 }
 
-template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS>
+// GATHER: the reorder's gather is folded into this pass. Particle i of the NEW order is read from
+// src.p[..][perm[i]] (the old arrays) and written to x..vz[i] (the other buffer), its id is copied along.
+struct GatherSrc {
+  const float* p[6];
+  const uint32_t* id;
+  uint32_t* id_out;
+  const uint32_t* perm;
+};
+template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS, bool GATHER = false>
 __global__ void __launch_bounds__(SWEEP_T, 2)
 k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
         float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, uint32_t* __restrict__ key_out,
-        const uint32_t* __restrict__ chunk, uint32_t nbricks, const float* __restrict__ rec, u64* __restrict__ sums) {
+        const uint32_t* __restrict__ chunk, uint32_t nbricks, const float* __restrict__ rec, u64* __restrict__ sums,
+        GatherSrc gs) {
   extern __shared__ int tile[];
   const int T0 = (1 << BS::s0(G)) + 2 * HALO, T1 = (1 << BS::s1(G)) + 2 * HALO, T2 = (1 << BS::s2(G)) + 2 * HALO;
   const int tcells = T0 * T1 * T2;
@@ -259,12 +269,36 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
   // software pipeline: the loads of the next particle are in flight while this one is processed
   uint32_t i = i0 + threadIdx.x;
   float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f, p4 = 0.f, p5 = 0.f;
-  if (i < i1) { p0 = x[i]; p1 = y[i]; p2 = z[i]; p3 = vx[i]; p4 = vy[i]; p5 = vz[i]; }
+  // GATHER: id of the particle in flight; source indices of the particles 1, 2 and 3 iterations ahead (the
+  // first feeds the register prefetch, the second an L2 prefetch of its seven lines, the third is in flight)
+  uint32_t pid = 0, jn = 0, jn2 = 0, jn3 = 0;
+  if (GATHER) {
+    if (i < i1) {
+      const uint32_t j = gs.perm[i];
+      p0 = gs.p[0][j]; p1 = gs.p[1][j]; p2 = gs.p[2][j]; p3 = gs.p[3][j]; p4 = gs.p[4][j]; p5 = gs.p[5][j]; pid = gs.id[j];
+    }
+    if (i + SWEEP_T < i1) jn = gs.perm[i + SWEEP_T];
+    if (i + 2 * SWEEP_T < i1) jn2 = gs.perm[i + 2 * SWEEP_T];
+    if (i + 3 * SWEEP_T < i1) jn3 = gs.perm[i + 3 * SWEEP_T];
+  } else if (i < i1) { p0 = x[i]; p1 = y[i]; p2 = z[i]; p3 = vx[i]; p4 = vy[i]; p5 = vz[i]; }
   for (; i < i1; i += SWEEP_T) {
     float r[3] = {p0, p1, p2}, v[3] = {p3, p4, p5};
     const uint32_t inext = i + SWEEP_T;
-    if (inext < i1) { p0 = x[inext]; p1 = y[inext]; p2 = z[inext]; p3 = vx[inext]; p4 = vy[inext]; p5 = vz[inext]; }
-    {   // pull the lines of a later iteration into L2: the register prefetch above then pays L2, not DRAM, latency
+    if (GATHER) {
+      gs.id_out[i] = pid;
+      if (inext < i1) {
+        const uint32_t j = jn;
+        p0 = gs.p[0][j]; p1 = gs.p[1][j]; p2 = gs.p[2][j]; p3 = gs.p[3][j]; p4 = gs.p[4][j]; p5 = gs.p[5][j]; pid = gs.id[j];
+        jn = jn2; jn2 = jn3;
+        if (i + 2 * SWEEP_T < i1) {
+#pragma unroll
+          for (int a = 0; a < 6; ++a) asm volatile("prefetch.global.L2 [%0];" ::"l"(gs.p[a] + jn));
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(gs.id + jn));
+        }
+        if (i + 4 * SWEEP_T < i1) jn3 = gs.perm[i + 4 * SWEEP_T];
+      }
+    } else if (inext < i1) { p0 = x[inext]; p1 = y[inext]; p2 = z[inext]; p3 = vx[inext]; p4 = vy[inext]; p5 = vz[inext]; }
+    if (!GATHER) {   // pull the lines of a later iteration into L2: the register prefetch above then pays L2, not DRAM, latency
       const uint32_t ifar = i + PF_DIST * SWEEP_T;
       if (ifar < i1) {
         asm volatile("prefetch.global.L2 [%0];" ::"l"(x + ifar));
@@ -797,26 +831,37 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const uint32_t* __restric
 }
 
 // ---- reorder by (key, id) -----------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_scatter_ids(size_t n, const uint32_t* __restrict__ key, const uint32_t* __restrict__ id,
-                                                     const uint32_t* __restrict__ offset, uint32_t* __restrict__ cursor,
-                                                     uint32_t* __restrict__ slot_id) {
+// Step 1: every particle takes a slot of its cell segment in arrival order. Particles of one cell are
+// mostly lane neighbours (the array is still nearly sorted), so the lanes of a warp with the same key
+// share ONE cursor atomic (match.any + leader), which is what bounds this kernel otherwise.
+__global__ void __launch_bounds__(256) k_scatter_slots(size_t n, const uint32_t* __restrict__ key, const uint32_t* __restrict__ id,
+                                                       const uint32_t* __restrict__ offset, uint32_t* __restrict__ cursor,
+                                                       uint2* __restrict__ slot) {
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const uint32_t k = key[i];
-  const uint32_t s = offset[k] + atomicAdd(&cursor[k], 1u);
-  slot_id[s] = id[i];
+  const unsigned lane = threadIdx.x & 31u;
+  const unsigned grp = __match_any_sync(__activemask(), k);
+  const int leader = __ffs(grp) - 1;
+  uint32_t base = 0;
+  if ((int)lane == leader) base = atomicAdd(&cursor[k], (uint32_t)__popc(grp));
+  base = __shfl_sync(grp, base, leader);
+  const uint32_t s = offset[k] + base + (uint32_t)__popc(grp & ((1u << lane) - 1u));
+  slot[s] = make_uint2(id[i], (uint32_t)i);   // one 8-byte store: (id, source index)
 }
-// rank of a particle inside its cell = number of cell mates with a smaller id (U4)
-__global__ void __launch_bounds__(256) k_rank(size_t n, const uint32_t* __restrict__ key, const uint32_t* __restrict__ id,
-                                              const uint32_t* __restrict__ offset, const uint32_t* __restrict__ slot_id,
-                                              uint32_t* __restrict__ perm) {
-  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const uint32_t k = key[i], me = id[i];
+// Step 2, one thread per slot: rank of the slot's particle inside its cell = number of cell mates with a
+// smaller id (U4); perm[first slot of the cell + rank] = source index. Reads and writes of a
+// warp stay inside the few segments its 32 consecutive slots belong to.
+__global__ void __launch_bounds__(256) k_rank(size_t n, const uint32_t* __restrict__ key, const uint32_t* __restrict__ offset,
+                                              const uint2* __restrict__ slot, uint32_t* __restrict__ perm) {
+  const size_t s = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  const uint2 me = slot[s];
+  const uint32_t k = key[me.y];
   const uint32_t b = offset[k], e = offset[k + 1];
   uint32_t r = 0;
-  for (uint32_t j = b; j < e; ++j) r += (slot_id[j] < me) ? 1u : 0u;
-  perm[b + r] = (uint32_t)i;
+  for (uint32_t j = b; j < e; ++j) r += (slot[j].x < me.x) ? 1u : 0u;
+  perm[b + r] = me.y;
 }
 struct Arrays8 { void* p[8]; };
 template <int NA>
@@ -844,27 +889,29 @@ __device__ __forceinline__ void renorm(float& p, int& ex) {   // p = m * 2^e wit
   ex += (bits >> 23) - 126;
   p = __int_as_float((bits & 0x007fffff) | 0x3f000000);
 }
+// 2^24 * u01_oc(w): the power-of-two scale of every uniform is banked in the exponent instead (exact)
+__device__ __forceinline__ float u24_oc(uint32_t w) { return (float)((w >> 8) + 1u); }
 __device__ float mbs_energy(const Geo& G, uint32_t cid, uint32_t Nc) {
   const uint32_t f = 3u * (Nc - 1u), M = f >> 1, odd = f & 1u;
   const uint32_t full = M >> 2;                  // blocks whose four uniforms all enter the product
   float p = 1.0f;
-  int ex = 0;
+  int ex = -24 * (int)M;                         // M uniforms enter the product, each carried as 2^24 u
   uint32_t sub = 0;
   for (; sub < full; ++sub) {
-    const Block4 o = philox(cid, sub, G.t, TAG_MBS, G.k0, G.k1);
-    p *= (u01_oc(o.a) * u01_oc(o.b)) * (u01_oc(o.c) * u01_oc(o.d));   // >= 2^-96: cannot underflow
+    const Block4 o = philox_rk(cid, sub, G.t, TAG_MBS, G.rk);
+    p *= (u24_oc(o.a) * u24_oc(o.b)) * (u24_oc(o.c) * u24_oc(o.d));   // < 2^96: cannot overflow
     renorm(p, ex);
   }
   // tail: positions 4*full .. M-1 still enter the product, M and M+1 feed the half squared normal
   float um = 1.0f, ua = 0.0f;
   const uint32_t need = M + 2u * odd;
   for (uint32_t base = full << 2; base < need; base += 4, ++sub) {
-    const Block4 o = philox(cid, sub, G.t, TAG_MBS, G.k0, G.k1);
+    const Block4 o = philox_rk(cid, sub, G.t, TAG_MBS, G.rk);
     const uint32_t w[4] = {o.a, o.b, o.c, o.d};
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const uint32_t pos = base + q;
-      p *= (pos < M) ? u01_oc(w[q]) : 1.0f;
+      p *= (pos < M) ? u24_oc(w[q]) : 1.0f;
       um = (pos == M) ? u01_oc(w[q]) : um;
       ua = (pos == M + 1u) ? u01_co(w[q]) : ua;
     }
@@ -924,7 +971,7 @@ __global__ void __launch_bounds__(128) k_cell(Geo G, int cpb_shift, u64* __restr
       if (cut && (int)nreal < G.nbar) {
         const uint32_t nv = (uint32_t)G.nbar - nreal;
         for (uint32_t j = 0; j < nv; ++j) {
-          const Block4 o = philox(cid, j, G.t, TAG_WALL, G.k0, G.k1);
+          const Block4 o = philox_rk(cid, j, G.t, TAG_WALL, G.rk);
           float g0, g1, g2;
           normals3(o, g0, g1, g2);
           const double a = (double)(G.sigma * g0), b = (double)(G.sigma * g1), c = (double)(G.sigma * g2);
@@ -944,7 +991,7 @@ __global__ void __launch_bounds__(128) k_cell(Geo G, int cpb_shift, u64* __restr
       }
     }
     r0.w = kappa;
-    const Block4 o = philox(cid, 0u, G.t, TAG_AXIS, G.k0, G.k1);
+    const Block4 o = philox_rk(cid, 0u, G.t, TAG_AXIS, G.rk);
     const float zz = 2.0f * u01_co(o.a) - 1.0f;
     const float rr = sqrtf((1.0f - zz) * (1.0f + zz));
     float sp, cp;
@@ -1038,9 +1085,9 @@ __global__ void __launch_bounds__(256) k_export_cells(Geo G, const u64* __restri
 // =================================================================================================
 using namespace mpc;
 
-enum Family { F_SWEEP = 0, F_CELL, F_COLLIDE, F_SCAN, F_SCATTER, F_RANK, F_GATHER, F_MEMSET, F_STREAM, F_ACCUM, F_OBS, F_COUNT };
-static const char* const FAMILY_NAMES[F_COUNT] = {"sweep", "cell", "collide", "scan", "scatter_ids", "rank", "gather", "memset",
-                                                  "stream_key", "accum", "observables"};
+enum Family { F_SWEEP = 0, F_CELL, F_COLLIDE, F_SCAN, F_SCATTER, F_RANK, F_GATHER, F_MEMSET, F_STREAM, F_ACCUM, F_OBS, F_SWEEPG, F_COUNT };
+static const char* const FAMILY_NAMES[F_COUNT] = {"sweep", "cell", "collide", "scan", "scatter_slots", "rank", "gather", "memset",
+                                                  "stream_key", "accum", "observables", "sweep_gather"};
 constexpr int PROF_MAX_PAIRS = 16384;
 
 struct mpc_ctx {
@@ -1049,7 +1096,7 @@ struct mpc_ctx {
   unsigned long long seed;
   uint32_t t;
   size_t n, n_max;
-  bool bound, have_state, have_cells, have_order, compact, sticky, fast_brick, vec4, sums_clean;
+  bool bound, have_state, have_cells, have_order, compact, sticky, fast_brick, vec4, sums_clean, gather_pending, no_fuse_gather;
   cudaStream_t stream;
   char* ws;
   size_t ws_bytes;
@@ -1088,12 +1135,14 @@ Layout make_layout(size_t n_max, size_t nkeys, int sw, int rw, bool compact) {
   Layout l;
   size_t o = 0;
   auto take = [&](size_t bytes) { const size_t r = o; o = align_up(o + bytes, 256); return r; };
-  const size_t pn = (n_max ? n_max : 1) * 4;
+  const size_t pn = align_up((n_max ? n_max : 1) * 4, 256);   // whole 256-byte units: consecutive arrays are contiguous
   for (int a = 0; a < 7; ++a) l.off_A[a] = take(pn);
   if (compact) { l.off_B[0] = take(pn); for (int a = 1; a < 7; ++a) l.off_B[a] = l.off_B[0]; }
   else for (int a = 0; a < 7; ++a) l.off_B[a] = take(pn);
   l.off_key = take(pn);
-  l.off_slot = take(pn);
+  // (id, source index) per slot: 8 bytes; with the second copy present the slots live in its first two arrays
+  // (contiguous, unused until the gather) and this array only receives the sorted keys of the unfused path
+  l.off_slot = take(compact ? pn * 2 : pn);
   l.off_perm = take(pn);
   l.off_cursor = take(nkeys * 4);
   l.off_offset = take((nkeys + 1) * 4);
@@ -1149,7 +1198,8 @@ void host_shift(const mpc_ctx* c, uint32_t t, float s[3]) {
 }
 
 // counting-sort reorder by (key, id); counts = low word of word 0 of the sums; c->key holds the keys
-int do_reorder(mpc_ctx* c) {
+// defer_gather: leave the permutation in c->perm for the next sweep to apply (launch_sweep<.., GATHER>)
+int do_reorder(mpc_ctx* c, bool defer_gather = false) {
   const size_t n = c->n, nk = c->G.nkeys, nb = (nk + SCAN_TILE - 1) / SCAN_TILE;
   const uint32_t* cnt = reinterpret_cast<const uint32_t*>(c->sums);
   const int stride = c->G.sw * 2;
@@ -1163,16 +1213,19 @@ int do_reorder(mpc_ctx* c) {
     LAUNCH_CHECK("k_scan_apply");
   }
   { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->cursor, 0, nk * 4, c->stream)); }
+  uint2* slot2 = reinterpret_cast<uint2*>(c->compact ? c->slot_id : c->Bf[0]);
   {
     FamilyTimer ft(c, F_SCATTER);
-    k_scatter_ids<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->key, c->A[6], c->offset, c->cursor, c->slot_id);
-    LAUNCH_CHECK("k_scatter_ids");
+    k_scatter_slots<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->key, c->A[6], c->offset, c->cursor, slot2);
+    LAUNCH_CHECK("k_scatter_slots");
   }
   {
     FamilyTimer ft(c, F_RANK);
-    k_rank<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->key, c->A[6], c->offset, c->slot_id, c->perm);
+    k_rank<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->key, c->offset, slot2, c->perm);
     LAUNCH_CHECK("k_rank");
   }
+  c->have_order = true;
+  if (defer_gather) { c->gather_pending = true; return MPC_OK; }
   FamilyTimer ftg(c, F_GATHER);
   const bool need_key = c->G.generic != 0;     // the unfused path reads the sorted keys afterwards
   if (!c->compact) {
@@ -1183,7 +1236,7 @@ int do_reorder(mpc_ctx* c) {
     else k_gather<7><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
     LAUNCH_CHECK("k_gather");
     for (int a = 0; a < 7; ++a) { uint32_t* t = c->A[a]; c->A[a] = c->Bf[a]; c->Bf[a] = t; }
-    if (need_key) { uint32_t* t = c->key; c->key = c->slot_id; c->slot_id = t; }
+    if (need_key) CU(cudaMemcpyAsync(c->key, c->slot_id, n * 4, cudaMemcpyDeviceToDevice, c->stream));   // the slot array is larger: no pointer swap
   } else {
     // property-wise through one temporary array
     Arrays8 src, dst;
@@ -1202,30 +1255,38 @@ int do_reorder(mpc_ctx* c) {
 typedef BrickShape<-1, -1, -1> BSgeneric;
 typedef BrickShape<4, 4, 3> BSfast;   // {16,16,8}
 
-template <bool COLLIDE, bool WKEY, class BS>
+// GATHER: read the particles through c->perm from the current arrays, write the other buffer, then swap
+template <bool COLLIDE, bool WKEY, class BS, bool GATHER>
 int launch_sweep_bs(mpc_ctx* c, const float sp[3]) {
   const Geo& G = c->G;
-  float** F = reinterpret_cast<float**>(c->A);
+  float** F = reinterpret_cast<float**>(GATHER ? c->Bf : c->A);
+  GatherSrc gs;
+  for (int a = 0; a < 6; ++a) gs.p[a] = reinterpret_cast<const float*>(c->A[a]);
+  gs.id = c->A[6]; gs.id_out = c->Bf[6]; gs.perm = c->perm;
   const uint32_t* chunk = c->have_order ? c->offset : nullptr;
   const bool wall = G.wall >= 0, grav = (G.g[0] != 0.f || G.g[1] != 0.f || G.g[2] != 0.f);
 #define SWEEP_ARGS G, sp[0], sp[1], sp[2], (uint32_t)c->n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, chunk, c->nbricks, c->rec, c->sums
-  if (c->vec4) {
+  if (c->vec4 && !GATHER) {
     if (wall && grav) k_sweep4<COLLIDE, true, true, WKEY, BS><<<c->nbricks, SWEEP4_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
     else if (wall) k_sweep4<COLLIDE, true, false, WKEY, BS><<<c->nbricks, SWEEP4_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
     else if (grav) k_sweep4<COLLIDE, false, true, WKEY, BS><<<c->nbricks, SWEEP4_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
     else k_sweep4<COLLIDE, false, false, WKEY, BS><<<c->nbricks, SWEEP4_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
   } else
-  if (wall && grav) k_sweep<COLLIDE, true, true, WKEY, BS><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
-  else if (wall) k_sweep<COLLIDE, true, false, WKEY, BS><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
-  else if (grav) k_sweep<COLLIDE, false, true, WKEY, BS><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
-  else k_sweep<COLLIDE, false, false, WKEY, BS><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
+  if (wall && grav) k_sweep<COLLIDE, true, true, WKEY, BS, GATHER><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, gs);
+  else if (wall) k_sweep<COLLIDE, true, false, WKEY, BS, GATHER><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, gs);
+  else if (grav) k_sweep<COLLIDE, false, true, WKEY, BS, GATHER><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, gs);
+  else k_sweep<COLLIDE, false, false, WKEY, BS, GATHER><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, gs);
 #undef SWEEP_ARGS
   LAUNCH_CHECK("k_sweep");
+  if (GATHER) {
+    for (int a = 0; a < 7; ++a) { uint32_t* t = c->A[a]; c->A[a] = c->Bf[a]; c->Bf[a] = t; }
+    c->gather_pending = false;
+  }
   return MPC_OK;
 }
-template <bool COLLIDE, bool WKEY>
+template <bool COLLIDE, bool WKEY, bool GATHER = false>
 int launch_sweep(mpc_ctx* c, const float sp[3]) {
-  return c->fast_brick ? launch_sweep_bs<COLLIDE, WKEY, BSfast>(c, sp) : launch_sweep_bs<COLLIDE, WKEY, BSgeneric>(c, sp);
+  return c->fast_brick ? launch_sweep_bs<COLLIDE, WKEY, BSfast, GATHER>(c, sp) : launch_sweep_bs<COLLIDE, WKEY, BSgeneric, GATHER>(c, sp);
 }
 
 template <bool COLLIDE, bool WKEY, class BS>
@@ -1235,6 +1296,12 @@ cudaError_t sweep_attr_bs(size_t bytes) {
   if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, false, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
   if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, true, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
   if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, false, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+  if (COLLIDE) {
+    if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, true, WKEY, BS, COLLIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+    if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, false, WKEY, BS, COLLIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+    if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, true, WKEY, BS, COLLIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+    if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, false, WKEY, BS, COLLIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+  }
   if ((e = cudaFuncSetAttribute(k_sweep4<COLLIDE, true, true, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
   if ((e = cudaFuncSetAttribute(k_sweep4<COLLIDE, true, false, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
   if ((e = cudaFuncSetAttribute(k_sweep4<COLLIDE, false, true, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
@@ -1259,13 +1326,15 @@ int steps_srd(mpc_ctx* c, int nsteps) {
     c->sums_clean = false;
     if (n) {
       {
-        FamilyTimer ft(c, F_SWEEP);
+        FamilyTimer ft(c, c->gather_pending ? F_SWEEPG : F_SWEEP);
         int rc;
         if (k == 0) rc = rebin ? launch_sweep<false, true>(c, sp) : launch_sweep<false, false>(c, sp);
+        else if (c->gather_pending) rc = rebin ? launch_sweep<true, true, true>(c, sp) : launch_sweep<true, false, true>(c, sp);
         else rc = rebin ? launch_sweep<true, true>(c, sp) : launch_sweep<true, false>(c, sp);
         if (rc) return rc;
       }
-      if (rebin) { const int rc = do_reorder(c); if (rc) return rc; }
+      // the gather of a reorder is folded into the next step's sweep when there is one in this call
+      if (rebin) { const int rc = do_reorder(c, !c->compact && !c->no_fuse_gather && k + 1 < nsteps); if (rc) return rc; }
       FamilyTimer ft(c, F_CELL);
       // all but the last step of the call: k_cell clears the sums it has read (the last step's stay for
       // mpc_observables / mpc_get_cells)
@@ -1354,7 +1423,7 @@ int set_state_impl(mpc_ctx* c, unsigned long long n, const float* const src[6], 
     if (id) CU(cudaMemcpyAsync(c->A[6], id, n * 4, kind, c->stream));
     else { k_iota<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->A[6]); LAUNCH_CHECK("k_iota"); }
   }
-  c->n = n; c->t = step; c->have_state = true; c->have_cells = false; c->have_order = false;
+  c->n = n; c->t = step; c->have_state = true; c->have_cells = false; c->have_order = false; c->gather_pending = false;
   return MPC_OK;
 }
 int get_state_impl(mpc_ctx* c, float* const dst[6], unsigned* id, cudaMemcpyKind kind) {
@@ -1423,6 +1492,7 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   c->tile_bytes = tile_cells * TILE_W * 4;
   c->fast_brick = (G.bs[0] == 4 && G.bs[1] == 4 && G.bs[2] == 3);
   { const char* e = getenv("MPC_SWEEP_VEC"); c->vec4 = (e && e[0] == '4'); }
+  { const char* e = getenv("MPC_NO_FUSE_GATHER"); c->no_fuse_gather = (e && e[0] == '1'); }
   {
     const int bvs = G.bs[0] + G.bs[1] + G.bs[2];
     c->cell_cpb_shift = bvs > 7 ? bvs - 7 : 0;
@@ -1433,6 +1503,7 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   G.sigma = (float)sqrt((double)p->kT / (double)p->mass);
   G.cosa = (float)cos((double)p->alpha); G.sina = (float)sin((double)p->alpha);
   G.k0 = (uint32_t)(seed & 0xffffffffull); G.k1 = (uint32_t)(seed >> 32);
+  philox_round_keys(G.k0, G.k1, G.rk);
   G.nbar = (int)lround((double)n_per_cell);
   const int ue = (int)lround(log2((double)G.sigma));        // thermal velocity rounded to a power of two
   G.fxv = (float)ldexp(1.0, 22 - ue); G.fxv_inv = ldexp(1.0, ue - 22);
@@ -1473,7 +1544,7 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
   c->bsum = (uint32_t*)(c->ws + l.off_bsum);
   c->sums = (u64*)(c->ws + l.off_sums); c->rec = (float*)(c->ws + l.off_rec); c->obs = (double*)(c->ws + l.off_obs);
   c->nsing = (u64*)(c->ws + l.off_obs + OBS_HOST_DOUBLES * 8);
-  c->bound = true; c->have_state = false; c->have_cells = false; c->have_order = false; c->sums_clean = false; c->n = 0;
+  c->bound = true; c->have_state = false; c->have_cells = false; c->have_order = false; c->sums_clean = false; c->gather_pending = false; c->n = 0;
   if (c->tile_bytes > 48 * 1024) {
     cudaError_t e;
     if ((e = sweep_attr<false, false>(c->tile_bytes)) || (e = sweep_attr<false, true>(c->tile_bytes)) ||
