@@ -225,20 +225,33 @@ __device__ __forceinline__ int fold(int k, int m) {
   return k;
 }
 
-// GATHER: the reorder's gather is folded into this pass. Particle i of the NEW order is read from
-// src.p[..][perm[i]] (the old arrays) and written to x..vz[i] (the other buffer), its id is copied along.
-struct GatherSrc {
-  const float* p[6];
-  const uint32_t* id;
-  uint32_t* id_out;
-  const uint32_t* perm;
+// Reorder folded into two consecutive sweeps (IO = 1 on the reorder step, IO = 2 on the step after it):
+//   IO_AOS_OUT  the pass writes every particle as ONE 32-byte record {r, v, id, 0} into a staging buffer
+//               instead of updating the SoA arrays in place;
+//   IO_GATHER   particle i of the new order is read with one 256-bit load from staging[perm[i]] (a whole
+//               sector, every byte used) and written to the SoA arrays at i.
+// A gather of the SoA arrays themselves costs ~4.5 sectors of L2 traffic per useful one (measured).
+enum { IO_PLAIN = 0, IO_AOS_OUT = 1, IO_GATHER = 2 };
+struct SweepIO {
+  const float* aos_in;      // IO_GATHER: staging records in the old order
+  float* aos_out;           // IO_AOS_OUT
+  const uint32_t* perm;     // IO_GATHER
+  uint32_t* id;             // IO_AOS_OUT: read at i; IO_GATHER: written at i
 };
-template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS, bool GATHER = false>
+__device__ __forceinline__ void ld256(const float* p, float (&a)[8]) {
+  asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=f"(a[0]), "=f"(a[1]), "=f"(a[2]), "=f"(a[3]), "=f"(a[4]), "=f"(a[5]), "=f"(a[6]), "=f"(a[7]) : "l"(p));
+}
+__device__ __forceinline__ void st256(float* p, const float (&a)[8]) {
+  asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+               :: "l"(p), "f"(a[0]), "f"(a[1]), "f"(a[2]), "f"(a[3]), "f"(a[4]), "f"(a[5]), "f"(a[6]), "f"(a[7]) : "memory");
+}
+template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS, int IO = IO_PLAIN>
 __global__ void __launch_bounds__(SWEEP_T, 2)
 k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
         float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, uint32_t* __restrict__ key_out,
         const uint32_t* __restrict__ chunk, uint32_t nbricks, const float* __restrict__ rec, u64* __restrict__ sums,
-        GatherSrc gs) {
+        SweepIO io) {
   extern __shared__ int tile[];
   const int T0 = (1 << BS::s0(G)) + 2 * HALO, T1 = (1 << BS::s1(G)) + 2 * HALO, T2 = (1 << BS::s2(G)) + 2 * HALO;
   const int tcells = T0 * T1 * T2;
@@ -269,36 +282,42 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
   // software pipeline: the loads of the next particle are in flight while this one is processed
   uint32_t i = i0 + threadIdx.x;
   float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f, p4 = 0.f, p5 = 0.f;
-  // GATHER: id of the particle in flight; source indices of the particles 1, 2 and 3 iterations ahead (the
-  // first feeds the register prefetch, the second an L2 prefetch of its seven lines, the third is in flight)
-  uint32_t pid = 0, jn = 0, jn2 = 0, jn3 = 0;
-  if (GATHER) {
+  // IO_GATHER: source indices of the particles 1, 2 and 3 iterations ahead (the first feeds the register
+  // prefetch, the second an L2 prefetch of its record, the third is in flight); pid = id of the particle in flight
+  float pid = 0.f;
+  uint32_t jn = 0, jn2 = 0, jn3 = 0;
+  if (IO == IO_GATHER) {
     if (i < i1) {
-      const uint32_t j = gs.perm[i];
-      p0 = gs.p[0][j]; p1 = gs.p[1][j]; p2 = gs.p[2][j]; p3 = gs.p[3][j]; p4 = gs.p[4][j]; p5 = gs.p[5][j]; pid = gs.id[j];
+      float q[8];
+      ld256(io.aos_in + (size_t)io.perm[i] * 8, q);
+      p0 = q[0]; p1 = q[1]; p2 = q[2]; p3 = q[3]; p4 = q[4]; p5 = q[5]; pid = q[6];
     }
-    if (i + SWEEP_T < i1) jn = gs.perm[i + SWEEP_T];
-    if (i + 2 * SWEEP_T < i1) jn2 = gs.perm[i + 2 * SWEEP_T];
-    if (i + 3 * SWEEP_T < i1) jn3 = gs.perm[i + 3 * SWEEP_T];
-  } else if (i < i1) { p0 = x[i]; p1 = y[i]; p2 = z[i]; p3 = vx[i]; p4 = vy[i]; p5 = vz[i]; }
+    if (i + SWEEP_T < i1) jn = io.perm[i + SWEEP_T];
+    if (i + 2 * SWEEP_T < i1) jn2 = io.perm[i + 2 * SWEEP_T];
+    if (i + 3 * SWEEP_T < i1) jn3 = io.perm[i + 3 * SWEEP_T];
+  } else if (i < i1) {
+    p0 = x[i]; p1 = y[i]; p2 = z[i]; p3 = vx[i]; p4 = vy[i]; p5 = vz[i];
+    if (IO == IO_AOS_OUT) pid = __uint_as_float(io.id[i]);
+  }
   for (; i < i1; i += SWEEP_T) {
     float r[3] = {p0, p1, p2}, v[3] = {p3, p4, p5};
+    const float idbits = pid;
     const uint32_t inext = i + SWEEP_T;
-    if (GATHER) {
-      gs.id_out[i] = pid;
+    if (IO == IO_GATHER) {
+      io.id[i] = __float_as_uint(idbits);
       if (inext < i1) {
-        const uint32_t j = jn;
-        p0 = gs.p[0][j]; p1 = gs.p[1][j]; p2 = gs.p[2][j]; p3 = gs.p[3][j]; p4 = gs.p[4][j]; p5 = gs.p[5][j]; pid = gs.id[j];
+        float q[8];
+        ld256(io.aos_in + (size_t)jn * 8, q);
+        p0 = q[0]; p1 = q[1]; p2 = q[2]; p3 = q[3]; p4 = q[4]; p5 = q[5]; pid = q[6];
         jn = jn2; jn2 = jn3;
-        if (i + 2 * SWEEP_T < i1) {
-#pragma unroll
-          for (int a = 0; a < 6; ++a) asm volatile("prefetch.global.L2 [%0];" ::"l"(gs.p[a] + jn));
-          asm volatile("prefetch.global.L2 [%0];" ::"l"(gs.id + jn));
-        }
-        if (i + 4 * SWEEP_T < i1) jn3 = gs.perm[i + 4 * SWEEP_T];
+        if (i + 2 * SWEEP_T < i1) asm volatile("prefetch.global.L2 [%0];" ::"l"(io.aos_in + (size_t)jn * 8));
+        if (i + 4 * SWEEP_T < i1) jn3 = io.perm[i + 4 * SWEEP_T];
       }
-    } else if (inext < i1) { p0 = x[inext]; p1 = y[inext]; p2 = z[inext]; p3 = vx[inext]; p4 = vy[inext]; p5 = vz[inext]; }
-    if (!GATHER) {   // pull the lines of a later iteration into L2: the register prefetch above then pays L2, not DRAM, latency
+    } else if (inext < i1) {
+      p0 = x[inext]; p1 = y[inext]; p2 = z[inext]; p3 = vx[inext]; p4 = vy[inext]; p5 = vz[inext];
+      if (IO == IO_AOS_OUT) pid = __uint_as_float(io.id[inext]);
+    }
+    if (IO != IO_GATHER) {   // pull the lines of a later iteration into L2: the register prefetch above then pays L2, not DRAM, latency
       const uint32_t ifar = i + PF_DIST * SWEEP_T;
       if (ifar < i1) {
         asm volatile("prefetch.global.L2 [%0];" ::"l"(x + ifar));
@@ -320,8 +339,13 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       srd_apply(G, r0, ax, v);
     }
     stream_one<WALL, GRAV>(G, r, v);
-    x[i] = r[0]; y[i] = r[1]; z[i] = r[2];
-    vx[i] = v[0]; vy[i] = v[1]; vz[i] = v[2];
+    if (IO == IO_AOS_OUT) {
+      const float q[8] = {r[0], r[1], r[2], v[0], v[1], v[2], idbits, 0.f};
+      st256(io.aos_out + (size_t)i * 8, q);
+    } else {
+      x[i] = r[0]; y[i] = r[1]; z[i] = r[2];
+      vx[i] = v[0]; vy[i] = v[1]; vz[i] = v[2];
+    }
     int cx = cell_raw(G, r[0], G.s[0]) + w0, cy = cell_raw(G, r[1], G.s[1]) + w1, cz = cell_raw(G, r[2], G.s[2]) + w2;
     if (WALL) { if (G.bc[0]) cx = max(0, min(cx, m0 - 1)); if (G.bc[1]) cy = max(0, min(cy, m1 - 1)); if (G.bc[2]) cz = max(0, min(cz, m2 - 1)); }
     const int a0 = __float2int_rn(v[0] * G.fxv), a1 = __float2int_rn(v[1] * G.fxv), a2 = __float2int_rn(v[2] * G.fxv);
@@ -831,6 +855,23 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const uint32_t* __restric
 }
 
 // ---- reorder by (key, id) -----------------------------------------------------------------------
+// Lanes of a warp that hold the same key as their neighbours form runs (the array is still nearly sorted):
+// one cursor atomic per run. Returns the first slot of this lane within its cell segment's arrival order.
+// (match.any would also merge non-adjacent lanes but runs at a fraction of the rate: measured 72 % pipe busy.)
+__device__ __forceinline__ uint32_t run_slot(uint32_t k, uint32_t* __restrict__ cursor) {
+  const unsigned lane = threadIdx.x & 31u;
+  const unsigned act = __activemask();                      // a prefix of the warp (i < n)
+  const uint32_t kprev = __shfl_up_sync(act, k, 1);
+  const unsigned heads = __ballot_sync(act, lane == 0u || kprev != k);
+  const unsigned le = 0xffffffffu >> (31u - lane);          // lanes <= lane
+  const int leader = 31 - __clz((int)(heads & le));
+  const unsigned above = heads & ~le;
+  const int end = above ? (__ffs((int)above) - 1) : __popc(act);
+  uint32_t base = 0;
+  if ((int)lane == leader) base = atomicAdd(&cursor[k], (uint32_t)(end - leader));
+  base = __shfl_sync(act, base, leader);
+  return base + (lane - (unsigned)leader);
+}
 // Step 1: every particle takes a slot of its cell segment in arrival order. Particles of one cell are
 // mostly lane neighbours (the array is still nearly sorted), so the lanes of a warp with the same key
 // share ONE cursor atomic (match.any + leader), which is what bounds this kernel otherwise.
@@ -840,13 +881,7 @@ __global__ void __launch_bounds__(256) k_scatter_slots(size_t n, const uint32_t*
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const uint32_t k = key[i];
-  const unsigned lane = threadIdx.x & 31u;
-  const unsigned grp = __match_any_sync(__activemask(), k);
-  const int leader = __ffs(grp) - 1;
-  uint32_t base = 0;
-  if ((int)lane == leader) base = atomicAdd(&cursor[k], (uint32_t)__popc(grp));
-  base = __shfl_sync(grp, base, leader);
-  const uint32_t s = offset[k] + base + (uint32_t)__popc(grp & ((1u << lane) - 1u));
+  const uint32_t s = offset[k] + run_slot(k, cursor);
   slot[s] = make_uint2(id[i], (uint32_t)i);   // one 8-byte store: (id, source index)
 }
 // Step 2, one thread per slot: rank of the slot's particle inside its cell = number of cell mates with a
@@ -862,6 +897,29 @@ __global__ void __launch_bounds__(256) k_rank(size_t n, const uint32_t* __restri
   uint32_t r = 0;
   for (uint32_t j = b; j < e; ++j) r += (slot[j].x < me.x) ? 1u : 0u;
   perm[b + r] = me.y;
+}
+// Hot-path variant (SRD): the order inside a cell does not enter the physics (integer cell sums), so the
+// reorder only groups the particles by key: perm[slot] = source index, slots in arrival order. The canonical
+// (key, id) order is restored by k_rank_cells + gather before the state is read (canonicalise()).
+__global__ void __launch_bounds__(256) k_scatter_src(size_t n, const uint32_t* __restrict__ key, const uint32_t* __restrict__ offset,
+                                                     uint32_t* __restrict__ cursor, uint32_t* __restrict__ perm) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t k = key[i];
+  perm[offset[k] + run_slot(k, cursor)] = (uint32_t)i;
+}
+// one thread per cell: the particles of segment [offset[k], offset[k+1]) ranked by id
+__global__ void __launch_bounds__(256) k_rank_cells(size_t nkeys, const uint32_t* __restrict__ offset, const uint32_t* __restrict__ id,
+                                                    uint32_t* __restrict__ perm) {
+  const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= nkeys) return;
+  const uint32_t b = offset[k], e = offset[k + 1];
+  for (uint32_t j = b; j < e; ++j) {
+    const uint32_t me = id[j];
+    uint32_t r = 0;
+    for (uint32_t m = b; m < e; ++m) r += (id[m] < me) ? 1u : 0u;
+    perm[b + r] = j;
+  }
 }
 struct Arrays8 { void* p[8]; };
 template <int NA>
@@ -1096,8 +1154,11 @@ struct mpc_ctx {
   unsigned long long seed;
   uint32_t t;
   size_t n, n_max;
-  bool bound, have_state, have_cells, have_order, compact, sticky, fast_brick, vec4, sums_clean, gather_pending, no_fuse_gather;
+  bool bound, have_state, have_cells, have_order, compact, sticky, fast_brick, vec4, sums_clean, gather_pending, no_fuse_gather, order_canonical, eager_canonical;
   cudaStream_t stream;
+  cudaStream_t stream2;       // side stream: PROCESS_CELLS of a reorder step runs beside the reorder's scatter
+  cudaEvent_t ev_scan, ev_cell;
+  bool side_ready, no_overlap;
   char* ws;
   size_t ws_bytes;
   uint32_t nbricks;
@@ -1137,12 +1198,13 @@ Layout make_layout(size_t n_max, size_t nkeys, int sw, int rw, bool compact) {
   auto take = [&](size_t bytes) { const size_t r = o; o = align_up(o + bytes, 256); return r; };
   const size_t pn = align_up((n_max ? n_max : 1) * 4, 256);   // whole 256-byte units: consecutive arrays are contiguous
   for (int a = 0; a < 7; ++a) l.off_A[a] = take(pn);
+  // the slot array sits between the two particle copies: either copy plus it = 8 contiguous arrays (aos_base)
+  l.off_slot = take(compact ? pn * 2 : pn);
   if (compact) { l.off_B[0] = take(pn); for (int a = 1; a < 7; ++a) l.off_B[a] = l.off_B[0]; }
   else for (int a = 0; a < 7; ++a) l.off_B[a] = take(pn);
   l.off_key = take(pn);
-  // (id, source index) per slot: 8 bytes; with the second copy present the slots live in its first two arrays
-  // (contiguous, unused until the gather) and this array only receives the sorted keys of the unfused path
-  l.off_slot = take(compact ? pn * 2 : pn);
+  // (the slot array holds (id, source index) pairs, 8 bytes each, in compact mode; with the second copy present
+  // those live in its first two arrays and the slot array only receives the sorted keys of the unfused path)
   l.off_perm = take(pn);
   l.off_cursor = take(nkeys * 4);
   l.off_offset = take((nkeys + 1) * 4);
@@ -1163,16 +1225,16 @@ int cuda_fail(mpc_ctx* c, cudaError_t e, const char* where) {
   return MPC_ECUDA;
 }
 struct FamilyTimer {   // records an event pair around the launches of one kernel family
-  mpc_ctx* c; int slot;
-  FamilyTimer(mpc_ctx* c_, int fam) : c(c_), slot(-1) {
+  mpc_ctx* c; int slot; cudaStream_t st;
+  FamilyTimer(mpc_ctx* c_, int fam, cudaStream_t st_ = nullptr) : c(c_), slot(-1), st(st_ ? st_ : c_->stream) {
     if (!c->prof_on) return;
     c->prof_launches[fam]++;
     if (c->prof_pairs >= PROF_MAX_PAIRS) return;
     slot = c->prof_pairs++;
     c->prof_fam[slot] = fam;
-    cudaEventRecord(c->prof_ev[2 * slot], c->stream);
+    cudaEventRecord(c->prof_ev[2 * slot], st);
   }
-  ~FamilyTimer() { if (slot >= 0) cudaEventRecord(c->prof_ev[2 * slot + 1], c->stream); }
+  ~FamilyTimer() { if (slot >= 0) cudaEventRecord(c->prof_ev[2 * slot + 1], st); }
 };
 #define CU(call)                                                 \
   do {                                                           \
@@ -1197,9 +1259,38 @@ void host_shift(const mpc_ctx* c, uint32_t t, float s[3]) {
   s[2] = (u01_co(o.c) - 0.5f) * c->G.a;
 }
 
+// particle arrays (and the keys, if asked) gathered through c->perm: new[i] = old[perm[i]]
+int apply_perm(mpc_ctx* c, bool need_key) {
+  const size_t n = c->n;
+  FamilyTimer ftg(c, F_GATHER);
+  if (!c->compact) {
+    Arrays8 src, dst;
+    for (int a = 0; a < 7; ++a) { src.p[a] = c->A[a]; dst.p[a] = c->Bf[a]; }
+    src.p[7] = c->key; dst.p[7] = c->slot_id;
+    if (need_key) k_gather<8><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
+    else k_gather<7><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
+    LAUNCH_CHECK("k_gather");
+    for (int a = 0; a < 7; ++a) { uint32_t* t = c->A[a]; c->A[a] = c->Bf[a]; c->Bf[a] = t; }
+    if (need_key) CU(cudaMemcpyAsync(c->key, c->slot_id, n * 4, cudaMemcpyDeviceToDevice, c->stream));
+  } else {
+    // property-wise through one temporary array (PAPER.md:156-162)
+    Arrays8 src, dst;
+    for (int a = 0; a < (need_key ? 8 : 7); ++a) {
+      uint32_t* arr = a < 7 ? c->A[a] : c->key;
+      CU(cudaMemcpyAsync(c->Bf[0], arr, n * 4, cudaMemcpyDeviceToDevice, c->stream));
+      src.p[0] = c->Bf[0]; dst.p[0] = arr;
+      k_gather<1><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
+      LAUNCH_CHECK("k_gather");
+    }
+  }
+  return MPC_OK;
+}
+
 // counting-sort reorder by (key, id); counts = low word of word 0 of the sums; c->key holds the keys
 // defer_gather: leave the permutation in c->perm for the next sweep to apply (launch_sweep<.., GATHER>)
-int do_reorder(mpc_ctx* c, bool defer_gather = false) {
+// canonical: rank the particles of a cell by id now (needed by MPC-AT); otherwise group by key only
+// cell_zero >= 0: launch k_cell(zero = cell_zero) on the side stream once the counts have been scanned
+int do_reorder(mpc_ctx* c, bool defer_gather, bool canonical, int cell_zero = -1) {
   const size_t n = c->n, nk = c->G.nkeys, nb = (nk + SCAN_TILE - 1) / SCAN_TILE;
   const uint32_t* cnt = reinterpret_cast<const uint32_t*>(c->sums);
   const int stride = c->G.sw * 2;
@@ -1212,81 +1303,91 @@ int do_reorder(mpc_ctx* c, bool defer_gather = false) {
     k_scan_apply<<<(unsigned)nb, SCAN_T, 0, c->stream>>>(cnt, stride, nk, c->bsum, c->offset);
     LAUNCH_CHECK("k_scan_apply");
   }
-  { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->cursor, 0, nk * 4, c->stream)); }
-  uint2* slot2 = reinterpret_cast<uint2*>(c->compact ? c->slot_id : c->Bf[0]);
-  {
-    FamilyTimer ft(c, F_SCATTER);
-    k_scatter_slots<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->key, c->A[6], c->offset, c->cursor, slot2);
-    LAUNCH_CHECK("k_scatter_slots");
+  if (cell_zero >= 0) {
+    CU(cudaEventRecord(c->ev_scan, c->stream));
+    CU(cudaStreamWaitEvent(c->stream2, c->ev_scan, 0));
+    {
+      FamilyTimer ft(c, F_CELL, c->stream2);
+      k_cell<<<c->cell_grid, 128, 0, c->stream2>>>(c->G, c->cell_cpb_shift, c->sums, c->rec, cell_zero);
+      LAUNCH_CHECK("k_cell");
+    }
+    CU(cudaEventRecord(c->ev_cell, c->stream2));
   }
-  {
+  { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->cursor, 0, nk * 4, c->stream)); }
+  if (canonical) {
+    uint2* slot2 = reinterpret_cast<uint2*>(c->compact ? c->slot_id : c->Bf[0]);
+    {
+      FamilyTimer ft(c, F_SCATTER);
+      k_scatter_slots<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->key, c->A[6], c->offset, c->cursor, slot2);
+      LAUNCH_CHECK("k_scatter_slots");
+    }
     FamilyTimer ft(c, F_RANK);
     k_rank<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->key, c->offset, slot2, c->perm);
     LAUNCH_CHECK("k_rank");
-  }
-  c->have_order = true;
-  if (defer_gather) { c->gather_pending = true; return MPC_OK; }
-  FamilyTimer ftg(c, F_GATHER);
-  const bool need_key = c->G.generic != 0;     // the unfused path reads the sorted keys afterwards
-  if (!c->compact) {
-    Arrays8 src, dst;
-    for (int a = 0; a < 7; ++a) { src.p[a] = c->A[a]; dst.p[a] = c->Bf[a]; }
-    src.p[7] = c->key; dst.p[7] = c->slot_id;   // slot_id is free after k_rank
-    if (need_key) k_gather<8><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
-    else k_gather<7><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
-    LAUNCH_CHECK("k_gather");
-    for (int a = 0; a < 7; ++a) { uint32_t* t = c->A[a]; c->A[a] = c->Bf[a]; c->Bf[a] = t; }
-    if (need_key) CU(cudaMemcpyAsync(c->key, c->slot_id, n * 4, cudaMemcpyDeviceToDevice, c->stream));   // the slot array is larger: no pointer swap
   } else {
-    // property-wise through one temporary array (PAPER.md:156-162)
-    Arrays8 src, dst;
-    for (int a = 0; a < (need_key ? 8 : 7); ++a) {
-      uint32_t* arr = a < 7 ? c->A[a] : c->key;
-      CU(cudaMemcpyAsync(c->Bf[0], arr, n * 4, cudaMemcpyDeviceToDevice, c->stream));
-      src.p[0] = c->Bf[0]; dst.p[0] = arr;
-      k_gather<1><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
-      LAUNCH_CHECK("k_gather");
-    }
+    FamilyTimer ft(c, F_SCATTER);
+    k_scatter_src<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->key, c->offset, c->cursor, c->perm);
+    LAUNCH_CHECK("k_scatter_src");
   }
   c->have_order = true;
-  return MPC_OK;
+  c->order_canonical = canonical;
+  int rc = MPC_OK;
+  if (defer_gather) c->gather_pending = true;
+  else rc = apply_perm(c, c->G.generic != 0);     // the unfused path reads the sorted keys afterwards
+  if (cell_zero >= 0) CU(cudaStreamWaitEvent(c->stream, c->ev_cell, 0));
+  return rc;
+}
+
+// restore the canonical (key, id) order inside the cell segments of the last reorder (U4); called
+// before the state is read when the hot path has left the particles grouped by key only
+int canonicalise(mpc_ctx* c) {
+  if (!c->have_order || c->order_canonical || c->n == 0) return MPC_OK;
+  {
+    FamilyTimer ft(c, F_RANK);
+    k_rank_cells<<<nblk(c->G.nkeys, 256), 256, 0, c->stream>>>(c->G.nkeys, c->offset, c->A[6], c->perm);
+    LAUNCH_CHECK("k_rank_cells");
+  }
+  const int rc = apply_perm(c, false);
+  if (rc == MPC_OK) c->order_canonical = true;
+  return rc;
 }
 
 typedef BrickShape<-1, -1, -1> BSgeneric;
 typedef BrickShape<4, 4, 3> BSfast;   // {16,16,8}
 
-// GATHER: read the particles through c->perm from the current arrays, write the other buffer, then swap
-template <bool COLLIDE, bool WKEY, class BS, bool GATHER>
+// staging buffer of the folded reorder (32 bytes per particle): the unused SoA copy plus the slot array, which
+// the workspace layout places between the two copies so that either copy extends to 8 arrays
+inline float* aos_base(const mpc_ctx* c) {
+  return reinterpret_cast<float*>(c->A[0] < c->Bf[0] ? c->slot_id : c->Bf[0]);
+}
+template <bool COLLIDE, bool WKEY, class BS, int IO>
 int launch_sweep_bs(mpc_ctx* c, const float sp[3]) {
   const Geo& G = c->G;
-  float** F = reinterpret_cast<float**>(GATHER ? c->Bf : c->A);
-  GatherSrc gs;
-  for (int a = 0; a < 6; ++a) gs.p[a] = reinterpret_cast<const float*>(c->A[a]);
-  gs.id = c->A[6]; gs.id_out = c->Bf[6]; gs.perm = c->perm;
+  float** F = reinterpret_cast<float**>(c->A);
+  SweepIO io;
+  io.aos_in = io.aos_out = aos_base(c);
+  io.perm = c->perm; io.id = c->A[6];
   const uint32_t* chunk = c->have_order ? c->offset : nullptr;
   const bool wall = G.wall >= 0, grav = (G.g[0] != 0.f || G.g[1] != 0.f || G.g[2] != 0.f);
 #define SWEEP_ARGS G, sp[0], sp[1], sp[2], (uint32_t)c->n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, chunk, c->nbricks, c->rec, c->sums
-  if (c->vec4 && !GATHER) {
+  if (c->vec4 && IO == IO_PLAIN) {
     if (wall && grav) k_sweep4<COLLIDE, true, true, WKEY, BS><<<c->nbricks, SWEEP4_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
     else if (wall) k_sweep4<COLLIDE, true, false, WKEY, BS><<<c->nbricks, SWEEP4_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
     else if (grav) k_sweep4<COLLIDE, false, true, WKEY, BS><<<c->nbricks, SWEEP4_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
     else k_sweep4<COLLIDE, false, false, WKEY, BS><<<c->nbricks, SWEEP4_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS);
   } else
-  if (wall && grav) k_sweep<COLLIDE, true, true, WKEY, BS, GATHER><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, gs);
-  else if (wall) k_sweep<COLLIDE, true, false, WKEY, BS, GATHER><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, gs);
-  else if (grav) k_sweep<COLLIDE, false, true, WKEY, BS, GATHER><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, gs);
-  else k_sweep<COLLIDE, false, false, WKEY, BS, GATHER><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, gs);
+  if (wall && grav) k_sweep<COLLIDE, true, true, WKEY, BS, IO><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, io);
+  else if (wall) k_sweep<COLLIDE, true, false, WKEY, BS, IO><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, io);
+  else if (grav) k_sweep<COLLIDE, false, true, WKEY, BS, IO><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, io);
+  else k_sweep<COLLIDE, false, false, WKEY, BS, IO><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, io);
 #undef SWEEP_ARGS
   LAUNCH_CHECK("k_sweep");
-  if (GATHER) {
-    for (int a = 0; a < 7; ++a) { uint32_t* t = c->A[a]; c->A[a] = c->Bf[a]; c->Bf[a] = t; }
-    c->gather_pending = false;
-  }
+  if (IO == IO_GATHER) c->gather_pending = false;
   return MPC_OK;
 }
-template <bool COLLIDE, bool WKEY, bool GATHER = false>
+template <bool COLLIDE, bool WKEY, int IO = IO_PLAIN>
 int launch_sweep(mpc_ctx* c, const float sp[3]) {
-  return c->fast_brick ? launch_sweep_bs<COLLIDE, WKEY, BSfast, GATHER>(c, sp) : launch_sweep_bs<COLLIDE, WKEY, BSgeneric, GATHER>(c, sp);
+  return c->fast_brick ? launch_sweep_bs<COLLIDE, WKEY, BSfast, IO>(c, sp) : launch_sweep_bs<COLLIDE, WKEY, BSgeneric, IO>(c, sp);
 }
 
 template <bool COLLIDE, bool WKEY, class BS>
@@ -1296,12 +1397,11 @@ cudaError_t sweep_attr_bs(size_t bytes) {
   if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, false, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
   if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, true, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
   if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, false, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
-  if (COLLIDE) {
-    if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, true, WKEY, BS, COLLIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
-    if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, false, WKEY, BS, COLLIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
-    if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, true, WKEY, BS, COLLIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
-    if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, false, WKEY, BS, COLLIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
-  }
+  constexpr int IOX = WKEY ? IO_AOS_OUT : (COLLIDE ? IO_GATHER : IO_PLAIN);   // the staged variant that exists for these flags
+  if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, true, WKEY, BS, IOX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+  if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, false, WKEY, BS, IOX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+  if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, true, WKEY, BS, IOX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+  if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, false, WKEY, BS, IOX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
   if ((e = cudaFuncSetAttribute(k_sweep4<COLLIDE, true, true, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
   if ((e = cudaFuncSetAttribute(k_sweep4<COLLIDE, true, false, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
   if ((e = cudaFuncSetAttribute(k_sweep4<COLLIDE, false, true, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
@@ -1324,23 +1424,34 @@ int steps_srd(mpc_ctx* c, int nsteps) {
     const bool rebin = (c->t % (uint32_t)c->p.rebin_every) == 0u;
     if (!c->sums_clean) { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * G.sw * 8, c->stream)); }
     c->sums_clean = false;
+    // reorder folded into this sweep (writes the 32-byte staging records) and the next one (reads them through
+    // the permutation): needs a next step in this call, the second particle copy, and rebin_every >= 2
+    const bool stage = rebin && !c->compact && !c->no_fuse_gather && !c->eager_canonical && k + 1 < nsteps && c->p.rebin_every >= 2;
     if (n) {
       {
-        FamilyTimer ft(c, c->gather_pending ? F_SWEEPG : F_SWEEP);
+        FamilyTimer ft(c, (c->gather_pending || stage) ? F_SWEEPG : F_SWEEP);
         int rc;
-        if (k == 0) rc = rebin ? launch_sweep<false, true>(c, sp) : launch_sweep<false, false>(c, sp);
-        else if (c->gather_pending) rc = rebin ? launch_sweep<true, true, true>(c, sp) : launch_sweep<true, false, true>(c, sp);
+        if (c->gather_pending) rc = launch_sweep<true, false, IO_GATHER>(c, sp);      // stage implies rebin_every >= 2
+        else if (stage) rc = (k == 0) ? launch_sweep<false, true, IO_AOS_OUT>(c, sp) : launch_sweep<true, true, IO_AOS_OUT>(c, sp);
+        else if (k == 0) rc = rebin ? launch_sweep<false, true>(c, sp) : launch_sweep<false, false>(c, sp);
         else rc = rebin ? launch_sweep<true, true>(c, sp) : launch_sweep<true, false>(c, sp);
         if (rc) return rc;
       }
-      // the gather of a reorder is folded into the next step's sweep when there is one in this call
-      if (rebin) { const int rc = do_reorder(c, !c->compact && !c->no_fuse_gather && k + 1 < nsteps); if (rc) return rc; }
-      FamilyTimer ft(c, F_CELL);
       // all but the last step of the call: k_cell clears the sums it has read (the last step's stay for
       // mpc_observables / mpc_get_cells)
       const int zero = (k + 1 < nsteps) ? 1 : 0;
-      k_cell<<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec, zero);
-      LAUNCH_CHECK("k_cell");
+      const bool overlap = rebin && c->side_ready && !c->no_overlap;
+      // the gather of a reorder is folded into the next step's sweep when there is one in this call;
+      // PROCESS_CELLS of a reorder step runs on the side stream beside the scatter (both wait for the scan)
+      if (rebin) {
+        const int rc = do_reorder(c, stage, c->eager_canonical, overlap ? zero : -1);
+        if (rc) return rc;
+      }
+      if (!overlap) {
+        FamilyTimer ft(c, F_CELL);
+        k_cell<<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, c->sums, c->rec, zero);
+        LAUNCH_CHECK("k_cell");
+      }
       c->sums_clean = zero != 0;
     }
     sp[0] = G.s[0]; sp[1] = G.s[1]; sp[2] = G.s[2];
@@ -1382,7 +1493,7 @@ int steps_generic(mpc_ctx* c, int nsteps) {
         else k_stream_key<false, false><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, c->sums);
         LAUNCH_CHECK("k_stream_key");
       }
-      if (rebin) { const int rc = do_reorder(c); if (rc) return rc; }
+      if (rebin) { const int rc = do_reorder(c, false, true); if (rc) return rc; }
       F = reinterpret_cast<float**>(c->A);
       {
         FamilyTimer ft(c, F_ACCUM);
@@ -1423,13 +1534,14 @@ int set_state_impl(mpc_ctx* c, unsigned long long n, const float* const src[6], 
     if (id) CU(cudaMemcpyAsync(c->A[6], id, n * 4, kind, c->stream));
     else { k_iota<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->A[6]); LAUNCH_CHECK("k_iota"); }
   }
-  c->n = n; c->t = step; c->have_state = true; c->have_cells = false; c->have_order = false; c->gather_pending = false;
+  c->n = n; c->t = step; c->have_state = true; c->have_cells = false; c->have_order = false; c->gather_pending = false; c->order_canonical = true;
   return MPC_OK;
 }
 int get_state_impl(mpc_ctx* c, float* const dst[6], unsigned* id, cudaMemcpyKind kind) {
   if (!c) return MPC_EINVAL;
   if (c->sticky) return MPC_ECUDA;
   if (!c->have_state) return fail(c, MPC_ESTATE, "mpc_get_state before mpc_set_state");
+  { const int rc = canonicalise(c); if (rc) return rc; }
   for (int a = 0; a < 6; ++a)
     if (dst[a] && c->n) CU(cudaMemcpyAsync(dst[a], c->A[a], c->n * 4, kind, c->stream));
   if (id && c->n) CU(cudaMemcpyAsync(id, c->A[6], c->n * 4, kind, c->stream));
@@ -1493,6 +1605,10 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   c->fast_brick = (G.bs[0] == 4 && G.bs[1] == 4 && G.bs[2] == 3);
   { const char* e = getenv("MPC_SWEEP_VEC"); c->vec4 = (e && e[0] == '4'); }
   { const char* e = getenv("MPC_NO_FUSE_GATHER"); c->no_fuse_gather = (e && e[0] == '1'); }
+  { const char* e = getenv("MPC_EAGER_CANONICAL"); c->eager_canonical = (e && e[0] == '1'); }
+  // measured: no gain (k_cell beside the scatter slows the scatter down by as much), so off unless asked for
+  { const char* e = getenv("MPC_OVERLAP_CELL"); c->no_overlap = !(e && e[0] == '1'); }
+  c->side_ready = false;
   {
     const int bvs = G.bs[0] + G.bs[1] + G.bs[2];
     c->cell_cpb_shift = bvs > 7 ? bvs - 7 : 0;
@@ -1544,6 +1660,12 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
   c->bsum = (uint32_t*)(c->ws + l.off_bsum);
   c->sums = (u64*)(c->ws + l.off_sums); c->rec = (float*)(c->ws + l.off_rec); c->obs = (double*)(c->ws + l.off_obs);
   c->nsing = (u64*)(c->ws + l.off_obs + OBS_HOST_DOUBLES * 8);
+  if (!c->side_ready) {
+    CU(cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking));
+    CU(cudaEventCreateWithFlags(&c->ev_scan, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&c->ev_cell, cudaEventDisableTiming));
+    c->side_ready = true;
+  }
   c->bound = true; c->have_state = false; c->have_cells = false; c->have_order = false; c->sums_clean = false; c->gather_pending = false; c->n = 0;
   if (c->tile_bytes > 48 * 1024) {
     cudaError_t e;
@@ -1698,6 +1820,7 @@ const char* mpc_last_error(const mpc_ctx* c) { return c ? c->err : "null context
 int mpc_destroy(mpc_ctx* c) {
   if (c) {
     delete[] c->hbuf;
+    if (c->side_ready) { cudaStreamDestroy(c->stream2); cudaEventDestroy(c->ev_scan); cudaEventDestroy(c->ev_cell); }
     if (c->prof_ev) for (int i = 0; i < 2 * PROF_MAX_PAIRS; ++i) cudaEventDestroy(c->prof_ev[i]);
     delete[] c->prof_ev;
     delete[] c->prof_fam;
