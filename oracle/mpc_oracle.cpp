@@ -240,8 +240,12 @@ inline double mbs_energy_over_kT(const Ctx& c, uint32_t cid, uint32_t t, unsigne
   };
   for (unsigned j = 0; j < M; ++j) e -= std::log(u_oc(next()));
   if (f & 1u) {
-    const double l = -std::log(u_oc(next()));
-    const double cs = std::cos(TWO_PI * u_co(next()));
+    // the two uniforms of the half squared normal are words 2 and 3 of the cell's TAG_AXIS block of this
+    // step (words 0 and 1 give the rotation axis): independent of both, and no extra block (reading U6)
+    uint32_t a[4];
+    draw(c, cid, 0u, t, TAG_AXIS, a);
+    const double l = -std::log(u_oc(a[2]));
+    const double cs = std::cos(TWO_PI * u_co(a[3]));
     e += l * cs * cs;                                   // = G^2/2 with G = sqrt(-2 ln U) cos(2 pi U')
   }
   return e;

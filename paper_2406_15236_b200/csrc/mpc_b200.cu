@@ -949,9 +949,10 @@ __device__ __forceinline__ void renorm(float& p, int& ex) {   // p = m * 2^e wit
 }
 // 2^24 * u01_oc(w): the power-of-two scale of every uniform is banked in the exponent instead (exact)
 __device__ __forceinline__ float u24_oc(uint32_t w) { return (float)((w >> 8) + 1u); }
-__device__ float mbs_energy(const Geo& G, uint32_t cid, uint32_t Nc) {
+// wm, wa: words 2 and 3 of the cell's TAG_AXIS block, the two uniforms of the half squared normal (f odd)
+__device__ float mbs_energy(const Geo& G, uint32_t cid, uint32_t Nc, uint32_t wm, uint32_t wa) {
   const uint32_t f = 3u * (Nc - 1u), M = f >> 1, odd = f & 1u;
-  const uint32_t full = M >> 2;                  // blocks whose four uniforms all enter the product
+  const uint32_t full = M >> 2, rem = M & 3u;    // blocks whose four uniforms all enter the product; uniforms of the last one
   float p = 1.0f;
   int ex = -24 * (int)M;                         // M uniforms enter the product, each carried as 2^24 u
   uint32_t sub = 0;
@@ -960,25 +961,18 @@ __device__ float mbs_energy(const Geo& G, uint32_t cid, uint32_t Nc) {
     p *= (u24_oc(o.a) * u24_oc(o.b)) * (u24_oc(o.c) * u24_oc(o.d));   // < 2^96: cannot overflow
     renorm(p, ex);
   }
-  // tail: positions 4*full .. M-1 still enter the product, M and M+1 feed the half squared normal
-  float um = 1.0f, ua = 0.0f;
-  const uint32_t need = M + 2u * odd;
-  for (uint32_t base = full << 2; base < need; base += 4, ++sub) {
-    const Block4 o = philox_rk(cid, sub, G.t, TAG_MBS, G.rk);
-    const uint32_t w[4] = {o.a, o.b, o.c, o.d};
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      const uint32_t pos = base + q;
-      p *= (pos < M) ? u24_oc(w[q]) : 1.0f;
-      um = (pos == M) ? u01_oc(w[q]) : um;
-      ua = (pos == M + 1u) ? u01_co(w[q]) : ua;
-    }
+  if (rem) {
+    const Block4 o = philox_rk(cid, full, G.t, TAG_MBS, G.rk);
+    float q = u24_oc(o.a);
+    q *= (rem > 1u) ? u24_oc(o.b) : 1.0f;
+    q *= (rem > 2u) ? u24_oc(o.c) : 1.0f;
+    p *= q;
     renorm(p, ex);
   }
   float e = -(float)((double)logf(p) + (double)ex * 0.6931471805599453);
   if (odd) {
-    const float cs = cospif(2.0f * ua);
-    e -= logf(um) * cs * cs;
+    const float cs = cospif(2.0f * u01_co(wa));
+    e -= logf(u01_oc(wm)) * cs * cs;
   }
   return e;
 }
@@ -1040,16 +1034,16 @@ __global__ void __launch_bounds__(128) k_cell(Geo G, int cpb_shift, u64* __restr
     }
     const double inv = 1.0 / (double)Nc;
     r0.x = (float)(S0 * inv); r0.y = (float)(S1 * inv); r0.z = (float)(S2 * inv);
+    const Block4 o = philox_rk(cid, 0u, G.t, TAG_AXIS, G.rk);
     float kappa = 1.0f;
     if (G.thermostat && Nc >= 2u) {
       const double W2 = E - (S0 * S0 + S1 * S1 + S2 * S2) * inv;   // sum |v - vcm|^2
       if (W2 > 0.0) {
-        const float ek = G.kT * mbs_energy(G, cid, Nc);
+        const float ek = G.kT * mbs_energy(G, cid, Nc, o.c, o.d);
         kappa = sqrtf(2.0f * ek / (G.mass * (float)W2));
       }
     }
     r0.w = kappa;
-    const Block4 o = philox_rk(cid, 0u, G.t, TAG_AXIS, G.rk);
     const float zz = 2.0f * u01_co(o.a) - 1.0f;
     const float rr = sqrtf((1.0f - zz) * (1.0f + zz));
     float sp, cp;
