@@ -196,15 +196,23 @@ def main():
     brick = brick * 3 if len(brick) == 1 else brick
     kw.update(rebin_every=wl["rebin_every"], brick=brick)
     compact = args.compact or (n * 72 + int(np.prod(cells)) * 80 > 150e9)
-    sim = MPC(box, cells, nbar, 1234 + rank, n_max=n, device=str(device), compact=compact, **kw)
     rest = "g" in kw
-    st = list(uniform_maxwell_cuda(box, n, 1234 + rank, device=str(device)))
+    # a state that does not fit beside the workspace (20 per cell: 64 GB + 138 GB) is made array by array on the
+    # device, parked in pinned host memory and handed over through the host-pointer ABI
+    via_host = n * 24 + n * 52 + int(np.prod(cells)) * 80 > 170e9
+    st = list(uniform_maxwell_cuda(box, n, 1234 + rank, device=str(device), to_host=via_host))
     if rest:
         for v in st[3:]:
             v.zero_()
-    sim.set_state(*st)
+    torch.cuda.empty_cache()
+    sim = MPC(box, cells, nbar, 1234 + rank, n_max=n, device=str(device), compact=compact, **kw)
+    if via_host:
+        sim.set_state_host(*st)
+    else:
+        sim.set_state(*st)
     torch.cuda.synchronize()
     del st
+    sim._keep = None
     torch.cuda.empty_cache()
 
     def barrier():
@@ -249,8 +257,13 @@ def main():
         # per launch of the dominant kernel: its share of the step's algorithmic bytes
         fam_bytes = kernel_algorithmic_bytes(dom, n, int(np.prod(cells)), nbar)
         ach = fam_bytes / (dms / dcnt * 1e-3) / 1e9
+        # DRAM bytes of one launch of the steady-state sweep from the committed ncu --set full capture
+        # (profiles/r01b_ncu_full.md: dram__bytes_read.sum 41.47 GB + dram__bytes_write.sum 35.90 GB at config 5,
+        # 10 particles per cell); other workloads have no capture: null
+        traffic = 77.37e9 if (dom == "sweep" and args.workload == "cfg5" and nbar == 10 and args.cells is None) else None
         roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                    "traffic": None, "peak_source": peak_src, "avg_ms": dms / dcnt, "launches_timed": dcnt,
+                    "traffic": traffic, "traffic_source": "profiles/r01b_ncu_full.md" if traffic else None,
+                    "peak_source": peak_src, "avg_ms": dms / dcnt, "launches_timed": dcnt,
                     "algorithmic_bytes_per_launch": fam_bytes,
                     "step_frac_of_roofline": value / world * balg / 1e9 / peak,
                     "step_frac_of_8000": value / world * balg / 1e9 / 8000.0,

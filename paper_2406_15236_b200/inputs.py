@@ -31,9 +31,11 @@ def uniform_maxwell(box, n, seed, kT=1.0, mass=1.0, zero_momentum=True, rest=Fal
     return (*pos, *vel, ids)
 
 
-def uniform_maxwell_cuda(box, n, seed, kT=1.0, mass=1.0, device="cuda:0"):
+def uniform_maxwell_cuda(box, n, seed, kT=1.0, mass=1.0, device="cuda:0", to_host=False):
     """Device twin for sizes the host cannot hold comfortably: same distributions from torch's
-    CUDA generator. Returns six float32 device tensors (ids are implied 0..n-1)."""
+    CUDA generator. Returns six float32 device tensors (ids are implied 0..n-1); with to_host=True each
+    array is moved to pinned host memory as soon as it is made (for states that do not fit beside the
+    library's workspace: config 5 at 20 particles per cell)."""
     import torch
 
     g = torch.Generator(device=device)
@@ -43,10 +45,23 @@ def uniform_maxwell_cuda(box, n, seed, kT=1.0, mass=1.0, device="cuda:0"):
         r = torch.rand(n, device=device, dtype=torch.float32, generator=g)
         r.mul_(float(box[d]))
         r.masked_fill_(r >= float(box[d]), 0.0)
-        out.append(r)
+        out.append(_park(r, to_host))
     for d in range(3):
         v = torch.randn(n, device=device, dtype=torch.float32, generator=g)
         v.mul_(float(np.sqrt(kT / mass)))
-        v.sub_(v.mean(dtype=torch.float64).to(torch.float32))
-        out.append(v)
+        tot = 0.0                       # mean in float64, chunk by chunk (no second full-size array)
+        for c in v.split(1 << 28):
+            tot += float(c.sum(dtype=torch.float64))
+        v.sub_(tot / n)
+        out.append(_park(v, to_host))
     return tuple(out)
+
+
+def _park(t, to_host):
+    if not to_host:
+        return t
+    import torch
+
+    h = torch.empty(t.shape, dtype=t.dtype, pin_memory=True)
+    h.copy_(t)
+    return h
