@@ -30,7 +30,7 @@ WORKLOADS = {
     # name: (cells, nbar, params, default steps, default warmup)
     "cfg1": dict(cells=(16, 16, 16), nbar=10, kw=dict(), rebin_every=1),
     "cfg2": dict(cells=(64, 64, 64), nbar=10, kw=dict(thermostat=1), rebin_every=1),
-    "cfg3": dict(cells=(128, 128, 128), nbar=10, kw=dict(collision=1, dt=0.02), rebin_every=1),   # +a: see DESIGN.md
+    "cfg3": dict(cells=(128, 128, 128), nbar=10, kw=dict(collision=1, conserve_L=1, dt=0.02), rebin_every=1),
     "cfg4": dict(cells=(256, 64, 64), nbar=10, kw=dict(thermostat=1, bc=(0, 0, 1), g=(0.001, 0, 0)), rebin_every=1),
     "cfg5": dict(cells=(512, 512, 512), nbar=10, kw=dict(thermostat=1), rebin_every=10),
 }
