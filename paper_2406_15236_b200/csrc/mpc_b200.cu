@@ -511,6 +511,66 @@ __global__ void __launch_bounds__(256) k_accum_a(Geo G, size_t n, const float* _
   atomicAdd(s + 9, pack_ss(fv(l1), fv(l2)));
 }
 
+// Segmented variant of k_accum_at / k_accum_a for a step that has just reordered: the particles of cell k are
+// the contiguous segment [offset[k], offset[k+1]) in (key, id) order, so one thread sums its cell in registers
+// and stores the packed words: no atomics (the atomic versions are bound by ~190 G global atomics/s) and the same
+// integers (two's-complement adds of the same addends, any order).
+template <bool AT, bool PLUS_A>
+__global__ void __launch_bounds__(128) k_accum_seg(Geo G, int cpb_shift, const float* __restrict__ x, const float* __restrict__ y,
+                                                   const float* __restrict__ z, const float* __restrict__ vx,
+                                                   const float* __restrict__ vy, const float* __restrict__ vz,
+                                                   const uint32_t* __restrict__ offset, u64* __restrict__ sums) {
+  const int b0 = G.bs[0], b1 = G.bs[1], b2 = G.bs[2];
+  const uint32_t bx = blockIdx.x >> cpb_shift, by = blockIdx.y, bz = blockIdx.z;
+  const uint32_t local = ((blockIdx.x & ((1u << cpb_shift) - 1u)) << 7) | threadIdx.x;
+  if (local >= (1u << (b0 + b1 + b2))) return;
+  const uint32_t brick = (bz * (uint32_t)G.mb[1] + by) * (uint32_t)G.mb[0] + bx;
+  const uint32_t k = (brick << (b0 + b1 + b2)) | local;
+  const uint32_t jb = offset[k], je = offset[k + 1];
+  if (jb == je) return;
+  const int ix = (int)((bx << b0) | (local & ((1u << b0) - 1u)));
+  const int iy = (int)((by << b1) | ((local >> b0) & ((1u << b1) - 1u)));
+  const int iz = (int)((bz << b2) | (local >> (b0 + b1)));
+  const uint32_t cid = canonical_id(G, ix, iy, iz);
+  float ax = 0.f, ay = 0.f, az = 0.f;
+  if (!AT) srd_axis(G, cid, ax, ay, az);
+  int S[18];
+#pragma unroll
+  for (int q = 0; q < 18; ++q) S[q] = 0;
+  auto fv = [&](float a) { return __float2int_rn(a * G.fxv); };
+  auto fq = [&](float a) { return __float2int_rn(a * FX_RHO); };
+  for (uint32_t j = jb; j < je; ++j) {
+    const float v[3] = {vx[j], vy[j], vz[j]};
+    float u[3], g[3] = {0.f, 0.f, 0.f};
+    if (AT) {
+      const Block4 o = philox(cid, j - jb, G.t, TAG_AT, G.k0, G.k1);
+      normals3(o, g[0], g[1], g[2]);
+      g[0] *= G.sigma; g[1] *= G.sigma; g[2] *= G.sigma;
+      u[0] = v[0] - g[0]; u[1] = v[1] - g[1]; u[2] = v[2] - g[2];
+    } else {
+      float d[3];
+      rotate(G, ax, ay, az, v, d);
+      u[0] = v[0] - d[0]; u[1] = v[1] - d[1]; u[2] = v[2] - d[2];
+    }
+    S[0] += fv(v[0]); S[1] += fv(v[1]); S[2] += fv(v[2]);
+    if (AT) { S[3] += fv(g[0]); S[4] += fv(g[1]); S[5] += fv(g[2]); }
+    if (PLUS_A) {
+      const float r0 = cell_frac(G, x[j], G.s[0]), r1 = cell_frac(G, y[j], G.s[1]), r2 = cell_frac(G, z[j], G.s[2]);
+      const float l0 = fmaf(r1, u[2], -(r2 * u[1])), l1 = fmaf(r2, u[0], -(r0 * u[2])), l2 = fmaf(r0, u[1], -(r1 * u[0]));
+      S[6] += fq(r0); S[7] += fq(r1); S[8] += fq(r2); S[9] += fq(r0 * r0); S[10] += fq(r1 * r1); S[11] += fq(r2 * r2);
+      S[12] += fq(r0 * r1); S[13] += fq(r0 * r2); S[14] += fq(r1 * r2); S[15] += fv(l0); S[16] += fv(l1); S[17] += fv(l2);
+    }
+  }
+  u64* s = sums + (size_t)k * G.sw;
+  s[1] = pack_ss(S[0], S[1]);
+  s[2] = pack_ss(S[2], S[3]);
+  if (AT) s[3] = pack_ss(S[4], S[5]);
+  if (PLUS_A) {
+    s[4] = pack_ss(S[6], S[7]); s[5] = pack_ss(S[8], S[9]); s[6] = pack_ss(S[10], S[11]);
+    s[7] = pack_ss(S[12], S[13]); s[8] = pack_ss(S[14], S[15]); s[9] = pack_ss(S[16], S[17]);
+  }
+}
+
 // rec[key] (16 floats) = { base.xyz, 1 | axis.xyz, - | omega.xyz, - | rho_cm.xyz, - }
 //   SRD+a: base = v_cm ; AT+a: base = v_cm - mean(v_ran)
 template <bool AT>
@@ -1329,6 +1389,11 @@ int steps_generic(mpc_ctx* c, int nsteps) {
       F = reinterpret_cast<float**>(c->A);
       {
         FamilyTimer ft(c, F_ACCUM);
+        if (rebin) {   // fresh (key, id) order: per-cell segmented sums, no atomics
+          if (plus_a && at) k_accum_seg<true, true><<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, F[0], F[1], F[2], F[3], F[4], F[5], c->offset, c->sums);
+          else if (plus_a) k_accum_seg<false, true><<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, F[0], F[1], F[2], F[3], F[4], F[5], c->offset, c->sums);
+          else k_accum_seg<true, false><<<c->cell_grid, 128, 0, c->stream>>>(G, c->cell_cpb_shift, F[0], F[1], F[2], F[3], F[4], F[5], c->offset, c->sums);
+        } else
         if (plus_a && at) k_accum_a<true><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, c->offset, c->sums);
         else if (plus_a) k_accum_a<false><<<gb, 256, 0, c->stream>>>(G, n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, c->offset, c->sums);
         else k_accum_at<<<gb, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->key, c->offset, c->sums);
