@@ -106,11 +106,22 @@ int mpc_set_state_host(mpc_ctx*, unsigned long long n, const float* x, const flo
                        const float* vx, const float* vy, const float* vz, const unsigned* id, unsigned step);
 
 /* Advance nsteps MPC steps (nsteps >= 0). Asynchronous: only kernel launches and memsets on the
- * bound stream, no host synchronisation. Requires max |v| h < L/2 (single periodic wrap, U2). */
+ * bound stream, no host synchronisation. Requires max |v| h < L/2 (single periodic wrap, U2).
+ * One call of n steps gives bit-identical results to n calls of one step; it is faster because the
+ * collision of step t is fused into the streaming pass of step t+1 and a reorder is folded into the
+ * sweeps of its own and the next step.
+ * Diagnostic switches read from the environment at mpc_create (all change speed only, never results):
+ * MPC_NO_FUSE_GATHER=1 (separate gather kernel), MPC_EAGER_CANONICAL=1 (rank by id at every reorder),
+ * MPC_OVERLAP_CELL=1 (PROCESS_CELLS of a reorder step on a side stream). */
 int mpc_step(mpc_ctx*, int nsteps);
 
 /* Copy the state out, in the current internal order, with ids. Any pointer may be NULL (skipped).
- * Device pointers: asynchronous. Host pointers: synchronises the stream before returning. */
+ * Device pointers: asynchronous. Host pointers: synchronises the stream before returning.
+ * Order: particles sorted by (memory key, id) as of the last reorder step (U3/U4).
+ * The SRD hot path keeps the particles grouped by key only between reads (the order inside a cell does not
+ * enter the physics: cell sums are integers); this call first restores the id order inside every cell
+ * (a rank kernel and one gather on the bound stream), so what it returns is always the canonical order and
+ * does not depend on how the steps were split over mpc_step calls. Calling it again costs only the copies. */
 int mpc_get_state(mpc_ctx*, float* x, float* y, float* z, float* vx, float* vy, float* vz, unsigned* id);
 int mpc_get_state_host(mpc_ctx*, float* x, float* y, float* z, float* vx, float* vy, float* vz, unsigned* id);
 
