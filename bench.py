@@ -113,6 +113,23 @@ def oracle_rate(wl, nbar, budget_s=12.0):
     return n * steps / dt, f"{cells[0]}x{cells[1]}x{cells[2]} cells x {nbar}/cell ({n} particles), {steps} steps, same parameters", steps, dt / steps
 
 
+def max_over_ranks(dist, ms, device):
+    """Replicas only: the only exchange between ranks is this MAX of the device-timed
+    milliseconds (and the barriers around the timed region)."""
+    if dist is None:
+        return float(ms)
+    import torch
+
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(world, n_per_rank, steps, ms):
+    """Whole-job particle-updates/s: every rank advances its own replica of n_per_rank particles (weak scaling)."""
+    return world * n_per_rank * steps / (ms * 1e-3)
+
+
 def run_reference(args, wl, rank, world):
     if rank != 0:
         return
@@ -238,12 +255,9 @@ def main():
     launches = sim.launch_count - l0
     prof = sim.profile_read()
     sim.profile_enable(False)
-    if dist is not None:
-        t = torch.tensor([ms], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(dist, ms, device)
     ob = sim.observables()
-    value = world * n * args.steps / (ms * 1e-3)
+    value = whole_job_rate(world, n, args.steps, ms)
 
     # ---- roofline of the dominant kernel family (live CUDA-event times from the timed region) ----
     peak, peak_src = measured_peaks()
