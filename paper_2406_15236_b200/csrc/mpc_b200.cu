@@ -44,6 +44,7 @@ typedef unsigned long long u64;
 #endif
 constexpr int HALO = MPC_HALO;        // tile halo in cells on every side of a brick
 constexpr int SWEEP_T = MPC_SWEEP_T;  // threads per sweep CTA
+constexpr int SWEEP_T3 = 384;         // ... of the steady-state sweep when three tiles fit in an SM's shared memory
 constexpr int PF_DIST = 4;           // L2 prefetch distance of the sweep, in iterations of SWEEP_T particles
 constexpr int TILE_W = 5;             // int32 words per tile cell: N, Sx, Sy, Sz, E
 constexpr int REC_W = 8;              // floats per cell record (32 B, one sector)
@@ -251,8 +252,10 @@ __device__ __forceinline__ void st256(float* p, const float (&a)[8]) {
   asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
                :: "l"(p), "f"(a[0]), "f"(a[1]), "f"(a[2]), "f"(a[3]), "f"(a[4]), "f"(a[5]), "f"(a[6]), "f"(a[7]) : "memory");
 }
-template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS, int IO = IO_PLAIN>
-__global__ void __launch_bounds__(SWEEP_T, MPC_SWEEP_MINB)
+// T = threads per CTA: 512 (2 CTAs per SM), or 384 (3 CTAs per SM at <= 56 registers: the steady-state sweep is
+// 2 % faster that way, the staged reorder sweeps are not)
+template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS, int IO = IO_PLAIN, int T = SWEEP_T>
+__global__ void __launch_bounds__(T, T <= 384 ? 3 : 2)
 k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
         float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, uint32_t* __restrict__ key_out,
         const uint32_t* __restrict__ chunk, uint32_t nbricks, const float* __restrict__ rec, u64* __restrict__ sums,
@@ -260,7 +263,7 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
   extern __shared__ int tile[];
   const int T0 = (1 << BS::s0(G)) + 2 * HALO, T1 = (1 << BS::s1(G)) + 2 * HALO, T2 = (1 << BS::s2(G)) + 2 * HALO;
   const int tcells = T0 * T1 * T2;
-  for (int i = threadIdx.x; i < tcells * TILE_W; i += SWEEP_T) tile[i] = 0;
+  for (int i = threadIdx.x; i < tcells * TILE_W; i += T) tile[i] = 0;
   const uint32_t b = blockIdx.x;
   const int m0 = G.m[0], m1 = G.m[1], m2 = G.m[2];
   int ox, oy, oz;
@@ -298,17 +301,17 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       ld256(io.aos_in + (size_t)io.perm[i] * 8, q);
       p0 = q[0]; p1 = q[1]; p2 = q[2]; p3 = q[3]; p4 = q[4]; p5 = q[5]; pid = q[6];
     }
-    if (i + SWEEP_T < i1) jn = io.perm[i + SWEEP_T];
-    if (i + 2 * SWEEP_T < i1) jn2 = io.perm[i + 2 * SWEEP_T];
-    if (i + 3 * SWEEP_T < i1) jn3 = io.perm[i + 3 * SWEEP_T];
+    if (i + T < i1) jn = io.perm[i + T];
+    if (i + 2 * T < i1) jn2 = io.perm[i + 2 * T];
+    if (i + 3 * T < i1) jn3 = io.perm[i + 3 * T];
   } else if (i < i1) {
     p0 = x[i]; p1 = y[i]; p2 = z[i]; p3 = vx[i]; p4 = vy[i]; p5 = vz[i];
     if (IO == IO_AOS_OUT) pid = __uint_as_float(io.id[i]);
   }
-  for (; i < i1; i += SWEEP_T) {
+  for (; i < i1; i += T) {
     float r[3] = {p0, p1, p2}, v[3] = {p3, p4, p5};
     const float idbits = pid;
-    const uint32_t inext = i + SWEEP_T;
+    const uint32_t inext = i + T;
     if (IO == IO_GATHER) {
       io.id[i] = __float_as_uint(idbits);
       if (inext < i1) {
@@ -316,15 +319,15 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
         ld256(io.aos_in + (size_t)jn * 8, q);
         p0 = q[0]; p1 = q[1]; p2 = q[2]; p3 = q[3]; p4 = q[4]; p5 = q[5]; pid = q[6];
         jn = jn2; jn2 = jn3;
-        if (i + 2 * SWEEP_T < i1) asm volatile("prefetch.global.L2 [%0];" ::"l"(io.aos_in + (size_t)jn * 8));
-        if (i + 4 * SWEEP_T < i1) jn3 = io.perm[i + 4 * SWEEP_T];
+        if (i + 2 * T < i1) asm volatile("prefetch.global.L2 [%0];" ::"l"(io.aos_in + (size_t)jn * 8));
+        if (i + 4 * T < i1) jn3 = io.perm[i + 4 * T];
       }
     } else if (inext < i1) {
       p0 = x[inext]; p1 = y[inext]; p2 = z[inext]; p3 = vx[inext]; p4 = vy[inext]; p5 = vz[inext];
       if (IO == IO_AOS_OUT) pid = __uint_as_float(io.id[inext]);
     }
     if (IO != IO_GATHER) {   // pull the lines of a later iteration into L2: the register prefetch above then pays L2, not DRAM, latency
-      const uint32_t ifar = i + PF_DIST * SWEEP_T;
+      const uint32_t ifar = i + PF_DIST * T;
       if (ifar < i1) {
         asm volatile("prefetch.global.L2 [%0];" ::"l"(x + ifar));
         asm volatile("prefetch.global.L2 [%0];" ::"l"(y + ifar));
@@ -374,7 +377,7 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
   }
   __syncthreads();
   // flush the tile: one packed 64-bit reduction per pair of sums, empty cells skipped
-  for (int c = threadIdx.x; c < tcells; c += SWEEP_T) {
+  for (int c = threadIdx.x; c < tcells; c += T) {
     const int* s = tile + c * TILE_W;
     const int cnt = s[0];
     if (cnt == 0) continue;
@@ -1098,7 +1101,7 @@ struct mpc_ctx {
   unsigned long long seed;
   uint32_t t;
   size_t n, n_max;
-  bool bound, have_state, have_cells, have_order, compact, sticky, fast_brick, sums_clean, gather_pending, no_fuse_gather, order_canonical, eager_canonical;
+  bool bound, have_state, have_cells, have_order, compact, sticky, fast_brick, sums_clean, gather_pending, no_fuse_gather, order_canonical, eager_canonical, three_ctas;
   cudaStream_t stream;
   cudaStream_t stream2;       // side stream: PROCESS_CELLS of a reorder step runs beside the reorder's scatter
   cudaEvent_t ev_scan, ev_cell;
@@ -1314,6 +1317,12 @@ int launch_sweep_bs(mpc_ctx* c, const float sp[3]) {
   const uint32_t* chunk = c->have_order ? c->offset : nullptr;
   const bool wall = G.wall >= 0, grav = (G.g[0] != 0.f || G.g[1] != 0.f || G.g[2] != 0.f);
 #define SWEEP_ARGS G, sp[0], sp[1], sp[2], (uint32_t)c->n, F[0], F[1], F[2], F[3], F[4], F[5], c->key, chunk, c->nbricks, c->rec, c->sums
+  if (IO == IO_PLAIN && !WKEY && c->three_ctas) {   // steady-state sweep: 3 CTAs of 384 threads per SM
+    if (wall && grav) k_sweep<COLLIDE, true, true, false, BS, IO_PLAIN, SWEEP_T3><<<c->nbricks, SWEEP_T3, c->tile_bytes, c->stream>>>(SWEEP_ARGS, io);
+    else if (wall) k_sweep<COLLIDE, true, false, false, BS, IO_PLAIN, SWEEP_T3><<<c->nbricks, SWEEP_T3, c->tile_bytes, c->stream>>>(SWEEP_ARGS, io);
+    else if (grav) k_sweep<COLLIDE, false, true, false, BS, IO_PLAIN, SWEEP_T3><<<c->nbricks, SWEEP_T3, c->tile_bytes, c->stream>>>(SWEEP_ARGS, io);
+    else k_sweep<COLLIDE, false, false, false, BS, IO_PLAIN, SWEEP_T3><<<c->nbricks, SWEEP_T3, c->tile_bytes, c->stream>>>(SWEEP_ARGS, io);
+  } else
   if (wall && grav) k_sweep<COLLIDE, true, true, WKEY, BS, IO><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, io);
   else if (wall) k_sweep<COLLIDE, true, false, WKEY, BS, IO><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, io);
   else if (grav) k_sweep<COLLIDE, false, true, WKEY, BS, IO><<<c->nbricks, SWEEP_T, c->tile_bytes, c->stream>>>(SWEEP_ARGS, io);
@@ -1335,6 +1344,12 @@ cudaError_t sweep_attr_bs(size_t bytes) {
   if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, false, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
   if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, true, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
   if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, false, WKEY, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+  if (!WKEY) {
+    if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, true, false, BS, IO_PLAIN, SWEEP_T3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+    if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, false, false, BS, IO_PLAIN, SWEEP_T3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+    if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, true, false, BS, IO_PLAIN, SWEEP_T3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+    if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, false, false, false, BS, IO_PLAIN, SWEEP_T3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
+  }
   constexpr int IOX = WKEY ? IO_AOS_OUT : (COLLIDE ? IO_GATHER : IO_PLAIN);   // the staged variant that exists for these flags
   if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, true, WKEY, BS, IOX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
   if ((e = cudaFuncSetAttribute(k_sweep<COLLIDE, true, false, WKEY, BS, IOX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes))) return e;
@@ -1542,6 +1557,7 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   G.nkeys = (uint32_t)nk;
   c->nbricks = (uint32_t)nbr;
   c->tile_bytes = tile_cells * TILE_W * 4;
+  c->three_ctas = 3 * (c->tile_bytes + 1024) <= 227 * 1024 && !getenv("MPC_SWEEP_2CTA");
   c->fast_brick = (G.bs[0] == 4 && G.bs[1] == 4 && G.bs[2] == 3);
   { const char* e = getenv("MPC_NO_FUSE_GATHER"); c->no_fuse_gather = (e && e[0] == '1'); }
   { const char* e = getenv("MPC_EAGER_CANONICAL"); c->eager_canonical = (e && e[0] == '1'); }
