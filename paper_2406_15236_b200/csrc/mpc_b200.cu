@@ -7,9 +7,13 @@
 //                  PAPER.md:29-37,68,70,176
 //   k_cell         PROCESS_CELLS: v_cm, axis, kappa, virtual wall particles
 //   k_collide_pos  trailing collision of the last step of an mpc_step call       Eqs. (2),(5)
-//   k_scan_* / k_scatter_slots / k_rank / k_gather*   counting-sort reorder by (key, id)
-//   k_stream_key / k_accum_at / k_collide_at        MPC-AT path (needs the rank of a particle in its
-//                  sorted cell segment, so it reorders every step and is not fused)
+//                  Variants IO_AOS_OUT / IO_GATHER fold a reorder into the sweeps of its own and the
+//                  next step through 32-byte staging records.
+//   k_scan_* / k_scatter_src (hot path: group by key) / k_scatter_slots + k_rank (rank by id) /
+//   k_rank_cells (lazy canonical order) / k_gather*   counting-sort reorder
+//   k_stream_key / k_accum_at / k_accum_a / k_accum_seg / k_cell_a / k_collide_at / k_collide_a
+//                  MPC-AT and +a path (needs the rank of a particle in its sorted cell segment or
+//                  22 sums per cell: not fused; per-cell segmented sums when the order is fresh)
 //   k_obs_*        observables
 // Cell sums are 32-bit fixed point (the paper's reproducibility option), two per
 // 64-bit word, added with integer atomics: order-independent, so a trajectory is bit-reproducible and
