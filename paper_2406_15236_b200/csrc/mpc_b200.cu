@@ -937,10 +937,10 @@ __device__ float mbs_energy(const Geo& G, uint32_t cid, uint32_t Nc, uint32_t wm
 // rec[key] = SRD: { vcm.x, vcm.y, vcm.z, kappa, n.x, n.y, n.z, - }   AT: { (vcm - mean v_ran).xyz, ... }
 // grid = (mb0 * CTAs-per-brick, mb1, mb2): the brick coordinates come from blockIdx, no division
 // zero != 0: the sums of a cell are cleared once read, which saves the memset before the next step's sweep
-__global__ void __launch_bounds__(128) k_cell(Geo G, int cpb_shift, u64* __restrict__ sums, float* __restrict__ rec, int zero) {
+// one cell: (bx, by, bz) = brick coordinates, local = index of the cell inside its brick
+__device__ __forceinline__ void cell_finalize(const Geo& G, uint32_t bx, uint32_t by, uint32_t bz, uint32_t local,
+                                              u64* __restrict__ sums, float* __restrict__ rec, int zero) {
   const int b0 = G.bs[0], b1 = G.bs[1], b2 = G.bs[2];
-  const uint32_t bx = blockIdx.x >> cpb_shift, by = blockIdx.y, bz = blockIdx.z;
-  const uint32_t local = ((blockIdx.x & ((1u << cpb_shift) - 1u)) << 7) | threadIdx.x;
   if (local >= (1u << (b0 + b1 + b2))) return;
   const uint32_t brick = (bz * (uint32_t)G.mb[1] + by) * (uint32_t)G.mb[0] + bx;
   const uint32_t k = (brick << (b0 + b1 + b2)) | local;
@@ -1009,6 +1009,10 @@ __global__ void __launch_bounds__(128) k_cell(Geo G, int cpb_shift, u64* __restr
   }
   reinterpret_cast<float4*>(rec)[(size_t)k * 2] = r0;
   reinterpret_cast<float4*>(rec)[(size_t)k * 2 + 1] = r1;
+}
+__global__ void __launch_bounds__(128) k_cell(Geo G, int cpb_shift, u64* __restrict__ sums, float* __restrict__ rec, int zero) {
+  cell_finalize(G, blockIdx.x >> cpb_shift, blockIdx.y, blockIdx.z, ((blockIdx.x & ((1u << cpb_shift) - 1u)) << 7) | threadIdx.x,
+                sums, rec, zero);
 }
 
 // ---- observables ---------------------------------------------------------------------------------
