@@ -272,11 +272,11 @@ def main():
         fam_bytes = kernel_algorithmic_bytes(dom, n, int(np.prod(cells)), nbar)
         ach = fam_bytes / (dms / dcnt * 1e-3) / 1e9
         # DRAM bytes of one launch of the steady-state sweep from the committed ncu --set full capture
-        # (profiles/r01c_ncu_full.md: dram__bytes_read.sum 41.06 GB + dram__bytes_write.sum 35.79 GB at config 5,
+        # (profiles/r01d_profile.md: dram__bytes_read.sum 41.59 GB + dram__bytes_write.sum 36.08 GB at config 5,
         # 10 particles per cell); other workloads have no capture: null
-        traffic = 76.85e9 if (dom == "sweep" and args.workload == "cfg5" and nbar == 10 and args.cells is None) else None
+        traffic = 77.67e9 if (dom == "sweep" and args.workload == "cfg5" and nbar == 10 and args.cells is None) else None
         roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                    "traffic": traffic, "traffic_source": "profiles/r01c_ncu_full.md" if traffic else None,
+                    "traffic": traffic, "traffic_source": "profiles/r01d_profile.md" if traffic else None,
                     "peak_source": peak_src, "avg_ms": dms / dcnt, "launches_timed": dcnt,
                     "algorithmic_bytes_per_launch": fam_bytes,
                     "step_frac_of_roofline": value / world * balg / 1e9 / peak,
