@@ -41,7 +41,8 @@ struct Params {
   float alpha;        // SRD rotation angle [rad]
   float dt, kT, mass;
   float g[3];         // constant acceleration
-  int   bc[3];        // 0 periodic, 1 no-slip walls at 0 and L
+  int   bc[3];        // 0 periodic, 1 no-slip walls at 0 and L (bounce-back + virtual wall particles), 2 slip walls
+                      // (specular reflection, no virtual particles; reading U20)
   int   grid_shift;   // 1 = random lattice shift every step
   int   rebin_every;  // reorder interval
   int   brick[3];     // brick dims of the brick-major key layout ({1,1,1} = row-major); memory order only
@@ -182,7 +183,7 @@ inline void advance(const Ctx& c, float r[3], float v[3], float tau) {
 inline void stream_one(const Ctx& c, float r[3], float v[3]) {
   const float h = c.p.dt;
   int w = -1;
-  for (int d = 0; d < 3; ++d) if (c.p.bc[d] == 1) w = d;   // at most one wall axis (create checks)
+  for (int d = 0; d < 3; ++d) if (c.p.bc[d] != 0) w = d;   // at most one wall axis (create checks)
   bool bounced = false;
   if (w >= 0) {
     const float z1 = fmaf(v[w], h, r[w]);
@@ -193,7 +194,8 @@ inline void stream_one(const Ctx& c, float r[3], float v[3]) {
       if (tc > h) tc = h;
       advance(c, r, v, tc);
       r[w] = zw;
-      v[0] = -v[0]; v[1] = -v[1]; v[2] = -v[2];            // bounce-back: v -> -v
+      if (c.p.bc[w] == 1) { v[0] = -v[0]; v[1] = -v[1]; v[2] = -v[2]; }   // no-slip, bounce-back: v -> -v
+      else v[w] = -v[w];                                                   // slip, specular reflection
       const float tr = h - tc;
       advance(c, r, v, tr);
       if (r[w] < 0.0f) r[w] = 0.0f;
@@ -502,8 +504,8 @@ int oracle_create(void** out, const float box[3], const int cells[3], float n_pe
   for (int d = 0; d < 3; ++d) if (p->brick[d] < 1) return E_INVAL;
   int nwall = 0;
   for (int d = 0; d < 3; ++d) {
-    if (p->bc[d] != 0 && p->bc[d] != 1) return E_INVAL;
-    if (p->bc[d] == 1) { nwall++; if (p->g[d] != 0.0f) return E_INVAL; }   // no force along the wall normal
+    if (p->bc[d] < 0 || p->bc[d] > 2) return E_INVAL;
+    if (p->bc[d] != 0) { nwall++; if (p->g[d] != 0.0f) return E_INVAL; }   // no force along the wall normal
   }
   if (nwall > 1) return E_INVAL;                                            // slit geometry only
   if (nwall && (p->conserve_L || p->collision == 1)) return E_INVAL;        // needs explicit phantom sets (U8)
@@ -515,7 +517,7 @@ int oracle_create(void** out, const float box[3], const int cells[3], float n_pe
   c->nkeys = 1;
   for (int d = 0; d < 3; ++d) {
     c->L[d] = box[d]; c->n[d] = cells[d];
-    c->m[d] = cells[d] + (p->bc[d] == 1 ? 2 : 0);
+    c->m[d] = cells[d] + (p->bc[d] != 0 ? 2 : 0);
     c->B[d] = p->brick[d];
     c->mb[d] = (c->m[d] + c->B[d] - 1) / c->B[d];
     c->nkeys *= (size_t)c->mb[d] * (size_t)c->B[d];
@@ -616,7 +618,7 @@ int oracle_observables(void* h, Obs* o, float* profile) {
   }
   if (profile) {
     int pa = 2, fa = 0;
-    for (int d = 0; d < 3; ++d) if (c->p.bc[d] == 1) pa = d;
+    for (int d = 0; d < 3; ++d) if (c->p.bc[d] != 0) pa = d;
     for (int d = 2; d >= 0; --d) if (c->p.g[d] != 0.0f) fa = d;
     const int nb = c->n[pa];
     std::vector<double> sv(nb, 0.0), cnt(nb, 0.0);

@@ -129,3 +129,62 @@ def test_poiseuille_profile_matches_analytic_viscosity():
     assert abs(prof - prof[::-1]).max() < 0.02                 # symmetric
     ob = o.observables()
     assert ob["kT_cell"] == pytest.approx(1.0, rel=0.03)        # thermostat holds k_BT under forcing
+
+
+# ---- slip walls: specular reflection, no virtual wall particles (reading U20) ----------
+
+def test_specular_reflection_hand_cases():
+    o = Oracle((8, 8, 8), (8, 8, 8), 10, 1, bc=(0, 0, 2), dt=0.1, thermostat=1)
+    # hits z = 0 after half the step: only the normal component is reversed, the tangential motion goes on
+    r, v = o.stream_one([3.0, 4.0, 0.05], [0.5, -0.25, -1.0])
+    assert np.allclose(r, [3.05, 3.975, 0.05], atol=3e-7)
+    assert np.array_equal(v, np.array([0.5, -0.25, 1.0], np.float32))
+    # upper wall: wall at t = 0.02, 0.08 back
+    r, v = o.stream_one([3.0, 4.0, 7.98], [1.0, 0.0, 1.0])
+    assert r[2] == pytest.approx(7.92, abs=1e-6) and v[2] == -1.0 and v[0] == 1.0
+    assert r[0] == pytest.approx(3.1, abs=1e-6)
+    # no crossing: plain streaming
+    r, v = o.stream_one([3.0, 4.0, 4.0], [0.0, 0.0, 1.0])
+    assert r[2] == pytest.approx(4.1, abs=1e-6) and v[2] == 1.0
+
+
+def test_slip_walls_are_frictionless():
+    # Between slip walls nothing exchanges tangential momentum with the walls (specular reflection keeps the
+    # tangential components, there are no virtual wall particles, collisions conserve momentum per cell), so
+    # (1) without force and thermostat: tangential momentum and kinetic energy are conserved to rounding, the
+    #     wall-normal momentum is not;
+    # (2) with a body force g along x the whole fluid accelerates as one: P_x(t) = N m g t exactly (to rounding),
+    #     and the profile stays flat (plug flow), unlike the no-slip parabola.
+    box, cells, nbar = (8.0, 8.0, 8.0), (8, 8, 8), 10
+    n = 8 * 8 * 8 * nbar
+    st = uniform_maxwell(box, n, 11)
+    o = Oracle(box, cells, nbar, 5, bc=(0, 0, 2))
+    o.set_state(*st)
+    a = o.observables()
+    o.step(40)
+    b = o.observables()
+    assert abs(b["P"][0] - a["P"][0]) < 2e-3 and abs(b["P"][1] - a["P"][1]) < 2e-3
+    assert abs(b["P"][2] - a["P"][2]) > 1.0                           # the walls do take normal momentum
+    assert b["E_kin"] == pytest.approx(a["E_kin"], rel=2e-6)
+    assert b["n"] == n
+
+    g, h, steps = 0.01, 0.1, 200
+    o = Oracle(box, cells, nbar, 5, bc=(0, 0, 2), g=(g, 0, 0), thermostat=1)
+    o.set_state(*st)
+    p0 = o.observables()["P"][0]
+    o.step(steps)
+    ob = o.observables(8)
+    assert ob["P"][0] - p0 == pytest.approx(n * g * steps * h, rel=1e-5)
+    prof = ob["profile"]
+    assert np.abs(prof - g * steps * h).max() < 0.08                  # flat: thermal noise of 640 particles per layer
+    assert abs(prof[:2].mean() - prof[3:5].mean()) < 0.08             # no wall layer lagging behind
+
+
+def test_slip_wall_cells_get_no_virtual_particles():
+    # one particle alone in a wall-cut cell: with no-slip walls it collides with nbar-1 virtual particles
+    # (test above), with slip walls it is alone and keeps its velocity
+    o = Oracle((8, 8, 8), (8, 8, 8), 10, 1, bc=(0, 0, 2), thermostat=1)
+    o.set_state([0.7], [1.2], [0.02], [0.3], [-0.4], [0.5], step=0)
+    o.step(1)
+    *_p, vx, vy, vz, _ = o.get_state()
+    assert (vx[0], vy[0], vz[0]) == (np.float32(0.3), np.float32(-0.4), np.float32(0.5))
