@@ -54,7 +54,9 @@ typedef struct {
   float kT;          /* k_B T of the thermostat / of virtual wall particles / of MPC-AT                */
   float mass;        /* particle mass m (all fluid particles are identical)               */
   float g[3];        /* constant acceleration (force / mass); must be 0 along a wall normal            */
-  int   bc[3];       /* per axis: 0 = periodic; 1 = no-slip walls at 0 and L (at most one wall axis)   */
+  int   bc[3];       /* per axis: 0 = periodic; 1 = no-slip walls at 0 and L: bounce-back v -> -v plus      */
+                     /* virtual wall particles in wall-cut cells; 2 = slip walls: specular reflection, no  */
+                     /* virtual particles (U7, U8, U20). At most one wall axis       */
   int   grid_shift;  /* 1 = random lattice shift in [-a/2,a/2)^3 every step; 0 = off     */
   int   rebin_every; /* reorder when step % rebin_every == 0; >= 1; MPC-AT requires 1                  */
   int   brick[3];    /* brick dims (powers of two <= 64) of the brick-major memory key; {1,1,1} = row-major.

@@ -64,8 +64,9 @@ struct Geo {
   int m[3];       // cell layers incl. wall layers
   int mb[3];      // bricks per axis
   int bs[3];      // log2(brick dims)
-  int bc[3];
+  int bc[3];      // 0 periodic, 1 no-slip walls, 2 slip walls
   int wall;       // wall axis or -1
+  int slip;       // 1: the walls reflect specularly and have no virtual particles (U20)
   float g[3];
   float dt;
   float s[3];     // lattice shift of this step
@@ -167,7 +168,9 @@ __device__ __forceinline__ void stream_one(const Geo& G, float (&r)[3], float (&
       tc = fminf(fmaxf(tc, 0.0f), G.dt);
       advance<GRAV>(G, r, v, tc);
       if (w == 0) r[0] = zw; else if (w == 1) r[1] = zw; else r[2] = zw;
-      v[0] = -v[0]; v[1] = -v[1]; v[2] = -v[2];
+      if (G.slip) {   // specular reflection: only the wall-normal component turns round
+        if (w == 0) v[0] = -v[0]; else if (w == 1) v[1] = -v[1]; else v[2] = -v[2];
+      } else { v[0] = -v[0]; v[1] = -v[1]; v[2] = -v[2]; }   // bounce-back
       advance<GRAV>(G, r, v, G.dt - tc);
       if (w == 0) r[0] = fminf(fmaxf(r[0], 0.0f), Lw);
       else if (w == 1) r[1] = fminf(fmaxf(r[1], 0.0f), Lw);
@@ -970,7 +973,7 @@ __device__ __forceinline__ void cell_finalize(const Geo& G, uint32_t bx, uint32_
   } else {
     double E = (double)(w0 >> 16) * G.fxe_inv;
     uint32_t Nc = nreal;
-    if (G.wall >= 0) {
+    if (G.wall >= 0 && !G.slip) {
       // virtual wall particles fill wall-cut cells up to nbar (U8)
       const int w = G.wall;
       const int iw = (w == 0) ? ix : (w == 1) ? iy : iz;
@@ -1536,8 +1539,8 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   if (tile_cells * TILE_W * 4 > MAX_TILE_BYTES) return MPC_EINVAL;
   int nwall = 0, wall = -1;
   for (int d = 0; d < 3; ++d) {
-    if (p->bc[d] != 0 && p->bc[d] != 1) return MPC_EINVAL;
-    if (p->bc[d] == 1) { nwall++; wall = d; if (p->g[d] != 0.0f) return MPC_EINVAL; }
+    if (p->bc[d] < 0 || p->bc[d] > 2) return MPC_EINVAL;
+    if (p->bc[d] != 0) { nwall++; wall = d; if (p->g[d] != 0.0f) return MPC_EINVAL; }
   }
   if (nwall > 1) return MPC_EINVAL;
   if (nwall && (p->conserve_L || p->collision == 1)) return MPC_EINVAL;
@@ -1549,14 +1552,14 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   c->hbuf = new (std::nothrow) double[OBS_HOST_DOUBLES];
   if (!c->hbuf) { delete c; return MPC_ENOMEM; }
   Geo& G = c->G;
-  G.a = a; G.inv_a = 1.0f / a; G.wall = wall;
+  G.a = a; G.inv_a = 1.0f / a; G.wall = wall; G.slip = (wall >= 0 && p->bc[wall] == 2) ? 1 : 0;
   unsigned long long nk = 1, nbr = 1;
   for (int d = 0; d < 3; ++d) {
     int bs = 0;
     while ((1 << bs) < p->brick[d]) ++bs;
     G.bs[d] = bs;
     G.L[d] = box[d]; G.n[d] = cells[d]; G.bc[d] = p->bc[d]; G.g[d] = p->g[d];
-    G.m[d] = cells[d] + (p->bc[d] == 1 ? 2 : 0);
+    G.m[d] = cells[d] + (p->bc[d] != 0 ? 2 : 0);
     G.mb[d] = (G.m[d] + p->brick[d] - 1) >> bs;
     nk *= (unsigned long long)G.mb[d] << bs;
     nbr *= (unsigned long long)G.mb[d];
@@ -1677,7 +1680,7 @@ int mpc_observables(mpc_ctx* c, mpc_obs* out, float* profile_host) {
   double* part = c->obs;
   double* prof = c->obs + (size_t)OBS_BLOCKS * 8;
   int pa = 2, fa = 0;
-  for (int d = 0; d < 3; ++d) if (G.bc[d] == 1) pa = d;
+  for (int d = 0; d < 3; ++d) if (G.bc[d] != 0) pa = d;
   for (int d = 2; d >= 0; --d) if (G.g[d] != 0.0f) fa = d;
   const int nb = G.n[pa];
   if (profile_host && nb > MAX_PROFILE) return fail(c, MPC_EINVAL, "profile axis longer than 2048 layers");

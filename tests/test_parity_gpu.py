@@ -79,6 +79,9 @@ CASES = {
     "srd_brick_4x2x1_ragged": dict(cells=(10, 7, 5), nbar=6, kw=dict(thermostat=1, brick=(4, 2, 1))),
     "walls_gravity_brick16x16x8": dict(cells=(16, 16, 16), nbar=10,
                                        kw=dict(thermostat=1, bc=(0, 0, 1), g=(0.001, 0, 0), brick=(16, 16, 8))),
+    # slip walls (specular reflection, no virtual particles; U20)
+    "slip_walls_gravity": dict(cells=(16, 8, 8), nbar=10, kw=dict(thermostat=1, bc=(0, 0, 2), g=(0.01, 0, 0))),
+    "slip_walls_y_brick16x16x8": dict(cells=(16, 16, 16), nbar=10, kw=dict(bc=(0, 2, 0), dt=0.3, brick=(16, 16, 8))),
 }
 
 
@@ -98,7 +101,7 @@ def test_single_step_parity(name):
     compare_step(o, g, a=a)
 
 
-@pytest.mark.parametrize("name", ["cfg1_srd", "srd_mbs_brick4", "at", "walls_gravity"])
+@pytest.mark.parametrize("name", ["cfg1_srd", "srd_mbs_brick4", "at", "walls_gravity", "slip_walls_gravity"])
 def test_lockstep_parity_many_steps(name):
     # U15: after every step the oracle state is copied to the GPU, then both advance one step
     c = CASES[name]
@@ -351,3 +354,21 @@ def test_reorder_code_paths_agree(kw, monkeypatch):
     for r in res[1:]:
         for x, y in zip(res[0], r):
             assert np.array_equal(x, y)
+
+
+def test_slip_walls_plug_flow_on_gpu():
+    # frictionless walls: under a body force the fluid accelerates as one, P_x(t) = N m g t to rounding, in a
+    # multi-step call (fused sweep, staged reorder) as well; the same law pins the oracle (test_oracle_walls.py)
+    cells, nbar = (32, 16, 16), 10
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    gx, h, steps = 0.01, 0.1, 200
+    st = uniform_maxwell(box, n, 12)
+    g = MPC(box, cells, nbar, 9, n_max=n, thermostat=1, bc=(0, 0, 2), g=(gx, 0, 0), rebin_every=10, brick=(16, 16, 8))
+    gpu_set(g, st)
+    p0 = g.observables()["P"][0]
+    g.step(steps)
+    ob = g.observables(16)
+    assert ob["P"][0] - p0 == pytest.approx(n * gx * steps * h, rel=2e-5)
+    assert np.abs(ob["profile"] - gx * steps * h).max() < 0.03          # flat profile (5,120 particles per layer)
+    assert ob["kT_cell"] == pytest.approx(1.0, rel=1e-2)
