@@ -1231,14 +1231,16 @@ int apply_perm(mpc_ctx* c, bool need_key) {
     for (int a = 0; a < 7; ++a) { uint32_t* t = c->A[a]; c->A[a] = c->Bf[a]; c->Bf[a] = t; }
     if (need_key) CU(cudaMemcpyAsync(c->key, c->slot_id, n * 4, cudaMemcpyDeviceToDevice, c->stream));
   } else {
-    // property-wise through one temporary array
+    // property-wise through one temporary array: each property is gathered into the spare array,
+    // which then takes its place; the array it came from is the spare for the next property (no copy back)
     Arrays8 src, dst;
     for (int a = 0; a < (need_key ? 8 : 7); ++a) {
-      uint32_t* arr = a < 7 ? c->A[a] : c->key;
-      CU(cudaMemcpyAsync(c->Bf[0], arr, n * 4, cudaMemcpyDeviceToDevice, c->stream));
-      src.p[0] = c->Bf[0]; dst.p[0] = arr;
+      uint32_t*& arr = a < 7 ? c->A[a] : c->key;
+      src.p[0] = arr; dst.p[0] = c->Bf[0];
       k_gather<1><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
       LAUNCH_CHECK("k_gather");
+      uint32_t* t = arr; arr = c->Bf[0];
+      for (int b = 0; b < 7; ++b) c->Bf[b] = t;     // compact mode: all seven alias the one spare array
     }
   }
   return MPC_OK;
