@@ -75,3 +75,33 @@ def test_no_cpu_fallback_without_library(monkeypatch):
     monkeypatch.setattr(binding, "LIB_PATH", "/nonexistent/libmpc_b200.so")
     with pytest.raises(binding.MPCError):
         binding.load()
+
+
+def test_wall_kinds_are_validated(lib):
+    # bc: 0 periodic, 1 no-slip, 2 slip (reading U20); anything else, two wall axes, a force along the wall normal,
+    # or walls with MPC-AT / +a (would need explicit phantom sets, U8) are rejected
+    for bc, extra, ok in (((0, 0, 2), {}, True), ((2, 0, 0), {}, True), ((0, 0, 3), {}, False), ((0, 1, 2), {}, False),
+                          ((0, 0, 2), dict(g=(0.0, 0.0, 0.1)), False), ((0, 0, 2), dict(collision=1), False),
+                          ((0, 0, 2), dict(conserve_L=1), False)):
+        rc, h = _create(lib, bc=bc, **extra)
+        assert (rc == 0) == ok, (bc, extra, rc)
+        if rc == 0:
+            nk = C.c_ulonglong()
+            assert lib.mpc_num_keys(h, C.byref(nk)) == 0 and nk.value == 8 * 8 * 10      # two extra layers on the wall axis
+            lib.mpc_destroy(h)
+
+
+def test_workspace_sizes(lib):
+    # the compact workspace has no second copy of the particle arrays; both grow linearly with n_max
+    rc, h = _create(lib)
+    assert rc == 0
+    full, comp, full2 = C.c_size_t(), C.c_size_t(), C.c_size_t()
+    assert lib.mpc_workspace_bytes(h, 1 << 20, 0, C.byref(full)) == 0
+    assert lib.mpc_workspace_bytes(h, 1 << 20, 1, C.byref(comp)) == 0
+    assert lib.mpc_workspace_bytes(h, 1 << 21, 0, C.byref(full2)) == 0
+    n = 1 << 20
+    assert comp.value < full.value
+    assert 17 * 4 * n <= full.value <= 17 * 4 * n + (1 << 20)        # 7 + 7 arrays, slot, key, perm, + cell data
+    assert 12 * 4 * n <= comp.value <= 12 * 4 * n + (1 << 20)        # 7 arrays, 8-byte slots, spare, key, perm
+    assert full2.value - full.value == 17 * 4 * n
+    lib.mpc_destroy(h)
