@@ -166,3 +166,36 @@ def test_config5_sampled_cells_512cubed():
         assert np.max(np.abs(got - psum)) / l1 <= 1e-5
         tested += 1
     assert tested > 250
+
+
+def test_config5_fused_call_equals_single_steps_512cubed():
+    # At config 5's full size, in the launch configuration bench.py times: one call of 4 steps (first-step sweep, the
+    # steady-state 3-CTA sweep with the collision of the previous step fused in, the staged reorder pair around
+    # t = 10) must leave bit for bit the state that 4 calls of one step leave (unfused: sweep, cell, trailing collide
+    # each; that path is the one checked against the oracle cell by cell above and in lock-step at small sizes).
+    free, _total = torch.cuda.mem_get_info()
+    if free < 150e9:
+        pytest.skip("needs ~150 GB of device memory")
+    cells, nbar, seed = (512, 512, 512), 10, 1234
+    box = (512.0,) * 3
+    n = 512**3 * nbar
+    kw = dict(thermostat=1, rebin_every=10, brick=BRICK)
+    st = uniform_maxwell_cuda(box, n, seed)
+    g = MPC(box, cells, nbar, seed, n_max=n, **kw)
+    g.set_state(*st, step=8)                     # t = 8, 9 plain; t = 10 reorder (staged in the fused call); t = 11 gather
+    torch.cuda.synchronize()
+    del st
+    torch.cuda.empty_cache()
+    g.step(1)                                    # t = 8: brings the particles into the library's order once
+    pre = [t.cpu() for t in g.get_state()]       # host copy of the state at t = 9
+    torch.cuda.empty_cache()
+    for _ in range(4):
+        g.step(1)                                # t = 9, 10, 11, 12, one call each
+    ref = [t.cpu() for t in g.get_state()]
+    torch.cuda.empty_cache()
+    g.set_state_host(*[t.numpy() for t in pre[:6]], id=pre[6].numpy(), step=9)
+    g.step(4)                                    # the same four steps in one call
+    got = g.get_state()
+    for a, b in zip(ref, got):
+        assert torch.equal(a, b.cpu())
+    assert g.observables()["step"] == 13
