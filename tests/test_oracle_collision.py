@@ -123,6 +123,31 @@ def test_mbs_energy_sampler_is_gamma(Nc):
     assert o.mbs_energy(0, 0, 1) == 0.0
 
 
+def test_mbs_energy_stream_layout_from_raw_philox_words():
+    # Reading U6 fixes WHICH random words make E_k: word j of the cell's TAG_MBS (=2) blocks
+    # sub = 0, 1, ... in order for the floor(f/2) exponentials, words 2 and 3 of the cell's TAG_AXIS (=1)
+    # block for the half squared normal when f is odd. Recomputed here from raw blocks of the
+    # known-answer-pinned generator, so any change of the stream layout (tag, sub order, word order,
+    # open/closed interval) fails.
+    from oracle.binding import philox
+    seed = 0x1234_5678_9ABC_DEF0
+    o = Oracle((4, 4, 4), (4, 4, 4), 10, seed)
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    u_oc = lambda w: (float(w >> 8) + 1.0) / 16777216.0
+    u_co = lambda w: float(w >> 8) / 16777216.0
+    for cid, t, Nc in [(0, 0, 2), (5, 3, 3), (63, 7, 4), (17, 100, 10), (40, 2, 11), (9, 9, 26)]:
+        f = 3 * (Nc - 1)
+        M = f // 2
+        words = []
+        for sub in range((M + 3) // 4):
+            words += [int(w) for w in philox([cid, sub, t, 2], key)]
+        e = -sum(np.log(u_oc(w)) for w in words[:M])
+        if f % 2:
+            a = philox([cid, 0, t, 1], key)
+            e += -np.log(u_oc(int(a[2]))) * np.cos(2 * np.pi * u_co(int(a[3]))) ** 2
+        assert o.mbs_energy(cid, t, Nc) == pytest.approx(e, rel=1e-13)
+
+
 def test_mbs_thermostat_sets_temperature():
     # start far from k_BT = 1: the cell-level thermostat must bring <m sum w^2 / 3(Nc-1)> to k_BT
     box = (8.0,) * 3
@@ -242,9 +267,16 @@ def test_at_momentum_and_temperature():
     ob = o.observables()
     # relative velocities are fresh N(0,1) with (Nc-1)/Nc of the variance; cm motion keeps 3.0/Nc -> relaxes
     assert ob["kT_cell"] == pytest.approx(1.0, rel=0.03)
+    # what MPC-AT sets (reading U5): the post-collision relative velocities of a cell are fresh normals minus
+    # their mean, so per component sum_cells sum_i w_d^2 / sum_cells (N_c - 1) = kT/m. The keys of the last step
+    # are the cells the collision happened in (positions do not change after the collision).
     *_p, vx, vy, vz, ids = o.get_state()
-    # per-cell relative temperature is what AT sets, check component variance of w
-    key = o.get_cells()[5]
+    cnt, *_s, key = o.get_cells()
+    dof = (cnt[cnt >= 1].astype(np.float64) - 1.0).sum()
+    for v in (vx, vy, vz):
+        vcm = cell_sums(key, o.nkeys, v)[0] / np.maximum(cnt, 1)
+        w = v.astype(np.float64) - vcm[key]
+        assert (w * w).sum() / dof == pytest.approx(1.0, rel=0.08)
 
 
 def test_at_random_velocities_are_standard_normal():

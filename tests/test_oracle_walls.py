@@ -102,6 +102,71 @@ def test_virtual_wall_particles_recomputed_by_hand():
     assert (vx[0], vy[0], vz[0]) == (np.float32(0.3), np.float32(-0.4), np.float32(0.5))
 
 
+def test_kappa_in_a_wall_cut_cell_counts_virtual_particles():
+    # PAPER.md:54-68 (Eqs. 5-7 + "Boundary conditions"), reading U8: in a wall-cut cell the thermostat sees the
+    # virtual particles too: v_cm, sum |v - v_cm|^2 and f = 3(N_c - 1) are taken over real + virtual particles
+    # (N_c = nbar). One real particle + nbar-1 virtual ones, thermostat ON; everything recomputed in numpy from
+    # the RNG hooks. Dropping the virtual terms from W2, or using the real count in f, fails this.
+    nbar, kT = 6, 0.7
+    o = Oracle((2.0, 2.0, 2.0), (2, 2, 2), nbar, 19, bc=(0, 0, 1), dt=1e-30, kT=kT, thermostat=1)
+    t = 0
+    while o.grid_shift(t)[2] <= 0:
+        t += 1
+    s = o.grid_shift(t)
+    r = np.array([1.3, 0.4, 0.07], np.float32)
+    v = np.array([-0.6, 0.2, 0.9], np.float32)
+    ijk, cid, _key, _ = o.cell_of(r, s)
+    assert ijk[2] == 1
+    o.set_state([r[0]], [r[1]], [r[2]], [v[0]], [v[1]], [v[2]], step=t)
+    o.step(1)
+    *_p, vx, vy, vz, _ = o.get_state()
+    sig = np.sqrt(kT)
+    virt = sig * np.array([o.normals(cid, k, t, 4)[:3] for k in range(nbar - 1)])
+    allv = np.vstack([v.astype(np.float64), virt])
+    vcm = allv.mean(0)
+    W2 = ((allv - vcm) ** 2).sum()                             # real + virtual
+    Ek = kT * o.mbs_energy(cid, t, nbar)                       # Gamma(3(nbar-1)/2) draw for N_c = nbar
+    kappa = np.sqrt(2.0 * Ek / W2)                             # Eq. (6), m = 1
+    ax = o.srd_axis(cid, t)
+    w = v - vcm
+    a = np.deg2rad(np.float32(130.0)).astype(np.float32).astype(np.float64)
+    wr = w * np.cos(a) + np.cross(ax, w) * np.sin(a) + ax * (ax @ w) * (1 - np.cos(a))
+    want = vcm + kappa * wr
+    assert np.allclose([vx[0], vy[0], vz[0]], want, atol=3e-7)
+    # the two plausible misreadings give measurably different answers for this case
+    W2_real = ((v - vcm) ** 2).sum()
+    assert abs(np.sqrt(2.0 * Ek / W2_real) - kappa) > 1e-2
+    assert abs(o.mbs_energy(cid, t, 1 + 1) - o.mbs_energy(cid, t, nbar)) > 1e-2
+
+
+@pytest.mark.parametrize("bc", [1, 2])
+def test_wall_hit_with_gravity_closed_form(bc):
+    # PAPER.md:68 (bounce-back / specular reflection) with PAPER.md:70 (constant acceleration), readings U7/U20:
+    # the particle flies ballistically under g for t_c, is reflected AT the wall, and flies for h - t_c.
+    # x0 = 3, v = (0.5, -0.25, -1), z0 = 0.03 -> t_c = 0.03 of h = 0.1; g = 2 along x.
+    g, h = 2.0, 0.1
+    o = Oracle((8, 8, 8), (8, 8, 8), 10, 1, bc=(0, 0, bc), dt=h, g=(g, 0, 0), thermostat=1)
+    r0 = np.array([3.0, 4.0, 0.03])
+    v0 = np.array([0.5, -0.25, -1.0])
+    r, v = o.stream_one(r0, v0)
+    tc, tr = 0.03, 0.07
+    x1 = r0[0] + v0[0] * tc + 0.5 * g * tc * tc
+    vx1 = v0[0] + g * tc
+    y1 = r0[1] + v0[1] * tc
+    if bc == 1:      # bounce-back: every component reverses at the wall
+        want_r = [x1 - vx1 * tr + 0.5 * g * tr * tr, y1 - v0[1] * tr, 1.0 * tr]
+        want_v = [-vx1 + g * tr, -v0[1], 1.0]
+    else:            # specular: only the normal component reverses; the tangential flight is the free one
+        want_r = [r0[0] + v0[0] * h + 0.5 * g * h * h, r0[1] + v0[1] * h, 1.0 * tr]
+        want_v = [v0[0] + g * h, v0[1], 1.0]
+    assert np.allclose(r, want_r, atol=1e-6)
+    assert np.allclose(v, want_v, atol=1e-6)
+    # and without a wall hit: plain ballistic flight with the half-step velocity
+    r, v = o.stream_one([3.0, 4.0, 4.0], v0)
+    assert np.allclose(r, [3.0 + 0.5 * h + 0.5 * g * h * h, 4.0 - 0.25 * h, 4.0 - h], atol=1e-6)
+    assert np.allclose(v, [0.5 + g * h, -0.25, -1.0], atol=1e-6)
+
+
 @pytest.mark.slow
 def test_poiseuille_profile_matches_analytic_viscosity():
     # gravity + two walls -> parabola; nu = 0.870 for <N_c>=10, h=0.1, alpha=130 deg.
