@@ -31,7 +31,8 @@ WORKLOADS = {
     "cfg1": dict(cells=(16, 16, 16), nbar=10, kw=dict(), rebin_every=1),
     "cfg2": dict(cells=(64, 64, 64), nbar=10, kw=dict(thermostat=1), rebin_every=1),
     "cfg3": dict(cells=(128, 128, 128), nbar=10, kw=dict(collision=1, conserve_L=1, dt=0.02), rebin_every=1),
-    "cfg4": dict(cells=(256, 64, 64), nbar=10, kw=dict(thermostat=1, bc=(0, 0, 1), g=(0.001, 0, 0)), rebin_every=1),
+    # config 4 does not name a reorder interval: 10, the value of its full-length test (tests/test_configs_freerun_gpu.py)
+    "cfg4": dict(cells=(256, 64, 64), nbar=10, kw=dict(thermostat=1, bc=(0, 0, 1), g=(0.001, 0, 0)), rebin_every=10),
     "cfg5": dict(cells=(512, 512, 512), nbar=10, kw=dict(thermostat=1), rebin_every=10),
 }
 # algorithmic bytes per particle-step (SURVEY.md 8d / DESIGN.md "Roofline"): read r,v 24 B + write r,v 24 B
@@ -154,58 +155,53 @@ def run_reference(args, wl, rank, world):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": args.workload, "cells": list(wl["cells"]), "n_per_cell": nbar,
                        "note": "CPU oracle (oracle/mpc_oracle.cpp, single thread) timed on a bounded sample of the workload"},
-            "cpu_baseline": {"value": val, "unit": "particle-updates/s", "cores": 1, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": "particle-updates/s", "cores": 1, "host_cores": os.cpu_count(), "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": "particle-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=30)
-    ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS))
-    ap.add_argument("--nbar", type=int, default=None, help="particles per cell (cfg5 sweep: 5, 10, 20)")
-    ap.add_argument("--brick", default="16,16,8", help="brick dims of the memory key, e.g. 16,16,8")
-    ap.add_argument("--rebin-every", type=int, default=None)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--compact", action="store_true", help="property-wise reorder workspace")
-    ap.add_argument("--cells", default=None, help="override the workload's cell grid, e.g. 256,256,256 (profiling runs)")
-    args = ap.parse_args()
-    wl = dict(WORKLOADS[args.workload])
-    if args.nbar is None:
-        args.nbar = wl["nbar"]
-    if args.rebin_every is not None:
-        wl["rebin_every"] = args.rebin_every
-    if args.cells:
-        wl["cells"] = tuple(int(t) for t in args.cells.split(","))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+def csrc_digest():
+    """sha256 over the CUDA sources: ties a committed ncu capture to the code it was taken from."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2406_15236_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
 
-    if args.impl == "reference":
-        run_reference(args, wl, rank, world)
-        return
 
+def captured_traffic(family, workload, nbar):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of a kernel family from the committed
+    `ncu --set full` capture (profiles/traffic.json, written by hand from the capture named there). Returns
+    (bytes or None, source, stale): stale = the capture was taken from other CUDA sources than the ones built now."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None, None, None
+    t = json.load(open(p))
+    e = t.get("kernels", {}).get(f"{family}:{workload}:nbar{nbar}")
+    if e is None:
+        return None, None, None
+    return float(e["dram_bytes_per_launch"]), e.get("source"), e.get("csrc_digest") != csrc_digest()
+
+
+def measure(args, workload, nbar, steps, warmup, rank, local_rank, world, dist, with_e2e, rebin_every=None, cells_override=None):
+    """One workload: W untimed warm-up steps, then EXACTLY K steps in one mpc_step call between two CUDA events on
+    the launching stream. Returns the JSON-able result dict (without cpu_baseline)."""
     import torch
 
     from paper_2406_15236_b200 import MPC
     from paper_2406_15236_b200.inputs import uniform_maxwell_cuda
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        torch.cuda.set_device(local_rank)
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    wl = dict(WORKLOADS[workload])
+    if rebin_every is not None:
+        wl["rebin_every"] = rebin_every
+    if cells_override:
+        wl["cells"] = cells_override
     device = torch.device(f"cuda:{local_rank}")
-    torch.cuda.set_device(device)
-
-    cells, nbar = wl["cells"], args.nbar
+    cells = wl["cells"]
     box = tuple(float(c) for c in cells)
     n = int(np.prod(cells)) * nbar
     kw = dict(wl["kw"])
@@ -239,7 +235,10 @@ def main():
             torch.cuda.synchronize()
 
     # ---- warm-up (untimed), then EXACTLY K timed steps, CUDA events on the launching stream ----
-    sim.step(args.warmup)
+    # The collision of the last step of a call stays pending and is applied inside the next call's first streaming
+    # pass: the timed call applies the warm-up's last collision and leaves its own last one pending,
+    # i.e. exactly K collisions, K streaming passes, K cell passes are inside the timed region.
+    sim.step(warmup)
     barrier()
     sim.profile_enable(True)
     sim.profile_read()
@@ -248,7 +247,7 @@ def main():
     with ClockSampler(local_rank) as clocks:
         barrier()
         ev0.record(sim.stream)
-        sim.step(args.steps)
+        sim.step(steps)
         ev1.record(sim.stream)
         barrier()
     ms = ev0.elapsed_time(ev1)
@@ -257,7 +256,7 @@ def main():
     sim.profile_enable(False)
     ms = max_over_ranks(dist, ms, device)
     ob = sim.observables()
-    value = whole_job_rate(world, n, args.steps, ms)
+    value = whole_job_rate(world, n, steps, ms)
 
     # ---- roofline of the dominant kernel family (live CUDA-event times from the timed region) ----
     peak, peak_src = measured_peaks()
@@ -268,43 +267,113 @@ def main():
     roofline = None
     if dom:
         dms, dcnt = fam[dom]
-        # per launch of the dominant kernel: its share of the step's algorithmic bytes
         fam_bytes = kernel_algorithmic_bytes(dom, n, int(np.prod(cells)), nbar)
         ach = fam_bytes / (dms / dcnt * 1e-3) / 1e9
-        # DRAM bytes of one launch of the steady-state sweep from the committed ncu --set full capture
-        # (profiles/r01d_profile.md: dram__bytes_read.sum 41.59 GB + dram__bytes_write.sum 36.08 GB at config 5,
-        # 10 particles per cell); other workloads have no capture: null
-        traffic = 77.67e9 if (dom == "sweep" and args.workload == "cfg5" and nbar == 10 and args.cells is None) else None
+        traffic, tsrc, stale = captured_traffic(dom, workload, nbar) if cells_override is None else (None, None, None)
         roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                    "traffic": traffic, "traffic_source": "profiles/r01d_profile.md" if traffic else None,
+                    "traffic": traffic, "traffic_source": tsrc, "traffic_capture_is_of_other_sources": stale,
                     "peak_source": peak_src, "avg_ms": dms / dcnt, "launches_timed": dcnt,
                     "algorithmic_bytes_per_launch": fam_bytes,
                     "step_frac_of_roofline": value / world * balg / 1e9 / peak,
                     "step_frac_of_8000": value / world * balg / 1e9 / 8000.0,
-                    "family_ms_per_step": {k: v[0] / args.steps for k, v in sorted(fam.items(), key=lambda kv: -kv[1][0])},
+                    "family_ms_per_step": {k: v[0] / steps for k, v in sorted(fam.items(), key=lambda kv: -kv[1][0])},
                     "family_share": {k: v[0] / total_fam_ms for k, v in fam.items()}}
+    res = {"value": value, "ms_per_step": ms / steps, "steps": steps, "warmup": warmup, "gpu_launches": int(launches),
+           "clocks": clocks.summary(), "roofline": roofline,
+           "config": {"workload": workload, "cells": list(cells), "n_per_cell": nbar, "particles": n,
+                      "collision": "MPC-AT" if kw.get("collision") else "SRD", "conserve_L": bool(kw.get("conserve_L", 0)),
+                      "thermostat": bool(kw.get("thermostat", 0)),
+                      "rebin_every": wl["rebin_every"], "brick": list(brick), "compact_workspace": bool(compact),
+                      "l2": "inputs larger than L2 (no flush)" if n * 24 > 4 * 126e6 else "state fits in L2; HBM fraction not meaningful",
+                      "parallelism": "replicas only" if world > 1 else "single GPU",
+                      "algorithmic_bytes_per_update": balg,
+                      "collisions_in_timed_region": "K (the warm-up's last collision is applied by the first timed sweep, the last timed one stays pending)"},
+           "check": {"kT_cell": ob["kT_cell"], "kT_est": ob["kT_est"], "max_cell_count": ob["max_cell_count"], "step": ob["step"],
+                     "n_range_overflows": ob["n_range_overflows"]}}
+    if with_e2e:
+        res["e2e"] = run_e2e(sim, n, steps)
+    sim.close()
+    del sim
+    torch.cuda.empty_cache()
+    return res, wl
 
-    line = {"metric": "MPC particle-updates/sec", "value": value, "unit": "particle-updates/s", "n_gpus": world,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS))
+    ap.add_argument("--nbar", type=int, default=None, help="particles per cell (cfg5 sweep: 5, 10, 20)")
+    ap.add_argument("--brick", default="16,16,8", help="brick dims of the memory key, e.g. 16,16,8")
+    ap.add_argument("--rebin-every", type=int, default=None)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the density sweep and the other workloads")
+    ap.add_argument("--compact", action="store_true", help="property-wise reorder workspace")
+    ap.add_argument("--cells", default=None, help="override the workload's cell grid, e.g. 256,256,256 (profiling runs)")
+    args = ap.parse_args()
+    wl = dict(WORKLOADS[args.workload])
+    explicit = args.nbar is not None or args.cells is not None or args.workload != "cfg5" or args.rebin_every is not None
+    if args.nbar is None:
+        args.nbar = wl["nbar"]
+    if args.rebin_every is not None:
+        wl["rebin_every"] = args.rebin_every
+    cells_override = tuple(int(t) for t in args.cells.split(",")) if args.cells else None
+    if cells_override:
+        wl["cells"] = cells_override
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        run_reference(args, wl, rank, world)
+        return
+
+    import torch
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    torch.cuda.set_device(torch.device(f"cuda:{local_rank}"))
+
+    res, wl = measure(args, args.workload, args.nbar, args.steps, args.warmup, rank, local_rank, world, dist,
+                      with_e2e=(not args.no_e2e and rank == 0 and world == 1), rebin_every=args.rebin_every,
+                      cells_override=cells_override)
+    line = {"metric": "MPC particle-updates/sec", "value": res["value"], "unit": "particle-updates/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": args.workload, "cells": list(cells), "n_per_cell": nbar, "particles": n,
-                       "collision": "MPC-AT" if kw.get("collision") else "SRD", "thermostat": bool(kw.get("thermostat", 0)),
-                       "rebin_every": wl["rebin_every"], "brick": list(brick), "compact_workspace": bool(compact),
-                       "l2": "inputs larger than L2 (no flush)" if n * 24 > 4 * 126e6 else "state fits in L2; HBM fraction not meaningful",
-                       "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "algorithmic_bytes_per_update": balg},
-            "gpu_launches": int(launches), "clocks": clocks.summary(), "roofline": roofline,
-            "check": {"kT_cell": ob["kT_cell"], "kT_est": ob["kT_est"], "max_cell_count": ob["max_cell_count"], "step": ob["step"]}}
+            "config": res["config"], "gpu_launches": res["gpu_launches"], "clocks": res["clocks"], "roofline": res["roofline"],
+            "check": res["check"]}
+    line["e2e"] = res.get("e2e") if world == 1 else None
 
-    # ---- e2e: the same job through the host-buffer C ABI (pinned host state in, K steps, state out) ----
-    if not args.no_e2e and rank == 0 and world == 1:
-        line["e2e"] = run_e2e(sim, n, args.steps)
-    elif world > 1:
-        line["e2e"] = None
+    # ---- extras of the default run (N = 1): the density sweep BASELINE.json configs[4] names, and configs 3 and 4 ----
+    if world == 1 and rank == 0 and not explicit and not args.no_extras:
+        sweep = []
+        for nb in (5, 20):
+            r, _ = measure(args, "cfg5", nb, args.steps, args.warmup, rank, local_rank, world, None, with_e2e=False)
+            sweep.append({"n_per_cell": nb, "particles": r["config"]["particles"], "ms_per_step": r["ms_per_step"], "value": r["value"],
+                          "step_frac_of_roofline": r["roofline"]["step_frac_of_roofline"], "step_frac_of_8000": r["roofline"]["step_frac_of_8000"],
+                          "compact_workspace": r["config"]["compact_workspace"], "clocks": r["clocks"],
+                          "family_ms_per_step": r["roofline"]["family_ms_per_step"], "check": r["check"]})
+        line["density_sweep"] = sweep
+        other = []
+        for w in ("cfg3", "cfg4"):
+            r, _ = measure(args, w, WORKLOADS[w]["nbar"], 100, 10, rank, local_rank, world, None, with_e2e=False)
+            other.append({"workload": w, "config": r["config"], "ms_per_step": r["ms_per_step"], "value": r["value"],
+                          "step_frac_of_roofline": r["roofline"]["step_frac_of_roofline"],
+                          "family_ms_per_step": r["roofline"]["family_ms_per_step"], "check": r["check"]})
+        line["other_workloads"] = other
     # ---- CPU oracle beside it (rank 0, N = 1 only) ----
     if not args.no_cpu_baseline and rank == 0 and world == 1:
-        v, sample, _, _ = oracle_rate(wl, nbar)
-        line["cpu_baseline"] = {"value": v, "unit": "particle-updates/s", "cores": 1, "kind": "oracle", "sample": sample}
+        v, sample, _, _ = oracle_rate(wl, args.nbar)
+        line["cpu_baseline"] = {"value": v, "unit": "particle-updates/s", "cores": 1, "host_cores": os.cpu_count(),
+                                "kind": "oracle", "sample": sample}
     if rank == 0:
         print(json.dumps(line), flush=True)
     if dist is not None:

@@ -42,6 +42,7 @@ extern "C" {
 #define MPC_ESTATE -2 /* call order: step before bind/set_state, get_cells before a step */
 #define MPC_ENOMEM -3 /* workspace too small for the requested number of particles      */
 #define MPC_ECUDA  -4 /* a CUDA call failed; sticky until mpc_destroy                   */
+#define MPC_ERANGE -5 /* mpc_observables: velocities left the range of the fixed-point cell sums */
 
 typedef struct mpc_ctx mpc_ctx; /* opaque */
 
@@ -73,6 +74,12 @@ typedef struct {
   unsigned max_cell_count;             /* largest N_c of the last step; 0 if no step was taken         */
   unsigned long long n_singular_cells; /* +a only: cells whose inertia tensor was rejected (U10)       */
   unsigned long long step;             /* step counter t                                               */
+  unsigned long long n_range_overflows;/* events since the last mpc_set_state in which a value left the range the
+                                          fixed-point cell sums are sized for ("overflows may occur ...
+                                          invalidating the results"): a particle with |v| >= 8 u, u = sqrt(kT/m) rounded
+                                          to a power of two, or a momentum sum of >= 64 particles within a factor two of
+                                          the 32-bit range |sum v_d| < 512 u. Energy sums cannot overflow below 65535
+                                          particles per cell. 0 in every supported run                            */
 } mpc_obs;
 
 /* Create a context. box[d] = L_d, cells[d] = number of fluid cells n_d; cells must be cubic
@@ -95,7 +102,9 @@ int mpc_workspace_bytes(const mpc_ctx*, unsigned long long n_max, int compact, s
 
 /* Hand the library its workspace (device pointer, 256-byte aligned, `bytes` long, zeroing not
  * required) and the CUDA stream (a cudaStream_t cast to void*; NULL = legacy default stream).
- * The mode (compact or not) is chosen from `bytes`. MPC_ENOMEM if too small for n_max. */
+ * The mode (compact or not) is chosen from `bytes`. MPC_ENOMEM if too small for n_max. The workspace must live
+ * on the CUDA device that is current at the call (MPC_EINVAL otherwise); every later call on this context makes
+ * that device current for its own duration. */
 int mpc_bind(mpc_ctx*, void* workspace, size_t bytes, unsigned long long n_max, void* cuda_stream);
 
 /* Copy a state in. Device pointers (mpc_set_state) or host pointers (mpc_set_state_host), n each.
@@ -112,10 +121,18 @@ int mpc_set_state_host(mpc_ctx*, unsigned long long n, const float* x, const flo
  * One call of n steps gives bit-identical results to n calls of one step; it is faster because the
  * collision of step t is fused into the streaming pass of step t+1 and a reorder is folded into the
  * sweeps of its own and the next step.
- * Diagnostic switches read from the environment at mpc_create (all change speed only, never results):
- * MPC_NO_FUSE_GATHER=1 (separate gather kernel), MPC_EAGER_CANONICAL=1 (rank by id at every reorder),
- * MPC_OVERLAP_CELL=1 (PROCESS_CELLS of a reorder step on a side stream). */
+ * The collision of the LAST step of a call stays pending inside the context: the next mpc_step applies it in its
+ * first streaming pass, and every call that reads velocities (mpc_get_state*, mpc_observables) applies it first,
+ * so the state seen through the API is always the fully collided one. */
 int mpc_step(mpc_ctx*, int nsteps);
+
+/* Diagnostic switches (change speed only, never results; the library reads no environment variables):
+ * a bitwise OR of the flags below, 0 = the default code paths. May be called at any time between steps. */
+#define MPC_DEBUG_NO_FUSE_GATHER  1u /* reorder: separate gather kernel instead of folding it into two sweeps      */
+#define MPC_DEBUG_EAGER_CANONICAL 2u /* reorder: rank by id at every reorder instead of lazily on read             */
+#define MPC_DEBUG_ATOMIC_SCATTER  4u /* reorder: cursor atomics per run of particles instead of the sweep's ranks   */
+#define MPC_DEBUG_EAGER_COLLIDE   8u /* apply the last step's collision at the end of mpc_step (separate pass)      */
+int mpc_set_debug(mpc_ctx*, unsigned flags);
 
 /* Copy the state out, in the current internal order, with ids. Any pointer may be NULL (skipped).
  * Device pointers: asynchronous. Host pointers: synchronises the stream before returning.
@@ -128,10 +145,12 @@ int mpc_get_state(mpc_ctx*, float* x, float* y, float* z, float* vx, float* vy, 
 int mpc_get_state_host(mpc_ctx*, float* x, float* y, float* z, float* vx, float* vy, float* vz, unsigned* id);
 
 /* System observables ("Properties<FINALIZE>") into a HOST struct; synchronises.
- * profile_host: NULL, or n_w host floats receiving the layer-averaged velocity component along the
+ * profile_host: NULL, or n_profile host floats receiving the layer-averaged velocity component along the
  * force axis (first axis with g != 0, else x) as a function of the layer floor(r_w / a) along the
- * wall axis w (z if there is no wall), the shear-profile binning of PAPER.md:212. */
-int mpc_observables(mpc_ctx*, mpc_obs* host_out, float* profile_host);
+ * wall axis w (z if there is no wall), the shear-profile binning of PAPER.md:212. n_profile must equal the
+ * number of fluid cells along that axis (MPC_EINVAL otherwise; ignored when profile_host is NULL).
+ * Returns MPC_ERANGE (with *host_out filled in) if n_range_overflows != 0. */
+int mpc_observables(mpc_ctx*, mpc_obs* host_out, float* profile_host, int n_profile);
 
 /* Test hook: the last step's pre-collision cell sums over real particles. Device pointers, any may
  * be NULL: count[K], px/py/pz[K] = m * sum v, e2[K] = sum |v|^2, key[n] = memory key of every

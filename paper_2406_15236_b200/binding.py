@@ -12,11 +12,12 @@ import numpy as np
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("MPC_B200_LIB", os.path.join(HERE, "libmpc_b200.so"))   # override: alternative builds
 
-MPC_OK, MPC_EINVAL, MPC_ESTATE, MPC_ENOMEM, MPC_ECUDA = 0, -1, -2, -3, -4
+MPC_OK, MPC_EINVAL, MPC_ESTATE, MPC_ENOMEM, MPC_ECUDA, MPC_ERANGE = 0, -1, -2, -3, -4, -5
+DEBUG_NO_FUSE_GATHER, DEBUG_EAGER_CANONICAL, DEBUG_ATOMIC_SCATTER, DEBUG_EAGER_COLLIDE = 1, 2, 4, 8
 
 # every symbol include/mpc_b200.h declares
 SYMBOLS = ["mpc_create", "mpc_num_keys", "mpc_workspace_bytes", "mpc_bind", "mpc_set_state", "mpc_set_state_host",
-           "mpc_step", "mpc_get_state", "mpc_get_state_host", "mpc_observables", "mpc_get_cells",
+           "mpc_step", "mpc_set_debug", "mpc_get_state", "mpc_get_state_host", "mpc_observables", "mpc_get_cells",
            "mpc_philox4x32_10", "mpc_launch_count", "mpc_profile_enable", "mpc_profile_read", "mpc_last_error",
            "mpc_destroy"]
 
@@ -31,7 +32,7 @@ class mpc_params(C.Structure):
 class mpc_obs(C.Structure):
     _fields_ = [("n", C.c_ulonglong), ("P", C.c_double * 3), ("E_kin", C.c_double),
                 ("kT_est", C.c_double), ("kT_cell", C.c_double), ("max_cell_count", C.c_uint),
-                ("n_singular_cells", C.c_ulonglong), ("step", C.c_ulonglong)]
+                ("n_singular_cells", C.c_ulonglong), ("step", C.c_ulonglong), ("n_range_overflows", C.c_ulonglong)]
 
 
 class MPCError(RuntimeError):
@@ -59,9 +60,10 @@ def load():
     L.mpc_set_state.argtypes = [vp, ull, fp, fp, fp, fp, fp, fp, up, C.c_uint]
     L.mpc_set_state_host.argtypes = L.mpc_set_state.argtypes
     L.mpc_step.argtypes = [vp, C.c_int]
+    L.mpc_set_debug.argtypes = [vp, C.c_uint]
     L.mpc_get_state.argtypes = [vp, fp, fp, fp, fp, fp, fp, up]
     L.mpc_get_state_host.argtypes = L.mpc_get_state.argtypes
-    L.mpc_observables.argtypes = [vp, C.POINTER(mpc_obs), vp]
+    L.mpc_observables.argtypes = [vp, C.POINTER(mpc_obs), vp, C.c_int]
     L.mpc_get_cells.argtypes = [vp, up, fp, fp, fp, fp, up]
     L.mpc_philox4x32_10.argtypes = [C.POINTER(C.c_uint), C.POINTER(C.c_uint), C.POINTER(C.c_uint)]
     L.mpc_philox4x32_10.restype = None
@@ -127,11 +129,11 @@ class MPC:
         nbytes = C.c_size_t()
         self._check(self.lib.mpc_workspace_bytes(self._h, self.n_max, 1 if compact else 0, C.byref(nbytes)))
         self.workspace_bytes = nbytes.value
-        with torch.cuda.device(self.device):
+        with torch.cuda.device(self.device):      # mpc_bind records the current device; later calls switch to it themselves
             self.workspace = torch.empty(nbytes.value, dtype=torch.uint8, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-        self._check(self.lib.mpc_bind(self._h, C.c_void_p(self.workspace.data_ptr()), nbytes.value, self.n_max,
-                                      C.c_void_p(self.stream.cuda_stream)))
+            self._check(self.lib.mpc_bind(self._h, C.c_void_p(self.workspace.data_ptr()), nbytes.value, self.n_max,
+                                          C.c_void_p(self.stream.cuda_stream)))
 
     def _check(self, rc):
         if rc != MPC_OK:
@@ -193,13 +195,29 @@ class MPC:
         self._check(self.lib.mpc_get_cells(self._h, _ptr(cnt), *[_ptr(t) for t in p], _ptr(key)))
         return cnt, p[0], p[1], p[2], p[3], key
 
-    def observables(self, profile_bins=0):
+    def set_debug(self, flags):
+        self._check(self.lib.mpc_set_debug(self._h, int(flags)))
+
+    @property
+    def profile_layers(self):
+        """Number of entries of the velocity profile: the fluid cells along the wall axis (z without walls)."""
+        bc = tuple(self.params.bc)
+        axis = max((d for d in range(3) if bc[d] != 0), default=2)
+        return self.cells[axis]
+
+    def observables(self, profile=False):
+        """System observables as a dict; profile=True adds the layer-averaged velocity profile (profile_layers floats).
+        A range overflow of the fixed-point sums (MPC_ERANGE) is reported as d["n_range_overflows"] != 0, not raised."""
         o = mpc_obs()
-        prof = np.zeros(max(profile_bins, 1), np.float32)
-        self._check(self.lib.mpc_observables(self._h, C.byref(o), prof.ctypes.data_as(C.c_void_p) if profile_bins else None))
+        nb = self.profile_layers
+        prof = np.zeros(nb, np.float32)            # sized by the library's own rule, never by the caller
+        rc = self.lib.mpc_observables(self._h, C.byref(o), prof.ctypes.data_as(C.c_void_p) if profile else None, nb)
+        if rc != MPC_ERANGE:
+            self._check(rc)
         d = dict(n=o.n, P=np.array(o.P[:]), E_kin=o.E_kin, kT_est=o.kT_est, kT_cell=o.kT_cell,
-                 max_cell_count=o.max_cell_count, n_singular_cells=o.n_singular_cells, step=o.step)
-        if profile_bins:
+                 max_cell_count=o.max_cell_count, n_singular_cells=o.n_singular_cells, step=o.step,
+                 n_range_overflows=o.n_range_overflows)
+        if profile:
             d["profile"] = prof
         return d
 

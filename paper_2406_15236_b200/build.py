@@ -6,12 +6,13 @@ import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = [os.path.join(HERE, "csrc", "mpc_b200.cu")]
-DEPS = SRC + [os.path.join(HERE, "csrc", "philox.cuh"), os.path.join(HERE, "..", "include", "mpc_b200.h")]
+SRC = [os.path.join(HERE, "csrc", f) for f in ("abi.cu", "sweep.cu", "cell.cu", "reorder.cu", "generic.cu", "observe.cu")]
+DEPS = SRC + [os.path.join(HERE, "csrc", "philox.cuh"), os.path.join(HERE, "csrc", "internal.cuh"),
+              os.path.join(HERE, "..", "include", "mpc_b200.h")]
 LIB = os.path.join(HERE, "libmpc_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "--fmad=false",
-         "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
+         "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "--threads", "0"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

@@ -1,0 +1,360 @@
+// reorder.cu -- REORDER: counting sort of the particles by (cell key, id). Counts come from the
+// cell sums (no separate histogram), an exclusive scan gives the cell offsets, a scatter gives the
+// permutation; the gather is folded into the next step's sweep or done property-wise through one
+// temporary array in the compact workspace.
+#include "internal.cuh"
+
+namespace mpc {
+
+// ---- exclusive scan of the per-cell counts (three kernels; tile = 2048) ----------------------------
+// `in` is read with a stride in 32-bit words: the count is the low 16 bits of word 0 of a cell's sums.
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t& total) {
+  __shared__ uint32_t wsum[33];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  uint32_t inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += t;
+  }
+  if (lane == 31) wsum[warp] = inc;
+  __syncthreads();
+  if (warp == 0) {
+    const uint32_t w = lane < nw ? wsum[lane] : 0u;
+    uint32_t winc = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, winc, o);
+      if (lane >= o) winc += t;
+    }
+    wsum[lane] = winc - w;            // exclusive offset of every warp
+    if (lane == 31) wsum[32] = winc;  // block total
+  }
+  __syncthreads();
+  const uint32_t res = wsum[warp] + inc - v;
+  total = wsum[32];
+  __syncthreads();                    // wsum is reused by the caller's next round
+  return res;
+}
+__global__ void __launch_bounds__(SCAN_T) k_scan_reduce(const uint32_t* __restrict__ in, int stride, size_t n, uint32_t* __restrict__ bsum) {
+  const size_t base = (size_t)blockIdx.x * SCAN_TILE;
+  uint32_t s = 0;
+#pragma unroll
+  for (int j = 0; j < SCAN_PER; ++j) {
+    const size_t i = base + (size_t)j * SCAN_T + threadIdx.x;
+    if (i < n) s += in[i * stride] & 0xffffu;
+  }
+  __shared__ uint32_t red[SCAN_T / 32];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t t = 0;
+    for (int w = 0; w < SCAN_T / 32; ++w) t += red[w];
+    bsum[blockIdx.x] = t;
+  }
+}
+__global__ void __launch_bounds__(1024) k_scan_top(uint32_t* __restrict__ bsum, size_t nb) {
+  uint32_t carry = 0;
+  for (size_t base = 0; base < nb; base += 1024) {
+    const size_t i = base + threadIdx.x;
+    const uint32_t v = i < nb ? bsum[i] : 0u;
+    uint32_t total;
+    const uint32_t ex = block_exclusive_scan(v, total);
+    if (i < nb) bsum[i] = carry + ex;
+    carry += total;
+  }
+}
+__global__ void __launch_bounds__(SCAN_T) k_scan_apply(const uint32_t* __restrict__ in, int stride, size_t n,
+                                                       const uint32_t* __restrict__ bsum, uint32_t* __restrict__ out) {
+  const size_t base = (size_t)blockIdx.x * SCAN_TILE + (size_t)threadIdx.x * SCAN_PER;
+  uint32_t v[SCAN_PER], s = 0;
+#pragma unroll
+  for (int j = 0; j < SCAN_PER; ++j) {
+    v[j] = (base + j < n) ? (in[(base + j) * stride] & 0xffffu) : 0u;
+    s += v[j];
+  }
+  uint32_t total;
+  uint32_t ex = block_exclusive_scan(s, total) + bsum[blockIdx.x];
+#pragma unroll
+  for (int j = 0; j < SCAN_PER; ++j) {
+    if (base + j < n) out[base + j] = ex;
+    ex += v[j];
+  }
+  if (blockIdx.x == gridDim.x - 1 && threadIdx.x == SCAN_T - 1) out[n] = ex;   // grand total
+}
+
+// ---- scatter --------------------------------------------------------------------------------------
+// Lanes of a warp that hold the same key as their neighbours form runs (the array is still nearly sorted):
+// one cursor atomic per run. Returns the first slot of this lane within its cell segment's arrival order.
+// (match.any would also merge non-adjacent lanes but runs at a fraction of the rate: measured 72 % pipe busy.)
+__device__ __forceinline__ uint32_t run_slot(uint32_t k, uint32_t* __restrict__ cursor) {
+  const unsigned lane = threadIdx.x & 31u;
+  const unsigned act = __activemask();                      // a prefix of the warp (i < n)
+  const uint32_t kprev = __shfl_up_sync(act, k, 1);
+  const unsigned heads = __ballot_sync(act, lane == 0u || kprev != k);
+  const unsigned le = 0xffffffffu >> (31u - lane);          // lanes <= lane
+  const int leader = 31 - __clz((int)(heads & le));
+  const unsigned above = heads & ~le;
+  const int end = above ? (__ffs((int)above) - 1) : __popc(act);
+  uint32_t base = 0;
+  if ((int)lane == leader) base = atomicAdd(&cursor[k], (uint32_t)(end - leader));
+  base = __shfl_sync(act, base, leader);
+  return base + (lane - (unsigned)leader);
+}
+// Canonical path, step 1: every particle takes a slot of its cell segment in arrival order
+__global__ void __launch_bounds__(256) k_scatter_slots(size_t n, const uint32_t* __restrict__ key, const uint32_t* __restrict__ id,
+                                                       const uint32_t* __restrict__ offset, uint32_t* __restrict__ cursor,
+                                                       uint2* __restrict__ slot) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t k = key[i];
+  const uint32_t s = offset[k] + run_slot(k, cursor);
+  slot[s] = make_uint2(id[i], (uint32_t)i);   // one 8-byte store: (id, source index)
+}
+// Canonical path, step 2, one thread per slot: rank of the slot's particle inside its cell = number of cell mates
+// with a smaller id (U4); perm[first slot of the cell + rank] = source index.
+__global__ void __launch_bounds__(256) k_rank(size_t n, const uint32_t* __restrict__ key, const uint32_t* __restrict__ offset,
+                                              const uint2* __restrict__ slot, uint32_t* __restrict__ perm) {
+  const size_t s = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  const uint2 me = slot[s];
+  const uint32_t k = key[me.y];
+  const uint32_t b = offset[k], e = offset[k + 1];
+  uint32_t r = 0;
+  for (uint32_t j = b; j < e; ++j) r += (slot[j].x < me.x) ? 1u : 0u;
+  perm[b + r] = me.y;
+}
+// Hot-path variant (SRD) when no order is known yet: the order inside a cell does not enter the physics (integer
+// cell sums), so the reorder only groups the particles by key: perm[slot] = source index, slots in arrival order
+// from one cursor atomic per run of equal keys. Four independent particles per thread: the kernel is bound by the
+// latency of the chain key load -> cursor atomic (with return) -> store.
+constexpr int SCAT_U = 4;
+__global__ void __launch_bounds__(256) k_scatter_src(size_t n, const uint32_t* __restrict__ key, const uint32_t* __restrict__ offset,
+                                                     uint32_t* __restrict__ cursor, uint32_t* __restrict__ perm) {
+  const size_t base = (size_t)blockIdx.x * (256 * SCAT_U) + threadIdx.x;
+  const unsigned lane = threadIdx.x & 31u, le = 0xffffffffu >> (31u - lane);
+  uint32_t k[SCAT_U], slot[SCAT_U];
+  bool ok[SCAT_U];
+  int leader[SCAT_U], len[SCAT_U];
+#pragma unroll
+  for (int j = 0; j < SCAT_U; ++j) {
+    const size_t i = base + (size_t)j * 256;
+    ok[j] = i < n;
+    k[j] = ok[j] ? key[i] : 0u;
+  }
+#pragma unroll
+  for (int j = 0; j < SCAT_U; ++j) {   // runs of equal keys among neighbouring lanes (run_slot, all 32 lanes take part)
+    const uint32_t kprev = __shfl_up_sync(0xffffffffu, k[j], 1);
+    const int okprev = __shfl_up_sync(0xffffffffu, (int)ok[j], 1);
+    const unsigned heads = __ballot_sync(0xffffffffu, lane == 0u || kprev != k[j] || okprev != (int)ok[j]);
+    leader[j] = 31 - __clz((int)(heads & le));
+    const unsigned above = heads & ~le;
+    len[j] = (above ? (__ffs((int)above) - 1) : 32) - leader[j];
+  }
+#pragma unroll
+  for (int j = 0; j < SCAT_U; ++j) {
+    slot[j] = 0;
+    if (ok[j] && (int)lane == leader[j]) slot[j] = atomicAdd(&cursor[k[j]], (uint32_t)len[j]);
+  }
+  uint32_t off[SCAT_U];
+#pragma unroll
+  for (int j = 0; j < SCAT_U; ++j) off[j] = ok[j] ? offset[k[j]] : 0u;
+#pragma unroll
+  for (int j = 0; j < SCAT_U; ++j) {
+    const uint32_t b = __shfl_sync(0xffffffffu, slot[j], leader[j]);
+    if (ok[j]) perm[off[j] + b + (lane - (unsigned)leader[j])] = (uint32_t)(base + (size_t)j * 256);
+  }
+}
+
+// Hot-path variant when the previous order is known: the staging sweep (k_sweep<.., IO_AOS_OUT>) has given every
+// particle its arrival rank inside (CTA, tile cell) -- the value its shared-memory count atomic returned -- and every
+// CTA the first slot of its particles inside each cell's segment (the value the tile flush's global atomic returned).
+// The slot of a particle is then offset[key] + first slot + rank: no atomics, no dependent chain, one CTA per brick
+// with the brick's slot table in shared memory. word = tile cell << 16 | rank, or bit 31 | rank for the few particles
+// that left their brick's tile (their key is recomputed from the staged position).
+__global__ void __launch_bounds__(256) k_save_chunks(const uint32_t* __restrict__ offset, int bvol_shift, uint32_t nbricks,
+                                                     uint32_t n, uint32_t* __restrict__ chunk0) {
+  const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b < nbricks) chunk0[b] = offset[(size_t)b << bvol_shift];
+  if (b == nbricks) chunk0[b] = n;
+}
+template <class BS>
+__global__ void __launch_bounds__(512) k_scatter_tile(Geo G, uint32_t n, const uint32_t* __restrict__ word, const uint32_t* __restrict__ chunk0,
+                                                      uint32_t nbricks, const uint32_t* __restrict__ offset, const uint32_t* __restrict__ tbase,
+                                                      const float* __restrict__ aos, uint32_t* __restrict__ perm) {
+  extern __shared__ uint32_t dest[];
+  const int T0 = (1 << BS::s0(G)) + 2 * HALO, T1 = (1 << BS::s1(G)) + 2 * HALO, T2 = (1 << BS::s2(G)) + 2 * HALO;
+  const int tcells = T0 * T1 * T2;
+  const uint32_t b = blockIdx.x;
+  const int m0 = G.m[0], m1 = G.m[1], m2 = G.m[2];
+  int ox, oy, oz;
+  {
+    const uint32_t bx = b % (uint32_t)G.mb[0], q = b / (uint32_t)G.mb[0];
+    const uint32_t by = q % (uint32_t)G.mb[1], bz = q / (uint32_t)G.mb[1];
+    ox = (int)(bx << BS::s0(G)) - HALO; oy = (int)(by << BS::s1(G)) - HALO; oz = (int)(bz << BS::s2(G)) - HALO;
+  }
+  uint32_t i0 = (chunk0[b] + 31u) & ~31u, i1 = chunk0[b + 1];
+  if (b + 1 != nbricks) i1 = min((i1 + 31u) & ~31u, n);      // the ranges of chunk_range() in sweep.cu
+  if (i0 >= i1) return;
+  for (int c = threadIdx.x; c < tcells; c += blockDim.x) {
+    const int l0 = c % T0, q = c / T0, l1 = q % T1, l2 = q / T1;
+    // wall axes do not wrap: tile cells beyond the last layer hold no particles, their slot is never read
+    const int kx = fold(ox + l0, m0), ky = fold(oy + l1, m1), kz = fold(oz + l2, m2);
+    dest[c] = offset[BS::key(G, kx, ky, kz)] + tbase[(size_t)b * tcells + c];
+  }
+  __syncthreads();
+  for (uint32_t i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
+    const uint32_t w = word[i];
+    uint32_t d;
+    if (w & 0x80000000u) {
+      const float* p = aos + (size_t)i * 8;
+      d = offset[key_of(G, p[0], p[1], p[2], G.s[0], G.s[1], G.s[2])] + (w & 0xffffu);
+    } else {
+      d = dest[w >> 16] + (w & 0xffffu);
+    }
+    perm[d] = i;
+  }
+}
+
+// one thread per cell: the particles of segment [offset[k], offset[k+1]) ranked by id
+__global__ void __launch_bounds__(256) k_rank_cells(size_t nkeys, const uint32_t* __restrict__ offset, const uint32_t* __restrict__ id,
+                                                    uint32_t* __restrict__ perm) {
+  const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= nkeys) return;
+  const uint32_t b = offset[k], e = offset[k + 1];
+  for (uint32_t j = b; j < e; ++j) {
+    const uint32_t me = id[j];
+    uint32_t r = 0;
+    for (uint32_t m = b; m < e; ++m) r += (id[m] < me) ? 1u : 0u;
+    perm[b + r] = j;
+  }
+}
+struct Arrays8 { void* p[8]; };
+template <int NA>
+__global__ void __launch_bounds__(256) k_gather(size_t n, const uint32_t* __restrict__ perm, Arrays8 src, Arrays8 dst) {
+  const size_t d = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (d >= n) return;
+  const uint32_t s = perm[d];
+  uint32_t v[NA];
+#pragma unroll
+  for (int a = 0; a < NA; ++a) v[a] = ((const uint32_t*)src.p[a])[s];
+#pragma unroll
+  for (int a = 0; a < NA; ++a) ((uint32_t*)dst.p[a])[d] = v[a];
+}
+
+__global__ void __launch_bounds__(256) k_iota(size_t n, uint32_t* __restrict__ id) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) id[i] = (uint32_t)i;
+}
+
+}  // namespace mpc
+
+using namespace mpc;
+
+int launch_iota(mpc_ctx* c) {
+  k_iota<<<nblk(c->n_max ? c->n_max : 1, 256), 256, 0, c->stream>>>(c->n_max, c->A[6]);
+  LAUNCH_CHECK("k_iota");
+  return MPC_OK;
+}
+
+namespace {
+
+// particle arrays gathered through c->perm: new[i] = old[perm[i]]
+int apply_perm(mpc_ctx* c) {
+  const size_t n = c->n;
+  FamilyTimer ftg(c, F_GATHER);
+  if (!c->compact) {
+    Arrays8 src, dst;
+    for (int a = 0; a < 7; ++a) { src.p[a] = c->A[a]; dst.p[a] = c->Bf[a]; }
+    src.p[7] = dst.p[7] = nullptr;
+    k_gather<7><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
+    LAUNCH_CHECK("k_gather");
+    for (int a = 0; a < 7; ++a) { uint32_t* t = c->A[a]; c->A[a] = c->Bf[a]; c->Bf[a] = t; }
+  } else {
+    // property-wise through one temporary array: each property is gathered into the spare array,
+    // which then takes its place; the array it came from is the spare for the next property (no copy back)
+    Arrays8 src, dst;
+    for (int a = 0; a < 7; ++a) {
+      uint32_t*& arr = c->A[a];
+      src.p[0] = arr; dst.p[0] = c->Bf[0];
+      k_gather<1><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
+      LAUNCH_CHECK("k_gather");
+      uint32_t* t = arr; arr = c->Bf[0];
+      for (int b = 0; b < 7; ++b) c->Bf[b] = t;     // compact mode: all seven alias the one spare array
+    }
+  }
+  return MPC_OK;
+}
+
+}  // namespace
+
+// counting-sort reorder by (key, id); counts = low word of word 0 of the sums; c->key holds the keys (or, after a
+// ranked staging sweep, the rank words)
+// defer_gather: leave the permutation in c->perm for the next sweep to apply (IO_GATHER)
+// canonical: rank the particles of a cell by id now (needed by MPC-AT); otherwise group by key only
+int do_reorder(mpc_ctx* c, bool defer_gather, bool canonical) {
+  const size_t n = c->n, nk = c->G.nkeys, nb = (nk + SCAN_TILE - 1) / SCAN_TILE;
+  const uint32_t* cnt = reinterpret_cast<const uint32_t*>(c->sums);
+  const int stride = c->G.sw * 2;
+  const bool ranked = c->ranked_keys && defer_gather && !canonical;
+  const int bvs = c->G.bs[0] + c->G.bs[1] + c->G.bs[2];
+  if (ranked) {   // the brick ranges of the old order, before the scan overwrites the offsets
+    FamilyTimer ft(c, F_SCAN);
+    k_save_chunks<<<nblk((size_t)c->nbricks + 1, 256), 256, 0, c->stream>>>(c->offset, bvs, c->nbricks, (uint32_t)n, c->chunk0);
+    LAUNCH_CHECK("k_save_chunks");
+  }
+  {
+    FamilyTimer ft(c, F_SCAN);
+    k_scan_reduce<<<(unsigned)nb, SCAN_T, 0, c->stream>>>(cnt, stride, nk, c->bsum);
+    LAUNCH_CHECK("k_scan_reduce");
+    k_scan_top<<<1, 1024, 0, c->stream>>>(c->bsum, nb);
+    LAUNCH_CHECK("k_scan_top");
+    k_scan_apply<<<(unsigned)nb, SCAN_T, 0, c->stream>>>(cnt, stride, nk, c->bsum, c->offset);
+    LAUNCH_CHECK("k_scan_apply");
+  }
+  if (ranked) {
+    FamilyTimer ft(c, F_SCATTER);
+    const float* aos = reinterpret_cast<const float*>(c->A[0] < c->Bf[0] ? c->slot_id : c->Bf[0]);
+    const size_t sh = c->tile_bytes / TILE_W;     // one uint32 per tile cell
+    if (c->fast_brick) k_scatter_tile<BSfast><<<c->nbricks, 512, sh, c->stream>>>(c->G, (uint32_t)n, c->key, c->chunk0, c->nbricks, c->offset, c->tbase, aos, c->perm);
+    else k_scatter_tile<BSgeneric><<<c->nbricks, 512, sh, c->stream>>>(c->G, (uint32_t)n, c->key, c->chunk0, c->nbricks, c->offset, c->tbase, aos, c->perm);
+    LAUNCH_CHECK("k_scatter_tile");
+  } else {
+    { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->cursor, 0, nk * 4, c->stream)); }
+    if (canonical) {
+      uint2* slot2 = reinterpret_cast<uint2*>(c->compact ? c->slot_id : c->Bf[0]);
+      {
+        FamilyTimer ft(c, F_SCATTER);
+        k_scatter_slots<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->key, c->A[6], c->offset, c->cursor, slot2);
+        LAUNCH_CHECK("k_scatter_slots");
+      }
+      FamilyTimer ft(c, F_RANK);
+      k_rank<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->key, c->offset, slot2, c->perm);
+      LAUNCH_CHECK("k_rank");
+    } else {
+      FamilyTimer ft(c, F_SCATTER);
+      k_scatter_src<<<nblk(n, 256 * SCAT_U), 256, 0, c->stream>>>(n, c->key, c->offset, c->cursor, c->perm);
+      LAUNCH_CHECK("k_scatter_src");
+    }
+  }
+  c->have_order = true;
+  c->order_canonical = canonical;
+  if (defer_gather) { c->gather_pending = true; return MPC_OK; }
+  return apply_perm(c);
+}
+
+// restore the canonical (key, id) order inside the cell segments of the last reorder (U4); called
+// before the state is read when the hot path has left the particles grouped by key only
+int canonicalise(mpc_ctx* c) {
+  if (!c->have_order || c->order_canonical || c->n == 0) return MPC_OK;
+  {
+    FamilyTimer ft(c, F_RANK);
+    k_rank_cells<<<nblk(c->G.nkeys, 256), 256, 0, c->stream>>>(c->G.nkeys, c->offset, c->A[6], c->perm);
+    LAUNCH_CHECK("k_rank_cells");
+  }
+  const int rc = apply_perm(c);
+  if (rc == MPC_OK) c->order_canonical = true;
+  return rc;
+}

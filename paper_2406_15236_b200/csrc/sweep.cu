@@ -1,0 +1,304 @@
+// sweep.cu -- the fused SRD sweep: ROTATE_VELOCITIES of step t-1 (Eqs. 2,5) + MOVE of step t (Eq. 1, PAPER.md:31;
+// gravity PAPER.md:70; walls PAPER.md:68) + lattice shift and cell index + the per-cell sums of
+// step t, in ONE pass over the particles.
+#include "internal.cuh"
+
+namespace mpc {
+
+// Reorder folded into two consecutive sweeps (IO = 1 on the reorder step, IO = 2 on the step after it):
+//   IO_AOS_OUT  the pass writes every particle as ONE 32-byte record {r, v, id, 0} into a staging buffer
+//               instead of updating the SoA arrays in place;
+//   IO_GATHER   particle i of the new order is read with one 256-bit load from staging[perm[i]] (a whole
+//               sector, every byte used) and written to the SoA arrays at i.
+// A gather of the SoA arrays themselves costs ~4.5 sectors of L2 traffic per useful one (measured).
+struct SweepIO {
+  const float* aos_in;      // IO_GATHER: staging records in the old order
+  float* aos_out;           // IO_AOS_OUT
+  const uint32_t* perm;     // IO_GATHER
+  uint32_t* id;             // IO_AOS_OUT: read at i; IO_GATHER: written at i
+  uint32_t* tbase;          // IO_AOS_OUT with ranks: first slot of this CTA's particles inside every tile cell's segment
+  int ranked;               // IO_AOS_OUT: key_out receives (tile cell << 16 | arrival rank) instead of the key
+};
+__device__ __forceinline__ void ld256(const float* p, float (&a)[8]) {
+  asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=f"(a[0]), "=f"(a[1]), "=f"(a[2]), "=f"(a[3]), "=f"(a[4]), "=f"(a[5]), "=f"(a[6]), "=f"(a[7]) : "l"(p));
+}
+__device__ __forceinline__ void st256(float* p, const float (&a)[8]) {
+  asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+               :: "l"(p), "f"(a[0]), "f"(a[1]), "f"(a[2]), "f"(a[3]), "f"(a[4]), "f"(a[5]), "f"(a[6]), "f"(a[7]) : "memory");
+}
+
+// One CTA per brick of cells. Its particles are the contiguous range that was sorted into the brick at
+// the last reorder (chunk[] = offset[] of the brick's first key); since then they have moved by a
+// fraction of a cell and the lattice shift has changed by less than a cell, so nearly all of them fall
+// into the brick's tile (brick + HALO cells on every side), held in shared memory as int32 sums. The
+// rest (and everything, if no order is known yet) goes to the global sums directly.
+// The CTA takes the 128-byte-aligned groups of 32 particles that START in its range: every group belongs to
+// exactly one CTA and every access of a warp is line-aligned (L1 tag requests per load 1.9 -> 1.0).
+__device__ __forceinline__ void chunk_range(const uint32_t* __restrict__ chunk, uint32_t b, uint32_t nbricks, uint32_t n,
+                                            int bvol_shift, uint32_t& i0, uint32_t& i1) {
+  if (chunk) {
+    i0 = chunk[(size_t)b << bvol_shift];
+    i1 = (b + 1 == nbricks) ? n : chunk[(size_t)(b + 1) << bvol_shift];
+  } else {   // no order known: even split, (almost) everything takes the global path
+    i0 = (uint32_t)((u64)n * b / nbricks);
+    i1 = (uint32_t)((u64)n * (b + 1) / nbricks);
+  }
+  i0 = (i0 + 31u) & ~31u;
+  if (b + 1 != nbricks) i1 = min((i1 + 31u) & ~31u, n);   // trailing empty bricks: chunk = n, do not round past the end
+}
+
+// T = threads per CTA: 512 (2 CTAs per SM), or 384 (3 CTAs per SM at <= 56 registers: the steady-state sweep is
+// 2 % faster that way, the staged reorder sweeps are not)
+template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS, int IO, int T>
+__global__ void __launch_bounds__(T, T <= 384 ? 3 : 2)
+k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
+        float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, uint32_t* __restrict__ key_out,
+        const uint32_t* __restrict__ chunk, uint32_t nbricks, const float* __restrict__ rec, u64* __restrict__ sums,
+        SweepIO io) {
+  extern __shared__ int tile[];
+  const int T0 = (1 << BS::s0(G)) + 2 * HALO, T1 = (1 << BS::s1(G)) + 2 * HALO, T2 = (1 << BS::s2(G)) + 2 * HALO;
+  const int tcells = T0 * T1 * T2;
+  for (int i = threadIdx.x; i < tcells * TILE_W; i += T) tile[i] = 0;
+  const uint32_t b = blockIdx.x;
+  const int m0 = G.m[0], m1 = G.m[1], m2 = G.m[2];
+  int ox, oy, oz;
+  {
+    const uint32_t bx = b % (uint32_t)G.mb[0], q = b / (uint32_t)G.mb[0];
+    const uint32_t by = q % (uint32_t)G.mb[1], bz = q / (uint32_t)G.mb[1];
+    ox = (int)(bx << BS::s0(G)) - HALO; oy = (int)(by << BS::s1(G)) - HALO; oz = (int)(bz << BS::s2(G)) - HALO;
+  }
+  uint32_t i0, i1;
+  chunk_range(chunk, b, nbricks, n, BS::s0(G) + BS::s1(G) + BS::s2(G), i0, i1);
+  const bool ranked = IO == IO_AOS_OUT && io.ranked != 0;
+  // index offsets added before the floor index is folded: +1 on a wall axis (layer 0 lies in the wall)
+  const int w0 = (WALL && G.bc[0]) ? 1 : 0, w1 = (WALL && G.bc[1]) ? 1 : 0, w2 = (WALL && G.bc[2]) ? 1 : 0;
+  unsigned nbad = 0;
+  __syncthreads();
+  // software pipeline: the loads of the next particle are in flight while this one is processed
+  uint32_t i = i0 + threadIdx.x;
+  float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f, p4 = 0.f, p5 = 0.f;
+  // IO_GATHER: source indices of the particles 1, 2 and 3 iterations ahead (the first feeds the register
+  // prefetch, the second an L2 prefetch of its record, the third is in flight); pid = id of the particle in flight
+  float pid = 0.f;
+  uint32_t jn = 0, jn2 = 0, jn3 = 0;
+  if (IO == IO_GATHER) {
+    if (i < i1) {
+      float q[8];
+      ld256(io.aos_in + (size_t)io.perm[i] * 8, q);
+      p0 = q[0]; p1 = q[1]; p2 = q[2]; p3 = q[3]; p4 = q[4]; p5 = q[5]; pid = q[6];
+    }
+    if (i + T < i1) jn = io.perm[i + T];
+    if (i + 2 * T < i1) jn2 = io.perm[i + 2 * T];
+    if (i + 3 * T < i1) jn3 = io.perm[i + 3 * T];
+  } else if (i < i1) {
+    p0 = x[i]; p1 = y[i]; p2 = z[i]; p3 = vx[i]; p4 = vy[i]; p5 = vz[i];
+    if (IO == IO_AOS_OUT) pid = __uint_as_float(io.id[i]);
+  }
+  for (; i < i1; i += T) {
+    float r[3] = {p0, p1, p2}, v[3] = {p3, p4, p5};
+    const float idbits = pid;
+    const uint32_t inext = i + T;
+    if (IO == IO_GATHER) {
+      io.id[i] = __float_as_uint(idbits);
+      if (inext < i1) {
+        float q[8];
+        ld256(io.aos_in + (size_t)jn * 8, q);
+        p0 = q[0]; p1 = q[1]; p2 = q[2]; p3 = q[3]; p4 = q[4]; p5 = q[5]; pid = q[6];
+        jn = jn2; jn2 = jn3;
+        if (i + 2 * T < i1) asm volatile("prefetch.global.L2 [%0];" ::"l"(io.aos_in + (size_t)jn * 8));
+        if (i + 4 * T < i1) jn3 = io.perm[i + 4 * T];
+      }
+    } else if (inext < i1) {
+      p0 = x[inext]; p1 = y[inext]; p2 = z[inext]; p3 = vx[inext]; p4 = vy[inext]; p5 = vz[inext];
+      if (IO == IO_AOS_OUT) pid = __uint_as_float(io.id[inext]);
+    }
+    if (IO != IO_GATHER) {   // pull the lines of a later iteration into L2: the register prefetch above then pays L2, not DRAM, latency
+      const uint32_t ifar = i + PF_DIST * T;
+      if (ifar < i1) {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(x + ifar));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(y + ifar));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(z + ifar));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(vx + ifar));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(vy + ifar));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(vz + ifar));
+      }
+    }
+    if (COLLIDE) {   // ROTATE_VELOCITIES of the previous step; its key is recomputed from r and that step's shift
+      int kx = cell_raw(G, r[0], sp0) + w0, ky = cell_raw(G, r[1], sp1) + w1, kz = cell_raw(G, r[2], sp2) + w2;
+      if (WALL) { kx = G.bc[0] ? max(0, min(kx, m0 - 1)) : fold(kx, m0); ky = G.bc[1] ? max(0, min(ky, m1 - 1)) : fold(ky, m1);
+                  kz = G.bc[2] ? max(0, min(kz, m2 - 1)) : fold(kz, m2); }
+      else { kx = fold(kx, m0); ky = fold(ky, m1); kz = fold(kz, m2); }
+      const uint32_t kp = BS::key(G, kx, ky, kz);
+      float4 r0, ax;
+      load_rec(rec, kp, r0, ax);
+      srd_apply(G, r0, ax, v);
+    }
+    stream_one<WALL, GRAV>(G, r, v);
+    if (IO == IO_AOS_OUT) {
+      const float q[8] = {r[0], r[1], r[2], v[0], v[1], v[2], idbits, 0.f};
+      st256(io.aos_out + (size_t)i * 8, q);
+    } else {
+      x[i] = r[0]; y[i] = r[1]; z[i] = r[2];
+      vx[i] = v[0]; vy[i] = v[1]; vz[i] = v[2];
+    }
+    int cx = cell_raw(G, r[0], G.s[0]) + w0, cy = cell_raw(G, r[1], G.s[1]) + w1, cz = cell_raw(G, r[2], G.s[2]) + w2;
+    if (WALL) { if (G.bc[0]) cx = max(0, min(cx, m0 - 1)); if (G.bc[1]) cy = max(0, min(cy, m1 - 1)); if (G.bc[2]) cz = max(0, min(cz, m2 - 1)); }
+    const int a0 = __float2int_rn(v[0] * G.fxv), a1 = __float2int_rn(v[1] * G.fxv), a2 = __float2int_rn(v[2] * G.fxv);
+    const unsigned e = __float2uint_rn(fmaf(v[0], v[0], fmaf(v[1], v[1], v[2] * v[2])) * G.fxe);
+    nbad += (e >= E_RANGE_LIMIT) ? 1u : 0u;     // |v| >= 8 u: outside the range of the fixed-point sums
+    // tile coordinates: one fold takes care of the periodic image of the cell and of the tile origin
+    const int l0 = fold(cx - ox, m0), l1 = fold(cy - oy, m1), l2 = fold(cz - oz, m2);
+    const bool inside = (l0 < T0) & (l1 < T1) & (l2 < T2);
+    uint32_t word = 0;
+    if (inside) {
+      const int tc = (l2 * T1 + l1) * T0 + l0;
+      int* s = tile + tc * TILE_W;
+      // word 0 = count (11 bits) | sum of the energies' high parts e >> 21 (21 bits); word 4 = sum of their low 21 bits:
+      // neither can overflow below 2048 particles per (CTA, cell) with e < 2^28 (U19)
+      const int w0add = 1 + (int)((e >> TILE_E_SHIFT) << TILE_N_BITS);
+      if (ranked) word = ((uint32_t)tc << 16) | ((uint32_t)atomicAdd(s, w0add) & TILE_N_MASK);   // arrival rank inside (CTA, cell)
+      else atomicAdd(s, w0add);
+      atomicAdd(s + 1, a0); atomicAdd(s + 2, a1); atomicAdd(s + 3, a2);
+      atomicAdd((unsigned*)s + 4, e & ((1u << TILE_E_SHIFT) - 1u));
+    }
+    if ((WKEY && !ranked) || !inside) {
+      const uint32_t kc = BS::key(G, fold(cx, m0), fold(cy, m1), fold(cz, m2));
+      if (!inside) {
+        u64* s = sums + (size_t)kc * G.sw;
+        if (ranked) word = 0x80000000u | (uint32_t)(atomicAdd(s, ((u64)e << 16) | 1ull) & 0xffffull);
+        else atomicAdd(s, ((u64)e << 16) | 1ull);
+        atomicAdd(s + 1, pack_ss(a0, a1)); atomicAdd(s + 2, pack_ss(a2, 0));
+      }
+      if (WKEY && !ranked) key_out[i] = kc;
+    }
+    if (WKEY && ranked) key_out[i] = word;
+  }
+  if (nbad) atomicAdd(G.nrange, (u64)nbad);
+  __syncthreads();
+  // flush the tile: one packed 64-bit reduction per pair of sums, empty cells skipped
+  for (int c = threadIdx.x; c < tcells; c += T) {
+    const int* s = tile + c * TILE_W;
+    const int cnt = (int)((unsigned)s[0] & TILE_N_MASK);
+    if (cnt == 0) continue;
+    const int l0 = c % T0, q = c / T0, l1 = q % T1, l2 = q / T1;
+    u64* g = sums + (size_t)BS::key(G, fold(ox + l0, m0), fold(oy + l1, m1), fold(oz + l2, m2)) * G.sw;
+    const u64 etile = ((u64)((unsigned)s[0] >> TILE_N_BITS) << TILE_E_SHIFT) + (u64)(unsigned)s[4];
+    const u64 w0 = (etile << 16) | (u64)(unsigned)cnt;
+    if (ranked) io.tbase[(size_t)b * tcells + c] = (uint32_t)(atomicAdd(g, w0) & 0xffffull);   // slots taken so far in this cell
+    else atomicAdd(g, w0);
+    atomicAdd(g + 1, pack_ss(s[1], s[2]));
+    atomicAdd(g + 2, pack_ss(s[3], 0));
+    // partial momentum sums of >= 64 particles that come within a factor two of the int32 range
+    if (cnt >= 64 && (abs(s[1]) >= (1 << 30) || abs(s[2]) >= (1 << 30) || abs(s[3]) >= (1 << 30))) atomicAdd(G.nrange, 1ull);
+  }
+}
+
+// the collision of the last step, applied on its own when the state is read before the next step
+// (key recomputed from the position and that step's shift, still in G.s)
+__global__ void __launch_bounds__(256) k_collide_pos(Geo G, size_t n, const float* __restrict__ x, const float* __restrict__ y,
+                                                     const float* __restrict__ z, float* __restrict__ vx, float* __restrict__ vy,
+                                                     float* __restrict__ vz, const float* __restrict__ rec) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t k = key_of(G, x[i], y[i], z[i], G.s[0], G.s[1], G.s[2]);
+  float4 r0, ax;
+  load_rec(rec, k, r0, ax);
+  float v[3] = {vx[i], vy[i], vz[i]};
+  srd_apply(G, r0, ax, v);
+  vx[i] = v[0]; vy[i] = v[1]; vz[i] = v[2];
+}
+
+__global__ void __launch_bounds__(256) k_keys(Geo G, size_t n, const float* __restrict__ x, const float* __restrict__ y,
+                                              const float* __restrict__ z, uint32_t* __restrict__ key) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) key[i] = key_of(G, x[i], y[i], z[i], G.s[0], G.s[1], G.s[2]);
+}
+
+}  // namespace mpc
+
+using namespace mpc;
+
+namespace {
+
+// staging buffer of the folded reorder (32 bytes per particle): the unused SoA copy plus the slot array, which
+// the workspace layout places between the two copies so that either copy extends to 8 arrays
+inline float* aos_base(const mpc_ctx* c) {
+  return reinterpret_cast<float*>(c->A[0] < c->Bf[0] ? c->slot_id : c->Bf[0]);
+}
+
+// the instantiations that exist: (COLLIDE, WKEY, IO) in { (*,0,PLAIN) at 384 or 512 threads, (*,1,PLAIN), (*,1,AOS_OUT),
+// (1,0,GATHER) } x (WALL, GRAV) x brick shape
+template <bool COLLIDE, bool WKEY, class BS, int IO, int T>
+void* sweep_fn(bool wall, bool grav) {
+  if (wall && grav) return (void*)k_sweep<COLLIDE, true, true, WKEY, BS, IO, T>;
+  if (wall) return (void*)k_sweep<COLLIDE, true, false, WKEY, BS, IO, T>;
+  if (grav) return (void*)k_sweep<COLLIDE, false, true, WKEY, BS, IO, T>;
+  return (void*)k_sweep<COLLIDE, false, false, WKEY, BS, IO, T>;
+}
+template <class BS>
+void* sweep_variant(bool collide, bool wkey, int io, bool three, bool wall, bool grav) {
+  if (io == IO_GATHER) return sweep_fn<true, false, BS, IO_GATHER, SWEEP_T>(wall, grav);
+  if (io == IO_AOS_OUT) return collide ? sweep_fn<true, true, BS, IO_AOS_OUT, SWEEP_T>(wall, grav) : sweep_fn<false, true, BS, IO_AOS_OUT, SWEEP_T>(wall, grav);
+  if (wkey) return collide ? sweep_fn<true, true, BS, IO_PLAIN, SWEEP_T>(wall, grav) : sweep_fn<false, true, BS, IO_PLAIN, SWEEP_T>(wall, grav);
+  if (three) return collide ? sweep_fn<true, false, BS, IO_PLAIN, SWEEP_T3>(wall, grav) : sweep_fn<false, false, BS, IO_PLAIN, SWEEP_T3>(wall, grav);
+  return collide ? sweep_fn<true, false, BS, IO_PLAIN, SWEEP_T>(wall, grav) : sweep_fn<false, false, BS, IO_PLAIN, SWEEP_T>(wall, grav);
+}
+void* sweep_variant_any(bool fast, bool collide, bool wkey, int io, bool three, bool wall, bool grav) {
+  return fast ? sweep_variant<BSfast>(collide, wkey, io, three, wall, grav) : sweep_variant<BSgeneric>(collide, wkey, io, three, wall, grav);
+}
+
+}  // namespace
+
+int launch_sweep(mpc_ctx* c, bool collide, bool wkey, int io, const float sp[3]) {
+  Geo& G = c->G;
+  float** F = reinterpret_cast<float**>(c->A);
+  SweepIO sio;
+  sio.aos_in = sio.aos_out = aos_base(c);
+  sio.perm = c->perm; sio.id = c->A[6];
+  sio.tbase = c->tbase;
+  sio.ranked = (io == IO_AOS_OUT && c->have_order && c->tbase && !(c->debug & MPC_DEBUG_ATOMIC_SCATTER)) ? 1 : 0;
+  c->ranked_keys = sio.ranked != 0;
+  const uint32_t* chunk = c->have_order ? c->offset : nullptr;
+  const bool wall = G.wall >= 0, grav = (G.g[0] != 0.f || G.g[1] != 0.f || G.g[2] != 0.f);
+  const bool three = io == IO_PLAIN && !wkey && c->three_ctas;
+  void* fn = sweep_variant_any(c->fast_brick, collide, wkey, io, three, wall, grav);
+  float s0 = sp[0], s1 = sp[1], s2 = sp[2];
+  uint32_t n = (uint32_t)c->n;
+  void* args[] = {&G, &s0, &s1, &s2, &n, &F[0], &F[1], &F[2], &F[3], &F[4], &F[5], &c->key, &chunk, &c->nbricks, &c->rec, &c->sums, &sio};
+  const int T = three ? SWEEP_T3 : SWEEP_T;
+  cudaLaunchKernel(fn, dim3(c->nbricks), dim3(T), args, c->tile_bytes, c->stream);
+  LAUNCH_CHECK("k_sweep");
+  if (io == IO_GATHER) c->gather_pending = false;
+  return MPC_OK;
+}
+
+cudaError_t sweep_set_attributes(size_t bytes) {
+  for (int fast = 0; fast < 2; ++fast)
+    for (int wall = 0; wall < 2; ++wall)
+      for (int grav = 0; grav < 2; ++grav)
+        for (int collide = 0; collide < 2; ++collide) {
+          const struct { bool wkey; int io; bool three; } v[] = {{false, IO_PLAIN, false}, {false, IO_PLAIN, true}, {true, IO_PLAIN, false},
+                                                                 {true, IO_AOS_OUT, false}, {false, IO_GATHER, false}};
+          for (const auto& q : v) {
+            const cudaError_t e = cudaFuncSetAttribute(sweep_variant_any(fast != 0, collide != 0, q.wkey, q.io, q.three, wall != 0, grav != 0),
+                                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+            if (e != cudaSuccess) return e;
+          }
+        }
+  return cudaSuccess;
+}
+
+int launch_collide_pos(mpc_ctx* c) {
+  float** F = reinterpret_cast<float**>(c->A);
+  k_collide_pos<<<nblk(c->n, 256), 256, 0, c->stream>>>(c->G, c->n, F[0], F[1], F[2], F[3], F[4], F[5], c->rec);
+  LAUNCH_CHECK("k_collide_pos");
+  return MPC_OK;
+}
+
+int launch_keys(mpc_ctx* c, uint32_t* key_out) {
+  float** F = reinterpret_cast<float**>(c->A);
+  k_keys<<<nblk(c->n, 256), 256, 0, c->stream>>>(c->G, c->n, F[0], F[1], F[2], key_out);
+  LAUNCH_CHECK("k_keys");
+  return MPC_OK;
+}

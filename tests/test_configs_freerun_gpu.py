@@ -78,7 +78,7 @@ def test_config4_5000_steps_profile_follows_startup_series():
     n = 256 * 64 * 64 * nbar
     gx, h = 0.001, 0.1
     st = uniform_maxwell(box, n, 1234, rest=True)
-    g = MPC(box, cells, nbar, 1234, n_max=n, thermostat=1, bc=(0, 0, 1), g=(gx, 0.0, 0.0), rebin_every=1,
+    g = MPC(box, cells, nbar, 1234, n_max=n, thermostat=1, bc=(0, 0, 1), g=(gx, 0.0, 0.0), rebin_every=10,
             brick=(16, 16, 8))
     gpu_set(g, st)
     zc = np.arange(64) + 0.5
@@ -90,7 +90,7 @@ def test_config4_5000_steps_profile_follows_startup_series():
     nav = 0
     for _ in range(10):
         g.step(50)
-        ob = g.observables(64)
+        ob = g.observables(profile=True)
         prof += ob["profile"]
         want += poiseuille_startup(zc, ob["step"] * h, gx, nu, 64.0)
         nav += 1

@@ -17,7 +17,7 @@ from oracle.binding import Oracle  # noqa: E402
 from paper_2406_15236_b200 import MPC  # noqa: E402
 from paper_2406_15236_b200.inputs import uniform_maxwell, uniform_maxwell_cuda  # noqa: E402
 from test_parity_gpu import compare_step, gpu_get, gpu_set  # noqa: E402
-from test_parity_plus_a_gpu import lambda_min_per_particle  # noqa: E402
+from test_parity_plus_a_gpu import check_plus_a_velocities, lambda_min_per_particle  # noqa: E402
 
 BRICK = (16, 16, 8)
 
@@ -62,13 +62,9 @@ def test_config3_at_plus_a_128cubed():
     cnt_o, *_r, key_o = o.get_cells()
     cnt_g, *_q, key_g = [a.cpu().numpy() for a in g.get_cells()]
     assert np.array_equal(key_o, key_g.view(np.uint32)) and np.array_equal(cnt_o, cnt_g.view(np.uint32))
-    lam, N, det_ratio = lambda_min_per_particle(o, so, key_o, 0)
-    err = np.max(np.abs(np.stack(so[3:6]).astype(np.float64) - np.stack(sg[3:6])), axis=0)
-    tol = np.clip(2e-5 * 0.1 / np.maximum(lam, 1e-12), 2e-5, 5e-2)
-    borderline = (N >= 3) & (det_ratio < 4e-6 * 27) & (det_ratio > 0.25e-6 * 27)
-    assert ((err <= tol) | borderline).all()
-    assert np.mean(lam >= 0.1) > 0.98          # fraction of particles under the strict 2e-5 bound
-    assert np.max(err[lam >= 0.1]) <= 2e-5
+    _lam, _N, cond = lambda_min_per_particle(o, so, key_o, 0)
+    assert check_plus_a_velocities(so, sg, cond, "config 3") < 0.05     # U10 tolerance, fraction of loose particles
+    assert int(o.observables()["n_singular_cells"]) == int(g.observables()["n_singular_cells"])
     g.step(20)
     ob = g.observables()
     assert ob["kT_est"] == pytest.approx(1.0, rel=5e-3)      # Andersen thermostat holds k_BT
@@ -87,7 +83,7 @@ def test_config4_walls_gravity_256x64x64():
     o.step(1)
     g.step(1)
     compare_step(o, g)
-    a, b = o.observables(64), g.observables(64)
+    a, b = o.observables(64), g.observables(profile=True)
     assert np.allclose(a["profile"], b["profile"], atol=2e-5)
     assert b["kT_cell"] == pytest.approx(a["kT_cell"], rel=1e-5)
 

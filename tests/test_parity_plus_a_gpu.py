@@ -1,9 +1,8 @@
 """GPU parity for the angular-momentum-conserving variants SRD+a (Eqs. 3-4) and
-MPC-AT+a (U5). Tolerance per DESIGN.md U10: 2e-5 sqrt(kT/m) where the cell's inertia tensor
-is well conditioned in absolute terms (smallest eigenvalue >= 0.1 m a^2; the typical value at
-<N_c> = 10 is ~1), growing as 1/lambda_min below that (omega = I^-1 dL amplifies the 2^-22 fixed-point
-quantum of the sums; measured: err * lambda_min <= 4.4e-6 over 2.1e7 particles), capped at 5e-2: a nearly
-collinear triplet has no well-defined omega, both answers conserve L."""
+MPC-AT+a (U5). Tolerance = SURVEY.md 8(c) reading U10: 2e-5 sqrt(kT/m) for particles of cells whose inertia
+tensor has condition number <= 10^2, 1e-3 otherwise (omega = I^-1 dL amplifies fp32 rounding of the per-particle
+omega x r_c by the conditioning); the fraction of loosely compared particles is printed. No cell is exempt: the
+rejection rule of U10 is evaluated in double on both sides, so both must reject the same cells (equal counts)."""
 import numpy as np
 import pytest
 
@@ -17,7 +16,8 @@ from test_parity_gpu import gpu_get, gpu_set  # noqa: E402
 
 
 def lambda_min_per_particle(o, so, key, step):
-    """Smallest eigenvalue of every cell's inertia tensor / (m a^2) (N=2: sum |r|^2), per particle."""
+    """Per particle: smallest eigenvalue of its cell's inertia tensor / (m a^2) (N=2: sum |r|^2), the cell's occupancy,
+    and the condition number of the tensor (1 for N <= 2, where U10 does not invert a tensor)."""
     s = o.grid_shift(step).astype(np.float32)
     q = np.stack(so[0:3], 1) + s
     rho = (q - np.floor(q)).astype(np.float64)
@@ -34,8 +34,20 @@ def lambda_min_per_particle(o, so, key, step):
     ev = np.linalg.eigvalsh(I)
     lam = np.where(N == 2, np.bincount(key, weights=r2, minlength=nk), ev[:, 0])
     with np.errstate(invalid="ignore", divide="ignore"):
-        det_ratio = np.where(N >= 3, np.prod(ev, axis=1) / np.maximum(ev.mean(axis=1), 1e-300) ** 3, 1.0)
-    return lam[key], N[key], det_ratio[key]
+        cond = np.where(N >= 3, ev[:, 2] / np.maximum(ev[:, 0], 1e-300), 1.0)
+    return lam[key], N[key], cond[key]
+
+
+def check_plus_a_velocities(so, sg, cond, label=""):
+    """U10 tolerance: 2e-5 where cond(I_c) <= 1e2, 1e-3 elsewhere; returns the fraction compared loosely."""
+    err = np.max(np.abs(np.stack(so[3:6]).astype(np.float64) - np.stack(sg[3:6])), axis=0)
+    loose = cond > 1e2
+    tol = np.where(loose, 1e-3, 2e-5)
+    worst = int(np.argmax(err / tol))
+    assert (err <= tol).all(), f"{label}: err {err[worst]:.3g} > tol {tol[worst]:.3g} at cond {cond[worst]:.3g}"
+    print(f"{label}: max err strict {err[~loose].max(initial=0):.3g}, loose {err[loose].max(initial=0):.3g}, "
+          f"loosely compared fraction {loose.mean():.4f}")
+    return loose.mean()
 
 
 @pytest.mark.parametrize("collision,nbar,every,brick", [(0, 10, 1, 4), (0, 10, 3, (16, 16, 8)), (0, 3, 1, 1),
@@ -61,19 +73,11 @@ def test_plus_a_parity(collision, nbar, every, brick):
         cnt_g, gx, gy, gz, _ge, key_g = [a.cpu().numpy() for a in g.get_cells()]
         assert np.array_equal(key_o, key_g.view(np.uint32))
         assert np.array_equal(cnt_o, cnt_g.view(np.uint32))
-        lam, N, det_ratio = lambda_min_per_particle(o, so, key_o, t)
-        err = np.max(np.abs(np.stack(so[3:6]).astype(np.float64) - np.stack(sg[3:6])), axis=0)
-        tol = np.clip(2e-5 * 0.1 / np.maximum(lam, 1e-12), 2e-5, 5e-2)
-        # cells whose determinant test (U10) sits within a factor 4 of its threshold may be decided
-        # differently in fp64-from-fp32-sums and in the oracle's direct fp64: compare them loosely
-        borderline = (N >= 3) & (det_ratio < 4e-6 * 27) & (det_ratio > 0.25e-6 * 27)
-        ok = (err <= tol) | borderline
-        assert ok.all(), f"worst err/tol = {np.max(err / tol):.2f} at lambda_min={lam[np.argmax(err / tol)]:.3g}"
-        assert borderline.mean() < 1e-3
+        _lam, _N, cond = lambda_min_per_particle(o, so, key_o, t)
+        frac = check_plus_a_velocities(so, sg, cond, f"collision={collision} nbar={nbar} t={t}")
         if nbar == 10:
-            assert np.mean(lam >= 0.1) > 0.97 and np.max(err[lam >= 0.1]) <= 2e-5
-        ns_o, ns_g = o.observables()["n_singular_cells"], g.observables()["n_singular_cells"]
-        assert abs(int(ns_o) - int(ns_g)) <= max(1, int(borderline.sum()))
+            assert frac < 0.05
+        assert int(o.observables()["n_singular_cells"]) == int(g.observables()["n_singular_cells"])
 
 
 @pytest.mark.parametrize("collision", [0, 1])
