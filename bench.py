@@ -102,8 +102,7 @@ def oracle_rate(wl, nbar, budget_s=12.0):
     kw = dict(wl["kw"])
     kw.update(rebin_every=wl["rebin_every"], brick=1)
     o = Oracle(box, cells, nbar, 1234, **kw)
-    rest = "g" in kw
-    o.set_state(*uniform_maxwell(box, n, 1234, rest=rest))
+    o.set_state(*uniform_maxwell(box, n, 1234))
     t0 = time.perf_counter()
     o.step(1)
     t1 = time.perf_counter() - t0
@@ -143,7 +142,7 @@ def run_reference(args, wl, rank, world):
     kw = dict(wl["kw"])
     kw.update(rebin_every=wl["rebin_every"], brick=1)
     o = Oracle(box, cells, nbar, 1234, **kw)
-    o.set_state(*uniform_maxwell(box, n, 1234, rest="g" in kw))
+    o.set_state(*uniform_maxwell(box, n, 1234))
     o.step(args.warmup)
     t0 = time.perf_counter()
     o.step(args.steps)
@@ -209,14 +208,10 @@ def measure(args, workload, nbar, steps, warmup, rank, local_rank, world, dist, 
     brick = brick * 3 if len(brick) == 1 else brick
     kw.update(rebin_every=wl["rebin_every"], brick=brick)
     compact = args.compact or (n * 72 + int(np.prod(cells)) * 80 > 150e9)
-    rest = "g" in kw
     # a state that does not fit beside the workspace (20 per cell: 64 GB + 138 GB) is made array by array on the
     # device, parked in pinned host memory and handed over through the host-pointer ABI
     via_host = n * 24 + n * 52 + int(np.prod(cells)) * 80 > 170e9
     st = list(uniform_maxwell_cuda(box, n, 1234 + rank, device=str(device), to_host=via_host))
-    if rest:
-        for v in st[3:]:
-            v.zero_()
     torch.cuda.empty_cache()
     sim = MPC(box, cells, nbar, 1234 + rank, n_max=n, device=str(device), compact=compact, **kw)
     if via_host:

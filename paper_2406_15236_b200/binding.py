@@ -177,6 +177,27 @@ class MPC:
         self._check(self.lib.mpc_get_state(self._h, *[_ptr(t) for t in out], _ptr(ids)))
         return (*out, ids)
 
+    def canonicalise(self):
+        """Bring the state into the form mpc_get_state returns (last collision applied, (key, id) order inside every
+        cell) without copying anything out: indices into the internal order stay valid until the next step."""
+        self._check(self.lib.mpc_get_state(self._h, *([None] * 7)))
+
+    def get_state_at(self, index):
+        """Particles `index` (a device int64 tensor of positions in the current internal order) as seven host numpy
+        arrays (x,y,z,vx,vy,vz,id). Pulls one full array at a time through mpc_get_state (NULL = skipped), so it needs
+        4 n bytes of device memory beside the workspace instead of 28 n."""
+        torch = self._torch
+        res = []
+        for a in range(7):
+            buf = torch.empty(self.n, dtype=torch.float32 if a < 6 else torch.int32, device=self.device)
+            ptrs = [None] * 7
+            ptrs[a] = C.c_void_p(buf.data_ptr())
+            self._check(self.lib.mpc_get_state(self._h, *ptrs))
+            res.append(buf[index].cpu().numpy())
+            del buf
+        res[6] = res[6].view(np.uint32)
+        return tuple(res)
+
     def get_state_host(self, out=None):
         """Returns numpy arrays (x,y,z,vx,vy,vz,id); `out` may supply 7 pre-allocated host tensors."""
         torch = self._torch

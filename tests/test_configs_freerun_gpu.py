@@ -70,14 +70,14 @@ def test_config3_500_steps_at_plus_a():
 
 def test_config4_5000_steps_profile_follows_startup_series():
     # config 4: SRD + MBS, 256x64x64 cells, no-slip walls at z = 0, 64 (bounce-back + virtual wall particles),
-    # g = 0.001 x, from rest, 5,000 steps of 0.1. One viscous relaxation time (U14): the profile is compared with
+    # g = 0.001 x, fluid at rest (Maxwell velocities, zero mean flow), 5,000 steps of 0.1. One viscous relaxation time (U14): the profile is compared with
     # the start-up series of plane Poiseuille flow for the analytic SRD viscosity nu = 0.8700, averaged over the
     # same sampling times, not with the steady parabola.
     cells, nbar = (256, 64, 64), 10
     box = (256.0, 64.0, 64.0)
     n = 256 * 64 * 64 * nbar
     gx, h = 0.001, 0.1
-    st = uniform_maxwell(box, n, 1234, rest=True)
+    st = uniform_maxwell(box, n, 1234)
     g = MPC(box, cells, nbar, 1234, n_max=n, thermostat=1, bc=(0, 0, 1), g=(gx, 0.0, 0.0), rebin_every=10,
             brick=(16, 16, 8))
     gpu_set(g, st)
@@ -105,3 +105,4 @@ def test_config4_5000_steps_profile_follows_startup_series():
     assert np.abs(prof - amp * want).max() < 0.03 * vmax
     assert np.abs(prof - prof[::-1]).max() < 0.02 * vmax                          # symmetric about the mid-plane
     assert ob["kT_cell"] == pytest.approx(1.0, rel=5e-3)                          # thermostat holds k_BT under forcing
+    assert ob["n_range_overflows"] == 0

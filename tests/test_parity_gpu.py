@@ -165,7 +165,7 @@ def test_one_call_of_k_steps_equals_k_calls(kw):
     cells, nbar = (32, 16, 16), 10
     box = tuple(float(c) for c in cells)
     n = int(np.prod(cells)) * nbar
-    st = uniform_maxwell(box, n, 31, rest="g" in kw)
+    st = uniform_maxwell(box, n, 31)
     res = []
     for calls in ((9,), (1,) * 9, (4, 5), (2, 3, 4)):
         g = MPC(box, cells, nbar, 17, n_max=n, **kw)
@@ -338,7 +338,7 @@ def test_reorder_code_paths_agree(kw):
     cells, nbar = (32, 16, 16), 10
     box = tuple(float(c) for c in cells)
     n = int(np.prod(cells)) * nbar - 13          # ragged tail: not a multiple of 32
-    st = uniform_maxwell(box, n, 77, rest="g" in kw)
+    st = uniform_maxwell(box, n, 77)
     res = []
     for flags in (0, B.DEBUG_NO_FUSE_GATHER, B.DEBUG_EAGER_CANONICAL, B.DEBUG_ATOMIC_SCATTER, B.DEBUG_EAGER_COLLIDE):
         g = MPC(box, cells, nbar, 23, n_max=n, **kw)
