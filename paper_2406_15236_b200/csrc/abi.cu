@@ -201,6 +201,7 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   c->tile_bytes = tile_cells * TILE_W * 4;
   c->three_ctas = 3 * (c->tile_bytes + 1024) <= 227 * 1024;
   c->fast_brick = (G.bs[0] == 4 && G.bs[1] == 4 && G.bs[2] == 3);
+  c->pow2_cells = wall < 0 && !(G.m[0] & (G.m[0] - 1)) && !(G.m[1] & (G.m[1] - 1)) && !(G.m[2] & (G.m[2] - 1));
   {
     const int bvs = G.bs[0] + G.bs[1] + G.bs[2];
     c->cell_cpb_shift = bvs > 8 ? bvs - 8 : 0;      // k_cell: CTAs of 256 cells

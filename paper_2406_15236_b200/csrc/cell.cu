@@ -43,76 +43,81 @@ __device__ __forceinline__ float mbs_exponentials(const Geo& G, uint32_t cid, ui
 // grid = (mb0 * CTAs-per-brick, mb1, mb2): the brick coordinates come from blockIdx, no division.
 // zero != 0: the sums of a cell are cleared once read, which saves the memset before the next step's sweep.
 // The number of Philox blocks a cell needs for its thermostat draw grows with its occupancy (Poisson), and a warp runs
-// as long as its fullest cell needs: the CT cells of a CTA are therefore counting-sorted by that number in shared memory
-// and the draws are made in sorted order (every warp gets cells of nearly equal cost); the owner thread finishes.
+// as long as its fullest cell needs. Two phases: (A) thread t reads the sums of cell t (coalesced), reduces them to
+// {v_cm, sum |v - v_cm|^2, N_c} and parks that in shared memory; the CT cells of the CTA are counting-sorted by their
+// number of Philox blocks; (B) thread j finishes the j-th cell of the sorted order (draw, kappa, axis, one 32-byte
+// record): every warp gets cells of nearly equal cost, and there is no barrier after the loop of variable length.
+struct CellWork { float vx, vy, vz, w2; uint32_t cid, nc; };
 template <int CT>
 __global__ void __launch_bounds__(CT) k_cell(Geo G, int cpb_shift, int ct_shift, u64* __restrict__ sums, float* __restrict__ rec, int zero) {
   __shared__ unsigned hist[32];
   __shared__ unsigned short order[CT];
-  __shared__ uint32_t s_cid[CT];
-  __shared__ unsigned short s_M[CT];
-  __shared__ float s_e[CT];
+  __shared__ CellWork work[CT];
   const unsigned tid = threadIdx.x;
   if (tid < 32) hist[tid] = 0u;
   const int b0 = G.bs[0], b1 = G.bs[1], b2 = G.bs[2];
   const uint32_t bx = blockIdx.x >> cpb_shift, by = blockIdx.y, bz = blockIdx.z;
-  const uint32_t local = ((blockIdx.x & ((1u << cpb_shift) - 1u)) << ct_shift) | tid;
+  const uint32_t lbase = (blockIdx.x & ((1u << cpb_shift) - 1u)) << ct_shift;
+  const uint32_t local = lbase | tid;
   const bool valid = local < (1u << (b0 + b1 + b2));
   const uint32_t brick = (bz * (uint32_t)G.mb[1] + by) * (uint32_t)G.mb[0] + bx;
-  const uint32_t k = (brick << (b0 + b1 + b2)) | local;
-  u64* s = sums + (size_t)k * G.sw;
+  const uint32_t kbase = (brick << (b0 + b1 + b2)) | lbase;
+  // ---- phase A ----
+  u64* s = sums + (size_t)(kbase + tid) * G.sw;
   u64 w0 = 0ull;
   if (valid) w0 = s[0];
   const uint32_t nreal = (uint32_t)(w0 & 0xffffull);
-  const bool live = valid && nreal != 0u;
-  uint32_t cid = 0u, Nc = nreal, M = 0u;
-  double S0 = 0.0, S1 = 0.0, S2 = 0.0, E = 0.0, W2 = 0.0, inv = 0.0;
-  if (live) {
+  CellWork cw = {0.f, 0.f, 0.f, 0.f, 0u, 0u};
+  uint32_t M = 0u;
+  if (valid && nreal != 0u) {
     const int ix = (int)((bx << b0) | (local & ((1u << b0) - 1u)));
     const int iy = (int)((by << b1) | ((local >> b0) & ((1u << b1) - 1u)));
     const int iz = (int)((bz << b2) | (local >> (b0 + b1)));
-    cid = canonical_id(G, ix, iy, iz);
+    cw.cid = canonical_id(G, ix, iy, iz);
     int sx, sy, sz, pad;
     unpack_ss(s[1], sx, sy);
     unpack_ss(s[2], sz, pad);
     if (zero) { s[0] = 0ull; s[1] = 0ull; s[2] = 0ull; }
-    S0 = (double)sx * G.fxv_inv; S1 = (double)sy * G.fxv_inv; S2 = (double)sz * G.fxv_inv;
+    double S0 = (double)sx * G.fxv_inv, S1 = (double)sy * G.fxv_inv, S2 = (double)sz * G.fxv_inv;
     // a cell total within a factor two of the int32 range of the momentum words, or too many particles for the tile's
     // packed count / energy words
     if (nreal >= 64u && (nreal >= MAX_CELL_COUNT || abs(sx) >= (1 << 30) || abs(sy) >= (1 << 30) || abs(sz) >= (1 << 30))) atomicAdd(G.nrange, 1ull);
-    {
-      E = (double)(w0 >> 16) * G.fxe_inv;
-      if (G.wall >= 0 && !G.slip) {
-        // virtual wall particles fill wall-cut cells up to nbar (U8)
-        const int w = G.wall;
-        const int iw = (w == 0) ? ix : (w == 1) ? iy : iz;
-        const float sw = (w == 0) ? G.s[0] : (w == 1) ? G.s[1] : G.s[2];
-        const int nw = (w == 0) ? G.n[0] : (w == 1) ? G.n[1] : G.n[2];
-        const bool cut = (sw > 0.0f) ? (iw == 1 || iw == nw + 1) : (sw < 0.0f) ? (iw == 0 || iw == nw) : false;
-        if (cut && (int)nreal < G.nbar) {
-          const uint32_t nv = (uint32_t)G.nbar - nreal;
-          for (uint32_t j = 0; j < nv; ++j) {
-            const Block4 o = philox_rk(cid, j, G.t, TAG_WALL, G.rk);
-            float g0, g1, g2;
-            normals3(o, g0, g1, g2);
-            const double a = (double)(G.sigma * g0), b = (double)(G.sigma * g1), c = (double)(G.sigma * g2);
-            S0 += a; S1 += b; S2 += c; E += a * a + b * b + c * c;
-          }
-          Nc += nv;
+    double E = (double)(w0 >> 16) * G.fxe_inv;
+    uint32_t Nc = nreal;
+    if (G.wall >= 0 && !G.slip) {
+      // virtual wall particles fill wall-cut cells up to nbar (U8)
+      const int w = G.wall;
+      const int iw = (w == 0) ? ix : (w == 1) ? iy : iz;
+      const float sw = (w == 0) ? G.s[0] : (w == 1) ? G.s[1] : G.s[2];
+      const int nw = (w == 0) ? G.n[0] : (w == 1) ? G.n[1] : G.n[2];
+      const bool cut = (sw > 0.0f) ? (iw == 1 || iw == nw + 1) : (sw < 0.0f) ? (iw == 0 || iw == nw) : false;
+      if (cut && (int)nreal < G.nbar) {
+        const uint32_t nv = (uint32_t)G.nbar - nreal;
+        for (uint32_t j = 0; j < nv; ++j) {
+          const Block4 o = philox_rk(cw.cid, j, G.t, TAG_WALL, G.rk);
+          float g0, g1, g2;
+          normals3(o, g0, g1, g2);
+          const double a = (double)(G.sigma * g0), b = (double)(G.sigma * g1), c = (double)(G.sigma * g2);
+          S0 += a; S1 += b; S2 += c; E += a * a + b * b + c * c;
         }
-      }
-      inv = 1.0 / (double)Nc;
-      if (G.thermostat && Nc >= 2u) {
-        W2 = E - (S0 * S0 + S1 * S1 + S2 * S2) * inv;   // sum |v - vcm|^2
-        if (W2 > 0.0) M = (3u * (Nc - 1u)) >> 1;
+        Nc += nv;
       }
     }
+    // 1 / N_c: float reciprocal refined by one Newton step in double (relative error < 1e-14; a double division costs twice as much)
+    double inv = (double)__frcp_rn((float)Nc);
+    inv = inv * (2.0 - (double)Nc * inv);
+    cw.vx = (float)(S0 * inv); cw.vy = (float)(S1 * inv); cw.vz = (float)(S2 * inv);
+    cw.nc = Nc;
+    if (G.thermostat && Nc >= 2u) {
+      const double W2 = E - (S0 * S0 + S1 * S1 + S2 * S2) * inv;   // sum |v - vcm|^2
+      if (W2 > 0.0) { M = (3u * (Nc - 1u)) >> 1; cw.w2 = (float)W2; }
+    }
   }
-  // ---- counting sort of the CTA's cells by the number of Philox blocks of their draw ----
-  const unsigned bin = min((M + 3u) >> 2, 31u);
+  // ---- counting sort of the CTA's cells by the number of Philox blocks of their draw (empty cells last) ----
+  const unsigned bin = cw.nc ? min((M + 3u) >> 2, 30u) : 31u;
   __syncthreads();
   const unsigned rank = atomicAdd(&hist[bin], 1u);
-  s_cid[tid] = cid; s_M[tid] = (unsigned short)M;
+  work[tid] = cw;
   __syncthreads();
   if (tid < 32) {
     const unsigned v = hist[tid];
@@ -127,37 +132,31 @@ __global__ void __launch_bounds__(CT) k_cell(Geo G, int cpb_shift, int ct_shift,
   __syncthreads();
   order[hist[bin] + rank] = (unsigned short)tid;
   __syncthreads();
-  {
-    const unsigned u = order[tid];
-    s_e[u] = mbs_exponentials(G, s_cid[u], s_M[u]);
-  }
-  __syncthreads();
-  if (!live) return;
-  float4 r0, r1;
-  {
-    r0.x = (float)(S0 * inv); r0.y = (float)(S1 * inv); r0.z = (float)(S2 * inv);
-    const Block4 o = philox_rk(cid, 0u, G.t, TAG_AXIS, G.rk);
-    float kappa = 1.0f;
-    if (M) {
-      float ek = s_e[tid];
-      if ((3u * (Nc - 1u)) & 1u) {   // f odd: half a squared normal from words 2, 3 of the axis block (U6)
-        // cos(2 pi u) = -cos(2 pi (u - 1/2)), argument in [-pi, pi): __cosf / __logf are accurate to ~4e-7 absolute there,
-        // far below the statistical meaning of the draw and the 2e-5 parity budget
-        const float cs = __cosf(6.2831853071795865f * (u01_co(o.d) - 0.5f));
-        ek -= __logf(u01_oc(o.c)) * cs * cs;
-      }
-      const float x = __fdividef(2.0f * (G.kT * ek), G.mass * (float)W2);
-      kappa = x * rsqrtf(fmaxf(x, 1e-37f));
+  // ---- phase B ----
+  const unsigned u = order[tid];
+  const CellWork c = work[u];
+  if (c.nc == 0u) return;
+  const Block4 o = philox_rk(c.cid, 0u, G.t, TAG_AXIS, G.rk);
+  float kappa = 1.0f;
+  if (c.w2 > 0.0f) {
+    const uint32_t f = 3u * (c.nc - 1u);
+    float ek = mbs_exponentials(G, c.cid, f >> 1);
+    if (f & 1u) {   // f odd: half a squared normal from words 2, 3 of the axis block (U6)
+      // cos(2 pi u) = -cos(2 pi (u - 1/2)), argument in [-pi, pi): __cosf / __logf are accurate to ~4e-7 absolute there,
+      // far below the statistical meaning of the draw and the 2e-5 parity budget
+      const float cs = __cosf(6.2831853071795865f * (u01_co(o.d) - 0.5f));
+      ek -= __logf(u01_oc(o.c)) * cs * cs;
     }
-    r0.w = kappa;
-    const float zz = 2.0f * u01_co(o.a) - 1.0f;
-    const float rr = sqrtf((1.0f - zz) * (1.0f + zz));
-    float sp, cp;
-    sincospif(2.0f * u01_co(o.b), &sp, &cp);
-    r1 = make_float4(rr * cp, rr * sp, zz, 0.0f);
+    const float x = __fdividef(2.0f * (G.kT * ek), G.mass * c.w2);
+    kappa = x * rsqrtf(fmaxf(x, 1e-37f));
   }
-  reinterpret_cast<float4*>(rec)[(size_t)k * 2] = r0;
-  reinterpret_cast<float4*>(rec)[(size_t)k * 2 + 1] = r1;
+  const float zz = 2.0f * u01_co(o.a) - 1.0f;
+  const float rr = sqrtf((1.0f - zz) * (1.0f + zz));
+  float sp, cp;
+  sincospif(2.0f * u01_co(o.b), &sp, &cp);
+  float4* out = reinterpret_cast<float4*>(rec) + (size_t)(kbase + u) * 2;
+  out[0] = make_float4(c.vx, c.vy, c.vz, kappa);
+  out[1] = make_float4(rr * cp, rr * sp, zz, 0.0f);
 }
 
 }  // namespace mpc

@@ -34,7 +34,7 @@ typedef unsigned long long u64;
 constexpr int HALO = 1;               // tile halo in cells on every side of a brick
 constexpr int SWEEP_T = 512;          // threads per sweep CTA (2 CTAs per SM): first-step and staged reorder sweeps
 constexpr int SWEEP_T3 = 384;         // ... of the steady-state sweep when three tiles fit in an SM's shared memory
-constexpr int PF_DIST = 4;            // L2 prefetch distance of the sweep, in iterations of T particles
+constexpr int PF_DIST = 4;            // L2 prefetch distance of the sweep, in iterations of T particles (3..6 equal, 8: +2.5 %)
 constexpr int TILE_W = 5;             // int32 words per tile cell: N, Sx, Sy, Sz, E
 constexpr int REC_W = 8;              // floats per cell record (32 B, one sector)
 constexpr int OBS_BLOCKS = 1184;      // 148 SMs x 8
@@ -257,6 +257,7 @@ struct mpc_ctx {
   // the collision of the last step of an mpc_step call stays pending: the next call's first sweep
   // applies it; every call that reads particle velocities applies it first (flush_collide)
   bool collide_pending;
+  bool pow2_cells;      // no walls and every m[d] a power of two: the sweep folds indices with a mask
   bool ranked_keys;     // the last staging sweep wrote (tile cell, arrival rank) words into key[] instead of keys
   unsigned debug;       // MPC_DEBUG_* flags
   int device;           // CUDA device of the workspace

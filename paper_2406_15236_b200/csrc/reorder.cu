@@ -168,12 +168,12 @@ __global__ void __launch_bounds__(256) k_scatter_src(size_t n, const uint32_t* _
   }
 }
 
-// Hot-path variant when the previous order is known: the staging sweep (k_sweep<.., IO_AOS_OUT>) has given every
-// particle its arrival rank inside (CTA, tile cell) -- the value its shared-memory count atomic returned -- and every
-// CTA the first slot of its particles inside each cell's segment (the value the tile flush's global atomic returned).
-// The slot of a particle is then offset[key] + first slot + rank: no atomics, no dependent chain, one CTA per brick
-// with the brick's slot table in shared memory. word = tile cell << 16 | rank, or bit 31 | rank for the few particles
-// that left their brick's tile (their key is recomputed from the staged position).
+// Hot-path variant when the previous order is known: the staging sweep (k_sweep<.., IO_AOS_OUT>) has written every
+// particle's tile cell, and its tile flush has given every CTA the first slot of its particles inside each cell's
+// segment (the value the flush's global atomic returned). One CTA per brick then hands out the slots with
+// shared-memory counters: slot = offset[key] + first slot of the CTA + arrival rank in (CTA, cell). No global atomics,
+// no dependent global chain. word = tile cell, or bit 31 | slot-in-segment for the few particles that left their
+// brick's tile (their key is recomputed from the staged position).
 __global__ void __launch_bounds__(256) k_save_chunks(const uint32_t* __restrict__ offset, int bvol_shift, uint32_t nbricks,
                                                      uint32_t n, uint32_t* __restrict__ chunk0) {
   const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
@@ -184,7 +184,7 @@ template <class BS>
 __global__ void __launch_bounds__(512) k_scatter_tile(Geo G, uint32_t n, const uint32_t* __restrict__ word, const uint32_t* __restrict__ chunk0,
                                                       uint32_t nbricks, const uint32_t* __restrict__ offset, const uint32_t* __restrict__ tbase,
                                                       const float* __restrict__ aos, uint32_t* __restrict__ perm) {
-  extern __shared__ uint32_t dest[];
+  extern __shared__ uint32_t dest[];     // per tile cell: next free slot
   const int T0 = (1 << BS::s0(G)) + 2 * HALO, T1 = (1 << BS::s1(G)) + 2 * HALO, T2 = (1 << BS::s2(G)) + 2 * HALO;
   const int tcells = T0 * T1 * T2;
   const uint32_t b = blockIdx.x;
@@ -212,7 +212,7 @@ __global__ void __launch_bounds__(512) k_scatter_tile(Geo G, uint32_t n, const u
       const float* p = aos + (size_t)i * 8;
       d = offset[key_of(G, p[0], p[1], p[2], G.s[0], G.s[1], G.s[2])] + (w & 0xffffu);
     } else {
-      d = dest[w >> 16] + (w & 0xffffu);
+      d = atomicAdd(&dest[w], 1u);
     }
     perm[d] = i;
   }

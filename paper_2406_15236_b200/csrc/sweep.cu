@@ -16,8 +16,8 @@ struct SweepIO {
   float* aos_out;           // IO_AOS_OUT
   const uint32_t* perm;     // IO_GATHER
   uint32_t* id;             // IO_AOS_OUT: read at i; IO_GATHER: written at i
-  uint32_t* tbase;          // IO_AOS_OUT with ranks: first slot of this CTA's particles inside every tile cell's segment
-  int ranked;               // IO_AOS_OUT: key_out receives (tile cell << 16 | arrival rank) instead of the key
+  uint32_t* tbase;          // IO_AOS_OUT, ranked: first slot of this CTA's particles inside every tile cell's segment
+  int ranked;               // IO_AOS_OUT: key_out receives the tile cell (or bit 31 | slot, outside the tile) instead of the key
 };
 __device__ __forceinline__ void ld256(const float* p, float (&a)[8]) {
   asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
@@ -50,7 +50,11 @@ __device__ __forceinline__ void chunk_range(const uint32_t* __restrict__ chunk, 
 
 // T = threads per CTA: 512 (2 CTAs per SM), or 384 (3 CTAs per SM at <= 56 registers: the steady-state sweep is
 // 2 % faster that way, the staged reorder sweeps are not)
-template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS, int IO, int T>
+// P2: the cell-layer counts m[] are powers of two (and there are no walls): folding an index into [0, m) is one AND
+template <bool P2>
+__device__ __forceinline__ int foldp(int k, int m) { return P2 ? (k & (m - 1)) : fold(k, m); }
+
+template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS, int IO, int T, bool P2>
 __global__ void __launch_bounds__(T, T <= 384 ? 3 : 2)
 k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
         float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, uint32_t* __restrict__ key_out,
@@ -113,22 +117,28 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       p0 = x[inext]; p1 = y[inext]; p2 = z[inext]; p3 = vx[inext]; p4 = vy[inext]; p5 = vz[inext];
       if (IO == IO_AOS_OUT) pid = __uint_as_float(io.id[inext]);
     }
-    if (IO != IO_GATHER) {   // pull the lines of a later iteration into L2: the register prefetch above then pays L2, not DRAM, latency
+    if (IO != IO_GATHER && threadIdx.x == 0) {
+      // pull the lines of a later iteration into L2: the register prefetch above then pays L2, not DRAM, latency. ONE bulk
+      // prefetch per array and CTA iteration (cp.async.bulk.prefetch.L2): a per-thread prefetch.global.L2 costs every warp
+      // six more requests in the L1TEX pipe that bounds this kernel (sweep 15.0 -> 14.3 ms at config 5; none at all: 16.6)
       const uint32_t ifar = i + PF_DIST * T;
       if (ifar < i1) {
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(x + ifar));
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(y + ifar));
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(z + ifar));
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(vx + ifar));
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(vy + ifar));
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(vz + ifar));
+        const uint32_t bytes = (min((uint32_t)T, i1 - ifar) * 4u) & ~15u;
+        if (bytes) {
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(x + ifar), "r"(bytes));
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(y + ifar), "r"(bytes));
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(z + ifar), "r"(bytes));
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(vx + ifar), "r"(bytes));
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(vy + ifar), "r"(bytes));
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(vz + ifar), "r"(bytes));
+        }
       }
     }
     if (COLLIDE) {   // ROTATE_VELOCITIES of the previous step; its key is recomputed from r and that step's shift
       int kx = cell_raw(G, r[0], sp0) + w0, ky = cell_raw(G, r[1], sp1) + w1, kz = cell_raw(G, r[2], sp2) + w2;
-      if (WALL) { kx = G.bc[0] ? max(0, min(kx, m0 - 1)) : fold(kx, m0); ky = G.bc[1] ? max(0, min(ky, m1 - 1)) : fold(ky, m1);
-                  kz = G.bc[2] ? max(0, min(kz, m2 - 1)) : fold(kz, m2); }
-      else { kx = fold(kx, m0); ky = fold(ky, m1); kz = fold(kz, m2); }
+      if (WALL) { kx = G.bc[0] ? max(0, min(kx, m0 - 1)) : foldp<P2>(kx, m0); ky = G.bc[1] ? max(0, min(ky, m1 - 1)) : foldp<P2>(ky, m1);
+                  kz = G.bc[2] ? max(0, min(kz, m2 - 1)) : foldp<P2>(kz, m2); }
+      else { kx = foldp<P2>(kx, m0); ky = foldp<P2>(ky, m1); kz = foldp<P2>(kz, m2); }
       const uint32_t kp = BS::key(G, kx, ky, kz);
       float4 r0, ax;
       load_rec(rec, kp, r0, ax);
@@ -148,7 +158,7 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
     const unsigned e = __float2uint_rn(fmaf(v[0], v[0], fmaf(v[1], v[1], v[2] * v[2])) * G.fxe);
     nbad += (e >= E_RANGE_LIMIT) ? 1u : 0u;     // |v| >= 8 u: outside the range of the fixed-point sums
     // tile coordinates: one fold takes care of the periodic image of the cell and of the tile origin
-    const int l0 = fold(cx - ox, m0), l1 = fold(cy - oy, m1), l2 = fold(cz - oz, m2);
+    const int l0 = foldp<P2>(cx - ox, m0), l1 = foldp<P2>(cy - oy, m1), l2 = foldp<P2>(cz - oz, m2);
     const bool inside = (l0 < T0) & (l1 < T1) & (l2 < T2);
     uint32_t word = 0;
     if (inside) {
@@ -157,13 +167,13 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       // word 0 = count (11 bits) | sum of the energies' high parts e >> 21 (21 bits); word 4 = sum of their low 21 bits:
       // neither can overflow below 2048 particles per (CTA, cell) with e < 2^28 (U19)
       const int w0add = 1 + (int)((e >> TILE_E_SHIFT) << TILE_N_BITS);
-      if (ranked) word = ((uint32_t)tc << 16) | ((uint32_t)atomicAdd(s, w0add) & TILE_N_MASK);   // arrival rank inside (CTA, cell)
-      else atomicAdd(s, w0add);
+      atomicAdd(s, w0add);
+      word = (uint32_t)tc;
       atomicAdd(s + 1, a0); atomicAdd(s + 2, a1); atomicAdd(s + 3, a2);
       atomicAdd((unsigned*)s + 4, e & ((1u << TILE_E_SHIFT) - 1u));
     }
     if ((WKEY && !ranked) || !inside) {
-      const uint32_t kc = BS::key(G, fold(cx, m0), fold(cy, m1), fold(cz, m2));
+      const uint32_t kc = BS::key(G, foldp<P2>(cx, m0), foldp<P2>(cy, m1), foldp<P2>(cz, m2));
       if (!inside) {
         u64* s = sums + (size_t)kc * G.sw;
         if (ranked) word = 0x80000000u | (uint32_t)(atomicAdd(s, ((u64)e << 16) | 1ull) & 0xffffull);
@@ -182,7 +192,7 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
     const int cnt = (int)((unsigned)s[0] & TILE_N_MASK);
     if (cnt == 0) continue;
     const int l0 = c % T0, q = c / T0, l1 = q % T1, l2 = q / T1;
-    u64* g = sums + (size_t)BS::key(G, fold(ox + l0, m0), fold(oy + l1, m1), fold(oz + l2, m2)) * G.sw;
+    u64* g = sums + (size_t)BS::key(G, foldp<P2>(ox + l0, m0), foldp<P2>(oy + l1, m1), foldp<P2>(oz + l2, m2)) * G.sw;
     const u64 etile = ((u64)((unsigned)s[0] >> TILE_N_BITS) << TILE_E_SHIFT) + (u64)(unsigned)s[4];
     const u64 w0 = (etile << 16) | (u64)(unsigned)cnt;
     if (ranked) io.tbase[(size_t)b * tcells + c] = (uint32_t)(atomicAdd(g, w0) & 0xffffull);   // slots taken so far in this cell
@@ -230,22 +240,24 @@ inline float* aos_base(const mpc_ctx* c) {
 // the instantiations that exist: (COLLIDE, WKEY, IO) in { (*,0,PLAIN) at 384 or 512 threads, (*,1,PLAIN), (*,1,AOS_OUT),
 // (1,0,GATHER) } x (WALL, GRAV) x brick shape
 template <bool COLLIDE, bool WKEY, class BS, int IO, int T>
-void* sweep_fn(bool wall, bool grav) {
-  if (wall && grav) return (void*)k_sweep<COLLIDE, true, true, WKEY, BS, IO, T>;
-  if (wall) return (void*)k_sweep<COLLIDE, true, false, WKEY, BS, IO, T>;
-  if (grav) return (void*)k_sweep<COLLIDE, false, true, WKEY, BS, IO, T>;
-  return (void*)k_sweep<COLLIDE, false, false, WKEY, BS, IO, T>;
+void* sweep_fn(bool wall, bool grav, bool p2) {
+  if (wall && grav) return (void*)k_sweep<COLLIDE, true, true, WKEY, BS, IO, T, false>;
+  if (wall) return (void*)k_sweep<COLLIDE, true, false, WKEY, BS, IO, T, false>;
+  if (p2) return grav ? (void*)k_sweep<COLLIDE, false, true, WKEY, BS, IO, T, true> : (void*)k_sweep<COLLIDE, false, false, WKEY, BS, IO, T, true>;
+  if (grav) return (void*)k_sweep<COLLIDE, false, true, WKEY, BS, IO, T, false>;
+  return (void*)k_sweep<COLLIDE, false, false, WKEY, BS, IO, T, false>;
 }
 template <class BS>
-void* sweep_variant(bool collide, bool wkey, int io, bool three, bool wall, bool grav) {
-  if (io == IO_GATHER) return sweep_fn<true, false, BS, IO_GATHER, SWEEP_T>(wall, grav);
-  if (io == IO_AOS_OUT) return collide ? sweep_fn<true, true, BS, IO_AOS_OUT, SWEEP_T>(wall, grav) : sweep_fn<false, true, BS, IO_AOS_OUT, SWEEP_T>(wall, grav);
-  if (wkey) return collide ? sweep_fn<true, true, BS, IO_PLAIN, SWEEP_T>(wall, grav) : sweep_fn<false, true, BS, IO_PLAIN, SWEEP_T>(wall, grav);
-  if (three) return collide ? sweep_fn<true, false, BS, IO_PLAIN, SWEEP_T3>(wall, grav) : sweep_fn<false, false, BS, IO_PLAIN, SWEEP_T3>(wall, grav);
-  return collide ? sweep_fn<true, false, BS, IO_PLAIN, SWEEP_T>(wall, grav) : sweep_fn<false, false, BS, IO_PLAIN, SWEEP_T>(wall, grav);
+void* sweep_variant(bool collide, bool wkey, int io, bool three, bool wall, bool grav, bool p2) {
+  if (io == IO_GATHER) return sweep_fn<true, false, BS, IO_GATHER, SWEEP_T>(wall, grav, p2);
+  if (io == IO_AOS_OUT) return collide ? sweep_fn<true, true, BS, IO_AOS_OUT, SWEEP_T>(wall, grav, p2) : sweep_fn<false, true, BS, IO_AOS_OUT, SWEEP_T>(wall, grav, p2);
+  if (wkey) return collide ? sweep_fn<true, true, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2) : sweep_fn<false, true, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2);
+  if (three) return collide ? sweep_fn<true, false, BS, IO_PLAIN, SWEEP_T3>(wall, grav, p2) : sweep_fn<false, false, BS, IO_PLAIN, SWEEP_T3>(wall, grav, p2);
+  return collide ? sweep_fn<true, false, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2) : sweep_fn<false, false, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2);
 }
-void* sweep_variant_any(bool fast, bool collide, bool wkey, int io, bool three, bool wall, bool grav) {
-  return fast ? sweep_variant<BSfast>(collide, wkey, io, three, wall, grav) : sweep_variant<BSgeneric>(collide, wkey, io, three, wall, grav);
+// the power-of-two variants exist for the {16,16,8} brick only (the shape the large boxes use)
+void* sweep_variant_any(bool fast, bool collide, bool wkey, int io, bool three, bool wall, bool grav, bool p2) {
+  return fast ? sweep_variant<BSfast>(collide, wkey, io, three, wall, grav, p2) : sweep_variant<BSgeneric>(collide, wkey, io, three, wall, grav, false);
 }
 
 }  // namespace
@@ -262,7 +274,7 @@ int launch_sweep(mpc_ctx* c, bool collide, bool wkey, int io, const float sp[3])
   const uint32_t* chunk = c->have_order ? c->offset : nullptr;
   const bool wall = G.wall >= 0, grav = (G.g[0] != 0.f || G.g[1] != 0.f || G.g[2] != 0.f);
   const bool three = io == IO_PLAIN && !wkey && c->three_ctas;
-  void* fn = sweep_variant_any(c->fast_brick, collide, wkey, io, three, wall, grav);
+  void* fn = sweep_variant_any(c->fast_brick, collide, wkey, io, three, wall, grav, c->pow2_cells);
   float s0 = sp[0], s1 = sp[1], s2 = sp[2];
   uint32_t n = (uint32_t)c->n;
   void* args[] = {&G, &s0, &s1, &s2, &n, &F[0], &F[1], &F[2], &F[3], &F[4], &F[5], &c->key, &chunk, &c->nbricks, &c->rec, &c->sums, &sio};
@@ -274,14 +286,14 @@ int launch_sweep(mpc_ctx* c, bool collide, bool wkey, int io, const float sp[3])
 }
 
 cudaError_t sweep_set_attributes(size_t bytes) {
-  for (int fast = 0; fast < 2; ++fast)
+  for (int fast = 0; fast < 4; ++fast)            // bit 0: {16,16,8} brick, bit 1: power-of-two variant
     for (int wall = 0; wall < 2; ++wall)
       for (int grav = 0; grav < 2; ++grav)
         for (int collide = 0; collide < 2; ++collide) {
           const struct { bool wkey; int io; bool three; } v[] = {{false, IO_PLAIN, false}, {false, IO_PLAIN, true}, {true, IO_PLAIN, false},
                                                                  {true, IO_AOS_OUT, false}, {false, IO_GATHER, false}};
           for (const auto& q : v) {
-            const cudaError_t e = cudaFuncSetAttribute(sweep_variant_any(fast != 0, collide != 0, q.wkey, q.io, q.three, wall != 0, grav != 0),
+            const cudaError_t e = cudaFuncSetAttribute(sweep_variant_any((fast & 1) != 0, collide != 0, q.wkey, q.io, q.three, wall != 0, grav != 0, (fast & 2) != 0),
                                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
             if (e != cudaSuccess) return e;
           }
