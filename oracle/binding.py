@@ -20,7 +20,7 @@ class OracleParams(C.Structure):
     _fields_ = [("collision", C.c_int), ("conserve_L", C.c_int), ("thermostat", C.c_int),
                 ("alpha", C.c_float), ("dt", C.c_float), ("kT", C.c_float), ("mass", C.c_float),
                 ("g", C.c_float * 3), ("bc", C.c_int * 3), ("grid_shift", C.c_int),
-                ("rebin_every", C.c_int), ("brick", C.c_int * 3)]
+                ("rebin_every", C.c_int), ("brick", C.c_int * 3), ("shear_rate", C.c_float)]
 
 
 class OracleObs(C.Structure):
@@ -54,6 +54,10 @@ def lib():
         _lib.oracle_cell_of.argtypes = [C.c_void_p, _f32p, _f32p, _i32p, C.POINTER(C.c_uint), C.POINTER(C.c_uint), _f32p]
         _lib.oracle_stream_one.argtypes = [C.c_void_p, _f32p, _f32p]
         _lib.oracle_collide_one_cell.argtypes = [C.c_void_p, C.c_uint, C.c_uint, C.c_void_p, C.c_void_p]
+        _lib.oracle_stream_one_at.argtypes = [C.c_void_p, C.c_uint, _f32p, _f32p]
+        _lib.oracle_cell_of_le.argtypes = [C.c_void_p, C.c_uint, _f32p, _f32p, _i32p, C.POINTER(C.c_uint), C.POINTER(C.c_uint),
+                                           C.POINTER(C.c_int)]
+        _lib.oracle_le_offset.argtypes = [C.c_void_p, C.c_uint, C.POINTER(C.c_float), C.POINTER(C.c_float)]
     return _lib
 
 
@@ -64,8 +68,9 @@ def philox(ctr, key):
 
 
 def make_params(collision=0, conserve_L=0, thermostat=0, alpha_deg=130.0, dt=0.1, kT=1.0, mass=1.0,
-                g=(0.0, 0.0, 0.0), bc=(0, 0, 0), grid_shift=1, rebin_every=1, brick=1):
+                g=(0.0, 0.0, 0.0), bc=(0, 0, 0), grid_shift=1, rebin_every=1, brick=1, shear_rate=0.0):
     p = OracleParams()
+    p.shear_rate = shear_rate
     p.collision, p.conserve_L, p.thermostat = collision, conserve_L, thermostat
     p.alpha = np.float32(np.deg2rad(alpha_deg))
     p.dt, p.kT, p.mass = dt, kT, mass
@@ -178,6 +183,24 @@ class Oracle:
         v = np.array(v, np.float32)
         lib().oracle_stream_one(self._h, r, v)
         return r, v
+
+    def stream_one_at(self, t, r, v):
+        r = np.array(r, np.float32)
+        v = np.array(v, np.float32)
+        lib().oracle_stream_one_at(self._h, t, r, v)
+        return r, v
+
+    def cell_of_le(self, t, r, s):
+        ijk = np.zeros(3, np.int32)
+        cid, key, im = C.c_uint(), C.c_uint(), C.c_int()
+        lib().oracle_cell_of_le(self._h, t, np.asarray(r, np.float32), np.asarray(s, np.float32), ijk, C.byref(cid),
+                                C.byref(key), C.byref(im))
+        return ijk, cid.value, key.value, im.value
+
+    def le_offset(self, t):
+        d, u = C.c_float(), C.c_float()
+        lib().oracle_le_offset(self._h, t, C.byref(d), C.byref(u))
+        return d.value, u.value
 
     def collide_one_cell(self, cid=0, t=0, axis=None, kappa=None):
         ax = np.asarray(axis, np.float64) if axis is not None else None

@@ -46,6 +46,7 @@ struct Params {
   int   grid_shift;   // 1 = random lattice shift every step
   int   rebin_every;  // reorder interval
   int   brick[3];     // brick dims of the brick-major key layout ({1,1,1} = row-major); memory order only
+  float shear_rate;   // Lees-Edwards shear ("shear flow can also be added", reading U21): d v_x / d z; 0 = off
 };
 
 struct Obs {
@@ -81,6 +82,7 @@ struct Ctx {
   std::vector<double> sx, sy, sz, se;      // per key: sum v, sum |v|^2
   unsigned long long n_singular = 0;
   float last_shift[3] = {0, 0, 0};
+  std::vector<signed char> img;            // Lees-Edwards: -1 / +1 if the particle collides as its image below / above (U21)
   std::string err;
 };
 
@@ -149,6 +151,31 @@ inline void cell_of(const Ctx& c, const float r[3], const float s[3], int i[3], 
     rho[d] = q - f;
   }
 }
+// ---- Lees-Edwards sheared periodic boundary along z, flow along x (reading U21) ----------
+// The periodic images of the box above / below are displaced by +-D(t) along x and move with +-U = +-gamma L_z.
+// D is taken at the time the positions refer to: (t+1) h for the wrap after MOVE of step t and for its collision.
+inline float le_velocity(const Ctx& c) { return (float)((double)c.p.shear_rate * (double)c.L[2]); }
+inline float le_offset(const Ctx& c, uint32_t t) {
+  const double Ud = (double)c.p.shear_rate * (double)c.L[2];
+  double d = std::fmod(Ud * (double)c.p.dt * ((double)t + 1.0), (double)c.L[0]);
+  if (d < 0.0) d += (double)c.L[0];
+  return (float)d;
+}
+// cell of a position under Lees-Edwards: a particle whose shifted z leaves [0, L_z) collides as its periodic image:
+// x -+ D (wrapped once), v_x -+ U. image = -1: image below the box top was used (particle above), +1: the reverse.
+inline void cell_of_le(const Ctx& c, uint32_t t, const float r[3], const float s[3], int i[3], float rho[3], int* image) {
+  float rr[3] = {r[0], r[1], r[2]};
+  int im = 0;
+  if (c.p.shear_rate != 0.0f) {
+    const float qz = (r[2] + s[2]) * c.inv_a;
+    const int kz = (int)floorf(qz);
+    const float D = le_offset(c, t);
+    if (kz < 0) { im = +1; rr[0] = r[0] + D; if (rr[0] >= c.L[0]) rr[0] -= c.L[0]; }
+    else if (kz >= c.n[2]) { im = -1; rr[0] = r[0] - D; if (rr[0] < 0.0f) rr[0] += c.L[0]; }
+  }
+  cell_of(c, rr, s, i, rho);
+  if (image) *image = im;
+}
 inline uint32_t canonical_id(const Ctx& c, const int i[3]) {
   return (uint32_t)i[0] + (uint32_t)c.m[0] * ((uint32_t)i[1] + (uint32_t)c.m[1] * (uint32_t)i[2]);
 }
@@ -180,7 +207,7 @@ inline void advance(const Ctx& c, float r[3], float v[3], float tau) {
     }
   }
 }
-inline void stream_one(const Ctx& c, float r[3], float v[3]) {
+inline void stream_one(const Ctx& c, float r[3], float v[3], uint32_t t) {
   const float h = c.p.dt;
   int w = -1;
   for (int d = 0; d < 3; ++d) if (c.p.bc[d] != 0) w = d;   // at most one wall axis (create checks)
@@ -206,6 +233,12 @@ inline void stream_one(const Ctx& c, float r[3], float v[3]) {
   if (!bounced) advance(c, r, v, h);
   for (int d = 0; d < 3; ++d) {
     if (c.p.bc[d] != 0) continue;
+    if (d == 2 && c.p.shear_rate != 0.0f) {                 // Lees-Edwards: crossing z = 0 / L_z enters the sheared image (U21)
+      const float D = le_offset(c, t), U = le_velocity(c);
+      if (r[2] < 0.0f) { r[2] += c.L[2]; r[0] += D; if (r[0] >= c.L[0]) r[0] -= c.L[0]; v[0] += U; }
+      if (r[2] >= c.L[2]) { r[2] -= c.L[2]; r[0] -= D; if (r[0] < 0.0f) r[0] += c.L[0]; v[0] -= U; }
+      continue;
+    }
     if (r[d] < 0.0f) r[d] += c.L[d];                        // reading U2: this order, single wrap
     if (r[d] >= c.L[d]) r[d] -= c.L[d];
   }
@@ -426,7 +459,7 @@ void one_step(Ctx& c) {
   // 1. MOVE (Eq. 1)
   for (size_t i = 0; i < N; ++i) {
     float r[3] = {c.x[i], c.y[i], c.z[i]}, v[3] = {c.vx[i], c.vy[i], c.vz[i]};
-    stream_one(c, r, v);
+    stream_one(c, r, v, t);
     c.x[i] = r[0]; c.y[i] = r[1]; c.z[i] = r[2];
     c.vx[i] = v[0]; c.vy[i] = v[1]; c.vz[i] = v[2];
   }
@@ -438,10 +471,15 @@ void one_step(Ctx& c) {
   for (int d = 0; d < 3; ++d) c.rho[d].resize(N);
   for (size_t i = 0; i < N; ++i) {
     const float r[3] = {c.x[i], c.y[i], c.z[i]};
-    int ic[3]; float rho[3];
-    cell_of(c, r, s, ic, rho);
+    int ic[3]; float rho[3]; int im;
+    cell_of_le(c, t, r, s, ic, rho, &im);
     c.key[i] = layout_key(c, ic);
     c.rho[0][i] = rho[0]; c.rho[1][i] = rho[1]; c.rho[2][i] = rho[2];
+    if (c.p.shear_rate != 0.0f) {       // collide in the frame of the image: v_x -+ U, one fp32 add (undone after the collision)
+      if (i == 0) c.img.assign(N, 0);
+      c.img[i] = (signed char)im;
+      if (im) c.vx[i] = c.vx[i] + (float)im * le_velocity(c);
+    }
   }
   // 4. REORDER when due (readings U3,U4): ascending (key, id)
   if (t % (uint32_t)c.p.rebin_every == 0u) {
@@ -455,6 +493,7 @@ void one_step(Ctx& c) {
     permute(c.vx, order); permute(c.vy, order); permute(c.vz, order);
     permute(c.id, order); permute(c.key, order);
     permute(c.rho[0], order); permute(c.rho[1], order); permute(c.rho[2], order);
+    if (c.p.shear_rate != 0.0f) permute(c.img, order);
   }
   // members of every cell, in ascending id
   c.count.assign(c.nkeys, 0u);
@@ -483,6 +522,8 @@ void one_step(Ctx& c) {
     key_to_cell(c, (uint32_t)k, ic);
     collide_cell(c, canonical_id(c, ic), ic, s, t, &mem[off[k]], c.count[k], nullptr, nullptr);
   }
+  if (c.p.shear_rate != 0.0f)
+    for (size_t i = 0; i < N; ++i) if (c.img[i]) c.vx[i] = c.vx[i] - (float)c.img[i] * le_velocity(c);
   c.have_cells = true;
   c.t = t + 1u;
 }
@@ -511,6 +552,7 @@ int oracle_create(void** out, const float box[3], const int cells[3], float n_pe
   if (nwall && (p->conserve_L || p->collision == 1)) return E_INVAL;        // needs explicit phantom sets (U8)
   if (p->collision == 0 && p->conserve_L && p->thermostat) return E_INVAL;  // ambiguous (U6)
   if (!(n_per_cell > 0.0f)) return E_INVAL;
+  if (p->shear_rate != 0.0f && (nwall || p->collision == 1 || p->conserve_L)) return E_INVAL;   // Lees-Edwards: periodic SRD only (U21)
   Ctx* c = new Ctx();
   c->p = *p; c->seed = seed; c->t = 0; c->a = a; c->inv_a = 1.0f / a;
   c->nbar = (int)std::lround((double)n_per_cell);
@@ -674,7 +716,29 @@ int oracle_cell_of(void* h, const float r[3], const float s[3], int ijk[3], unsi
 }
 int oracle_stream_one(void* h, float r[3], float v[3]) {
   if (!h) return E_INVAL;
-  stream_one(*(Ctx*)h, r, v);
+  stream_one(*(Ctx*)h, r, v, ((Ctx*)h)->t);
+  return E_OK;
+}
+// Lees-Edwards hooks: MOVE of step t, and the cell (with the image used: -1, 0, +1) of a position at step t
+int oracle_stream_one_at(void* h, unsigned t, float r[3], float v[3]) {
+  if (!h) return E_INVAL;
+  stream_one(*(Ctx*)h, r, v, t);
+  return E_OK;
+}
+int oracle_cell_of_le(void* h, unsigned t, const float r[3], const float s[3], int ijk[3], unsigned* cid, unsigned* key, int* image) {
+  if (!h) return E_INVAL;
+  Ctx& c = *(Ctx*)h;
+  int ic[3]; float rr[3];
+  cell_of_le(c, t, r, s, ic, rr, image);
+  for (int d = 0; d < 3; ++d) if (ijk) ijk[d] = ic[d];
+  if (cid) *cid = canonical_id(c, ic);
+  if (key) *key = layout_key(c, ic);
+  return E_OK;
+}
+int oracle_le_offset(void* h, unsigned t, float* D, float* U) {
+  if (!h) return E_INVAL;
+  if (D) *D = le_offset(*(Ctx*)h, t);
+  if (U) *U = le_velocity(*(Ctx*)h);
   return E_OK;
 }
 // Collide the whole current state as ONE cell (cell id `cid`, step t) with a prescribed axis and/or
