@@ -62,6 +62,9 @@ typedef struct {
   int   rebin_every; /* reorder when step % rebin_every == 0; >= 1; MPC-AT requires 1                  */
   int   brick[3];    /* brick dims (powers of two <= 64) of the brick-major memory key; {1,1,1} = row-major.
                         Memory order only: results do not depend on it. {16,16,8} is the fast choice          */
+  float shear_rate;  /* Lees-Edwards shear d v_x / d z (U21): the periodic images above /
+                        below the box along z are displaced by +-shear_rate L_z t along x and move with
+                        +-shear_rate L_z. 0 = off. Needs periodic boundaries on all axes, SRD without +a             */
 } mpc_params;
 
 typedef struct {
@@ -87,7 +90,7 @@ typedef struct {
  * (round(n_per_cell)) and for sizing. Allocates nothing on the device.
  * MPC_EINVAL: NULL argument, fewer than 3 cells along an axis, non-cubic cells, non-positive sizes/dt/kT/mass, rebin_every < 1,
  * brick dims not powers of two in 1..64 or tile too large for shared memory, more than one wall axis, force along a wall normal, walls with +a or MPC-AT,
- * SRD+a with thermostat (U6), MPC-AT with rebin_every != 1, key space >= 2^32. */
+ * SRD+a with thermostat (U6), MPC-AT with rebin_every != 1, key space >= 2^32, shear_rate != 0 with walls, MPC-AT or +a. */
 int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_per_cell,
                const mpc_params* p, unsigned long long seed);
 

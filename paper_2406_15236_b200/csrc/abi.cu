@@ -58,6 +58,15 @@ void host_shift(const mpc_ctx* c, uint32_t t, float s[3]) {
   s[2] = (u01_co(o.c) - 0.5f) * c->G.a;
 }
 
+// Lees-Edwards displacement of the image above at the time the positions of step t refer to, (t + 1) h (U21)
+float host_le_offset(const mpc_ctx* c, uint32_t t) {
+  if (c->p.shear_rate == 0.0f) return 0.0f;
+  const double Ud = (double)c->p.shear_rate * (double)c->G.L[2];
+  double d = fmod(Ud * (double)c->p.dt * ((double)t + 1.0), (double)c->G.L[0]);
+  if (d < 0.0) d += (double)c->G.L[0];
+  return (float)d;
+}
+
 // SRD: step t = sweep (collision of t-1 if one is pending + MOVE of t + sums of t), [reorder], PROCESS_CELLS of t.
 // The collision of the last step stays pending: the next call's first sweep applies it (flush_collide otherwise).
 int steps_srd(mpc_ctx* c, int nsteps) {
@@ -67,6 +76,8 @@ int steps_srd(mpc_ctx* c, int nsteps) {
   for (int k = 0; k < nsteps; ++k) {
     G.t = c->t;
     host_shift(c, c->t, G.s);
+    c->le_dprev = G.le_d;
+    G.le_d = host_le_offset(c, c->t);
     const bool rebin = (c->t % (uint32_t)c->p.rebin_every) == 0u;
     if (!c->sums_clean) { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * G.sw * 8, c->stream)); }
     c->sums_clean = false;
@@ -177,6 +188,7 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   if (nwall && (p->conserve_L || p->collision == 1)) return MPC_EINVAL;
   if (p->collision == 0 && p->conserve_L && p->thermostat) return MPC_EINVAL;
   if (p->collision == 1 && p->rebin_every != 1) return MPC_EINVAL;
+  if (p->shear_rate != 0.0f && (nwall || p->collision == 1 || p->conserve_L)) return MPC_EINVAL;   // Lees-Edwards: periodic SRD only (U21)
   mpc_ctx* c = new (std::nothrow) mpc_ctx();   // value-initialised: all zero
   if (!c) return MPC_ENOMEM;
   c->p = *p; c->seed = seed;
@@ -220,6 +232,9 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   G.fxv = (float)ldexp(1.0, 22 - ue); G.fxv_inv = ldexp(1.0, ue - 22);
   G.fxe = (float)ldexp(1.0, 22 - 2 * ue); G.fxe_inv = ldexp(1.0, 2 * ue - 22);
   G.vmax = (float)ldexp(1.0, ue + 3);
+  G.shear = p->shear_rate != 0.0f ? 1 : 0;
+  G.le_u = (float)((double)p->shear_rate * (double)box[2]);
+  G.le_d = 0.0f;
   G.collision = p->collision; G.thermostat = p->thermostat; G.conserve_L = p->conserve_L;
   G.generic = (p->collision == 1 || p->conserve_L) ? 1 : 0;
   G.sw = (p->collision == 0 && p->conserve_L) ? 16 : 3;

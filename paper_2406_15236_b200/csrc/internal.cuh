@@ -82,6 +82,9 @@ struct Geo {
   int rw;         // floats per cell record (8, or 16 with +a)
   uint32_t nkeys;
   u64* nrange;    // device counter of range overflows since the last mpc_set_state
+  int shear;      // Lees-Edwards shear along z, flow along x (U21)
+  float le_u;     // velocity of the image above: shear_rate * L_z
+  float le_d;     // x displacement of the image above at the time the positions of this step refer to
 };
 
 // ---- packed sums ---------------------------------------------------------------------------------
@@ -129,7 +132,22 @@ __device__ __forceinline__ int cell_coord(const Geo& G, int d, float r, float s)
   }
   return k;
 }
-__device__ __forceinline__ uint32_t key_of(const Geo& G, float x, float y, float z, float s0, float s1, float s2) {
+// Lees-Edwards (U21): a particle whose shifted z leaves [0, L_z) collides as its periodic image, x -+ D
+// (wrapped once) and v_x -+ U. Returns the x to bin with; vs = what is added to v_x for the collision (and taken off
+// again afterwards).
+__device__ __forceinline__ float le_image(const Geo& G, float x, float z, float sz, float D, float& vs) {
+  vs = 0.0f;
+  const int kz = __float2int_rd((z + sz) * G.inv_a);
+  float xe = x;
+  if (kz < 0) { xe = x + D; if (xe >= G.L[0]) xe -= G.L[0]; vs = G.le_u; }
+  else if (kz >= G.n[2]) { xe = x - D; if (xe < 0.0f) xe += G.L[0]; vs = -G.le_u; }
+  return xe;
+}
+// memory key of a position for lattice shift s (and the Lees-Edwards displacement G.le_d of the same step)
+__device__ __forceinline__ uint32_t key_of(const Geo& G, float x, float y, float z, float s0, float s1, float s2, float* vs_out = nullptr) {
+  float vs = 0.0f;
+  if (G.shear) x = le_image(G, x, z, s2, G.le_d, vs);
+  if (vs_out) *vs_out = vs;
   return layout_key(G, cell_coord(G, 0, x, s0), cell_coord(G, 1, y, s1), cell_coord(G, 2, z, s2));
 }
 
@@ -147,7 +165,7 @@ __device__ __forceinline__ void advance(const Geo& G, float (&r)[3], float (&v)[
     }
   }
 }
-template <bool WALL, bool GRAV>
+template <bool WALL, bool GRAV, bool SHEAR = false>
 __device__ __forceinline__ void stream_one(const Geo& G, float (&r)[3], float (&v)[3]) {
   bool bounced = false;
   if (WALL) {
@@ -176,6 +194,11 @@ __device__ __forceinline__ void stream_one(const Geo& G, float (&r)[3], float (&
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     if (WALL && G.bc[d] != 0) continue;
+    if (SHEAR && d == 2) {   // crossing z = 0 / L_z enters the sheared image (U21)
+      if (r[2] < 0.0f) { r[2] += G.L[2]; r[0] += G.le_d; if (r[0] >= G.L[0]) r[0] -= G.L[0]; v[0] += G.le_u; }
+      if (r[2] >= G.L[2]) { r[2] -= G.L[2]; r[0] -= G.le_d; if (r[0] < 0.0f) r[0] += G.L[0]; v[0] -= G.le_u; }
+      continue;
+    }
     if (r[d] < 0.0f) r[d] += G.L[d];
     if (r[d] >= G.L[d]) r[d] -= G.L[d];
   }
@@ -259,6 +282,7 @@ struct mpc_ctx {
   bool collide_pending;
   bool pow2_cells;      // no walls and every m[d] a power of two: the sweep folds indices with a mask
   bool ranked_keys;     // the last staging sweep wrote (tile cell, arrival rank) words into key[] instead of keys
+  float le_dprev;       // Lees-Edwards displacement of the step whose collision is pending
   unsigned debug;       // MPC_DEBUG_* flags
   int device;           // CUDA device of the workspace
   cudaStream_t stream;

@@ -18,6 +18,7 @@ struct SweepIO {
   uint32_t* id;             // IO_AOS_OUT: read at i; IO_GATHER: written at i
   uint32_t* tbase;          // IO_AOS_OUT, ranked: first slot of this CTA's particles inside every tile cell's segment
   int ranked;               // IO_AOS_OUT: key_out receives the tile cell (or bit 31 | slot, outside the tile) instead of the key
+  float le_dprev;           // Lees-Edwards displacement of the previous step (for its collision)
 };
 __device__ __forceinline__ void ld256(const float* p, float (&a)[8]) {
   asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
@@ -54,7 +55,9 @@ __device__ __forceinline__ void chunk_range(const uint32_t* __restrict__ chunk, 
 template <bool P2>
 __device__ __forceinline__ int foldp(int k, int m) { return P2 ? (k & (m - 1)) : fold(k, m); }
 
-template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS, int IO, int T, bool P2>
+// SHEAR: Lees-Edwards boundary along z (U21); the few particles that collide as their image are binned at
+// x -+ D, usually far from their brick: they take the global path
+template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS, int IO, int T, bool P2, bool SHEAR>
 __global__ void __launch_bounds__(T, T <= 384 ? 3 : 2)
 k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
         float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, uint32_t* __restrict__ key_out,
@@ -135,16 +138,20 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       }
     }
     if (COLLIDE) {   // ROTATE_VELOCITIES of the previous step; its key is recomputed from r and that step's shift
-      int kx = cell_raw(G, r[0], sp0) + w0, ky = cell_raw(G, r[1], sp1) + w1, kz = cell_raw(G, r[2], sp2) + w2;
+      float vsp = 0.0f;
+      const float xp = SHEAR ? le_image(G, r[0], r[2], sp2, io.le_dprev, vsp) : r[0];
+      int kx = cell_raw(G, xp, sp0) + w0, ky = cell_raw(G, r[1], sp1) + w1, kz = cell_raw(G, r[2], sp2) + w2;
       if (WALL) { kx = G.bc[0] ? max(0, min(kx, m0 - 1)) : foldp<P2>(kx, m0); ky = G.bc[1] ? max(0, min(ky, m1 - 1)) : foldp<P2>(ky, m1);
                   kz = G.bc[2] ? max(0, min(kz, m2 - 1)) : foldp<P2>(kz, m2); }
       else { kx = foldp<P2>(kx, m0); ky = foldp<P2>(ky, m1); kz = foldp<P2>(kz, m2); }
       const uint32_t kp = BS::key(G, kx, ky, kz);
       float4 r0, ax;
       load_rec(rec, kp, r0, ax);
+      if (SHEAR) v[0] += vsp;
       srd_apply(G, r0, ax, v);
+      if (SHEAR) v[0] -= vsp;
     }
-    stream_one<WALL, GRAV>(G, r, v);
+    stream_one<WALL, GRAV, SHEAR>(G, r, v);
     if (IO == IO_AOS_OUT) {
       const float q[8] = {r[0], r[1], r[2], v[0], v[1], v[2], idbits, 0.f};
       st256(io.aos_out + (size_t)i * 8, q);
@@ -152,7 +159,10 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       x[i] = r[0]; y[i] = r[1]; z[i] = r[2];
       vx[i] = v[0]; vy[i] = v[1]; vz[i] = v[2];
     }
-    int cx = cell_raw(G, r[0], G.s[0]) + w0, cy = cell_raw(G, r[1], G.s[1]) + w1, cz = cell_raw(G, r[2], G.s[2]) + w2;
+    float vsn = 0.0f;
+    const float xn = SHEAR ? le_image(G, r[0], r[2], G.s[2], G.le_d, vsn) : r[0];
+    if (SHEAR) v[0] += vsn;        // the sums are taken in the frame of the image (v is not stored after this point)
+    int cx = cell_raw(G, xn, G.s[0]) + w0, cy = cell_raw(G, r[1], G.s[1]) + w1, cz = cell_raw(G, r[2], G.s[2]) + w2;
     if (WALL) { if (G.bc[0]) cx = max(0, min(cx, m0 - 1)); if (G.bc[1]) cy = max(0, min(cy, m1 - 1)); if (G.bc[2]) cz = max(0, min(cz, m2 - 1)); }
     const int a0 = __float2int_rn(v[0] * G.fxv), a1 = __float2int_rn(v[1] * G.fxv), a2 = __float2int_rn(v[2] * G.fxv);
     const unsigned e = __float2uint_rn(fmaf(v[0], v[0], fmaf(v[1], v[1], v[2] * v[2])) * G.fxe);
@@ -211,12 +221,13 @@ __global__ void __launch_bounds__(256) k_collide_pos(Geo G, size_t n, const floa
                                                      float* __restrict__ vz, const float* __restrict__ rec) {
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  const uint32_t k = key_of(G, x[i], y[i], z[i], G.s[0], G.s[1], G.s[2]);
+  float vs;
+  const uint32_t k = key_of(G, x[i], y[i], z[i], G.s[0], G.s[1], G.s[2], &vs);
   float4 r0, ax;
   load_rec(rec, k, r0, ax);
-  float v[3] = {vx[i], vy[i], vz[i]};
+  float v[3] = {vx[i] + vs, vy[i], vz[i]};
   srd_apply(G, r0, ax, v);
-  vx[i] = v[0]; vy[i] = v[1]; vz[i] = v[2];
+  vx[i] = v[0] - vs; vy[i] = v[1]; vz[i] = v[2];
 }
 
 __global__ void __launch_bounds__(256) k_keys(Geo G, size_t n, const float* __restrict__ x, const float* __restrict__ y,
@@ -240,24 +251,25 @@ inline float* aos_base(const mpc_ctx* c) {
 // the instantiations that exist: (COLLIDE, WKEY, IO) in { (*,0,PLAIN) at 384 or 512 threads, (*,1,PLAIN), (*,1,AOS_OUT),
 // (1,0,GATHER) } x (WALL, GRAV) x brick shape
 template <bool COLLIDE, bool WKEY, class BS, int IO, int T>
-void* sweep_fn(bool wall, bool grav, bool p2) {
-  if (wall && grav) return (void*)k_sweep<COLLIDE, true, true, WKEY, BS, IO, T, false>;
-  if (wall) return (void*)k_sweep<COLLIDE, true, false, WKEY, BS, IO, T, false>;
-  if (p2) return grav ? (void*)k_sweep<COLLIDE, false, true, WKEY, BS, IO, T, true> : (void*)k_sweep<COLLIDE, false, false, WKEY, BS, IO, T, true>;
-  if (grav) return (void*)k_sweep<COLLIDE, false, true, WKEY, BS, IO, T, false>;
-  return (void*)k_sweep<COLLIDE, false, false, WKEY, BS, IO, T, false>;
+void* sweep_fn(bool wall, bool grav, bool p2, bool shear) {
+  if (shear) return grav ? (void*)k_sweep<COLLIDE, false, true, WKEY, BS, IO, T, false, true> : (void*)k_sweep<COLLIDE, false, false, WKEY, BS, IO, T, false, true>;
+  if (wall && grav) return (void*)k_sweep<COLLIDE, true, true, WKEY, BS, IO, T, false, false>;
+  if (wall) return (void*)k_sweep<COLLIDE, true, false, WKEY, BS, IO, T, false, false>;
+  if (p2) return grav ? (void*)k_sweep<COLLIDE, false, true, WKEY, BS, IO, T, true, false> : (void*)k_sweep<COLLIDE, false, false, WKEY, BS, IO, T, true, false>;
+  if (grav) return (void*)k_sweep<COLLIDE, false, true, WKEY, BS, IO, T, false, false>;
+  return (void*)k_sweep<COLLIDE, false, false, WKEY, BS, IO, T, false, false>;
 }
 template <class BS>
-void* sweep_variant(bool collide, bool wkey, int io, bool three, bool wall, bool grav, bool p2) {
-  if (io == IO_GATHER) return sweep_fn<true, false, BS, IO_GATHER, SWEEP_T>(wall, grav, p2);
-  if (io == IO_AOS_OUT) return collide ? sweep_fn<true, true, BS, IO_AOS_OUT, SWEEP_T>(wall, grav, p2) : sweep_fn<false, true, BS, IO_AOS_OUT, SWEEP_T>(wall, grav, p2);
-  if (wkey) return collide ? sweep_fn<true, true, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2) : sweep_fn<false, true, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2);
-  if (three) return collide ? sweep_fn<true, false, BS, IO_PLAIN, SWEEP_T3>(wall, grav, p2) : sweep_fn<false, false, BS, IO_PLAIN, SWEEP_T3>(wall, grav, p2);
-  return collide ? sweep_fn<true, false, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2) : sweep_fn<false, false, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2);
+void* sweep_variant(bool collide, bool wkey, int io, bool three, bool wall, bool grav, bool p2, bool shear) {
+  if (io == IO_GATHER) return sweep_fn<true, false, BS, IO_GATHER, SWEEP_T>(wall, grav, p2, shear);
+  if (io == IO_AOS_OUT) return collide ? sweep_fn<true, true, BS, IO_AOS_OUT, SWEEP_T>(wall, grav, p2, shear) : sweep_fn<false, true, BS, IO_AOS_OUT, SWEEP_T>(wall, grav, p2, shear);
+  if (wkey) return collide ? sweep_fn<true, true, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2, shear) : sweep_fn<false, true, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2, shear);
+  if (three) return collide ? sweep_fn<true, false, BS, IO_PLAIN, SWEEP_T3>(wall, grav, p2, shear) : sweep_fn<false, false, BS, IO_PLAIN, SWEEP_T3>(wall, grav, p2, shear);
+  return collide ? sweep_fn<true, false, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2, shear) : sweep_fn<false, false, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2, shear);
 }
 // the power-of-two variants exist for the {16,16,8} brick only (the shape the large boxes use)
-void* sweep_variant_any(bool fast, bool collide, bool wkey, int io, bool three, bool wall, bool grav, bool p2) {
-  return fast ? sweep_variant<BSfast>(collide, wkey, io, three, wall, grav, p2) : sweep_variant<BSgeneric>(collide, wkey, io, three, wall, grav, false);
+void* sweep_variant_any(bool fast, bool collide, bool wkey, int io, bool three, bool wall, bool grav, bool p2, bool shear) {
+  return fast ? sweep_variant<BSfast>(collide, wkey, io, three, wall, grav, p2, shear) : sweep_variant<BSgeneric>(collide, wkey, io, three, wall, grav, false, shear);
 }
 
 }  // namespace
@@ -274,7 +286,8 @@ int launch_sweep(mpc_ctx* c, bool collide, bool wkey, int io, const float sp[3])
   const uint32_t* chunk = c->have_order ? c->offset : nullptr;
   const bool wall = G.wall >= 0, grav = (G.g[0] != 0.f || G.g[1] != 0.f || G.g[2] != 0.f);
   const bool three = io == IO_PLAIN && !wkey && c->three_ctas;
-  void* fn = sweep_variant_any(c->fast_brick, collide, wkey, io, three, wall, grav, c->pow2_cells);
+  sio.le_dprev = c->le_dprev;
+  void* fn = sweep_variant_any(c->fast_brick, collide, wkey, io, three, wall, grav, c->pow2_cells, G.shear != 0);
   float s0 = sp[0], s1 = sp[1], s2 = sp[2];
   uint32_t n = (uint32_t)c->n;
   void* args[] = {&G, &s0, &s1, &s2, &n, &F[0], &F[1], &F[2], &F[3], &F[4], &F[5], &c->key, &chunk, &c->nbricks, &c->rec, &c->sums, &sio};
@@ -286,18 +299,20 @@ int launch_sweep(mpc_ctx* c, bool collide, bool wkey, int io, const float sp[3])
 }
 
 cudaError_t sweep_set_attributes(size_t bytes) {
-  for (int fast = 0; fast < 4; ++fast)            // bit 0: {16,16,8} brick, bit 1: power-of-two variant
+  for (int mode = 0; mode < 6; ++mode) {          // bit 0: {16,16,8} brick; modes 2,3: power-of-two variant; 4,5: Lees-Edwards
+    const bool fast = (mode & 1) != 0, p2 = (mode >> 1) == 1, shear = (mode >> 1) == 2;
     for (int wall = 0; wall < 2; ++wall)
       for (int grav = 0; grav < 2; ++grav)
         for (int collide = 0; collide < 2; ++collide) {
           const struct { bool wkey; int io; bool three; } v[] = {{false, IO_PLAIN, false}, {false, IO_PLAIN, true}, {true, IO_PLAIN, false},
                                                                  {true, IO_AOS_OUT, false}, {false, IO_GATHER, false}};
           for (const auto& q : v) {
-            const cudaError_t e = cudaFuncSetAttribute(sweep_variant_any((fast & 1) != 0, collide != 0, q.wkey, q.io, q.three, wall != 0, grav != 0, (fast & 2) != 0),
+            const cudaError_t e = cudaFuncSetAttribute(sweep_variant_any(fast, collide != 0, q.wkey, q.io, q.three, wall != 0, grav != 0, p2, shear),
                                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
             if (e != cudaSuccess) return e;
           }
         }
+  }
   return cudaSuccess;
 }
 

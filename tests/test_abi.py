@@ -64,6 +64,13 @@ def test_create_validates_arguments(lib):
     assert _create(lib, bc=(0, 0, 1), g=(0, 0, 0.1))[0] == binding.MPC_EINVAL
     assert _create(lib, collision=1, rebin_every=2)[0] == binding.MPC_EINVAL
     assert _create(lib, conserve_L=1, thermostat=1)[0] == binding.MPC_EINVAL
+    # Lees-Edwards shear (U21): periodic SRD without +a only
+    rc, h = _create(lib, shear_rate=0.05, thermostat=1)
+    assert rc == 0
+    lib.mpc_destroy(h)
+    assert _create(lib, shear_rate=0.05, bc=(0, 0, 1))[0] == binding.MPC_EINVAL
+    assert _create(lib, shear_rate=0.05, collision=1)[0] == binding.MPC_EINVAL
+    assert _create(lib, shear_rate=0.05, conserve_L=1)[0] == binding.MPC_EINVAL
     rc, h = _create(lib, cells=(8, 8, 8), bc=(0, 0, 1), thermostat=1, brick=4)
     assert rc == 0
     assert lib.mpc_num_keys(h, C.byref(nk)) == 0 and nk.value == 8 * 8 * 12     # 10 layers padded to 3 bricks of 4

@@ -82,6 +82,10 @@ CASES = {
     # slip walls (specular reflection, no virtual particles; U20)
     "slip_walls_gravity": dict(cells=(16, 8, 8), nbar=10, kw=dict(thermostat=1, bc=(0, 0, 2), g=(0.01, 0, 0))),
     "slip_walls_y_brick16x16x8": dict(cells=(16, 16, 16), nbar=10, kw=dict(bc=(0, 2, 0), dt=0.3, brick=(16, 16, 8))),
+    # Lees-Edwards shear (U21): strong shear and a long step so that many particles cross the sheared face
+    "shear": dict(cells=(12, 12, 12), nbar=10, kw=dict(thermostat=1, shear_rate=0.05, dt=0.3)),
+    "shear_brick16x16x8": dict(cells=(32, 16, 16), nbar=10, kw=dict(shear_rate=0.11, brick=(16, 16, 8))),
+    "shear_negative_brick4": dict(cells=(8, 12, 8), nbar=5, kw=dict(thermostat=1, shear_rate=-0.07, brick=4)),
 }
 
 
@@ -101,7 +105,8 @@ def test_single_step_parity(name):
     compare_step(o, g, a=a)
 
 
-@pytest.mark.parametrize("name", ["cfg1_srd", "srd_mbs_brick4", "at", "walls_gravity", "slip_walls_gravity"])
+@pytest.mark.parametrize("name", ["cfg1_srd", "srd_mbs_brick4", "at", "walls_gravity", "slip_walls_gravity", "shear",
+                                  "shear_brick16x16x8"])
 def test_lockstep_parity_many_steps(name):
     # U15: after every step the oracle state is copied to the GPU, then both advance one step
     c = CASES[name]
@@ -326,7 +331,8 @@ def test_compact_workspace_gives_identical_results():
 @pytest.mark.gpu
 @pytest.mark.parametrize("kw", [dict(thermostat=1, brick=(16, 16, 8), rebin_every=2),
                                 dict(thermostat=1, bc=(0, 0, 1), g=(0.01, 0, 0), brick=4, rebin_every=3),
-                                dict(brick=(4, 2, 1), rebin_every=5)])
+                                dict(brick=(4, 2, 1), rebin_every=5),
+                                dict(thermostat=1, shear_rate=0.05, brick=(16, 16, 8), rebin_every=3)])
 def test_reorder_code_paths_agree(kw):
     # Ways to apply a reorder inside a multi-step call: (a) default: folded into two sweeps through 32-byte staging
     # records, slots from the staging sweep's arrival ranks (no atomics in the scatter), particles grouped by key only,
@@ -362,6 +368,8 @@ def test_reorder_code_paths_agree(kw):
     ("second step after a staged reorder", dict(thermostat=1, brick=(16, 16, 8), rebin_every=4), 2, 5),
     ("walls + gravity, staged reorder", dict(thermostat=1, bc=(0, 0, 1), g=(0.01, 0, 0), brick=4, rebin_every=3), 1, 4),
     ("no thermostat, small bricks", dict(brick=(4, 2, 1), rebin_every=5), 3, 4),
+    ("Lees-Edwards shear, staged reorder", dict(thermostat=1, shear_rate=0.08, brick=(16, 16, 8), rebin_every=3), 1, 4),
+    ("Lees-Edwards shear, plain fused step", dict(shear_rate=0.08, dt=0.3, brick=4, rebin_every=10), 5, 3),
 ])
 def test_fused_path_directly_against_oracle(name, kw, t0, k):
     # The multi-step call runs code no single-step call runs: the collision of step t-1 inside the sweep of step t,
@@ -460,3 +468,25 @@ def test_slip_walls_plug_flow_on_gpu():
     assert ob["P"][0] - p0 == pytest.approx(n * gx * steps * h, rel=2e-5)
     assert np.abs(ob["profile"] - gx * steps * h).max() < 0.06          # flat profile (5,120 particles per layer: 4 sigma)
     assert ob["kT_cell"] == pytest.approx(1.0, rel=1e-2)
+
+
+def test_shear_flow_on_gpu_keeps_the_linear_profile():
+    # Lees-Edwards shear (U21) in one fused multi-step call on the GPU: started on the steady profile
+    # v_x = gamma (z - L_z/2), the fluid must stay on it (a wrong image displacement or velocity jump at the sheared
+    # face shows up as a kink or a drift within a few hundred steps), and the thermostat must hold k_BT.
+    cells, nbar, gam = (32, 16, 16), 10, 0.02
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    st = list(uniform_maxwell(box, n, 5))
+    st[3] = (st[3] + gam * (st[2] - box[2] / 2)).astype(np.float32)
+    g = MPC(box, cells, nbar, 3, n_max=n, thermostat=1, shear_rate=gam, rebin_every=10, brick=(16, 16, 8))
+    gpu_set(g, st)
+    prof = np.zeros(16)
+    for _ in range(10):
+        g.step(60)
+        ob = g.observables(profile=True)
+        prof += ob["profile"] / 10
+    zmid = np.arange(16) + 0.5
+    assert np.polyfit(zmid, prof, 1)[0] == pytest.approx(gam, rel=0.04)
+    assert np.abs(prof - gam * (zmid - 8.0)).max() < 0.02              # 5,120 particles per layer, 10 samples
+    assert ob["kT_cell"] == pytest.approx(1.0, rel=1e-2) and ob["n_range_overflows"] == 0
