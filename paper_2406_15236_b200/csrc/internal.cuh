@@ -33,7 +33,7 @@ typedef unsigned long long u64;
 // path; the 16x16x8 brick's tile is 18x18x10 cells = 65 KB, three of them fit in an SM's shared memory
 constexpr int HALO = 1;               // tile halo in cells on every side of a brick
 constexpr int SWEEP_T = 512;          // threads per sweep CTA (2 CTAs per SM): first-step and staged reorder sweeps
-constexpr int SWEEP_T3 = 384;         // ... of the steady-state sweep when three tiles fit in an SM's shared memory
+constexpr int SWEEP_T3 = 384;         // ... of the steady-state sweep when three tiles fit in an SM's shared memory (320: +5 %, 448: +10 %, 512 x 2: +4 %)
 constexpr int PF_DIST = 4;            // L2 prefetch distance of the sweep, in iterations of T particles (3..6 equal, 8: +2.5 %)
 constexpr int TILE_W = 5;             // int32 words per tile cell: N, Sx, Sy, Sz, E
 constexpr int REC_W = 8;              // floats per cell record (32 B, one sector)

@@ -196,21 +196,37 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
   }
   if (nbad) atomicAdd(G.nrange, (u64)nbad);
   __syncthreads();
-  // flush the tile: one packed 64-bit reduction per pair of sums, empty cells skipped
-  for (int c = threadIdx.x; c < tcells; c += T) {
-    const int* s = tile + c * TILE_W;
-    const int cnt = (int)((unsigned)s[0] & TILE_N_MASK);
-    if (cnt == 0) continue;
-    const int l0 = c % T0, q = c / T0, l1 = q % T1, l2 = q / T1;
-    u64* g = sums + (size_t)BS::key(G, foldp<P2>(ox + l0, m0), foldp<P2>(oy + l1, m1), foldp<P2>(oz + l2, m2)) * G.sw;
-    const u64 etile = ((u64)((unsigned)s[0] >> TILE_N_BITS) << TILE_E_SHIFT) + (u64)(unsigned)s[4];
-    const u64 w0 = (etile << 16) | (u64)(unsigned)cnt;
-    if (ranked) io.tbase[(size_t)b * tcells + c] = (uint32_t)(atomicAdd(g, w0) & 0xffffull);   // slots taken so far in this cell
-    else atomicAdd(g, w0);
-    atomicAdd(g + 1, pack_ss(s[1], s[2]));
-    atomicAdd(g + 2, pack_ss(s[3], 0));
-    // partial momentum sums of >= 64 particles that come within a factor two of the int32 range
-    if (cnt >= 64 && (abs(s[1]) >= (1 << 30) || abs(s[2]) >= (1 << 30) || abs(s[3]) >= (1 << 30))) atomicAdd(G.nrange, 1ull);
+  // flush the tile: one packed 64-bit reduction per pair of sums, empty cells skipped. The staging sweep of a ranked
+  // reorder needs what the count atomic returns (the slots taken so far in the cell = the first slot of this CTA's
+  // particles): FLUSH_U atomics are in flight per thread before the first return is used (one at a time cost 1.9 ms
+  // per launch at config 5: the loop is in-order, every use waits a full L2 round trip)
+  constexpr int FLUSH_U = 4;
+  for (int c0 = threadIdx.x; c0 < tcells; c0 += FLUSH_U * T) {
+    u64 old[FLUSH_U];
+#pragma unroll
+    for (int k = 0; k < FLUSH_U; ++k) {
+      const int c = c0 + k * T;
+      old[k] = ~0ull;
+      if (c >= tcells) continue;
+      const int* s = tile + c * TILE_W;
+      const int cnt = (int)((unsigned)s[0] & TILE_N_MASK);
+      if (cnt == 0) continue;
+      const int l0 = c % T0, q = c / T0, l1 = q % T1, l2 = q / T1;
+      u64* g = sums + (size_t)BS::key(G, foldp<P2>(ox + l0, m0), foldp<P2>(oy + l1, m1), foldp<P2>(oz + l2, m2)) * G.sw;
+      const u64 etile = ((u64)((unsigned)s[0] >> TILE_N_BITS) << TILE_E_SHIFT) + (u64)(unsigned)s[4];
+      const u64 w0 = (etile << 16) | (u64)(unsigned)cnt;
+      if (ranked) old[k] = atomicAdd(g, w0);
+      else atomicAdd(g, w0);
+      atomicAdd(g + 1, pack_ss(s[1], s[2]));
+      atomicAdd(g + 2, pack_ss(s[3], 0));
+      // partial momentum sums of >= 64 particles that come within a factor two of the int32 range
+      if (cnt >= 64 && (abs(s[1]) >= (1 << 30) || abs(s[2]) >= (1 << 30) || abs(s[3]) >= (1 << 30))) atomicAdd(G.nrange, 1ull);
+    }
+    if (ranked) {
+#pragma unroll
+      for (int k = 0; k < FLUSH_U; ++k)
+        if (old[k] != ~0ull) io.tbase[(size_t)b * tcells + c0 + k * T] = (uint32_t)(old[k] & 0xffffull);   // slots taken so far in this cell
+    }
   }
 }
 
