@@ -20,7 +20,8 @@ class OracleParams(C.Structure):
     _fields_ = [("collision", C.c_int), ("conserve_L", C.c_int), ("thermostat", C.c_int),
                 ("alpha", C.c_float), ("dt", C.c_float), ("kT", C.c_float), ("mass", C.c_float),
                 ("g", C.c_float * 3), ("bc", C.c_int * 3), ("grid_shift", C.c_int),
-                ("rebin_every", C.c_int), ("brick", C.c_int * 3), ("shear_rate", C.c_float)]
+                ("rebin_every", C.c_int), ("brick", C.c_int * 3), ("shear_rate", C.c_float),
+                ("phantoms", C.c_int), ("solute_id0", C.c_uint), ("solute_mass", C.c_float), ("wall_velocity", C.c_float)]
 
 
 class OracleObs(C.Structure):
@@ -57,6 +58,7 @@ def lib():
         _lib.oracle_stream_one_at.argtypes = [C.c_void_p, C.c_uint, _f32p, _f32p]
         _lib.oracle_cell_of_le.argtypes = [C.c_void_p, C.c_uint, _f32p, _f32p, _i32p, C.POINTER(C.c_uint), C.POINTER(C.c_uint),
                                            C.POINTER(C.c_int)]
+        _lib.oracle_phantoms.argtypes = [C.c_void_p, _i32p, _f32p, C.c_uint, C.c_int, _f64p, _f64p, C.POINTER(C.c_int)]
         _lib.oracle_le_offset.argtypes = [C.c_void_p, C.c_uint, C.POINTER(C.c_float), C.POINTER(C.c_float)]
     return _lib
 
@@ -68,8 +70,10 @@ def philox(ctr, key):
 
 
 def make_params(collision=0, conserve_L=0, thermostat=0, alpha_deg=130.0, dt=0.1, kT=1.0, mass=1.0,
-                g=(0.0, 0.0, 0.0), bc=(0, 0, 0), grid_shift=1, rebin_every=1, brick=1, shear_rate=0.0):
+                g=(0.0, 0.0, 0.0), bc=(0, 0, 0), grid_shift=1, rebin_every=1, brick=1, shear_rate=0.0,
+                phantoms=0, solute_id0=0, solute_mass=0.0, wall_velocity=0.0):
     p = OracleParams()
+    p.phantoms, p.solute_id0, p.solute_mass, p.wall_velocity = phantoms, solute_id0, solute_mass, wall_velocity
     p.shear_rate = shear_rate
     p.collision, p.conserve_L, p.thermostat = collision, conserve_L, thermostat
     p.alpha = np.float32(np.deg2rad(alpha_deg))
@@ -196,6 +200,14 @@ class Oracle:
         lib().oracle_cell_of_le(self._h, t, np.asarray(r, np.float32), np.asarray(s, np.float32), ijk, C.byref(cid),
                                 C.byref(key), C.byref(im))
         return ijk, cid.value, key.value, im.value
+
+    def phantoms(self, ijk, s, t, cap=256):
+        """Explicit phantom particles (reading U22) of cell ijk: (rho[n,3] cell-local coordinates, v[n,3])."""
+        rho, v, n = np.zeros(3 * cap), np.zeros(3 * cap), C.c_int()
+        rc = lib().oracle_phantoms(self._h, np.asarray(ijk, np.int32), np.asarray(s, np.float32), t, cap, rho, v, C.byref(n))
+        if rc != 0:
+            raise RuntimeError(f"oracle_phantoms failed: {rc}")
+        return rho[:3 * n.value].reshape(-1, 3), v[:3 * n.value].reshape(-1, 3)
 
     def le_offset(self, t):
         d, u = C.c_float(), C.c_float()

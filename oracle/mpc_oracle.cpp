@@ -47,6 +47,12 @@ struct Params {
   int   rebin_every;  // reorder interval
   int   brick[3];     // brick dims of the brick-major key layout ({1,1,1} = row-major); memory order only
   float shear_rate;   // Lees-Edwards shear ("shear flow can also be added", reading U21): d v_x / d z; 0 = off
+  int   phantoms;     // 1 = explicit phantom-particle set in wall-cut cells (reading U22) instead of the
+                      // velocity-only virtual particles of U8; needed for +a and MPC-AT at walls
+  unsigned solute_id0;// embedded point-particle solutes (reading U23): particles with id >= solute_id0
+  float solute_mass;  // ... have this mass instead of `mass` (0 = no solutes); they take part in the collision with their mass
+  float wall_velocity;// moving no-slip walls (Couette; "no-slip (... also supporting shear flow)", reading U24):
+                      // the wall at L moves with +wall_velocity along x, the wall at 0 with -wall_velocity
 };
 
 struct Obs {
@@ -56,7 +62,7 @@ struct Obs {
   unsigned long long n_singular_cells, step;
 };
 
-enum { TAG_SHIFT = 0, TAG_AXIS = 1, TAG_MBS = 2, TAG_AT = 3, TAG_WALL = 4 };
+enum { TAG_SHIFT = 0, TAG_AXIS = 1, TAG_MBS = 2, TAG_AT = 3, TAG_WALL = 4, TAG_PHANTOM = 5 };
 enum { E_OK = 0, E_INVAL = -1, E_STATE = -2 };
 
 struct Ctx {
@@ -221,7 +227,13 @@ inline void stream_one(const Ctx& c, float r[3], float v[3], uint32_t t) {
       if (tc > h) tc = h;
       advance(c, r, v, tc);
       r[w] = zw;
-      if (c.p.bc[w] == 1) { v[0] = -v[0]; v[1] = -v[1]; v[2] = -v[2]; }   // no-slip, bounce-back: v -> -v
+      if (c.p.bc[w] == 1) {                                                // no-slip, bounce-back: v -> -v in the frame of the wall
+        v[0] = -v[0]; v[1] = -v[1]; v[2] = -v[2];
+        if (c.p.wall_velocity != 0.0f) {                                   // moving wall (reading U24): v -> 2 u_wall - v
+          const float uw = (z1 < 0.0f) ? -c.p.wall_velocity : c.p.wall_velocity;
+          v[0] = fmaf(2.0f, uw, v[0]);
+        }
+      }
       else v[w] = -v[w];                                                   // slip, specular reflection
       const float tr = h - tc;
       advance(c, r, v, tr);
@@ -302,9 +314,157 @@ inline bool solve_inertia(const double I[6] /*xx,yy,zz,xy,xz,yz*/, const double 
 
 // ---- collision of ONE cell -------------------------------------------------------------------
 // idx[0..n) = particle indices of the cell in ascending-id order (rank = position, U4/U5).
+// ---- explicit phantom particles of a wall-cut cell (reading U22) ----------------------------
+// "The part of these collision cells in walls ... are filled with uniformly distributed phantom particles, which are
+// identical to MPC particles, such that the whole collision cell contains the same average number <N_c>", "created in
+// the subdomain where they are to be processed while random shifts are taken into account". With sigma+ = the
+// fractional part of s_w / a in (0,1): the wall occupies the cell-local range [0, sigma+) of the cut layer at the
+// wall at 0 and [sigma+, 1) of the cut layer at the wall at L. Number of phantoms of a cut cell: the wall volume
+// fraction phi times <N_c>, rounded stochastically (fp32: floorf(fmaf(nbar, phi, u))), positions uniform in the
+// wall part, velocities Gaussian about the wall velocity.
+struct Phantom { double rho[3], v[3]; };
+inline float wall_fraction(const Ctx& c, int w, const int icell[3], const float s[3], bool* top) {
+  if (c.p.bc[w] != 1 || s[w] == 0.0f) return 0.0f;
+  const float sg = s[w] * c.inv_a;
+  const float sp = (sg > 0.0f) ? sg : 1.0f + sg;
+  const int lo = (s[w] > 0.0f) ? 1 : 0, hi = (s[w] > 0.0f) ? c.n[w] + 1 : c.n[w];
+  if (icell[w] == lo) { *top = false; return sp; }
+  if (icell[w] == hi) { *top = true; return 1.0f - sp; }
+  return 0.0f;
+}
+void make_phantoms(const Ctx& c, uint32_t cid, const int icell[3], const float s[3], uint32_t t, std::vector<Phantom>& ph) {
+  ph.clear();
+  if (!c.p.phantoms) return;
+  int w = -1;
+  for (int d = 0; d < 3; ++d) if (c.p.bc[d] == 1) w = d;
+  if (w < 0) return;
+  bool top = false;
+  const float phi = wall_fraction(c, w, icell, s, &top);
+  if (!(phi > 0.0f)) return;
+  uint32_t o[4];
+  draw(c, cid, 0u, t, TAG_PHANTOM, o);
+  const float u = (float)(o[0] >> 8) * 5.9604644775390625e-08f;
+  const int nph = (int)floorf(fmaf((float)c.nbar, phi, u));
+  const float sg = s[w] * c.inv_a, sp = (sg > 0.0f) ? sg : 1.0f + sg;
+  const double sig = std::sqrt((double)c.p.kT / (double)c.p.mass);
+  const double uw = (c.p.wall_velocity != 0.0f) ? (top ? (double)c.p.wall_velocity : -(double)c.p.wall_velocity) : 0.0;
+  for (int k = 0; k < nph; ++k) {
+    Phantom q;
+    uint32_t P[4], V[4]; double g[4];
+    draw(c, cid, 1u + 2u * (uint32_t)k, t, TAG_PHANTOM, P);
+    draw(c, cid, 2u + 2u * (uint32_t)k, t, TAG_PHANTOM, V);
+    const float ua = (float)(P[0] >> 8) * 5.9604644775390625e-08f, ub = (float)(P[1] >> 8) * 5.9604644775390625e-08f;
+    const float zeta = (float)(P[2] >> 8) * 5.9604644775390625e-08f;
+    const float rw = top ? fmaf(zeta, phi, sp) : zeta * phi;
+    int e = 0;
+    for (int d = 0; d < 3; ++d) q.rho[d] = (d == w) ? (double)rw : (double)((e++ == 0) ? ua : ub);
+    normals4(V, g);
+    for (int d = 0; d < 3; ++d) q.v[d] = sig * g[d] + (d == 0 ? uw : 0.0);
+    ph.push_back(q);
+  }
+}
+
+inline double particle_mass(const Ctx& c, uint32_t id) {
+  return (c.p.solute_mass > 0.0f && id >= c.p.solute_id0) ? (double)c.p.solute_mass : (double)c.p.mass;
+}
+
+// ---- collision of ONE cell with particle masses (embedded solutes, reading U23) and explicit phantoms (U22) ----
+// The same equations with every sum weighted by the particle mass: v_cm = sum m_i v_i / sum m_i,
+// Eq. (2), Eqs. (3)-(4) with I = sum m_i (r^2 1 - r r^T) and r_cm mass-weighted, Eq. (6) with sum m_i v_ic^2 and
+// f = 3 (N_c - 1); MPC-AT: v_ran,i ~ N(0, kT / m_i), v' = v_cm + v_ran,i - sum m_j v_ran,j / sum m_j (U5).
+// Members = the real particles (ascending id) followed by the phantoms; phantoms are discarded afterwards.
+void collide_cell_ext(Ctx& c, uint32_t cid, const int icell[3], const float s[3], uint32_t t,
+                      const uint32_t* idx, unsigned n, const double* forced_axis, const double* forced_kappa) {
+  std::vector<Phantom> ph;
+  make_phantoms(c, cid, icell, s, t, ph);
+  const unsigned N = n + (unsigned)ph.size();
+  struct Mem { double m, v[3], rho[3]; };
+  std::vector<Mem> mem(N);
+  for (unsigned k = 0; k < n; ++k) {
+    const uint32_t i = idx[k];
+    mem[k].m = particle_mass(c, c.id[i]);
+    mem[k].v[0] = c.vx[i]; mem[k].v[1] = c.vy[i]; mem[k].v[2] = c.vz[i];
+    for (int d = 0; d < 3; ++d) mem[k].rho[d] = c.rho[d][i];
+  }
+  for (unsigned k = n; k < N; ++k) {
+    mem[k].m = c.p.mass;
+    for (int d = 0; d < 3; ++d) { mem[k].v[d] = ph[k - n].v[d]; mem[k].rho[d] = ph[k - n].rho[d]; }
+  }
+  if (N < 2) return;                                           // a lone particle keeps its velocity
+  double Ms = 0.0, S[3] = {0, 0, 0};
+  for (unsigned k = 0; k < N; ++k) { Ms += mem[k].m; for (int d = 0; d < 3; ++d) S[d] += mem[k].m * mem[k].v[d]; }
+  const double vcm[3] = {S[0] / Ms, S[1] / Ms, S[2] / Ms};
+  // velocity of every member after the collision rule without the +a term, relative to v_cm
+  std::vector<double> vnew(3 * (size_t)N);
+  double kappa = 1.0;
+  if (c.p.collision == 0) {
+    double axis[3];
+    if (forced_axis) { axis[0] = forced_axis[0]; axis[1] = forced_axis[1]; axis[2] = forced_axis[2]; }
+    else srd_axis(c, cid, t, axis);
+    if (forced_kappa) kappa = *forced_kappa;
+    else if (c.p.thermostat) {
+      double W2 = 0.0;                                          // sum m_i |v_i - v_cm|^2 (Eq. 6)
+      for (unsigned k = 0; k < N; ++k) for (int d = 0; d < 3; ++d) { const double w = mem[k].v[d] - vcm[d]; W2 += mem[k].m * w * w; }
+      if (W2 > 0.0) kappa = std::sqrt(2.0 * (double)c.p.kT * mbs_energy_over_kT(c, cid, t, N) / W2);
+    }
+    for (unsigned k = 0; k < N; ++k) {
+      const double w[3] = {mem[k].v[0] - vcm[0], mem[k].v[1] - vcm[1], mem[k].v[2] - vcm[2]};
+      rotate(axis, c.cosa, c.sina, w, &vnew[3 * k]);
+    }
+  } else {
+    double R[3] = {0, 0, 0};
+    for (unsigned k = 0; k < N; ++k) {
+      uint32_t o[4]; double g[4];
+      draw(c, cid, k, t, TAG_AT, o);                            // k = rank among the members
+      normals4(o, g);
+      const double sg = std::sqrt((double)c.p.kT / mem[k].m);
+      for (int d = 0; d < 3; ++d) { vnew[3 * k + d] = sg * g[d]; R[d] += mem[k].m * vnew[3 * k + d]; }
+    }
+    for (unsigned k = 0; k < N; ++k) for (int d = 0; d < 3; ++d) vnew[3 * k + d] -= R[d] / Ms;
+  }
+  double om[3] = {0, 0, 0};
+  std::vector<double> rc;
+  if (c.p.conserve_L) {
+    double rcm[3] = {0, 0, 0};
+    for (unsigned k = 0; k < N; ++k) for (int d = 0; d < 3; ++d) rcm[d] += mem[k].m * mem[k].rho[d];
+    for (int d = 0; d < 3; ++d) rcm[d] /= Ms;
+    rc.resize(3 * (size_t)N);
+    double I[6] = {0, 0, 0, 0, 0, 0}, dL[3] = {0, 0, 0}, R2 = 0.0;
+    for (unsigned k = 0; k < N; ++k) {
+      double* r = &rc[3 * k];
+      const double m = mem[k].m;
+      for (int d = 0; d < 3; ++d) r[d] = (mem[k].rho[d] - rcm[d]) * (double)c.a;
+      // change of the relative velocity by the collision rule without +a: (v - v_cm) - v_new
+      const double dv[3] = {mem[k].v[0] - vcm[0] - vnew[3 * k], mem[k].v[1] - vcm[1] - vnew[3 * k + 1], mem[k].v[2] - vcm[2] - vnew[3 * k + 2]};
+      dL[0] += m * (r[1] * dv[2] - r[2] * dv[1]);
+      dL[1] += m * (r[2] * dv[0] - r[0] * dv[2]);
+      dL[2] += m * (r[0] * dv[1] - r[1] * dv[0]);
+      const double r2 = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+      R2 += m * r2;
+      I[0] += m * (r2 - r[0] * r[0]); I[1] += m * (r2 - r[1] * r[1]); I[2] += m * (r2 - r[2] * r[2]);
+      I[3] -= m * r[0] * r[1]; I[4] -= m * r[0] * r[2]; I[5] -= m * r[1] * r[2];
+    }
+    if (N == 2) {
+      if (R2 > 0.0) for (int d = 0; d < 3; ++d) om[d] = dL[d] / R2;
+    } else if (!solve_inertia(I, dL, om)) c.n_singular++;
+  }
+  for (unsigned k = 0; k < n; ++k) {                            // phantoms are discarded
+    const uint32_t i = idx[k];
+    double o3[3] = {vcm[0] + kappa * vnew[3 * k], vcm[1] + kappa * vnew[3 * k + 1], vcm[2] + kappa * vnew[3 * k + 2]};
+    if (!rc.empty()) {
+      const double* r = &rc[3 * k];
+      o3[0] += om[1] * r[2] - om[2] * r[1];
+      o3[1] += om[2] * r[0] - om[0] * r[2];
+      o3[2] += om[0] * r[1] - om[1] * r[0];
+    }
+    c.vx[i] = (float)o3[0]; c.vy[i] = (float)o3[1]; c.vz[i] = (float)o3[2];
+  }
+}
+
 void collide_cell(Ctx& c, uint32_t cid, const int icell[3], const float s[3], uint32_t t,
                   const uint32_t* idx, unsigned n, const double* forced_axis, const double* forced_kappa) {
   if (n == 0) return;
+  if (c.p.phantoms || c.p.solute_mass > 0.0f) { collide_cell_ext(c, cid, icell, s, t, idx, n, forced_axis, forced_kappa); return; }
   const double m = c.p.mass, sig = std::sqrt((double)c.p.kT / (double)c.p.mass);
   // PROCESS: cell sums over real particles
   double S[3] = {0, 0, 0};
@@ -321,7 +481,9 @@ void collide_cell(Ctx& c, uint32_t cid, const int icell[3], const float s[3], ui
         uint32_t o[4]; double g[4];
         draw(c, cid, k, t, TAG_WALL, o);
         normals4(o, g);
-        for (int e = 0; e < 3; ++e) { virt.push_back(sig * g[e]); S[e] += sig * g[e]; }
+        // virtual particles of a moving wall are thermal about the wall velocity (reading U24)
+        const double uw = (c.p.wall_velocity != 0.0f) ? ((icell[d] <= 1) ? -(double)c.p.wall_velocity : (double)c.p.wall_velocity) : 0.0;
+        for (int e = 0; e < 3; ++e) { const double ve = sig * g[e] + (e == 0 ? uw : 0.0); virt.push_back(ve); S[e] += ve; }
       }
       Nc += nv;
     }
@@ -512,7 +674,8 @@ void one_step(Ctx& c) {
   for (size_t i = 0; i < N; ++i) {
     const uint32_t k = c.key[i];
     const double a = c.vx[i], b = c.vy[i], d = c.vz[i];
-    c.sx[k] += a; c.sy[k] += b; c.sz[k] += d; c.se[k] += a * a + b * b + d * d;
+    const double mr = particle_mass(c, c.id[i]) / (double)c.p.mass;     // 1 for a fluid particle (solutes: reading U23)
+    c.sx[k] += mr * a; c.sy[k] += mr * b; c.sz[k] += mr * d; c.se[k] += mr * (a * a + b * b + d * d);
   }
   // 6.-7. PROCESS_CELLS + ROTATE_VELOCITIES
   c.n_singular = 0;
@@ -549,7 +712,11 @@ int oracle_create(void** out, const float box[3], const int cells[3], float n_pe
     if (p->bc[d] != 0) { nwall++; if (p->g[d] != 0.0f) return E_INVAL; }   // no force along the wall normal
   }
   if (nwall > 1) return E_INVAL;                                            // slit geometry only
-  if (nwall && (p->conserve_L || p->collision == 1)) return E_INVAL;        // needs explicit phantom sets (U8)
+  if (nwall && (p->conserve_L || p->collision == 1) && !p->phantoms) return E_INVAL;   // needs explicit phantom sets (U8, U22)
+  if (p->phantoms < 0 || p->phantoms > 1 || (p->phantoms && !nwall)) return E_INVAL;
+  if (p->solute_mass < 0.0f) return E_INVAL;
+  if (p->wall_velocity != 0.0f && (!nwall || p->bc[0] != 0)) return E_INVAL;            // moving walls: no-slip wall axis y or z, flow along x (U24)
+  for (int d = 0; d < 3; ++d) if (p->wall_velocity != 0.0f && p->bc[d] == 2) return E_INVAL;
   if (p->collision == 0 && p->conserve_L && p->thermostat) return E_INVAL;  // ambiguous (U6)
   if (!(n_per_cell > 0.0f)) return E_INVAL;
   if (p->shear_rate != 0.0f && (nwall || p->collision == 1 || p->conserve_L)) return E_INVAL;   // Lees-Edwards: periodic SRD only (U21)
@@ -635,24 +802,25 @@ int oracle_observables(void* h, Obs* o, float* profile) {
   if (!c->have_state) return E_STATE;
   const size_t N = c->x.size();
   const double m = c->p.mass;
-  double P[3] = {0, 0, 0}, E = 0;
+  double P[3] = {0, 0, 0}, E = 0, Mr = 0;   // in units of the fluid-particle mass
   for (size_t i = 0; i < N; ++i) {
     const double a = c->vx[i], b = c->vy[i], d = c->vz[i];
-    P[0] += a; P[1] += b; P[2] += d; E += a * a + b * b + d * d;
+    const double mr = particle_mass(*c, c->id[i]) / m;
+    P[0] += mr * a; P[1] += mr * b; P[2] += mr * d; E += mr * (a * a + b * b + d * d); Mr += mr;
   }
   o->n = N; o->step = c->t;
   for (int d = 0; d < 3; ++d) o->P[d] = m * P[d];
   o->E_kin = 0.5 * m * E;
-  // global estimate: m sum |v - <v>|^2 / (3 (N-1))
-  o->kT_est = (N > 1) ? m * (E - (P[0] * P[0] + P[1] * P[1] + P[2] * P[2]) / (double)N) / (3.0 * (double)(N - 1)) : 0.0;
+  // global estimate: sum m_i |v_i - <v>|^2 / (3 (N-1)), <v> = sum m_i v_i / sum m_i
+  o->kT_est = (N > 1) ? m * (E - (P[0] * P[0] + P[1] * P[1] + P[2] * P[2]) / Mr) / (3.0 * (double)(N - 1)) : 0.0;
   // cell-level estimate from the last step's pre-collision sums: <m sum w^2> / <3 (N_c - 1)>
   o->kT_cell = 0.0; o->max_cell_count = 0; o->n_singular_cells = c->n_singular;
   if (c->have_cells) {
-    double num = 0, den = 0;
+    double num = 0, den = 0;   // (with solutes the sums are mass-weighted and this estimate is not formed: 0)
     for (size_t k = 0; k < c->nkeys; ++k) {
       const unsigned nc = c->count[k];
       if (nc > o->max_cell_count) o->max_cell_count = nc;
-      if (nc < 2) continue;
+      if (nc < 2 || c->p.solute_mass > 0.0f) continue;
       num += m * (c->se[k] - (c->sx[k] * c->sx[k] + c->sy[k] * c->sy[k] + c->sz[k] * c->sz[k]) / nc);
       den += 3.0 * (nc - 1);
     }
@@ -739,6 +907,18 @@ int oracle_le_offset(void* h, unsigned t, float* D, float* U) {
   if (!h) return E_INVAL;
   if (D) *D = le_offset(*(Ctx*)h, t);
   if (U) *U = le_velocity(*(Ctx*)h);
+  return E_OK;
+}
+// explicit phantom particles (reading U22) of cell ijk for lattice shift s at step t: up to `cap` of them as
+// rho[3k..3k+2] (cell-local coordinates) and v[3k..3k+2]; *n = their number
+int oracle_phantoms(void* h, const int ijk[3], const float s[3], unsigned t, int cap, double* rho, double* v, int* n) {
+  if (!h || !ijk || !s || !n) return E_INVAL;
+  Ctx& c = *(Ctx*)h;
+  std::vector<Phantom> ph;
+  make_phantoms(c, canonical_id(c, ijk), ijk, s, t, ph);
+  *n = (int)ph.size();
+  for (int k = 0; k < (int)ph.size() && k < cap; ++k)
+    for (int d = 0; d < 3; ++d) { if (rho) rho[3 * k + d] = ph[k].rho[d]; if (v) v[3 * k + d] = ph[k].v[d]; }
   return E_OK;
 }
 // Collide the whole current state as ONE cell (cell id `cid`, step t) with a prescribed axis and/or
