@@ -65,6 +65,17 @@ typedef struct {
   float shear_rate;  /* Lees-Edwards shear d v_x / d z (U21): the periodic images above /
                         below the box along z are displaced by +-shear_rate L_z t along x and move with
                         +-shear_rate L_z. 0 = off. Needs periodic boundaries on all axes, SRD without +a             */
+  int   phantoms;    /* 1 = explicit phantom-particle set in the wall part of wall-cut cells (U22):
+                        positions uniform in the wall part, velocities Gaussian about the wall velocity, number = wall
+                        fraction x round(n_per_cell), rounded stochastically. Needs a no-slip wall axis and rebin_every = 1.
+                        Required for +a and MPC-AT at walls. 0 = the velocity-only virtual particles of U8 (SRD -a only)  */
+  unsigned solute_id0; /* embedded point-particle solutes (U23): particles with id >= solute_id0 */
+  float solute_mass; /* ... have this mass instead of `mass` and take part in the collision with it (all cell sums are
+                        mass-weighted; MPC-AT draws them from N(0, kT/solute_mass)). 0 = no solutes. Needs rebin_every = 1;
+                        not with Lees-Edwards shear. Solutes stream ballistically like fluid particles                   */
+  float wall_velocity; /* moving no-slip walls (plane Couette flow; U24): the wall at L moves with
+                        +wall_velocity along x, the wall at 0 with -wall_velocity; bounce-back in the frame of the wall
+                        (v -> 2 u_wall - v), wall / phantom particles thermal about u_wall. Needs bc = 1 on y or z            */
 } mpc_params;
 
 typedef struct {
@@ -89,7 +100,9 @@ typedef struct {
  * (L_x/n_x == L_y/n_y == L_z/n_z == a). n_per_cell = <N_c>, used for the virtual-wall-particle fill
  * (round(n_per_cell)) and for sizing. Allocates nothing on the device.
  * MPC_EINVAL: NULL argument, fewer than 3 cells along an axis, non-cubic cells, non-positive sizes/dt/kT/mass, rebin_every < 1,
- * brick dims not powers of two in 1..64 or tile too large for shared memory, more than one wall axis, force along a wall normal, walls with +a or MPC-AT,
+ * brick dims not powers of two in 1..64 or tile too large for shared memory, more than one wall axis, force along a wall normal, walls with +a or MPC-AT
+ * but without phantoms, phantoms without a no-slip wall, phantoms or solutes with rebin_every != 1 or with shear_rate, wall_velocity without a no-slip
+ * wall on y or z,
  * SRD+a with thermostat (U6), MPC-AT with rebin_every != 1, key space >= 2^32, shear_rate != 0 with walls, MPC-AT or +a. */
 int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_per_cell,
                const mpc_params* p, unsigned long long seed);

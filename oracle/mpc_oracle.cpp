@@ -713,7 +713,9 @@ int oracle_create(void** out, const float box[3], const int cells[3], float n_pe
   }
   if (nwall > 1) return E_INVAL;                                            // slit geometry only
   if (nwall && (p->conserve_L || p->collision == 1) && !p->phantoms) return E_INVAL;   // needs explicit phantom sets (U8, U22)
-  if (p->phantoms < 0 || p->phantoms > 1 || (p->phantoms && !nwall)) return E_INVAL;
+  bool noslip = false;
+  for (int d = 0; d < 3; ++d) if (p->bc[d] == 1) noslip = true;
+  if (p->phantoms < 0 || p->phantoms > 1 || (p->phantoms && !noslip)) return E_INVAL;   // phantoms fill no-slip walls (U20: none at slip walls)
   if (p->solute_mass < 0.0f) return E_INVAL;
   if (p->wall_velocity != 0.0f && (!nwall || p->bc[0] != 0)) return E_INVAL;            // moving walls: no-slip wall axis y or z, flow along x (U24)
   for (int d = 0; d < 3; ++d) if (p->wall_velocity != 0.0f && p->bc[d] == 2) return E_INVAL;

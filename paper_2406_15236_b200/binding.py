@@ -26,7 +26,8 @@ class mpc_params(C.Structure):
     _fields_ = [("collision", C.c_int), ("conserve_L", C.c_int), ("thermostat", C.c_int),
                 ("alpha", C.c_float), ("dt", C.c_float), ("kT", C.c_float), ("mass", C.c_float),
                 ("g", C.c_float * 3), ("bc", C.c_int * 3), ("grid_shift", C.c_int),
-                ("rebin_every", C.c_int), ("brick", C.c_int * 3), ("shear_rate", C.c_float)]
+                ("rebin_every", C.c_int), ("brick", C.c_int * 3), ("shear_rate", C.c_float),
+                ("phantoms", C.c_int), ("solute_id0", C.c_uint), ("solute_mass", C.c_float), ("wall_velocity", C.c_float)]
 
 
 class mpc_obs(C.Structure):
@@ -89,8 +90,10 @@ def philox4x32_10(ctr, key):
 
 
 def make_params(collision=0, conserve_L=0, thermostat=0, alpha_deg=130.0, dt=0.1, kT=1.0, mass=1.0,
-                g=(0.0, 0.0, 0.0), bc=(0, 0, 0), grid_shift=1, rebin_every=1, brick=1, shear_rate=0.0):
+                g=(0.0, 0.0, 0.0), bc=(0, 0, 0), grid_shift=1, rebin_every=1, brick=1, shear_rate=0.0,
+                phantoms=0, solute_id0=0, solute_mass=0.0, wall_velocity=0.0):
     p = mpc_params()
+    p.phantoms, p.solute_id0, p.solute_mass, p.wall_velocity = phantoms, solute_id0, solute_mass, wall_velocity
     p.shear_rate = shear_rate
     p.collision, p.conserve_L, p.thermostat = collision, conserve_L, thermostat
     p.alpha = np.float32(np.deg2rad(alpha_deg))

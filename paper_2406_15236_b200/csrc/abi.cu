@@ -185,7 +185,11 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
     if (p->bc[d] != 0) { nwall++; wall = d; if (p->g[d] != 0.0f) return MPC_EINVAL; }
   }
   if (nwall > 1) return MPC_EINVAL;
-  if (nwall && (p->conserve_L || p->collision == 1)) return MPC_EINVAL;
+  if (nwall && (p->conserve_L || p->collision == 1) && !p->phantoms) return MPC_EINVAL;     // needs explicit phantoms (U8, U22)
+  if (p->phantoms < 0 || p->phantoms > 1 || (p->phantoms && (!nwall || p->bc[wall] != 1))) return MPC_EINVAL;
+  if (p->solute_mass < 0.0f) return MPC_EINVAL;
+  if ((p->phantoms || p->solute_mass > 0.0f) && (p->rebin_every != 1 || p->shear_rate != 0.0f)) return MPC_EINVAL;   // per-cell segment pass only
+  if (p->wall_velocity != 0.0f && (!nwall || wall == 0 || p->bc[wall] != 1)) return MPC_EINVAL;    // moving walls: no-slip, flow along x (U24)
   if (p->collision == 0 && p->conserve_L && p->thermostat) return MPC_EINVAL;
   if (p->collision == 1 && p->rebin_every != 1) return MPC_EINVAL;
   if (p->shear_rate != 0.0f && (nwall || p->collision == 1 || p->conserve_L)) return MPC_EINVAL;   // Lees-Edwards: periodic SRD only (U21)
@@ -236,7 +240,8 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   G.le_u = (float)((double)p->shear_rate * (double)box[2]);
   G.le_d = 0.0f;
   G.collision = p->collision; G.thermostat = p->thermostat; G.conserve_L = p->conserve_L;
-  G.generic = (p->collision == 1 || p->conserve_L) ? 1 : 0;
+  G.phantoms = p->phantoms; G.solute_id0 = p->solute_id0; G.solute_mass = p->solute_mass; G.wall_u = p->wall_velocity;
+  G.generic = (p->collision == 1 || p->conserve_L || p->phantoms || p->solute_mass > 0.0f) ? 1 : 0;
   G.sw = (p->collision == 0 && p->conserve_L) ? 16 : 3;
   G.rw = p->conserve_L ? 16 : REC_W;
   *out = c;

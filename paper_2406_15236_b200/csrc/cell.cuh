@@ -42,6 +42,22 @@ __device__ __forceinline__ float mbs_exponentials(const Geo& G, uint32_t cid, ui
   return -(float)((double)__logf(p) + (double)ex * 0.6931471805599453);
 }
 
+
+// kappa of Eq. (6) for a cell of nc >= 2 members with mw2 = sum m_i |v_i - v_cm|^2 > 0; o = the cell's TAG_AXIS block,
+// whose words 2, 3 give the half squared normal when f = 3 (nc - 1) is odd (U6)
+__device__ __forceinline__ float mbs_kappa(const Geo& G, uint32_t cid, const Block4& o, uint32_t nc, float mw2) {
+  const uint32_t f = 3u * (nc - 1u);
+  float ek = mbs_exponentials(G, cid, f >> 1);
+  if (f & 1u) {
+    // cos(2 pi u) = -cos(2 pi (u - 1/2)), argument in [-pi, pi): __cosf / __logf are accurate to ~4e-7 absolute there,
+    // far below the statistical meaning of the draw and the 2e-5 parity budget
+    const float cs = __cosf(6.2831853071795865f * (u01_co(o.d) - 0.5f));
+    ek -= __logf(u01_oc(o.c)) * cs * cs;
+  }
+  const float x = __fdividef(2.0f * (G.kT * ek), mw2);
+  return x * rsqrtf(fmaxf(x, 1e-37f));
+}
+
 // rec[key] = { vcm.x, vcm.y, vcm.z, kappa, n.x, n.y, n.z, - }
 // grid = (mb0 * CTAs-per-brick, mb1, mb2): the brick coordinates come from blockIdx, no division.
 // zero != 0: the sums of a cell are cleared once read, which saves the memset before the next step's sweep.
@@ -99,11 +115,12 @@ __device__ __forceinline__ void cell_batch(const Geo& G, uint32_t bx, uint32_t b
       const bool cut = (sw > 0.0f) ? (iw == 1 || iw == nw + 1) : (sw < 0.0f) ? (iw == 0 || iw == nw) : false;
       if (cut && (int)nreal < G.nbar) {
         const uint32_t nv = (uint32_t)G.nbar - nreal;
+        const double uw = (iw <= 1) ? -(double)G.wall_u : (double)G.wall_u;   // thermal about the wall velocity (U24)
         for (uint32_t j = 0; j < nv; ++j) {
           const Block4 o = philox_rk(cw.cid, j, G.t, TAG_WALL, G.rk);
           float g0, g1, g2;
           normals3(o, g0, g1, g2);
-          const double a = (double)(G.sigma * g0), b = (double)(G.sigma * g1), c = (double)(G.sigma * g2);
+          const double a = (double)(G.sigma * g0) + uw, b = (double)(G.sigma * g1), c = (double)(G.sigma * g2);
           S0 += a; S1 += b; S2 += c; E += a * a + b * b + c * c;
         }
         Nc += nv;
@@ -143,19 +160,7 @@ __device__ __forceinline__ void cell_batch(const Geo& G, uint32_t bx, uint32_t b
   const CellWork c = work[u];
   if (c.nc == 0u) return;
   const Block4 o = philox_rk(c.cid, 0u, G.t, TAG_AXIS, G.rk);
-  float kappa = 1.0f;
-  if (c.w2 > 0.0f) {
-    const uint32_t f = 3u * (c.nc - 1u);
-    float ek = mbs_exponentials(G, c.cid, f >> 1);
-    if (f & 1u) {   // f odd: half a squared normal from words 2, 3 of the axis block (U6)
-      // cos(2 pi u) = -cos(2 pi (u - 1/2)), argument in [-pi, pi): __cosf / __logf are accurate to ~4e-7 absolute there,
-      // far below the statistical meaning of the draw and the 2e-5 parity budget
-      const float cs = __cosf(6.2831853071795865f * (u01_co(o.d) - 0.5f));
-      ek -= __logf(u01_oc(o.c)) * cs * cs;
-    }
-    const float x = __fdividef(2.0f * (G.kT * ek), G.mass * c.w2);
-    kappa = x * rsqrtf(fmaxf(x, 1e-37f));
-  }
+  const float kappa = (c.w2 > 0.0f) ? mbs_kappa(G, c.cid, o, c.nc, G.mass * c.w2) : 1.0f;
   const float zz = 2.0f * u01_co(o.a) - 1.0f;
   const float rr = sqrtf((1.0f - zz) * (1.0f + zz));
   float sp, cp;

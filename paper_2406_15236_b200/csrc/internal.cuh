@@ -85,6 +85,10 @@ struct Geo {
   int shear;      // Lees-Edwards shear along z, flow along x (U21)
   float le_u;     // velocity of the image above: shear_rate * L_z
   float le_d;     // x displacement of the image above at the time the positions of this step refer to
+  int phantoms;        // explicit phantom particles in wall-cut cells (U22)
+  uint32_t solute_id0; // particles with id >= solute_id0 have mass solute_mass (if > 0; U23)
+  float solute_mass;
+  float wall_u;        // moving no-slip walls: +wall_u along x at L, -wall_u at 0 (U24)
 };
 
 // ---- packed sums ---------------------------------------------------------------------------------
@@ -182,7 +186,10 @@ __device__ __forceinline__ void stream_one(const Geo& G, float (&r)[3], float (&
       if (w == 0) r[0] = zw; else if (w == 1) r[1] = zw; else r[2] = zw;
       if (G.slip) {   // specular reflection: only the wall-normal component turns round
         if (w == 0) v[0] = -v[0]; else if (w == 1) v[1] = -v[1]; else v[2] = -v[2];
-      } else { v[0] = -v[0]; v[1] = -v[1]; v[2] = -v[2]; }   // bounce-back
+      } else {                                                // bounce-back, in the frame of a moving wall (U24): v -> 2 u_wall - v
+        v[0] = -v[0]; v[1] = -v[1]; v[2] = -v[2];
+        if (G.wall_u != 0.0f) v[0] = fmaf(2.0f, (z1 < 0.0f) ? -G.wall_u : G.wall_u, v[0]);
+      }
       advance<GRAV>(G, r, v, G.dt - tc);
       if (w == 0) r[0] = fminf(fmaxf(r[0], 0.0f), Lw);
       else if (w == 1) r[1] = fminf(fmaxf(r[1], 0.0f), Lw);

@@ -14,16 +14,20 @@ __device__ __forceinline__ double block_sum(double v, double* sh) {
   __syncthreads();
   return t;
 }
-__global__ void __launch_bounds__(256) k_obs_particles(size_t n, const float* __restrict__ vx, const float* __restrict__ vy,
-                                                       const float* __restrict__ vz, double* __restrict__ part) {
+// sums of m_i v_i, m_i |v_i|^2 and m_i in units of the fluid-particle mass (solutes: DESIGN.md U23)
+__global__ void __launch_bounds__(256) k_obs_particles(Geo G, size_t n, const float* __restrict__ vx, const float* __restrict__ vy,
+                                                       const float* __restrict__ vz, const uint32_t* __restrict__ id, double* __restrict__ part) {
   __shared__ double sh[8];
-  double a = 0, b = 0, c = 0, e = 0;
+  double a = 0, b = 0, c = 0, e = 0, ms = 0;
+  const bool solutes = G.solute_mass > 0.0f;
+  const double mrs = (double)G.solute_mass / (double)G.mass;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
     const double p = vx[i], q = vy[i], r = vz[i];
-    a += p; b += q; c += r; e += p * p + q * q + r * r;
+    const double mr = (solutes && id[i] >= G.solute_id0) ? mrs : 1.0;
+    a += mr * p; b += mr * q; c += mr * r; e += mr * (p * p + q * q + r * r); ms += mr;
   }
-  a = block_sum(a, sh); b = block_sum(b, sh); c = block_sum(c, sh); e = block_sum(e, sh);
-  if (threadIdx.x == 0) { double* o = part + (size_t)blockIdx.x * 8; o[0] = a; o[1] = b; o[2] = c; o[3] = e; }
+  a = block_sum(a, sh); b = block_sum(b, sh); c = block_sum(c, sh); e = block_sum(e, sh); ms = block_sum(ms, sh);
+  if (threadIdx.x == 0) { double* o = part + (size_t)blockIdx.x * 8; o[0] = a; o[1] = b; o[2] = c; o[3] = e; o[7] = ms; }
 }
 __global__ void __launch_bounds__(256) k_obs_cells(Geo G, const u64* __restrict__ sums, double* __restrict__ part) {
   __shared__ double sh[8];
@@ -125,7 +129,7 @@ int observables_impl(mpc_ctx* c, mpc_obs* out, float* profile_host, int n_profil
     FamilyTimer ft(c, F_OBS);
     CU(cudaMemsetAsync(c->obs, 0, OBS_HOST_DOUBLES * 8, c->stream));
     if (n) {
-      k_obs_particles<<<OBS_BLOCKS, 256, 0, c->stream>>>(n, F[3], F[4], F[5], part);
+      k_obs_particles<<<OBS_BLOCKS, 256, 0, c->stream>>>(G, n, F[3], F[4], F[5], c->A[6], part);
       LAUNCH_CHECK("k_obs_particles");
       if (profile_host) {
         k_obs_profile<<<OBS_BLOCKS, 256, (size_t)2 * nb * 8, c->stream>>>(G, n, nb, F[pa], F[3 + fa], prof);
@@ -143,17 +147,17 @@ int observables_impl(mpc_ctx* c, mpc_obs* out, float* profile_host, int n_profil
   if (c->have_cells && G.conserve_L) CU(cudaMemcpyAsync(&nsing, c->nsing, 8, cudaMemcpyDeviceToHost, c->stream));
   CU(cudaMemcpyAsync(&nrange, c->nrange, 8, cudaMemcpyDeviceToHost, c->stream));
   CU(cudaStreamSynchronize(c->stream));
-  double P[3] = {0, 0, 0}, E = 0, num = 0, den = 0, mx = 0;
+  double P[3] = {0, 0, 0}, E = 0, num = 0, den = 0, mx = 0, Mr = 0;
   for (int b = 0; b < OBS_BLOCKS; ++b) {
     const double* o = hbuf + (size_t)b * 8;
-    P[0] += o[0]; P[1] += o[1]; P[2] += o[2]; E += o[3]; num += o[4]; den += o[5];
+    P[0] += o[0]; P[1] += o[1]; P[2] += o[2]; E += o[3]; num += o[4]; den += o[5]; Mr += o[7];
     if (o[6] > mx) mx = o[6];
   }
   const double m = G.mass;
   out->n = n; out->step = c->t;
   for (int d = 0; d < 3; ++d) out->P[d] = m * P[d];
   out->E_kin = 0.5 * m * E;
-  out->kT_est = n > 1 ? m * (E - (P[0] * P[0] + P[1] * P[1] + P[2] * P[2]) / (double)n) / (3.0 * (double)(n - 1)) : 0.0;
+  out->kT_est = n > 1 ? m * (E - (P[0] * P[0] + P[1] * P[1] + P[2] * P[2]) / Mr) / (3.0 * (double)(n - 1)) : 0.0;
   out->kT_cell = (!G.generic && den > 0) ? num / den : 0.0;
   out->max_cell_count = (unsigned)mx;
   out->n_singular_cells = nsing;

@@ -6,7 +6,7 @@
 
 namespace mpc {
 
-enum : uint32_t { TAG_SHIFT = 0, TAG_AXIS = 1, TAG_MBS = 2, TAG_AT = 3, TAG_WALL = 4 };
+enum : uint32_t { TAG_SHIFT = 0, TAG_AXIS = 1, TAG_MBS = 2, TAG_AT = 3, TAG_WALL = 4, TAG_PHANTOM = 5 };
 
 struct Block4 { uint32_t a, b, c, d; };
 
