@@ -214,6 +214,8 @@ def measure(args, workload, nbar, steps, warmup, rank, local_rank, world, dist, 
     st = list(uniform_maxwell_cuda(box, n, 1234 + rank, device=str(device), to_host=via_host))
     torch.cuda.empty_cache()
     sim = MPC(box, cells, nbar, 1234 + rank, n_max=n, device=str(device), compact=compact, **kw)
+    if args.debug:
+        sim.set_debug(args.debug)
     if via_host:
         sim.set_state_host(*st)
     else:
@@ -307,6 +309,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the density sweep and the other workloads")
     ap.add_argument("--compact", action="store_true", help="property-wise reorder workspace")
+    ap.add_argument("--debug", type=int, default=0, help="mpc_set_debug flags (A/B runs of the diagnostic code paths; changes speed only)")
     ap.add_argument("--cells", default=None, help="override the workload's cell grid, e.g. 256,256,256 (profiling runs)")
     args = ap.parse_args()
     wl = dict(WORKLOADS[args.workload])

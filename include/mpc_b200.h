@@ -148,6 +148,7 @@ int mpc_step(mpc_ctx*, int nsteps);
 #define MPC_DEBUG_EAGER_CANONICAL 2u /* reorder: rank by id at every reorder instead of lazily on read             */
 #define MPC_DEBUG_ATOMIC_SCATTER  4u /* reorder: cursor atomics per run of particles instead of the sweep's ranks   */
 #define MPC_DEBUG_EAGER_COLLIDE   8u /* apply the last step's collision at the end of mpc_step (separate pass)      */
+#define MPC_DEBUG_NO_LANE_SPREAD 16u /* reorder: plain cell order in memory instead of the lane-spread order (5a)  */
 int mpc_set_debug(mpc_ctx*, unsigned flags);
 
 /* Copy the state out, in the current internal order, with ids. Any pointer may be NULL (skipped).

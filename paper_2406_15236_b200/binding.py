@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("MPC_B200_LIB", os.path.join(HERE, "libmpc_b200.so"))   # override: alternative builds
 
 MPC_OK, MPC_EINVAL, MPC_ESTATE, MPC_ENOMEM, MPC_ECUDA, MPC_ERANGE = 0, -1, -2, -3, -4, -5
-DEBUG_NO_FUSE_GATHER, DEBUG_EAGER_CANONICAL, DEBUG_ATOMIC_SCATTER, DEBUG_EAGER_COLLIDE = 1, 2, 4, 8
+DEBUG_NO_FUSE_GATHER, DEBUG_EAGER_CANONICAL, DEBUG_ATOMIC_SCATTER, DEBUG_EAGER_COLLIDE, DEBUG_NO_LANE_SPREAD = 1, 2, 4, 8, 16
 
 # every symbol include/mpc_b200.h declares
 SYMBOLS = ["mpc_create", "mpc_num_keys", "mpc_workspace_bytes", "mpc_bind", "mpc_set_state", "mpc_set_state_host",

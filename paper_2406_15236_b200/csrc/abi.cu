@@ -131,7 +131,7 @@ int set_state_impl(mpc_ctx* c, unsigned long long n, const float* const src[6], 
   }
   CU(cudaMemsetAsync(c->nrange, 0, 8, c->stream));
   c->n = n; c->t = step; c->have_state = true; c->have_cells = false; c->have_order = false; c->gather_pending = false;
-  c->order_canonical = true; c->collide_pending = false;
+  c->order_canonical = true; c->order_spread = false; c->collide_pending = false;
   return MPC_OK;
 }
 int get_state_impl(mpc_ctx* c, float* const dst[6], unsigned* id, cudaMemcpyKind kind) {
@@ -292,7 +292,7 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
   c->chunk0 = staged ? (uint32_t*)(c->ws + l.off_chunk0) : nullptr;
   CU(cudaMemsetAsync(c->nrange, 0, 8, c->stream));
   c->bound = true; c->have_state = false; c->have_cells = false; c->have_order = false; c->sums_clean = false; c->gather_pending = false;
-  c->collide_pending = false; c->ranked_keys = false; c->n = 0;
+  c->collide_pending = false; c->ranked_keys = false; c->order_spread = false; c->n = 0;
   if (c->tile_bytes > 48 * 1024) {
     const cudaError_t e = sweep_set_attributes(c->tile_bytes);
     if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(k_sweep, MaxDynamicSharedMemorySize)");
@@ -302,7 +302,7 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
 
 int mpc_set_debug(mpc_ctx* c, unsigned flags) {
   if (!c) return MPC_EINVAL;
-  if (flags & ~(MPC_DEBUG_NO_FUSE_GATHER | MPC_DEBUG_EAGER_CANONICAL | MPC_DEBUG_ATOMIC_SCATTER | MPC_DEBUG_EAGER_COLLIDE)) return fail(c, MPC_EINVAL, "unknown debug flag");
+  if (flags & ~(MPC_DEBUG_NO_FUSE_GATHER | MPC_DEBUG_EAGER_CANONICAL | MPC_DEBUG_ATOMIC_SCATTER | MPC_DEBUG_EAGER_COLLIDE | MPC_DEBUG_NO_LANE_SPREAD)) return fail(c, MPC_EINVAL, "unknown debug flag");
   if (c->gather_pending) return fail(c, MPC_ESTATE, "internal: gather pending");   // cannot happen between API calls
   c->debug = flags;
   return MPC_OK;

@@ -288,6 +288,7 @@ struct mpc_ctx {
   // applies it; every call that reads particle velocities applies it first (flush_collide)
   bool collide_pending;
   bool pow2_cells;      // no walls and every m[d] a power of two: the sweep folds indices with a mask
+  bool order_spread;    // the particles of every group of 32 keys are stored lane-spread (reorder.cu, spread_slot)
   bool ranked_keys;     // the last staging sweep wrote (tile cell, arrival rank) words into key[] instead of keys
   float le_dprev;       // Lees-Edwards displacement of the step whose collision is pending
   unsigned debug;       // MPC_DEBUG_* flags

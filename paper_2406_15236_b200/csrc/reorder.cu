@@ -86,6 +86,26 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const uint32_t* __restric
 }
 
 // ---- scatter --------------------------------------------------------------------------------------
+// ---- lane-spread order inside a group of 32 cells (hot path) ---------------------------
+// The sweep's shared-memory atomics serialise on lanes of a warp that hit the same cell; in plain cell order a warp's
+// 32 consecutive particles sit in ~3 cells. The hot-path reorder therefore stores the n_g particles of every aligned
+// group of 32 keys (one contiguous range [g0, g1) of the counting sort, always inside one brick) TRANSPOSED: with
+// R = n_g / 32, sorted position p < 32 R goes to row p % R, column p / R of an R x 32 matrix, so neighbouring lanes
+// hold particles R ~ <N_c> sorted positions apart: (mostly) different cells. The tail p >= 32 R stays where it is.
+// The brick ranges the sweep works on are unchanged; the order inside a cell does not enter the physics (integer sums);
+// canonicalise() reads the cells back through the same map.
+__device__ __forceinline__ uint32_t spread_slot(uint32_t slot, uint32_t g0, uint32_t g1) {
+  const uint32_t R = (g1 - g0) >> 5, p = slot - g0;
+  if (p >= (R << 5)) return slot;
+  const uint32_t col = p / R, row = p - col * R;
+  return g0 + (row << 5) + col;
+}
+__device__ __forceinline__ uint32_t spread_key(const uint32_t* __restrict__ offset, uint32_t k, uint32_t slot, int spread) {
+  if (!spread) return slot;
+  const uint32_t kg = k & ~31u;
+  return spread_slot(slot, offset[kg], offset[kg + 32u]);
+}
+
 // Lanes of a warp that hold the same key as their neighbours form runs (the array is still nearly sorted):
 // one cursor atomic per run. Returns the first slot of this lane within its cell segment's arrival order.
 // (match.any would also merge non-adjacent lanes but runs at a fraction of the rate: measured 72 % pipe busy.)
@@ -132,7 +152,7 @@ __global__ void __launch_bounds__(256) k_rank(size_t n, const uint32_t* __restri
 // latency of the chain key load -> cursor atomic (with return) -> store.
 constexpr int SCAT_U = 4;
 __global__ void __launch_bounds__(256) k_scatter_src(size_t n, const uint32_t* __restrict__ key, const uint32_t* __restrict__ offset,
-                                                     uint32_t* __restrict__ cursor, uint32_t* __restrict__ perm) {
+                                                     uint32_t* __restrict__ cursor, uint32_t* __restrict__ perm, int spread) {
   const size_t base = (size_t)blockIdx.x * (256 * SCAT_U) + threadIdx.x;
   const unsigned lane = threadIdx.x & 31u, le = 0xffffffffu >> (31u - lane);
   uint32_t k[SCAT_U], slot[SCAT_U];
@@ -164,7 +184,7 @@ __global__ void __launch_bounds__(256) k_scatter_src(size_t n, const uint32_t* _
 #pragma unroll
   for (int j = 0; j < SCAT_U; ++j) {
     const uint32_t b = __shfl_sync(0xffffffffu, slot[j], leader[j]);
-    if (ok[j]) perm[off[j] + b + (lane - (unsigned)leader[j])] = (uint32_t)(base + (size_t)j * 256);
+    if (ok[j]) perm[spread_key(offset, k[j], off[j] + b + (lane - (unsigned)leader[j]), spread)] = (uint32_t)(base + (size_t)j * 256);
   }
 }
 
@@ -183,8 +203,8 @@ __global__ void __launch_bounds__(256) k_save_chunks(const uint32_t* __restrict_
 template <class BS>
 __global__ void __launch_bounds__(512) k_scatter_tile(Geo G, uint32_t n, const uint32_t* __restrict__ word, const uint32_t* __restrict__ chunk0,
                                                       uint32_t nbricks, const uint32_t* __restrict__ offset, const uint32_t* __restrict__ tbase,
-                                                      const float* __restrict__ aos, uint32_t* __restrict__ perm) {
-  extern __shared__ uint32_t dest[];     // per tile cell: next free slot
+                                                      const float* __restrict__ aos, uint32_t* __restrict__ perm, int spread) {
+  extern __shared__ uint32_t dest[];     // per tile cell: next free slot; then (spread) first slot and size of the cell's group of 32 keys
   const int T0 = (1 << BS::s0(G)) + 2 * HALO, T1 = (1 << BS::s1(G)) + 2 * HALO, T2 = (1 << BS::s2(G)) + 2 * HALO;
   const int tcells = T0 * T1 * T2;
   const uint32_t b = blockIdx.x;
@@ -202,33 +222,54 @@ __global__ void __launch_bounds__(512) k_scatter_tile(Geo G, uint32_t n, const u
     const int l0 = c % T0, q = c / T0, l1 = q % T1, l2 = q / T1;
     // wall axes do not wrap: tile cells beyond the last layer hold no particles, their slot is never read
     const int kx = fold(ox + l0, m0), ky = fold(oy + l1, m1), kz = fold(oz + l2, m2);
-    dest[c] = offset[BS::key(G, kx, ky, kz)] + tbase[(size_t)b * tcells + c];
+    const uint32_t k = BS::key(G, kx, ky, kz);
+    dest[c] = offset[k] + tbase[(size_t)b * tcells + c];
+    if (spread) { const uint32_t g0 = offset[k & ~31u]; dest[tcells + c] = g0; dest[2 * tcells + c] = offset[(k & ~31u) + 32u] - g0; }
   }
   __syncthreads();
-  for (uint32_t i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
-    const uint32_t w = word[i];
-    uint32_t d;
-    if (w & 0x80000000u) {
-      const float* p = aos + (size_t)i * 8;
-      d = offset[key_of(G, p[0], p[1], p[2], G.s[0], G.s[1], G.s[2])] + (w & 0xffffu);
-    } else {
-      d = atomicAdd(&dest[w], 1u);
+  // SCAT_TU independent particles per thread: the kernel is bound by the latency of the chain word load -> shared
+  // counter (with return) -> store, so the loads of several iterations are put in flight together
+  constexpr int SCAT_TU = 4;
+  for (uint32_t ib = i0 + threadIdx.x; ib < i1; ib += SCAT_TU * blockDim.x) {
+    uint32_t w[SCAT_TU];
+#pragma unroll
+    for (int j = 0; j < SCAT_TU; ++j) {
+      const uint32_t i = ib + j * blockDim.x;
+      w[j] = (i < i1) ? word[i] : 0u;
     }
-    perm[d] = i;
+#pragma unroll
+    for (int j = 0; j < SCAT_TU; ++j) {
+      const uint32_t i = ib + j * blockDim.x;
+      if (i >= i1) break;
+      uint32_t d;
+      if (w[j] & 0x80000000u) {
+        const float* p = aos + (size_t)i * 8;
+        const uint32_t k = key_of(G, p[0], p[1], p[2], G.s[0], G.s[1], G.s[2]);
+        d = spread_key(offset, k, offset[k] + (w[j] & 0xffffu), spread);
+      } else {
+        d = atomicAdd(&dest[w[j]], 1u);
+        if (spread) { const uint32_t g0 = dest[tcells + w[j]]; d = spread_slot(d, g0, g0 + dest[2 * tcells + w[j]]); }
+      }
+      perm[d] = i;
+    }
   }
 }
 
 // one thread per cell: the particles of segment [offset[k], offset[k+1]) ranked by id
+// (spread: the cell's particles sit at spread_slot() of the segment's positions)
 __global__ void __launch_bounds__(256) k_rank_cells(size_t nkeys, const uint32_t* __restrict__ offset, const uint32_t* __restrict__ id,
-                                                    uint32_t* __restrict__ perm) {
+                                                    uint32_t* __restrict__ perm, int spread) {
   const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= nkeys) return;
   const uint32_t b = offset[k], e = offset[k + 1];
+  if (b == e) return;
+  uint32_t g0 = 0, g1 = 0;               // R = 0: spread_slot is the identity
+  if (spread) { g0 = offset[k & ~(size_t)31]; g1 = offset[(k & ~(size_t)31) + 32]; }
   for (uint32_t j = b; j < e; ++j) {
-    const uint32_t me = id[j];
+    const uint32_t pj = spread_slot(j, g0, g1), me = id[pj];
     uint32_t r = 0;
-    for (uint32_t m = b; m < e; ++m) r += (id[m] < me) ? 1u : 0u;
-    perm[b + r] = j;
+    for (uint32_t m = b; m < e; ++m) r += (id[spread_slot(m, g0, g1)] < me) ? 1u : 0u;
+    perm[b + r] = pj;
   }
 }
 struct Arrays8 { void* p[8]; };
@@ -300,6 +341,8 @@ int do_reorder(mpc_ctx* c, bool defer_gather, bool canonical) {
   const int stride = c->G.sw * 2;
   const bool ranked = c->ranked_keys && defer_gather && !canonical;
   const int bvs = c->G.bs[0] + c->G.bs[1] + c->G.bs[2];
+  // lane-spread order inside every group of 32 keys: hot path only, bricks of whole groups (spread_slot)
+  const int spread = (!canonical && bvs >= 5 && !(c->debug & MPC_DEBUG_NO_LANE_SPREAD)) ? 1 : 0;
   if (ranked) {   // the brick ranges of the old order, before the scan overwrites the offsets
     FamilyTimer ft(c, F_SCAN);
     k_save_chunks<<<nblk((size_t)c->nbricks + 1, 256), 256, 0, c->stream>>>(c->offset, bvs, c->nbricks, (uint32_t)n, c->chunk0);
@@ -317,9 +360,13 @@ int do_reorder(mpc_ctx* c, bool defer_gather, bool canonical) {
   if (ranked) {
     FamilyTimer ft(c, F_SCATTER);
     const float* aos = reinterpret_cast<const float*>(c->A[0] < c->Bf[0] ? c->slot_id : c->Bf[0]);
-    const size_t sh = c->tile_bytes / TILE_W;     // one uint32 per tile cell
-    if (c->fast_brick) k_scatter_tile<BSfast><<<c->nbricks, 512, sh, c->stream>>>(c->G, (uint32_t)n, c->key, c->chunk0, c->nbricks, c->offset, c->tbase, aos, c->perm);
-    else k_scatter_tile<BSgeneric><<<c->nbricks, 512, sh, c->stream>>>(c->G, (uint32_t)n, c->key, c->chunk0, c->nbricks, c->offset, c->tbase, aos, c->perm);
+    const size_t sh = (c->tile_bytes / TILE_W) * (spread ? 3 : 1);     // one uint32 per tile cell (three with the lane spread)
+    if (sh > 48 * 1024) {
+      CU(cudaFuncSetAttribute(k_scatter_tile<BSfast>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
+      CU(cudaFuncSetAttribute(k_scatter_tile<BSgeneric>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
+    }
+    if (c->fast_brick) k_scatter_tile<BSfast><<<c->nbricks, 512, sh, c->stream>>>(c->G, (uint32_t)n, c->key, c->chunk0, c->nbricks, c->offset, c->tbase, aos, c->perm, spread);
+    else k_scatter_tile<BSgeneric><<<c->nbricks, 512, sh, c->stream>>>(c->G, (uint32_t)n, c->key, c->chunk0, c->nbricks, c->offset, c->tbase, aos, c->perm, spread);
     LAUNCH_CHECK("k_scatter_tile");
   } else {
     { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->cursor, 0, nk * 4, c->stream)); }
@@ -335,12 +382,13 @@ int do_reorder(mpc_ctx* c, bool defer_gather, bool canonical) {
       LAUNCH_CHECK("k_rank");
     } else {
       FamilyTimer ft(c, F_SCATTER);
-      k_scatter_src<<<nblk(n, 256 * SCAT_U), 256, 0, c->stream>>>(n, c->key, c->offset, c->cursor, c->perm);
+      k_scatter_src<<<nblk(n, 256 * SCAT_U), 256, 0, c->stream>>>(n, c->key, c->offset, c->cursor, c->perm, spread);
       LAUNCH_CHECK("k_scatter_src");
     }
   }
   c->have_order = true;
   c->order_canonical = canonical;
+  c->order_spread = spread != 0;
   if (defer_gather) { c->gather_pending = true; return MPC_OK; }
   return apply_perm(c);
 }
@@ -351,10 +399,10 @@ int canonicalise(mpc_ctx* c) {
   if (!c->have_order || c->order_canonical || c->n == 0) return MPC_OK;
   {
     FamilyTimer ft(c, F_RANK);
-    k_rank_cells<<<nblk(c->G.nkeys, 256), 256, 0, c->stream>>>(c->G.nkeys, c->offset, c->A[6], c->perm);
+    k_rank_cells<<<nblk(c->G.nkeys, 256), 256, 0, c->stream>>>(c->G.nkeys, c->offset, c->A[6], c->perm, c->order_spread ? 1 : 0);
     LAUNCH_CHECK("k_rank_cells");
   }
   const int rc = apply_perm(c);
-  if (rc == MPC_OK) c->order_canonical = true;
+  if (rc == MPC_OK) { c->order_canonical = true; c->order_spread = false; }
   return rc;
 }

@@ -338,7 +338,8 @@ def test_reorder_code_paths_agree(kw):
     # records, slots from the staging sweep's arrival ranks (no atomics in the scatter), particles grouped by key only,
     # canonical (key, id) order restored when the state is read; (b) separate gather kernel; (c) eager canonical order
     # (scatter + rank by id + gather), the path the lock-step parity tests exercise with mpc_step(1); (d) cursor
-    # atomics in the scatter; (e) the last collision of a call applied at once instead of staying pending.
+    # atomics in the scatter; (e) the last collision of a call applied at once instead of staying pending; (f) plain cell
+    # order in memory between reads instead of the lane-spread order of every group of 32 cells.
     # State AND memory order must be identical.
     from paper_2406_15236_b200 import binding as B
     cells, nbar = (32, 16, 16), 10
@@ -346,7 +347,8 @@ def test_reorder_code_paths_agree(kw):
     n = int(np.prod(cells)) * nbar - 13          # ragged tail: not a multiple of 32
     st = uniform_maxwell(box, n, 77)
     res = []
-    for flags in (0, B.DEBUG_NO_FUSE_GATHER, B.DEBUG_EAGER_CANONICAL, B.DEBUG_ATOMIC_SCATTER, B.DEBUG_EAGER_COLLIDE):
+    for flags in (0, B.DEBUG_NO_FUSE_GATHER, B.DEBUG_EAGER_CANONICAL, B.DEBUG_ATOMIC_SCATTER, B.DEBUG_EAGER_COLLIDE, B.DEBUG_NO_LANE_SPREAD,
+                  B.DEBUG_NO_LANE_SPREAD | B.DEBUG_ATOMIC_SCATTER, B.DEBUG_NO_FUSE_GATHER | B.DEBUG_ATOMIC_SCATTER):
         g = MPC(box, cells, nbar, 23, n_max=n, **kw)
         g.set_debug(flags)
         gpu_set(g, st)
