@@ -81,16 +81,20 @@ int steps_srd(mpc_ctx* c, int nsteps) {
     const bool rebin = (c->t % (uint32_t)c->p.rebin_every) == 0u;
     if (!c->sums_clean) { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * G.sw * 8, c->stream)); }
     c->sums_clean = false;
-    // reorder folded into this sweep (writes the 32-byte staging records) and the next one (reads them through
-    // the permutation): needs a next step in this call, the second particle copy, and rebin_every >= 2
-    const bool stage = rebin && !c->compact && !(c->debug & (MPC_DEBUG_NO_FUSE_GATHER | MPC_DEBUG_EAGER_CANONICAL)) && k + 1 < nsteps &&
-                       c->p.rebin_every >= 2;
+    // reorder folded into this sweep (rank pass) and the next two (scatter into the new order through 32-byte staging
+    // records, read back): needs two more steps in this call, the order of the last reorder, the second particle copy,
+    // and rebin_every >= 3
+    const bool stage = rebin && c->reorder_stage == 0 && c->have_order && c->tbase && !c->compact &&
+                       !(c->debug & (MPC_DEBUG_NO_FUSE_GATHER | MPC_DEBUG_EAGER_CANONICAL | MPC_DEBUG_ATOMIC_SCATTER)) && k + 2 < nsteps &&
+                       c->p.rebin_every >= 3;
     if (n) {
       {
-        FamilyTimer ft(c, (c->gather_pending || stage) ? F_SWEEPG : F_SWEEP);
-        const int io = c->gather_pending ? IO_GATHER : (stage ? IO_AOS_OUT : IO_PLAIN);
-        const int rc = launch_sweep(c, c->collide_pending, rebin && !c->gather_pending, io, sp);
+        const int io = c->reorder_stage == 1 ? IO_SCATTER : c->reorder_stage == 2 ? IO_AOS_IN : (stage ? IO_RANK : IO_PLAIN);
+        FamilyTimer ft(c, io != IO_PLAIN ? F_SWEEPG : F_SWEEP);
+        const int rc = launch_sweep(c, c->collide_pending, rebin && !stage, io, sp);
         if (rc) return rc;
+        if (io == IO_SCATTER) c->reorder_stage = 2;
+        else if (io == IO_AOS_IN) c->reorder_stage = 0;
       }
       // all but the last step of the call: k_cell clears the sums it has read (the last step's stay for
       // mpc_observables / mpc_get_cells)
@@ -130,7 +134,7 @@ int set_state_impl(mpc_ctx* c, unsigned long long n, const float* const src[6], 
     else { const int rc = launch_iota(c); if (rc) return rc; }    // ids 0..n_max-1
   }
   CU(cudaMemsetAsync(c->nrange, 0, 8, c->stream));
-  c->n = n; c->t = step; c->have_state = true; c->have_cells = false; c->have_order = false; c->gather_pending = false;
+  c->n = n; c->t = step; c->have_state = true; c->have_cells = false; c->have_order = false; c->reorder_stage = 0;
   c->order_canonical = true; c->order_spread = false; c->collide_pending = false;
   return MPC_OK;
 }
@@ -291,8 +295,8 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
   c->tbase = staged ? (uint32_t*)(c->ws + l.off_tbase) : nullptr;
   c->chunk0 = staged ? (uint32_t*)(c->ws + l.off_chunk0) : nullptr;
   CU(cudaMemsetAsync(c->nrange, 0, 8, c->stream));
-  c->bound = true; c->have_state = false; c->have_cells = false; c->have_order = false; c->sums_clean = false; c->gather_pending = false;
-  c->collide_pending = false; c->ranked_keys = false; c->order_spread = false; c->n = 0;
+  c->bound = true; c->have_state = false; c->have_cells = false; c->have_order = false; c->sums_clean = false; c->reorder_stage = 0;
+  c->collide_pending = false; c->order_spread = false; c->n = 0;
   if (c->tile_bytes > 48 * 1024) {
     const cudaError_t e = sweep_set_attributes(c->tile_bytes);
     if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(k_sweep, MaxDynamicSharedMemorySize)");
@@ -303,7 +307,7 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
 int mpc_set_debug(mpc_ctx* c, unsigned flags) {
   if (!c) return MPC_EINVAL;
   if (flags & ~(MPC_DEBUG_NO_FUSE_GATHER | MPC_DEBUG_EAGER_CANONICAL | MPC_DEBUG_ATOMIC_SCATTER | MPC_DEBUG_EAGER_COLLIDE | MPC_DEBUG_NO_LANE_SPREAD)) return fail(c, MPC_EINVAL, "unknown debug flag");
-  if (c->gather_pending) return fail(c, MPC_ESTATE, "internal: gather pending");   // cannot happen between API calls
+  if (c->reorder_stage) return fail(c, MPC_ESTATE, "internal: reorder in flight");   // cannot happen between API calls
   c->debug = flags;
   return MPC_OK;
 }

@@ -262,6 +262,19 @@ typedef BrickShape<4, 4, 3> BSfast;   // {16,16,8}
 
 // floor index of a coordinate, not yet folded into [0, m)
 __device__ __forceinline__ int cell_raw(const Geo& G, float r, float s) { return __float2int_rd((r + s) * G.inv_a); }
+// Lane-spread order inside a group of 32 cells (hot path). The sweep's shared-memory atomics serialise on
+// lanes of a warp that hit the same cell; in plain cell order a warp's 32 consecutive particles sit in ~3 cells. The
+// hot-path reorder therefore stores the n_g particles of every aligned group of 32 keys (one contiguous range [g0, g1)
+// of the counting sort, always inside one brick) TRANSPOSED: with R = n_g / 32, sorted position p < 32 R goes to row
+// p % R, column p / R of an R x 32 matrix, so neighbouring lanes hold particles R ~ <N_c> sorted positions apart:
+// (mostly) different cells. The tail p >= 32 R stays where it is. The brick ranges the sweep works on are unchanged; the
+// order inside a cell does not enter the physics (integer sums); canonicalise() reads the cells back through the same map.
+__device__ __forceinline__ uint32_t spread_slot(uint32_t slot, uint32_t g0, uint32_t g1) {
+  const uint32_t R = (g1 - g0) >> 5, p = slot - g0;
+  if (p >= (R << 5)) return slot;
+  const uint32_t col = p / R, row = p - col * R;
+  return g0 + (row << 5) + col;
+}
 // fold an index known to lie in [-m, 2m) into [0, m)
 __device__ __forceinline__ int fold(int k, int m) {
   k += (k < 0) ? m : 0;
@@ -283,13 +296,13 @@ struct mpc_ctx {
   unsigned long long seed;
   uint32_t t;
   size_t n, n_max;
-  bool bound, have_state, have_cells, have_order, compact, sticky, fast_brick, sums_clean, gather_pending, order_canonical, three_ctas;
+  bool bound, have_state, have_cells, have_order, compact, sticky, fast_brick, sums_clean, order_canonical, three_ctas;
   // the collision of the last step of an mpc_step call stays pending: the next call's first sweep
   // applies it; every call that reads particle velocities applies it first (flush_collide)
   bool collide_pending;
   bool pow2_cells;      // no walls and every m[d] a power of two: the sweep folds indices with a mask
   bool order_spread;    // the particles of every group of 32 keys are stored lane-spread (reorder.cu, spread_slot)
-  bool ranked_keys;     // the last staging sweep wrote (tile cell, arrival rank) words into key[] instead of keys
+  int reorder_stage;    // folded reorder: 0 none in flight, 1 the next sweep scatters into the new order, 2 the next sweep reads the staged records
   float le_dprev;       // Lees-Edwards displacement of the step whose collision is pending
   unsigned debug;       // MPC_DEBUG_* flags
   int device;           // CUDA device of the workspace
@@ -360,7 +373,7 @@ inline unsigned nblk(size_t n, int t) { return (unsigned)((n + t - 1) / t); }
 
 // ---- entry points of the translation units ---------------------------------------------------------
 // sweep.cu
-enum { IO_PLAIN = 0, IO_AOS_OUT = 1, IO_GATHER = 2 };
+enum { IO_PLAIN = 0, IO_RANK = 1, IO_SCATTER = 2, IO_AOS_IN = 3 };   // sweep.cu: the reorder folded into three sweeps
 int launch_sweep(mpc_ctx* c, bool collide, bool wkey, int io, const float sp[3]);
 cudaError_t sweep_set_attributes(size_t tile_bytes);
 int launch_collide_pos(mpc_ctx* c);

@@ -86,20 +86,7 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const uint32_t* __restric
 }
 
 // ---- scatter --------------------------------------------------------------------------------------
-// ---- lane-spread order inside a group of 32 cells (hot path) ---------------------------
-// The sweep's shared-memory atomics serialise on lanes of a warp that hit the same cell; in plain cell order a warp's
-// 32 consecutive particles sit in ~3 cells. The hot-path reorder therefore stores the n_g particles of every aligned
-// group of 32 keys (one contiguous range [g0, g1) of the counting sort, always inside one brick) TRANSPOSED: with
-// R = n_g / 32, sorted position p < 32 R goes to row p % R, column p / R of an R x 32 matrix, so neighbouring lanes
-// hold particles R ~ <N_c> sorted positions apart: (mostly) different cells. The tail p >= 32 R stays where it is.
-// The brick ranges the sweep works on are unchanged; the order inside a cell does not enter the physics (integer sums);
-// canonicalise() reads the cells back through the same map.
-__device__ __forceinline__ uint32_t spread_slot(uint32_t slot, uint32_t g0, uint32_t g1) {
-  const uint32_t R = (g1 - g0) >> 5, p = slot - g0;
-  if (p >= (R << 5)) return slot;
-  const uint32_t col = p / R, row = p - col * R;
-  return g0 + (row << 5) + col;
-}
+// lane-spread order inside a group of 32 cells: spread_slot (internal.cuh)
 __device__ __forceinline__ uint32_t spread_key(const uint32_t* __restrict__ offset, uint32_t k, uint32_t slot, int spread) {
   if (!spread) return slot;
   const uint32_t kg = k & ~31u;
@@ -188,73 +175,14 @@ __global__ void __launch_bounds__(256) k_scatter_src(size_t n, const uint32_t* _
   }
 }
 
-// Hot-path variant when the previous order is known: the staging sweep (k_sweep<.., IO_AOS_OUT>) has written every
-// particle's tile cell, and its tile flush has given every CTA the first slot of its particles inside each cell's
-// segment (the value the flush's global atomic returned). One CTA per brick then hands out the slots with
-// shared-memory counters: slot = offset[key] + first slot of the CTA + arrival rank in (CTA, cell). No global atomics,
-// no dependent global chain. word = tile cell, or bit 31 | slot-in-segment for the few particles that left their
-// brick's tile (their key is recomputed from the staged position).
+// brick ranges of the old order, saved before the scan of a folded reorder overwrites the offsets: the scatter pass
+// (k_sweep<.., IO_SCATTER>) still walks the old order
 __global__ void __launch_bounds__(256) k_save_chunks(const uint32_t* __restrict__ offset, int bvol_shift, uint32_t nbricks,
                                                      uint32_t n, uint32_t* __restrict__ chunk0) {
   const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b < nbricks) chunk0[b] = offset[(size_t)b << bvol_shift];
   if (b == nbricks) chunk0[b] = n;
 }
-template <class BS>
-__global__ void __launch_bounds__(512) k_scatter_tile(Geo G, uint32_t n, const uint32_t* __restrict__ word, const uint32_t* __restrict__ chunk0,
-                                                      uint32_t nbricks, const uint32_t* __restrict__ offset, const uint32_t* __restrict__ tbase,
-                                                      const float* __restrict__ aos, uint32_t* __restrict__ perm, int spread) {
-  extern __shared__ uint32_t dest[];     // per tile cell: next free slot; then (spread) first slot and size of the cell's group of 32 keys
-  const int T0 = (1 << BS::s0(G)) + 2 * HALO, T1 = (1 << BS::s1(G)) + 2 * HALO, T2 = (1 << BS::s2(G)) + 2 * HALO;
-  const int tcells = T0 * T1 * T2;
-  const uint32_t b = blockIdx.x;
-  const int m0 = G.m[0], m1 = G.m[1], m2 = G.m[2];
-  int ox, oy, oz;
-  {
-    const uint32_t bx = b % (uint32_t)G.mb[0], q = b / (uint32_t)G.mb[0];
-    const uint32_t by = q % (uint32_t)G.mb[1], bz = q / (uint32_t)G.mb[1];
-    ox = (int)(bx << BS::s0(G)) - HALO; oy = (int)(by << BS::s1(G)) - HALO; oz = (int)(bz << BS::s2(G)) - HALO;
-  }
-  uint32_t i0 = (chunk0[b] + 31u) & ~31u, i1 = chunk0[b + 1];
-  if (b + 1 != nbricks) i1 = min((i1 + 31u) & ~31u, n);      // the ranges of chunk_range() in sweep.cu
-  if (i0 >= i1) return;
-  for (int c = threadIdx.x; c < tcells; c += blockDim.x) {
-    const int l0 = c % T0, q = c / T0, l1 = q % T1, l2 = q / T1;
-    // wall axes do not wrap: tile cells beyond the last layer hold no particles, their slot is never read
-    const int kx = fold(ox + l0, m0), ky = fold(oy + l1, m1), kz = fold(oz + l2, m2);
-    const uint32_t k = BS::key(G, kx, ky, kz);
-    dest[c] = offset[k] + tbase[(size_t)b * tcells + c];
-    if (spread) { const uint32_t g0 = offset[k & ~31u]; dest[tcells + c] = g0; dest[2 * tcells + c] = offset[(k & ~31u) + 32u] - g0; }
-  }
-  __syncthreads();
-  // SCAT_TU independent particles per thread: the kernel is bound by the latency of the chain word load -> shared
-  // counter (with return) -> store, so the loads of several iterations are put in flight together
-  constexpr int SCAT_TU = 4;
-  for (uint32_t ib = i0 + threadIdx.x; ib < i1; ib += SCAT_TU * blockDim.x) {
-    uint32_t w[SCAT_TU];
-#pragma unroll
-    for (int j = 0; j < SCAT_TU; ++j) {
-      const uint32_t i = ib + j * blockDim.x;
-      w[j] = (i < i1) ? word[i] : 0u;
-    }
-#pragma unroll
-    for (int j = 0; j < SCAT_TU; ++j) {
-      const uint32_t i = ib + j * blockDim.x;
-      if (i >= i1) break;
-      uint32_t d;
-      if (w[j] & 0x80000000u) {
-        const float* p = aos + (size_t)i * 8;
-        const uint32_t k = key_of(G, p[0], p[1], p[2], G.s[0], G.s[1], G.s[2]);
-        d = spread_key(offset, k, offset[k] + (w[j] & 0xffffu), spread);
-      } else {
-        d = atomicAdd(&dest[w[j]], 1u);
-        if (spread) { const uint32_t g0 = dest[tcells + w[j]]; d = spread_slot(d, g0, g0 + dest[2 * tcells + w[j]]); }
-      }
-      perm[d] = i;
-    }
-  }
-}
-
 // one thread per cell: the particles of segment [offset[k], offset[k+1]) ranked by id
 // (spread: the cell's particles sit at spread_slot() of the segment's positions)
 __global__ void __launch_bounds__(256) k_rank_cells(size_t nkeys, const uint32_t* __restrict__ offset, const uint32_t* __restrict__ id,
@@ -331,19 +259,19 @@ int apply_perm(mpc_ctx* c) {
 
 }  // namespace
 
-// counting-sort reorder by (key, id); counts = low word of word 0 of the sums; c->key holds the keys (or, after a
-// ranked staging sweep, the rank words)
-// defer_gather: leave the permutation in c->perm for the next sweep to apply (IO_GATHER)
+// counting-sort reorder by (key, id); counts = low word of word 0 of the sums
+// folded: the sweep of this step was the rank pass (IO_RANK): only the scan is done here, the next two sweeps move the
+//         particles (IO_SCATTER, IO_AOS_IN); otherwise c->key holds the keys and scatter + gather kernels run now
 // canonical: rank the particles of a cell by id now (needed by MPC-AT); otherwise group by key only
-int do_reorder(mpc_ctx* c, bool defer_gather, bool canonical) {
+int do_reorder(mpc_ctx* c, bool folded, bool canonical) {
   const size_t n = c->n, nk = c->G.nkeys, nb = (nk + SCAN_TILE - 1) / SCAN_TILE;
   const uint32_t* cnt = reinterpret_cast<const uint32_t*>(c->sums);
   const int stride = c->G.sw * 2;
-  const bool ranked = c->ranked_keys && defer_gather && !canonical;
   const int bvs = c->G.bs[0] + c->G.bs[1] + c->G.bs[2];
+  if (folded && canonical) return fail(c, MPC_ESTATE, "internal: folded reorder cannot rank by id");
   // lane-spread order inside every group of 32 keys: hot path only, bricks of whole groups (spread_slot)
   const int spread = (!canonical && bvs >= 5 && !(c->debug & MPC_DEBUG_NO_LANE_SPREAD)) ? 1 : 0;
-  if (ranked) {   // the brick ranges of the old order, before the scan overwrites the offsets
+  if (folded) {   // the brick ranges of the old order, before the scan overwrites the offsets
     FamilyTimer ft(c, F_SCAN);
     k_save_chunks<<<nblk((size_t)c->nbricks + 1, 256), 256, 0, c->stream>>>(c->offset, bvs, c->nbricks, (uint32_t)n, c->chunk0);
     LAUNCH_CHECK("k_save_chunks");
@@ -357,18 +285,7 @@ int do_reorder(mpc_ctx* c, bool defer_gather, bool canonical) {
     k_scan_apply<<<(unsigned)nb, SCAN_T, 0, c->stream>>>(cnt, stride, nk, c->bsum, c->offset);
     LAUNCH_CHECK("k_scan_apply");
   }
-  if (ranked) {
-    FamilyTimer ft(c, F_SCATTER);
-    const float* aos = reinterpret_cast<const float*>(c->A[0] < c->Bf[0] ? c->slot_id : c->Bf[0]);
-    const size_t sh = (c->tile_bytes / TILE_W) * (spread ? 3 : 1);     // one uint32 per tile cell (three with the lane spread)
-    if (sh > 48 * 1024) {
-      CU(cudaFuncSetAttribute(k_scatter_tile<BSfast>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
-      CU(cudaFuncSetAttribute(k_scatter_tile<BSgeneric>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
-    }
-    if (c->fast_brick) k_scatter_tile<BSfast><<<c->nbricks, 512, sh, c->stream>>>(c->G, (uint32_t)n, c->key, c->chunk0, c->nbricks, c->offset, c->tbase, aos, c->perm, spread);
-    else k_scatter_tile<BSgeneric><<<c->nbricks, 512, sh, c->stream>>>(c->G, (uint32_t)n, c->key, c->chunk0, c->nbricks, c->offset, c->tbase, aos, c->perm, spread);
-    LAUNCH_CHECK("k_scatter_tile");
-  } else {
+  if (!folded) {
     { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->cursor, 0, nk * 4, c->stream)); }
     if (canonical) {
       uint2* slot2 = reinterpret_cast<uint2*>(c->compact ? c->slot_id : c->Bf[0]);
@@ -389,7 +306,7 @@ int do_reorder(mpc_ctx* c, bool defer_gather, bool canonical) {
   c->have_order = true;
   c->order_canonical = canonical;
   c->order_spread = spread != 0;
-  if (defer_gather) { c->gather_pending = true; return MPC_OK; }
+  if (folded) { c->reorder_stage = 1; return MPC_OK; }
   return apply_perm(c);
 }
 

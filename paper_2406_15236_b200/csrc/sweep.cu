@@ -5,19 +5,26 @@
 
 namespace mpc {
 
-// Reorder folded into two consecutive sweeps (IO = 1 on the reorder step, IO = 2 on the step after it):
-//   IO_AOS_OUT  the pass writes every particle as ONE 32-byte record {r, v, id, 0} into a staging buffer
-//               instead of updating the SoA arrays in place;
-//   IO_GATHER   particle i of the new order is read with one 256-bit load from staging[perm[i]] (a whole
-//               sector, every byte used) and written to the SoA arrays at i.
-// A gather of the SoA arrays themselves costs ~4.5 sectors of L2 traffic per useful one (measured).
+// Reorder folded into three consecutive sweeps, IO = 1, 2, 3 on the reorder step t and the two after it:
+//   IO_RANK     step t: the pass works in place as always and also writes one word per particle: its arrival rank
+//               inside (this CTA, its cell), which the tile's count atomic returns (or bit 31 | its slot in the cell's
+//               segment, from the returning global atomic, for the few particles outside the tile); the tile flush
+//               uses the returning form of the count atomic: what it returns is the first slot of this CTA's particles
+//               inside the cell's segment (tbase). A scan of the counts follows (reorder.cu).
+//   IO_SCATTER  step t+1: still in the old order (coalesced SoA reads); the cell of step t is recomputed for the
+//               collision anyway, so slot = offset[cell] + tbase[CTA, cell] + rank is known, and the particle
+//               (after collision and MOVE) is written as ONE 32-byte record {r, v, id, 0} at its slot of the new
+//               order in the staging buffer (a whole sector per store);
+//   IO_AOS_IN   step t+2: in the new order; records read back with coalesced 256-bit loads, SoA arrays written at i.
+// No permutation array, no scatter kernel, no random reads: 32 bytes per particle more than three plain sweeps.
+// (A gather of the SoA arrays themselves costs ~4.5 sectors of L2 traffic per useful one.)
 struct SweepIO {
-  const float* aos_in;      // IO_GATHER: staging records in the old order
-  float* aos_out;           // IO_AOS_OUT
-  const uint32_t* perm;     // IO_GATHER
-  uint32_t* id;             // IO_AOS_OUT: read at i; IO_GATHER: written at i
-  uint32_t* tbase;          // IO_AOS_OUT, ranked: first slot of this CTA's particles inside every tile cell's segment
-  int ranked;               // IO_AOS_OUT: key_out receives the tile cell (or bit 31 | slot, outside the tile) instead of the key
+  float* aos;               // IO_SCATTER: written at the slot; IO_AOS_IN: read at i
+  uint32_t* id;             // IO_SCATTER: read at i; IO_AOS_IN: written at i
+  uint32_t* tbase;          // IO_RANK: written by the flush; IO_SCATTER: read: first slot of this CTA's particles inside every tile cell's segment
+  const uint32_t* offset;   // IO_SCATTER: cell offsets of the new order
+  int spread;               // IO_SCATTER: lane-spread order inside every group of 32 cells (spread_slot)
+  int chunk_shift;          // chunk[b << chunk_shift] = first particle of brick b
   float le_dprev;           // Lees-Edwards displacement of the previous step (for its collision)
 };
 __device__ __forceinline__ void ld256(const float* p, float (&a)[8]) {
@@ -63,6 +70,7 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
         float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, uint32_t* __restrict__ key_out,
         const uint32_t* __restrict__ chunk, uint32_t nbricks, const float* __restrict__ rec, u64* __restrict__ sums,
         SweepIO io) {
+  static_assert(IO != IO_SCATTER || COLLIDE, "the scatter pass sorts by the cell of the collision it applies");
   extern __shared__ int tile[];
   const int T0 = (1 << BS::s0(G)) + 2 * HALO, T1 = (1 << BS::s1(G)) + 2 * HALO, T2 = (1 << BS::s2(G)) + 2 * HALO;
   const int tcells = T0 * T1 * T2;
@@ -76,8 +84,8 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
     ox = (int)(bx << BS::s0(G)) - HALO; oy = (int)(by << BS::s1(G)) - HALO; oz = (int)(bz << BS::s2(G)) - HALO;
   }
   uint32_t i0, i1;
-  chunk_range(chunk, b, nbricks, n, BS::s0(G) + BS::s1(G) + BS::s2(G), i0, i1);
-  const bool ranked = IO == IO_AOS_OUT && io.ranked != 0;
+  chunk_range(chunk, b, nbricks, n, io.chunk_shift, i0, i1);
+  constexpr bool ranked = IO == IO_RANK;
   // index offsets added before the floor index is folded: +1 on a wall axis (layer 0 lies in the wall)
   const int w0 = (WALL && G.bc[0]) ? 1 : 0, w1 = (WALL && G.bc[1]) ? 1 : 0, w2 = (WALL && G.bc[2]) ? 1 : 0;
   unsigned nbad = 0;
@@ -85,42 +93,36 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
   // software pipeline: the loads of the next particle are in flight while this one is processed
   uint32_t i = i0 + threadIdx.x;
   float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f, p4 = 0.f, p5 = 0.f;
-  // IO_GATHER: source indices of the particles 1, 2 and 3 iterations ahead (the first feeds the register
-  // prefetch, the second an L2 prefetch of its record, the third is in flight); pid = id of the particle in flight
+  // pid = id of the particle in flight (IO_SCATTER, IO_AOS_IN), pw = its rank word (IO_SCATTER)
   float pid = 0.f;
-  uint32_t jn = 0, jn2 = 0, jn3 = 0;
-  if (IO == IO_GATHER) {
+  uint32_t pw = 0;
+  if (IO == IO_AOS_IN) {
     if (i < i1) {
       float q[8];
-      ld256(io.aos_in + (size_t)io.perm[i] * 8, q);
+      ld256(io.aos + (size_t)i * 8, q);
       p0 = q[0]; p1 = q[1]; p2 = q[2]; p3 = q[3]; p4 = q[4]; p5 = q[5]; pid = q[6];
     }
-    if (i + T < i1) jn = io.perm[i + T];
-    if (i + 2 * T < i1) jn2 = io.perm[i + 2 * T];
-    if (i + 3 * T < i1) jn3 = io.perm[i + 3 * T];
   } else if (i < i1) {
     p0 = x[i]; p1 = y[i]; p2 = z[i]; p3 = vx[i]; p4 = vy[i]; p5 = vz[i];
-    if (IO == IO_AOS_OUT) pid = __uint_as_float(io.id[i]);
+    if (IO == IO_SCATTER) { pid = __uint_as_float(io.id[i]); pw = key_out[i]; }
   }
   for (; i < i1; i += T) {
     float r[3] = {p0, p1, p2}, v[3] = {p3, p4, p5};
     const float idbits = pid;
+    const uint32_t w = pw;
     const uint32_t inext = i + T;
-    if (IO == IO_GATHER) {
+    if (IO == IO_AOS_IN) {
       io.id[i] = __float_as_uint(idbits);
       if (inext < i1) {
         float q[8];
-        ld256(io.aos_in + (size_t)jn * 8, q);
+        ld256(io.aos + (size_t)inext * 8, q);
         p0 = q[0]; p1 = q[1]; p2 = q[2]; p3 = q[3]; p4 = q[4]; p5 = q[5]; pid = q[6];
-        jn = jn2; jn2 = jn3;
-        if (i + 2 * T < i1) asm volatile("prefetch.global.L2 [%0];" ::"l"(io.aos_in + (size_t)jn * 8));
-        if (i + 4 * T < i1) jn3 = io.perm[i + 4 * T];
       }
     } else if (inext < i1) {
       p0 = x[inext]; p1 = y[inext]; p2 = z[inext]; p3 = vx[inext]; p4 = vy[inext]; p5 = vz[inext];
-      if (IO == IO_AOS_OUT) pid = __uint_as_float(io.id[inext]);
+      if (IO == IO_SCATTER) { pid = __uint_as_float(io.id[inext]); pw = key_out[inext]; }
     }
-    if (IO != IO_GATHER && threadIdx.x == 0) {
+    if (threadIdx.x == 0) {
       // pull the lines of a later iteration into L2: the register prefetch above then pays L2, not DRAM, latency. ONE bulk
       // prefetch per array and CTA iteration (cp.async.bulk.prefetch.L2): a per-thread prefetch.global.L2 costs every warp
       // six more requests in the L1TEX pipe that bounds this kernel (sweep 15.0 -> 14.3 ms at config 5; none at all: 16.6)
@@ -128,15 +130,24 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       if (ifar < i1) {
         const uint32_t bytes = (min((uint32_t)T, i1 - ifar) * 4u) & ~15u;
         if (bytes) {
-          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(x + ifar), "r"(bytes));
-          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(y + ifar), "r"(bytes));
-          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(z + ifar), "r"(bytes));
-          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(vx + ifar), "r"(bytes));
-          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(vy + ifar), "r"(bytes));
-          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(vz + ifar), "r"(bytes));
+          if (IO == IO_AOS_IN) {
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(io.aos + (size_t)ifar * 8), "r"(bytes * 8u));
+          } else {
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(x + ifar), "r"(bytes));
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(y + ifar), "r"(bytes));
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(z + ifar), "r"(bytes));
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(vx + ifar), "r"(bytes));
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(vy + ifar), "r"(bytes));
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(vz + ifar), "r"(bytes));
+            if (IO == IO_SCATTER) {
+              asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(io.id + ifar), "r"(bytes));
+              asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(key_out + ifar), "r"(bytes));
+            }
+          }
         }
       }
     }
+    uint32_t slot = 0;   // IO_SCATTER: the particle's place in the new order
     if (COLLIDE) {   // ROTATE_VELOCITIES of the previous step; its key is recomputed from r and that step's shift
       float vsp = 0.0f;
       const float xp = SHEAR ? le_image(G, r[0], r[2], sp2, io.le_dprev, vsp) : r[0];
@@ -147,14 +158,23 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       const uint32_t kp = BS::key(G, kx, ky, kz);
       float4 r0, ax;
       load_rec(rec, kp, r0, ax);
+      if (IO == IO_SCATTER) {   // kp is the cell the reorder sorts by: slot = cell offset + first slot of this CTA + arrival rank
+        slot = io.offset[kp];
+        if (w & 0x80000000u) slot += w & 0xffffu;
+        else {
+          const int l0 = foldp<P2>(kx - ox, m0), l1 = foldp<P2>(ky - oy, m1), l2 = foldp<P2>(kz - oz, m2);
+          slot += io.tbase[(size_t)b * tcells + (l2 * T1 + l1) * T0 + l0] + w;
+        }
+        if (io.spread) { const uint32_t kg = kp & ~31u; slot = spread_slot(slot, io.offset[kg], io.offset[kg + 32u]); }
+      }
       if (SHEAR) v[0] += vsp;
       srd_apply(G, r0, ax, v);
       if (SHEAR) v[0] -= vsp;
     }
     stream_one<WALL, GRAV, SHEAR>(G, r, v);
-    if (IO == IO_AOS_OUT) {
+    if (IO == IO_SCATTER) {
       const float q[8] = {r[0], r[1], r[2], v[0], v[1], v[2], idbits, 0.f};
-      st256(io.aos_out + (size_t)i * 8, q);
+      st256(io.aos + (size_t)slot * 8, q);
     } else {
       x[i] = r[0]; y[i] = r[1]; z[i] = r[2];
       vx[i] = v[0]; vy[i] = v[1]; vz[i] = v[2];
@@ -170,19 +190,19 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
     // tile coordinates: one fold takes care of the periodic image of the cell and of the tile origin
     const int l0 = foldp<P2>(cx - ox, m0), l1 = foldp<P2>(cy - oy, m1), l2 = foldp<P2>(cz - oz, m2);
     const bool inside = (l0 < T0) & (l1 < T1) & (l2 < T2);
-    uint32_t word = 0;
+    uint32_t word = 0;   // IO_RANK: rank word of the particle
     if (inside) {
       const int tc = (l2 * T1 + l1) * T0 + l0;
       int* s = tile + tc * TILE_W;
       // word 0 = count (11 bits) | sum of the energies' high parts e >> 21 (21 bits); word 4 = sum of their low 21 bits:
       // neither can overflow below 2048 particles per (CTA, cell) with e < 2^28 (U19)
       const int w0add = 1 + (int)((e >> TILE_E_SHIFT) << TILE_N_BITS);
-      atomicAdd(s, w0add);
-      word = (uint32_t)tc;
+      if (ranked) word = (uint32_t)atomicAdd(s, w0add) & TILE_N_MASK;   // arrival rank inside (CTA, cell)
+      else atomicAdd(s, w0add);
       atomicAdd(s + 1, a0); atomicAdd(s + 2, a1); atomicAdd(s + 3, a2);
       atomicAdd((unsigned*)s + 4, e & ((1u << TILE_E_SHIFT) - 1u));
     }
-    if ((WKEY && !ranked) || !inside) {
+    if (WKEY || !inside) {
       const uint32_t kc = BS::key(G, foldp<P2>(cx, m0), foldp<P2>(cy, m1), foldp<P2>(cz, m2));
       if (!inside) {
         u64* s = sums + (size_t)kc * G.sw;
@@ -190,9 +210,9 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
         else atomicAdd(s, ((u64)e << 16) | 1ull);
         atomicAdd(s + 1, pack_ss(a0, a1)); atomicAdd(s + 2, pack_ss(a2, 0));
       }
-      if (WKEY && !ranked) key_out[i] = kc;
+      if (WKEY) key_out[i] = kc;
     }
-    if (WKEY && ranked) key_out[i] = word;
+    if (ranked) key_out[i] = word;
   }
   if (nbad) atomicAdd(G.nrange, (u64)nbad);
   __syncthreads();
@@ -264,8 +284,8 @@ inline float* aos_base(const mpc_ctx* c) {
   return reinterpret_cast<float*>(c->A[0] < c->Bf[0] ? c->slot_id : c->Bf[0]);
 }
 
-// the instantiations that exist: (COLLIDE, WKEY, IO) in { (*,0,PLAIN) at 384 or 512 threads, (*,1,PLAIN), (*,1,AOS_OUT),
-// (1,0,GATHER) } x (WALL, GRAV) x brick shape
+// the instantiations that exist: (COLLIDE, WKEY, IO) in { (*,0,PLAIN) at 384 or 512 threads, (*,1,PLAIN), (*,0,RANK),
+// (1,0,SCATTER), (1,0,AOS_IN) } x (WALL, GRAV) x brick shape
 template <bool COLLIDE, bool WKEY, class BS, int IO, int T>
 void* sweep_fn(bool wall, bool grav, bool p2, bool shear) {
   if (shear) return grav ? (void*)k_sweep<COLLIDE, false, true, WKEY, BS, IO, T, false, true> : (void*)k_sweep<COLLIDE, false, false, WKEY, BS, IO, T, false, true>;
@@ -277,8 +297,9 @@ void* sweep_fn(bool wall, bool grav, bool p2, bool shear) {
 }
 template <class BS>
 void* sweep_variant(bool collide, bool wkey, int io, bool three, bool wall, bool grav, bool p2, bool shear) {
-  if (io == IO_GATHER) return sweep_fn<true, false, BS, IO_GATHER, SWEEP_T>(wall, grav, p2, shear);
-  if (io == IO_AOS_OUT) return collide ? sweep_fn<true, true, BS, IO_AOS_OUT, SWEEP_T>(wall, grav, p2, shear) : sweep_fn<false, true, BS, IO_AOS_OUT, SWEEP_T>(wall, grav, p2, shear);
+  if (io == IO_AOS_IN) return sweep_fn<true, false, BS, IO_AOS_IN, SWEEP_T>(wall, grav, p2, shear);
+  if (io == IO_SCATTER) return sweep_fn<true, false, BS, IO_SCATTER, SWEEP_T>(wall, grav, p2, shear);
+  if (io == IO_RANK) return collide ? sweep_fn<true, false, BS, IO_RANK, SWEEP_T>(wall, grav, p2, shear) : sweep_fn<false, false, BS, IO_RANK, SWEEP_T>(wall, grav, p2, shear);
   if (wkey) return collide ? sweep_fn<true, true, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2, shear) : sweep_fn<false, true, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2, shear);
   if (three) return collide ? sweep_fn<true, false, BS, IO_PLAIN, SWEEP_T3>(wall, grav, p2, shear) : sweep_fn<false, false, BS, IO_PLAIN, SWEEP_T3>(wall, grav, p2, shear);
   return collide ? sweep_fn<true, false, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2, shear) : sweep_fn<false, false, BS, IO_PLAIN, SWEEP_T>(wall, grav, p2, shear);
@@ -293,24 +314,26 @@ void* sweep_variant_any(bool fast, bool collide, bool wkey, int io, bool three, 
 int launch_sweep(mpc_ctx* c, bool collide, bool wkey, int io, const float sp[3]) {
   Geo& G = c->G;
   float** F = reinterpret_cast<float**>(c->A);
+  if (io == IO_SCATTER && !collide) return fail(c, MPC_ESTATE, "internal: scatter pass without a pending collision");
   SweepIO sio;
-  sio.aos_in = sio.aos_out = aos_base(c);
-  sio.perm = c->perm; sio.id = c->A[6];
+  sio.aos = aos_base(c);
+  sio.id = c->A[6];
   sio.tbase = c->tbase;
-  sio.ranked = (io == IO_AOS_OUT && c->have_order && c->tbase && !(c->debug & MPC_DEBUG_ATOMIC_SCATTER)) ? 1 : 0;
-  c->ranked_keys = sio.ranked != 0;
-  const uint32_t* chunk = c->have_order ? c->offset : nullptr;
+  sio.offset = c->offset;
+  sio.spread = c->order_spread ? 1 : 0;
+  // the scatter pass still walks the old order: its brick ranges were saved before the scan overwrote the offsets
+  const uint32_t* chunk = (io == IO_SCATTER) ? c->chunk0 : (c->have_order ? c->offset : nullptr);
+  sio.chunk_shift = (io == IO_SCATTER) ? 0 : G.bs[0] + G.bs[1] + G.bs[2];
   const bool wall = G.wall >= 0, grav = (G.g[0] != 0.f || G.g[1] != 0.f || G.g[2] != 0.f);
   const bool three = io == IO_PLAIN && !wkey && c->three_ctas;
   sio.le_dprev = c->le_dprev;
-  void* fn = sweep_variant_any(c->fast_brick, collide, wkey, io, three, wall, grav, c->pow2_cells, G.shear != 0);
+  void* fn = sweep_variant_any(c->fast_brick, collide, wkey && io == IO_PLAIN, io, three, wall, grav, c->pow2_cells, G.shear != 0);
   float s0 = sp[0], s1 = sp[1], s2 = sp[2];
   uint32_t n = (uint32_t)c->n;
   void* args[] = {&G, &s0, &s1, &s2, &n, &F[0], &F[1], &F[2], &F[3], &F[4], &F[5], &c->key, &chunk, &c->nbricks, &c->rec, &c->sums, &sio};
   const int T = three ? SWEEP_T3 : SWEEP_T;
   cudaLaunchKernel(fn, dim3(c->nbricks), dim3(T), args, c->tile_bytes, c->stream);
   LAUNCH_CHECK("k_sweep");
-  if (io == IO_GATHER) c->gather_pending = false;
   return MPC_OK;
 }
 
@@ -321,8 +344,9 @@ cudaError_t sweep_set_attributes(size_t bytes) {
       for (int grav = 0; grav < 2; ++grav)
         for (int collide = 0; collide < 2; ++collide) {
           const struct { bool wkey; int io; bool three; } v[] = {{false, IO_PLAIN, false}, {false, IO_PLAIN, true}, {true, IO_PLAIN, false},
-                                                                 {true, IO_AOS_OUT, false}, {false, IO_GATHER, false}};
+                                                                 {false, IO_RANK, false}, {false, IO_SCATTER, false}, {false, IO_AOS_IN, false}};
           for (const auto& q : v) {
+            if (!collide && (q.io == IO_SCATTER || q.io == IO_AOS_IN)) continue;
             const cudaError_t e = cudaFuncSetAttribute(sweep_variant_any(fast, collide != 0, q.wkey, q.io, q.three, wall != 0, grav != 0, p2, shear),
                                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
             if (e != cudaSuccess) return e;
