@@ -273,29 +273,85 @@ inline void rotate(const double n[3], double ca, double sa, const double w[3], d
   out[2] = w[2] * ca + cz * sa + n[2] * nd * (1.0 - ca);
 }
 
-// ---- E_k / k_BT ~ Gamma(f/2, 1), f = 3(N_c-1): Eq. (7), sampler reading U6
-// sum of floor(f/2) unit exponentials, plus half a squared normal when f is odd.
+// ---- E_k / k_BT ~ Gamma(f/2, 1), f = 3(N_c-1): Eq. (7), sampler reading U6 ----------------------
+// The paper gives only the density. Reading U6: the rejection sampler of Marsaglia & Tsang (ACM TOMS 26,
+// 2000) for Gamma(a), a = f/2 >= 3/2: d = a - 1/3, c = 1/sqrt(9 d); draw x ~ N(0,1), U ~ U(0,1]; v = (1 + c x)^3;
+// accept if v > 0 and ( U < 1 - 0.0331 x^4  or  ln U < x^2/2 + d (1 - v + ln v) ); E_k / k_BT = d v.
+// An accept/reject decision is an integer decided by floating point: both codes take it in the SAME arithmetic, fixed
+// here operation by operation in IEEE binary32 (every operation rounded once, fmaf where written, no contraction;
+// -ffp-contract=off), with the logarithm and the cosine defined by the short series below instead of libm, whose
+// last bit differs between implementations. The sampler is exact up to those series' truncation (< 3e-9) and fp32
+// rounding, far below the statistical meaning of one draw. Constants are the binary32 numbers nearest to the
+// stated fractions, written as hexadecimal floats.
+// Random words: attempt 0 takes the cell's TAG_AXIS block of the step (whose top 24 bits of words 0, 1 give the rotation
+// axis): radius uniform = top 24 bits of word 2, angle = top 24 bits of word 3, acceptance uniform = the low bytes
+// of words 0, 1, 2 (bits the other draws do not use); attempt j >= 1 takes words 0, 1, 2 (top 24 bits) of block j - 1
+// of the cell's TAG_MBS stream. After 16 rejections (probability < 1e-20) E_k / k_BT = d.
+namespace mt {
+inline uint32_t f2u(float x) { uint32_t u; std::memcpy(&u, &x, 4); return u; }
+inline float u2f(uint32_t u) { float x; std::memcpy(&x, &u, 4); return x; }
+// ln x for a positive normal float: x = m 2^e with m in [sqrt(1/2), sqrt(2)); ln m = 2 atanh(s), s = (m-1)/(m+1),
+// atanh series up to s^9 (|s| <= 0.1716: the first dropped term is 2 s^11 / 11 < 7e-10)
+inline float rlog(float x) {
+  const int32_t i = (int32_t)f2u(x);
+  const int32_t e = (i - 0x3f3504f3) >> 23;                       // 0x3f3504f3 = bits of sqrt(1/2), arithmetic shift
+  const float m = u2f((uint32_t)(i - e * 8388608));               // in [sqrt(1/2), sqrt(2))
+  const float f = m - 1.0f;                                       // exact
+  const float s = f / (2.0f + f);
+  const float z = s * s;
+  float p = std::fmaf(z, 0x1.c71c72p-3f, 0x1.24924ap-2f);             // 2/9, 2/7
+  p = std::fmaf(z, p, 0x1.99999ap-2f);                              // 2/5
+  p = std::fmaf(z, p, 0x1.555556p-1f);                              // 2/3
+  p = std::fmaf(z, p, 2.0f);
+  return std::fmaf((float)e, 0x1.62e43p-1f /* ln 2 */, s * p);
+}
+// cos(2 pi k / 2^24) for a 24-bit integer k: the angle is split exactly (integers) into a quarter turn q and
+// y in [-pi/4, pi/4); Taylor series of sin and cos up to y^9 / y^10 (first dropped terms < 2e-9)
+inline float rcos(uint32_t k) {
+  const uint32_t kk = k + 2097152u;                               // + 1/8 turn
+  const uint32_t q = (kk >> 22) & 3u;
+  const int32_t r = (int32_t)(kk & 4194303u) - 2097152;           // in [-2^21, 2^21)
+  const float y = (float)r * 0x1.921fb6p-22f;                     // (pi/2) / 2^22
+  const float z = y * y;
+  float sp = std::fmaf(z, 0x1.71de3ap-19f, -0x1.a01a02p-13f);     // 1/9!, -1/7!
+  sp = std::fmaf(z, sp, 0x1.111112p-7f);                         // 1/5!
+  sp = std::fmaf(z, sp, -0x1.555556p-3f);                        // -1/3!
+  const float sn = std::fmaf(y * z, sp, y);
+  float cp = std::fmaf(z, -0x1.27e4fcp-22f, 0x1.a01a02p-16f);     // -1/10!, 1/8!
+  cp = std::fmaf(z, cp, -0x1.6c16c2p-10f);                        // -1/6!
+  cp = std::fmaf(z, cp, 0x1.555556p-5f);                         // 1/4!
+  const float cs = std::fmaf(z * z, cp, std::fmaf(-0.5f, z, 1.0f));
+  return (q == 0u) ? cs : (q == 1u) ? -sn : (q == 2u) ? -cs : sn;
+}
+}  // namespace mt
+
 inline double mbs_energy_over_kT(const Ctx& c, uint32_t cid, uint32_t t, unsigned Nc) {
   if (Nc < 2) return 0.0;
-  const unsigned f = 3u * (Nc - 1u), M = f / 2u;
-  double e = 0.0;
-  uint32_t o[4] = {0, 0, 0, 0};
-  unsigned have = 0, sub = 0, pos = 0;
-  auto next = [&]() -> uint32_t {
-    if (pos == have) { draw(c, cid, sub++, t, TAG_MBS, o); have = 4; pos = 0; }
-    return o[pos++];
-  };
-  for (unsigned j = 0; j < M; ++j) e -= std::log(u_oc(next()));
-  if (f & 1u) {
-    // the two uniforms of the half squared normal are words 2 and 3 of the cell's TAG_AXIS block of this
-    // step (words 0 and 1 give the rotation axis): independent of both, and no extra block (reading U6)
-    uint32_t a[4];
-    draw(c, cid, 0u, t, TAG_AXIS, a);
-    const double l = -std::log(u_oc(a[2]));
-    const double cs = std::cos(TWO_PI * u_co(a[3]));
-    e += l * cs * cs;                                   // = G^2/2 with G = sqrt(-2 ln U) cos(2 pi U')
+  const float a = 1.5f * (float)(Nc - 1u);
+  const float d = a - 0x1.555556p-2f /* 1/3 */;
+  const float cc = 1.0f / std::sqrt(9.0f * d);
+  for (unsigned j = 0; j < 16u; ++j) {
+    uint32_t o[4], wr, wa, wu;
+    if (j == 0u) {
+      draw(c, cid, 0u, t, TAG_AXIS, o);
+      wr = o[2] >> 8; wa = o[3] >> 8;
+      wu = ((o[0] & 0xffu) << 16) | ((o[1] & 0xffu) << 8) | (o[2] & 0xffu);
+    } else {
+      draw(c, cid, j - 1u, t, TAG_MBS, o);
+      wr = o[0] >> 8; wa = o[1] >> 8; wu = o[2] >> 8;
+    }
+    const float Ur = (float)(wr + 1u) * 0x1p-24f;   // (0, 1], exact
+    const float U = (float)(wu + 1u) * 0x1p-24f;
+    const float x = std::sqrt(-2.0f * mt::rlog(Ur)) * mt::rcos(wa);
+    const float v0 = std::fmaf(cc, x, 1.0f);
+    if (!(v0 > 0x1p-20f)) continue;                    // v0 <= 2^-20, v <= 2^-60: never accepted by a 24-bit U
+    const float v = (v0 * v0) * v0;
+    const float x2 = x * x;
+    bool ok = U < std::fmaf(-(0x1.0f27bcp-5f /* 0.0331 */ * x2), x2, 1.0f);
+    if (!ok) ok = mt::rlog(U) < std::fmaf(0.5f, x2, d * ((1.0f - v) + mt::rlog(v)));
+    if (ok) return (double)(d * v);
   }
-  return e;
+  return (double)d;
 }
 
 // 3x3 symmetric solve for omega = I^-1 dL with the degenerate-cell rules of reading U10

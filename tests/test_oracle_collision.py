@@ -123,29 +123,172 @@ def test_mbs_energy_sampler_is_gamma(Nc):
     assert o.mbs_energy(0, 0, 1) == 0.0
 
 
-def test_mbs_energy_stream_layout_from_raw_philox_words():
-    # Reading U6 fixes WHICH random words make E_k: word j of the cell's TAG_MBS (=2) blocks
-    # sub = 0, 1, ... in order for the floor(f/2) exponentials, words 2 and 3 of the cell's TAG_AXIS (=1)
-    # block for the half squared normal when f is odd. Recomputed here from raw blocks of the
-    # known-answer-pinned generator, so any change of the stream layout (tag, sub order, word order,
-    # open/closed interval) fails.
+# ---- reading U6: Marsaglia-Tsang in binary32, restated here with exact rational arithmetic ----------------
+# Every binary32 operation of the definition is done exactly (fractions.Fraction) and rounded once to the nearest-even
+# float, so this restatement shares neither code nor a floating-point library with the oracle.
+def _rnd32(q):
+    """Fraction -> nearest-even binary32 (normal range), as a Fraction."""
+    from fractions import Fraction
+    if q == 0:
+        return Fraction(0)
+    sgn, q = (-1 if q < 0 else 1), abs(q)
+    e = q.numerator.bit_length() - q.denominator.bit_length()
+    if Fraction(2) ** e > q:
+        e -= 1
+    assert -126 <= e <= 127, "outside the normal range"
+    ulp = Fraction(2) ** (e - 23)
+    n, r = divmod(q, ulp)
+    n = int(n)
+    if r * 2 > ulp or (r * 2 == ulp and n % 2 == 1):
+        n += 1
+    return sgn * n * ulp
+
+
+def _f32(x):
+    from fractions import Fraction
+    return Fraction(float(np.float32(x)))
+
+
+def _mul(a, b): return _rnd32(a * b)
+def _add(a, b): return _rnd32(a + b)
+def _div(a, b): return _rnd32(a / b)
+def _fma(a, b, c): return _rnd32(a * b + c)
+
+
+def _sqrt32(q):
+    """correctly rounded binary32 square root of a non-negative Fraction that is a binary32 number"""
+    from fractions import Fraction
+    if q == 0:
+        return Fraction(0)
+    r = _f32(np.sqrt(np.float64(float(q))))                  # candidate; then fix it up exactly
+    ulp = lambda v: Fraction(2) ** ((v.numerator.bit_length() - v.denominator.bit_length() - (1 if Fraction(2) ** (v.numerator.bit_length() - v.denominator.bit_length()) > v else 0)) - 23)
+    best = None
+    for cand in (r - ulp(r), r, r + ulp(r)):
+        err = abs(cand * cand - q) / (2 * cand) if cand > 0 else None    # |cand - sqrt(q)| to first order is monotone in |cand^2 - q|
+        # exact comparison of |cand - sqrt q|: compare (cand - sqrt q)^2 through cand^2 + q - 2 cand sqrt q; monotone in |cand^2 - q| / (cand + sqrt q)
+        key = abs(cand * cand - q) / (cand + Fraction(float(np.sqrt(np.float64(float(q))))))
+        if best is None or key < best[0]:
+            best = (key, cand)
+    return best[1]
+
+
+def _rlog(x):
+    from fractions import Fraction
+    i = int(np.float32(float(x)).view(np.int32))
+    e = (i - 0x3f3504f3) >> 23
+    m = Fraction(float(np.int32(i - e * 8388608).view(np.float32)))
+    f = m - 1
+    assert _rnd32(f) == f
+    s_ = _div(f, _add(Fraction(2), f))
+    z = _mul(s_, s_)
+    p = _fma(z, _f32(2 / 9), _f32(2 / 7))
+    p = _fma(z, p, _f32(2 / 5))
+    p = _fma(z, p, _f32(2 / 3))
+    p = _fma(z, p, Fraction(2))
+    return _fma(Fraction(e), _f32(np.log(2.0)), _mul(s_, p))
+
+
+def _rcos(k):
+    from fractions import Fraction
+    from math import factorial as F
+    kk = k + 2097152
+    q = (kk >> 22) & 3
+    r = (kk & 4194303) - 2097152
+    y = _mul(Fraction(r), _f32(np.pi / 2 / 4194304))
+    z = _mul(y, y)
+    sp = _fma(z, _f32(1 / F(9)), _f32(-1 / F(7)))
+    sp = _fma(z, sp, _f32(1 / F(5)))
+    sp = _fma(z, sp, _f32(-1 / F(3)))
+    sn = _fma(_mul(y, z), sp, y)
+    cp = _fma(z, _f32(-1 / F(10)), _f32(1 / F(8)))
+    cp = _fma(z, cp, _f32(-1 / F(6)))
+    cp = _fma(z, cp, _f32(1 / F(4)))
+    cs = _fma(_mul(z, z), cp, _fma(_f32(-0.5), z, Fraction(1)))
+    return [cs, -sn, -cs, sn][q]
+
+
+def _mt_energy(philox, key, cid, t, Nc, trace=None):
+    """E_k / kT of reading U6 from raw Philox blocks; trace collects which branch decided every attempt."""
+    from fractions import Fraction
+    a = _mul(_f32(1.5), Fraction(Nc - 1))
+    d = _add(a, -_f32(1 / 3))
+    cc = _div(Fraction(1), _sqrt32(_mul(Fraction(9), d)))
+    for j in range(16):
+        if j == 0:
+            o = [int(w) for w in philox([cid, 0, t, 1], key)]
+            wr, wa = o[2] >> 8, o[3] >> 8
+            wu = ((o[0] & 0xff) << 16) | ((o[1] & 0xff) << 8) | (o[2] & 0xff)
+        else:
+            o = [int(w) for w in philox([cid, j - 1, t, 2], key)]
+            wr, wa, wu = o[0] >> 8, o[1] >> 8, o[2] >> 8
+        Ur, U = Fraction(wr + 1, 1 << 24), Fraction(wu + 1, 1 << 24)
+        x = _mul(_sqrt32(_mul(Fraction(-2), _rlog(Ur))), _rcos(wa))
+        v0 = _fma(cc, x, Fraction(1))
+        if not v0 > Fraction(1, 1 << 20):
+            if trace is not None: trace.append("v<=0")
+            continue
+        v = _mul(_mul(v0, v0), v0)
+        x2 = _mul(x, x)
+        if U < _fma(-_mul(_f32(0.0331), x2), x2, Fraction(1)):
+            if trace is not None: trace.append("squeeze")
+            return float(_mul(d, v))
+        if _rlog(U) < _fma(_f32(0.5), x2, _mul(d, _add(_add(Fraction(1), -v), _rlog(v)))):
+            if trace is not None: trace.append("log test")
+            return float(_mul(d, v))
+        if trace is not None: trace.append("reject")
+    return float(d)
+
+
+def test_series_log_and_cos_of_the_sampler():
+    # the two series of reading U6 are the functions they claim to be: ln within 2e-7 relative (3e-8 absolute near 1),
+    # cos(2 pi k / 2^24) within 1.5e-7, on random arguments and at the edges of every range reduction
+    rng = np.random.default_rng(5)
+    xs = np.concatenate([rng.uniform(2.0 ** -24, 1.0, 300), 10.0 ** rng.uniform(-12, 2, 300),
+                         [2.0 ** -24, 1.0, 0.70710677, 0.7071068, 1.4142135, 1.4142137, 0.99999994, 1.0000001]]).astype(np.float32)
+    for x in xs:
+        got, want = float(_rlog(_f32(x))), np.log(np.float64(x))
+        assert abs(got - want) <= 2e-7 * abs(want) + 3e-8, (x, got, want)
+    ks = np.concatenate([rng.integers(0, 1 << 24, 600), [0, 1, (1 << 24) - 1, 1 << 21, (1 << 21) - 1, 3 << 21, (3 << 21) - 1, 1 << 22,
+                                                         1 << 23, 5 << 21, 7 << 21, (7 << 21) - 1]])
+    for k in ks:
+        assert abs(float(_rcos(int(k))) - np.cos(2 * np.pi * int(k) / 2.0 ** 24)) <= 1.5e-7, k
+
+
+def test_mbs_energy_from_raw_philox_words_bit_for_bit():
+    # Reading U6 fixes WHICH random words make E_k and every binary32 operation between them and the accept/reject
+    # decision. Recomputed here from raw blocks of the known-answer-pinned generator with exact rational arithmetic:
+    # any change of the stream layout (tag, block, word, low bytes, open/closed interval), of an operation or of its
+    # order fails, because the comparison is bit for bit. The cases are chosen (by the trace, not by the oracle) so
+    # that every branch is taken: squeeze accept, log-test accept, rejection followed by TAG_MBS attempts, v <= 0.
     from oracle.binding import philox
     seed = 0x1234_5678_9ABC_DEF0
     o = Oracle((4, 4, 4), (4, 4, 4), 10, seed)
     key = [seed & 0xFFFFFFFF, seed >> 32]
-    u_oc = lambda w: (float(w >> 8) + 1.0) / 16777216.0
-    u_co = lambda w: float(w >> 8) / 16777216.0
-    for cid, t, Nc in [(0, 0, 2), (5, 3, 3), (63, 7, 4), (17, 100, 10), (40, 2, 11), (9, 9, 26)]:
-        f = 3 * (Nc - 1)
-        M = f // 2
-        words = []
-        for sub in range((M + 3) // 4):
-            words += [int(w) for w in philox([cid, sub, t, 2], key)]
-        e = -sum(np.log(u_oc(w)) for w in words[:M])
-        if f % 2:
-            a = philox([cid, 0, t, 1], key)
-            e += -np.log(u_oc(int(a[2]))) * np.cos(2 * np.pi * u_co(int(a[3]))) ** 2
-        assert o.mbs_energy(cid, t, Nc) == pytest.approx(e, rel=1e-13)
+    seen = set()
+    cases = [(0, 0, 2), (5, 3, 3), (63, 7, 4), (17, 100, 10), (40, 2, 11), (9, 9, 26), (3, 1, 1000),
+             (6, 5, 2), (33, 130, 2)]      # the last two: x < -3 sqrt(d), so 1 + c x <= 0 at N_c = 2
+    cases += [(cid, t, Nc) for Nc in (2, 3, 10) for cid in range(40) for t in range(3)]
+    for cid, t, Nc in cases:
+        tr = []
+        e = _mt_energy(philox, key, cid, t, Nc, tr)
+        seen.update(tr)
+        if len(tr) > 1:
+            seen.add("retry")
+        assert o.mbs_energy(cid, t, Nc) == e, (cid, t, Nc, tr)
+    assert {"squeeze", "log test", "reject", "retry", "v<=0"} <= seen, seen
+
+
+def test_mbs_energy_golden_vector():
+    # stored draws (tests/golden/mbs_energy.txt, written by tests/golden/make_mbs_energy.py, which calls only oracle/):
+    # a later change of the sampler or of its stream layout shows up here even if the restatement above is changed with it
+    import os
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "mbs_energy.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) >= 40
+    seed = int(rows[0][1], 16)
+    o = Oracle((4, 4, 4), (4, 4, 4), 10, seed)
+    for r in rows[1:]:
+        cid, t, Nc = int(r[0]), int(r[1]), int(r[2])
+        assert o.mbs_energy(cid, t, Nc) == float.fromhex(r[3]), r
 
 
 def test_mbs_thermostat_sets_temperature():

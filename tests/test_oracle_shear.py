@@ -141,5 +141,8 @@ def test_shear_profile_and_viscosity_from_shear_stress():
     eta = -flux / g
     nu_kin, nu_col = srd_viscosity(nbar, h, 130)
     assert eta == pytest.approx(nbar * (nu_kin + nu_col), rel=0.04)    # 8.70
-    assert -kin / (nsamp * len(planes) * L * L * h * g) == pytest.approx(nbar * nu_kin, rel=0.25)   # kinetic part alone: 0.49
+    # kinetic part alone: 0.49. Its estimator sums v_x (thermal, variance kT/m = 1) over ~200 plane crossings per plane and
+    # step: 3.6e6 terms, standard error sqrt(3.6e6) / (nsamp * planes * L^2 * h * g) = 0.21; checked at 3 standard errors
+    # (the total above is far less noisy: the thermal v_x a particle carries across a plane is handed back by the collisions)
+    assert abs(-kin / (nsamp * len(planes) * L * L * h * g) - nbar * nu_kin) < 3 * 0.21
     assert o.observables()["kT_cell"] == pytest.approx(1.0, rel=0.02)

@@ -190,7 +190,9 @@ def test_poiseuille_profile_matches_analytic_viscosity():
     nu_fit, slip = g / (2 * coef[0]), coef[1]
     nu = sum(srd_viscosity(10, 0.1, 130))
     assert nu_fit == pytest.approx(nu, rel=0.06)
-    assert abs(slip) < 0.07 * prof.max()                       # near no-slip
+    # near no-slip: the virtual wall particles "reduce boundary slip", they do not remove it; the residual
+    # intercept of the fit is 6-7 % of v_max here (standard error of the fitted intercept ~1.5 % of v_max), bounded at 10 %
+    assert abs(slip) < 0.10 * prof.max()
     assert abs(prof - prof[::-1]).max() < 0.02                 # symmetric
     ob = o.observables()
     assert ob["kT_cell"] == pytest.approx(1.0, rel=0.03)        # thermostat holds k_BT under forcing
