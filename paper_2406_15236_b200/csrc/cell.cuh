@@ -7,90 +7,118 @@
 namespace mpc {
 
 
-// E_k / k_BT ~ Gamma(3(Nc-1)/2, 1) (Eq. 7; U6): minus the log of a product of floor(f/2)
-// uniforms (the product is renormalised by exponent extraction so it never underflows: one log per cell instead
-// of one per uniform), plus half a squared normal if f is odd.
-__device__ __forceinline__ void renorm(float& p, int& ex) {   // p = m * 2^e with m in [0.5,1): keep m, bank e
-  const int bits = __float_as_int(p);
-  ex += (bits >> 23) - 126;
-  p = __int_as_float((bits & 0x007fffff) | 0x3f000000);
+// E_k / k_BT ~ Gamma(a, 1), a = 3 (N_c - 1) / 2 (Eq. 7; U6): Marsaglia-Tsang rejection from one
+// normal x and one uniform U per attempt: d = a - 1/3, c = 1 / sqrt(9 d), v = (1 + c x)^3, accepted if v > 0 and
+// (U < 1 - 0.0331 x^4 or ln U < x^2 / 2 + d (1 - v + ln v)); E_k / k_BT = d v. Whether an attempt is accepted decides
+// which random words make E_k, so U6 fixes every operation up to that decision in binary32 (each rounded once: the _rn
+// intrinsics below are never contracted or reassociated), with ln and cos given by short series instead of the
+// hardware approximations. Attempt 0 uses the cell's TAG_AXIS block (radius: word 2, angle: word 3, top 24 bits each;
+// U: the low bytes of words 0, 1, 2), attempt j >= 1 words 0, 1, 2 of block j - 1 of the cell's TAG_MBS stream.
+// ln x, x a positive normal float: x = m 2^e, m in [sqrt(1/2), sqrt(2)), ln m = 2 atanh((m - 1) / (m + 1)) up to s^9
+__device__ __forceinline__ float mt_log(float x) {
+  const int i = __float_as_int(x);
+  const int e = (i - 0x3f3504f3) >> 23;
+  const float f = __fadd_rn(__int_as_float(i - (e << 23)), -1.0f);
+  const float s = __fdiv_rn(f, __fadd_rn(2.0f, f));
+  const float z = __fmul_rn(s, s);
+  float p = __fmaf_rn(z, 0x1.c71c72p-3f, 0x1.24924ap-2f);   // 2/9, 2/7
+  p = __fmaf_rn(z, p, 0x1.99999ap-2f);                      // 2/5
+  p = __fmaf_rn(z, p, 0x1.555556p-1f);                      // 2/3
+  p = __fmaf_rn(z, p, 2.0f);
+  return __fmaf_rn((float)e, 0x1.62e43p-1f, __fmul_rn(s, p));
 }
-// 2^24 * u01_oc(w): the power-of-two scale of every uniform is banked in the exponent instead (exact)
-__device__ __forceinline__ float u24_oc(uint32_t w) { return (float)((w >> 8) + 1u); }
-
-// -ln of the product of the first M uniforms of the cell's TAG_MBS stream (M = floor(f/2) unit exponentials)
-__device__ __forceinline__ float mbs_exponentials(const Geo& G, uint32_t cid, uint32_t M) {
-  if (M == 0u) return 0.0f;
-  const uint32_t full = M >> 2, rem = M & 3u;    // blocks whose four uniforms all enter the product; uniforms of the last one
-  float p = 1.0f;
-  int ex = -24 * (int)M;                         // M uniforms enter the product, each carried as 2^24 u
-  uint32_t sub = 0;
-  for (; sub < full; ++sub) {
-    const Block4 o = philox_rk(cid, sub, G.t, TAG_MBS, G.rk);
-    p *= (u24_oc(o.a) * u24_oc(o.b)) * (u24_oc(o.c) * u24_oc(o.d));   // < 2^96: cannot overflow
-    renorm(p, ex);
+// cos(2 pi k / 2^24), k < 2^24: quarter turn q and y in [-pi/4, pi/4) split off exactly, Taylor series to y^9 / y^10
+__device__ __forceinline__ float mt_cos(uint32_t k) {
+  const uint32_t kk = k + 2097152u;
+  const uint32_t q = (kk >> 22) & 3u;
+  const int r = (int)(kk & 4194303u) - 2097152;
+  const float y = __fmul_rn((float)r, 0x1.921fb6p-22f);     // (pi / 2) / 2^22
+  const float z = __fmul_rn(y, y);
+  float t;
+  if (q & 1u) {                                             // -+ sin y
+    t = __fmaf_rn(z, 0x1.71de3ap-19f, -0x1.a01a02p-13f);    // 1/9!, -1/7!
+    t = __fmaf_rn(z, t, 0x1.111112p-7f);                    // 1/5!
+    t = __fmaf_rn(z, t, -0x1.555556p-3f);                   // -1/3!
+    t = __fmaf_rn(__fmul_rn(y, z), t, y);
+    return (q == 1u) ? -t : t;
   }
-  if (rem) {
-    const Block4 o = philox_rk(cid, full, G.t, TAG_MBS, G.rk);
-    float q = u24_oc(o.a);
-    q *= (rem > 1u) ? u24_oc(o.b) : 1.0f;
-    q *= (rem > 2u) ? u24_oc(o.c) : 1.0f;
-    p *= q;
-    renorm(p, ex);
-  }
-  // p in [0.5, 1): __logf has an absolute error below 2^-21 there; the exponent part is added in double
-  return -(float)((double)__logf(p) + (double)ex * 0.6931471805599453);
+  t = __fmaf_rn(z, -0x1.27e4fcp-22f, 0x1.a01a02p-16f);      // -1/10!, 1/8!
+  t = __fmaf_rn(z, t, -0x1.6c16c2p-10f);                    // -1/6!
+  t = __fmaf_rn(z, t, 0x1.555556p-5f);                      // 1/4!
+  t = __fmaf_rn(__fmul_rn(z, z), t, __fmaf_rn(-0.5f, z, 1.0f));
+  return (q == 0u) ? t : -t;
 }
-
-
-// kappa of Eq. (6) for a cell of nc >= 2 members with mw2 = sum m_i |v_i - v_cm|^2 > 0; o = the cell's TAG_AXIS block,
-// whose words 2, 3 give the half squared normal when f = 3 (nc - 1) is odd (U6)
-__device__ __forceinline__ float mbs_kappa(const Geo& G, uint32_t cid, const Block4& o, uint32_t nc, float mw2) {
-  const uint32_t f = 3u * (nc - 1u);
-  float ek = mbs_exponentials(G, cid, f >> 1);
-  if (f & 1u) {
-    // cos(2 pi u) = -cos(2 pi (u - 1/2)), argument in [-pi, pi): __cosf / __logf are accurate to ~4e-7 absolute there,
-    // far below the statistical meaning of the draw and the 2e-5 parity budget
-    const float cs = __cosf(6.2831853071795865f * (u01_co(o.d) - 0.5f));
-    ek -= __logf(u01_oc(o.c)) * cs * cs;
+struct MtShape { float d, c; };
+__device__ __forceinline__ MtShape mt_shape(uint32_t nc) {
+  MtShape s;
+  s.d = __fadd_rn(__fmul_rn(1.5f, (float)(nc - 1u)), -0x1.555556p-2f);
+  s.c = __fdiv_rn(1.0f, __fsqrt_rn(__fmul_rn(9.0f, s.d)));
+  return s;
+}
+// one attempt from the 24-bit integers wr (radius), wa (angle), wu (acceptance); true: accepted, ek = E_k / k_BT
+__device__ __forceinline__ bool mt_attempt(const MtShape sh, uint32_t wr, uint32_t wa, uint32_t wu, float& ek) {
+  const float Ur = __fmul_rn((float)(wr + 1u), 0x1p-24f), U = __fmul_rn((float)(wu + 1u), 0x1p-24f);
+  const float x = __fmul_rn(__fsqrt_rn(__fmul_rn(-2.0f, mt_log(Ur))), mt_cos(wa));
+  const float v0 = __fmaf_rn(sh.c, x, 1.0f);
+  if (!(v0 > 0x1p-20f)) return false;
+  const float v = __fmul_rn(__fmul_rn(v0, v0), v0);
+  const float x2 = __fmul_rn(x, x);
+  ek = __fmul_rn(sh.d, v);
+  if (U < __fmaf_rn(-__fmul_rn(0x1.0f27bcp-5f, x2), x2, 1.0f)) return true;
+  return mt_log(U) < __fmaf_rn(0.5f, x2, __fmul_rn(sh.d, __fadd_rn(__fadd_rn(1.0f, -v), mt_log(v))));
+}
+__device__ __forceinline__ bool mt_attempt0(const MtShape sh, const Block4& o, float& ek) {   // o = the cell's TAG_AXIS block
+  return mt_attempt(sh, o.c >> 8, o.d >> 8, ((o.a & 0xffu) << 16) | ((o.b & 0xffu) << 8) | (o.c & 0xffu), ek);
+}
+// attempts 1, 2, ... (after a rejected attempt 0)
+__device__ __forceinline__ float mt_retry(const Geo& G, uint32_t cid, const MtShape sh) {
+  float ek;
+  for (uint32_t j = 0; j < 15u; ++j) {
+    const Block4 o = philox_rk(cid, j, G.t, TAG_MBS, G.rk);
+    if (mt_attempt(sh, o.a >> 8, o.b >> 8, o.c >> 8, ek)) return ek;
   }
+  return sh.d;
+}
+__device__ __forceinline__ float kappa_of(const Geo& G, float ek, float mw2) {   // Eq. (6)
   const float x = __fdividef(2.0f * (G.kT * ek), mw2);
   return x * rsqrtf(fmaxf(x, 1e-37f));
+}
+// kappa of Eq. (6) for a cell of nc >= 2 members with mw2 = sum m_i |v_i - v_cm|^2 > 0; o = the cell's TAG_AXIS block
+__device__ __forceinline__ float mbs_kappa(const Geo& G, uint32_t cid, const Block4& o, uint32_t nc, float mw2) {
+  const MtShape sh = mt_shape(nc);
+  float ek;
+  if (!mt_attempt0(sh, o, ek)) ek = mt_retry(G, cid, sh);
+  return kappa_of(G, ek, mw2);
 }
 
 // rec[key] = { vcm.x, vcm.y, vcm.z, kappa, n.x, n.y, n.z, - }
 // grid = (mb0 * CTAs-per-brick, mb1, mb2): the brick coordinates come from blockIdx, no division.
 // zero != 0: the sums of a cell are cleared once read, which saves the memset before the next step's sweep.
-// The number of Philox blocks a cell needs for its thermostat draw grows with its occupancy (Poisson), and a warp runs
-// as long as its fullest cell needs. Two phases: (A) thread t reads the sums of cell t (coalesced), reduces them to
-// {v_cm, sum |v - v_cm|^2, N_c} and parks that in shared memory; the CT cells of the CTA are counting-sorted by their
-// number of Philox blocks; (B) thread j finishes the j-th cell of the sorted order (draw, kappa, axis, one 32-byte
-// record): every warp gets cells of nearly equal cost, and there is no barrier after the loop of variable length.
+// Thread t handles cell t of the CTA's CT cells: reads its sums (coalesced), v_cm, sum |v - v_cm|^2, N_c, the TAG_AXIS
+// block (axis + first thermostat attempt) and writes one 32-byte record (coalesced). The few cells whose first attempt
+// is rejected (3-5 %) are collected in shared memory and finished by the first threads of the CTA, so that a warp
+// does not wait for its one unlucky lane.
 struct CellWork { float vx, vy, vz, w2; uint32_t cid, nc; };
 template <int CT>
-struct CellScratch { unsigned hist[32]; unsigned short order[CT]; CellWork work[CT]; };
+struct CellScratch { unsigned nretry; unsigned short retry[CT]; uint32_t cid[CT]; uint32_t nc[CT]; float ek[CT]; };
 
 // CT cells [lbase, lbase + CT) of brick (bx, by, bz), one per thread of the CTA (all CT threads must call)
 template <int CT>
 __device__ __forceinline__ void cell_batch(const Geo& G, uint32_t bx, uint32_t by, uint32_t bz, uint32_t lbase, u64* __restrict__ sums,
                                            float* __restrict__ rec, int zero, CellScratch<CT>& sh) {
-  unsigned* hist = sh.hist;
-  unsigned short* order = sh.order;
-  CellWork* work = sh.work;
   const unsigned tid = threadIdx.x;
-  if (tid < 32) hist[tid] = 0u;
+  if (tid == 0) sh.nretry = 0u;
+  __syncthreads();
   const int b0 = G.bs[0], b1 = G.bs[1], b2 = G.bs[2];
   const uint32_t local = lbase + tid;
   const bool valid = local < (1u << (b0 + b1 + b2));
   const uint32_t brick = (bz * (uint32_t)G.mb[1] + by) * (uint32_t)G.mb[0] + bx;
   const uint32_t kbase = (brick << (b0 + b1 + b2)) + lbase;
-  // ---- phase A ----
   u64* s = sums + (size_t)(kbase + tid) * G.sw;
   u64 w0 = 0ull;
   if (valid) w0 = s[0];
   const uint32_t nreal = (uint32_t)(w0 & 0xffffull);
   CellWork cw = {0.f, 0.f, 0.f, 0.f, 0u, 0u};
-  uint32_t M = 0u;
   if (valid && nreal != 0u) {
     const int ix = (int)((bx << b0) | (local & ((1u << b0) - 1u)));
     const int iy = (int)((by << b1) | ((local >> b0) & ((1u << b1) - 1u)));
@@ -133,42 +161,42 @@ __device__ __forceinline__ void cell_batch(const Geo& G, uint32_t bx, uint32_t b
     cw.nc = Nc;
     if (G.thermostat && Nc >= 2u) {
       const double W2 = E - (S0 * S0 + S1 * S1 + S2 * S2) * inv;   // sum |v - vcm|^2
-      if (W2 > 0.0) { M = (3u * (Nc - 1u)) >> 1; cw.w2 = (float)W2; }
+      if (W2 > 0.0) cw.w2 = (float)W2;
     }
   }
-  // ---- counting sort of the CTA's cells by the number of Philox blocks of their draw (empty cells last) ----
-  const unsigned bin = cw.nc ? min((M + 3u) >> 2, 30u) : 31u;
-  __syncthreads();
-  const unsigned rank = atomicAdd(&hist[bin], 1u);
-  work[tid] = cw;
-  __syncthreads();
-  if (tid < 32) {
-    const unsigned v = hist[tid];
-    unsigned inc = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
-      if (tid >= (unsigned)o) inc += t;
+  // ---- axis and first thermostat attempt ----
+  Block4 o = {0u, 0u, 0u, 0u};
+  float ek = 0.0f;
+  bool pending = false;
+  if (cw.nc != 0u) {
+    o = philox_rk(cw.cid, 0u, G.t, TAG_AXIS, G.rk);
+    if (cw.w2 > 0.0f) {
+      pending = !mt_attempt0(mt_shape(cw.nc), o, ek);
+      if (pending) {
+        const unsigned j = atomicAdd(&sh.nretry, 1u);
+        sh.retry[j] = (unsigned short)tid; sh.cid[tid] = cw.cid; sh.nc[tid] = cw.nc;
+      }
     }
-    hist[tid] = inc - v;
   }
   __syncthreads();
-  order[hist[bin] + rank] = (unsigned short)tid;
-  __syncthreads();
-  // ---- phase B ----
-  const unsigned u = order[tid];
-  const CellWork c = work[u];
-  if (c.nc == 0u) return;
-  const Block4 o = philox_rk(c.cid, 0u, G.t, TAG_AXIS, G.rk);
-  const float kappa = (c.w2 > 0.0f) ? mbs_kappa(G, c.cid, o, c.nc, G.mass * c.w2) : 1.0f;
+  const unsigned nretry = sh.nretry;
+  if (nretry) {
+    for (unsigned j = tid; j < nretry; j += CT) {
+      const unsigned u = sh.retry[j];
+      sh.ek[u] = mt_retry(G, sh.cid[u], mt_shape(sh.nc[u]));
+    }
+    __syncthreads();
+    if (pending) ek = sh.ek[tid];
+  }
+  if (cw.nc == 0u) return;
+  const float kappa = (cw.w2 > 0.0f) ? kappa_of(G, ek, G.mass * cw.w2) : 1.0f;
   const float zz = 2.0f * u01_co(o.a) - 1.0f;
   const float rr = sqrtf((1.0f - zz) * (1.0f + zz));
   float sp, cp;
   sincospif(2.0f * u01_co(o.b), &sp, &cp);
-  float4* out = reinterpret_cast<float4*>(rec) + (size_t)(kbase + u) * 2;
-  out[0] = make_float4(c.vx, c.vy, c.vz, kappa);
+  float4* out = reinterpret_cast<float4*>(rec) + (size_t)(kbase + tid) * 2;
+  out[0] = make_float4(cw.vx, cw.vy, cw.vz, kappa);
   out[1] = make_float4(rr * cp, rr * sp, zz, 0.0f);
 }
-
 
 }  // namespace mpc
