@@ -14,7 +14,7 @@ namespace {
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  size_t off_A[7], off_B[7], off_key, off_slot, off_perm, off_cursor, off_offset, off_bsum, off_sums, off_rec, off_obs,
+  size_t off_A[7], off_B[7], off_key, off_slot, off_perm, off_cursor, off_offset, off_bsum, off_sums, off_rec, off_obs, off_mt,
       off_tbase, off_chunk0, total;
 };
 // tile_cells: cells of one brick's shared-memory tile; tbase (first slot of every CTA inside every tile cell's segment,
@@ -39,6 +39,7 @@ Layout make_layout(size_t n_max, size_t nkeys, size_t nbricks, size_t tile_cells
   l.off_sums = take(nkeys * (size_t)sw * 8);
   l.off_rec = take(nkeys * (size_t)rw * 4);
   l.off_obs = take(OBS_HOST_DOUBLES * 8 + 256);
+  l.off_mt = take(MT_TABLE * 4);
   const bool staged = !compact && !generic;
   l.off_tbase = take(staged ? nbricks * tile_cells * 4 : 4);
   l.off_chunk0 = take(staged ? (nbricks + 1) * 4 : 4);
@@ -99,13 +100,19 @@ int steps_srd(mpc_ctx* c, int nsteps) {
       // all but the last step of the call: k_cell clears the sums it has read (the last step's stay for
       // mpc_observables / mpc_get_cells)
       const int zero = (k + 1 < nsteps) ? 1 : 0;
-      if (rebin) {
-        const int rc = do_reorder(c, stage, (c->debug & MPC_DEBUG_EAGER_CANONICAL) != 0);
+      // a folded reorder scans compact counts that k_cell writes while it reads the sums anyway (the scan would otherwise
+      // read every cell's 24 bytes twice); the other reorders read the counts from the sums, before k_cell clears them
+      if (rebin && !stage) {
+        const int rc = do_reorder(c, false, (c->debug & MPC_DEBUG_EAGER_CANONICAL) != 0);
         if (rc) return rc;
       }
       {
         FamilyTimer ft(c, F_CELL);
-        const int rc = launch_cell(c, zero);
+        const int rc = launch_cell(c, zero, stage ? c->cursor : nullptr);
+        if (rc) return rc;
+      }
+      if (stage) {
+        const int rc = do_reorder(c, true, false);
         if (rc) return rc;
       }
       c->sums_clean = zero != 0;
@@ -291,6 +298,11 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
   c->nsing = (u64*)(c->ws + l.off_obs + OBS_HOST_DOUBLES * 8);
   c->nrange = c->nsing + 1;
   c->G.nrange = c->nrange;
+  {   // table of the thermostat draw (cell.cuh)
+    fill_mt_table(c->mt_host);
+    CU(cudaMemcpyAsync(c->ws + l.off_mt, c->mt_host, MT_TABLE * 4, cudaMemcpyHostToDevice, c->stream));
+    c->G.mt_c = (const float*)(c->ws + l.off_mt);
+  }
   const bool staged = !compact && !c->G.generic;
   c->tbase = staged ? (uint32_t*)(c->ws + l.off_tbase) : nullptr;
   c->chunk0 = staged ? (uint32_t*)(c->ws + l.off_chunk0) : nullptr;

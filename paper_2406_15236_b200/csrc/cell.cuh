@@ -49,10 +49,26 @@ __device__ __forceinline__ float mt_cos(uint32_t k) {
   return (q == 0u) ? t : -t;
 }
 struct MtShape { float d, c; };
-__device__ __forceinline__ MtShape mt_shape(uint32_t nc) {
+// c = 1 / sqrt(9 d) for N_c < MT_TABLE comes from a table made on the host with the same IEEE operations (mt_c_host)
+__host__ __device__ __forceinline__ float mt_d_of(uint32_t nc) {
+#ifdef __CUDA_ARCH__
+  return __fadd_rn(__fmul_rn(1.5f, (float)(nc - 1u)), -0x1.555556p-2f);
+#else
+  volatile float a = 1.5f * (float)(nc - 1u);      // volatile: every operation rounded to binary32 on the host as well
+  volatile float d = a - 0x1.555556p-2f;
+  return d;
+#endif
+}
+inline float mt_c_host(uint32_t nc) {
+  volatile float t = 9.0f * mt_d_of(nc);
+  volatile float r = sqrtf(t);
+  volatile float c = 1.0f / r;
+  return c;
+}
+__device__ __forceinline__ MtShape mt_shape(const Geo& G, uint32_t nc) {
   MtShape s;
-  s.d = __fadd_rn(__fmul_rn(1.5f, (float)(nc - 1u)), -0x1.555556p-2f);
-  s.c = __fdiv_rn(1.0f, __fsqrt_rn(__fmul_rn(9.0f, s.d)));
+  s.d = mt_d_of(nc);
+  s.c = (nc < (uint32_t)MT_TABLE) ? __ldg(G.mt_c + nc) : __fdiv_rn(1.0f, __fsqrt_rn(__fmul_rn(9.0f, s.d)));
   return s;
 }
 // one attempt from the 24-bit integers wr (radius), wa (angle), wu (acceptance); true: accepted, ek = E_k / k_BT
@@ -85,7 +101,7 @@ __device__ __forceinline__ float kappa_of(const Geo& G, float ek, float mw2) {  
 }
 // kappa of Eq. (6) for a cell of nc >= 2 members with mw2 = sum m_i |v_i - v_cm|^2 > 0; o = the cell's TAG_AXIS block
 __device__ __forceinline__ float mbs_kappa(const Geo& G, uint32_t cid, const Block4& o, uint32_t nc, float mw2) {
-  const MtShape sh = mt_shape(nc);
+  const MtShape sh = mt_shape(G, nc);
   float ek;
   if (!mt_attempt0(sh, o, ek)) ek = mt_retry(G, cid, sh);
   return kappa_of(G, ek, mw2);
@@ -95,20 +111,14 @@ __device__ __forceinline__ float mbs_kappa(const Geo& G, uint32_t cid, const Blo
 // grid = (mb0 * CTAs-per-brick, mb1, mb2): the brick coordinates come from blockIdx, no division.
 // zero != 0: the sums of a cell are cleared once read, which saves the memset before the next step's sweep.
 // Thread t handles cell t of the CTA's CT cells: reads its sums (coalesced), v_cm, sum |v - v_cm|^2, N_c, the TAG_AXIS
-// block (axis + first thermostat attempt) and writes one 32-byte record (coalesced). The few cells whose first attempt
-// is rejected (3-5 %) are collected in shared memory and finished by the first threads of the CTA, so that a warp
-// does not wait for its one unlucky lane.
+// block (axis + first thermostat attempt) and writes one 32-byte record (coalesced). 0.3 % of the first attempts are
+// rejected at <N_c> = 10; those lanes retry in place (8 % of the warps wait for one).
 struct CellWork { float vx, vy, vz, w2; uint32_t cid, nc; };
-template <int CT>
-struct CellScratch { unsigned nretry; unsigned short retry[CT]; uint32_t cid[CT]; uint32_t nc[CT]; float ek[CT]; };
 
 // CT cells [lbase, lbase + CT) of brick (bx, by, bz), one per thread of the CTA (all CT threads must call)
-template <int CT>
 __device__ __forceinline__ void cell_batch(const Geo& G, uint32_t bx, uint32_t by, uint32_t bz, uint32_t lbase, u64* __restrict__ sums,
-                                           float* __restrict__ rec, int zero, CellScratch<CT>& sh) {
+                                           float* __restrict__ rec, int zero, uint32_t* __restrict__ counts) {
   const unsigned tid = threadIdx.x;
-  if (tid == 0) sh.nretry = 0u;
-  __syncthreads();
   const int b0 = G.bs[0], b1 = G.bs[1], b2 = G.bs[2];
   const uint32_t local = lbase + tid;
   const bool valid = local < (1u << (b0 + b1 + b2));
@@ -118,6 +128,7 @@ __device__ __forceinline__ void cell_batch(const Geo& G, uint32_t bx, uint32_t b
   u64 w0 = 0ull;
   if (valid) w0 = s[0];
   const uint32_t nreal = (uint32_t)(w0 & 0xffffull);
+  if (counts && valid) counts[kbase + tid] = nreal;      // compact per-cell counts for the scan of a folded reorder
   CellWork cw = {0.f, 0.f, 0.f, 0.f, 0u, 0u};
   if (valid && nreal != 0u) {
     const int ix = (int)((bx << b0) | (local & ((1u << b0) - 1u)));
@@ -164,39 +175,19 @@ __device__ __forceinline__ void cell_batch(const Geo& G, uint32_t bx, uint32_t b
       if (W2 > 0.0) cw.w2 = (float)W2;
     }
   }
-  // ---- axis and first thermostat attempt ----
-  Block4 o = {0u, 0u, 0u, 0u};
-  float ek = 0.0f;
-  bool pending = false;
-  if (cw.nc != 0u) {
-    o = philox_rk(cw.cid, 0u, G.t, TAG_AXIS, G.rk);
-    if (cw.w2 > 0.0f) {
-      pending = !mt_attempt0(mt_shape(cw.nc), o, ek);
-      if (pending) {
-        const unsigned j = atomicAdd(&sh.nretry, 1u);
-        sh.retry[j] = (unsigned short)tid; sh.cid[tid] = cw.cid; sh.nc[tid] = cw.nc;
-      }
-    }
-  }
-  __syncthreads();
-  const unsigned nretry = sh.nretry;
-  if (nretry) {
-    for (unsigned j = tid; j < nretry; j += CT) {
-      const unsigned u = sh.retry[j];
-      sh.ek[u] = mt_retry(G, sh.cid[u], mt_shape(sh.nc[u]));
-    }
-    __syncthreads();
-    if (pending) ek = sh.ek[tid];
-  }
   if (cw.nc == 0u) return;
-  const float kappa = (cw.w2 > 0.0f) ? kappa_of(G, ek, G.mass * cw.w2) : 1.0f;
+  // ---- axis and thermostat draw ----
+  const Block4 o = philox_rk(cw.cid, 0u, G.t, TAG_AXIS, G.rk);
+  const float kappa = (cw.w2 > 0.0f) ? mbs_kappa(G, cw.cid, o, cw.nc, G.mass * cw.w2) : 1.0f;
+  // axis: z = 2 u0 - 1, phi = 2 pi u1 (U11). cos / sin of phi - pi in [-pi, pi) with the hardware approximations (absolute
+  // error ~4e-7 there, inside the 2e-5 parity budget of the velocities): cos phi = -cos(phi - pi), sin phi = -sin(phi - pi)
   const float zz = 2.0f * u01_co(o.a) - 1.0f;
-  const float rr = sqrtf((1.0f - zz) * (1.0f + zz));
-  float sp, cp;
-  sincospif(2.0f * u01_co(o.b), &sp, &cp);
+  const float t2 = (1.0f - zz) * (1.0f + zz);
+  const float rr = -t2 * rsqrtf(fmaxf(t2, 1e-30f));
+  const float ph = 6.2831853071795865f * (u01_co(o.b) - 0.5f);
   float4* out = reinterpret_cast<float4*>(rec) + (size_t)(kbase + tid) * 2;
   out[0] = make_float4(cw.vx, cw.vy, cw.vz, kappa);
-  out[1] = make_float4(rr * cp, rr * sp, zz, 0.0f);
+  out[1] = make_float4(rr * __cosf(ph), rr * __sinf(ph), zz, 0.0f);
 }
 
 }  // namespace mpc

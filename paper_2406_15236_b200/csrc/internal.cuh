@@ -39,6 +39,7 @@ constexpr int TILE_W = 5;             // int32 words per tile cell: N, Sx, Sy, S
 constexpr int REC_W = 8;              // floats per cell record (32 B, one sector)
 constexpr int OBS_BLOCKS = 1184;      // 148 SMs x 8
 constexpr int MAX_PROFILE = 2048;
+constexpr int MT_TABLE = 64;          // thermostat draw: table of c(N_c) for N_c < 64 (cell.cuh)
 constexpr size_t OBS_HOST_DOUBLES = (size_t)OBS_BLOCKS * 8 + 2 * MAX_PROFILE;
 constexpr size_t MAX_TILE_BYTES = 110 * 1024;
 constexpr int SCAN_T = 256, SCAN_PER = 8, SCAN_TILE = SCAN_T * SCAN_PER;
@@ -89,6 +90,7 @@ struct Geo {
   uint32_t solute_id0; // particles with id >= solute_id0 have mass solute_mass (if > 0; U23)
   float solute_mass;
   float wall_u;        // moving no-slip walls: +wall_u along x at L, -wall_u at 0 (U24)
+  const float* mt_c;   // device table of MT_TABLE floats: c(N_c) of the thermostat draw (cell.cuh)
 };
 
 // ---- packed sums ---------------------------------------------------------------------------------
@@ -326,6 +328,7 @@ struct mpc_ctx {
   mpc::u64* nsing;  // +a: number of rejected inertia tensors in the last step
   mpc::u64* nrange; // range overflows since the last mpc_set_state
   double* hbuf;     // host staging for mpc_observables
+  float mt_host[mpc::MT_TABLE];   // host copy of the thermostat table
   // optional per-family timing with CUDA events on the bound stream (mpc_profile_*)
   bool prof_on;
   cudaEvent_t* prof_ev;
@@ -379,7 +382,8 @@ cudaError_t sweep_set_attributes(size_t tile_bytes);
 int launch_collide_pos(mpc_ctx* c);
 int launch_keys(mpc_ctx* c, uint32_t* key_out);
 // cell.cu
-int launch_cell(mpc_ctx* c, int zero);
+int launch_cell(mpc_ctx* c, int zero, uint32_t* counts);   // counts != nullptr: also writes the per-cell particle counts (one word per key)
+void fill_mt_table(float* host);
 // reorder.cu
 int do_reorder(mpc_ctx* c, bool defer_gather, bool canonical);
 int canonicalise(mpc_ctx* c);

@@ -265,8 +265,9 @@ int apply_perm(mpc_ctx* c) {
 // canonical: rank the particles of a cell by id now (needed by MPC-AT); otherwise group by key only
 int do_reorder(mpc_ctx* c, bool folded, bool canonical) {
   const size_t n = c->n, nk = c->G.nkeys, nb = (nk + SCAN_TILE - 1) / SCAN_TILE;
-  const uint32_t* cnt = reinterpret_cast<const uint32_t*>(c->sums);
-  const int stride = c->G.sw * 2;
+  // folded: compact counts written by k_cell into c->cursor (the sums are already cleared)
+  const uint32_t* cnt = folded ? c->cursor : reinterpret_cast<const uint32_t*>(c->sums);
+  const int stride = folded ? 1 : c->G.sw * 2;
   const int bvs = c->G.bs[0] + c->G.bs[1] + c->G.bs[2];
   if (folded && canonical) return fail(c, MPC_ESTATE, "internal: folded reorder cannot rank by id");
   // lane-spread order inside every group of 32 keys: hot path only, bricks of whole groups (spread_slot)
