@@ -142,7 +142,7 @@ int set_state_impl(mpc_ctx* c, unsigned long long n, const float* const src[6], 
   }
   CU(cudaMemsetAsync(c->nrange, 0, 8, c->stream));
   c->n = n; c->t = step; c->have_state = true; c->have_cells = false; c->have_order = false; c->reorder_stage = 0;
-  c->order_canonical = true; c->order_spread = false; c->collide_pending = false;
+  c->order_canonical = true; c->order_spread = 0; c->collide_pending = false;
   return MPC_OK;
 }
 int get_state_impl(mpc_ctx* c, float* const dst[6], unsigned* id, cudaMemcpyKind kind) {
@@ -308,7 +308,7 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
   c->chunk0 = staged ? (uint32_t*)(c->ws + l.off_chunk0) : nullptr;
   CU(cudaMemsetAsync(c->nrange, 0, 8, c->stream));
   c->bound = true; c->have_state = false; c->have_cells = false; c->have_order = false; c->sums_clean = false; c->reorder_stage = 0;
-  c->collide_pending = false; c->order_spread = false; c->n = 0;
+  c->collide_pending = false; c->order_spread = 0; c->n = 0;
   if (c->tile_bytes > 48 * 1024) {
     const cudaError_t e = sweep_set_attributes(c->tile_bytes);
     if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(k_sweep, MaxDynamicSharedMemorySize)");

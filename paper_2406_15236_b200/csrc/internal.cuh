@@ -39,6 +39,7 @@ constexpr int TILE_W = 5;             // int32 words per tile cell: N, Sx, Sy, S
 constexpr int REC_W = 8;              // floats per cell record (32 B, one sector)
 constexpr int OBS_BLOCKS = 1184;      // 148 SMs x 8
 constexpr int MAX_PROFILE = 2048;
+constexpr int SPREAD_GROUP_SHIFT = 5;  // lane-spread order: groups of 32 cells (spread_slot); 64: equal, 128: sweep +4 % (gathered cell records spread over more lines)
 constexpr int MT_TABLE = 64;          // thermostat draw: table of c(N_c) for N_c < 64 (cell.cuh)
 constexpr size_t OBS_HOST_DOUBLES = (size_t)OBS_BLOCKS * 8 + 2 * MAX_PROFILE;
 constexpr size_t MAX_TILE_BYTES = 110 * 1024;
@@ -303,7 +304,7 @@ struct mpc_ctx {
   // applies it; every call that reads particle velocities applies it first (flush_collide)
   bool collide_pending;
   bool pow2_cells;      // no walls and every m[d] a power of two: the sweep folds indices with a mask
-  bool order_spread;    // the particles of every group of 32 keys are stored lane-spread (reorder.cu, spread_slot)
+  int order_spread;     // log2 of the cells per group whose particles are stored lane-spread (spread_slot); 0 = plain cell order
   int reorder_stage;    // folded reorder: 0 none in flight, 1 the next sweep scatters into the new order, 2 the next sweep reads the staged records
   float le_dprev;       // Lees-Edwards displacement of the step whose collision is pending
   unsigned debug;       // MPC_DEBUG_* flags

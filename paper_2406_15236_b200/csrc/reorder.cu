@@ -89,8 +89,8 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const uint32_t* __restric
 // lane-spread order inside a group of 32 cells: spread_slot (internal.cuh)
 __device__ __forceinline__ uint32_t spread_key(const uint32_t* __restrict__ offset, uint32_t k, uint32_t slot, int spread) {
   if (!spread) return slot;
-  const uint32_t kg = k & ~31u;
-  return spread_slot(slot, offset[kg], offset[kg + 32u]);
+  const uint32_t kg = k & ~((1u << spread) - 1u);
+  return spread_slot(slot, offset[kg], offset[kg + (1u << spread)]);
 }
 
 // Lanes of a warp that hold the same key as their neighbours form runs (the array is still nearly sorted):
@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(256) k_rank_cells(size_t nkeys, const uint32_t
   const uint32_t b = offset[k], e = offset[k + 1];
   if (b == e) return;
   uint32_t g0 = 0, g1 = 0;               // R = 0: spread_slot is the identity
-  if (spread) { g0 = offset[k & ~(size_t)31]; g1 = offset[(k & ~(size_t)31) + 32]; }
+  if (spread) { const size_t kg = k & ~(((size_t)1 << spread) - 1); g0 = offset[kg]; g1 = offset[kg + ((size_t)1 << spread)]; }
   for (uint32_t j = b; j < e; ++j) {
     const uint32_t pj = spread_slot(j, g0, g1), me = id[pj];
     uint32_t r = 0;
@@ -271,7 +271,8 @@ int do_reorder(mpc_ctx* c, bool folded, bool canonical) {
   const int bvs = c->G.bs[0] + c->G.bs[1] + c->G.bs[2];
   if (folded && canonical) return fail(c, MPC_ESTATE, "internal: folded reorder cannot rank by id");
   // lane-spread order inside every group of 32 keys: hot path only, bricks of whole groups (spread_slot)
-  const int spread = (!canonical && bvs >= 5 && !(c->debug & MPC_DEBUG_NO_LANE_SPREAD)) ? 1 : 0;
+  const int gs = SPREAD_GROUP_SHIFT;
+  const int spread = (!canonical && bvs >= gs && !(c->debug & MPC_DEBUG_NO_LANE_SPREAD)) ? gs : 0;
   if (folded) {   // the brick ranges of the old order, before the scan overwrites the offsets
     FamilyTimer ft(c, F_SCAN);
     k_save_chunks<<<nblk((size_t)c->nbricks + 1, 256), 256, 0, c->stream>>>(c->offset, bvs, c->nbricks, (uint32_t)n, c->chunk0);
@@ -306,7 +307,7 @@ int do_reorder(mpc_ctx* c, bool folded, bool canonical) {
   }
   c->have_order = true;
   c->order_canonical = canonical;
-  c->order_spread = spread != 0;
+  c->order_spread = spread;
   if (folded) { c->reorder_stage = 1; return MPC_OK; }
   return apply_perm(c);
 }
@@ -317,10 +318,10 @@ int canonicalise(mpc_ctx* c) {
   if (!c->have_order || c->order_canonical || c->n == 0) return MPC_OK;
   {
     FamilyTimer ft(c, F_RANK);
-    k_rank_cells<<<nblk(c->G.nkeys, 256), 256, 0, c->stream>>>(c->G.nkeys, c->offset, c->A[6], c->perm, c->order_spread ? 1 : 0);
+    k_rank_cells<<<nblk(c->G.nkeys, 256), 256, 0, c->stream>>>(c->G.nkeys, c->offset, c->A[6], c->perm, c->order_spread);
     LAUNCH_CHECK("k_rank_cells");
   }
   const int rc = apply_perm(c);
-  if (rc == MPC_OK) { c->order_canonical = true; c->order_spread = false; }
+  if (rc == MPC_OK) { c->order_canonical = true; c->order_spread = 0; }
   return rc;
 }

@@ -23,7 +23,7 @@ struct SweepIO {
   uint32_t* id;             // IO_SCATTER: read at i; IO_AOS_IN: written at i
   uint32_t* tbase;          // IO_RANK: written by the flush; IO_SCATTER: read: first slot of this CTA's particles inside every tile cell's segment
   const uint32_t* offset;   // IO_SCATTER: cell offsets of the new order
-  int spread;               // IO_SCATTER: lane-spread order inside every group of 32 cells (spread_slot)
+  int spread;               // IO_SCATTER: log2 of the cells per group of the lane-spread order (spread_slot), 0 = plain cell order
   int chunk_shift;          // chunk[b << chunk_shift] = first particle of brick b
   float le_dprev;           // Lees-Edwards displacement of the previous step (for its collision)
 };
@@ -165,7 +165,7 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
           const int l0 = foldp<P2>(kx - ox, m0), l1 = foldp<P2>(ky - oy, m1), l2 = foldp<P2>(kz - oz, m2);
           slot += io.tbase[(size_t)b * tcells + (l2 * T1 + l1) * T0 + l0] + w;
         }
-        if (io.spread) { const uint32_t kg = kp & ~31u; slot = spread_slot(slot, io.offset[kg], io.offset[kg + 32u]); }
+        if (io.spread) { const uint32_t kg = kp & ~((1u << io.spread) - 1u); slot = spread_slot(slot, io.offset[kg], io.offset[kg + (1u << io.spread)]); }
       }
       if (SHEAR) v[0] += vsp;
       srd_apply(G, r0, ax, v);
@@ -323,7 +323,7 @@ int launch_sweep(mpc_ctx* c, bool collide, bool wkey, int io, const float sp[3])
   sio.id = c->A[6];
   sio.tbase = c->tbase;
   sio.offset = c->offset;
-  sio.spread = c->order_spread ? 1 : 0;
+  sio.spread = c->order_spread;
   // the scatter pass still walks the old order: its brick ranges were saved before the scan overwrote the offsets
   const uint32_t* chunk = (io == IO_SCATTER) ? c->chunk0 : (c->have_order ? c->offset : nullptr);
   sio.chunk_shift = (io == IO_SCATTER) ? 0 : G.bs[0] + G.bs[1] + G.bs[2];
