@@ -276,7 +276,7 @@ inline void rotate(const double n[3], double ca, double sa, const double w[3], d
 // ---- E_k / k_BT ~ Gamma(f/2, 1), f = 3(N_c-1): Eq. (7), sampler reading U6 ----------------------
 // The paper gives only the density. Reading U6: the rejection sampler of Marsaglia & Tsang (ACM TOMS 26,
 // 2000) for Gamma(a), a = f/2 >= 3/2: d = a - 1/3, c = 1/sqrt(9 d); draw x ~ N(0,1), U ~ U(0,1]; v = (1 + c x)^3;
-// accept if v > 0 and ( U < 1 - 0.0331 x^4  or  ln U < x^2/2 + d (1 - v + ln v) ); E_k / k_BT = d v.
+// accept if v > 0 and ( U < 1 - k x^4  or  ln U < x^2/2 + d (1 - v + ln v) ); E_k / k_BT = d v (k: below).
 // An accept/reject decision is an integer decided by floating point: both codes take it in the SAME arithmetic, fixed
 // here operation by operation in IEEE binary32 (every operation rounded once, fmaf where written, no contraction;
 // -ffp-contract=off), with the logarithm and the cosine defined by the short series below instead of libm, whose
@@ -330,6 +330,12 @@ inline double mbs_energy_over_kT(const Ctx& c, uint32_t cid, uint32_t t, unsigne
   const float a = 1.5f * (float)(Nc - 1u);
   const float d = a - 0x1.555556p-2f /* 1/3 */;
   const float cc = 1.0f / std::sqrt(9.0f * d);
+  // squeeze U < 1 - k x^4: valid whenever k >= -g(x) / x^4 for every reachable x (|x| <= sqrt(48 ln 2) = 5.77 from a
+  // 24-bit uniform), g(x) = x^2/2 + d (1 - v + ln v), because exp(g) >= 1 + g. Marsaglia and Tsang's k = 0.0331 holds for
+  // every a >= 1; for N_c >= 7 the bound k = (0.0093 + 0.0145 / sqrt(d) + 0.06 / d) / d is 4..30 times tighter (the series
+  // of g starts with -x^4 / (108 d) + x^5 / (405 d^1.5)); checked numerically in tests/test_oracle_collision.py
+  const float kq = (Nc < 7u) ? 0x1.0f27bcp-5f /* 0.0331 */
+                             : (0x1.30be0ep-7f /* 0.0093 */ + 0x1.db22d0p-7f /* 0.0145 */ / std::sqrt(d) + 0x1.eb851ep-5f /* 0.06 */ / d) / d;
   for (unsigned j = 0; j < 16u; ++j) {
     uint32_t o[4], wr, wa, wu;
     if (j == 0u) {
@@ -347,7 +353,7 @@ inline double mbs_energy_over_kT(const Ctx& c, uint32_t cid, uint32_t t, unsigne
     if (!(v0 > 0x1p-20f)) continue;                    // v0 <= 2^-20, v <= 2^-60: never accepted by a 24-bit U
     const float v = (v0 * v0) * v0;
     const float x2 = x * x;
-    bool ok = U < std::fmaf(-(0x1.0f27bcp-5f /* 0.0331 */ * x2), x2, 1.0f);
+    bool ok = U < std::fmaf(-(kq * x2), x2, 1.0f);
     if (!ok) ok = mt::rlog(U) < std::fmaf(0.5f, x2, d * ((1.0f - v) + mt::rlog(v)));
     if (ok) return (double)(d * v);
   }

@@ -213,6 +213,10 @@ def _mt_energy(philox, key, cid, t, Nc, trace=None):
     a = _mul(_f32(1.5), Fraction(Nc - 1))
     d = _add(a, -_f32(1 / 3))
     cc = _div(Fraction(1), _sqrt32(_mul(Fraction(9), d)))
+    if Nc < 7:
+        kq = _f32(0.0331)
+    else:
+        kq = _div(_add(_add(_f32(0.0093), _div(_f32(0.0145), _sqrt32(d))), _div(_f32(0.06), d)), d)
     for j in range(16):
         if j == 0:
             o = [int(w) for w in philox([cid, 0, t, 1], key)]
@@ -229,7 +233,7 @@ def _mt_energy(philox, key, cid, t, Nc, trace=None):
             continue
         v = _mul(_mul(v0, v0), v0)
         x2 = _mul(x, x)
-        if U < _fma(-_mul(_f32(0.0331), x2), x2, Fraction(1)):
+        if U < _fma(-_mul(kq, x2), x2, Fraction(1)):
             if trace is not None: trace.append("squeeze")
             return float(_mul(d, v))
         if _rlog(U) < _fma(_f32(0.5), x2, _mul(d, _add(_add(Fraction(1), -v), _rlog(v)))):
@@ -254,6 +258,37 @@ def test_series_log_and_cos_of_the_sampler():
         assert abs(float(_rcos(int(k))) - np.cos(2 * np.pi * int(k) / 2.0 ** 24)) <= 1.5e-7, k
 
 
+def test_squeeze_of_the_sampler_is_a_lower_bound():
+    # Reading U6: "accept if U < 1 - k x^4" is only a shortcut for the exact test ln U < g(x), g = x^2/2 + d (1 - v + ln v),
+    # if 1 - k x^4 <= exp(g(x)) wherever it can fire. With exp(g) >= 1 + g that holds if k >= -g(x) / x^4 on the reachable
+    # range |x| <= sqrt(48 ln 2) < 5.78 (24-bit radius uniform), v > 0. Checked in 40-digit arithmetic on a dense grid
+    # for the N_c-dependent k of N_c >= 7 (with the binary32 value of k, 0.1 % margin) and for 0.0331 below (where the
+    # bound must hold against exp(g) itself: near v -> 0 the ratio -g / x^4 diverges but 1 - k x^4 is negative there).
+    from mpmath import mp, mpf, log, sqrt, exp
+    mp.dps = 40
+    xmax = mpf("5.78")
+    for Nc in list(range(2, 80)) + [100, 150, 200, 500, 1000, 1500, 2000, 3000, 5000, 10**4, 10**5, 10**6]:
+        d = mpf(3) * (Nc - 1) / 2 - mpf(1) / 3
+        c = 1 / sqrt(9 * d)
+        d32 = np.float32(1.5) * np.float32(Nc - 1) - np.float32(1 / 3)
+        if Nc < 7:
+            k = mpf(float(np.float32(0.0331)))
+        else:
+            k = mpf(float((np.float32(0.0093) + np.float32(0.0145) / np.sqrt(d32) + np.float32(0.06) / d32) / d32))
+        lo = max(-xmax, -1 / c)
+        for i in range(1, 3001):
+            x = lo + (xmax - lo) * i / 3000
+            v0 = 1 + c * x
+            if v0 <= 0 or abs(x) < mpf("1e-3"):
+                continue
+            v = v0 ** 3
+            g = x * x / 2 + d * (1 - v + log(v))
+            if Nc < 7:
+                assert 1 - k * x ** 4 <= exp(g), (Nc, float(x))
+            else:
+                assert -g / x ** 4 <= k * (1 - mpf("1e-3")), (Nc, float(x), float(-g / x ** 4), float(k))
+
+
 def test_mbs_energy_from_raw_philox_words_bit_for_bit():
     # Reading U6 fixes WHICH random words make E_k and every binary32 operation between them and the accept/reject
     # decision. Recomputed here from raw blocks of the known-answer-pinned generator with exact rational arithmetic:
@@ -267,7 +302,7 @@ def test_mbs_energy_from_raw_philox_words_bit_for_bit():
     seen = set()
     cases = [(0, 0, 2), (5, 3, 3), (63, 7, 4), (17, 100, 10), (40, 2, 11), (9, 9, 26), (3, 1, 1000),
              (6, 5, 2), (33, 130, 2)]      # the last two: x < -3 sqrt(d), so 1 + c x <= 0 at N_c = 2
-    cases += [(cid, t, Nc) for Nc in (2, 3, 10) for cid in range(40) for t in range(3)]
+    cases += [(cid, t, Nc) for Nc in (2, 3, 7, 10) for cid in range(40) for t in range(3)]
     for cid, t, Nc in cases:
         tr = []
         e = _mt_energy(philox, key, cid, t, Nc, tr)
