@@ -39,7 +39,7 @@ Layout make_layout(size_t n_max, size_t nkeys, size_t nbricks, size_t tile_cells
   l.off_sums = take(nkeys * (size_t)sw * 8);
   l.off_rec = take(nkeys * (size_t)rw * 4);
   l.off_obs = take(OBS_HOST_DOUBLES * 8 + 256);
-  l.off_mt = take(MT_TABLE * 4);
+  l.off_mt = take(MT_TABLE * 8);
   const bool staged = !compact && !generic;
   l.off_tbase = take(staged ? nbricks * tile_cells * 4 : 4);
   l.off_chunk0 = take(staged ? (nbricks + 1) * 4 : 4);
@@ -300,7 +300,7 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
   c->G.nrange = c->nrange;
   {   // table of the thermostat draw (cell.cuh)
     fill_mt_table(c->mt_host);
-    CU(cudaMemcpyAsync(c->ws + l.off_mt, c->mt_host, MT_TABLE * 4, cudaMemcpyHostToDevice, c->stream));
+    CU(cudaMemcpyAsync(c->ws + l.off_mt, c->mt_host, MT_TABLE * 8, cudaMemcpyHostToDevice, c->stream));
     c->G.mt_c = (const float*)(c->ws + l.off_mt);
   }
   const bool staged = !compact && !c->G.generic;

@@ -9,7 +9,8 @@ namespace mpc {
 
 // E_k / k_BT ~ Gamma(a, 1), a = 3 (N_c - 1) / 2 (Eq. 7; U6): Marsaglia-Tsang rejection from one
 // normal x and one uniform U per attempt: d = a - 1/3, c = 1 / sqrt(9 d), v = (1 + c x)^3, accepted if v > 0 and
-// (U < 1 - 0.0331 x^4 or ln U < x^2 / 2 + d (1 - v + ln v)); E_k / k_BT = d v. Whether an attempt is accepted decides
+// (U < 1 - k x^4 or ln U < x^2 / 2 + d (1 - v + ln v)), k = 0.0331 for N_c < 7 and (0.0093 + 0.0145 / sqrt(d) + 0.06 / d) / d
+// above; E_k / k_BT = d v. Whether an attempt is accepted decides
 // which random words make E_k, so U6 fixes every operation up to that decision in binary32 (each rounded once: the _rn
 // intrinsics below are never contracted or reassociated), with ln and cos given by short series instead of the
 // hardware approximations. Attempt 0 uses the cell's TAG_AXIS block (radius: word 2, angle: word 3, top 24 bits each;
@@ -48,8 +49,8 @@ __device__ __forceinline__ float mt_cos(uint32_t k) {
   t = __fmaf_rn(__fmul_rn(z, z), t, __fmaf_rn(-0.5f, z, 1.0f));
   return (q == 0u) ? t : -t;
 }
-struct MtShape { float d, c; };
-// c = 1 / sqrt(9 d) for N_c < MT_TABLE comes from a table made on the host with the same IEEE operations (mt_c_host)
+struct MtShape { float d, c, k; };   // d = a - 1/3, c = 1 / sqrt(9 d), k = constant of the squeeze U < 1 - k x^4 (U6)
+// (c, k) for N_c < MT_TABLE come from a table made on the host with the same IEEE operations (mt_shape_host)
 __host__ __device__ __forceinline__ float mt_d_of(uint32_t nc) {
 #ifdef __CUDA_ARCH__
   return __fadd_rn(__fmul_rn(1.5f, (float)(nc - 1u)), -0x1.555556p-2f);
@@ -59,16 +60,31 @@ __host__ __device__ __forceinline__ float mt_d_of(uint32_t nc) {
   return d;
 #endif
 }
-inline float mt_c_host(uint32_t nc) {
-  volatile float t = 9.0f * mt_d_of(nc);
+inline void mt_shape_host(uint32_t nc, float& c_out, float& k_out) {
+  const float d = mt_d_of(nc);
+  volatile float t = 9.0f * d;
   volatile float r = sqrtf(t);
   volatile float c = 1.0f / r;
-  return c;
+  c_out = c;
+  if (nc < 7u) { k_out = 0x1.0f27bcp-5f; return; }              // 0.0331
+  volatile float sd = sqrtf(d);
+  volatile float q1 = 0x1.db22d0p-7f / sd;                       // 0.0145 / sqrt(d)
+  volatile float q2 = 0x1.eb851ep-5f / d;                        // 0.06 / d
+  volatile float s1 = 0x1.30be0ep-7f + q1;                       // 0.0093 + ...
+  volatile float s2 = s1 + q2;
+  volatile float k = s2 / d;
+  k_out = k;
 }
 __device__ __forceinline__ MtShape mt_shape(const Geo& G, uint32_t nc) {
   MtShape s;
   s.d = mt_d_of(nc);
-  s.c = (nc < (uint32_t)MT_TABLE) ? __ldg(G.mt_c + nc) : __fdiv_rn(1.0f, __fsqrt_rn(__fmul_rn(9.0f, s.d)));
+  if (nc < (uint32_t)MT_TABLE) {
+    const float2 ck = __ldg(reinterpret_cast<const float2*>(G.mt_c) + nc);
+    s.c = ck.x; s.k = ck.y;
+  } else {
+    s.c = __fdiv_rn(1.0f, __fsqrt_rn(__fmul_rn(9.0f, s.d)));
+    s.k = __fdiv_rn(__fadd_rn(__fadd_rn(0x1.30be0ep-7f, __fdiv_rn(0x1.db22d0p-7f, __fsqrt_rn(s.d))), __fdiv_rn(0x1.eb851ep-5f, s.d)), s.d);
+  }
   return s;
 }
 // one attempt from the 24-bit integers wr (radius), wa (angle), wu (acceptance); true: accepted, ek = E_k / k_BT
@@ -80,7 +96,7 @@ __device__ __forceinline__ bool mt_attempt(const MtShape sh, uint32_t wr, uint32
   const float v = __fmul_rn(__fmul_rn(v0, v0), v0);
   const float x2 = __fmul_rn(x, x);
   ek = __fmul_rn(sh.d, v);
-  if (U < __fmaf_rn(-__fmul_rn(0x1.0f27bcp-5f, x2), x2, 1.0f)) return true;
+  if (U < __fmaf_rn(-__fmul_rn(sh.k, x2), x2, 1.0f)) return true;
   return mt_log(U) < __fmaf_rn(0.5f, x2, __fmul_rn(sh.d, __fadd_rn(__fadd_rn(1.0f, -v), mt_log(v))));
 }
 __device__ __forceinline__ bool mt_attempt0(const MtShape sh, const Block4& o, float& ek) {   // o = the cell's TAG_AXIS block

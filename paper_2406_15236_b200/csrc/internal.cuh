@@ -40,7 +40,7 @@ constexpr int REC_W = 8;              // floats per cell record (32 B, one secto
 constexpr int OBS_BLOCKS = 1184;      // 148 SMs x 8
 constexpr int MAX_PROFILE = 2048;
 constexpr int SPREAD_GROUP_SHIFT = 5;  // lane-spread order: groups of 32 cells (spread_slot); 64: equal, 128: sweep +4 % (gathered cell records spread over more lines)
-constexpr int MT_TABLE = 64;          // thermostat draw: table of c(N_c) for N_c < 64 (cell.cuh)
+constexpr int MT_TABLE = 64;          // thermostat draw: table of (c, k)(N_c) for N_c < 64 (cell.cuh)
 constexpr size_t OBS_HOST_DOUBLES = (size_t)OBS_BLOCKS * 8 + 2 * MAX_PROFILE;
 constexpr size_t MAX_TILE_BYTES = 110 * 1024;
 constexpr int SCAN_T = 256, SCAN_PER = 8, SCAN_TILE = SCAN_T * SCAN_PER;
@@ -91,7 +91,7 @@ struct Geo {
   uint32_t solute_id0; // particles with id >= solute_id0 have mass solute_mass (if > 0; U23)
   float solute_mass;
   float wall_u;        // moving no-slip walls: +wall_u along x at L, -wall_u at 0 (U24)
-  const float* mt_c;   // device table of MT_TABLE floats: c(N_c) of the thermostat draw (cell.cuh)
+  const float* mt_c;   // device table of MT_TABLE float pairs: (c, k)(N_c) of the thermostat draw (cell.cuh)
 };
 
 // ---- packed sums ---------------------------------------------------------------------------------
@@ -329,7 +329,7 @@ struct mpc_ctx {
   mpc::u64* nsing;  // +a: number of rejected inertia tensors in the last step
   mpc::u64* nrange; // range overflows since the last mpc_set_state
   double* hbuf;     // host staging for mpc_observables
-  float mt_host[mpc::MT_TABLE];   // host copy of the thermostat table
+  float mt_host[2 * mpc::MT_TABLE];   // host copy of the thermostat table: (c, k) per N_c
   // optional per-family timing with CUDA events on the bound stream (mpc_profile_*)
   bool prof_on;
   cudaEvent_t* prof_ev;
