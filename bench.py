@@ -281,7 +281,7 @@ def measure(args, workload, nbar, steps, warmup, rank, local_rank, world, dist, 
                       "collision": "MPC-AT" if kw.get("collision") else "SRD", "conserve_L": bool(kw.get("conserve_L", 0)),
                       "thermostat": bool(kw.get("thermostat", 0)),
                       "rebin_every": wl["rebin_every"], "brick": list(brick), "compact_workspace": bool(compact),
-                      "l2": "inputs larger than L2 (no flush)" if n * 24 > 4 * 126e6 else "state fits in L2; HBM fraction not meaningful",
+                      "l2": "inputs larger than L2 (no flush)" if n * 24 > 4 * 126e6 else "state within 4x L2 (partly L2-resident): HBM fraction not meaningful",
                       "parallelism": "replicas only" if world > 1 else "single GPU",
                       "algorithmic_bytes_per_update": balg,
                       "collisions_in_timed_region": "K (the warm-up's last collision is applied by the first timed sweep, the last timed one stays pending)"},
@@ -381,7 +381,7 @@ def main():
 def kernel_algorithmic_bytes(family, n, ncells, nbar):
     """Algorithmic bytes one launch of a kernel family must move."""
     per_particle = {"stream_key": 24 + 12 + 4, "accum": 12 + 4, "collide": 12 + 4 + 12, "gather": 4 + 32 + 32,
-                    "scatter_slots": 8 + 8, "rank": 12 + 4, "sweep": 48, "sweep_gather": 48 + 8 + 4}.get(family, 0)
+                    "scatter_slots": 8 + 8, "rank": 12 + 4, "sweep": 48, "sweep_gather": 48 + 32 / 3.0}.get(family, 0)
     # sweep: the per-cell record is read once (32 B) and the cell sums written once (20 B of payload)
     per_cell = {"accum": 20, "cell": 20 + 32, "collide": 32, "scan": 8, "memset": 24, "sweep": 20 + 20, "sweep_gather": 20 + 20}.get(family, 0)
     return float(per_particle) * n + float(per_cell) * ncells
