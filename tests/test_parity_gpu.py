@@ -69,6 +69,9 @@ CASES = {
     "cfg1_srd": dict(cells=(16, 16, 16), nbar=10, kw=dict()),
     "srd_mbs_brick4": dict(cells=(16, 12, 8), nbar=10, kw=dict(thermostat=1, brick=4)),
     "srd_mbs_low_density": dict(cells=(12, 12, 12), nbar=3, kw=dict(thermostat=1)),
+    # thermostat draw (U6) outside the table of (c, k) pairs the kernel reads for N_c < 64, and with a wall fill of 80
+    "srd_mbs_high_density": dict(cells=(6, 6, 6), nbar=80, kw=dict(thermostat=1, brick=2)),
+    "walls_high_density": dict(cells=(6, 6, 6), nbar=80, kw=dict(thermostat=1, bc=(0, 0, 1), g=(0.001, 0, 0))),
     "srd_a2": dict(cells=(8, 8, 8), nbar=10, kw=dict(thermostat=1), a=2.0),
     "at": dict(cells=(12, 12, 12), nbar=10, kw=dict(collision=1, dt=0.02)),
     "at_brick2": dict(cells=(10, 12, 6), nbar=5, kw=dict(collision=1, dt=0.02, brick=2)),
