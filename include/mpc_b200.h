@@ -76,6 +76,14 @@ typedef struct {
   float wall_velocity; /* moving no-slip walls (plane Couette flow; U24): the wall at L moves with
                         +wall_velocity along x, the wall at 0 with -wall_velocity; bounce-back in the frame of the wall
                         (v -> 2 u_wall - v), wall / phantom particles thermal about u_wall. Needs bc = 1 on y or z            */
+  int   sub_z0;      /* slab subdomain of a multi-GPU run: this context owns the cell layers    */
+  int   sub_nz;      /* [sub_z0, sub_z0 + sub_nz) along z of the box given to mpc_create (the WHOLE box: cells[2] = all layers) and
+                        holds one brick layer (brick[2] cell layers) of halo on either side. 0, 0 = the whole box (default).
+                        Both multiples of brick[2]; sub_nz >= 2 brick[2]; sub_nz + 2 brick[2] <= cells[2]. Periodic SRD without +a,
+                        walls, shear or force. The caller gives the rank the particles whose z lies in its layers; particles may
+                        drift up to one brick layer outside (further: counted in n_range_overflows, results invalid); moving
+                        them to the owning rank is the caller's job between steps (mpc_get_state / mpc_set_state).
+                        See mpc_sub_connect, mpc_sub_begin, mpc_sub_end                                                        */
 } mpc_params;
 
 typedef struct {
@@ -141,6 +149,25 @@ int mpc_set_state_host(mpc_ctx*, unsigned long long n, const float* x, const flo
  * first streaming pass, and every call that reads velocities (mpc_get_state*, mpc_observables) applies it first,
  * so the state seen through the API is always the fully collided one. */
 int mpc_step(mpc_ctx*, int nsteps);
+
+/* ---- slab subdomains (multi-GPU domain decomposition; one context per rank) ----------------------------
+ * The step is split at its one exchange point. Every rank streams its own particles and adds their cell sums into
+ * its own array; the sums of the cells in the four brick layers it shares with its two neighbours (its halo and first /
+ * last own brick layer on either side) are ALSO added, inside the same kernel, into the neighbours' arrays with integer
+ * reductions over peer memory (NVLink). Integer sums commute: after a barrier every rank holds the complete sums of
+ * all its local cells, computes the same cell records from them as its neighbours do for the shared cells (the random
+ * numbers are indexed by the cell's id in the whole box), and no particle is ever sent for a collision (the paper
+ * exchanges the particles). The trajectory equals the single-GPU one bit for bit.
+ *   mpc_sub_sums     device pointer and local brick-layer count of this rank's sums (to hand to its neighbours)
+ *   mpc_sub_connect  the neighbours' pointers and layer counts (below = towards smaller z); clears the sums. The memory
+ *                    must be reachable from this device (same device, or peer access / IPC mapping enabled by the caller)
+ *   mpc_sub_begin    MOVE + sums of the next step (+ the pending collision). Then: barrier over all ranks
+ *   mpc_sub_end      PROCESS_CELLS (+ the local reorder when due). Then: barrier over all ranks
+ * mpc_step returns MPC_ESTATE on a subdomain context. mpc_observables reports this rank's particles (kT_cell = 0). */
+int mpc_sub_sums(mpc_ctx*, void** sums_device, int* brick_layers);
+int mpc_sub_connect(mpc_ctx*, void* sums_below, int brick_layers_below, void* sums_above, int brick_layers_above);
+int mpc_sub_begin(mpc_ctx*);
+int mpc_sub_end(mpc_ctx*);
 
 /* Diagnostic switches (change speed only, never results; the library reads no environment variables):
  * a bitwise OR of the flags below, 0 = the default code paths. May be called at any time between steps. */

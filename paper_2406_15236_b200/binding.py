@@ -19,7 +19,7 @@ DEBUG_NO_FUSE_GATHER, DEBUG_EAGER_CANONICAL, DEBUG_ATOMIC_SCATTER, DEBUG_EAGER_C
 SYMBOLS = ["mpc_create", "mpc_num_keys", "mpc_workspace_bytes", "mpc_bind", "mpc_set_state", "mpc_set_state_host",
            "mpc_step", "mpc_set_debug", "mpc_get_state", "mpc_get_state_host", "mpc_observables", "mpc_get_cells",
            "mpc_philox4x32_10", "mpc_launch_count", "mpc_profile_enable", "mpc_profile_read", "mpc_last_error",
-           "mpc_destroy"]
+           "mpc_destroy", "mpc_sub_sums", "mpc_sub_connect", "mpc_sub_begin", "mpc_sub_end"]
 
 
 class mpc_params(C.Structure):
@@ -27,7 +27,8 @@ class mpc_params(C.Structure):
                 ("alpha", C.c_float), ("dt", C.c_float), ("kT", C.c_float), ("mass", C.c_float),
                 ("g", C.c_float * 3), ("bc", C.c_int * 3), ("grid_shift", C.c_int),
                 ("rebin_every", C.c_int), ("brick", C.c_int * 3), ("shear_rate", C.c_float),
-                ("phantoms", C.c_int), ("solute_id0", C.c_uint), ("solute_mass", C.c_float), ("wall_velocity", C.c_float)]
+                ("phantoms", C.c_int), ("solute_id0", C.c_uint), ("solute_mass", C.c_float), ("wall_velocity", C.c_float),
+                ("sub_z0", C.c_int), ("sub_nz", C.c_int)]
 
 
 class mpc_obs(C.Structure):
@@ -75,6 +76,10 @@ def load():
     L.mpc_last_error.argtypes = [vp]
     L.mpc_last_error.restype = C.c_char_p
     L.mpc_destroy.argtypes = [vp]
+    L.mpc_sub_sums.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_int)]
+    L.mpc_sub_connect.argtypes = [vp, vp, C.c_int, vp, C.c_int]
+    L.mpc_sub_begin.argtypes = [vp]
+    L.mpc_sub_end.argtypes = [vp]
     for s in SYMBOLS:
         getattr(L, s)
     _lib = L
@@ -91,8 +96,9 @@ def philox4x32_10(ctr, key):
 
 def make_params(collision=0, conserve_L=0, thermostat=0, alpha_deg=130.0, dt=0.1, kT=1.0, mass=1.0,
                 g=(0.0, 0.0, 0.0), bc=(0, 0, 0), grid_shift=1, rebin_every=1, brick=1, shear_rate=0.0,
-                phantoms=0, solute_id0=0, solute_mass=0.0, wall_velocity=0.0):
+                phantoms=0, solute_id0=0, solute_mass=0.0, wall_velocity=0.0, sub=(0, 0)):
     p = mpc_params()
+    p.sub_z0, p.sub_nz = sub
     p.phantoms, p.solute_id0, p.solute_mass, p.wall_velocity = phantoms, solute_id0, solute_mass, wall_velocity
     p.shear_rate = shear_rate
     p.collision, p.conserve_L, p.thermostat = collision, conserve_L, thermostat
@@ -143,6 +149,23 @@ class MPC:
         if rc != MPC_OK:
             msg = self.lib.mpc_last_error(self._h).decode() if self._h else ""
             raise MPCError(f"mpc error {rc}: {msg}")
+
+    # ---- slab subdomains of a multi-GPU run (include/mpc_b200.h "slab subdomains") ----
+    def sub_sums(self):
+        """(device pointer, local brick layers) of this rank's cell sums, to hand to its two neighbours"""
+        p, nb = C.c_void_p(), C.c_int()
+        self._check(self.lib.mpc_sub_sums(self._h, C.byref(p), C.byref(nb)))
+        return p.value, nb.value
+
+    def sub_connect(self, below, above):
+        """below / above = sub_sums() of the neighbours towards smaller / larger z (peer memory reachable from this device)"""
+        self._check(self.lib.mpc_sub_connect(self._h, C.c_void_p(below[0]), below[1], C.c_void_p(above[0]), above[1]))
+
+    def sub_begin(self):
+        self._check(self.lib.mpc_sub_begin(self._h))
+
+    def sub_end(self):
+        self._check(self.lib.mpc_sub_end(self._h))
 
     def close(self):
         if getattr(self, "_h", None):

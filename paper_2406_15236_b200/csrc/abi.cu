@@ -14,12 +14,12 @@ namespace {
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  size_t off_A[7], off_B[7], off_key, off_slot, off_perm, off_cursor, off_offset, off_bsum, off_sums, off_rec, off_obs, off_mt,
+  size_t off_A[7], off_B[7], off_key, off_slot, off_perm, off_cursor, off_offset, off_bsum, off_sums, off_lcount, off_rec, off_obs, off_mt,
       off_tbase, off_chunk0, total;
 };
 // tile_cells: cells of one brick's shared-memory tile; tbase (first slot of every CTA inside every tile cell's segment,
 // written by the staging sweep of a reorder) exists only where the staged reorder does: second particle copy, SRD path
-Layout make_layout(size_t n_max, size_t nkeys, size_t nbricks, size_t tile_cells, int sw, int rw, bool compact, bool generic) {
+Layout make_layout(bool sub, size_t n_max, size_t nkeys, size_t nbricks, size_t tile_cells, int sw, int rw, bool compact, bool generic) {
   Layout l;
   size_t o = 0;
   auto take = [&](size_t bytes) { const size_t r = o; o = align_up(o + bytes, 256); return r; };
@@ -37,6 +37,7 @@ Layout make_layout(size_t n_max, size_t nkeys, size_t nbricks, size_t tile_cells
   l.off_offset = take((nkeys + 1) * 4);
   l.off_bsum = take(((nkeys + SCAN_TILE - 1) / SCAN_TILE + 1) * 4);
   l.off_sums = take(nkeys * (size_t)sw * 8);
+  l.off_lcount = take(sub ? nkeys * 4 : 4);            // slab subdomain: this rank's own counts of the shared cells
   l.off_rec = take(nkeys * (size_t)rw * 4);
   l.off_obs = take(OBS_HOST_DOUBLES * 8 + 256);
   l.off_mt = take(MT_TABLE * 8);
@@ -47,7 +48,7 @@ Layout make_layout(size_t n_max, size_t nkeys, size_t nbricks, size_t tile_cells
   return l;
 }
 Layout ctx_layout(const mpc_ctx* c, size_t n_max, bool compact) {
-  return make_layout(n_max, c->G.nkeys, c->nbricks, c->tile_bytes / (TILE_W * 4), c->G.sw, c->G.rw, compact, c->G.generic != 0);
+  return make_layout(c->G.sub != 0, n_max, c->G.nkeys, c->nbricks, c->tile_bytes / (TILE_W * 4), c->G.sw, c->G.rw, compact, c->G.generic != 0);
 }
 
 void host_shift(const mpc_ctx* c, uint32_t t, float s[3]) {
@@ -70,26 +71,28 @@ float host_le_offset(const mpc_ctx* c, uint32_t t) {
 
 // SRD: step t = sweep (collision of t-1 if one is pending + MOVE of t + sums of t), [reorder], PROCESS_CELLS of t.
 // The collision of the last step stays pending: the next call's first sweep applies it (flush_collide otherwise).
-int steps_srd(mpc_ctx* c, int nsteps) {
+// phase: 0 = whole steps; slab subdomains run ONE step in two calls around the barrier of the ranks: 1 = the sweep,
+// 2 = PROCESS_CELLS and the local reorder (mpc_sub_begin / mpc_sub_end)
+int steps_srd(mpc_ctx* c, int nsteps, int phase = 0) {
   Geo& G = c->G;
   const size_t n = c->n;
   float sp[3] = {G.s[0], G.s[1], G.s[2]};          // shift of the pending step (if any)
   for (int k = 0; k < nsteps; ++k) {
-    G.t = c->t;
-    host_shift(c, c->t, G.s);
-    c->le_dprev = G.le_d;
-    G.le_d = host_le_offset(c, c->t);
     const bool rebin = (c->t % (uint32_t)c->p.rebin_every) == 0u;
-    if (!c->sums_clean) { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * G.sw * 8, c->stream)); }
-    c->sums_clean = false;
     // reorder folded into this sweep (rank pass) and the next two (scatter into the new order through 32-byte staging
     // records, read back): needs two more steps in this call, the order of the last reorder, the second particle copy,
     // and rebin_every >= 3
-    const bool stage = rebin && c->reorder_stage == 0 && c->have_order && c->tbase && !c->compact &&
+    const bool stage = phase == 0 && rebin && c->reorder_stage == 0 && c->have_order && c->tbase && !c->compact &&
                        !(c->debug & (MPC_DEBUG_NO_FUSE_GATHER | MPC_DEBUG_EAGER_CANONICAL | MPC_DEBUG_ATOMIC_SCATTER)) && k + 2 < nsteps &&
                        c->p.rebin_every >= 3;
-    if (n) {
-      {
+    if (phase != 2) {
+      G.t = c->t;
+      host_shift(c, c->t, G.s);
+      c->le_dprev = G.le_d;
+      G.le_d = host_le_offset(c, c->t);
+      if (!c->sums_clean) { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * G.sw * 8, c->stream)); }
+      c->sums_clean = false;
+      if (n) {
         const int io = c->reorder_stage == 1 ? IO_SCATTER : c->reorder_stage == 2 ? IO_AOS_IN : (stage ? IO_RANK : IO_PLAIN);
         FamilyTimer ft(c, io != IO_PLAIN ? F_SWEEPG : F_SWEEP);
         const int rc = launch_sweep(c, c->collide_pending, rebin && !stage, io, sp);
@@ -97,26 +100,31 @@ int steps_srd(mpc_ctx* c, int nsteps) {
         if (io == IO_SCATTER) c->reorder_stage = 2;
         else if (io == IO_AOS_IN) c->reorder_stage = 0;
       }
-      // all but the last step of the call: k_cell clears the sums it has read (the last step's stay for
-      // mpc_observables / mpc_get_cells)
-      const int zero = (k + 1 < nsteps) ? 1 : 0;
-      // a folded reorder scans compact counts that k_cell writes while it reads the sums anyway (the scan would otherwise
-      // read every cell's 24 bytes twice); the other reorders read the counts from the sums, before k_cell clears them
-      if (rebin && !stage) {
-        const int rc = do_reorder(c, false, (c->debug & MPC_DEBUG_EAGER_CANONICAL) != 0);
-        if (rc) return rc;
-      }
-      {
-        FamilyTimer ft(c, F_CELL);
-        const int rc = launch_cell(c, zero, stage ? c->cursor : nullptr);
-        if (rc) return rc;
-      }
-      if (stage) {
-        const int rc = do_reorder(c, true, false);
-        if (rc) return rc;
-      }
+      if (phase == 1) return MPC_OK;
+    }
+    // all but the last step of the call: k_cell clears the sums it has read (the last step's stay for
+    // mpc_observables / mpc_get_cells). Slab subdomains always clear: the neighbours add into these sums in the next sweep
+    const int zero = (k + 1 < nsteps || phase == 2) ? 1 : 0;
+    // a folded reorder scans compact counts that k_cell writes while it reads the sums anyway (the scan would otherwise
+    // read every cell's 24 bytes twice); the other reorders read the counts from the sums, before k_cell clears them
+    // (slab subdomains: always the compact counts: the sums of shared cells include the neighbours' particles)
+    const bool compact_counts = stage || G.sub;
+    if (rebin && !compact_counts && n) {
+      const int rc = do_reorder(c, false, (c->debug & MPC_DEBUG_EAGER_CANONICAL) != 0, false);
+      if (rc) return rc;
+    }
+    {   // (a slab subdomain without particles still has cells: its neighbours' particles in the shared layers)
+      FamilyTimer ft(c, F_CELL);
+      const int rc = (n || G.sub) ? launch_cell(c, zero, (rebin && compact_counts) ? c->cursor : nullptr) : MPC_OK;
+      if (rc) return rc;
+    }
+    if (rebin && compact_counts && n) {
+      const int rc = do_reorder(c, stage, false, true);
+      if (rc) return rc;
+    }
+    if (n || G.sub) {
       c->sums_clean = zero != 0;
-      c->collide_pending = true;
+      c->collide_pending = n != 0;
     }
     sp[0] = G.s[0]; sp[1] = G.s[1]; sp[2] = G.s[2];
     c->t++;
@@ -141,7 +149,7 @@ int set_state_impl(mpc_ctx* c, unsigned long long n, const float* const src[6], 
     else { const int rc = launch_iota(c); if (rc) return rc; }    // ids 0..n_max-1
   }
   CU(cudaMemsetAsync(c->nrange, 0, 8, c->stream));
-  c->n = n; c->t = step; c->have_state = true; c->have_cells = false; c->have_order = false; c->reorder_stage = 0;
+  c->n = n; c->t = step; c->have_state = true; c->have_cells = false; c->have_order = false; c->reorder_stage = 0; c->sub_open = false;
   c->order_canonical = true; c->order_spread = 0; c->collide_pending = false;
   return MPC_OK;
 }
@@ -204,6 +212,13 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   if (p->collision == 0 && p->conserve_L && p->thermostat) return MPC_EINVAL;
   if (p->collision == 1 && p->rebin_every != 1) return MPC_EINVAL;
   if (p->shear_rate != 0.0f && (nwall || p->collision == 1 || p->conserve_L)) return MPC_EINVAL;   // Lees-Edwards: periodic SRD only (U21)
+  const bool sub = p->sub_nz != 0 || p->sub_z0 != 0;
+  if (sub) {   // slab subdomain: periodic SRD -a without force, whole brick layers, one brick layer of halo
+    const int bz = p->brick[2];
+    if (nwall || p->collision != 0 || p->conserve_L || p->shear_rate != 0.0f || p->phantoms || p->solute_mass > 0.0f) return MPC_EINVAL;
+    if (p->g[0] != 0.0f || p->g[1] != 0.0f || p->g[2] != 0.0f) return MPC_EINVAL;
+    if (p->sub_z0 < 0 || p->sub_z0 >= cells[2] || p->sub_z0 % bz || p->sub_nz % bz || p->sub_nz < 2 * bz || p->sub_nz + 2 * bz > cells[2]) return MPC_EINVAL;
+  }
   mpc_ctx* c = new (std::nothrow) mpc_ctx();   // value-initialised: all zero
   if (!c) return MPC_ENOMEM;
   c->p = *p; c->seed = seed;
@@ -218,6 +233,7 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
     G.bs[d] = bs;
     G.L[d] = box[d]; G.n[d] = cells[d]; G.bc[d] = p->bc[d]; G.g[d] = p->g[d];
     G.m[d] = cells[d] + (p->bc[d] != 0 ? 2 : 0);
+    if (sub && d == 2) G.m[d] = p->sub_nz + 2 * p->brick[2];    // local layers: own + one brick layer of halo on either side
     G.mb[d] = (G.m[d] + p->brick[d] - 1) >> bs;
     nk *= (unsigned long long)G.mb[d] << bs;
     nbr *= (unsigned long long)G.mb[d];
@@ -228,7 +244,8 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
   c->tile_bytes = tile_cells * TILE_W * 4;
   c->three_ctas = 3 * (c->tile_bytes + 1024) <= 227 * 1024;
   c->fast_brick = (G.bs[0] == 4 && G.bs[1] == 4 && G.bs[2] == 3);
-  c->pow2_cells = wall < 0 && !(G.m[0] & (G.m[0] - 1)) && !(G.m[1] & (G.m[1] - 1)) && !(G.m[2] & (G.m[2] - 1));
+  c->pow2_cells = wall < 0 && !(G.m[0] & (G.m[0] - 1)) && !(G.m[1] & (G.m[1] - 1)) && (sub || !(G.m[2] & (G.m[2] - 1)));
+  if (sub) { G.sub = 1; G.nzg = cells[2]; G.zoff = p->sub_z0 - p->brick[2]; G.nbz = G.mb[2]; }
   {
     const int bvs = G.bs[0] + G.bs[1] + G.bs[2];
     c->cell_cpb_shift = bvs > 8 ? bvs - 8 : 0;      // k_cell: CTAs of 256 cells
@@ -298,6 +315,8 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
   c->nsing = (u64*)(c->ws + l.off_obs + OBS_HOST_DOUBLES * 8);
   c->nrange = c->nsing + 1;
   c->G.nrange = c->nrange;
+  c->G.lcount = c->G.sub ? (uint32_t*)(c->ws + l.off_lcount) : nullptr;
+  c->G.peer[0] = c->G.peer[1] = nullptr;
   {   // table of the thermostat draw (cell.cuh)
     fill_mt_table(c->mt_host);
     CU(cudaMemcpyAsync(c->ws + l.off_mt, c->mt_host, MT_TABLE * 8, cudaMemcpyHostToDevice, c->stream));
@@ -339,9 +358,48 @@ int mpc_step(mpc_ctx* c, int nsteps) {
   if (!c || nsteps < 0) return MPC_EINVAL;
   if (c->sticky) return MPC_ECUDA;
   if (!c->bound || !c->have_state) return fail(c, MPC_ESTATE, "mpc_step before mpc_bind / mpc_set_state");
+  if (c->G.sub) return fail(c, MPC_ESTATE, "slab subdomain: use mpc_sub_begin / mpc_sub_end around the barrier of the ranks");
   CU(cudaSetDevice(c->device));
   return c->G.generic ? steps_generic(c, nsteps) : steps_srd(c, nsteps);
 }
+
+int mpc_sub_sums(mpc_ctx* c, void** sums_device, int* brick_layers) {
+  if (!c || !sums_device || !brick_layers) return MPC_EINVAL;
+  if (!c->G.sub) return fail(c, MPC_ESTATE, "not a slab subdomain");
+  if (!c->bound) return fail(c, MPC_ESTATE, "mpc_sub_sums before mpc_bind");
+  *sums_device = c->sums; *brick_layers = c->G.nbz;
+  return MPC_OK;
+}
+
+int mpc_sub_connect(mpc_ctx* c, void* sums_below, int brick_layers_below, void* sums_above, int brick_layers_above) {
+  if (!c || !sums_below || !sums_above || brick_layers_below < 4 || brick_layers_above < 4) return MPC_EINVAL;
+  if (c->sticky) return MPC_ECUDA;
+  if (!c->G.sub) return fail(c, MPC_ESTATE, "not a slab subdomain");
+  if (!c->bound) return fail(c, MPC_ESTATE, "mpc_sub_connect before mpc_bind");
+  CU(cudaSetDevice(c->device));
+  Geo& G = c->G;
+  const long long layer_keys = ((long long)G.mb[0] * G.mb[1]) << (G.bs[0] + G.bs[1] + G.bs[2]);   // keys of one brick layer
+  G.peer[0] = (u64*)sums_below; G.peer_koff[0] = (long long)(brick_layers_below - 2) * layer_keys;   // my layers 0, 1 = its last two
+  G.peer[1] = (u64*)sums_above; G.peer_koff[1] = -(long long)(G.nbz - 2) * layer_keys;              // my last two = its layers 0, 1
+  const int rc = launch_sub_clear(c);
+  if (rc) return rc;
+  c->sums_clean = true;
+  return MPC_OK;
+}
+
+static int sub_phase(mpc_ctx* c, int phase) {
+  if (!c) return MPC_EINVAL;
+  if (c->sticky) return MPC_ECUDA;
+  if (!c->G.sub) return fail(c, MPC_ESTATE, "not a slab subdomain");
+  if (!c->bound || !c->have_state || !c->G.peer[0]) return fail(c, MPC_ESTATE, "slab subdomain: needs mpc_bind, mpc_sub_connect and mpc_set_state first");
+  if ((phase == 1) == c->sub_open) return fail(c, MPC_ESTATE, "mpc_sub_begin and mpc_sub_end must alternate");
+  CU(cudaSetDevice(c->device));
+  const int rc = steps_srd(c, 1, phase);
+  if (rc == MPC_OK) c->sub_open = (phase == 1);
+  return rc;
+}
+int mpc_sub_begin(mpc_ctx* c) { return sub_phase(c, 1); }
+int mpc_sub_end(mpc_ctx* c) { return sub_phase(c, 2); }
 
 int mpc_get_state(mpc_ctx* c, float* x, float* y, float* z, float* vx, float* vy, float* vz, unsigned* id) {
   float* const dst[6] = {x, y, z, vx, vy, vz};

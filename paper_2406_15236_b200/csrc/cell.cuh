@@ -144,7 +144,14 @@ __device__ __forceinline__ void cell_batch(const Geo& G, uint32_t bx, uint32_t b
   u64 w0 = 0ull;
   if (valid) w0 = s[0];
   const uint32_t nreal = (uint32_t)(w0 & 0xffffull);
-  if (counts && valid) counts[kbase + tid] = nreal;      // compact per-cell counts for the scan of a folded reorder
+  if (G.sub && valid && sub_shared(G, (int)((bz << b2) | (local >> (b0 + b1)))) >= 0) {
+    // slab subdomain: the count in the (now complete) sums of a shared cell includes the neighbour's particles; the local
+    // reorder needs this rank's own count
+    const uint32_t mine = G.lcount[kbase + tid];
+    if (counts) counts[kbase + tid] = mine;
+    if (zero && mine) G.lcount[kbase + tid] = 0u;
+  } else
+  if (counts && valid) counts[kbase + tid] = nreal;      // compact per-cell counts for the scan of a reorder
   CellWork cw = {0.f, 0.f, 0.f, 0.f, 0u, 0u};
   if (valid && nreal != 0u) {
     const int ix = (int)((bx << b0) | (local & ((1u << b0) - 1u)));

@@ -484,7 +484,7 @@ int steps_generic(mpc_ctx* c, int nsteps) {
         LAUNCH_CHECK("k_stream_key");
       }
       if (rebin) {
-        const int rc = do_reorder(c, false, true);
+        const int rc = do_reorder(c, false, true, false);
         if (rc) return rc;
         F = reinterpret_cast<float**>(c->A);
         FamilyTimer ft(c, F_CELL);

@@ -92,6 +92,17 @@ struct Geo {
   float solute_mass;
   float wall_u;        // moving no-slip walls: +wall_u along x at L, -wall_u at 0 (U24)
   const float* mt_c;   // device table of MT_TABLE float pairs: (c, k)(N_c) of the thermostat draw (cell.cuh)
+  // Slab subdomain of a multi-GPU run: this context holds the cell layers
+  // [sub_z0 - bz, sub_z0 + sub_nz + bz) of a periodic box of nzg layers (bz = brick size along z: one brick layer of halo on
+  // either side); m[2] = local layers. Local layer = global layer - zoff (mod nzg). Cell sums of the four brick layers it
+  // shares with its two neighbours are ALSO added into the neighbours' arrays (integer REDs over peer memory), so that after
+  // a barrier every rank holds the complete sums of all its local cells.
+  int sub;              // 1 = slab subdomain
+  int zoff, nzg;        // first local layer (may be negative), global number of layers along z
+  int nbz;              // local brick layers along z
+  u64* peer[2];         // cell sums of the neighbour below / above (device pointers, peer memory)
+  long long peer_koff[2];   // key of a shared cell in that neighbour's array = local key + peer_koff
+  uint32_t* lcount;     // particle counts of THIS rank only, for the cells of the shared brick layers (indexed by local key)
 };
 
 // ---- packed sums ---------------------------------------------------------------------------------
@@ -124,12 +135,24 @@ __device__ __forceinline__ void key_to_cell(const Geo& G, uint32_t key, int& ix,
   iz = oz + (int)(local >> (b0 + b1));
 }
 __device__ __forceinline__ uint32_t canonical_id(const Geo& G, int ix, int iy, int iz) {
+  if (G.sub) {   // slab subdomain: the id of the cell in the whole box (every rank draws the same numbers for it)
+    iz += G.zoff;
+    iz += (iz < 0) ? G.nzg : 0;
+    iz -= (iz >= G.nzg) ? G.nzg : 0;
+  }
   return (uint32_t)ix + (uint32_t)G.m[0] * ((uint32_t)iy + (uint32_t)G.m[1] * (uint32_t)iz);
 }
 // cell coordinate of position r along axis d for lattice shift s
 __device__ __forceinline__ int cell_coord(const Geo& G, int d, float r, float s) {
   const float q = (r + s) * G.inv_a;
   int k = (int)floorf(q);
+  if (d == 2 && G.sub) {   // slab subdomain: local layer (clamped; the sweep counts particles outside the slab)
+    int t = k - G.zoff;
+    t += (t < 0) ? G.nzg : 0;
+    t -= (t >= G.nzg) ? G.nzg : 0;
+    t -= (t >= G.nzg) ? G.nzg : 0;
+    return min(t, G.m[2] - 1);
+  }
   if (G.bc[d] == 0) {
     if (k < 0) k += G.n[d];
     if (k >= G.n[d]) k -= G.n[d];
@@ -285,6 +308,21 @@ __device__ __forceinline__ int fold(int k, int m) {
   return k;
 }
 
+// ---- slab subdomain (Geo::sub) ---------------------------------------------------------------------
+// local layer of the global (unfolded, in [-1, nzg]) layer index kz; -1 if the layer is not held by this rank
+__device__ __forceinline__ int sub_layer(const Geo& G, int kz) {
+  int t = kz - G.zoff;
+  t += (t < 0) ? G.nzg : 0;
+  t -= (t >= G.nzg) ? G.nzg : 0;
+  t -= (t >= G.nzg) ? G.nzg : 0;
+  return (t < G.m[2]) ? t : -1;
+}
+// which neighbour shares the cell of local layer iz (0 below, 1 above, -1 none)
+__device__ __forceinline__ int sub_shared(const Geo& G, int iz) {
+  const int bl = iz >> G.bs[2];
+  return (bl <= 1) ? 0 : (bl >= G.nbz - 2) ? 1 : -1;
+}
+
 }  // namespace mpc
 
 // =================================================================================================
@@ -305,6 +343,7 @@ struct mpc_ctx {
   bool collide_pending;
   bool pow2_cells;      // no walls and every m[d] a power of two: the sweep folds indices with a mask
   int order_spread;     // log2 of the cells per group whose particles are stored lane-spread (spread_slot); 0 = plain cell order
+  bool sub_open;        // slab subdomain: mpc_sub_begin has run, mpc_sub_end has not
   int reorder_stage;    // folded reorder: 0 none in flight, 1 the next sweep scatters into the new order, 2 the next sweep reads the staged records
   float le_dprev;       // Lees-Edwards displacement of the step whose collision is pending
   unsigned debug;       // MPC_DEBUG_* flags
@@ -379,6 +418,7 @@ inline unsigned nblk(size_t n, int t) { return (unsigned)((n + t - 1) / t); }
 // sweep.cu
 enum { IO_PLAIN = 0, IO_RANK = 1, IO_SCATTER = 2, IO_AOS_IN = 3 };   // sweep.cu: the reorder folded into three sweeps
 int launch_sweep(mpc_ctx* c, bool collide, bool wkey, int io, const float sp[3]);
+int launch_sub_clear(mpc_ctx* c);
 cudaError_t sweep_set_attributes(size_t tile_bytes);
 int launch_collide_pos(mpc_ctx* c);
 int launch_keys(mpc_ctx* c, uint32_t* key_out);
@@ -386,7 +426,7 @@ int launch_keys(mpc_ctx* c, uint32_t* key_out);
 int launch_cell(mpc_ctx* c, int zero, uint32_t* counts);   // counts != nullptr: also writes the per-cell particle counts (one word per key)
 void fill_mt_table(float* host);
 // reorder.cu
-int do_reorder(mpc_ctx* c, bool defer_gather, bool canonical);
+int do_reorder(mpc_ctx* c, bool folded, bool canonical, bool counts_in_cursor);
 int canonicalise(mpc_ctx* c);
 int launch_iota(mpc_ctx* c);
 // generic.cu

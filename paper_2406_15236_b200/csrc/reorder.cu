@@ -263,11 +263,13 @@ int apply_perm(mpc_ctx* c) {
 // folded: the sweep of this step was the rank pass (IO_RANK): only the scan is done here, the next two sweeps move the
 //         particles (IO_SCATTER, IO_AOS_IN); otherwise c->key holds the keys and scatter + gather kernels run now
 // canonical: rank the particles of a cell by id now (needed by MPC-AT); otherwise group by key only
-int do_reorder(mpc_ctx* c, bool folded, bool canonical) {
+int do_reorder(mpc_ctx* c, bool folded, bool canonical, bool counts_in_cursor) {
   const size_t n = c->n, nk = c->G.nkeys, nb = (nk + SCAN_TILE - 1) / SCAN_TILE;
-  // folded: compact counts written by k_cell into c->cursor (the sums are already cleared)
-  const uint32_t* cnt = folded ? c->cursor : reinterpret_cast<const uint32_t*>(c->sums);
-  const int stride = folded ? 1 : c->G.sw * 2;
+  // counts_in_cursor: compact counts written by k_cell into c->cursor (the sums are already cleared); otherwise the low
+  // 16 bits of word 0 of the sums
+  const uint32_t* cnt = counts_in_cursor ? c->cursor : reinterpret_cast<const uint32_t*>(c->sums);
+  const int stride = counts_in_cursor ? 1 : c->G.sw * 2;
+  if (folded && !counts_in_cursor) return fail(c, MPC_ESTATE, "internal: folded reorder without compact counts");
   const int bvs = c->G.bs[0] + c->G.bs[1] + c->G.bs[2];
   if (folded && canonical) return fail(c, MPC_ESTATE, "internal: folded reorder cannot rank by id");
   // lane-spread order inside every group of 32 keys: hot path only, bricks of whole groups (spread_slot)

@@ -64,7 +64,9 @@ __device__ __forceinline__ int foldp(int k, int m) { return P2 ? (k & (m - 1)) :
 
 // SHEAR: Lees-Edwards boundary along z (U21); the few particles that collide as their image are binned at
 // x -+ D, usually far from their brick: they take the global path
-template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS, int IO, int T, bool P2, bool SHEAR>
+// SUB: slab subdomain of a multi-GPU run (Geo::sub): the z axis holds local layers and does not wrap; the sums of the cells
+// shared with a neighbour are also added into the neighbour's array (peer memory)
+template <bool COLLIDE, bool WALL, bool GRAV, bool WKEY, class BS, int IO, int T, bool P2, bool SHEAR, bool SUB = false>
 __global__ void __launch_bounds__(T, T <= 384 ? 3 : 2)
 k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
         float* __restrict__ vx, float* __restrict__ vy, float* __restrict__ vz, uint32_t* __restrict__ key_out,
@@ -154,7 +156,7 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       int kx = cell_raw(G, xp, sp0) + w0, ky = cell_raw(G, r[1], sp1) + w1, kz = cell_raw(G, r[2], sp2) + w2;
       if (WALL) { kx = G.bc[0] ? max(0, min(kx, m0 - 1)) : foldp<P2>(kx, m0); ky = G.bc[1] ? max(0, min(ky, m1 - 1)) : foldp<P2>(ky, m1);
                   kz = G.bc[2] ? max(0, min(kz, m2 - 1)) : foldp<P2>(kz, m2); }
-      else { kx = foldp<P2>(kx, m0); ky = foldp<P2>(ky, m1); kz = foldp<P2>(kz, m2); }
+      else { kx = foldp<P2>(kx, m0); ky = foldp<P2>(ky, m1); kz = SUB ? max(sub_layer(G, kz), 0) : foldp<P2>(kz, m2); }
       const uint32_t kp = BS::key(G, kx, ky, kz);
       float4 r0, ax;
       load_rec(rec, kp, r0, ax);
@@ -184,12 +186,16 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
     if (SHEAR) v[0] += vsn;        // the sums are taken in the frame of the image (v is not stored after this point)
     int cx = cell_raw(G, xn, G.s[0]) + w0, cy = cell_raw(G, r[1], G.s[1]) + w1, cz = cell_raw(G, r[2], G.s[2]) + w2;
     if (WALL) { if (G.bc[0]) cx = max(0, min(cx, m0 - 1)); if (G.bc[1]) cy = max(0, min(cy, m1 - 1)); if (G.bc[2]) cz = max(0, min(cz, m2 - 1)); }
+    if (SUB) {   // local layer; a particle outside the layers this rank holds invalidates the run (counted)
+      cz = sub_layer(G, cz);
+      if (cz < 0) { cz = 0; nbad++; }
+    }
     const int a0 = __float2int_rn(v[0] * G.fxv), a1 = __float2int_rn(v[1] * G.fxv), a2 = __float2int_rn(v[2] * G.fxv);
     const unsigned e = __float2uint_rn(fmaf(v[0], v[0], fmaf(v[1], v[1], v[2] * v[2])) * G.fxe);
     nbad += (e >= E_RANGE_LIMIT) ? 1u : 0u;     // |v| >= 8 u: outside the range of the fixed-point sums
     // tile coordinates: one fold takes care of the periodic image of the cell and of the tile origin
-    const int l0 = foldp<P2>(cx - ox, m0), l1 = foldp<P2>(cy - oy, m1), l2 = foldp<P2>(cz - oz, m2);
-    const bool inside = (l0 < T0) & (l1 < T1) & (l2 < T2);
+    const int l0 = foldp<P2>(cx - ox, m0), l1 = foldp<P2>(cy - oy, m1), l2 = SUB ? cz - oz : foldp<P2>(cz - oz, m2);
+    const bool inside = (l0 < T0) & (l1 < T1) & ((unsigned)l2 < (unsigned)T2);
     uint32_t word = 0;   // IO_RANK: rank word of the particle
     if (inside) {
       const int tc = (l2 * T1 + l1) * T0 + l0;
@@ -203,12 +209,20 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       atomicAdd((unsigned*)s + 4, e & ((1u << TILE_E_SHIFT) - 1u));
     }
     if (WKEY || !inside) {
-      const uint32_t kc = BS::key(G, foldp<P2>(cx, m0), foldp<P2>(cy, m1), foldp<P2>(cz, m2));
+      const uint32_t kc = BS::key(G, foldp<P2>(cx, m0), foldp<P2>(cy, m1), SUB ? cz : foldp<P2>(cz, m2));
       if (!inside) {
         u64* s = sums + (size_t)kc * G.sw;
         if (ranked) word = 0x80000000u | (uint32_t)(atomicAdd(s, ((u64)e << 16) | 1ull) & 0xffffull);
         else atomicAdd(s, ((u64)e << 16) | 1ull);
         atomicAdd(s + 1, pack_ss(a0, a1)); atomicAdd(s + 2, pack_ss(a2, 0));
+        if (SUB) {
+          const int side = sub_shared(G, cz);
+          if (side >= 0) {
+            u64* q = G.peer[side] + (size_t)((long long)kc + G.peer_koff[side]) * G.sw;
+            atomicAdd(q, ((u64)e << 16) | 1ull); atomicAdd(q + 1, pack_ss(a0, a1)); atomicAdd(q + 2, pack_ss(a2, 0));
+            atomicAdd(G.lcount + kc, 1u);
+          }
+        }
       }
       if (WKEY) key_out[i] = kc;
     }
@@ -232,13 +246,22 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       const int cnt = (int)((unsigned)s[0] & TILE_N_MASK);
       if (cnt == 0) continue;
       const int l0 = c % T0, q = c / T0, l1 = q % T1, l2 = q / T1;
-      u64* g = sums + (size_t)BS::key(G, foldp<P2>(ox + l0, m0), foldp<P2>(oy + l1, m1), foldp<P2>(oz + l2, m2)) * G.sw;
+      const uint32_t kf = BS::key(G, foldp<P2>(ox + l0, m0), foldp<P2>(oy + l1, m1), SUB ? oz + l2 : foldp<P2>(oz + l2, m2));
+      u64* g = sums + (size_t)kf * G.sw;
       const u64 etile = ((u64)((unsigned)s[0] >> TILE_N_BITS) << TILE_E_SHIFT) + (u64)(unsigned)s[4];
       const u64 w0 = (etile << 16) | (u64)(unsigned)cnt;
       if (ranked) old[k] = atomicAdd(g, w0);
       else atomicAdd(g, w0);
       atomicAdd(g + 1, pack_ss(s[1], s[2]));
       atomicAdd(g + 2, pack_ss(s[3], 0));
+      if (SUB) {   // the same sums into the neighbour that also holds this cell (integer adds commute: no staging, no ordering)
+        const int side = sub_shared(G, oz + l2);
+        if (side >= 0) {
+          u64* pq = G.peer[side] + (size_t)((long long)kf + G.peer_koff[side]) * G.sw;
+          atomicAdd(pq, w0); atomicAdd(pq + 1, pack_ss(s[1], s[2])); atomicAdd(pq + 2, pack_ss(s[3], 0));
+          atomicAdd(G.lcount + kf, (uint32_t)cnt);
+        }
+      }
       // partial momentum sums of >= 64 particles that come within a factor two of the int32 range
       if (cnt >= 64 && (abs(s[1]) >= (1 << 30) || abs(s[2]) >= (1 << 30) || abs(s[3]) >= (1 << 30))) atomicAdd(G.nrange, 1ull);
     }
@@ -295,6 +318,20 @@ void* sweep_fn(bool wall, bool grav, bool p2, bool shear) {
   if (grav) return (void*)k_sweep<COLLIDE, false, true, WKEY, BS, IO, T, false, false>;
   return (void*)k_sweep<COLLIDE, false, false, WKEY, BS, IO, T, false, false>;
 }
+// slab subdomains: periodic SRD without force; plain and key-writing sweeps only (local reorders are not folded)
+template <class BS>
+void* sweep_variant_sub(bool collide, bool wkey, bool three, bool p2) {
+  if (wkey) {
+    if (p2) return collide ? (void*)k_sweep<true, false, false, true, BS, IO_PLAIN, SWEEP_T, true, false, true> : (void*)k_sweep<false, false, false, true, BS, IO_PLAIN, SWEEP_T, true, false, true>;
+    return collide ? (void*)k_sweep<true, false, false, true, BS, IO_PLAIN, SWEEP_T, false, false, true> : (void*)k_sweep<false, false, false, true, BS, IO_PLAIN, SWEEP_T, false, false, true>;
+  }
+  if (three) {
+    if (p2) return collide ? (void*)k_sweep<true, false, false, false, BS, IO_PLAIN, SWEEP_T3, true, false, true> : (void*)k_sweep<false, false, false, false, BS, IO_PLAIN, SWEEP_T3, true, false, true>;
+    return collide ? (void*)k_sweep<true, false, false, false, BS, IO_PLAIN, SWEEP_T3, false, false, true> : (void*)k_sweep<false, false, false, false, BS, IO_PLAIN, SWEEP_T3, false, false, true>;
+  }
+  if (p2) return collide ? (void*)k_sweep<true, false, false, false, BS, IO_PLAIN, SWEEP_T, true, false, true> : (void*)k_sweep<false, false, false, false, BS, IO_PLAIN, SWEEP_T, true, false, true>;
+  return collide ? (void*)k_sweep<true, false, false, false, BS, IO_PLAIN, SWEEP_T, false, false, true> : (void*)k_sweep<false, false, false, false, BS, IO_PLAIN, SWEEP_T, false, false, true>;
+}
 template <class BS>
 void* sweep_variant(bool collide, bool wkey, int io, bool three, bool wall, bool grav, bool p2, bool shear) {
   if (io == IO_AOS_IN) return sweep_fn<true, false, BS, IO_AOS_IN, SWEEP_T>(wall, grav, p2, shear);   // 384 x 3: 15.8 instead of 14.4 ms
@@ -331,6 +368,10 @@ int launch_sweep(mpc_ctx* c, bool collide, bool wkey, int io, const float sp[3])
   const bool three = ((io == IO_PLAIN && !wkey) || io == IO_RANK) && c->three_ctas;   // rank pass: 14.8 instead of 15.9 ms
   sio.le_dprev = c->le_dprev;
   void* fn = sweep_variant_any(c->fast_brick, collide, wkey && io == IO_PLAIN, io, three, wall, grav, c->pow2_cells, G.shear != 0);
+  if (G.sub) {
+    if (io != IO_PLAIN) return fail(c, MPC_ESTATE, "internal: folded reorder on a slab subdomain");
+    fn = c->fast_brick ? sweep_variant_sub<BSfast>(collide, wkey, three, c->pow2_cells) : sweep_variant_sub<BSgeneric>(collide, wkey, three, false);
+  }
   float s0 = sp[0], s1 = sp[1], s2 = sp[2];
   uint32_t n = (uint32_t)c->n;
   void* args[] = {&G, &s0, &s1, &s2, &n, &F[0], &F[1], &F[2], &F[3], &F[4], &F[5], &c->key, &chunk, &c->nbricks, &c->rec, &c->sums, &sio};
@@ -341,6 +382,19 @@ int launch_sweep(mpc_ctx* c, bool collide, bool wkey, int io, const float sp[3])
 }
 
 cudaError_t sweep_set_attributes(size_t bytes) {
+  for (int m = 0; m < 16; ++m) {
+    const bool fast = m & 1, collide = m & 2, wkey = m & 4, alt = m & 8;   // alt: three CTAs (no keys) / power-of-two cell counts
+    void* fn = fast ? sweep_variant_sub<BSfast>(collide, wkey, !wkey && alt, wkey ? alt : false)
+                    : sweep_variant_sub<BSgeneric>(collide, wkey, !wkey && alt, false);
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e != cudaSuccess) return e;
+    if (fast && !wkey) {   // (three, p2) combinations of the fast brick
+      for (int t3 = 0; t3 < 2; ++t3) for (int p2 = 0; p2 < 2; ++p2) {
+        e = cudaFuncSetAttribute(sweep_variant_sub<BSfast>(collide, false, t3 != 0, p2 != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        if (e != cudaSuccess) return e;
+      }
+    }
+  }
   for (int mode = 0; mode < 6; ++mode) {          // bit 0: {16,16,8} brick; modes 2,3: power-of-two variant; 4,5: Lees-Edwards
     const bool fast = (mode & 1) != 0, p2 = (mode >> 1) == 1, shear = (mode >> 1) == 2;
     for (int wall = 0; wall < 2; ++wall)
@@ -357,6 +411,12 @@ cudaError_t sweep_set_attributes(size_t bytes) {
         }
   }
   return cudaSuccess;
+}
+
+int launch_sub_clear(mpc_ctx* c) {   // slab subdomain, before the first step: sums (the neighbours add into them) and local counts
+  if (cudaMemsetAsync(c->sums, 0, (size_t)c->G.nkeys * c->G.sw * 8, c->stream) != cudaSuccess ||
+      cudaMemsetAsync(c->G.lcount, 0, (size_t)c->G.nkeys * 4, c->stream) != cudaSuccess) return cuda_fail(c, cudaGetLastError(), "cudaMemsetAsync");
+  return MPC_OK;
 }
 
 int launch_collide_pos(mpc_ctx* c) {

@@ -1,0 +1,148 @@
+"""Slab subdomains (multi-GPU domain decomposition) on ONE GPU: R
+subdomain contexts in one process, run one after the other (nothing waits on anything: a barrier of the ranks is the
+end of a Python loop here), each adding the sums of its shared cells into its neighbours' arrays (device pointers: on
+several GPUs the same pointers are peer mappings). Integer sums commute and every cell draws its random numbers by its
+id in the whole box, so the decomposed trajectory must equal the single-domain one BIT FOR BIT."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2406_15236_b200 import MPC
+from paper_2406_15236_b200.binding import MPCError
+from paper_2406_15236_b200.inputs import uniform_maxwell
+from paper_2406_15236_b200.slab import slab_neighbours, slab_owner, slab_partition
+
+pytestmark = pytest.mark.gpu
+
+
+def to_dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def by_id(state):
+    s = [t.cpu().numpy() for t in state]
+    order = np.argsort(s[6].view(np.uint32))
+    return [a[order] for a in s]
+
+
+def make_ranks(box, cells, nbar, seed, st, world, brick, **kw):
+    parts = slab_partition(cells[2], world, brick[2])
+    a = box[2] / cells[2]
+    owner = slab_owner(st[2], a, parts)
+    ranks = []
+    for r, (z0, nz) in enumerate(parts):
+        sel = np.nonzero(owner == r)[0]
+        g = MPC(box, cells, nbar, seed, n_max=max(2 * len(sel), 1), brick=brick, sub=(z0, nz), **kw)
+        ranks.append((g, sel))
+    for r, (g, _) in enumerate(ranks):
+        below, above = slab_neighbours(r, world)
+        g.sub_connect(ranks[below][0].sub_sums(), ranks[above][0].sub_sums())
+    for g, sel in ranks:
+        g.set_state(*[to_dev(st[d][sel]) for d in range(6)], id=to_dev(st[6][sel].view(np.int32)))
+    return ranks
+
+
+def step_all(ranks, n):
+    for _ in range(n):
+        for g, _ in ranks:
+            g.sub_begin()
+        torch.cuda.synchronize()          # barrier of the ranks
+        for g, _ in ranks:
+            g.sub_end()
+        torch.cuda.synchronize()          # barrier of the ranks
+
+
+@pytest.mark.parametrize("world,cells,brick,kw", [
+    (2, (32, 16, 64), (16, 16, 8), dict(thermostat=1, rebin_every=5)),
+    (4, (32, 16, 64), (16, 16, 8), dict(thermostat=1, rebin_every=4)),
+    (3, (16, 16, 48), (16, 16, 8), dict(rebin_every=3)),
+    (2, (12, 10, 24), (4, 2, 4), dict(thermostat=1, rebin_every=2)),      # generic bricks, ragged x / y
+    (2, (32, 16, 32), (16, 16, 8), dict(thermostat=1, rebin_every=1)),    # every layer of the box is held by both ranks
+])
+def test_slabs_equal_the_single_domain_run_bit_for_bit(world, cells, brick, kw):
+    nbar = 10
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar - 7
+    st = uniform_maxwell(box, n, 11)
+    steps = 12
+    ref = MPC(box, cells, nbar, 77, n_max=n, brick=brick, **kw)
+    ref.set_state(*[to_dev(st[d]) for d in range(6)], id=to_dev(st[6].view(np.int32)))
+    ref.step(steps)
+    want = by_id(ref.get_state())
+    ranks = make_ranks(box, cells, nbar, 77, st, world, brick, **kw)
+    step_all(ranks, steps)
+    parts = [g.get_state() for g, _ in ranks]
+    got = by_id([torch.cat([p[d] for p in parts]) for d in range(7)])
+    assert np.array_equal(got[6], want[6])                       # nobody lost, nobody doubled
+    for d in range(6):
+        assert np.array_equal(got[d], want[d]), d                # positions and velocities: bit for bit
+    for g, _ in ranks:
+        ob = g.observables()
+        assert ob["n_range_overflows"] == 0 and ob["step"] == steps
+
+
+def test_particles_handed_to_their_owners_between_steps():
+    # the caller's part of PAPER.md:152 ("particles that have left the subdomain are sent to the new one when the particles
+    # are sorted"): read the states, deal the particles to their owners, set the states; the run continues bit for bit
+    world, cells, brick, nbar = 2, (16, 16, 48), (16, 16, 8), 10
+    kw = dict(thermostat=1, rebin_every=5, dt=0.5)              # a long step: particles cross the slab faces quickly
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    st = uniform_maxwell(box, n, 12)
+    ref = MPC(box, cells, nbar, 5, n_max=n, brick=brick, **kw)
+    ref.set_state(*[to_dev(st[d]) for d in range(6)], id=to_dev(st[6].view(np.int32)))
+    ranks = make_ranks(box, cells, nbar, 5, st, world, brick, **kw)
+    parts = slab_partition(cells[2], world, brick[2])
+    t = 0
+    for leg in range(4):
+        ref.step(5)
+        step_all(ranks, 5)
+        t += 5
+        states = [[a.cpu().numpy() for a in g.get_state()] for g, _ in ranks]
+        allp = [np.concatenate([s[d] for s in states]) for d in range(7)]
+        owner = slab_owner(allp[2], 1.0, parts)
+        moved = 0
+        for r, (g, _) in enumerate(ranks):
+            sel = np.nonzero(owner == r)[0]
+            moved += int((owner[:len(states[0][0])] != 0).sum()) if r == 0 else 0
+            g.set_state(*[to_dev(allp[d][sel]) for d in range(6)], id=to_dev(allp[6][sel].view(np.int32)), step=t)
+        assert moved > 0                                          # the test does exercise the hand-over
+    want = by_id(ref.get_state())
+    got = by_id([torch.cat([g.get_state()[d] for g, _ in ranks]) for d in range(7)])
+    for d in range(7):
+        assert np.array_equal(got[d], want[d]), d
+
+
+def test_a_particle_outside_its_slab_is_reported():
+    world, cells, brick, nbar = 2, (16, 16, 48), (16, 16, 8), 10
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    st = list(uniform_maxwell(box, n, 13))
+    ranks = make_ranks(box, cells, nbar, 5, st, world, brick, thermostat=1, rebin_every=5)
+    g, sel = ranks[0]
+    z = st[2][sel].copy()
+    z[0] = 40.5                                                   # rank 0 holds the layers 40..47 and 0..31: 40.5 is in its halo
+    z[1] = 36.0                                                   # ... but layer 36 is not held by rank 0
+    g.set_state(*[to_dev(a) for a in (st[0][sel], st[1][sel], z, st[3][sel], st[4][sel], st[5][sel])], id=to_dev(st[6][sel].view(np.int32)))
+    step_all(ranks, 1)
+    assert g.observables()["n_range_overflows"] == 1              # mpc_observables returns MPC_ERANGE: the run is invalid
+    assert ranks[1][0].observables()["n_range_overflows"] == 0
+
+
+def test_subdomain_rules():
+    box, cells = (32.0, 16.0, 64.0), (32, 16, 64)
+    for bad in (dict(sub=(0, 8)), dict(sub=(4, 32)), dict(sub=(0, 56)), dict(sub=(0, 32), bc=(0, 1, 0)), dict(sub=(0, 32), collision=1),
+                dict(sub=(0, 32), g=(0.01, 0, 0)), dict(sub=(0, 32), shear_rate=0.1)):
+        with pytest.raises(MPCError):
+            MPC(box, cells, 10, 1, n_max=100, brick=(16, 16, 8), **bad)
+    g = MPC(box, cells, 10, 1, n_max=100, brick=(16, 16, 8), sub=(0, 32))
+    with pytest.raises(MPCError):
+        g.sub_begin()                                             # not connected, no state
+    h = MPC(box, cells, 10, 1, n_max=100, brick=(16, 16, 8), sub=(32, 32))
+    g.sub_connect(h.sub_sums(), h.sub_sums())
+    z = torch.zeros(4, device="cuda")
+    g.set_state(z, z, z, z, z, z)
+    with pytest.raises(MPCError):
+        g.step(1)                                                 # mpc_step is for whole boxes
+    with pytest.raises(MPCError):
+        g.sub_end()                                               # begin first
