@@ -163,10 +163,18 @@ int mpc_step(mpc_ctx*, int nsteps);
  *                    must be reachable from this device (same device, or peer access / IPC mapping enabled by the caller)
  *   mpc_sub_begin    MOVE + sums of the next step (+ the pending collision). Then: barrier over all ranks
  *   mpc_sub_end      PROCESS_CELLS (+ the local reorder when due). Then: barrier over all ranks
+ *   mpc_sub_pack     between steps: the state split into the particles this rank keeps and those of its two neighbours
  * mpc_step returns MPC_ESTATE on a subdomain context. mpc_observables reports this rank's particles (kT_cell = 0). */
 int mpc_sub_sums(mpc_ctx*, void** sums_device, int* brick_layers);
 int mpc_sub_connect(mpc_ctx*, void* sums_below, int brick_layers_below, void* sums_above, int brick_layers_above);
 int mpc_sub_begin(mpc_ctx*);
+/* Particles by owner ("sent to the new subdomain when the particles are sorted"): applies the pending
+ * collision, then copies the state into the seven DEVICE arrays (capacity: the current particle count each) class by
+ * class: first the particles whose layer floor(z / a) is one of this rank's own, then those of the neighbour below,
+ * then those of the neighbour above; counts[0..2] (host) = the three class sizes. Synchronises the stream. The caller
+ * sends the two tails to the neighbours and gives mpc_set_state the particles it now owns. */
+int mpc_sub_pack(mpc_ctx*, float* x, float* y, float* z, float* vx, float* vy, float* vz, unsigned* id,
+                 unsigned long long counts[3]);
 int mpc_sub_end(mpc_ctx*);
 
 /* Diagnostic switches (change speed only, never results; the library reads no environment variables):

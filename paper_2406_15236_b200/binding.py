@@ -19,7 +19,7 @@ DEBUG_NO_FUSE_GATHER, DEBUG_EAGER_CANONICAL, DEBUG_ATOMIC_SCATTER, DEBUG_EAGER_C
 SYMBOLS = ["mpc_create", "mpc_num_keys", "mpc_workspace_bytes", "mpc_bind", "mpc_set_state", "mpc_set_state_host",
            "mpc_step", "mpc_set_debug", "mpc_get_state", "mpc_get_state_host", "mpc_observables", "mpc_get_cells",
            "mpc_philox4x32_10", "mpc_launch_count", "mpc_profile_enable", "mpc_profile_read", "mpc_last_error",
-           "mpc_destroy", "mpc_sub_sums", "mpc_sub_connect", "mpc_sub_begin", "mpc_sub_end"]
+           "mpc_destroy", "mpc_sub_sums", "mpc_sub_connect", "mpc_sub_begin", "mpc_sub_end", "mpc_sub_pack"]
 
 
 class mpc_params(C.Structure):
@@ -80,6 +80,7 @@ def load():
     L.mpc_sub_connect.argtypes = [vp, vp, C.c_int, vp, C.c_int]
     L.mpc_sub_begin.argtypes = [vp]
     L.mpc_sub_end.argtypes = [vp]
+    L.mpc_sub_pack.argtypes = [vp, fp, fp, fp, fp, fp, fp, up, C.POINTER(ull)]
     for s in SYMBOLS:
         getattr(L, s)
     _lib = L
@@ -119,7 +120,9 @@ class MPC:
     """One MPC system on one GPU. Tensors passed in/out are torch CUDA tensors (device API) or
     pinned/pageable host tensors / numpy arrays (the *_host API)."""
 
-    def __init__(self, box, cells, n_per_cell, seed, n_max, device="cuda:0", compact=False, stream=None, **kw):
+    def __init__(self, box, cells, n_per_cell, seed, n_max, device="cuda:0", compact=False, stream=None, workspace_alloc=None, **kw):
+        """workspace_alloc: optional callable bytes -> device pointer (int) for a workspace the caller owns (e.g. memory that
+        can be shared with other processes: slab_run.py); default: a torch uint8 tensor"""
         import torch
 
         self._torch = torch
@@ -140,9 +143,14 @@ class MPC:
         self._check(self.lib.mpc_workspace_bytes(self._h, self.n_max, 1 if compact else 0, C.byref(nbytes)))
         self.workspace_bytes = nbytes.value
         with torch.cuda.device(self.device):      # mpc_bind records the current device; later calls switch to it themselves
-            self.workspace = torch.empty(nbytes.value, dtype=torch.uint8, device=self.device)
+            if workspace_alloc is None:
+                self.workspace = torch.empty(nbytes.value, dtype=torch.uint8, device=self.device)
+                self.workspace_ptr = self.workspace.data_ptr()
+            else:
+                self.workspace = None
+                self.workspace_ptr = int(workspace_alloc(nbytes.value))
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-            self._check(self.lib.mpc_bind(self._h, C.c_void_p(self.workspace.data_ptr()), nbytes.value, self.n_max,
+            self._check(self.lib.mpc_bind(self._h, C.c_void_p(self.workspace_ptr), nbytes.value, self.n_max,
                                           C.c_void_p(self.stream.cuda_stream)))
 
     def _check(self, rc):
@@ -166,6 +174,16 @@ class MPC:
 
     def sub_end(self):
         self._check(self.lib.mpc_sub_end(self._h))
+
+    def sub_pack(self):
+        """the state class by class: ([x, y, z, vx, vy, vz, id] device tensors of the current length, (n_stay, n_below, n_above))"""
+        torch = self._torch
+        n = max(self.n, 1)
+        with torch.cuda.device(self.device):
+            out = [torch.empty(n, dtype=torch.float32, device=self.device) for _ in range(6)] + [torch.empty(n, dtype=torch.int32, device=self.device)]
+        cnt = (C.c_ulonglong * 3)()
+        self._check(self.lib.mpc_sub_pack(self._h, *[_ptr(t) for t in out], cnt))
+        return [t[:self.n] for t in out], tuple(int(v) for v in cnt)
 
     def close(self):
         if getattr(self, "_h", None):

@@ -398,6 +398,16 @@ static int sub_phase(mpc_ctx* c, int phase) {
   if (rc == MPC_OK) c->sub_open = (phase == 1);
   return rc;
 }
+int mpc_sub_pack(mpc_ctx* c, float* x, float* y, float* z, float* vx, float* vy, float* vz, unsigned* id, unsigned long long counts[3]) {
+  if (!c || !x || !y || !z || !vx || !vy || !vz || !id || !counts) return MPC_EINVAL;
+  if (c->sticky) return MPC_ECUDA;
+  if (!c->G.sub) return fail(c, MPC_ESTATE, "not a slab subdomain");
+  if (!c->have_state || c->sub_open) return fail(c, MPC_ESTATE, "mpc_sub_pack needs a state and no open step");
+  CU(cudaSetDevice(c->device));
+  { const int rc = flush_collide(c); if (rc) return rc; }
+  float* const out[6] = {x, y, z, vx, vy, vz};
+  return sub_pack_impl(c, out, id, counts);
+}
 int mpc_sub_begin(mpc_ctx* c) { return sub_phase(c, 1); }
 int mpc_sub_end(mpc_ctx* c) { return sub_phase(c, 2); }
 

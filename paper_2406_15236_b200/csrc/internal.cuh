@@ -433,6 +433,7 @@ int launch_iota(mpc_ctx* c);
 int steps_generic(mpc_ctx* c, int nsteps);
 // observe.cu
 int observables_impl(mpc_ctx* c, mpc_obs* out, float* profile_host, int n_profile);
+int sub_pack_impl(mpc_ctx* c, float* const out[6], unsigned* id_out, unsigned long long counts[3]);
 int get_cells_impl(mpc_ctx* c, unsigned* count, float* px, float* py, float* pz, float* e2, unsigned* key);
 // abi.cu
 int flush_collide(mpc_ctx* c);

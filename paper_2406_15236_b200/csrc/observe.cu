@@ -108,9 +108,76 @@ __global__ void __launch_bounds__(256) k_export_cells(Geo G, const u64* __restri
   if (e2) e2[k] = G.generic ? 0.0f : (float)((double)(s[0] >> 16) * G.fxe_inv);
 }
 
+// ---- slab subdomains: particles by owner ---------------------------------
+// class of a particle of a slab subdomain: 0 = its layer floor(z / a) is one of this rank's own, 1 / 2 = it belongs to the
+// neighbour below / above (the nearer one, periodically)
+__device__ __forceinline__ int sub_class(const Geo& G, float z) {
+  int l = __float2int_rd(z * G.inv_a);
+  l = max(0, min(l, G.nzg - 1));
+  const int z0 = G.zoff + (1 << G.bs[2]), nz = G.m[2] - (2 << G.bs[2]);      // own layers [z0, z0 + nz)
+  int up = l - z0; up += (up < 0) ? G.nzg : 0;                               // layers above the slab's first layer, periodic
+  if (up < nz) return 0;
+  return (up - nz < G.nzg - up) ? 2 : 1;
+}
+// counts[0..2] += particles per class; then, with cursor[0..2] set to the first slot of every class, the second kernel
+// writes the particles class by class (order inside a class: as it comes; the physics does not depend on it)
+__global__ void __launch_bounds__(256) k_sub_count(Geo G, size_t n, const float* __restrict__ z, uint32_t* __restrict__ counts) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int cl = (i < n) ? sub_class(G, z[i]) : 3;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const unsigned m = __ballot_sync(0xffffffffu, cl == k);
+    if (m && (threadIdx.x & 31) == (unsigned)(__ffs((int)m) - 1)) atomicAdd(counts + k, (uint32_t)__popc(m));
+  }
+}
+struct Arrays7 { const uint32_t* src[7]; uint32_t* dst[7]; };
+__global__ void __launch_bounds__(256) k_sub_split(Geo G, size_t n, Arrays7 a, uint32_t* __restrict__ cursor) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned lane = threadIdx.x & 31u;
+  const int cl = (i < n) ? sub_class(G, __uint_as_float(a.src[2][i])) : 3;
+  uint32_t slot = 0;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const unsigned m = __ballot_sync(0xffffffffu, cl == k);
+    if (!m) continue;
+    const int leader = __ffs((int)m) - 1;
+    uint32_t base = 0;
+    if ((int)lane == leader) base = atomicAdd(cursor + k, (uint32_t)__popc(m));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (cl == k) slot = base + (uint32_t)__popc(m & ((1u << lane) - 1u));
+  }
+  if (cl < 3) {
+#pragma unroll
+    for (int q = 0; q < 7; ++q) a.dst[q][slot] = a.src[q][i];
+  }
+}
+
 }  // namespace mpc
 
 using namespace mpc;
+
+int sub_pack_impl(mpc_ctx* c, float* const out[6], unsigned* id_out, unsigned long long counts[3]) {
+  const size_t n = c->n;
+  counts[0] = counts[1] = counts[2] = 0;
+  if (n == 0) return MPC_OK;
+  uint32_t h[3] = {0, 0, 0};
+  CU(cudaMemsetAsync(c->cursor, 0, 16, c->stream));
+  k_sub_count<<<nblk(n, 256), 256, 0, c->stream>>>(c->G, n, reinterpret_cast<const float*>(c->A[2]), c->cursor);
+  LAUNCH_CHECK("k_sub_count");
+  CU(cudaMemcpyAsync(h, c->cursor, 12, cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  const uint32_t base[3] = {0u, h[0], h[0] + h[1]};
+  CU(cudaMemcpyAsync(c->cursor, base, 12, cudaMemcpyHostToDevice, c->stream));
+  Arrays7 a;
+  for (int q = 0; q < 7; ++q) a.src[q] = c->A[q];
+  for (int q = 0; q < 6; ++q) a.dst[q] = reinterpret_cast<uint32_t*>(out[q]);
+  a.dst[6] = id_out;
+  k_sub_split<<<nblk(n, 256), 256, 0, c->stream>>>(c->G, n, a, c->cursor);
+  LAUNCH_CHECK("k_sub_split");
+  CU(cudaStreamSynchronize(c->stream));      // `base` is read by the copy above
+  for (int k = 0; k < 3; ++k) counts[k] = h[k];
+  return MPC_OK;
+}
 
 int observables_impl(mpc_ctx* c, mpc_obs* out, float* profile_host, int n_profile) {
   memset(out, 0, sizeof(*out));

@@ -146,3 +146,56 @@ def test_subdomain_rules():
         g.step(1)                                                 # mpc_step is for whole boxes
     with pytest.raises(MPCError):
         g.sub_end()                                               # begin first
+
+
+WORKER = r"""
+import os, sys
+import numpy as np
+import torch, torch.distributed as dist
+sys.path.insert(0, sys.argv[1])
+from paper_2406_15236_b200 import MPC
+from paper_2406_15236_b200.inputs import uniform_maxwell
+from paper_2406_15236_b200.slab_run import SlabRank
+rank, world = int(sys.argv[3]), int(sys.argv[4])
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:" + sys.argv[2], rank=rank, world_size=world)
+cells, nbar, brick = (16, 16, 64), 10, (16, 16, 8)
+box = tuple(float(c) for c in cells)
+n = int(np.prod(cells)) * nbar
+st = uniform_maxwell(box, n, 21)
+kw = dict(thermostat=1, rebin_every=5, dt=0.4)
+r = SlabRank(box, cells, nbar, 9, brick, n_max=n, device="cuda:0", **kw)
+r.set_global_state(st)
+r.step(17)                                 # hand-overs at t = 5, 10, 15
+got = r.gather_state()
+moved = r.migrate()
+if rank == 0:
+    ref = MPC(box, cells, nbar, 9, n_max=n, brick=brick, **kw)
+    ref.set_state(*[torch.from_numpy(st[d]).cuda() for d in range(6)], id=torch.from_numpy(st[6].view(np.int32)).cuda())
+    ref.step(17)
+    want = [t.cpu().numpy() for t in ref.get_state()]
+    order = np.argsort(want[6].view(np.uint32))
+    for d in range(7):
+        assert np.array_equal(got[d], want[d][order]), d
+assert r.sim.observables()["n_range_overflows"] == 0
+r.close()
+print("ok", rank, moved)
+"""
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_one_process_per_rank_with_ipc_mappings(world, tmp_path):
+    # the deployment path: one process per rank, the neighbours' workspaces mapped with CUDA IPC, a process group for the
+    # barriers and the hand-over of particles. All ranks share this box's one GPU (their kernels never wait on one
+    # another: the barriers are host-side), which exercises every line of the plumbing but measures nothing.
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "worker.py"
+    script.write_text(WORKER)
+    port = str(29700 + os.getpid() % 200 + world)
+    procs = [subprocess.Popen([sys.executable, str(script), root, port, str(r), str(world)], stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+             for r in range(world)]
+    outs = [p.communicate(timeout=600)[0] for p in procs]
+    for r, (p, o) in enumerate(zip(procs, outs)):
+        assert p.returncode == 0 and f"ok {r}" in o, o[-3000:]
