@@ -413,6 +413,11 @@ struct FamilyTimer {   // records an event pair around the launches of one kerne
   } while (0)
 
 inline unsigned nblk(size_t n, int t) { return (unsigned)((n + t - 1) / t); }
+// staging buffer of the reorder (32 bytes per particle): the unused SoA copy plus the slot array, which the workspace
+// layout places between the two copies so that either copy extends to 8 arrays (non-compact workspace only)
+inline float* aos_base(const mpc_ctx* c) {
+  return reinterpret_cast<float*>(c->A[0] < c->Bf[0] ? c->slot_id : c->Bf[0]);
+}
 
 // ---- entry points of the translation units ---------------------------------------------------------
 // sweep.cu

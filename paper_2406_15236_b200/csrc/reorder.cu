@@ -175,6 +175,63 @@ __global__ void __launch_bounds__(256) k_scatter_src(size_t n, const uint32_t* _
   }
 }
 
+// The same, moving the particles at once (non-compact workspace): instead of a permutation for a 7-fold random 4-byte
+// gather (k_gather<7>: 4.5 sectors of traffic per useful one, 208 ms at config 5), every particle is read where it is
+// (coalesced) and written as ONE 32-byte record {r, v, id, 0} at its slot of the staging buffer (a full sector);
+// k_unstage then copies the records back into the SoA arrays (coalesced both ways).
+struct Soa7 { const uint32_t* p[7]; };
+__global__ void __launch_bounds__(256) k_scatter_rec(size_t n, const uint32_t* __restrict__ key, const uint32_t* __restrict__ offset,
+                                                     uint32_t* __restrict__ cursor, Soa7 src, float* __restrict__ aos, int spread) {
+  const size_t base = (size_t)blockIdx.x * (256 * SCAT_U) + threadIdx.x;
+  const unsigned lane = threadIdx.x & 31u, le = 0xffffffffu >> (31u - lane);
+  uint32_t k[SCAT_U], slot[SCAT_U];
+  bool ok[SCAT_U];
+  int leader[SCAT_U], len[SCAT_U];
+#pragma unroll
+  for (int j = 0; j < SCAT_U; ++j) {
+    const size_t i = base + (size_t)j * 256;
+    ok[j] = i < n;
+    k[j] = ok[j] ? key[i] : 0u;
+  }
+#pragma unroll
+  for (int j = 0; j < SCAT_U; ++j) {   // runs of equal keys among neighbouring lanes (as in k_scatter_src)
+    const uint32_t kprev = __shfl_up_sync(0xffffffffu, k[j], 1);
+    const int okprev = __shfl_up_sync(0xffffffffu, (int)ok[j], 1);
+    const unsigned heads = __ballot_sync(0xffffffffu, lane == 0u || kprev != k[j] || okprev != (int)ok[j]);
+    leader[j] = 31 - __clz((int)(heads & le));
+    const unsigned above = heads & ~le;
+    len[j] = (above ? (__ffs((int)above) - 1) : 32) - leader[j];
+  }
+#pragma unroll
+  for (int j = 0; j < SCAT_U; ++j) {
+    slot[j] = 0;
+    if (ok[j] && (int)lane == leader[j]) slot[j] = atomicAdd(&cursor[k[j]], (uint32_t)len[j]);
+  }
+  uint32_t off[SCAT_U];
+#pragma unroll
+  for (int j = 0; j < SCAT_U; ++j) off[j] = ok[j] ? offset[k[j]] : 0u;
+#pragma unroll
+  for (int j = 0; j < SCAT_U; ++j) {
+    const uint32_t b = __shfl_sync(0xffffffffu, slot[j], leader[j]);
+    if (!ok[j]) continue;
+    const size_t i = base + (size_t)j * 256;
+    const uint32_t d = spread_key(offset, k[j], off[j] + b + (lane - (unsigned)leader[j]), spread);
+    const uint4 lo = make_uint4(src.p[0][i], src.p[1][i], src.p[2][i], src.p[3][i]);
+    const uint4 hi = make_uint4(src.p[4][i], src.p[5][i], src.p[6][i], 0u);
+    uint4* o = reinterpret_cast<uint4*>(aos + (size_t)d * 8);
+    o[0] = lo; o[1] = hi;
+  }
+}
+struct Soa7w { uint32_t* p[7]; };
+__global__ void __launch_bounds__(256) k_unstage(size_t n, const float* __restrict__ aos, Soa7w dst) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint4* r = reinterpret_cast<const uint4*>(aos + i * 8);
+  const uint4 lo = r[0], hi = r[1];
+  dst.p[0][i] = lo.x; dst.p[1][i] = lo.y; dst.p[2][i] = lo.z; dst.p[3][i] = lo.w;
+  dst.p[4][i] = hi.x; dst.p[5][i] = hi.y; dst.p[6][i] = hi.z;
+}
+
 // brick ranges of the old order, saved before the scan of a folded reorder overwrites the offsets: the scatter pass
 // (k_sweep<.., IO_SCATTER>) still walks the old order
 __global__ void __launch_bounds__(256) k_save_chunks(const uint32_t* __restrict__ offset, int bvol_shift, uint32_t nbricks,
@@ -186,7 +243,7 @@ __global__ void __launch_bounds__(256) k_save_chunks(const uint32_t* __restrict_
 // one thread per cell: the particles of segment [offset[k], offset[k+1]) ranked by id
 // (spread: the cell's particles sit at spread_slot() of the segment's positions)
 __global__ void __launch_bounds__(256) k_rank_cells(size_t nkeys, const uint32_t* __restrict__ offset, const uint32_t* __restrict__ id,
-                                                    uint32_t* __restrict__ perm, int spread) {
+                                                    uint32_t* __restrict__ perm, int spread, int inverse) {
   const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= nkeys) return;
   const uint32_t b = offset[k], e = offset[k + 1];
@@ -197,8 +254,18 @@ __global__ void __launch_bounds__(256) k_rank_cells(size_t nkeys, const uint32_t
     const uint32_t pj = spread_slot(j, g0, g1), me = id[pj];
     uint32_t r = 0;
     for (uint32_t m = b; m < e; ++m) r += (id[spread_slot(m, g0, g1)] < me) ? 1u : 0u;
-    perm[b + r] = pj;
+    if (inverse) perm[pj] = b + r;      // where the particle at pj goes
+    else perm[b + r] = pj;              // which particle comes to b + r
   }
+}
+// particle i goes to slot dest[i]: read where it is (coalesced), written as one 32-byte record (see k_scatter_rec)
+__global__ void __launch_bounds__(256) k_move_rec(size_t n, const uint32_t* __restrict__ dest, Soa7 src, float* __restrict__ aos) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint4 lo = make_uint4(src.p[0][i], src.p[1][i], src.p[2][i], src.p[3][i]);
+  const uint4 hi = make_uint4(src.p[4][i], src.p[5][i], src.p[6][i], 0u);
+  uint4* o = reinterpret_cast<uint4*>(aos + (size_t)dest[i] * 8);
+  o[0] = lo; o[1] = hi;
 }
 struct Arrays8 { void* p[8]; };
 template <int NA>
@@ -301,6 +368,23 @@ int do_reorder(mpc_ctx* c, bool folded, bool canonical, bool counts_in_cursor) {
       FamilyTimer ft(c, F_RANK);
       k_rank<<<nblk(n, 256), 256, 0, c->stream>>>(n, c->key, c->offset, slot2, c->perm);
       LAUNCH_CHECK("k_rank");
+    } else if (!c->compact) {   // group by key and move at once, through 32-byte records
+      {
+        FamilyTimer ft(c, F_SCATTER);
+        Soa7 src;
+        for (int a = 0; a < 7; ++a) src.p[a] = c->A[a];
+        k_scatter_rec<<<nblk(n, 256 * SCAT_U), 256, 0, c->stream>>>(n, c->key, c->offset, c->cursor, src, aos_base(c), spread);
+        LAUNCH_CHECK("k_scatter_rec");
+      }
+      FamilyTimer ft(c, F_GATHER);
+      Soa7w dst;
+      for (int a = 0; a < 7; ++a) dst.p[a] = c->A[a];
+      k_unstage<<<nblk(n, 256), 256, 0, c->stream>>>(n, aos_base(c), dst);
+      LAUNCH_CHECK("k_unstage");
+      c->have_order = true;
+      c->order_canonical = false;
+      c->order_spread = spread;
+      return MPC_OK;
     } else {
       FamilyTimer ft(c, F_SCATTER);
       k_scatter_src<<<nblk(n, 256 * SCAT_U), 256, 0, c->stream>>>(n, c->key, c->offset, c->cursor, c->perm, spread);
@@ -320,10 +404,20 @@ int canonicalise(mpc_ctx* c) {
   if (!c->have_order || c->order_canonical || c->n == 0) return MPC_OK;
   {
     FamilyTimer ft(c, F_RANK);
-    k_rank_cells<<<nblk(c->G.nkeys, 256), 256, 0, c->stream>>>(c->G.nkeys, c->offset, c->A[6], c->perm, c->order_spread);
+    k_rank_cells<<<nblk(c->G.nkeys, 256), 256, 0, c->stream>>>(c->G.nkeys, c->offset, c->A[6], c->perm, c->order_spread, c->compact ? 0 : 1);
     LAUNCH_CHECK("k_rank_cells");
   }
-  const int rc = apply_perm(c);
+  int rc = MPC_OK;
+  if (c->compact) rc = apply_perm(c);
+  else {   // through 32-byte records instead of a 7-fold random gather
+    FamilyTimer ftg(c, F_GATHER);
+    Soa7 src; Soa7w dst;
+    for (int a = 0; a < 7; ++a) { src.p[a] = c->A[a]; dst.p[a] = c->A[a]; }
+    k_move_rec<<<nblk(c->n, 256), 256, 0, c->stream>>>(c->n, c->perm, src, aos_base(c));
+    LAUNCH_CHECK("k_move_rec");
+    k_unstage<<<nblk(c->n, 256), 256, 0, c->stream>>>(c->n, aos_base(c), dst);
+    LAUNCH_CHECK("k_unstage");
+  }
   if (rc == MPC_OK) { c->order_canonical = true; c->order_spread = 0; }
   return rc;
 }

@@ -301,11 +301,6 @@ using namespace mpc;
 
 namespace {
 
-// staging buffer of the folded reorder (32 bytes per particle): the unused SoA copy plus the slot array, which
-// the workspace layout places between the two copies so that either copy extends to 8 arrays
-inline float* aos_base(const mpc_ctx* c) {
-  return reinterpret_cast<float*>(c->A[0] < c->Bf[0] ? c->slot_id : c->Bf[0]);
-}
 
 // the instantiations that exist: (COLLIDE, WKEY, IO) in { (*,0,PLAIN) at 384 or 512 threads, (*,1,PLAIN), (*,0,RANK),
 // (1,0,SCATTER), (1,0,AOS_IN) } x (WALL, GRAV) x brick shape
