@@ -295,6 +295,72 @@ def measure(args, workload, nbar, steps, warmup, rank, local_rank, world, dist, 
     return res, wl
 
 
+def measure_slabs(args, cells, nbar, world_sub, steps, warmup, rebin_every):
+    """Work inflation of the slab decomposition on ONE GPU: the box once as a whole and once as `world_sub`
+    slab subdomain contexts run one after the other (a barrier of the ranks = the end of a Python loop here), same seeded
+    input, same number of steps; both timed with CUDA events. Not a scaling number: nothing runs in parallel, there is no
+    NVLink in it. It says how much more work the ranks do together than the single-domain run."""
+    import torch
+
+    from paper_2406_15236_b200 import MPC
+    from paper_2406_15236_b200.inputs import uniform_maxwell_cuda
+    from paper_2406_15236_b200.slab import slab_neighbours, slab_partition
+
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    brick = (16, 16, 8)
+    kw = dict(thermostat=1, rebin_every=rebin_every, brick=brick)
+    st = list(uniform_maxwell_cuda(box, n, 4321, device="cuda:0", to_host=False))
+    out = {}
+    whole = MPC(box, cells, nbar, 99, n_max=n, **kw)
+    whole.set_state(*st)
+    whole.step(warmup)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(whole.stream); whole.step(steps); e1.record(whole.stream)
+    torch.cuda.synchronize()
+    out["whole_ms_per_step"] = e0.elapsed_time(e1) / steps
+    whole.close()
+    del whole
+    torch.cuda.empty_cache()
+    parts = slab_partition(cells[2], world_sub, brick[2])
+    layer = torch.floor(st[2]).to(torch.int64)                      # a = 1 in the bench boxes
+    ranks = []
+    for z0, nz in parts:
+        sel = torch.nonzero((layer >= z0) & (layer < z0 + nz)).flatten()
+        g = MPC(box, cells, nbar, 99, n_max=int(1.1 * sel.numel()) + 1024, sub=(z0, nz), **kw)
+        ranks.append((g, sel))
+    for r, (g, _) in enumerate(ranks):
+        below, above = slab_neighbours(r, world_sub)
+        g.sub_connect(ranks[below][0].sub_sums(), ranks[above][0].sub_sums())
+    for g, sel in ranks:
+        g.set_state(*[a[sel].contiguous() for a in st[:6]], id=sel.to(torch.int32))      # ids = index in the whole box
+    del st, layer
+    torch.cuda.empty_cache()
+
+    def run(k):
+        for _ in range(k):
+            for g, _ in ranks:
+                g.sub_begin()
+            for g, _ in ranks:
+                g.sub_end()
+
+    run(warmup)
+    torch.cuda.synchronize()
+    s = ranks[0][0].stream
+    e0.record(s); run(steps); e1.record(s)
+    torch.cuda.synchronize()
+    out["slabs_ms_per_step_summed_over_ranks"] = e0.elapsed_time(e1) / steps
+    out["ranks"] = world_sub
+    out["inflation"] = out["slabs_ms_per_step_summed_over_ranks"] / out["whole_ms_per_step"]
+    out["range_overflows"] = sum(int(g.observables()["n_range_overflows"]) for g, _ in ranks)
+    out["config"] = {"cells": list(cells), "n_per_cell": nbar, "particles": n, "rebin_every": rebin_every, "steps": steps, "warmup": warmup,
+                     "note": "one GPU, ranks run one after the other; local reorders of the subdomains are the unfolded ones, no hand-over of particles inside the timed steps"}
+    for g, _ in ranks:
+        g.close()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -310,6 +376,7 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the density sweep and the other workloads")
     ap.add_argument("--compact", action="store_true", help="property-wise reorder workspace")
     ap.add_argument("--debug", type=int, default=0, help="mpc_set_debug flags (A/B runs of the diagnostic code paths; changes speed only)")
+    ap.add_argument("--slabs", type=int, default=0, help="R >= 2: instead of the benchmark, time the box as a whole and as R slab subdomains on this one GPU (work inflation of the decomposition, DESIGN.md 9)")
     ap.add_argument("--cells", default=None, help="override the workload's cell grid, e.g. 256,256,256 (profiling runs)")
     args = ap.parse_args()
     wl = dict(WORKLOADS[args.workload])
@@ -340,6 +407,10 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
     torch.cuda.set_device(torch.device(f"cuda:{local_rank}"))
 
+    if args.slabs >= 2:
+        cells = cells_override or (512, 512, 256)
+        print(json.dumps({"slab_work_inflation": measure_slabs(args, cells, args.nbar, args.slabs, args.steps, args.warmup, wl["rebin_every"])}), flush=True)
+        return
     res, wl = measure(args, args.workload, args.nbar, args.steps, args.warmup, rank, local_rank, world, dist,
                       with_e2e=(not args.no_e2e and rank == 0 and world == 1), rebin_every=args.rebin_every,
                       cells_override=cells_override)
