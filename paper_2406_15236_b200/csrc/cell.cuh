@@ -132,6 +132,7 @@ __device__ __forceinline__ float mbs_kappa(const Geo& G, uint32_t cid, const Blo
 struct CellWork { float vx, vy, vz, w2; uint32_t cid, nc; };
 
 // CT cells [lbase, lbase + CT) of brick (bx, by, bz), one per thread of the CTA (all CT threads must call)
+template <bool SUB>
 __device__ __forceinline__ void cell_batch(const Geo& G, uint32_t bx, uint32_t by, uint32_t bz, uint32_t lbase, u64* __restrict__ sums,
                                            float* __restrict__ rec, int zero, uint32_t* __restrict__ counts) {
   const unsigned tid = threadIdx.x;
@@ -144,7 +145,7 @@ __device__ __forceinline__ void cell_batch(const Geo& G, uint32_t bx, uint32_t b
   u64 w0 = 0ull;
   if (valid) w0 = s[0];
   const uint32_t nreal = (uint32_t)(w0 & 0xffffull);
-  if (G.sub && valid && sub_shared(G, (int)((bz << b2) | (local >> (b0 + b1)))) >= 0) {
+  if (SUB && valid && sub_shared(G, (int)((bz << b2) | (local >> (b0 + b1)))) >= 0) {
     // slab subdomain: the count in the (now complete) sums of a shared cell includes the neighbour's particles; the local
     // reorder needs this rank's own count
     const uint32_t mine = G.lcount[kbase + tid];
@@ -157,7 +158,7 @@ __device__ __forceinline__ void cell_batch(const Geo& G, uint32_t bx, uint32_t b
     const int ix = (int)((bx << b0) | (local & ((1u << b0) - 1u)));
     const int iy = (int)((by << b1) | ((local >> b0) & ((1u << b1) - 1u)));
     const int iz = (int)((bz << b2) | (local >> (b0 + b1)));
-    cw.cid = canonical_id(G, ix, iy, iz);
+    cw.cid = SUB ? canonical_id_sub(G, ix, iy, iz) : canonical_id(G, ix, iy, iz);
     int sx, sy, sz, pad;
     unpack_ss(s[1], sx, sy);
     unpack_ss(s[2], sz, pad);

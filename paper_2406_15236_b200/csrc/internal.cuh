@@ -135,12 +135,14 @@ __device__ __forceinline__ void key_to_cell(const Geo& G, uint32_t key, int& ix,
   iz = oz + (int)(local >> (b0 + b1));
 }
 __device__ __forceinline__ uint32_t canonical_id(const Geo& G, int ix, int iy, int iz) {
-  if (G.sub) {   // slab subdomain: the id of the cell in the whole box (every rank draws the same numbers for it)
-    iz += G.zoff;
-    iz += (iz < 0) ? G.nzg : 0;
-    iz -= (iz >= G.nzg) ? G.nzg : 0;
-  }
   return (uint32_t)ix + (uint32_t)G.m[0] * ((uint32_t)iy + (uint32_t)G.m[1] * (uint32_t)iz);
+}
+// slab subdomain: the id of the cell in the whole box (every rank draws the same numbers for it); iz = local layer
+__device__ __forceinline__ uint32_t canonical_id_sub(const Geo& G, int ix, int iy, int iz) {
+  iz += G.zoff;
+  iz += (iz < 0) ? G.nzg : 0;
+  iz -= (iz >= G.nzg) ? G.nzg : 0;
+  return canonical_id(G, ix, iy, iz);
 }
 // cell coordinate of position r along axis d for lattice shift s
 __device__ __forceinline__ int cell_coord(const Geo& G, int d, float r, float s) {
