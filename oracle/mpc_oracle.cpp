@@ -3,7 +3,7 @@
 //
 // Plain, slow, single-threaded CPU restatement of one multiparticle-collision-dynamics
 // (MPC) time step as defined in /root/reference/PAPER.md (arXiv 2406.15236, "HTMPC"),
-// Sec. II, with the readings U1..U16 listed in DESIGN.md ("Readings of the paper").
+// Sec. II, with the readings U1..U24 listed in DESIGN.md ("Readings of the paper").
 // It exists to check the CUDA library (paper_2406_15236_b200/csrc) element by element.
 //
 //   * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
@@ -19,8 +19,10 @@
 //
 // Pins (tests/test_oracle_*.py): Philox known-answer vectors, the hand-computed SRD cell
 // of DESIGN.md, exact per-cell momentum / energy / angular-momentum invariants,
-// gamma-sampler moments, Maxwell statistics, the analytic SRD viscosity from a forced
-// Poiseuille profile. Parity unpinned: none; U7/U8 (wall details) pinned statistically.
+// the thermostat's gamma sampler (restated with exact rational arithmetic, bit for bit; moments,
+// KS, golden vector), Maxwell statistics, the analytic SRD viscosity from a forced Poiseuille
+// profile and from the Lees-Edwards shear stress. Parity unpinned: none; U7/U8 (wall details)
+// pinned by hand cases and statistically.
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off -fPIC -shared  (see oracle/build.py)
 // =====================================================================================

@@ -77,6 +77,7 @@ class SlabRank:
             ends.append((int(base) + info["offset"], info["layers"]))
         self.sim.sub_connect(ends[0], ends[1])
         self.t = 0
+        self._overflows = 0          # range overflows counted before earlier hand-overs (mpc_set_state restarts the library's count)
         self.barrier()
 
     # ---- plumbing ----
@@ -123,6 +124,7 @@ class SlabRank:
     def migrate(self):
         """particles that have left the rank's layers go to their new owner"""
         torch = self.torch
+        self._overflows += int(self.sim.observables()["n_range_overflows"])
         arrs, (n_stay, n_below, n_above) = self.sim.sub_pack()
         rows = torch.stack([a.view(torch.float32) for a in arrs], dim=1)          # (n, 7) bit patterns
         got = self._exchange(rows[n_stay:n_stay + n_below], rows[n_stay + n_below:n_stay + n_below + n_above])
@@ -143,6 +145,11 @@ class SlabRank:
             self.sim.sub_end()
             self.barrier()
             self.t += 1
+
+    def range_overflows(self):
+        """events in which a particle was outside the layers this rank holds (or a velocity outside the range of the
+        fixed-point sums) since the start of the run, on this rank; non-zero: the run is invalid (MPC_ERANGE)"""
+        return self._overflows + int(self.sim.observables()["n_range_overflows"])
 
     def gather_state(self):
         """the whole box on every rank, ordered by id (tests, output): [x, y, z, vx, vy, vz, id] numpy arrays"""
@@ -191,7 +198,7 @@ def main():
     r.set_global_state(st)
     r.step(a.steps)
     ob = r.sim.observables()
-    tot = torch.tensor([ob["n"], ob["E_kin"], ob["n_range_overflows"]], dtype=torch.float64)
+    tot = torch.tensor([ob["n"], ob["E_kin"], r.range_overflows()], dtype=torch.float64)
     if backend == "nccl":
         tot = tot.cuda()
     dist.all_reduce(tot)
