@@ -82,7 +82,7 @@ typedef struct {
                         Both multiples of brick[2]; sub_nz >= 2 brick[2]; sub_nz + 2 brick[2] <= cells[2]. Periodic SRD without +a,
                         walls, shear or force. The caller gives the rank the particles whose z lies in its layers; particles may
                         drift up to one brick layer outside (further: counted in n_range_overflows, results invalid); moving
-                        them to the owning rank is the caller's job between steps (mpc_get_state / mpc_set_state).
+                        them to the owning rank rides on the reorder (mpc_sub_begin) or is done with mpc_sub_pack.
                         See mpc_sub_connect, mpc_sub_begin, mpc_sub_end                                                        */
 } mpc_params;
 
@@ -118,6 +118,10 @@ int mpc_create(mpc_ctx** out, const float box[3], const int cells[3], float n_pe
 /* Number of keys K of the memory-order cell index (>= number of cells; brick padding and wall
  * layers included). Per-cell outputs of mpc_get_cells have K entries. */
 int mpc_num_keys(const mpc_ctx*, unsigned long long* nkeys);
+
+/* Current number of particles of the context: what mpc_set_state gave it; on a slab subdomain it changes when a reorder
+ * hands particles over (after the step that completes the reorder). Size mpc_get_state's arrays with it. */
+int mpc_num_particles(const mpc_ctx*, unsigned long long* n);
 
 /* Bytes of device workspace needed for up to n_max particles. `compact` = 0: reorder through a
  * second copy of the particle arrays (fastest); 1: reorder property-wise through one 4-byte-per-
@@ -158,18 +162,27 @@ int mpc_step(mpc_ctx*, int nsteps);
  * all its local cells, computes the same cell records from them as its neighbours do for the shared cells (the random
  * numbers are indexed by the cell's id in the whole box), and no particle is ever sent for a collision (the paper
  * exchanges the particles). The trajectory equals the single-GPU one bit for bit.
- *   mpc_sub_sums     device pointer and local brick-layer count of this rank's sums (to hand to its neighbours)
+ * Particles change owner at the reorder, inside its kernels: the reorder of a subdomain is the one folded
+ * into three sweeps; the particles whose cell of the reorder step lies in a halo layer are written by the
+ * scatter pass straight into the new owner's staging buffer (peer memory), behind the owner's own particles of the cell;
+ * the owner's read-back pass picks them up. This needs two further steps after the reorder step (steps_ahead below);
+ * a reorder without them stays local (unfolded) and hands nothing over. mpc_sub_pack is the explicit alternative.
+ *   mpc_sub_export   device pointers {cell sums, cell offsets, staging buffer (NULL: compact workspace)} and the local
+ *                    brick-layer count of this rank, to hand to its neighbours
  *   mpc_sub_connect  the neighbours' pointers and layer counts (below = towards smaller z); clears the sums. The memory
  *                    must be reachable from this device (same device, or peer access / IPC mapping enabled by the caller)
- *   mpc_sub_begin    MOVE + sums of the next step (+ the pending collision). Then: barrier over all ranks
- *   mpc_sub_end      PROCESS_CELLS (+ the local reorder when due). Then: barrier over all ranks
+ *   mpc_sub_begin    MOVE + sums of the next step (+ the pending collision). steps_ahead = how many further
+ *                    mpc_sub_begin calls the caller promises before it reads or replaces the state (mpc_get_state*,
+ *                    mpc_observables, mpc_sub_pack, mpc_set_state*; MPC_ESTATE while a folded reorder is in flight);
+ *                    all ranks must pass the same value. Then: barrier over all ranks
+ *   mpc_sub_end      PROCESS_CELLS (+ the scan of a reorder). Then: barrier over all ranks
  *   mpc_sub_pack     between steps: the state split into the particles this rank keeps and those of its two neighbours
  * mpc_step returns MPC_ESTATE on a subdomain context. mpc_observables reports this rank's particles (kT_cell = 0). */
-int mpc_sub_sums(mpc_ctx*, void** sums_device, int* brick_layers);
-int mpc_sub_connect(mpc_ctx*, void* sums_below, int brick_layers_below, void* sums_above, int brick_layers_above);
-int mpc_sub_begin(mpc_ctx*);
-/* Particles by owner ("sent to the new subdomain when the particles are sorted"): applies the pending
- * collision, then copies the state into the seven DEVICE arrays (capacity: the current particle count each) class by
+int mpc_sub_export(mpc_ctx*, void* device_ptrs[3], int* brick_layers);
+int mpc_sub_connect(mpc_ctx*, void* const below[3], int brick_layers_below, void* const above[3], int brick_layers_above);
+int mpc_sub_begin(mpc_ctx*, int steps_ahead);
+/* Particles by owner ("sent to the new subdomain when the particles are sorted"), explicitly: applies the
+ * pending collision, then copies the state into the seven DEVICE arrays (capacity: the current particle count each) class by
  * class: first the particles whose layer floor(z / a) is one of this rank's own, then those of the neighbour below,
  * then those of the neighbour above; counts[0..2] (host) = the three class sizes. Synchronises the stream. The caller
  * sends the two tails to the neighbours and gives mpc_set_state the particles it now owns. */

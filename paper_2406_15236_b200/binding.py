@@ -16,10 +16,10 @@ MPC_OK, MPC_EINVAL, MPC_ESTATE, MPC_ENOMEM, MPC_ECUDA, MPC_ERANGE = 0, -1, -2, -
 DEBUG_NO_FUSE_GATHER, DEBUG_EAGER_CANONICAL, DEBUG_ATOMIC_SCATTER, DEBUG_EAGER_COLLIDE, DEBUG_NO_LANE_SPREAD = 1, 2, 4, 8, 16
 
 # every symbol include/mpc_b200.h declares
-SYMBOLS = ["mpc_create", "mpc_num_keys", "mpc_workspace_bytes", "mpc_bind", "mpc_set_state", "mpc_set_state_host",
+SYMBOLS = ["mpc_create", "mpc_num_keys", "mpc_num_particles", "mpc_workspace_bytes", "mpc_bind", "mpc_set_state", "mpc_set_state_host",
            "mpc_step", "mpc_set_debug", "mpc_get_state", "mpc_get_state_host", "mpc_observables", "mpc_get_cells",
            "mpc_philox4x32_10", "mpc_launch_count", "mpc_profile_enable", "mpc_profile_read", "mpc_last_error",
-           "mpc_destroy", "mpc_sub_sums", "mpc_sub_connect", "mpc_sub_begin", "mpc_sub_end", "mpc_sub_pack"]
+           "mpc_destroy", "mpc_sub_export", "mpc_sub_connect", "mpc_sub_begin", "mpc_sub_end", "mpc_sub_pack"]
 
 
 class mpc_params(C.Structure):
@@ -57,6 +57,7 @@ def load():
     L.mpc_create.argtypes = [C.POINTER(vp), C.POINTER(C.c_float), C.POINTER(C.c_int), C.c_float,
                              C.POINTER(mpc_params), ull]
     L.mpc_num_keys.argtypes = [vp, C.POINTER(ull)]
+    L.mpc_num_particles.argtypes = [vp, C.POINTER(ull)]
     L.mpc_workspace_bytes.argtypes = [vp, ull, C.c_int, C.POINTER(C.c_size_t)]
     L.mpc_bind.argtypes = [vp, vp, C.c_size_t, ull, vp]
     L.mpc_set_state.argtypes = [vp, ull, fp, fp, fp, fp, fp, fp, up, C.c_uint]
@@ -76,9 +77,9 @@ def load():
     L.mpc_last_error.argtypes = [vp]
     L.mpc_last_error.restype = C.c_char_p
     L.mpc_destroy.argtypes = [vp]
-    L.mpc_sub_sums.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_int)]
-    L.mpc_sub_connect.argtypes = [vp, vp, C.c_int, vp, C.c_int]
-    L.mpc_sub_begin.argtypes = [vp]
+    L.mpc_sub_export.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_int)]
+    L.mpc_sub_connect.argtypes = [vp, C.POINTER(vp), C.c_int, C.POINTER(vp), C.c_int]
+    L.mpc_sub_begin.argtypes = [vp, C.c_int]
     L.mpc_sub_end.argtypes = [vp]
     L.mpc_sub_pack.argtypes = [vp, fp, fp, fp, fp, fp, fp, up, C.POINTER(ull)]
     for s in SYMBOLS:
@@ -137,7 +138,7 @@ class MPC:
         nk = C.c_ulonglong()
         self._check(self.lib.mpc_num_keys(self._h, C.byref(nk)))
         self.nkeys = nk.value
-        self.box, self.cells, self.n_max, self.n = tuple(box), tuple(cells), int(n_max), 0
+        self.box, self.cells, self.n_max = tuple(box), tuple(cells), int(n_max)
         self.device = torch.device(device)
         nbytes = C.c_size_t()
         self._check(self.lib.mpc_workspace_bytes(self._h, self.n_max, 1 if compact else 0, C.byref(nbytes)))
@@ -153,24 +154,32 @@ class MPC:
             self._check(self.lib.mpc_bind(self._h, C.c_void_p(self.workspace_ptr), nbytes.value, self.n_max,
                                           C.c_void_p(self.stream.cuda_stream)))
 
+    @property
+    def n(self):
+        """current number of particles (a slab subdomain's changes when a reorder hands particles over)"""
+        v = C.c_ulonglong()
+        self._check(self.lib.mpc_num_particles(self._h, C.byref(v)))
+        return int(v.value)
+
     def _check(self, rc):
         if rc != MPC_OK:
             msg = self.lib.mpc_last_error(self._h).decode() if self._h else ""
             raise MPCError(f"mpc error {rc}: {msg}")
 
     # ---- slab subdomains of a multi-GPU run (include/mpc_b200.h "slab subdomains") ----
-    def sub_sums(self):
-        """(device pointer, local brick layers) of this rank's cell sums, to hand to its two neighbours"""
-        p, nb = C.c_void_p(), C.c_int()
-        self._check(self.lib.mpc_sub_sums(self._h, C.byref(p), C.byref(nb)))
-        return p.value, nb.value
+    def sub_export(self):
+        """([cell sums, cell offsets, staging buffer] device pointers, local brick layers) of this rank, to hand to its neighbours"""
+        p, nb = (C.c_void_p * 3)(), C.c_int()
+        self._check(self.lib.mpc_sub_export(self._h, p, C.byref(nb)))
+        return [int(v or 0) for v in p], nb.value
 
     def sub_connect(self, below, above):
-        """below / above = sub_sums() of the neighbours towards smaller / larger z (peer memory reachable from this device)"""
-        self._check(self.lib.mpc_sub_connect(self._h, C.c_void_p(below[0]), below[1], C.c_void_p(above[0]), above[1]))
+        """below / above = sub_export() of the neighbours towards smaller / larger z (peer memory reachable from this device)"""
+        pb, pa = (C.c_void_p * 3)(*below[0]), (C.c_void_p * 3)(*above[0])
+        self._check(self.lib.mpc_sub_connect(self._h, pb, below[1], pa, above[1]))
 
-    def sub_begin(self):
-        self._check(self.lib.mpc_sub_begin(self._h))
+    def sub_begin(self, steps_ahead=0):
+        self._check(self.lib.mpc_sub_begin(self._h, int(steps_ahead)))
 
     def sub_end(self):
         self._check(self.lib.mpc_sub_end(self._h))
@@ -198,8 +207,7 @@ class MPC:
         ts = [x, y, z, vx, vy, vz]
         for t in ts:
             assert t.is_cuda and t.dtype == self._torch.float32 and t.is_contiguous()
-        self.n = ts[0].numel()
-        self._check(self.lib.mpc_set_state(self._h, self.n, *[_ptr(t) for t in ts], _ptr(id), step))
+        self._check(self.lib.mpc_set_state(self._h, ts[0].numel(), *[_ptr(t) for t in ts], _ptr(id), step))
 
     def set_state_host(self, x, y, z, vx, vy, vz, id=None, step=0):
         """Host arrays: numpy arrays or CPU torch tensors (pinned makes the copies asynchronous)."""
@@ -208,9 +216,8 @@ class MPC:
         for t in ts:
             assert (not t.is_cuda) and t.dtype == torch.float32 and t.is_contiguous()
         idt = None if id is None else torch.as_tensor(id)
-        self.n = ts[0].numel()
         self._keep = (ts, idt)
-        self._check(self.lib.mpc_set_state_host(self._h, self.n, *[_ptr(t) for t in ts], _ptr(idt), step))
+        self._check(self.lib.mpc_set_state_host(self._h, ts[0].numel(), *[_ptr(t) for t in ts], _ptr(idt), step))
 
     def step(self, nsteps=1):
         self._check(self.lib.mpc_step(self._h, int(nsteps)))

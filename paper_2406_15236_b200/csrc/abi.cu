@@ -14,7 +14,7 @@ namespace {
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  size_t off_A[7], off_B[7], off_key, off_slot, off_perm, off_cursor, off_offset, off_bsum, off_sums, off_lcount, off_rec, off_obs, off_mt,
+  size_t off_A[7], off_B[7], off_key, off_slot, off_perm, off_cursor, off_offset, off_bsum, off_sums, off_lcount, off_abase, off_rec, off_obs, off_mt,
       off_tbase, off_chunk0, total;
 };
 // tile_cells: cells of one brick's shared-memory tile; tbase (first slot of every CTA inside every tile cell's segment,
@@ -38,6 +38,7 @@ Layout make_layout(bool sub, size_t n_max, size_t nkeys, size_t nbricks, size_t 
   l.off_bsum = take(((nkeys + SCAN_TILE - 1) / SCAN_TILE + 1) * 4);
   l.off_sums = take(nkeys * (size_t)sw * 8);
   l.off_lcount = take(sub ? nkeys * 4 : 4);            // slab subdomain: this rank's own counts of the shared cells
+  l.off_abase = take(sub ? nkeys * 4 : 4);             // ... first slot of handed-over particles inside the owner's cell segment
   l.off_rec = take(nkeys * (size_t)rw * 4);
   l.off_obs = take(OBS_HOST_DOUBLES * 8 + 256);
   l.off_mt = take(MT_TABLE * 8);
@@ -75,16 +76,20 @@ float host_le_offset(const mpc_ctx* c, uint32_t t) {
 // 2 = PROCESS_CELLS and the local reorder (mpc_sub_begin / mpc_sub_end)
 int steps_srd(mpc_ctx* c, int nsteps, int phase = 0) {
   Geo& G = c->G;
-  const size_t n = c->n;
+  const size_t n = c->n;                           // (slab subdomains: c->n changes when a folded reorder completes; one step per call there)
   float sp[3] = {G.s[0], G.s[1], G.s[2]};          // shift of the pending step (if any)
   for (int k = 0; k < nsteps; ++k) {
     const bool rebin = (c->t % (uint32_t)c->p.rebin_every) == 0u;
     // reorder folded into this sweep (rank pass) and the next two (scatter into the new order through 32-byte staging
     // records, read back): needs two more steps in this call, the order of the last reorder, the second particle copy,
     // and rebin_every >= 3
-    const bool stage = phase == 0 && rebin && c->reorder_stage == 0 && c->have_order && c->tbase && !c->compact &&
-                       !(c->debug & (MPC_DEBUG_NO_FUSE_GATHER | MPC_DEBUG_EAGER_CANONICAL | MPC_DEBUG_ATOMIC_SCATTER)) && k + 2 < nsteps &&
-                       c->p.rebin_every >= 3;
+    // (slab subdomains: the caller promises the further steps in mpc_sub_begin; the folded reorder there also hands the
+    // particles of the halo layers over to their new owners)
+    bool stage = rebin && c->reorder_stage == 0 && c->have_order && c->tbase && !c->compact && n != 0 &&
+                 !(c->debug & (MPC_DEBUG_NO_FUSE_GATHER | MPC_DEBUG_EAGER_CANONICAL | MPC_DEBUG_ATOMIC_SCATTER)) &&
+                 (phase == 0 ? k + 2 < nsteps : c->sub_ahead >= 2) && c->p.rebin_every >= 3;
+    if (phase == 1) c->sub_stage = stage;
+    if (phase == 2) stage = c->sub_stage;
     if (phase != 2) {
       G.t = c->t;
       host_shift(c, c->t, G.s);
@@ -92,7 +97,14 @@ int steps_srd(mpc_ctx* c, int nsteps, int phase = 0) {
       G.le_d = host_le_offset(c, c->t);
       if (!c->sums_clean) { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * G.sw * 8, c->stream)); }
       c->sums_clean = false;
-      if (n) {
+      if (G.sub && c->reorder_stage == 2) {   // the new order holds the particles that have arrived, not those that have left
+        uint32_t nn = 0;
+        CU(cudaMemcpyAsync(&nn, c->offset + G.nkeys, 4, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        if (nn > c->n_max) return fail(c, MPC_ENOMEM, "slab subdomain: more particles have arrived than n_max holds");
+        c->n = nn;
+      }
+      if (c->n) {
         const int io = c->reorder_stage == 1 ? IO_SCATTER : c->reorder_stage == 2 ? IO_AOS_IN : (stage ? IO_RANK : IO_PLAIN);
         FamilyTimer ft(c, io != IO_PLAIN ? F_SWEEPG : F_SWEEP);
         const int rc = launch_sweep(c, c->collide_pending, rebin && !stage, io, sp);
@@ -115,7 +127,7 @@ int steps_srd(mpc_ctx* c, int nsteps, int phase = 0) {
     }
     {   // (a slab subdomain without particles still has cells: its neighbours' particles in the shared layers)
       FamilyTimer ft(c, F_CELL);
-      const int rc = (n || G.sub) ? launch_cell(c, zero, (rebin && compact_counts) ? c->cursor : nullptr) : MPC_OK;
+      const int rc = (n || G.sub) ? launch_cell(c, zero, (rebin && compact_counts) ? c->cursor : nullptr, G.sub && stage) : MPC_OK;
       if (rc) return rc;
     }
     if (rebin && compact_counts && n) {
@@ -157,6 +169,7 @@ int get_state_impl(mpc_ctx* c, float* const dst[6], unsigned* id, cudaMemcpyKind
   if (!c) return MPC_EINVAL;
   if (c->sticky) return MPC_ECUDA;
   if (!c->have_state) return fail(c, MPC_ESTATE, "mpc_get_state before mpc_set_state");
+  if (c->reorder_stage) return fail(c, MPC_ESTATE, "slab subdomain: a folded reorder is in flight (run the steps promised to mpc_sub_begin first)");
   CU(cudaSetDevice(c->device));
   { const int rc = flush_collide(c); if (rc) return rc; }
   { const int rc = canonicalise(c); if (rc) return rc; }
@@ -282,6 +295,12 @@ int mpc_num_keys(const mpc_ctx* c, unsigned long long* nkeys) {
   return MPC_OK;
 }
 
+int mpc_num_particles(const mpc_ctx* c, unsigned long long* n) {
+  if (!c || !n) return MPC_EINVAL;
+  *n = c->n;
+  return MPC_OK;
+}
+
 int mpc_workspace_bytes(const mpc_ctx* c, unsigned long long n_max, int compact, size_t* bytes) {
   if (!c || !bytes || n_max > 0xffffffffull) return MPC_EINVAL;
   *bytes = ctx_layout(c, (size_t)n_max, compact != 0).total;
@@ -316,6 +335,7 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
   c->nrange = c->nsing + 1;
   c->G.nrange = c->nrange;
   c->G.lcount = c->G.sub ? (uint32_t*)(c->ws + l.off_lcount) : nullptr;
+  c->G.abase = c->G.sub ? (uint32_t*)(c->ws + l.off_abase) : nullptr;
   c->G.peer[0] = c->G.peer[1] = nullptr;
   {   // table of the thermostat draw (cell.cuh)
     fill_mt_table(c->mt_host);
@@ -363,37 +383,44 @@ int mpc_step(mpc_ctx* c, int nsteps) {
   return c->G.generic ? steps_generic(c, nsteps) : steps_srd(c, nsteps);
 }
 
-int mpc_sub_sums(mpc_ctx* c, void** sums_device, int* brick_layers) {
-  if (!c || !sums_device || !brick_layers) return MPC_EINVAL;
+int mpc_sub_export(mpc_ctx* c, void* device_ptrs[3], int* brick_layers) {
+  if (!c || !device_ptrs || !brick_layers) return MPC_EINVAL;
   if (!c->G.sub) return fail(c, MPC_ESTATE, "not a slab subdomain");
-  if (!c->bound) return fail(c, MPC_ESTATE, "mpc_sub_sums before mpc_bind");
-  *sums_device = c->sums; *brick_layers = c->G.nbz;
+  if (!c->bound) return fail(c, MPC_ESTATE, "mpc_sub_export before mpc_bind");
+  device_ptrs[0] = c->sums; device_ptrs[1] = c->offset; device_ptrs[2] = c->compact ? nullptr : aos_base(c);
+  *brick_layers = c->G.nbz;
   return MPC_OK;
 }
 
-int mpc_sub_connect(mpc_ctx* c, void* sums_below, int brick_layers_below, void* sums_above, int brick_layers_above) {
-  if (!c || !sums_below || !sums_above || brick_layers_below < 4 || brick_layers_above < 4) return MPC_EINVAL;
+int mpc_sub_connect(mpc_ctx* c, void* const below[3], int brick_layers_below, void* const above[3], int brick_layers_above) {
+  if (!c || !below || !above || !below[0] || !above[0] || !below[1] || !above[1] || brick_layers_below < 4 || brick_layers_above < 4) return MPC_EINVAL;
   if (c->sticky) return MPC_ECUDA;
   if (!c->G.sub) return fail(c, MPC_ESTATE, "not a slab subdomain");
   if (!c->bound) return fail(c, MPC_ESTATE, "mpc_sub_connect before mpc_bind");
   CU(cudaSetDevice(c->device));
   Geo& G = c->G;
   const long long layer_keys = ((long long)G.mb[0] * G.mb[1]) << (G.bs[0] + G.bs[1] + G.bs[2]);   // keys of one brick layer
-  G.peer[0] = (u64*)sums_below; G.peer_koff[0] = (long long)(brick_layers_below - 2) * layer_keys;   // my layers 0, 1 = its last two
-  G.peer[1] = (u64*)sums_above; G.peer_koff[1] = -(long long)(G.nbz - 2) * layer_keys;              // my last two = its layers 0, 1
+  G.peer_koff[0] = (long long)(brick_layers_below - 2) * layer_keys;   // my layers 0, 1 = its last two
+  G.peer_koff[1] = -(long long)(G.nbz - 2) * layer_keys;               // my last two = its layers 0, 1
+  void* const* side[2] = {below, above};
+  for (int d = 0; d < 2; ++d) {
+    G.peer[d] = (u64*)side[d][0]; G.peer_offset[d] = (const uint32_t*)side[d][1]; G.peer_aos[d] = (float*)side[d][2];
+  }
+  if (!G.peer_aos[0] || !G.peer_aos[1] || c->compact) c->tbase = nullptr;   // no staging buffers: local reorders stay unfolded, hand-over by mpc_sub_pack
   const int rc = launch_sub_clear(c);
   if (rc) return rc;
   c->sums_clean = true;
   return MPC_OK;
 }
 
-static int sub_phase(mpc_ctx* c, int phase) {
-  if (!c) return MPC_EINVAL;
+static int sub_phase(mpc_ctx* c, int phase, int steps_ahead) {
+  if (!c || steps_ahead < 0) return MPC_EINVAL;
   if (c->sticky) return MPC_ECUDA;
   if (!c->G.sub) return fail(c, MPC_ESTATE, "not a slab subdomain");
   if (!c->bound || !c->have_state || !c->G.peer[0]) return fail(c, MPC_ESTATE, "slab subdomain: needs mpc_bind, mpc_sub_connect and mpc_set_state first");
   if ((phase == 1) == c->sub_open) return fail(c, MPC_ESTATE, "mpc_sub_begin and mpc_sub_end must alternate");
   CU(cudaSetDevice(c->device));
+  if (phase == 1) c->sub_ahead = steps_ahead;
   const int rc = steps_srd(c, 1, phase);
   if (rc == MPC_OK) c->sub_open = (phase == 1);
   return rc;
@@ -402,14 +429,14 @@ int mpc_sub_pack(mpc_ctx* c, float* x, float* y, float* z, float* vx, float* vy,
   if (!c || !x || !y || !z || !vx || !vy || !vz || !id || !counts) return MPC_EINVAL;
   if (c->sticky) return MPC_ECUDA;
   if (!c->G.sub) return fail(c, MPC_ESTATE, "not a slab subdomain");
-  if (!c->have_state || c->sub_open) return fail(c, MPC_ESTATE, "mpc_sub_pack needs a state and no open step");
+  if (!c->have_state || c->sub_open || c->reorder_stage) return fail(c, MPC_ESTATE, "mpc_sub_pack needs a state, no open step and no reorder in flight");
   CU(cudaSetDevice(c->device));
   { const int rc = flush_collide(c); if (rc) return rc; }
   float* const out[6] = {x, y, z, vx, vy, vz};
   return sub_pack_impl(c, out, id, counts);
 }
-int mpc_sub_begin(mpc_ctx* c) { return sub_phase(c, 1); }
-int mpc_sub_end(mpc_ctx* c) { return sub_phase(c, 2); }
+int mpc_sub_begin(mpc_ctx* c, int steps_ahead) { return sub_phase(c, 1, steps_ahead); }
+int mpc_sub_end(mpc_ctx* c) { return sub_phase(c, 2, 0); }
 
 int mpc_get_state(mpc_ctx* c, float* x, float* y, float* z, float* vx, float* vy, float* vz, unsigned* id) {
   float* const dst[6] = {x, y, z, vx, vy, vz};
@@ -424,6 +451,7 @@ int mpc_observables(mpc_ctx* c, mpc_obs* out, float* profile_host, int n_profile
   if (!c || !out) return MPC_EINVAL;
   if (c->sticky) return MPC_ECUDA;
   if (!c->have_state) return fail(c, MPC_ESTATE, "mpc_observables before mpc_set_state");
+  if (c->reorder_stage) return fail(c, MPC_ESTATE, "slab subdomain: a folded reorder is in flight (run the steps promised to mpc_sub_begin first)");
   CU(cudaSetDevice(c->device));
   { const int rc = flush_collide(c); if (rc) return rc; }
   return observables_impl(c, out, profile_host, n_profile);

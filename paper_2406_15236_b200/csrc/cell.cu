@@ -6,7 +6,7 @@ namespace mpc {
 // grid = (mb0 * CTAs-per-brick, mb1, mb2): the brick coordinates come from blockIdx, no division
 constexpr int PF_CTAS = 1024;   // about the number of resident CTAs (148 SMs x 5..6) and a bit
 template <int CT, bool SUB>
-__global__ void __launch_bounds__(CT) k_cell(Geo G, int cpb_shift, int ct_shift, u64* __restrict__ sums, float* __restrict__ rec, int zero, uint32_t* __restrict__ counts) {
+__global__ void __launch_bounds__(CT) k_cell(Geo G, int cpb_shift, int ct_shift, u64* __restrict__ sums, float* __restrict__ rec, int zero, uint32_t* __restrict__ counts, int handover) {
   // CTAs are dispatched in the order of their linear index L, and CTA L reads the CT cells from key L * CT on: pull the
   // sums of the CTA PF_CTAS further on into L2 now (every thread of this kernel loads once, computes for ~400
   // instructions, stores once: it is bound by the latency of that first load)
@@ -17,7 +17,7 @@ __global__ void __launch_bounds__(CT) k_cell(Geo G, int cpb_shift, int ct_shift,
       asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(sums + L * (size_t)(CT * G.sw)), "r"(bytes));
     }
   }
-  cell_batch<SUB>(G, blockIdx.x >> cpb_shift, blockIdx.y, blockIdx.z, (blockIdx.x & ((1u << cpb_shift) - 1u)) << ct_shift, sums, rec, zero, counts);
+  cell_batch<SUB>(G, blockIdx.x >> cpb_shift, blockIdx.y, blockIdx.z, (blockIdx.x & ((1u << cpb_shift) - 1u)) << ct_shift, sums, rec, zero, counts, handover);
 }
 
 }  // namespace mpc
@@ -32,9 +32,9 @@ void fill_mt_table(float* host) {
   }
 }
 
-int launch_cell(mpc_ctx* c, int zero, uint32_t* counts) {
-  if (c->G.sub) k_cell<256, true><<<c->cell_grid, 256, 0, c->stream>>>(c->G, c->cell_cpb_shift, 8, c->sums, c->rec, zero, counts);
-  else k_cell<256, false><<<c->cell_grid, 256, 0, c->stream>>>(c->G, c->cell_cpb_shift, 8, c->sums, c->rec, zero, counts);
+int launch_cell(mpc_ctx* c, int zero, uint32_t* counts, bool handover) {
+  if (c->G.sub) k_cell<256, true><<<c->cell_grid, 256, 0, c->stream>>>(c->G, c->cell_cpb_shift, 8, c->sums, c->rec, zero, counts, handover ? 1 : 0);
+  else k_cell<256, false><<<c->cell_grid, 256, 0, c->stream>>>(c->G, c->cell_cpb_shift, 8, c->sums, c->rec, zero, counts, 0);
   LAUNCH_CHECK("k_cell");
   return MPC_OK;
 }

@@ -134,7 +134,7 @@ struct CellWork { float vx, vy, vz, w2; uint32_t cid, nc; };
 // CT cells [lbase, lbase + CT) of brick (bx, by, bz), one per thread of the CTA (all CT threads must call)
 template <bool SUB>
 __device__ __forceinline__ void cell_batch(const Geo& G, uint32_t bx, uint32_t by, uint32_t bz, uint32_t lbase, u64* __restrict__ sums,
-                                           float* __restrict__ rec, int zero, uint32_t* __restrict__ counts) {
+                                           float* __restrict__ rec, int zero, uint32_t* __restrict__ counts, int handover) {
   const unsigned tid = threadIdx.x;
   const int b0 = G.bs[0], b1 = G.bs[1], b2 = G.bs[2];
   const uint32_t local = lbase + tid;
@@ -146,10 +146,17 @@ __device__ __forceinline__ void cell_batch(const Geo& G, uint32_t bx, uint32_t b
   if (valid) w0 = s[0];
   const uint32_t nreal = (uint32_t)(w0 & 0xffffull);
   if (SUB && valid && sub_shared(G, (int)((bz << b2) | (local >> (b0 + b1)))) >= 0) {
-    // slab subdomain: the count in the (now complete) sums of a shared cell includes the neighbour's particles; the local
-    // reorder needs this rank's own count
+    // slab subdomain: the count in the (now complete) sums of a shared cell includes the neighbour's particles.
+    // Unfolded local reorder (handover = 0): every particle stays, the scan needs this rank's own count. Folded reorder
+    // with hand-over (handover = 1): the particles in the halo layers leave (count 0; abase = the owner's own count, behind
+    // which they are placed in the owner's new order), those of the neighbour in this rank's own layers arrive (complete count)
     const uint32_t mine = G.lcount[kbase + tid];
-    if (counts) counts[kbase + tid] = mine;
+    const uint32_t bl = bz, nb = (uint32_t)G.nbz;
+    if (counts) {
+      if (!handover) counts[kbase + tid] = mine;
+      else if (bl == 0u || bl == nb - 1u) { counts[kbase + tid] = 0u; G.abase[kbase + tid] = nreal - mine; }
+      else counts[kbase + tid] = nreal;
+    }
     if (zero && mine) G.lcount[kbase + tid] = 0u;
   } else
   if (counts && valid) counts[kbase + tid] = nreal;      // compact per-cell counts for the scan of a reorder

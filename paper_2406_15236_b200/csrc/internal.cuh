@@ -103,6 +103,12 @@ struct Geo {
   u64* peer[2];         // cell sums of the neighbour below / above (device pointers, peer memory)
   long long peer_koff[2];   // key of a shared cell in that neighbour's array = local key + peer_koff
   uint32_t* lcount;     // particle counts of THIS rank only, for the cells of the shared brick layers (indexed by local key)
+  // hand-over of particles riding on the folded reorder (sweep.cu, IO_SCATTER): the neighbours' new cell offsets and staging
+  // buffers (peer memory), and for every cell of this rank's halo layers the neighbour's own count of the cell at the reorder
+  // step (the first slot, inside the cell's segment of the neighbour's new order, of the particles this rank hands over)
+  const uint32_t* peer_offset[2];
+  float* peer_aos[2];
+  uint32_t* abase;
 };
 
 // ---- packed sums ---------------------------------------------------------------------------------
@@ -346,6 +352,8 @@ struct mpc_ctx {
   bool pow2_cells;      // no walls and every m[d] a power of two: the sweep folds indices with a mask
   int order_spread;     // log2 of the cells per group whose particles are stored lane-spread (spread_slot); 0 = plain cell order
   bool sub_open;        // slab subdomain: mpc_sub_begin has run, mpc_sub_end has not
+  bool sub_stage;       // ... and it started a folded reorder with hand-over (decided in mpc_sub_begin, used by mpc_sub_end)
+  int sub_ahead;        // ... steps the caller has promised to run after the open one before it reads or replaces the state
   int reorder_stage;    // folded reorder: 0 none in flight, 1 the next sweep scatters into the new order, 2 the next sweep reads the staged records
   float le_dprev;       // Lees-Edwards displacement of the step whose collision is pending
   unsigned debug;       // MPC_DEBUG_* flags
@@ -430,7 +438,7 @@ cudaError_t sweep_set_attributes(size_t tile_bytes);
 int launch_collide_pos(mpc_ctx* c);
 int launch_keys(mpc_ctx* c, uint32_t* key_out);
 // cell.cu
-int launch_cell(mpc_ctx* c, int zero, uint32_t* counts);   // counts != nullptr: also writes the per-cell particle counts (one word per key)
+int launch_cell(mpc_ctx* c, int zero, uint32_t* counts, bool handover = false);   // counts != nullptr: also writes the per-cell particle counts (one word per key)
 void fill_mt_table(float* host);
 // reorder.cu
 int do_reorder(mpc_ctx* c, bool folded, bool canonical, bool counts_in_cursor);

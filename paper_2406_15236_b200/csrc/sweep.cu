@@ -150,6 +150,7 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       }
     }
     uint32_t slot = 0;   // IO_SCATTER: the particle's place in the new order
+    int leave_side = -1; // ... of the neighbour below / above, if the particle changes owner (slab subdomains)
     if (COLLIDE) {   // ROTATE_VELOCITIES of the previous step; its key is recomputed from r and that step's shift
       float vsp = 0.0f;
       const float xp = SHEAR ? le_image(G, r[0], r[2], sp2, io.le_dprev, vsp) : r[0];
@@ -164,10 +165,32 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
         slot = io.offset[kp];
         if (w & 0x80000000u) slot += w & 0xffffu;
         else {
-          const int l0 = foldp<P2>(kx - ox, m0), l1 = foldp<P2>(ky - oy, m1), l2 = foldp<P2>(kz - oz, m2);
+          const int l0 = foldp<P2>(kx - ox, m0), l1 = foldp<P2>(ky - oy, m1), l2 = SUB ? kz - oz : foldp<P2>(kz - oz, m2);
           slot += io.tbase[(size_t)b * tcells + (l2 * T1 + l1) * T0 + l0] + w;
         }
         if (io.spread) { const uint32_t kg = kp & ~((1u << io.spread) - 1u); slot = spread_slot(slot, io.offset[kg], io.offset[kg + (1u << io.spread)]); }
+        if (SUB) {
+          // hand-over riding on the reorder: a particle whose cell of the reorder step lies in a halo layer now
+          // belongs to the neighbour that owns the layer. Its record goes straight into that neighbour's staging buffer
+          // (peer memory), behind the neighbour's own particles of the cell: the neighbour's scan has left room for it
+          // (its count of the cell is the complete one), and abase = that neighbour's own count = complete - this rank's
+          const int bl = kz >> BS::s2(G);
+          const int side = (bl == 0) ? 0 : (bl == G.nbz - 1) ? 1 : -1;
+          if (side >= 0) {
+            const uint32_t* poff = G.peer_offset[side];
+            const uint32_t pk = (uint32_t)((long long)kp + G.peer_koff[side]);
+            uint32_t r_in_cell;
+            if (w & 0x80000000u) r_in_cell = w & 0xffffu;
+            else {
+              const int l0 = foldp<P2>(kx - ox, m0), l1 = foldp<P2>(ky - oy, m1), l2 = kz - oz;
+              r_in_cell = io.tbase[(size_t)b * tcells + (l2 * T1 + l1) * T0 + l0] + w;
+            }
+            uint32_t ps = poff[pk] + G.abase[kp] + r_in_cell;
+            if (io.spread) { const uint32_t kg = pk & ~((1u << io.spread) - 1u); ps = spread_slot(ps, poff[kg], poff[kg + (1u << io.spread)]); }
+            slot = ps;
+            leave_side = side;
+          }
+        }
       }
       if (SHEAR) v[0] += vsp;
       srd_apply(G, r0, ax, v);
@@ -176,7 +199,7 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
     stream_one<WALL, GRAV, SHEAR>(G, r, v);
     if (IO == IO_SCATTER) {
       const float q[8] = {r[0], r[1], r[2], v[0], v[1], v[2], idbits, 0.f};
-      st256(io.aos + (size_t)slot * 8, q);
+      st256(((SUB && leave_side >= 0) ? G.peer_aos[leave_side] : io.aos) + (size_t)slot * 8, q);
     } else {
       x[i] = r[0]; y[i] = r[1]; z[i] = r[2];
       vx[i] = v[0]; vy[i] = v[1]; vz[i] = v[2];
@@ -212,16 +235,17 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       const uint32_t kc = BS::key(G, foldp<P2>(cx, m0), foldp<P2>(cy, m1), SUB ? cz : foldp<P2>(cz, m2));
       if (!inside) {
         u64* s = sums + (size_t)kc * G.sw;
-        if (ranked) word = 0x80000000u | (uint32_t)(atomicAdd(s, ((u64)e << 16) | 1ull) & 0xffffull);
+        const int side = SUB ? sub_shared(G, cz) : -1;
+        // (a shared cell's count word also receives the neighbour's particles: this rank's own count, which numbers
+        // its particles inside the cell, is kept apart)
+        if (ranked && side < 0) word = 0x80000000u | (uint32_t)(atomicAdd(s, ((u64)e << 16) | 1ull) & 0xffffull);
         else atomicAdd(s, ((u64)e << 16) | 1ull);
         atomicAdd(s + 1, pack_ss(a0, a1)); atomicAdd(s + 2, pack_ss(a2, 0));
-        if (SUB) {
-          const int side = sub_shared(G, cz);
-          if (side >= 0) {
-            u64* q = G.peer[side] + (size_t)((long long)kc + G.peer_koff[side]) * G.sw;
-            atomicAdd(q, ((u64)e << 16) | 1ull); atomicAdd(q + 1, pack_ss(a0, a1)); atomicAdd(q + 2, pack_ss(a2, 0));
-            atomicAdd(G.lcount + kc, 1u);
-          }
+        if (SUB && side >= 0) {
+          u64* q = G.peer[side] + (size_t)((long long)kc + G.peer_koff[side]) * G.sw;
+          atomicAdd(q, ((u64)e << 16) | 1ull); atomicAdd(q + 1, pack_ss(a0, a1)); atomicAdd(q + 2, pack_ss(a2, 0));
+          if (ranked) word = 0x80000000u | (atomicAdd(G.lcount + kc, 1u) & 0xffffu);
+          else atomicAdd(G.lcount + kc, 1u);
         }
       }
       if (WKEY) key_out[i] = kc;
@@ -250,17 +274,16 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       u64* g = sums + (size_t)kf * G.sw;
       const u64 etile = ((u64)((unsigned)s[0] >> TILE_N_BITS) << TILE_E_SHIFT) + (u64)(unsigned)s[4];
       const u64 w0 = (etile << 16) | (u64)(unsigned)cnt;
-      if (ranked) old[k] = atomicAdd(g, w0);
+      const int side = SUB ? sub_shared(G, oz + l2) : -1;
+      if (ranked && side < 0) old[k] = atomicAdd(g, w0);
       else atomicAdd(g, w0);
       atomicAdd(g + 1, pack_ss(s[1], s[2]));
       atomicAdd(g + 2, pack_ss(s[3], 0));
-      if (SUB) {   // the same sums into the neighbour that also holds this cell (integer adds commute: no staging, no ordering)
-        const int side = sub_shared(G, oz + l2);
-        if (side >= 0) {
-          u64* pq = G.peer[side] + (size_t)((long long)kf + G.peer_koff[side]) * G.sw;
-          atomicAdd(pq, w0); atomicAdd(pq + 1, pack_ss(s[1], s[2])); atomicAdd(pq + 2, pack_ss(s[3], 0));
-          atomicAdd(G.lcount + kf, (uint32_t)cnt);
-        }
+      if (SUB && side >= 0) {   // the same sums into the neighbour that also holds this cell (integer adds commute: no staging, no ordering)
+        u64* pq = G.peer[side] + (size_t)((long long)kf + G.peer_koff[side]) * G.sw;
+        atomicAdd(pq, w0); atomicAdd(pq + 1, pack_ss(s[1], s[2])); atomicAdd(pq + 2, pack_ss(s[3], 0));
+        if (ranked) old[k] = (u64)atomicAdd(G.lcount + kf, (uint32_t)cnt);   // this rank's particles already numbered in the cell
+        else atomicAdd(G.lcount + kf, (uint32_t)cnt);
       }
       // partial momentum sums of >= 64 particles that come within a factor two of the int32 range
       if (cnt >= 64 && (abs(s[1]) >= (1 << 30) || abs(s[2]) >= (1 << 30) || abs(s[3]) >= (1 << 30))) atomicAdd(G.nrange, 1ull);
@@ -313,19 +336,19 @@ void* sweep_fn(bool wall, bool grav, bool p2, bool shear) {
   if (grav) return (void*)k_sweep<COLLIDE, false, true, WKEY, BS, IO, T, false, false>;
   return (void*)k_sweep<COLLIDE, false, false, WKEY, BS, IO, T, false, false>;
 }
-// slab subdomains: periodic SRD without force; plain and key-writing sweeps only (local reorders are not folded)
-template <class BS>
-void* sweep_variant_sub(bool collide, bool wkey, bool three, bool p2) {
-  if (wkey) {
-    if (p2) return collide ? (void*)k_sweep<true, false, false, true, BS, IO_PLAIN, SWEEP_T, true, false, true> : (void*)k_sweep<false, false, false, true, BS, IO_PLAIN, SWEEP_T, true, false, true>;
-    return collide ? (void*)k_sweep<true, false, false, true, BS, IO_PLAIN, SWEEP_T, false, false, true> : (void*)k_sweep<false, false, false, true, BS, IO_PLAIN, SWEEP_T, false, false, true>;
-  }
-  if (three) {
-    if (p2) return collide ? (void*)k_sweep<true, false, false, false, BS, IO_PLAIN, SWEEP_T3, true, false, true> : (void*)k_sweep<false, false, false, false, BS, IO_PLAIN, SWEEP_T3, true, false, true>;
-    return collide ? (void*)k_sweep<true, false, false, false, BS, IO_PLAIN, SWEEP_T3, false, false, true> : (void*)k_sweep<false, false, false, false, BS, IO_PLAIN, SWEEP_T3, false, false, true>;
-  }
-  if (p2) return collide ? (void*)k_sweep<true, false, false, false, BS, IO_PLAIN, SWEEP_T, true, false, true> : (void*)k_sweep<false, false, false, false, BS, IO_PLAIN, SWEEP_T, true, false, true>;
-  return collide ? (void*)k_sweep<true, false, false, false, BS, IO_PLAIN, SWEEP_T, false, false, true> : (void*)k_sweep<false, false, false, false, BS, IO_PLAIN, SWEEP_T, false, false, true>;
+// slab subdomains: periodic SRD without force
+template <class BS, bool P2>
+void* sweep_variant_sub2(bool collide, bool wkey, int io, bool three) {
+  if (io == IO_AOS_IN) return (void*)k_sweep<true, false, false, false, BS, IO_AOS_IN, SWEEP_T, P2, false, true>;
+  if (io == IO_SCATTER) return (void*)k_sweep<true, false, false, false, BS, IO_SCATTER, SWEEP_T, P2, false, true>;
+  if (io == IO_RANK) return collide ? (void*)k_sweep<true, false, false, false, BS, IO_RANK, SWEEP_T, P2, false, true> : (void*)k_sweep<false, false, false, false, BS, IO_RANK, SWEEP_T, P2, false, true>;
+  if (wkey) return collide ? (void*)k_sweep<true, false, false, true, BS, IO_PLAIN, SWEEP_T, P2, false, true> : (void*)k_sweep<false, false, false, true, BS, IO_PLAIN, SWEEP_T, P2, false, true>;
+  if (three) return collide ? (void*)k_sweep<true, false, false, false, BS, IO_PLAIN, SWEEP_T3, P2, false, true> : (void*)k_sweep<false, false, false, false, BS, IO_PLAIN, SWEEP_T3, P2, false, true>;
+  return collide ? (void*)k_sweep<true, false, false, false, BS, IO_PLAIN, SWEEP_T, P2, false, true> : (void*)k_sweep<false, false, false, false, BS, IO_PLAIN, SWEEP_T, P2, false, true>;
+}
+void* sweep_variant_sub(bool fast, bool collide, bool wkey, int io, bool three, bool p2) {
+  if (!fast) return sweep_variant_sub2<BSgeneric, false>(collide, wkey, io, three);
+  return p2 ? sweep_variant_sub2<BSfast, true>(collide, wkey, io, three) : sweep_variant_sub2<BSfast, false>(collide, wkey, io, three);
 }
 template <class BS>
 void* sweep_variant(bool collide, bool wkey, int io, bool three, bool wall, bool grav, bool p2, bool shear) {
@@ -363,31 +386,27 @@ int launch_sweep(mpc_ctx* c, bool collide, bool wkey, int io, const float sp[3])
   const bool three = ((io == IO_PLAIN && !wkey) || io == IO_RANK) && c->three_ctas;   // rank pass: 14.8 instead of 15.9 ms
   sio.le_dprev = c->le_dprev;
   void* fn = sweep_variant_any(c->fast_brick, collide, wkey && io == IO_PLAIN, io, three, wall, grav, c->pow2_cells, G.shear != 0);
-  if (G.sub) {
-    if (io != IO_PLAIN) return fail(c, MPC_ESTATE, "internal: folded reorder on a slab subdomain");
-    fn = c->fast_brick ? sweep_variant_sub<BSfast>(collide, wkey, three, c->pow2_cells) : sweep_variant_sub<BSgeneric>(collide, wkey, three, false);
-  }
+  const bool three_sub = io == IO_PLAIN && !wkey && c->three_ctas;       // (the rank pass of a subdomain runs 2 x 512)
+  if (G.sub) fn = sweep_variant_sub(c->fast_brick, collide, wkey && io == IO_PLAIN, io, three_sub, c->pow2_cells);
   float s0 = sp[0], s1 = sp[1], s2 = sp[2];
   uint32_t n = (uint32_t)c->n;
   void* args[] = {&G, &s0, &s1, &s2, &n, &F[0], &F[1], &F[2], &F[3], &F[4], &F[5], &c->key, &chunk, &c->nbricks, &c->rec, &c->sums, &sio};
-  const int T = three ? SWEEP_T3 : SWEEP_T;
+  const int T = (G.sub ? three_sub : three) ? SWEEP_T3 : SWEEP_T;
   cudaLaunchKernel(fn, dim3(c->nbricks), dim3(T), args, c->tile_bytes, c->stream);
   LAUNCH_CHECK("k_sweep");
   return MPC_OK;
 }
 
 cudaError_t sweep_set_attributes(size_t bytes) {
-  for (int m = 0; m < 16; ++m) {
-    const bool fast = m & 1, collide = m & 2, wkey = m & 4, alt = m & 8;   // alt: three CTAs (no keys) / power-of-two cell counts
-    void* fn = fast ? sweep_variant_sub<BSfast>(collide, wkey, !wkey && alt, wkey ? alt : false)
-                    : sweep_variant_sub<BSgeneric>(collide, wkey, !wkey && alt, false);
-    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-    if (e != cudaSuccess) return e;
-    if (fast && !wkey) {   // (three, p2) combinations of the fast brick
-      for (int t3 = 0; t3 < 2; ++t3) for (int p2 = 0; p2 < 2; ++p2) {
-        e = cudaFuncSetAttribute(sweep_variant_sub<BSfast>(collide, false, t3 != 0, p2 != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-        if (e != cudaSuccess) return e;
-      }
+  for (int m = 0; m < 8; ++m) {   // slab subdomain variants
+    const bool fast = m & 1, collide = m & 2, p2 = m & 4;
+    if (p2 && !fast) continue;
+    const struct { bool wkey; int io; bool three; } v[] = {{false, IO_PLAIN, false}, {false, IO_PLAIN, true}, {true, IO_PLAIN, false},
+                                                           {false, IO_RANK, false}, {false, IO_SCATTER, false}, {false, IO_AOS_IN, false}};
+    for (const auto& q : v) {
+      if (!collide && (q.io == IO_SCATTER || q.io == IO_AOS_IN)) continue;
+      const cudaError_t e = cudaFuncSetAttribute(sweep_variant_sub(fast, collide, q.wkey, q.io, q.three, p2), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+      if (e != cudaSuccess) return e;
     }
   }
   for (int mode = 0; mode < 6; ++mode) {          // bit 0: {16,16,8} brick; modes 2,3: power-of-two variant; 4,5: Lees-Edwards

@@ -55,10 +55,11 @@ class SlabRank:
 
         self.sim = MPC(box, cells, n_per_cell, seed, n_max=n_max, device=device, brick=brick, sub=self.parts[self.rank],
                        workspace_alloc=alloc, **kw)
-        # trade (IPC handle of the workspace, offset of the sums in it, local brick layers) with the neighbours
-        sums_ptr, layers = self.sim.sub_sums()
+        # trade (IPC handle of the workspace, offsets of the exported arrays in it, local brick layers) with the neighbours
+        ptrs, layers = self.sim.sub_export()
         handle = _ok(cudart.cudaIpcGetMemHandle(self.sim.workspace_ptr))
-        mine = dict(rank=self.rank, pid=os.getpid(), handle=bytes(handle.reserved), offset=sums_ptr - self.sim.workspace_ptr, layers=layers)
+        mine = dict(rank=self.rank, pid=os.getpid(), handle=bytes(handle.reserved),
+                    offsets=[(p - self.sim.workspace_ptr) if p else None for p in ptrs], layers=layers)
         everyone = [None] * self.world
         dist.all_gather_object(everyone, mine, group=group)
         self._opened = {}
@@ -74,7 +75,7 @@ class SlabRank:
                 h.reserved = info["handle"]
                 base = _ok(cudart.cudaIpcOpenMemHandle(h, cudart.cudaIpcMemLazyEnablePeerAccess))
                 self._opened[nb] = base
-            ends.append((int(base) + info["offset"], info["layers"]))
+            ends.append(([(int(base) + o) if o is not None else 0 for o in info["offsets"]], info["layers"]))
         self.sim.sub_connect(ends[0], ends[1])
         self.t = 0
         self._overflows = 0          # range overflows counted before earlier hand-overs (mpc_set_state restarts the library's count)
@@ -135,16 +136,23 @@ class SlabRank:
         return n_below + n_above
 
     def step(self, nsteps, migrate_every=None):
-        """advance nsteps; hand particles over every `migrate_every` steps (default: at every reorder step, just before it)"""
-        every = migrate_every or self.sim.params.rebin_every
-        for _ in range(nsteps):
-            if self.t > 0 and self.t % every == 0:
-                self.migrate()
-            self.sim.sub_begin()
-            self.barrier()
-            self.sim.sub_end()
-            self.barrier()
-            self.t += 1
+        """advance nsteps. Particles change owner inside the reorder's kernels (the library is told how many steps follow, so
+        that a reorder can fold its passes into them); migrate_every = m additionally hands them over explicitly
+        (mpc_sub_pack + the process group) before every m-th step"""
+        i = 0
+        while i < nsteps:
+            run = nsteps - i
+            if migrate_every:
+                if self.t > 0 and self.t % migrate_every == 0:
+                    self.migrate()
+                run = min(run, migrate_every - self.t % migrate_every)
+            for j in range(run):
+                self.sim.sub_begin(run - 1 - j)
+                self.barrier()
+                self.sim.sub_end()
+                self.barrier()
+                self.t += 1
+            i += run
 
     def range_overflows(self):
         """events in which a particle was outside the layers this rank holds (or a velocity outside the range of the

@@ -36,16 +36,17 @@ def make_ranks(box, cells, nbar, seed, st, world, brick, **kw):
         ranks.append((g, sel))
     for r, (g, _) in enumerate(ranks):
         below, above = slab_neighbours(r, world)
-        g.sub_connect(ranks[below][0].sub_sums(), ranks[above][0].sub_sums())
+        g.sub_connect(ranks[below][0].sub_export(), ranks[above][0].sub_export())
     for g, sel in ranks:
         g.set_state(*[to_dev(st[d][sel]) for d in range(6)], id=to_dev(st[6][sel].view(np.int32)))
     return ranks
 
 
-def step_all(ranks, n):
-    for _ in range(n):
+def step_all(ranks, n, ahead=None):
+    """n steps of all ranks; ahead: the steps promised to the library after each one (default: the rest of this call)"""
+    for i in range(n):
         for g, _ in ranks:
-            g.sub_begin()
+            g.sub_begin(n - 1 - i if ahead is None else ahead)
         torch.cuda.synchronize()          # barrier of the ranks
         for g, _ in ranks:
             g.sub_end()
@@ -80,6 +81,55 @@ def test_slabs_equal_the_single_domain_run_bit_for_bit(world, cells, brick, kw):
     for g, _ in ranks:
         ob = g.observables()
         assert ob["n_range_overflows"] == 0 and ob["step"] == steps
+
+
+def test_particles_change_owner_inside_the_reorder():
+    # PAPER.md:152, in the kernels: with a long step the particles cross the slab faces quickly; every folded reorder
+    # (t = 4, 8, ..., each with two further steps promised) writes the particles of the halo layers into the new owner's
+    # staging buffer. No call of the test moves a particle, and the run still equals the single-domain one bit for bit.
+    world, cells, brick, nbar = 3, (16, 16, 72), (16, 16, 8), 10
+    kw = dict(thermostat=1, rebin_every=4, dt=0.5)
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    st = uniform_maxwell(box, n, 14)
+    ref = MPC(box, cells, nbar, 6, n_max=n, brick=brick, **kw)
+    ref.set_state(*[to_dev(st[d]) for d in range(6)], id=to_dev(st[6].view(np.int32)))
+    ref.step(31)
+    want = by_id(ref.get_state())
+    ranks = make_ranks(box, cells, nbar, 6, st, world, brick, **kw)
+    first = [set(st[6][sel].tolist()) for _, sel in ranks]
+    step_all(ranks, 31)
+    parts = slab_partition(cells[2], world, brick[2])
+    states = [[a.cpu().numpy() for a in g.get_state()] for g, _ in ranks]
+    changed = 0
+    for r, s in enumerate(states):
+        ids = set(s[6].view(np.uint32).tolist())
+        changed += len(ids - first[r])
+        # every particle sits in its rank's own layers or has drifted there since the last hand-over (t = 28): within the halo
+        layer = np.floor(s[2]).astype(int)
+        z0, nz = parts[r]
+        up = (layer - z0) % cells[2]
+        assert np.all((up < nz + 8) | (up >= cells[2] - 8))
+        assert np.mean(up < nz) > 0.9
+    assert changed > 0.05 * n                                     # a good part of the particles has changed owner
+    got = by_id([np.concatenate([s[d] for s in states]) for d in range(7)])
+    for d in range(7):
+        assert np.array_equal(got[d], want[d]), d
+    for g, _ in ranks:
+        assert g.observables()["n_range_overflows"] == 0
+    # a reorder step without two further steps promised stays local; reading the state in the middle of a folded reorder is refused
+    step_all(ranks, 1, ahead=3)                                   # t = 31
+    step_all(ranks, 1, ahead=2)                                   # t = 32: reorder step, folded
+    with pytest.raises(MPCError):
+        ranks[0][0].get_state()
+    step_all(ranks, 2, ahead=0)
+    ranks[0][0].get_state()
+
+
+def by_id(state):
+    s = [t.cpu().numpy() if hasattr(t, "cpu") else t for t in state]
+    order = np.argsort(s[6].view(np.uint32))
+    return [a[order] for a in s]
 
 
 def test_particles_handed_to_their_owners_between_steps():
@@ -140,7 +190,7 @@ def test_subdomain_rules():
     with pytest.raises(MPCError):
         g.sub_begin()                                             # not connected, no state
     h = MPC(box, cells, 10, 1, n_max=100, brick=(16, 16, 8), sub=(32, 32))
-    g.sub_connect(h.sub_sums(), h.sub_sums())
+    g.sub_connect(h.sub_export(), h.sub_export())
     z = torch.zeros(4, device="cuda")
     g.set_state(z, z, z, z, z, z)
     with pytest.raises(MPCError):
