@@ -189,6 +189,7 @@ def main():
     ap.add_argument("--cells", default="64,64,128")
     ap.add_argument("--nbar", type=int, default=10)
     ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--rebin-every", type=int, default=10)
     ap.add_argument("--backend", default=None, help="default: nccl if every rank has its own GPU, else gloo")
     ap.add_argument("--one-gpu", action="store_true", help="all ranks on cuda:0 (functional test of the plumbing)")
@@ -204,14 +205,26 @@ def main():
     st = uniform_maxwell(box, n, 1234)
     r = SlabRank(box, cells, a.nbar, 1234, (16, 16, 8), n_max=int(2.5 * n / world) + 1024, device=f"cuda:{local}", thermostat=1, rebin_every=a.rebin_every)
     r.set_global_state(st)
+    r.step(a.warmup)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    r.barrier()
+    e0.record(r.sim.stream)
     r.step(a.steps)
+    e1.record(r.sim.stream)
+    r.barrier()
+    ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64)
+    if backend == "nccl":
+        ms = ms.cuda()
+    dist.all_reduce(ms, op=dist.ReduceOp.MAX)
     ob = r.sim.observables()
     tot = torch.tensor([ob["n"], ob["E_kin"], r.range_overflows()], dtype=torch.float64)
     if backend == "nccl":
         tot = tot.cuda()
     dist.all_reduce(tot)
     if rank == 0:
-        print(f"slab run: {world} ranks, {int(tot[0])} particles, {a.steps} steps, kT = {2 * float(tot[1]) / (3 * float(tot[0])):.5f}, range overflows = {int(tot[2])}")
+        print(f"slab run: {world} ranks, {int(tot[0])} particles, {a.steps} timed steps after {a.warmup}: {float(ms) / a.steps:.3f} ms per step = "
+              f"{float(tot[0]) * a.steps / (float(ms) * 1e-3):.4g} particle-updates/s (device time of the slowest rank, host barriers included), "
+              f"kT = {2 * float(tot[1]) / (3 * float(tot[0])):.5f}, range overflows = {int(tot[2])}")
     r.close()
     dist.destroy_process_group()
 
