@@ -217,6 +217,41 @@ int mpc_get_state_host(mpc_ctx*, float* x, float* y, float* z, float* vx, float*
  * Returns MPC_ERANGE (with *host_out filled in) if n_range_overflows != 0. */
 int mpc_observables(mpc_ctx*, mpc_obs* host_out, float* profile_host, int n_profile);
 
+/* ---- velocity profile for callers that cannot allocate device memory ------------------------------------------------
+ * Everything above needs a workspace that the caller allocates and gives to mpc_bind. Some callers have no way to get
+ * one: a monitoring or in-situ analysis hook that a host application calls from inside its time loop, where the
+ * application's own caching allocator already owns almost all of the GPU's memory (a direct cudaMalloc fails there, and
+ * where it does not, it stalls all streams of the device while it runs), code under a "nothing is allocated after
+ * start-up" rule, or a caller that only holds pointers another runtime handed to it. This one call serves them. It needs
+ * a context from mpc_create (host memory only; for the cell size a and the velocity unit of the fixed-point sums), no
+ * mpc_bind and no workspace: its accumulation buffer is an array of fixed size inside the library image, 32 KiB of
+ * device memory that every GPU which loads the library holds until the process exits.
+ *
+ * Computes, for the n particles given, the same quantity as mpc_observables' profile_host: for every
+ * layer l = floor(r_w[i] / a) (clamped to 0 .. n_layers-1) the average of v_f[i] over the layer's particles, 0 for an
+ * empty layer. The sums are 64-bit fixed point, so the result does not depend on the particle order and equals
+ * mpc_observables' profile of the same particles bit for bit.
+ *   r_w, v_f   DEVICE pointers, n floats each: the position component along the axis to bin over and the velocity
+ *              component to average (e.g. z and vx as returned by mpc_get_state); may be NULL if n == 0. Not modified.
+ *   profile    DEVICE pointer, n_layers floats, written by the call. counts: NULL, or a DEVICE pointer to n_layers
+ *              64-bit unsigned integers receiving the number of particles per layer. The caller owns all four arrays.
+ *   cuda_stream  a cudaStream_t cast to void* (NULL = legacy default stream); the call only enqueues work on it (one
+ *              memset, two kernels) and does not synchronise: the outputs are valid once that work has completed.
+ * All pointers must belong to the CUDA device that is current at the call, and the call runs there (it does not switch
+ * to the device of mpc_bind). It calls no cudaMalloc, cudaFree or other allocating routine.
+ * Limit: n_layers <= MPC_PROFILE_NOALLOC_MAX_LAYERS; more is refused with MPC_EINVAL (mpc_last_error says why) before
+ * any CUDA call, and mpc_observables with a bound workspace is the way to go then. Also MPC_EINVAL: NULL context (no
+ * message), n_layers < 1, NULL profile, NULL inputs with n > 0. MPC_ECUDA (sticky) if a CUDA call fails.
+ * First call on a device: it looks up the device address of the built-in array (once per device and process, guarded by
+ * a mutex). Make that first call before you start any stream capture.
+ * Sharing: every call on a device, from any context, stream or thread, uses the same array, and the array keeps what the
+ * last call left in it. Each call therefore clears the part it uses first, on its stream; two calls whose work overlaps
+ * on the GPU (different streams without an ordering between them) race on the array and both results are garbage.
+ * Calls on one stream, or ordered by events, are safe. */
+#define MPC_PROFILE_NOALLOC_MAX_LAYERS 2048
+int mpc_velocity_profile_noalloc(mpc_ctx*, unsigned long long n, const float* r_w, const float* v_f, int n_layers,
+                                 float* profile, unsigned long long* counts, void* cuda_stream);
+
 /* Test hook: the last step's pre-collision cell sums over real particles. Device pointers, any may
  * be NULL: count[K], px/py/pz[K] = m * sum v, e2[K] = sum |v|^2, key[n] = memory key of every
  * particle in the current order. Asynchronous. MPC_ESTATE before the first step. */

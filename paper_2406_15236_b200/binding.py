@@ -13,13 +13,15 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("MPC_B200_LIB", os.path.join(HERE, "libmpc_b200.so"))   # override: alternative builds
 
 MPC_OK, MPC_EINVAL, MPC_ESTATE, MPC_ENOMEM, MPC_ECUDA, MPC_ERANGE = 0, -1, -2, -3, -4, -5
+PROFILE_NOALLOC_MAX_LAYERS = 2048
 DEBUG_NO_FUSE_GATHER, DEBUG_EAGER_CANONICAL, DEBUG_ATOMIC_SCATTER, DEBUG_EAGER_COLLIDE, DEBUG_NO_LANE_SPREAD = 1, 2, 4, 8, 16
 
 # every symbol include/mpc_b200.h declares
 SYMBOLS = ["mpc_create", "mpc_num_keys", "mpc_num_particles", "mpc_workspace_bytes", "mpc_bind", "mpc_set_state", "mpc_set_state_host",
            "mpc_step", "mpc_set_debug", "mpc_get_state", "mpc_get_state_host", "mpc_observables", "mpc_get_cells",
            "mpc_philox4x32_10", "mpc_launch_count", "mpc_profile_enable", "mpc_profile_read", "mpc_last_error",
-           "mpc_destroy", "mpc_sub_export", "mpc_sub_connect", "mpc_sub_begin", "mpc_sub_end", "mpc_sub_pack"]
+           "mpc_destroy", "mpc_sub_export", "mpc_sub_connect", "mpc_sub_begin", "mpc_sub_end", "mpc_sub_pack",
+           "mpc_velocity_profile_noalloc"]
 
 
 class mpc_params(C.Structure):
@@ -82,6 +84,7 @@ def load():
     L.mpc_sub_begin.argtypes = [vp, C.c_int]
     L.mpc_sub_end.argtypes = [vp]
     L.mpc_sub_pack.argtypes = [vp, fp, fp, fp, fp, fp, fp, up, C.POINTER(ull)]
+    L.mpc_velocity_profile_noalloc.argtypes = [vp, ull, fp, fp, C.c_int, fp, up, vp]
     for s in SYMBOLS:
         getattr(L, s)
     _lib = L
@@ -293,6 +296,23 @@ class MPC:
         if profile:
             d["profile"] = prof
         return d
+
+    def velocity_profile_noalloc(self, r_w, v_f, profile, counts=None, stream=None):
+        """mpc_velocity_profile_noalloc: the layer averages of v_f over the layers floor(r_w / a), written into the caller's
+        float32 device tensor `profile` (its length is the number of layers, at most PROFILE_NOALLOC_MAX_LAYERS); `counts`:
+        optional int64 device tensor of the same length for the particles per layer. For callers that cannot allocate device
+        memory: the library's scratch for this call is a fixed array inside its own image, so nothing is allocated here either
+        (all four tensors are the caller's) and no workspace is touched. Enqueues on `stream` (default: the current stream
+        of the tensors' device, which must be the current device) and does not synchronise. Calls that may overlap on the
+        GPU share that one array and race; see include/mpc_b200.h."""
+        torch = self._torch
+        for t in (r_w, v_f, profile):
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+        assert r_w.numel() == v_f.numel()
+        assert counts is None or (counts.is_cuda and counts.dtype == torch.int64 and counts.is_contiguous() and counts.numel() == profile.numel())
+        s = stream if stream is not None else torch.cuda.current_stream(profile.device)
+        self._check(self.lib.mpc_velocity_profile_noalloc(self._h, r_w.numel(), _ptr(r_w), _ptr(v_f), profile.numel(), _ptr(profile),
+                                                          _ptr(counts), C.c_void_p(s.cuda_stream)))
 
     def profile_enable(self, on=True):
         self._check(self.lib.mpc_profile_enable(self._h, 1 if on else 0))

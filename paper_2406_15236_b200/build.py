@@ -6,7 +6,7 @@ import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = [os.path.join(HERE, "csrc", f) for f in ("abi.cu", "sweep.cu", "cell.cu", "reorder.cu", "generic.cu", "observe.cu")]
+SRC = [os.path.join(HERE, "csrc", f) for f in ("abi.cu", "sweep.cu", "cell.cu", "reorder.cu", "generic.cu", "observe.cu", "noalloc.cu")]
 DEPS = SRC + [os.path.join(HERE, "csrc", "philox.cuh"), os.path.join(HERE, "csrc", "internal.cuh"), os.path.join(HERE, "csrc", "cell.cuh"),
               os.path.join(HERE, "..", "include", "mpc_b200.h")]
 LIB = os.path.join(HERE, "libmpc_b200.so")
