@@ -25,7 +25,8 @@
  *     (mpc_observables, mpc_get_state_host) synchronise that stream; the others do not.
  *   - Particle arrays are fp32 structure-of-arrays x,y,z,vx,vy,vz plus a uint32 id per particle
  *     (PAPER.md:170). The internal particle order changes at every reorder; get_state returns the
- *     current internal order together with the ids (the caller un-permutes by id).
+ *     particles sorted by (memory key, id) as of the last reorder step, together with the ids (see
+ *     mpc_get_state; the caller un-permutes by id).
  *   - Not thread-safe per context; different contexts are independent.
  */
 #ifndef MPC_B200_H
@@ -100,8 +101,9 @@ typedef struct {
                                           fixed-point cell sums are sized for ("overflows may occur ...
                                           invalidating the results"): a particle with |v| >= 8 u, u = sqrt(kT/m) rounded
                                           to a power of two, or a momentum sum of >= 64 particles within a factor two of
-                                          the 32-bit range |sum v_d| < 512 u. Energy sums cannot overflow below 65535
-                                          particles per cell. 0 in every supported run                            */
+                                          the 32-bit range |sum v_d| < 512 u, or a cell with 2048 or more particles (the
+                                          count and energy fields of the sweep's shared-memory sums hold fewer than 2048
+                                          particles per cell; U19). 0 in every supported run              */
 } mpc_obs;
 
 /* Create a context. box[d] = L_d, cells[d] = number of fluid cells n_d; cells must be cubic
@@ -138,7 +140,8 @@ int mpc_bind(mpc_ctx*, void* workspace, size_t bytes, unsigned long long n_max, 
 /* Copy a state in. Device pointers (mpc_set_state) or host pointers (mpc_set_state_host), n each.
  * id == NULL numbers the particles 0..n-1; ids given must be unique. `step` sets the step counter
  * t (the RNG streams depend on it). Positions must lie in [0, L_d) on periodic axes and in
- * [0, L_d] on the wall axis. Asynchronous on the bound stream. */
+ * [0, L_d] on the wall axis. Asynchronous on the bound stream. MPC_ESTATE on a slab subdomain between mpc_sub_begin
+ * and mpc_sub_end or while a folded reorder is in flight (mpc_bind starts the context afresh). */
 int mpc_set_state(mpc_ctx*, unsigned long long n, const float* x, const float* y, const float* z,
                   const float* vx, const float* vy, const float* vz, const unsigned* id, unsigned step);
 int mpc_set_state_host(mpc_ctx*, unsigned long long n, const float* x, const float* y, const float* z,
@@ -170,12 +173,23 @@ int mpc_step(mpc_ctx*, int nsteps);
  *   mpc_sub_export   device pointers {cell sums, cell offsets, staging buffer (NULL: compact workspace)} and the local
  *                    brick-layer count of this rank, to hand to its neighbours
  *   mpc_sub_connect  the neighbours' pointers and layer counts (below = towards smaller z); clears the sums. The memory
- *                    must be reachable from this device (same device, or peer access / IPC mapping enabled by the caller)
+ *                    must be reachable from this device (same device, or peer access / IPC mapping enabled by the caller).
+ *                    A NULL staging pointer on either side (or a compact workspace here) turns the folded reorder off on this
+ *                    rank; a rank that folds beside one that does not would write particles where nobody reads them, so if ANY
+ *                    rank of the run exports no staging buffer the caller passes NULL for it on EVERY rank (slab_run.py does)
  *   mpc_sub_begin    MOVE + sums of the next step (+ the pending collision). steps_ahead = how many further
  *                    mpc_sub_begin calls the caller promises before it reads or replaces the state (mpc_get_state*,
  *                    mpc_observables, mpc_sub_pack, mpc_set_state*; MPC_ESTATE while a folded reorder is in flight);
- *                    all ranks must pass the same value. Then: barrier over all ranks
- *   mpc_sub_end      PROCESS_CELLS (+ the scan of a reorder). Then: barrier over all ranks
+ *                    all ranks must pass the same value. Then: barrier over all ranks. Whether a reorder is folded (and hands
+ *                    particles over) is decided by every rank on its own, so it must come out the same everywhere: besides
+ *                    steps_ahead, all ranks need the same mpc_set_debug flags, the same rebin_every, their mpc_set_state at the
+ *                    same step, and staging buffers on all ranks or on none (mpc_sub_connect)
+ *   mpc_sub_end      PROCESS_CELLS (+ the scan of a reorder). Then: barrier over all ranks. On the step of a folded reorder
+ *                    this call synchronises the stream (it reads the rank's new particle count) and returns MPC_ENOMEM if the
+ *                    hand-over would bring more particles than n_max: the context is then dead (every later call fails), and
+ *                    the caller must keep EVERY rank from starting the next step, since that step's kernels of this rank and
+ *                    of its neighbours write the arrivals into this rank's staging buffer (share the status at the barrier,
+ *                    as slab_run.py does). All other mpc_sub_begin / mpc_sub_end calls only enqueue work
  *   mpc_sub_pack     between steps: the state split into the particles this rank keeps and those of its two neighbours
  * mpc_step returns MPC_ESTATE on a subdomain context. mpc_observables reports this rank's particles (kT_cell = 0). */
 int mpc_sub_export(mpc_ctx*, void* device_ptrs[3], int* brick_layers);

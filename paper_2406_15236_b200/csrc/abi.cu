@@ -85,7 +85,10 @@ int steps_srd(mpc_ctx* c, int nsteps, int phase = 0) {
     // and rebin_every >= 3
     // (slab subdomains: the caller promises the further steps in mpc_sub_begin; the folded reorder there also hands the
     // particles of the halo layers over to their new owners)
-    bool stage = rebin && c->reorder_stage == 0 && c->have_order && c->tbase && !c->compact && n != 0 &&
+    // (a slab rank decides from what ALL ranks share: the step, the promised steps, the debug flags, and staging buffers that
+    // either every rank has or none (mpc_sub_connect). Not from its own particle count: an empty slab takes part, it may be
+    // handed particles)
+    bool stage = rebin && c->reorder_stage == 0 && c->have_order && c->tbase && !c->compact && (n != 0 || G.sub) &&
                  !(c->debug & (MPC_DEBUG_NO_FUSE_GATHER | MPC_DEBUG_EAGER_CANONICAL | MPC_DEBUG_ATOMIC_SCATTER)) &&
                  (phase == 0 ? k + 2 < nsteps : c->sub_ahead >= 2) && c->p.rebin_every >= 3;
     if (phase == 1) c->sub_stage = stage;
@@ -97,19 +100,16 @@ int steps_srd(mpc_ctx* c, int nsteps, int phase = 0) {
       G.le_d = host_le_offset(c, c->t);
       if (!c->sums_clean) { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->sums, 0, (size_t)G.nkeys * G.sw * 8, c->stream)); }
       c->sums_clean = false;
-      if (G.sub && c->reorder_stage == 2) {   // the new order holds the particles that have arrived, not those that have left
-        uint32_t nn = 0;
-        CU(cudaMemcpyAsync(&nn, c->offset + G.nkeys, 4, cudaMemcpyDeviceToHost, c->stream));
-        CU(cudaStreamSynchronize(c->stream));
-        if (nn > c->n_max) return fail(c, MPC_ENOMEM, "slab subdomain: more particles have arrived than n_max holds");
-        c->n = nn;
-      }
-      if (c->n) {
+      // the new order holds the particles that have arrived, not those that have left (count read in mpc_sub_end of the reorder step)
+      if (G.sub && c->reorder_stage == 2) c->n = c->sub_nn;
+      {
         const int io = c->reorder_stage == 1 ? IO_SCATTER : c->reorder_stage == 2 ? IO_AOS_IN : (stage ? IO_RANK : IO_PLAIN);
-        FamilyTimer ft(c, io != IO_PLAIN ? F_SWEEPG : F_SWEEP);
-        const int rc = launch_sweep(c, c->collide_pending, rebin && !stage, io, sp);
-        if (rc) return rc;
-        if (io == IO_SCATTER) c->reorder_stage = 2;
+        if (c->n) {
+          FamilyTimer ft(c, io != IO_PLAIN ? F_SWEEPG : F_SWEEP);
+          const int rc = launch_sweep(c, c->collide_pending, rebin && !stage, io, sp);
+          if (rc) return rc;
+        }
+        if (io == IO_SCATTER) c->reorder_stage = 2;      // (also on a slab rank without particles: its neighbours' passes go on)
         else if (io == IO_AOS_IN) c->reorder_stage = 0;
       }
       if (phase == 1) return MPC_OK;
@@ -130,13 +130,27 @@ int steps_srd(mpc_ctx* c, int nsteps, int phase = 0) {
       const int rc = (n || G.sub) ? launch_cell(c, zero, (rebin && compact_counts) ? c->cursor : nullptr, G.sub && stage) : MPC_OK;
       if (rc) return rc;
     }
-    if (rebin && compact_counts && n) {
+    if (rebin && compact_counts && (n || G.sub)) {
       const int rc = do_reorder(c, stage, false, true);
       if (rc) return rc;
+      if (G.sub && stage) {
+        // Hand-over: the scan's total is this rank's particle count in the new order (own particles that stay + arrivals).
+        // It is checked HERE, before the barrier that ends the step: in the next step this rank and both neighbours write
+        // 32-byte records at slots up to that total into this rank's staging buffer, which holds n_max of them. Too many:
+        // the context is dead (sticky), and the caller must stop every rank before the next mpc_sub_begin.
+        uint32_t nn = 0;
+        CU(cudaMemcpyAsync(&nn, c->offset + G.nkeys, 4, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        if (nn > c->n_max) {
+          c->sticky = true;
+          return fail(c, MPC_ENOMEM, "slab subdomain: the reorder would hand this rank more particles than n_max holds; no rank may start the next step");
+        }
+        c->sub_nn = nn;
+      }
     }
     if (n || G.sub) {
       c->sums_clean = zero != 0;
-      c->collide_pending = n != 0;
+      c->collide_pending = n != 0 || G.sub;   // (slab rank: particles handed to an empty slab arrive with this collision still to apply)
     }
     sp[0] = G.s[0]; sp[1] = G.s[1]; sp[2] = G.s[2];
     c->t++;
@@ -153,6 +167,9 @@ int set_state_impl(mpc_ctx* c, unsigned long long n, const float* const src[6], 
   if (!c->bound) return fail(c, MPC_ESTATE, "mpc_set_state before mpc_bind");
   if (n > c->n_max) return fail(c, MPC_ENOMEM, "n exceeds the n_max given to mpc_bind");
   for (int a = 0; a < 6; ++a) if (n && !src[a]) return fail(c, MPC_EINVAL, "NULL state array");
+  // a slab rank in the middle of a step or of a folded reorder: its neighbours are writing (or about to write) particles into its staging buffer
+  if (c->G.sub && (c->reorder_stage || c->sub_open))
+    return fail(c, MPC_ESTATE, "slab subdomain: mpc_set_state between mpc_sub_begin and mpc_sub_end or while a folded reorder is in flight");
   CU(cudaSetDevice(c->device));
   for (int a = 0; a < 6; ++a)
     if (n) CU(cudaMemcpyAsync(c->A[a], src[a], n * 4, kind, c->stream));

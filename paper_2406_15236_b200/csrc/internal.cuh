@@ -354,6 +354,7 @@ struct mpc_ctx {
   bool sub_open;        // slab subdomain: mpc_sub_begin has run, mpc_sub_end has not
   bool sub_stage;       // ... and it started a folded reorder with hand-over (decided in mpc_sub_begin, used by mpc_sub_end)
   int sub_ahead;        // ... steps the caller has promised to run after the open one before it reads or replaces the state
+  uint32_t sub_nn;      // ... particle count of this rank once the folded reorder in flight has handed particles over
   int reorder_stage;    // folded reorder: 0 none in flight, 1 the next sweep scatters into the new order, 2 the next sweep reads the staged records
   float le_dprev;       // Lees-Edwards displacement of the step whose collision is pending
   unsigned debug;       // MPC_DEBUG_* flags

@@ -356,6 +356,12 @@ int do_reorder(mpc_ctx* c, bool folded, bool canonical, bool counts_in_cursor) {
     k_scan_apply<<<(unsigned)nb, SCAN_T, 0, c->stream>>>(cnt, stride, nk, c->bsum, c->offset);
     LAUNCH_CHECK("k_scan_apply");
   }
+  if (!folded && n == 0) {   // a slab rank without particles: the offsets (all zero) are what its neighbours and its next reorder need
+    c->have_order = true;
+    c->order_canonical = canonical;
+    c->order_spread = spread;
+    return MPC_OK;
+  }
   if (!folded) {
     { FamilyTimer ft(c, F_MEMSET); CU(cudaMemsetAsync(c->cursor, 0, nk * 4, c->stream)); }
     if (canonical) {

@@ -238,14 +238,18 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
         const int side = SUB ? sub_shared(G, cz) : -1;
         // (a shared cell's count word also receives the neighbour's particles: this rank's own count, which numbers
         // its particles inside the cell, is kept apart)
-        if (ranked && side < 0) word = 0x80000000u | (uint32_t)(atomicAdd(s, ((u64)e << 16) | 1ull) & 0xffffull);
-        else atomicAdd(s, ((u64)e << 16) | 1ull);
-        atomicAdd(s + 1, pack_ss(a0, a1)); atomicAdd(s + 2, pack_ss(a2, 0));
         if (SUB && side >= 0) {
+          // a shared cell's words are added to by two GPUs at once (this rank here, the neighbour through its peer
+          // mapping): both sides use system-scope reductions, the only scope at which atomicity across GPUs is defined
+          atomicAdd_system(s, ((u64)e << 16) | 1ull); atomicAdd_system(s + 1, pack_ss(a0, a1)); atomicAdd_system(s + 2, pack_ss(a2, 0));
           u64* q = G.peer[side] + (size_t)((long long)kc + G.peer_koff[side]) * G.sw;
-          atomicAdd(q, ((u64)e << 16) | 1ull); atomicAdd(q + 1, pack_ss(a0, a1)); atomicAdd(q + 2, pack_ss(a2, 0));
+          atomicAdd_system(q, ((u64)e << 16) | 1ull); atomicAdd_system(q + 1, pack_ss(a0, a1)); atomicAdd_system(q + 2, pack_ss(a2, 0));
           if (ranked) word = 0x80000000u | (atomicAdd(G.lcount + kc, 1u) & 0xffffu);
           else atomicAdd(G.lcount + kc, 1u);
+        } else {
+          if (ranked) word = 0x80000000u | (uint32_t)(atomicAdd(s, ((u64)e << 16) | 1ull) & 0xffffull);
+          else atomicAdd(s, ((u64)e << 16) | 1ull);
+          atomicAdd(s + 1, pack_ss(a0, a1)); atomicAdd(s + 2, pack_ss(a2, 0));
         }
       }
       if (WKEY) key_out[i] = kc;
@@ -275,15 +279,18 @@ k_sweep(Geo G, float sp0, float sp1, float sp2, uint32_t n, float* __restrict__ 
       const u64 etile = ((u64)((unsigned)s[0] >> TILE_N_BITS) << TILE_E_SHIFT) + (u64)(unsigned)s[4];
       const u64 w0 = (etile << 16) | (u64)(unsigned)cnt;
       const int side = SUB ? sub_shared(G, oz + l2) : -1;
-      if (ranked && side < 0) old[k] = atomicAdd(g, w0);
-      else atomicAdd(g, w0);
-      atomicAdd(g + 1, pack_ss(s[1], s[2]));
-      atomicAdd(g + 2, pack_ss(s[3], 0));
       if (SUB && side >= 0) {   // the same sums into the neighbour that also holds this cell (integer adds commute: no staging, no ordering)
+        // system scope on both copies: the neighbour's GPU adds into `g` at the same time as this one (see above)
+        atomicAdd_system(g, w0); atomicAdd_system(g + 1, pack_ss(s[1], s[2])); atomicAdd_system(g + 2, pack_ss(s[3], 0));
         u64* pq = G.peer[side] + (size_t)((long long)kf + G.peer_koff[side]) * G.sw;
-        atomicAdd(pq, w0); atomicAdd(pq + 1, pack_ss(s[1], s[2])); atomicAdd(pq + 2, pack_ss(s[3], 0));
+        atomicAdd_system(pq, w0); atomicAdd_system(pq + 1, pack_ss(s[1], s[2])); atomicAdd_system(pq + 2, pack_ss(s[3], 0));
         if (ranked) old[k] = (u64)atomicAdd(G.lcount + kf, (uint32_t)cnt);   // this rank's particles already numbered in the cell
         else atomicAdd(G.lcount + kf, (uint32_t)cnt);
+      } else {
+        if (ranked) old[k] = atomicAdd(g, w0);
+        else atomicAdd(g, w0);
+        atomicAdd(g + 1, pack_ss(s[1], s[2]));
+        atomicAdd(g + 2, pack_ss(s[3], 0));
       }
       // partial momentum sums of >= 64 particles that come within a factor two of the int32 range
       if (cnt >= 64 && (abs(s[1]) >= (1 << 30) || abs(s[2]) >= (1 << 30) || abs(s[3]) >= (1 << 30))) atomicAdd(G.nrange, 1ull);

@@ -14,7 +14,7 @@ import os
 
 import numpy as np
 
-from .binding import MPC
+from .binding import MPC, MPCError
 from .slab import slab_neighbours, slab_owner, slab_partition
 
 
@@ -62,6 +62,9 @@ class SlabRank:
                     offsets=[(p - self.sim.workspace_ptr) if p else None for p in ptrs], layers=layers)
         everyone = [None] * self.world
         dist.all_gather_object(everyone, mine, group=group)
+        # the folded reorder (with its hand-over) must be on for every rank or for none: one rank without a staging buffer
+        # (compact workspace) turns it off everywhere
+        fold = all(e["offsets"][2] is not None for e in everyone)
         self._opened = {}
         ends = []
         for nb in slab_neighbours(self.rank, self.world):
@@ -75,7 +78,10 @@ class SlabRank:
                 h.reserved = info["handle"]
                 base = _ok(cudart.cudaIpcOpenMemHandle(h, cudart.cudaIpcMemLazyEnablePeerAccess))
                 self._opened[nb] = base
-            ends.append(([(int(base) + o) if o is not None else 0 for o in info["offsets"]], info["layers"]))
+            ptrs_nb = [(int(base) + o) if o is not None else 0 for o in info["offsets"]]
+            if not fold:
+                ptrs_nb[2] = 0
+            ends.append((ptrs_nb, info["layers"]))
         self.sim.sub_connect(ends[0], ends[1])
         self.t = 0
         self._overflows = 0          # range overflows counted before earlier hand-overs (mpc_set_state restarts the library's count)
@@ -85,6 +91,19 @@ class SlabRank:
     def barrier(self):
         self.torch.cuda.synchronize(self.device)
         self.dist.barrier(group=self.group)
+
+    def _barrier_with_status(self, err):
+        """the barrier that ends a step, carrying each rank's status: if mpc_sub_end failed on ANY rank (a hand-over beyond
+        that rank's n_max), every rank raises here, before any of them starts the step whose kernels would write the arrivals"""
+        torch, dist = self.torch, self.dist
+        torch.cuda.synchronize(self.device)
+        nccl = dist.get_backend(self.group) == "nccl"
+        flag = torch.tensor([1 if err is not None else 0], dtype=torch.int32, device=self.device if nccl else "cpu")
+        dist.all_reduce(flag, op=dist.ReduceOp.MAX, group=self.group)
+        if err is not None:
+            raise err
+        if int(flag.item()):
+            raise MPCError("another rank's mpc_sub_end failed (hand-over beyond its n_max): the run stops on every rank")
 
     def _exchange(self, send_below, send_above):
         """rows of 7 columns (float32 bit patterns) to the two neighbours; returns what they sent here"""
@@ -149,8 +168,12 @@ class SlabRank:
             for j in range(run):
                 self.sim.sub_begin(run - 1 - j)
                 self.barrier()
-                self.sim.sub_end()
-                self.barrier()
+                err = None
+                try:
+                    self.sim.sub_end()
+                except MPCError as e:
+                    err = e
+                self._barrier_with_status(err)
                 self.t += 1
             i += run
 

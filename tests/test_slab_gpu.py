@@ -25,18 +25,22 @@ def by_id(state):
     return [a[order] for a in s]
 
 
-def make_ranks(box, cells, nbar, seed, st, world, brick, **kw):
+def make_ranks(box, cells, nbar, seed, st, world, brick, n_max_of=None, **kw):
     parts = slab_partition(cells[2], world, brick[2])
     a = box[2] / cells[2]
     owner = slab_owner(st[2], a, parts)
     ranks = []
     for r, (z0, nz) in enumerate(parts):
         sel = np.nonzero(owner == r)[0]
-        g = MPC(box, cells, nbar, seed, n_max=max(2 * len(sel), 1), brick=brick, sub=(z0, nz), **kw)
+        n_max = max(2 * len(sel), 1) if n_max_of is None else n_max_of(r, len(sel))
+        g = MPC(box, cells, nbar, seed, n_max=n_max, brick=brick, sub=(z0, nz), **kw)
         ranks.append((g, sel))
+    exports = [g.sub_export() for g, _ in ranks]
+    if not all(e[0][2] for e in exports):                         # staging buffers on all ranks or on none (mpc_sub_connect)
+        exports = [([e[0][0], e[0][1], 0], e[1]) for e in exports]
     for r, (g, _) in enumerate(ranks):
         below, above = slab_neighbours(r, world)
-        g.sub_connect(ranks[below][0].sub_export(), ranks[above][0].sub_export())
+        g.sub_connect(exports[below], exports[above])
     for g, sel in ranks:
         g.set_state(*[to_dev(st[d][sel]) for d in range(6)], id=to_dev(st[6][sel].view(np.int32)))
     return ranks
@@ -162,6 +166,89 @@ def test_particles_handed_to_their_owners_between_steps():
     got = by_id([torch.cat([g.get_state()[d] for g, _ in ranks]) for d in range(7)])
     for d in range(7):
         assert np.array_equal(got[d], want[d]), d
+
+
+def test_an_empty_slab_takes_part_and_is_handed_particles():
+    # rank 1 of 3 starts without a single particle. It must still scan its (complete) cell counts at every reorder, fold the
+    # reorder like its neighbours and read back what they hand over; the particles it receives still owe the collision of the
+    # step before. Bit for bit against the single-domain run of the same state.
+    world, cells, brick, nbar = 3, (16, 16, 72), (16, 16, 8), 10
+    kw = dict(thermostat=1, rebin_every=4, dt=0.1)              # (short step: particles fly freely through the empty part, and must
+    box = tuple(float(c) for c in cells)                        # not get further than the halo between two hand-overs)
+    n = int(np.prod(cells)) * nbar
+    st = uniform_maxwell(box, n, 23)
+    parts = slab_partition(cells[2], world, brick[2])
+    keep = slab_owner(st[2], 1.0, parts) != 1
+    st = [a[keep] for a in st]
+    ref = MPC(box, cells, nbar, 4, n_max=len(st[0]), brick=brick, **kw)
+    ref.set_state(*[to_dev(st[d]) for d in range(6)], id=to_dev(st[6].view(np.int32)))
+    ref.step(15)
+    want = by_id(ref.get_state())
+    ranks = make_ranks(box, cells, nbar, 4, st, world, brick, n_max_of=lambda r, m: 2 * m + 30000, **kw)
+    assert ranks[1][0].n == 0
+    step_all(ranks, 15)                                           # folded reorders with hand-over at t = 4, 8 (12: not enough steps left)
+    assert ranks[1][0].n > 1000                                   # particles have arrived in the empty slab
+    for g, _ in ranks:
+        assert g.observables()["n_range_overflows"] == 0
+    states = [[a.cpu().numpy() for a in g.get_state()] for g, _ in ranks]
+    got = by_id([np.concatenate([s[d] for s in states]) for d in range(7)])
+    for d in range(7):
+        assert np.array_equal(got[d], want[d]), d
+    for g, _ in ranks:
+        assert g.observables()["n_range_overflows"] == 0
+
+
+def test_hand_over_beyond_n_max_is_refused_before_anything_is_written():
+    # Rank 0 starts thin (40 % of the density) beside a full rank 1 and has room for 16 particles more than it holds: the
+    # first folded reorder (t = 4) would hand it far more. The rank's mpc_sub_end of that step must refuse (MPC_ENOMEM),
+    # i.e. BEFORE the next step, whose scatter passes (its own and its neighbours') write the arrivals into its staging
+    # buffer of n_max records; the context is dead afterwards, the neighbour's is untouched and still readable.
+    world, cells, brick, nbar = 2, (16, 16, 48), (16, 16, 8), 10
+    kw = dict(thermostat=1, rebin_every=4, dt=0.5)
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    st = uniform_maxwell(box, n, 21)
+    parts = slab_partition(cells[2], world, brick[2])
+    thin = (slab_owner(st[2], 1.0, parts) == 0) & (np.arange(n) % 5 >= 2)
+    st = [a[~thin] for a in st]
+    ranks = make_ranks(box, cells, nbar, 9, st, world, brick, n_max_of=lambda r, m: m + 16 if r == 0 else 2 * m, **kw)
+    n0 = ranks[0][0].n
+    step_all(ranks, 4, ahead=8)                                   # t = 0 (local reorder) .. 3
+    for g, _ in ranks:
+        g.sub_begin(8)                                            # t = 4: rank pass of a folded reorder
+    torch.cuda.synchronize()
+    with pytest.raises(MPCError, match="n_max"):
+        ranks[0][0].sub_end()
+    ranks[1][0].sub_end()                                         # the neighbour has room
+    torch.cuda.synchronize()
+    assert ranks[0][0].n == n0                                    # nothing was handed over
+    with pytest.raises(MPCError):
+        ranks[0][0].sub_begin(7)                                  # dead for good
+    with pytest.raises(MPCError):
+        ranks[0][0].get_state()
+
+
+def test_set_state_is_refused_in_the_middle_of_a_step():
+    world, cells, brick, nbar = 2, (16, 16, 48), (16, 16, 8), 10
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar
+    st = uniform_maxwell(box, n, 22)
+    ranks = make_ranks(box, cells, nbar, 9, st, world, brick, thermostat=1, rebin_every=4)
+    g, sel = ranks[0]
+    args = [to_dev(st[d][sel]) for d in range(6)]
+    step_all(ranks, 4, ahead=8)
+    for h, _ in ranks:
+        h.sub_begin(8)
+    with pytest.raises(MPCError):
+        g.set_state(*args)                                        # between mpc_sub_begin and mpc_sub_end
+    torch.cuda.synchronize()
+    for h, _ in ranks:
+        h.sub_end()
+    torch.cuda.synchronize()
+    with pytest.raises(MPCError):
+        g.set_state(*args)                                        # folded reorder in flight (t = 4 was its first step)
+    step_all(ranks, 2, ahead=0)
+    g.set_state(*args)                                            # between steps, nothing in flight: fine
 
 
 def test_a_particle_outside_its_slab_is_reported():
