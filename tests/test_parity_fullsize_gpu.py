@@ -105,12 +105,15 @@ def test_config5_sampled_cells_512cubed(nbar):
     # BASELINE.json configs[4], all three densities of its sweep, in the launch configuration bench.py times.
     # <N_c> = 20: 2,684,354,560 particles (> 2^31: unsigned 32-bit indices), compact workspace (property-wise reorder,
     # PAPER.md:156-162), state handed over through the host-pointer ABI as bench.py does.
-    # One call of 12 steps from t = 0: reorder of an unordered state at t = 0, nine fused steps on a stale order, the
-    # reorder at t = 10 (staged through 32-byte records with the rank-based slot scatter where the second particle copy
-    # exists, property-wise gather otherwise), and t = 11, the step checked here against the oracle, which reads the
-    # staged records through the permutation. No single-step call in the chain: the state before the last step comes
-    # from a run of 11 steps in one call (the GPU path is bit-reproducible, and independent of how steps are split
-    # over calls: test_config5_fused_call_equals_single_steps_512cubed).
+    # One call of 13 steps from t = 0: reorder of an unordered state at t = 0 (unfolded), nine fused steps on a stale order,
+    # the reorder at t = 10, which is folded into the sweeps of t = 10, 11, 12 where the second particle copy exists (arrival
+    # ranks, 32-byte records written at their slots of the new order, records read back) and property-wise
+    # otherwise (compact workspace, 20 per cell), and t = 12, the step checked here against the oracle: with the second copy
+    # it IS the read-back pass of the folded reorder, so every sampled particle has gone through all three passes (the
+    # kernel-family counters are asserted, the test cannot fall back to the unfolded path unnoticed). No single-step call
+    # in the chain: the state before the last step comes from a run of 12 steps in one call, which cannot fold the reorder
+    # at t = 10 (too few steps left) and so takes the unfolded one (the GPU path is bit-reproducible, and independent of how
+    # steps are split over calls: test_config5_fused_call_equals_single_steps_512cubed).
     gc.collect()
     torch.cuda.empty_cache()                     # blocks cached by earlier tests count as used
     free, _total = torch.cuda.mem_get_info()
@@ -121,7 +124,7 @@ def test_config5_sampled_cells_512cubed(nbar):
     n = 512**3 * nbar
     compact = nbar == 20
     kw = dict(thermostat=1, rebin_every=10, brick=BRICK)
-    nsteps = 12
+    nsteps = 13
     g = MPC(box, cells, nbar, seed, n_max=n, compact=compact, **kw)
     nkeys = g.nkeys
 
@@ -139,7 +142,11 @@ def test_config5_sampled_cells_512cubed(nbar):
 
     # run 1: the full call; sample cells and their members from the keys of the last step
     fresh_state()
+    g.profile_enable()
     g.step(nsteps)
+    fam = g.profile_read()
+    g.profile_enable(False)
+    assert fam["sweep_gather"][1] == (0 if compact else 3), fam   # rank, scatter and read-back passes of the reorder at t = 10
     g.canonicalise()                             # keys below are per particle of the CURRENT order: fix it first
     cnt, px, py, pz, e2, key = g.get_cells()
     assert int(cnt.sum(dtype=torch.int64)) == n
@@ -157,12 +164,12 @@ def test_config5_sampled_cells_512cubed(nbar):
     del cnt, px, py, pz, e2, key
     torch.cuda.empty_cache()
     Q = g.get_state_at(idx)                                      # post-collision state of the members, canonical order
-    # run 2: the same trajectory stopped one step earlier (11 steps in one call) -> state before the last step
+    # run 2: the same trajectory stopped one step earlier (12 steps in one call) -> state before the last step
     fresh_state()
     g.step(nsteps - 1)
     g.canonicalise()
     P = g.get_state_at(idx)
-    assert np.array_equal(P[6], Q[6])                            # t = 11 does not reorder: same memory order
+    assert np.array_equal(P[6], Q[6])                            # t = 12 does not reorder: same memory order
     if nbar == 20:
         assert int(idx.max()) > 2**31                            # indices beyond 2^31 are exercised
     o = Oracle(box, cells, nbar, seed, **kw)
@@ -203,10 +210,11 @@ def test_config5_sampled_cells_512cubed(nbar):
 
 
 def test_config5_fused_call_equals_single_steps_512cubed():
-    # At config 5's full size, in the launch configuration bench.py times: one call of 4 steps (first-step sweep, the
-    # steady-state 3-CTA sweep with the collision of the previous step fused in, the staged reorder pair around
-    # t = 10) must leave bit for bit the state that 4 calls of one step leave (unfused: sweep, cell, trailing collide
-    # each; that path is the one checked against the oracle cell by cell above and in lock-step at small sizes).
+    # At config 5's full size, in the launch configuration bench.py times: one call of 13 steps from t = 0 (first-step sweep,
+    # unfolded reorder of the unordered state at t = 0, the steady-state 3-CTA sweep with the collision of the previous step
+    # fused in, the reorder at t = 10 folded into the sweeps of t = 10, 11, 12: asserted from the kernel-family counters)
+    # must leave bit for bit the state that 13 calls of one step leave (unfused: sweep, cell, trailing collide each, every
+    # reorder unfolded; that path is the one checked against the oracle in lock-step at small sizes).
     gc.collect()
     torch.cuda.empty_cache()                     # blocks cached by earlier tests count as used
     free, _total = torch.cuda.mem_get_info()
@@ -216,21 +224,26 @@ def test_config5_fused_call_equals_single_steps_512cubed():
     box = (512.0,) * 3
     n = 512**3 * nbar
     kw = dict(thermostat=1, rebin_every=10, brick=BRICK)
-    st = uniform_maxwell_cuda(box, n, seed)
     g = MPC(box, cells, nbar, seed, n_max=n, **kw)
-    g.set_state(*st, step=8)                     # t = 8, 9 plain; t = 10 reorder (staged in the fused call); t = 11 gather
-    torch.cuda.synchronize()
-    del st
-    torch.cuda.empty_cache()
-    g.step(1)                                    # t = 8: brings the particles into the library's order once
-    pre = [t.cpu() for t in g.get_state()]       # host copy of the state at t = 9
-    torch.cuda.empty_cache()
-    for _ in range(4):
-        g.step(1)                                # t = 9, 10, 11, 12, one call each
+
+    def fresh_state():
+        st = uniform_maxwell_cuda(box, n, seed)  # the same seeded state both times
+        g.set_state(*st, step=0)
+        torch.cuda.synchronize()
+        del st
+        torch.cuda.empty_cache()
+
+    fresh_state()
+    for _ in range(13):
+        g.step(1)                                # t = 0 .. 12, one call each
     ref = [t.cpu() for t in g.get_state()]
     torch.cuda.empty_cache()
-    g.set_state_host(*[t.numpy() for t in pre[:6]], id=pre[6].numpy(), step=9)
-    g.step(4)                                    # the same four steps in one call
+    fresh_state()
+    g.profile_enable()
+    g.step(13)                                   # the same thirteen steps in one call
+    fam = g.profile_read()
+    g.profile_enable(False)
+    assert fam["sweep_gather"][1] == 3 and fam["sweep"][1] == 10, fam
     got = g.get_state()
     for a, b in zip(ref, got):
         assert torch.equal(a, b.cpu())

@@ -337,9 +337,10 @@ def test_compact_workspace_gives_identical_results():
                                 dict(brick=(4, 2, 1), rebin_every=5),
                                 dict(thermostat=1, shear_rate=0.05, brick=(16, 16, 8), rebin_every=3)])
 def test_reorder_code_paths_agree(kw):
-    # Ways to apply a reorder inside a multi-step call: (a) default: folded into two sweeps through 32-byte staging
-    # records, slots from the staging sweep's arrival ranks (no atomics in the scatter), particles grouped by key only,
-    # canonical (key, id) order restored when the state is read; (b) separate gather kernel; (c) eager canonical order
+    # Ways to apply a reorder inside a multi-step call (rebin_every >= 3 and two further steps in the call, else the unfolded
+    # reorder runs in every variant): (a) default: folded into three sweeps: arrival ranks from the sweep of the reorder step,
+    # 32-byte records written at their slots of the new order by the next sweep (no atomics), read back by the one after;
+    # particles grouped by key only, canonical (key, id) order restored when the state is read; (b) separate gather kernel; (c) eager canonical order
     # (scatter + rank by id + gather), the path the lock-step parity tests exercise with mpc_step(1); (d) cursor
     # atomics in the scatter; (e) the last collision of a call applied at once instead of staying pending; (f) plain cell
     # order in memory between reads instead of the lane-spread order of every group of 32 cells.
@@ -367,22 +368,39 @@ def test_reorder_code_paths_agree(kw):
             assert np.array_equal(x, y)
 
 
-@pytest.mark.parametrize("name,kw,t0,k", [
-    ("plain fused step", dict(thermostat=1, brick=(16, 16, 8), rebin_every=10), 1, 3),
-    ("step after a staged reorder (gathers the staging records)", dict(thermostat=1, brick=(16, 16, 8), rebin_every=4), 2, 4),
-    ("second step after a staged reorder", dict(thermostat=1, brick=(16, 16, 8), rebin_every=4), 2, 5),
-    ("walls + gravity, staged reorder", dict(thermostat=1, bc=(0, 0, 1), g=(0.01, 0, 0), brick=4, rebin_every=3), 1, 4),
-    ("no thermostat, small bricks", dict(brick=(4, 2, 1), rebin_every=5), 3, 4),
-    ("Lees-Edwards shear, staged reorder", dict(thermostat=1, shear_rate=0.08, brick=(16, 16, 8), rebin_every=3), 1, 4),
-    ("Lees-Edwards shear, plain fused step", dict(shear_rate=0.08, dt=0.3, brick=4, rebin_every=10), 5, 3),
+_FOLD = dict(thermostat=1, brick=(16, 16, 8), rebin_every=4)
+_FOLD_WALL = dict(thermostat=1, bc=(0, 0, 1), g=(0.01, 0, 0), brick=4, rebin_every=4)
+_FOLD_LE = dict(thermostat=1, shear_rate=0.08, brick=(16, 16, 8), rebin_every=4)
+
+
+@pytest.mark.parametrize("name,kw,t0,k,folded", [
+    ("plain fused step", dict(thermostat=1, brick=(16, 16, 8), rebin_every=10), 1, 3, False),
+    ("step after an unfolded reorder", dict(thermostat=1, brick=(16, 16, 8), rebin_every=4), 2, 4, False),
+    ("second step after an unfolded reorder", dict(thermostat=1, brick=(16, 16, 8), rebin_every=4), 2, 5, False),
+    ("walls + gravity, unfolded reorder", dict(thermostat=1, bc=(0, 0, 1), g=(0.01, 0, 0), brick=4, rebin_every=3), 1, 4, False),
+    ("no thermostat, small bricks", dict(brick=(4, 2, 1), rebin_every=5), 3, 4, False),
+    ("Lees-Edwards shear, unfolded reorder", dict(thermostat=1, shear_rate=0.08, brick=(16, 16, 8), rebin_every=3), 1, 4, False),
+    ("Lees-Edwards shear, plain fused step", dict(shear_rate=0.08, dt=0.3, brick=4, rebin_every=10), 5, 3, False),
+    # the reorder folded into three sweeps (the path bench.py times): from t = 0 the reorder at t = 0 is unfolded (no order
+    # yet), the one at t = 4 is folded when two more steps follow in the call: rank pass at t = 4, scatter pass at t = 5,
+    # read-back pass at t = 6 (the last step for k = 7), first plain sweep on the new lane-spread order at t = 7 (k = 8)
+    ("folded reorder: read-back pass", _FOLD, 0, 7, True),
+    ("folded reorder: first plain sweep on the new order", _FOLD, 0, 8, True),
+    ("folded reorder, walls + gravity: read-back pass", _FOLD_WALL, 0, 7, True),
+    ("folded reorder, walls + gravity: first plain sweep on the new order", _FOLD_WALL, 0, 8, True),
+    ("folded reorder, Lees-Edwards shear: read-back pass", _FOLD_LE, 0, 7, True),
+    ("folded reorder, Lees-Edwards shear: first plain sweep on the new order", _FOLD_LE, 0, 8, True),
 ])
-def test_fused_path_directly_against_oracle(name, kw, t0, k):
-    # The multi-step call runs code no single-step call runs: the collision of step t-1 inside the sweep of step t,
-    # the staged reorder (32-byte records out, gather in the next sweep), the rank-based slot scatter. Direct check
+def test_fused_path_directly_against_oracle(name, kw, t0, k, folded):
+    # The multi-step call runs code no single-step call runs: the collision of step t-1 inside the sweep of step t, and
+    # the reorder folded into three consecutive sweeps (arrival ranks written by the sweep of the reorder step, 32-byte
+    # records written at their slots of the new order by the next sweep, read back by the one after). Direct check
     # with no single-step call in the chain: a twin context advances k-1 steps in ONE call, the oracle takes the
-    # twin's state (the GPU is bit-reproducible, so this is exactly the state the first context had before its
-    # last step) and advances ONE step; the first context advances k steps in ONE call. Element-by-element parity
-    # of the k-th step, which ran entirely inside the fused path.
+    # twin's state and advances ONE step; the first context advances k steps in ONE call. Element-by-element parity
+    # of the k-th step, which ran entirely inside the fused path. (The twin's shorter call cannot fold the reorder at
+    # t = 4 - too few steps left - so the state the oracle starts from has come through the unfolded reorder.)
+    # The kernel-family counters say which path the first context took: the test fails if the folded reorder did not run
+    # where the case says it does.
     cells, nbar = (32, 16, 16), 10
     box = tuple(float(c) for c in cells)
     n = int(np.prod(cells)) * nbar - 5
@@ -391,7 +409,12 @@ def test_fused_path_directly_against_oracle(name, kw, t0, k):
     gpu_set(g, st, step=t0)
     gpu_set(twin, st, step=t0)
     twin.step(k - 1)
+    g.profile_enable()
     g.step(k)
+    fam = g.profile_read()
+    g.profile_enable(False)
+    assert fam["sweep_gather"][1] == (3 if folded else 0), fam    # rank, scatter and read-back passes of ONE folded reorder
+    assert fam["sweep"][1] + fam["sweep_gather"][1] == k
     o = Oracle(box, cells, nbar, 29, **kw)
     o.set_state(*gpu_get(twin), step=t0 + k - 1)
     o.step(1)

@@ -168,6 +168,45 @@ def test_particles_handed_to_their_owners_between_steps():
         assert np.array_equal(got[d], want[d]), d
 
 
+@pytest.mark.parametrize("world", [2, 3])
+def test_slab_step_with_hand_over_against_the_oracle(world):
+    # The decomposed path in front of the ORACLE (not only of the single-domain GPU run): the whole-box oracle takes the
+    # state before the last step and advances one step; the slab ranks advance 7 steps from t = 0, the last of which (t = 6)
+    # is the read-back pass of the reorder folded into t = 4, 5, 6, with the particles of the halo layers written into their
+    # new owners' staging buffers at t = 5. The state before the last step comes from a second set of ranks that runs 6 steps
+    # (too few to fold: its reorder at t = 4 stays local and hands nothing over). Element by element, matched by id, at the
+    # tolerances of tests/test_parity_gpu.py.
+    from oracle.binding import Oracle
+    cells, brick, nbar = (16, 16, 24 * world), (16, 16, 8), 10
+    kw = dict(thermostat=1, rebin_every=4, dt=0.5)
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar - 3
+    st = uniform_maxwell(box, n, 31)
+    twin = make_ranks(box, cells, nbar, 8, st, world, brick, **kw)
+    step_all(twin, 6)
+    before = by_id([torch.cat([g.get_state()[d] for g, _ in twin]) for d in range(7)])
+    assert all(g.n == len(sel) for g, sel in twin)                # nothing handed over there
+    ranks = make_ranks(box, cells, nbar, 8, st, world, brick, **kw)
+    for g, _ in ranks:
+        g.profile_enable()
+    step_all(ranks, 7)
+    for g, _ in ranks:
+        assert g.profile_read()["sweep_gather"][1] == 3           # rank, scatter and read-back pass of the folded reorder
+    assert sum(abs(g.n - len(sel)) for g, sel in ranks) > 0       # particles have changed owner
+    got = by_id([torch.cat([g.get_state()[d] for g, _ in ranks]) for d in range(7)])
+    o = Oracle(box, cells, nbar, 8, brick=brick, **kw)
+    o.set_state(*before[:6], before[6].view(np.uint32), step=6)
+    o.step(1)
+    want = by_id(o.get_state())
+    assert np.array_equal(got[6].view(np.uint32), want[6].view(np.uint32))
+    for d in range(3):
+        assert np.max(np.abs(want[d].astype(np.float64) - got[d])) <= 1e-5
+    for d in range(3, 6):
+        assert np.max(np.abs(want[d].astype(np.float64) - got[d])) <= 2e-5
+    for g, _ in ranks:
+        assert g.observables()["n_range_overflows"] == 0
+
+
 def test_an_empty_slab_takes_part_and_is_handed_particles():
     # rank 1 of 3 starts without a single particle. It must still scan its (complete) cell counts at every reorder, fold the
     # reorder like its neighbours and read back what they hand over; the particles it receives still owe the collision of the
