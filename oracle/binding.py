@@ -31,12 +31,13 @@ class OracleObs(C.Structure):
 
 
 _lib = None
+_lib_path = None     # set before the first call to load another build of the oracle (the sanitizer build: tests/test_oracle_sanitize.py)
 
 
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(_build.build())
+        _lib = C.CDLL(_lib_path or _build.build())
         _lib.oracle_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_float), C.POINTER(C.c_int), C.c_float,
                                        C.POINTER(OracleParams), C.c_ulonglong]
         _lib.oracle_destroy.argtypes = [C.c_void_p]

@@ -102,10 +102,11 @@ def test_shear_profile_and_viscosity_from_shear_stress():
     o = Oracle(box, cells, nbar, 77, thermostat=1, shear_rate=g, dt=h)
     o.set_state(*st)
     o.step(300)
-    planes = np.arange(1, L)
-    kin = col = 0.0
+    nplanes = L - 1                                                    # the interior planes z = 1 .. L-1
+    kin = col = kin_all = 0.0
     prof = np.zeros(L)
-    nsamp = 1200
+    nsamp = 2400
+    U = g * L
     x0, y0, z0, vx0, vy0, vz0, id0 = o.get_state()
     for it in range(nsamp):
         t = int(o.observables()["step"])
@@ -114,22 +115,23 @@ def test_shear_profile_and_viscosity_from_shear_stress():
         a0, a1 = np.argsort(id0), np.argsort(id1)
         zb, vzb, vxb = z0[a0].astype(np.float64), vz0[a0].astype(np.float64), vx0[a0].astype(np.float64)
         za = zb + vzb * h                                              # unwrapped end of the move
-        for p in planes:
-            up = (zb < p) & (za >= p)
-            dn = (zb >= p) & (za < p)
-            kin += vxb[up].sum() - vxb[dn].sum()
+        # a particle going from zb to za crosses the interior planes p with zb < p <= za upwards (or za < p <= zb downwards):
+        # their number, signed, is the difference of the two layer indices clipped to the box
+        crossed = np.clip(np.floor(za), 0, L - 1) - np.clip(np.floor(zb), 0, L - 1)
+        kin += (vxb * crossed).sum()
+        # the same flux averaged over ALL plane heights in (0, L) instead of the 15 integer ones: v_x times the stretch of z
+        # the particle covers (every particle contributes at every step, so the thermal noise is far smaller); the part of
+        # the stretch beyond the sheared face is covered in the image, where the particle's velocity is v_x -+ U
+        kin_all += (vxb * (np.clip(za, 0.0, L) - zb)).sum() + ((vxb - U) * np.maximum(za - L, 0.0)).sum() + ((vxb + U) * np.minimum(za, 0.0)).sum()
         # collision of step t: members of the cell layer that straddles a plane, by the side of the plane they are on
         s = o.grid_shift(t)
         zc = z1[a1].astype(np.float64)                                 # positions at the collision
         dvx = vx1[a1].astype(np.float64) - vxb
         # particles that crossed the sheared face while streaming changed v_x by -+U outside the collision: undo
-        U = g * L
         dvx += U * ((za >= L).astype(float) - (za < 0).astype(float))
         lay = np.floor(zc + s[2]).astype(int)                          # cell layer (unwrapped) of every particle
-        for p in planes:
-            k = p if s[2] > 0 else p - 1                               # the layer [k - s_z, k + 1 - s_z) contains p
-            m = (lay == k) & (zc >= p)
-            col += dvx[m].sum()
+        p = lay if s[2] > 0 else lay + 1                               # the plane inside the layer [lay - s_z, lay + 1 - s_z)
+        col += dvx[(p >= 1) & (p <= L - 1) & (zc >= p)].sum()          # handed to the members above the plane
         prof += o.observables(L)["profile"]
         x0, y0, z0, vx0, vy0, vz0, id0 = x1, y1, z1, vx1, vy1, vz1, id1
     prof /= nsamp
@@ -137,12 +139,18 @@ def test_shear_profile_and_viscosity_from_shear_stress():
     slope = np.polyfit(zmid, prof, 1)[0]
     assert slope == pytest.approx(g, rel=0.03)
     assert np.abs(prof - g * (zmid - L / 2)).max() < 0.015             # linear through the sheared face, no slip
-    flux = (kin + col) / (nsamp * len(planes) * L * L * h)             # x-momentum per area and time, upwards (m = 1)
+    flux = (kin + col) / (nsamp * nplanes * L * L * h)                 # x-momentum per area and time, upwards (m = 1)
     eta = -flux / g
     nu_kin, nu_col = srd_viscosity(nbar, h, 130)
     assert eta == pytest.approx(nbar * (nu_kin + nu_col), rel=0.04)    # 8.70
-    # kinetic part alone: 0.49. Its estimator sums v_x (thermal, variance kT/m = 1) over ~200 plane crossings per plane and
-    # step: 3.6e6 terms, standard error sqrt(3.6e6) / (nsamp * planes * L^2 * h * g) = 0.21; checked at 3 standard errors
-    # (the total above is far less noisy: the thermal v_x a particle carries across a plane is handed back by the collisions)
-    assert abs(-kin / (nsamp * len(planes) * L * L * h * g) - nbar * nu_kin) < 3 * 0.21
+    # kinetic part alone: eta_kin = rho nu_kin = 0.486, from the all-heights estimator: a sum of n = 40,960 terms v_x v_z h per
+    # step with variance (kT/m)^2 h^2 each, so its standard error is sqrt(n / nsamp) / (L^3 g) = 0.050. Checked at 3 standard
+    # errors, |eta_kin - 0.486| < 0.15: a missing kinetic part (0) and a doubled one (0.97) both fail. (The 15-plane
+    # estimator that the total uses has a standard error of 0.15 here on its kinetic part alone; in the total that noise
+    # cancels, because the thermal v_x a particle carries across a plane is handed back by the collisions.)
+    eta_kin = -kin_all / (nsamp * L * L * L * h * g)
+    se = np.sqrt(n / nsamp) / (L**3 * g)
+    assert se < 0.052
+    assert abs(eta_kin - nbar * nu_kin) < 3 * se, eta_kin
+    assert abs(-kin / (nsamp * nplanes * L * L * h * g) - eta_kin) < 3 * 0.15   # the two estimators agree
     assert o.observables()["kT_cell"] == pytest.approx(1.0, rel=0.02)

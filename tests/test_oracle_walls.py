@@ -174,25 +174,37 @@ def test_poiseuille_profile_matches_analytic_viscosity():
     box, cells = (16.0, 8.0, 16.0), (16, 8, 16)
     st = uniform_maxwell(box, 16 * 8 * 16 * 10, 5)
     g = 0.005
-    o = Oracle(box, cells, 10, 321, thermostat=1, g=(g, 0, 0), bc=(0, 0, 1))
-    o.set_state(*st)
-    o.step(1200)
-    prof = np.zeros(16)
-    nav = 0
-    for _ in range(440):
-        o.step(5)
-        prof += o.observables(16)["profile"]
-        nav += 1
-    prof /= nav
     zc = np.arange(16) + 0.5
     A = np.stack([zc * (16 - zc), np.ones(16)], 1)
-    coef, *_ = np.linalg.lstsq(A, prof, rcond=None)
-    nu_fit, slip = g / (2 * coef[0]), coef[1]
+
+    def steady_flow(fill):
+        # fill = the number the virtual wall particles top a wall-cut cell up to (U8): 10 = <N_c>, the method; 1 = a cell
+        # that holds a particle at all gets none, i.e. bounce-back walls WITHOUT virtual particles, the comparison case
+        o = Oracle(box, cells, fill, 321, thermostat=1, g=(g, 0, 0), bc=(0, 0, 1))
+        o.set_state(*st)
+        o.step(1200)
+        prof = np.zeros(16)
+        nav = 0
+        for _ in range(440):
+            o.step(5)
+            prof += o.observables(16)["profile"]
+            nav += 1
+        prof /= nav
+        coef, *_ = np.linalg.lstsq(A, prof, rcond=None)
+        return o, prof, g / (2 * coef[0]), coef[1]
+
+    o, prof, nu_fit, slip = steady_flow(10)
     nu = sum(srd_viscosity(10, 0.1, 130))
     assert nu_fit == pytest.approx(nu, rel=0.06)
-    # near no-slip: the virtual wall particles "reduce boundary slip", they do not remove it; the residual
-    # intercept of the fit is 6-7 % of v_max here (standard error of the fitted intercept ~1.5 % of v_max), bounded at 10 %
-    assert abs(slip) < 0.10 * prof.max()
+    # the virtual wall particles "reduce boundary slip"; they do not remove it, and the paper gives no number.
+    # The pin is therefore the statement itself: the fitted velocity at the wall (the intercept of the parabola) against
+    # the same flow without virtual particles. Measured over two seeds: 4-7 % of v_max with them (standard error of one
+    # fitted intercept ~1.5 % of v_max; a slip length of about a quarter of a cell), 21 % without. A fill that did
+    # nothing, or a wrong sign or scale of the virtual momentum, lands at or beyond the second number.
+    _, prof_bare, _, slip_bare = steady_flow(1)
+    assert slip_bare > 0.15 * prof_bare.max()                  # without virtual particles the fluid slips markedly
+    assert abs(slip) / prof.max() < 0.5 * slip_bare / prof_bare.max()
+    assert abs(slip) < 0.10 * prof.max()                       # (loose absolute bound, three standard errors above the measured value)
     assert abs(prof - prof[::-1]).max() < 0.02                 # symmetric
     ob = o.observables()
     assert ob["kT_cell"] == pytest.approx(1.0, rel=0.03)        # thermostat holds k_BT under forcing
