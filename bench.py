@@ -54,40 +54,64 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    """SM clock and throttle reasons during the timed region: ONE `nvidia-smi -lms 50` process streams a line every 50 ms
+    (starting a new nvidia-smi per sample takes longer than the whole timed region of a short run); it is started before the
+    warm-up, and mark_start() / mark_stop() around the timed region pick the lines that fall inside it. `samples` is that
+    number: below 5 the record cannot support a statement about the clock, and says so."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    PERIOD_MS = 50
 
     def __init__(self, index):
-        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+        self.index, self.rows, self._t, self._p = index, [], None, None
+        self.t0 = self.t1 = None
 
     def _run(self):
-        while not self._stop.is_set():
-            try:
-                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
-                                     capture_output=True, text=True, timeout=5).stdout.strip()
-                if out:
-                    self.rows.append([t.strip() for t in out.split(",")])
-            except Exception:
-                pass
-            self._stop.wait(0.2)
+        try:
+            for line in self._p.stdout:
+                cols = [t.strip() for t in line.strip().split(",")]
+                if len(cols) >= 7:
+                    self.rows.append((time.monotonic(), cols))
+        except Exception:
+            pass
 
     def __enter__(self):
-        self._t = threading.Thread(target=self._run, daemon=True)
-        self._t.start()
+        try:
+            self._p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                        "-lms", str(self.PERIOD_MS)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True, bufsize=1)
+            self._t = threading.Thread(target=self._run, daemon=True)
+            self._t.start()
+        except Exception:
+            self._p = None
         return self
 
+    def mark_start(self):
+        self.t0 = time.monotonic()
+
+    def mark_stop(self):
+        self.t1 = time.monotonic()
+
     def __exit__(self, *a):
-        self._stop.set()
-        self._t.join(timeout=6)
+        if self._p is not None:
+            self._p.terminate()
+            try:
+                self._p.wait(timeout=5)
+            except Exception:
+                self._p.kill()
+            self._t.join(timeout=5)
 
     def summary(self):
-        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        num = lambda t: t.replace(".", "", 1).isdigit()
+        inside = [c for (t, c) in self.rows if self.t0 is not None and self.t1 is not None and self.t0 <= t <= self.t1]
+        sm = [float(c[0]) for c in inside if num(c[0])]
+        mx = [float(c[1]) for (_, c) in self.rows if num(c[1])]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i].lower().startswith("active")})
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": reasons, "samples": len(self.rows)}
+        reasons = sorted({names[i] for c in inside for i in range(4) if c[3 + i].lower().startswith("active")})
+        out = {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+               "samples": len(inside), "sample_period_ms": self.PERIOD_MS, "samples_outside_timed_region": len(self.rows) - len(inside)}
+        if len(inside) < 5:
+            out["note"] = "fewer than 5 samples inside the timed region: insufficient for a statement about the clock under load"
+        return out
 
 
 def oracle_rate(wl, nbar, budget_s=12.0):
@@ -161,12 +185,13 @@ def run_reference(args, wl, rank, world):
 
 
 def csrc_digest():
-    """sha256 over the CUDA sources of the sweep: ties a committed ncu capture to the code it was taken from."""
+    """sha256 over every CUDA source of the library (all of them decide what a step launches): ties a committed ncu
+    capture to the code it was taken from."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2406_15236_b200", "csrc")
-    for f in ("sweep.cu", "internal.cuh", "philox.cuh"):          # the files that define the dominant kernel
-        if True:
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
             h.update(f.encode())
             h.update(open(os.path.join(d, f), "rb").read())
     return h.hexdigest()[:16]
@@ -186,7 +211,7 @@ def captured_traffic(family, workload, nbar):
     return float(e["dram_bytes_per_launch"]), e.get("source"), e.get("csrc_digest") != csrc_digest()
 
 
-def measure(args, workload, nbar, steps, warmup, rank, local_rank, world, dist, with_e2e, rebin_every=None, cells_override=None):
+def measure(args, workload, nbar, steps, warmup, rank, local_rank, world, dist, with_e2e, rebin_every=None):
     """One workload: W untimed warm-up steps, then EXACTLY K steps in one mpc_step call between two CUDA events on
     the launching stream. Returns the JSON-able result dict (without cpu_baseline)."""
     import torch
@@ -197,8 +222,6 @@ def measure(args, workload, nbar, steps, warmup, rank, local_rank, world, dist, 
     wl = dict(WORKLOADS[workload])
     if rebin_every is not None:
         wl["rebin_every"] = rebin_every
-    if cells_override:
-        wl["cells"] = cells_override
     device = torch.device(f"cuda:{local_rank}")
     cells = wl["cells"]
     box = tuple(float(c) for c in cells)
@@ -207,15 +230,13 @@ def measure(args, workload, nbar, steps, warmup, rank, local_rank, world, dist, 
     brick = tuple(int(t) for t in args.brick.split(","))
     brick = brick * 3 if len(brick) == 1 else brick
     kw.update(rebin_every=wl["rebin_every"], brick=brick)
-    compact = args.compact or (n * 72 + int(np.prod(cells)) * 80 > 150e9)
+    compact = n * 72 + int(np.prod(cells)) * 80 > 150e9
     # a state that does not fit beside the workspace (20 per cell: 64 GB + 138 GB) is made array by array on the
     # device, parked in pinned host memory and handed over through the host-pointer ABI
     via_host = n * 24 + n * 52 + int(np.prod(cells)) * 80 > 170e9
     st = list(uniform_maxwell_cuda(box, n, 1234 + rank, device=str(device), to_host=via_host))
     torch.cuda.empty_cache()
     sim = MPC(box, cells, nbar, 1234 + rank, n_max=n, device=str(device), compact=compact, **kw)
-    if args.debug:
-        sim.set_debug(args.debug)
     if via_host:
         sim.set_state_host(*st)
     else:
@@ -235,18 +256,20 @@ def measure(args, workload, nbar, steps, warmup, rank, local_rank, world, dist, 
     # The collision of the last step of a call stays pending and is applied inside the next call's first streaming
     # pass: the timed call applies the warm-up's last collision and leaves its own last one pending,
     # i.e. exactly K collisions, K streaming passes, K cell passes are inside the timed region.
-    sim.step(warmup)
-    barrier()
-    sim.profile_enable(True)
-    sim.profile_read()
-    l0 = sim.launch_count
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local_rank) as clocks:
+    with ClockSampler(local_rank) as clocks:     # streaming from before the warm-up on
+        sim.step(warmup)
         barrier()
+        sim.profile_enable(True)
+        sim.profile_read()
+        l0 = sim.launch_count
+        barrier()
+        clocks.mark_start()
         ev0.record(sim.stream)
         sim.step(steps)
         ev1.record(sim.stream)
         barrier()
+        clocks.mark_stop()
     ms = ev0.elapsed_time(ev1)
     launches = sim.launch_count - l0
     prof = sim.profile_read()
@@ -266,7 +289,7 @@ def measure(args, workload, nbar, steps, warmup, rank, local_rank, world, dist, 
         dms, dcnt = fam[dom]
         fam_bytes = kernel_algorithmic_bytes(dom, n, int(np.prod(cells)), nbar)
         ach = fam_bytes / (dms / dcnt * 1e-3) / 1e9
-        traffic, tsrc, stale = captured_traffic(dom, workload, nbar) if cells_override is None else (None, None, None)
+        traffic, tsrc, stale = captured_traffic(dom, workload, nbar)
         roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                     "traffic": traffic, "traffic_source": tsrc, "traffic_capture_is_of_other_sources": stale,
                     "peak_source": peak_src, "avg_ms": dms / dcnt, "launches_timed": dcnt,
@@ -281,7 +304,7 @@ def measure(args, workload, nbar, steps, warmup, rank, local_rank, world, dist, 
                       "collision": "MPC-AT" if kw.get("collision") else "SRD", "conserve_L": bool(kw.get("conserve_L", 0)),
                       "thermostat": bool(kw.get("thermostat", 0)),
                       "rebin_every": wl["rebin_every"], "brick": list(brick), "compact_workspace": bool(compact),
-                      "l2": "inputs larger than L2 (no flush)" if n * 24 > 4 * 126e6 else "state within 4x L2 (partly L2-resident): HBM fraction not meaningful",
+                      "l2": "inputs larger than L2 (no flush)" if n * 24 > 4 * 126e6 else ("state fits in L2 (L2-resident, launch-bound): HBM fraction not meaningful" if n * 24 < 126e6 else "state within 4x L2 (partly L2-resident): HBM fraction not meaningful"),
                       "parallelism": "replicas only" if world > 1 else "single GPU",
                       "algorithmic_bytes_per_update": balg,
                       "collisions_in_timed_region": "K (the warm-up's last collision is applied by the first timed sweep, the last timed one stays pending)"},
@@ -293,73 +316,6 @@ def measure(args, workload, nbar, steps, warmup, rank, local_rank, world, dist, 
     del sim
     torch.cuda.empty_cache()
     return res, wl
-
-
-def measure_slabs(args, cells, nbar, world_sub, steps, warmup, rebin_every):
-    """Work inflation of the slab decomposition on ONE GPU: the box once as a whole and once as `world_sub`
-    slab subdomain contexts run one after the other (a barrier of the ranks = the end of a Python loop here), same seeded
-    input, same number of steps; both timed with CUDA events. Not a scaling number: nothing runs in parallel, there is no
-    NVLink in it. It says how much more work the ranks do together than the single-domain run (halo cells finalised twice,
-    shared sums added twice, hand-over records)."""
-    import torch
-
-    from paper_2406_15236_b200 import MPC
-    from paper_2406_15236_b200.inputs import uniform_maxwell_cuda
-    from paper_2406_15236_b200.slab import slab_neighbours, slab_partition
-
-    box = tuple(float(c) for c in cells)
-    n = int(np.prod(cells)) * nbar
-    brick = (16, 16, 8)
-    kw = dict(thermostat=1, rebin_every=rebin_every, brick=brick)
-    st = list(uniform_maxwell_cuda(box, n, 4321, device="cuda:0", to_host=False))
-    out = {}
-    whole = MPC(box, cells, nbar, 99, n_max=n, **kw)
-    whole.set_state(*st)
-    whole.step(warmup)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    e0.record(whole.stream); whole.step(steps); e1.record(whole.stream)
-    torch.cuda.synchronize()
-    out["whole_ms_per_step"] = e0.elapsed_time(e1) / steps
-    whole.close()
-    del whole
-    torch.cuda.empty_cache()
-    parts = slab_partition(cells[2], world_sub, brick[2])
-    layer = torch.floor(st[2]).to(torch.int64)                      # a = 1 in the bench boxes
-    ranks = []
-    for z0, nz in parts:
-        sel = torch.nonzero((layer >= z0) & (layer < z0 + nz)).flatten()
-        g = MPC(box, cells, nbar, 99, n_max=int(1.1 * sel.numel()) + 1024, sub=(z0, nz), **kw)
-        ranks.append((g, sel))
-    for r, (g, _) in enumerate(ranks):
-        below, above = slab_neighbours(r, world_sub)
-        g.sub_connect(ranks[below][0].sub_export(), ranks[above][0].sub_export())
-    for g, sel in ranks:
-        g.set_state(*[a[sel].contiguous() for a in st[:6]], id=sel.to(torch.int32))      # ids = index in the whole box
-    del st, layer
-    torch.cuda.empty_cache()
-
-    def run(k):
-        for i in range(k):
-            for g, _ in ranks:
-                g.sub_begin(k - 1 - i)
-            for g, _ in ranks:
-                g.sub_end()
-
-    run(warmup)
-    torch.cuda.synchronize()
-    s = ranks[0][0].stream
-    e0.record(s); run(steps); e1.record(s)
-    torch.cuda.synchronize()
-    out["slabs_ms_per_step_summed_over_ranks"] = e0.elapsed_time(e1) / steps
-    out["ranks"] = world_sub
-    out["inflation"] = out["slabs_ms_per_step_summed_over_ranks"] / out["whole_ms_per_step"]
-    out["range_overflows"] = sum(int(g.observables()["n_range_overflows"]) for g, _ in ranks)
-    out["config"] = {"cells": list(cells), "n_per_cell": nbar, "particles": n, "rebin_every": rebin_every, "steps": steps, "warmup": warmup,
-                     "note": "one GPU, ranks run one after the other; the reorders of the subdomains are the folded ones and hand particles over inside their kernels"}
-    for g, _ in ranks:
-        g.close()
-    return out
 
 
 def main():
@@ -375,20 +331,13 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the density sweep and the other workloads")
-    ap.add_argument("--compact", action="store_true", help="property-wise reorder workspace")
-    ap.add_argument("--debug", type=int, default=0, help="mpc_set_debug flags (A/B runs of the diagnostic code paths; changes speed only)")
-    ap.add_argument("--slabs", type=int, default=0, help="R >= 2: instead of the benchmark, time the box as a whole and as R slab subdomains on this one GPU (work inflation of the decomposition, DESIGN.md 9)")
-    ap.add_argument("--cells", default=None, help="override the workload's cell grid, e.g. 256,256,256 (profiling runs)")
     args = ap.parse_args()
     wl = dict(WORKLOADS[args.workload])
-    explicit = args.nbar is not None or args.cells is not None or args.workload != "cfg5" or args.rebin_every is not None
+    explicit = args.nbar is not None or args.workload != "cfg5" or args.rebin_every is not None
     if args.nbar is None:
         args.nbar = wl["nbar"]
     if args.rebin_every is not None:
         wl["rebin_every"] = args.rebin_every
-    cells_override = tuple(int(t) for t in args.cells.split(",")) if args.cells else None
-    if cells_override:
-        wl["cells"] = cells_override
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -408,13 +357,8 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
     torch.cuda.set_device(torch.device(f"cuda:{local_rank}"))
 
-    if args.slabs >= 2:
-        cells = cells_override or (512, 512, 256)
-        print(json.dumps({"slab_work_inflation": measure_slabs(args, cells, args.nbar, args.slabs, args.steps, args.warmup, wl["rebin_every"])}), flush=True)
-        return
     res, wl = measure(args, args.workload, args.nbar, args.steps, args.warmup, rank, local_rank, world, dist,
-                      with_e2e=(not args.no_e2e and rank == 0 and world == 1), rebin_every=args.rebin_every,
-                      cells_override=cells_override)
+                      with_e2e=(not args.no_e2e and rank == 0 and world == 1), rebin_every=args.rebin_every)
     line = {"metric": "MPC particle-updates/sec", "value": res["value"], "unit": "particle-updates/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -433,9 +377,12 @@ def main():
                           "family_ms_per_step": r["roofline"]["family_ms_per_step"], "check": r["check"]})
         line["density_sweep"] = sweep
         other = []
-        for w in ("cfg3", "cfg4"):
-            r, _ = measure(args, w, WORKLOADS[w]["nbar"], 100, 10, rank, local_rank, world, None, with_e2e=False)
+        # configs 1 and 2 (40,960 and 2.6e6 particles) live in L2 and are bound by kernel launches, not by HBM: reported
+        # as updates/s, their "fraction of the HBM roofline" means nothing and is flagged in config.l2
+        for w, k in (("cfg1", 1000), ("cfg2", 300), ("cfg3", 100), ("cfg4", 100)):
+            r, _ = measure(args, w, WORKLOADS[w]["nbar"], k, 10, rank, local_rank, world, None, with_e2e=False)
             other.append({"workload": w, "config": r["config"], "ms_per_step": r["ms_per_step"], "value": r["value"],
+                          "steps": k, "gpu_launches": r["gpu_launches"],
                           "step_frac_of_roofline": r["roofline"]["step_frac_of_roofline"],
                           "family_ms_per_step": r["roofline"]["family_ms_per_step"], "check": r["check"]})
         line["other_workloads"] = other

@@ -10,7 +10,7 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("MPC_B200_LIB", os.path.join(HERE, "libmpc_b200.so"))   # override: alternative builds
+LIB_PATH = os.path.join(HERE, "libmpc_b200.so")
 
 MPC_OK, MPC_EINVAL, MPC_ESTATE, MPC_ENOMEM, MPC_ECUDA, MPC_ERANGE = 0, -1, -2, -3, -4, -5
 PROFILE_NOALLOC_MAX_LAYERS = 2048
