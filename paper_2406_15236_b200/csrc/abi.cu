@@ -44,7 +44,8 @@ Layout make_layout(bool sub, size_t n_max, size_t nkeys, size_t nbricks, size_t 
   l.off_mt = take(MT_TABLE * 8);
   const bool staged = !compact && !generic;
   l.off_tbase = take(staged ? nbricks * tile_cells * 4 : 4);
-  l.off_chunk0 = take(staged ? (nbricks + 1) * 4 : 4);
+  // (compact SRD workspace: ranges of the previous order for the windowed gather, groups of at least an eighth of a brick)
+  l.off_chunk0 = take(staged ? (nbricks + 1) * 4 : (compact && !generic) ? (8 * nbricks + 1) * 4 : 4);
   l.total = o;
   return l;
 }
@@ -361,7 +362,17 @@ int mpc_bind(mpc_ctx* c, void* workspace, size_t bytes, unsigned long long n_max
   }
   const bool staged = !compact && !c->G.generic;
   c->tbase = staged ? (uint32_t*)(c->ws + l.off_tbase) : nullptr;
-  c->chunk0 = staged ? (uint32_t*)(c->ws + l.off_chunk0) : nullptr;
+  c->chunk0 = (staged || (compact && !c->G.generic)) ? (uint32_t*)(c->ws + l.off_chunk0) : nullptr;
+  c->gwin_shift = 0; c->gwin_cap = 0;
+  if (compact && !c->G.generic) {
+    // window of k_gather_win: the largest aligned part of a brick (down to an eighth, at least 32 keys: the lane-spread order
+    // permutes inside groups of 32) whose mean particle number, plus 20 %, fits in 100 KB, so that two CTAs share an SM
+    const int bvs = c->G.bs[0] + c->G.bs[1] + c->G.bs[2];
+    for (int sh = bvs; sh >= bvs - 3 && sh >= SPREAD_GROUP_SHIFT; --sh) {
+      const double elems = 1.2 * (double)(1u << sh) * (double)c->G.nbar + 256.0;
+      if (elems * 4.0 <= 100.0 * 1024.0) { c->gwin_shift = sh; c->gwin_cap = (uint32_t)elems; break; }
+    }
+  }
   CU(cudaMemsetAsync(c->nrange, 0, 8, c->stream));
   c->bound = true; c->have_state = false; c->have_cells = false; c->have_order = false; c->sums_clean = false; c->reorder_stage = 0;
   c->collide_pending = false; c->order_spread = 0; c->n = 0;

@@ -373,6 +373,8 @@ struct mpc_ctx {
   uint32_t* Bf[7];  // second copy (non-compact); Bf[0] = 4-byte temp (compact)
   uint32_t *key, *slot_id, *perm, *cursor, *offset, *bsum;
   uint32_t *tbase, *chunk0;   // staged reorder: per (brick, tile cell) first slot; brick ranges of the previous order
+  int gwin_shift;             // compact workspace: log2 of the keys per shared-memory window of k_gather_win (0: not used); chunk0 then
+  uint32_t gwin_cap;          // ... holds the previous order's ranges of these groups; gwin_cap = elements per window
   mpc::u64* sums;
   float* rec;
   double* obs;      // OBS_BLOCKS*8 doubles + 2*MAX_PROFILE doubles

@@ -280,6 +280,26 @@ __global__ void __launch_bounds__(256) k_gather(size_t n, const uint32_t* __rest
   for (int a = 0; a < NA; ++a) ((uint32_t*)dst.p[a])[d] = v[a];
 }
 
+// Property-wise gather of the compact workspace when the particles already have an order: the particles
+// that land in a group of 2^gsh consecutive keys (a brick or an aligned part of one) come almost all from the same group's range of
+// the PREVIOUS order (old0, saved before the scan; a particle moves a fraction of a cell between two reorders). k_gather<1>
+// asks L2 for one 32-byte sector per 4-byte element and is bound by that request rate; here a CTA reads its group's old range
+// coalesced into shared memory once and gathers from there; the few sources outside the window are read from global memory.
+constexpr int GWIN_T = 512;
+__global__ void __launch_bounds__(GWIN_T) k_gather_win(const uint32_t* __restrict__ perm, const uint32_t* __restrict__ src, uint32_t* __restrict__ dst,
+                                                       const uint32_t* __restrict__ old0, const uint32_t* __restrict__ offset, int gsh, uint32_t cap) {
+  extern __shared__ uint32_t win[];
+  const uint32_t g = blockIdx.x;
+  const uint32_t w0 = old0[g], wl = min(old0[g + 1] - w0, cap);
+  for (uint32_t i = threadIdx.x; i < wl; i += GWIN_T) win[i] = src[w0 + i];
+  __syncthreads();
+  const uint32_t d0 = offset[(size_t)g << gsh], d1 = offset[((size_t)g + 1) << gsh];
+  for (uint32_t d = d0 + threadIdx.x; d < d1; d += GWIN_T) {
+    const uint32_t sidx = perm[d], u = sidx - w0;
+    dst[d] = (u < wl) ? win[u] : src[sidx];
+  }
+}
+
 __global__ void __launch_bounds__(256) k_iota(size_t n, uint32_t* __restrict__ id) {
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) id[i] = (uint32_t)i;
@@ -298,7 +318,7 @@ int launch_iota(mpc_ctx* c) {
 namespace {
 
 // particle arrays gathered through c->perm: new[i] = old[perm[i]]
-int apply_perm(mpc_ctx* c) {
+int apply_perm(mpc_ctx* c, bool windowed = false) {
   const size_t n = c->n;
   FamilyTimer ftg(c, F_GATHER);
   if (!c->compact) {
@@ -315,8 +335,15 @@ int apply_perm(mpc_ctx* c) {
     for (int a = 0; a < 7; ++a) {
       uint32_t*& arr = c->A[a];
       src.p[0] = arr; dst.p[0] = c->Bf[0];
-      k_gather<1><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
-      LAUNCH_CHECK("k_gather");
+      if (windowed) {   // c->chunk0: the group ranges of the previous order (do_reorder), c->offset: those of the new one
+        const size_t bytes = (size_t)c->gwin_cap * 4;
+        if (a == 0) CU(cudaFuncSetAttribute(k_gather_win, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+        k_gather_win<<<c->G.nkeys >> c->gwin_shift, GWIN_T, bytes, c->stream>>>(c->perm, arr, c->Bf[0], c->chunk0, c->offset, c->gwin_shift, c->gwin_cap);
+        LAUNCH_CHECK("k_gather_win");
+      } else {
+        k_gather<1><<<nblk(n, 256), 256, 0, c->stream>>>(n, c->perm, src, dst);
+        LAUNCH_CHECK("k_gather");
+      }
       uint32_t* t = arr; arr = c->Bf[0];
       for (int b = 0; b < 7; ++b) c->Bf[b] = t;     // compact mode: all seven alias the one spare array
     }
@@ -345,6 +372,16 @@ int do_reorder(mpc_ctx* c, bool folded, bool canonical, bool counts_in_cursor) {
   if (folded) {   // the brick ranges of the old order, before the scan overwrites the offsets
     FamilyTimer ft(c, F_SCAN);
     k_save_chunks<<<nblk((size_t)c->nbricks + 1, 256), 256, 0, c->stream>>>(c->offset, bvs, c->nbricks, (uint32_t)n, c->chunk0);
+    LAUNCH_CHECK("k_save_chunks");
+  }
+  // compact workspace with a previous order: the gather goes through shared-memory windows (k_gather_win) and needs the
+  // previous order's group ranges (MPC_DEBUG_NO_FUSE_GATHER: the plain element-wise gather, same result)
+  const bool windowed = c->compact && !folded && !canonical && c->have_order && c->chunk0 && c->gwin_shift > 0 && n != 0 &&
+                        !(c->debug & MPC_DEBUG_NO_FUSE_GATHER);
+  if (windowed) {
+    FamilyTimer ft(c, F_SCAN);
+    const uint32_t ng = c->G.nkeys >> c->gwin_shift;
+    k_save_chunks<<<nblk((size_t)ng + 1, 256), 256, 0, c->stream>>>(c->offset, c->gwin_shift, ng, (uint32_t)n, c->chunk0);
     LAUNCH_CHECK("k_save_chunks");
   }
   {
@@ -401,7 +438,7 @@ int do_reorder(mpc_ctx* c, bool folded, bool canonical, bool counts_in_cursor) {
   c->order_canonical = canonical;
   c->order_spread = spread;
   if (folded) { c->reorder_stage = 1; return MPC_OK; }
-  return apply_perm(c);
+  return apply_perm(c, windowed);
 }
 
 // restore the canonical (key, id) order inside the cell segments of the last reorder (U4); called

@@ -368,6 +368,38 @@ def test_reorder_code_paths_agree(kw):
             assert np.array_equal(x, y)
 
 
+@pytest.mark.parametrize("kw,nbar", [(dict(thermostat=1, brick=(16, 16, 8), rebin_every=3), 10),
+                                     (dict(thermostat=1, brick=(16, 16, 8), rebin_every=2), 20),      # window = half a brick
+                                     (dict(thermostat=1, bc=(0, 0, 1), g=(0.01, 0, 0), brick=4, rebin_every=3), 10),
+                                     (dict(brick=(4, 2, 1), rebin_every=2), 10)])                     # bricks below 32 cells: no windows
+def test_compact_workspace_gathers_agree(kw, nbar):
+    # compact workspace (property-wise reorder through one spare array): from the second reorder on the
+    # gather goes through shared-memory windows over the previous order's ranges (k_gather_win); with
+    # MPC_DEBUG_NO_FUSE_GATHER it is the plain element-wise gather; and the workspace with the second particle copy moves
+    # records instead. State AND memory order must be identical in all three, after several reorders and a long step that
+    # carries a good part of the particles out of their window.
+    from paper_2406_15236_b200 import binding as B
+    cells = (32, 16, 16)
+    box = tuple(float(c) for c in cells)
+    n = int(np.prod(cells)) * nbar - 13
+    st = uniform_maxwell(box, n, 78)
+    res = []
+    for compact, flags in ((True, 0), (True, B.DEBUG_NO_FUSE_GATHER), (False, 0)):
+        g = MPC(box, cells, nbar, 24, n_max=n, compact=compact, dt=0.5, **kw)
+        g.set_debug(flags)
+        gpu_set(g, st)
+        g.profile_enable()
+        g.step(7)
+        fam = g.profile_read()
+        g.step(4)
+        res.append(gpu_get(g) + [t.cpu().numpy() for t in g.get_cells()])
+        if compact:
+            assert fam["gather"][1] >= 2 and fam["sweep_gather"][1] == 0, fam    # property-wise reorders, nothing folded
+    for r in res[1:]:
+        for x, y in zip(res[0], r):
+            assert np.array_equal(x, y)
+
+
 _FOLD = dict(thermostat=1, brick=(16, 16, 8), rebin_every=4)
 _FOLD_WALL = dict(thermostat=1, bc=(0, 0, 1), g=(0.01, 0, 0), brick=4, rebin_every=4)
 _FOLD_LE = dict(thermostat=1, shear_rate=0.08, brick=(16, 16, 8), rebin_every=4)
