@@ -285,18 +285,63 @@ __global__ void __launch_bounds__(256) k_gather(size_t n, const uint32_t* __rest
 // the PREVIOUS order (old0, saved before the scan; a particle moves a fraction of a cell between two reorders). k_gather<1>
 // asks L2 for one 32-byte sector per 4-byte element and is bound by that request rate; here a CTA reads its group's old range
 // coalesced into shared memory once and gathers from there; the few sources outside the window are read from global memory.
+// The window is brought in by the TMA engine (cp.async.bulk global -> shared, completion on an mbarrier; SASS: UBLKCP): no
+// registers and no load instructions are spent on it, and with two CTAs per SM one CTA's copy runs under the other's gather.
+// Bulk copies want 16-byte aligned addresses and sizes: the window starts at the old range's start rounded down to 4 elements and
+// ends rounded up (the extra elements are particles of the neighbouring groups: valid sources like any other; the arrays are
+// padded to 256 bytes and followed by the next array of the workspace, so reading up to 12 bytes past n is safe).
 constexpr int GWIN_T = 512;
+constexpr uint32_t GWIN_CHUNK = 32768;   // bytes per bulk copy
 __global__ void __launch_bounds__(GWIN_T) k_gather_win(const uint32_t* __restrict__ perm, const uint32_t* __restrict__ src, uint32_t* __restrict__ dst,
                                                        const uint32_t* __restrict__ old0, const uint32_t* __restrict__ offset, int gsh, uint32_t cap) {
-  extern __shared__ uint32_t win[];
+  extern __shared__ __align__(16) uint32_t win[];
+  __shared__ __align__(8) unsigned long long bar;
   const uint32_t g = blockIdx.x;
-  const uint32_t w0 = old0[g], wl = min(old0[g + 1] - w0, cap);
-  for (uint32_t i = threadIdx.x; i < wl; i += GWIN_T) win[i] = src[w0 + i];
-  __syncthreads();
+  const uint32_t w0 = old0[g] & ~3u;
+  const uint32_t wl = min((old0[g + 1] - w0 + 3u) & ~3u, cap & ~3u);
+  const uint32_t bar_a = (uint32_t)__cvta_generic_to_shared(&bar), win_a = (uint32_t)__cvta_generic_to_shared(win);
+  if (threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_a));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if (wl) {
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_a), "r"(wl * 4u) : "memory");
+      for (uint32_t o = 0; o < wl * 4u; o += GWIN_CHUNK) {
+        const uint32_t bytes = min(GWIN_CHUNK, wl * 4u - o);
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(win_a + o), "l"(reinterpret_cast<const char*>(src + w0) + o), "r"(bytes), "r"(bar_a) : "memory");
+      }
+    }
+  }
+  __syncthreads();   // the barrier is initialised (and armed) before anyone waits on it
   const uint32_t d0 = offset[(size_t)g << gsh], d1 = offset[((size_t)g + 1) << gsh];
-  for (uint32_t d = d0 + threadIdx.x; d < d1; d += GWIN_T) {
-    const uint32_t sidx = perm[d], u = sidx - w0;
-    dst[d] = (u < wl) ? win[u] : src[sidx];
+  // GWIN_U independent index loads in flight per thread (one at a time left the kernel waiting on the latency of perm: 1024
+  // threads x 4 bytes per SM against the ~35 KB the DRAM pipe wants); the first batch is on its way while the window arrives
+  constexpr int GWIN_U = 8;
+  uint32_t base = d0 + threadIdx.x;
+  uint32_t sidx[GWIN_U];
+#pragma unroll
+  for (int k = 0; k < GWIN_U; ++k) { const uint32_t d = base + k * GWIN_T; sidx[k] = d < d1 ? perm[d] : 0u; }
+  if (wl) {
+    uint32_t done;
+    do {
+      asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\nselp.u32 %0, 1, 0, p;\n}" : "=r"(done) : "r"(bar_a) : "memory");
+    } while (!done);
+  }
+  for (; base < d1; base += GWIN_U * GWIN_T) {
+    uint32_t snext[GWIN_U];
+    const uint32_t nb = base + GWIN_U * GWIN_T;
+#pragma unroll
+    for (int k = 0; k < GWIN_U; ++k) { const uint32_t d = nb + k * GWIN_T; snext[k] = d < d1 ? perm[d] : 0u; }
+#pragma unroll
+    for (int k = 0; k < GWIN_U; ++k) {
+      const uint32_t d = base + k * GWIN_T;
+      if (d < d1) {
+        const uint32_t u = sidx[k] - w0;
+        dst[d] = (u < wl) ? win[u] : src[sidx[k]];
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < GWIN_U; ++k) sidx[k] = snext[k];
   }
 }
 
